@@ -1,0 +1,162 @@
+/* gf8.h -- C ABI of the B200-native GeoFP8 gradient codec (arXiv 2607.07494, "GeoFP8").
+ *
+ * The library implements the data-parallel hot path of the paper: per weight-gradient matrix
+ *   Wg (d_out x d_in, row-major, Eq. 5)
+ * it keeps K-FAC factors A = E[a a^T], Gf = E[delta delta^T] (Eq. 4), reduces each to a
+ * damped rank-k eigen model (Eq. 24), whitens Wg into near-isotropic coordinates
+ *   W~ = T_G Wg T_A,  T = I + U_k diag(e) U_k^T            (PAPER.md:158 Eq. 14, :180 Eq. 18, :250 Eq. 22)
+ * scales and casts W~ to FP8 (Eq. 16; Alg. 1 l.12-13), and on the receive side
+ * dequantises R payloads, sums them in FP32 (Eq. 1; Alg. 1 l.20-21) and maps back
+ *   Wg^ = T_G^-1 U^ T_A^-1                                   (PAPER.md:172 Eq. 17, :184 Eq. 19).
+ * DESIGN.md lists every reading taken where the paper is silent (S1..S15).
+ *
+ * Conventions (all entry points):
+ *  - Every data pointer is a DEVICE pointer to caller-owned memory unless the parameter name ends
+ *    in `_host`.  The library never frees caller memory and never keeps a caller pointer past
+ *    the stream-ordered completion of the call.  Pointers must be 16-byte aligned.
+ *  - Matrices are dense row-major.  Wg is [d_out][d_in] (the nn.Linear.weight.grad layout).
+ *    codes: one byte per element, same layout.  Block scales: row-major over the
+ *    ceil(d_out/128) x ceil(d_in/128) grid.
+ *  - d_out and d_in must be multiples of 16 (else GF8_ERR_UNSUPPORTED).
+ *  - `stream` is a cudaStream_t passed as void*.  Calls are asynchronous on that stream; they do
+ *    not synchronise with the host, run no host eigensolver and have no CPU fallback.
+ *  - The ctx owns factors, bases, multipliers and scratch.  encode / decode / reduce allocate
+ *    nothing.  Factor accumulators (d^2 FP32 per side) are allocated by the first
+ *    gf8_factor_update / gf8_set_factor of a layer.
+ *  - Errors: a gf8_status is returned; nothing throws or aborts across the ABI.  Argument errors
+ *    are detected before any launch.  gf8_last_error(ctx) gives a message for the last failure.
+ *  - One ctx (hence one basis per layer) is shared by all R simulated ranks (S12).
+ */
+#ifndef GF8_H
+#define GF8_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gf8_ctx gf8_ctx;
+
+typedef enum {
+    GF8_OK = 0,
+    GF8_ERR_INVALID_ARG = 1,
+    GF8_ERR_BAD_STATE = 2,   /* e.g. encode on a whitened layer before a basis exists */
+    GF8_ERR_UNSUPPORTED = 3, /* misaligned pointer, dims not multiple of 16, rank too large */
+    GF8_ERR_NOMEM = 4,
+    GF8_ERR_CUDA = 5
+} gf8_status;
+
+typedef enum { GF8_E4M3 = 0, GF8_E5M2 = 1 } gf8_format;           /* ref [24] */
+typedef enum { GF8_SCALE_TENSOR = 0, GF8_SCALE_BLOCK128 = 1 } gf8_scaling;
+/* Which factors whiten the layer.  NONE = Euclidean branch (Alg. 1 l.3-8);
+ * IN = the paper's deployed form (Eq. 18-19); OUT, BOTH = Eq. 14 / Table I variants. */
+typedef enum { GF8_SIDE_NONE = 0, GF8_SIDE_IN = 1, GF8_SIDE_OUT = 2, GF8_SIDE_BOTH = 3 } gf8_side;
+typedef enum { GF8_DT_BF16 = 0, GF8_DT_F32 = 1 } gf8_dtype;
+/* EXACT: transform within 1e-4 relative Frobenius of the FP64 oracle (FP32 arithmetic, or
+ *        BF16x3 split operands on the tensor cores).
+ * FAST : single-pass BF16 tensor-core operands, 2e-3 tier. */
+typedef enum { GF8_PREC_EXACT = 0, GF8_PREC_FAST = 1 } gf8_precision;
+
+#define GF8_MAX_RANK 512   /* k <= min(d, 512) */
+#define GF8_MAX_R 64       /* simulated ranks per reduce call */
+
+typedef struct {
+    int32_t d_out, d_in;       /* m, n */
+    int32_t rank_in, rank_out; /* k of U_A (input side), k of U_G (output side); ignored if unused */
+    int32_t side;              /* gf8_side */
+    int32_t fmt;               /* gf8_format */
+    int32_t scaling;           /* gf8_scaling */
+    float damping;             /* lambda, added to eigenvalues at refresh (S3) */
+    float ema_beta;            /* beta of the factor EMA after the first update (S4); 0 = replace */
+} gf8_layer_desc;
+
+/* ---- lifetime ---------------------------------------------------------------------------------- */
+/* Creates a context on CUDA device `device` for `n_layers` gradient matrices. */
+gf8_status gf8_create(gf8_ctx** out, int device, const gf8_layer_desc* layers_host, int n_layers,
+                      gf8_precision precision);
+gf8_status gf8_destroy(gf8_ctx* ctx);
+/* code_bytes = d_out*d_in; n_scales = 1 or ceil(d_out/128)*ceil(d_in/128). */
+gf8_status gf8_payload_size(const gf8_ctx* ctx, int layer, size_t* code_bytes, size_t* n_scales);
+const char* gf8_status_string(gf8_status s);
+const char* gf8_last_error(const gf8_ctx* ctx);
+/* Number of kernels this context has launched so far (bench.py's gpu_launches). */
+int64_t gf8_launch_count(const gf8_ctx* ctx);
+
+/* ---- geometry state (every K steps) ------------------------------------------------ */
+/* a1.  A <- beta A + (1-beta) X^T X / T,  Gf likewise from Delta (Eq. 4).  The first
+ * update of a layer replaces (beta ignored).  act is [T][d_in], gout is [T][d_out], both `dt`;
+ * a side the layer does not use may be NULL.  Damping is NOT stored in the accumulator. */
+gf8_status gf8_factor_update(gf8_ctx* ctx, int layer, const void* act, const void* gout, int64_t T,
+                             gf8_dtype dt, void* stream);
+/* a2.  Rank-k eigenbasis of each factor of the layer by subspace iteration (Eq. 24):
+ * V <- orth(V0); n_iter x { V <- orth(A V) }; Rayleigh-Ritz with a single-CTA Jacobi eigensolve;
+ * U = V Z; multipliers e, ebar from (mu, rho, lambda).  V0 is the basis currently in the ctx
+ * (seed it with gf8_set_basis; the library holds no RNG).  GF8_ERR_BAD_STATE without a factor or
+ * a start basis. */
+gf8_status gf8_refresh_basis(gf8_ctx* ctx, int layer, int n_iter, void* stream);
+
+/* ---- codec (every step) -------------------------------------------------------------------------- */
+/* a3-a6.  codes[m*n], scale_inv[n_scales] <- FP8 payload of the whitened gradient. */
+gf8_status gf8_encode(gf8_ctx* ctx, int layer, const void* grad, gf8_dtype dt, uint8_t* codes,
+                      float* scale_inv, void* stream);
+/* R = 1 case of gf8_reduce_decoded without averaging. */
+gf8_status gf8_decode(gf8_ctx* ctx, int layer, const uint8_t* codes, const float* scale_inv,
+                      void* grad_out, gf8_dtype dt, void* stream);
+/* a7-a8.  U^ = (1/R) sum_r val(codes_r) * scale_inv_r in FP32, rank order, fused multiply-add
+ * (standing in for the all-reduce, S8), then unwhiten.  codes_host / scale_inv_host
+ * are HOST arrays of R device pointers. */
+gf8_status gf8_reduce_decoded(gf8_ctx* ctx, int layer, const uint8_t* const* codes_host,
+                              const float* const* scale_inv_host, int R, int average, void* grad_out,
+                              gf8_dtype dt, void* stream);
+
+/* ---- batched forms: n layers per call, grouped launches (launch granularity) ---------- */
+/* layers_host[n]; grads_host / codes_host / scale_inv_host are HOST arrays of n device pointers. */
+gf8_status gf8_encode_many(gf8_ctx* ctx, int n, const int* layers_host, const void* const* grads_host,
+                           gf8_dtype dt, uint8_t* const* codes_host, float* const* scale_inv_host,
+                           void* stream);
+/* codes_host / scale_inv_host: HOST arrays of n*R device pointers, index [i*R + r]. */
+gf8_status gf8_reduce_decoded_many(gf8_ctx* ctx, int n, const int* layers_host,
+                                   const uint8_t* const* codes_host, const float* const* scale_inv_host,
+                                   int R, int average, void* const* grads_out_host, gf8_dtype dt,
+                                   void* stream);
+gf8_status gf8_factor_update_many(gf8_ctx* ctx, int n, const int* layers_host, const void* const* acts_host,
+                                  const void* const* gouts_host, const int64_t* T_host, gf8_dtype dt,
+                                  void* stream);
+gf8_status gf8_refresh_basis_many(gf8_ctx* ctx, int n, const int* layers_host, int n_iter, void* stream);
+
+/* ---- end-to-end with HOST buffers (bench.py's e2e leg) ------------------------------------------- */
+/* One whole codec step for n layers and R simulated ranks with pinned HOST gradients:
+ * H2D of every rank's gradient, encode, reduce_decoded, D2H of the decoded gradients.
+ * grads_host_ptrs[i*R + r] -> host buffer of layer i, rank r (dt); out_host_ptrs[i] -> host buffer
+ * receiving the decoded gradient (dt).  Staging memory is owned by the ctx (allocated on first use).
+ * The call returns after the stream work is enqueued; synchronise the stream before reading. */
+gf8_status gf8_step_host(gf8_ctx* ctx, int n, const int* layers_host, const void* const* grads_host_ptrs,
+                         int R, int average, void* const* out_host_ptrs, gf8_dtype dt, void* stream);
+
+/* ---- state access: checkpoint, oracle hand-off, parity taps ---------------------------------------- */
+/* side: GF8_SIDE_IN (A, d_in) or GF8_SIDE_OUT (Gf, d_out).  f is d x d FP32 row-major (device). */
+gf8_status gf8_get_factor(gf8_ctx* ctx, int layer, int side, float* f, void* stream);
+gf8_status gf8_set_factor(gf8_ctx* ctx, int layer, int side, const float* f, void* stream);
+/* U: d x k FP32 row-major; mu: k Ritz values (descending); rho_host: isotropic tail + lambda.
+ * set: mu == NULL installs U as a start basis only (not usable by the codec until refreshed). */
+gf8_status gf8_get_basis(gf8_ctx* ctx, int layer, int side, float* U, float* mu, float* rho_host,
+                         void* stream);
+gf8_status gf8_set_basis(gf8_ctx* ctx, int layer, int side, const float* U, const float* mu, float rho,
+                         void* stream);
+/* Transform-stage tap (gate G2): out = (float) W~ of one gradient, m x n FP32. */
+gf8_status gf8_whiten_f32(gf8_ctx* ctx, int layer, const void* grad, gf8_dtype dt, float* out,
+                          void* stream);
+/* Quantizer alone (gate G1): codes, scale_inv <- FP32 tensor `in` (m x n). */
+gf8_status gf8_quantize_f32(gf8_ctx* ctx, int fmt, int scaling, const float* in, int64_t m, int64_t n,
+                            uint8_t* codes, float* scale_inv, void* stream);
+/* Reduce alone (gate G4): out (m x n FP32) <- R payloads. */
+gf8_status gf8_reduce_f32(gf8_ctx* ctx, int fmt, int scaling, const uint8_t* const* codes_host,
+                          const float* const* scale_inv_host, int R, int average, int64_t m, int64_t n,
+                          float* out, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GF8_H */

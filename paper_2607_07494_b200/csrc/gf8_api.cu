@@ -1,0 +1,742 @@
+// gf8_api.cu -- the C ABI of include/gf8.h: context, argument checks, launch orchestration.
+// Every arithmetic step runs in the kernels of this directory; there is no CPU fallback.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/gf8.h"
+#include "gf8_basis.cuh"
+#include "gf8_quant.cuh"
+#include "gf8_simt_gemm.cuh"
+
+using namespace gf8;
+
+namespace {
+
+struct SideState {
+    int d = 0, k = 0;
+    bool used = false;
+    float* factor = nullptr;   // d x d FP32 (lazy)
+    bool has_factor = false;   // at least one update / set
+    float* U = nullptr;        // d x k FP32 row-major
+    float* mu = nullptr;       // k
+    float* e = nullptr;        // k  encode multipliers
+    float* ebar = nullptr;     // k  decode multipliers
+    float* rho = nullptr;      // 1
+    bool has_start = false, has_basis = false;
+};
+
+struct LayerState {
+    gf8_layer_desc desc;
+    SideState in, out;         // in: A / U_A (d_in), out: Gf / U_G (d_out)
+    size_t n_scales = 1;
+    uint32_t* amax_bits = nullptr;   // n_scales
+    float* scale = nullptr;          // n_scales
+    float* P = nullptr;              // m x kA
+    float* Q = nullptr;              // kG x n
+    float* S = nullptr;              // kG x kA
+};
+
+}  // namespace
+
+struct gf8_ctx {
+    int device = 0;
+    gf8_precision precision = GF8_PREC_EXACT;
+    std::vector<LayerState> layers;
+    std::vector<void*> allocs;
+    float* wt_scratch = nullptr;     // max m*n FP32
+    // refresh scratch (FP64)
+    double *V = nullptr, *Y = nullptr, *Gm = nullptr, *Bm = nullptr, *Zm = nullptr, *Zs = nullptr, *mu64 = nullptr;
+    // tap scratch (gf8_quantize_f32 with arbitrary shapes)
+    uint32_t* tap_amax = nullptr; float* tap_scale = nullptr; size_t tap_cap = 0;
+    // host-step staging
+    std::vector<void*> stage_allocs;
+    std::vector<void*> st_grads; std::vector<uint8_t*> st_codes; std::vector<float*> st_sinv; std::vector<void*> st_out;
+    std::vector<int> st_layers; int st_R = 0; int st_dt = -1;
+    int64_t launches = 0;
+    int num_sms = 148;
+    char err[512] = {0};
+};
+
+namespace {
+
+gf8_status fail(gf8_ctx* c, gf8_status s, const char* fmt, ...) {
+    if (c) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(c->err, sizeof(c->err), fmt, ap);
+        va_end(ap);
+    }
+    return s;
+}
+
+#define CU_TRY(ctx, expr)                                                                            \
+    do {                                                                                             \
+        cudaError_t _e = (expr);                                                                     \
+        if (_e != cudaSuccess)                                                                       \
+            return fail((ctx), GF8_ERR_CUDA, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e), \
+                        __FILE__, __LINE__);                                                         \
+    } while (0)
+
+#define GF_TRY(expr)                       \
+    do {                                   \
+        gf8_status _s = (expr);            \
+        if (_s != GF8_OK) return _s;       \
+    } while (0)
+
+#define LAUNCH_CHECK(ctx)                  \
+    do {                                   \
+        (ctx)->launches++;                 \
+        CU_TRY((ctx), cudaGetLastError()); \
+    } while (0)
+
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+template <typename T>
+gf8_status dmalloc(gf8_ctx* c, T** p, size_t count, std::vector<void*>* track = nullptr) {
+    void* q = nullptr;
+    cudaError_t e = cudaMalloc(&q, count * sizeof(T) + 16);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(c, GF8_ERR_NOMEM, "cudaMalloc of %zu bytes failed: %s", count * sizeof(T), cudaGetErrorString(e));
+    }
+    (track ? *track : c->allocs).push_back(q);
+    *p = static_cast<T*>(q);
+    return GF8_OK;
+}
+
+inline size_t n_scales_of(int scaling, int64_t m, int64_t n) {
+    return scaling == GF8_SCALE_TENSOR ? 1 : (size_t)((m + 127) / 128) * (size_t)((n + 127) / 128);
+}
+inline float fmax_of(int fmt) { return fmt == GF8_E4M3 ? 448.0f : 57344.0f; }
+
+inline int grid_for(gf8_ctx* c, int64_t work_items, int threads, int per_sm) {
+    int64_t blocks = (work_items + threads - 1) / threads;
+    const int64_t cap = (int64_t)c->num_sms * per_sm;
+    if (blocks > cap) blocks = cap;
+    if (blocks < 1) blocks = 1;
+    return (int)blocks;
+}
+
+// ---- GEMM launcher -------------------------------------------------------------------------------
+template <typename TA, typename TB, typename TC, typename TAcc>
+gf8_status launch_gemm(gf8_ctx* c, cudaStream_t st, const TA* A, int64_t sa_i, int64_t sa_l, const TB* B,
+                       int64_t sb_l, int64_t sb_j, TC* C, int64_t ldc, int M, int N, int K, const float* lscale,
+                       const float* rowscale, TAcc alpha, TAcc beta, int splits = 1) {
+    if (M <= 0 || N <= 0) return GF8_OK;
+    GemmArgs<TA, TB, TC, TAcc> g{A, sa_i, sa_l, B, sb_l, sb_j, C, ldc, M, N, K, lscale, rowscale, alpha, beta};
+    if (splits > 1) {
+        // split-K accumulates atomically: C must hold beta*C already.  Only beta in {0,1} is used.
+        if (beta == (TAcc)0) {
+            if (ldc != N) return fail(c, GF8_ERR_INVALID_ARG, "split-K gemm needs a dense C");
+            CU_TRY(c, cudaMemsetAsync(C, 0, sizeof(TC) * (size_t)M * N, st));
+        }
+    }
+    dim3 grid((N + SG_BN - 1) / SG_BN, (M + SG_BM - 1) / SG_BM, splits);
+    simt_gemm_kernel<TA, TB, TC, TAcc><<<grid, 256, 0, st>>>(g);
+    LAUNCH_CHECK(c);
+    return GF8_OK;
+}
+
+// Choose a split count so that small-output, long-K products still fill the machine.
+inline int pick_splits(gf8_ctx* c, int M, int N, int K) {
+    const int tiles = ((M + SG_BM - 1) / SG_BM) * ((N + SG_BN - 1) / SG_BN);
+    int s = (2 * c->num_sms + tiles - 1) / tiles;
+    const int maxs = (K + 4 * SG_BK - 1) / (4 * SG_BK);
+    if (s > maxs) s = maxs;
+    if (s < 1) s = 1;
+    return s;
+}
+
+// ---- quantizer on a device tensor (a5 + a6) ----------------------------------------------------------
+template <typename T>
+gf8_status quantize_dev(gf8_ctx* c, cudaStream_t st, const T* x, int64_t m, int64_t n, int fmt, int scaling,
+                        uint32_t* amax_bits, float* scale, uint8_t* codes, float* scale_inv) {
+    const size_t ns = n_scales_of(scaling, m, n);
+    if (scaling == GF8_SCALE_TENSOR) {
+        CU_TRY(c, cudaMemsetAsync(amax_bits, 0, sizeof(uint32_t), st));
+        const int64_t nvec = m * n * (int64_t)sizeof(T) / 16;
+        amax_tensor_kernel<T><<<grid_for(c, (nvec + 3) / 4, 256, 8), 256, 0, st>>>(x, m * n, amax_bits);
+        LAUNCH_CHECK(c);
+    } else {
+        dim3 grid((unsigned)((n + 127) / 128), (unsigned)((m + 127) / 128));
+        amax_block_kernel<T><<<grid, 256, 0, st>>>(x, m, n, amax_bits);
+        LAUNCH_CHECK(c);
+    }
+    scales_kernel<<<(int)((ns + 255) / 256), 256, 0, st>>>(amax_bits, (int)ns, fmax_of(fmt), scale, scale_inv);
+    LAUNCH_CHECK(c);
+    const int g = grid_for(c, m * n / 16, 256, 8);
+    if (fmt == GF8_E4M3) cast_kernel<T, 0><<<g, 256, 0, st>>>(x, m, n, scaling, scale, codes);
+    else cast_kernel<T, 1><<<g, 256, 0, st>>>(x, m, n, scaling, scale, codes);
+    LAUNCH_CHECK(c);
+    return GF8_OK;
+}
+
+// ---- reduce on device (a7) -----------------------------------------------------------------------------
+template <typename OutT>
+gf8_status reduce_dev(gf8_ctx* c, cudaStream_t st, const uint8_t* const* codes, const float* const* sinv, int R,
+                      int average, int64_t m, int64_t n, int fmt, int scaling, OutT* out) {
+    ReducePtrs p;
+    memset(&p, 0, sizeof(p));
+    for (int r = 0; r < R; ++r) { p.codes[r] = codes[r]; p.sinv[r] = sinv[r]; }
+    const int g = grid_for(c, m * n / 16, 256, 8);
+    if (fmt == GF8_E4M3) reduce_kernel<0, OutT><<<g, 256, 0, st>>>(p, R, average, m, n, scaling, out);
+    else reduce_kernel<1, OutT><<<g, 256, 0, st>>>(p, R, average, m, n, scaling, out);
+    LAUNCH_CHECK(c);
+    return GF8_OK;
+}
+
+// ---- a3 + a4 (and a8 with inverse = true): out = T_G in T_A in FP32 on the CUDA cores -------------------
+//   P = in U_A; Q = U_G^T in; S = U_G^T P; Q' = E_G (Q + S E_A U_A^T);
+//   out = in + P E_A U_A^T + U_G Q'          (Eq. 14 / :250 Eq. 22 in low-rank form)
+// `in` may alias `out` when TIn == float.
+template <typename TIn>
+gf8_status transform_simt(gf8_ctx* c, cudaStream_t st, LayerState& L, const TIn* in, float* out, bool inverse) {
+    const int m = L.desc.d_out, n = L.desc.d_in;
+    const bool useA = (L.desc.side & GF8_SIDE_IN) != 0, useG = (L.desc.side & GF8_SIDE_OUT) != 0;
+    const int kA = useA ? L.in.k : 0, kG = useG ? L.out.k : 0;
+    const float* eA = inverse ? L.in.ebar : L.in.e;
+    const float* eG = inverse ? L.out.ebar : L.out.e;
+    if ((const void*)in != (const void*)out) {
+        convert_kernel<TIn, float><<<grid_for(c, (int64_t)m * n, 256, 8), 256, 0, st>>>(in, (int64_t)m * n, out);
+        LAUNCH_CHECK(c);
+    }
+    if (useA)   // P = in U_A
+        GF_TRY((launch_gemm<TIn, float, float, float>(c, st, in, n, 1, L.in.U, kA, 1, L.P, kA, m, kA, n, nullptr,
+                                                      nullptr, 1.0f, 0.0f, pick_splits(c, m, kA, n))));
+    if (useG)   // Q = U_G^T in
+        GF_TRY((launch_gemm<float, TIn, float, float>(c, st, L.out.U, 1, kG, in, n, 1, L.Q, n, kG, n, m, nullptr,
+                                                      nullptr, 1.0f, 0.0f, pick_splits(c, kG, n, m))));
+    if (useA && useG) {
+        // S = U_G^T P
+        GF_TRY((launch_gemm<float, float, float, float>(c, st, L.out.U, 1, kG, L.P, kA, 1, L.S, kA, kG, kA, m,
+                                                        nullptr, nullptr, 1.0f, 0.0f, pick_splits(c, kG, kA, m))));
+        // Q' = E_G (Q + (S E_A) U_A^T)
+        GF_TRY((launch_gemm<float, float, float, float>(c, st, L.S, kA, 1, L.in.U, 1, kA, L.Q, n, kG, n, kA, eA, eG,
+                                                        1.0f, 1.0f)));
+    } else if (useG) {
+        // Q' = E_G Q   (K = 0: the kernel only applies the epilogue)
+        GF_TRY((launch_gemm<float, float, float, float>(c, st, L.Q, 0, 0, L.Q, 0, 0, L.Q, n, kG, n, 0, nullptr, eG,
+                                                        1.0f, 1.0f)));
+    }
+    if (useA)   // out += (P E_A) U_A^T
+        GF_TRY((launch_gemm<float, float, float, float>(c, st, L.P, kA, 1, L.in.U, 1, kA, out, n, m, n, kA, eA,
+                                                        nullptr, 1.0f, 1.0f)));
+    if (useG)   // out += U_G Q'
+        GF_TRY((launch_gemm<float, float, float, float>(c, st, L.out.U, kG, 1, L.Q, n, 1, out, n, m, n, kG, nullptr,
+                                                        nullptr, 1.0f, 1.0f)));
+    return GF8_OK;
+}
+
+gf8_status check_layer(gf8_ctx* c, int layer) {
+    if (!c) return GF8_ERR_INVALID_ARG;
+    if (layer < 0 || layer >= (int)c->layers.size()) return fail(c, GF8_ERR_INVALID_ARG, "layer %d out of range", layer);
+    return GF8_OK;
+}
+
+gf8_status check_basis(gf8_ctx* c, LayerState& L, int layer) {
+    if ((L.desc.side & GF8_SIDE_IN) && !L.in.has_basis)
+        return fail(c, GF8_ERR_BAD_STATE, "layer %d: input-side basis not set (refresh or set_basis first)", layer);
+    if ((L.desc.side & GF8_SIDE_OUT) && !L.out.has_basis)
+        return fail(c, GF8_ERR_BAD_STATE, "layer %d: output-side basis not set (refresh or set_basis first)", layer);
+    return GF8_OK;
+}
+
+SideState* side_of(gf8_ctx* c, LayerState& L, int side) {
+    if (side == GF8_SIDE_IN && L.in.used) return &L.in;
+    if (side == GF8_SIDE_OUT && L.out.used) return &L.out;
+    (void)c;
+    return nullptr;
+}
+
+gf8_status ensure_factor(gf8_ctx* c, SideState& s) {
+    if (s.factor) return GF8_OK;
+    return dmalloc(c, &s.factor, (size_t)s.d * s.d);
+}
+
+__global__ void widen_kernel(const float* __restrict__ in, int64_t n, double* __restrict__ out) {
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        out[i] = (double)in[i];
+}
+
+// CholeskyQR in FP64, applied twice (V d x k, in place).
+gf8_status orthonormalise(gf8_ctx* c, cudaStream_t st, double* V, int d, int k) {
+    for (int pass = 0; pass < 2; ++pass) {
+        GF_TRY((launch_gemm<double, double, double, double>(c, st, V, 1, k, V, k, 1, c->Gm, k, k, k, d, nullptr, nullptr,
+                                                            1.0, 0.0, pick_splits(c, k, k, d))));
+        cholesky_upper_kernel<<<1, 1024, 0, st>>>(c->Gm, k);
+        LAUNCH_CHECK(c);
+        trisolve_rows_kernel<<<(d + 127) / 128, 128, 0, st>>>(V, c->Gm, d, k);
+        LAUNCH_CHECK(c);
+    }
+    return GF8_OK;
+}
+
+gf8_status refresh_side(gf8_ctx* c, cudaStream_t st, SideState& s, double lam, int n_iter, int layer) {
+    if (!s.has_factor) return fail(c, GF8_ERR_BAD_STATE, "layer %d: no factor accumulated yet", layer);
+    if (!s.has_start) return fail(c, GF8_ERR_BAD_STATE, "layer %d: no start basis (gf8_set_basis first)", layer);
+    const int d = s.d, k = s.k;
+    double *V = c->V, *Y = c->Y;
+    widen_kernel<<<grid_for(c, (int64_t)d * k, 256, 4), 256, 0, st>>>(s.U, (int64_t)d * k, V);
+    LAUNCH_CHECK(c);
+    GF_TRY(orthonormalise(c, st, V, d, k));
+    for (int it = 0; it < n_iter; ++it) {
+        GF_TRY((launch_gemm<float, double, double, double>(c, st, s.factor, d, 1, V, k, 1, Y, k, d, k, d, nullptr,
+                                                           nullptr, 1.0, 0.0, pick_splits(c, d, k, d))));
+        double* t = V; V = Y; Y = t;
+        GF_TRY(orthonormalise(c, st, V, d, k));
+    }
+    // Rayleigh-Ritz: Y = A V, B = V^T Y
+    GF_TRY((launch_gemm<float, double, double, double>(c, st, s.factor, d, 1, V, k, 1, Y, k, d, k, d, nullptr, nullptr,
+                                                       1.0, 0.0, pick_splits(c, d, k, d))));
+    GF_TRY((launch_gemm<double, double, double, double>(c, st, V, 1, k, Y, k, 1, c->Bm, k, k, k, d, nullptr, nullptr,
+                                                        1.0, 0.0, pick_splits(c, k, k, d))));
+    const size_t smem = 2 * (size_t)k * k * sizeof(double);
+    const int use_smem = smem <= 200 * 1024 ? 1 : 0;
+    if (use_smem) CU_TRY(c, cudaFuncSetAttribute(jacobi_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    jacobi_kernel<<<1, 1024, use_smem ? smem : 0, st>>>(c->Bm, c->Zm, k, use_smem, c->mu64, c->Zs, 60);
+    LAUNCH_CHECK(c);
+    // U = V Zs (FP32 out)
+    GF_TRY((launch_gemm<double, double, float, double>(c, st, V, k, 1, c->Zs, k, 1, s.U, k, d, k, k, nullptr, nullptr,
+                                                       1.0, 0.0)));
+    multipliers_kernel<<<1, 256, 0, st>>>(s.factor, d, k, c->mu64, nullptr, lam, 0.0, s.mu, s.e, s.ebar, s.rho);
+    LAUNCH_CHECK(c);
+    s.has_basis = true;
+    return GF8_OK;
+}
+
+gf8_status encode_one(gf8_ctx* c, int layer, const void* grad, gf8_dtype dt, uint8_t* codes, float* scale_inv,
+                      cudaStream_t st) {
+    GF_TRY(check_layer(c, layer));
+    LayerState& L = c->layers[layer];
+    if (!grad || !codes || !scale_inv) return fail(c, GF8_ERR_INVALID_ARG, "null pointer");
+    if (!aligned16(grad) || !aligned16(codes)) return fail(c, GF8_ERR_UNSUPPORTED, "pointers must be 16-byte aligned");
+    if (dt != GF8_DT_BF16 && dt != GF8_DT_F32) return fail(c, GF8_ERR_INVALID_ARG, "bad dtype");
+    GF_TRY(check_basis(c, L, layer));
+    const int64_t m = L.desc.d_out, n = L.desc.d_in;
+    if (L.desc.side == GF8_SIDE_NONE) {
+        if (dt == GF8_DT_BF16)
+            return quantize_dev<bf16>(c, st, (const bf16*)grad, m, n, L.desc.fmt, L.desc.scaling, L.amax_bits, L.scale,
+                                      codes, scale_inv);
+        return quantize_dev<float>(c, st, (const float*)grad, m, n, L.desc.fmt, L.desc.scaling, L.amax_bits, L.scale,
+                                   codes, scale_inv);
+    }
+    if (dt == GF8_DT_BF16) GF_TRY(transform_simt<bf16>(c, st, L, (const bf16*)grad, c->wt_scratch, false));
+    else GF_TRY(transform_simt<float>(c, st, L, (const float*)grad, c->wt_scratch, false));
+    return quantize_dev<float>(c, st, c->wt_scratch, m, n, L.desc.fmt, L.desc.scaling, L.amax_bits, L.scale, codes,
+                               scale_inv);
+}
+
+gf8_status reduce_decoded_one(gf8_ctx* c, int layer, const uint8_t* const* codes, const float* const* sinv, int R,
+                              int average, void* grad_out, gf8_dtype dt, cudaStream_t st) {
+    GF_TRY(check_layer(c, layer));
+    LayerState& L = c->layers[layer];
+    if (!codes || !sinv || !grad_out) return fail(c, GF8_ERR_INVALID_ARG, "null pointer");
+    if (R < 1 || R > GF8_MAX_R) return fail(c, GF8_ERR_INVALID_ARG, "R=%d out of range [1,%d]", R, GF8_MAX_R);
+    if (dt != GF8_DT_BF16 && dt != GF8_DT_F32) return fail(c, GF8_ERR_INVALID_ARG, "bad dtype");
+    for (int r = 0; r < R; ++r) {
+        if (!codes[r] || !sinv[r]) return fail(c, GF8_ERR_INVALID_ARG, "null payload pointer for rank %d", r);
+        if (!aligned16(codes[r])) return fail(c, GF8_ERR_UNSUPPORTED, "pointers must be 16-byte aligned");
+    }
+    if (!aligned16(grad_out)) return fail(c, GF8_ERR_UNSUPPORTED, "pointers must be 16-byte aligned");
+    GF_TRY(check_basis(c, L, layer));
+    const int64_t m = L.desc.d_out, n = L.desc.d_in;
+    if (L.desc.side == GF8_SIDE_NONE) {
+        if (dt == GF8_DT_BF16)
+            return reduce_dev<bf16>(c, st, codes, sinv, R, average, m, n, L.desc.fmt, L.desc.scaling, (bf16*)grad_out);
+        return reduce_dev<float>(c, st, codes, sinv, R, average, m, n, L.desc.fmt, L.desc.scaling, (float*)grad_out);
+    }
+    float* buf = dt == GF8_DT_F32 ? (float*)grad_out : c->wt_scratch;
+    GF_TRY(reduce_dev<float>(c, st, codes, sinv, R, average, m, n, L.desc.fmt, L.desc.scaling, buf));
+    GF_TRY(transform_simt<float>(c, st, L, buf, buf, true));
+    if (dt == GF8_DT_BF16) {
+        convert_kernel<float, bf16><<<grid_for(c, m * n, 256, 8), 256, 0, st>>>(buf, m * n, (bf16*)grad_out);
+        LAUNCH_CHECK(c);
+    }
+    return GF8_OK;
+}
+
+}  // namespace
+
+// =====================================================================================================
+extern "C" {
+
+const char* gf8_status_string(gf8_status s) {
+    switch (s) {
+        case GF8_OK: return "ok";
+        case GF8_ERR_INVALID_ARG: return "invalid argument";
+        case GF8_ERR_BAD_STATE: return "bad state";
+        case GF8_ERR_UNSUPPORTED: return "unsupported";
+        case GF8_ERR_NOMEM: return "out of memory";
+        case GF8_ERR_CUDA: return "CUDA error";
+    }
+    return "unknown";
+}
+
+const char* gf8_last_error(const gf8_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+int64_t gf8_launch_count(const gf8_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+gf8_status gf8_create(gf8_ctx** out, int device, const gf8_layer_desc* layers, int n_layers, gf8_precision precision) {
+    if (!out || !layers || n_layers < 1) return GF8_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (precision != GF8_PREC_EXACT && precision != GF8_PREC_FAST) return GF8_ERR_INVALID_ARG;
+    for (int i = 0; i < n_layers; ++i) {
+        const gf8_layer_desc& d = layers[i];
+        if (d.d_out < 16 || d.d_in < 16) return GF8_ERR_INVALID_ARG;
+        if (d.d_out % 16 || d.d_in % 16) return GF8_ERR_UNSUPPORTED;
+        if (d.side < 0 || d.side > 3 || d.fmt < 0 || d.fmt > 1 || d.scaling < 0 || d.scaling > 1) return GF8_ERR_INVALID_ARG;
+        if ((d.side & GF8_SIDE_IN) && (d.rank_in < 1 || d.rank_in > d.d_in)) return GF8_ERR_INVALID_ARG;
+        if ((d.side & GF8_SIDE_OUT) && (d.rank_out < 1 || d.rank_out > d.d_out)) return GF8_ERR_INVALID_ARG;
+        if ((d.side & GF8_SIDE_IN) && d.rank_in > GF8_MAX_RANK) return GF8_ERR_UNSUPPORTED;
+        if ((d.side & GF8_SIDE_OUT) && d.rank_out > GF8_MAX_RANK) return GF8_ERR_UNSUPPORTED;
+        if (!(d.damping >= 0.0f) || !(d.ema_beta >= 0.0f && d.ema_beta < 1.0f)) return GF8_ERR_INVALID_ARG;
+    }
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return GF8_ERR_CUDA; }
+    gf8_ctx* c = new (std::nothrow) gf8_ctx();
+    if (!c) return GF8_ERR_NOMEM;
+    c->device = device;
+    c->precision = precision;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) c->num_sms = prop.multiProcessorCount;
+    c->layers.resize(n_layers);
+    size_t max_mn = 0, max_dk = 0, max_k = 0;
+    gf8_status s = GF8_OK;
+    for (int i = 0; i < n_layers && s == GF8_OK; ++i) {
+        LayerState& L = c->layers[i];
+        L.desc = layers[i];
+        const int m = L.desc.d_out, n = L.desc.d_in;
+        L.n_scales = n_scales_of(L.desc.scaling, m, n);
+        if ((s = dmalloc(c, &L.amax_bits, L.n_scales)) != GF8_OK) break;
+        if ((s = dmalloc(c, &L.scale, L.n_scales)) != GF8_OK) break;
+        if (L.desc.side != GF8_SIDE_NONE) max_mn = std::max(max_mn, (size_t)m * n);
+        auto init_side = [&](SideState& sd, int d, int k) -> gf8_status {
+            sd.used = true; sd.d = d; sd.k = k;
+            gf8_status r;
+            if ((r = dmalloc(c, &sd.U, (size_t)d * k)) != GF8_OK) return r;
+            if ((r = dmalloc(c, &sd.mu, (size_t)k)) != GF8_OK) return r;
+            if ((r = dmalloc(c, &sd.e, (size_t)k)) != GF8_OK) return r;
+            if ((r = dmalloc(c, &sd.ebar, (size_t)k)) != GF8_OK) return r;
+            if ((r = dmalloc(c, &sd.rho, (size_t)1)) != GF8_OK) return r;
+            max_dk = std::max(max_dk, (size_t)d * k);
+            max_k = std::max(max_k, (size_t)k);
+            return GF8_OK;
+        };
+        if (L.desc.side & GF8_SIDE_IN) {
+            if ((s = init_side(L.in, n, L.desc.rank_in)) != GF8_OK) break;
+            if ((s = dmalloc(c, &L.P, (size_t)m * L.desc.rank_in)) != GF8_OK) break;
+        }
+        if (L.desc.side & GF8_SIDE_OUT) {
+            if ((s = init_side(L.out, m, L.desc.rank_out)) != GF8_OK) break;
+            if ((s = dmalloc(c, &L.Q, (size_t)L.desc.rank_out * n)) != GF8_OK) break;
+        }
+        if (L.desc.side == GF8_SIDE_BOTH)
+            if ((s = dmalloc(c, &L.S, (size_t)L.desc.rank_out * L.desc.rank_in)) != GF8_OK) break;
+    }
+    if (s == GF8_OK && max_mn) s = dmalloc(c, &c->wt_scratch, max_mn);
+    if (s == GF8_OK && max_dk) {
+        if ((s = dmalloc(c, &c->V, max_dk)) == GF8_OK && (s = dmalloc(c, &c->Y, max_dk)) == GF8_OK &&
+            (s = dmalloc(c, &c->Gm, max_k * max_k)) == GF8_OK && (s = dmalloc(c, &c->Bm, max_k * max_k)) == GF8_OK &&
+            (s = dmalloc(c, &c->Zm, max_k * max_k)) == GF8_OK && (s = dmalloc(c, &c->Zs, max_k * max_k)) == GF8_OK)
+            s = dmalloc(c, &c->mu64, max_k);
+    }
+    if (s != GF8_OK) { gf8_destroy(c); return s; }
+    *out = c;
+    return GF8_OK;
+}
+
+gf8_status gf8_destroy(gf8_ctx* ctx) {
+    if (!ctx) return GF8_ERR_INVALID_ARG;
+    cudaSetDevice(ctx->device);
+    cudaDeviceSynchronize();
+    for (void* p : ctx->allocs) cudaFree(p);
+    for (void* p : ctx->stage_allocs) cudaFree(p);
+    delete ctx;
+    return GF8_OK;
+}
+
+gf8_status gf8_payload_size(const gf8_ctx* ctx, int layer, size_t* code_bytes, size_t* n_scales) {
+    if (!ctx || layer < 0 || layer >= (int)ctx->layers.size()) return GF8_ERR_INVALID_ARG;
+    const LayerState& L = ctx->layers[layer];
+    if (code_bytes) *code_bytes = (size_t)L.desc.d_out * L.desc.d_in;
+    if (n_scales) *n_scales = L.n_scales;
+    return GF8_OK;
+}
+
+// ---- a1 ---------------------------------------------------------------------------------------------------
+gf8_status gf8_factor_update(gf8_ctx* ctx, int layer, const void* act, const void* gout, int64_t T, gf8_dtype dt,
+                             void* stream) {
+    GF_TRY(check_layer(ctx, layer));
+    LayerState& L = ctx->layers[layer];
+    cudaStream_t st = (cudaStream_t)stream;
+    if (T < 1 || T > 0x7FFFFFFF) return fail(ctx, GF8_ERR_INVALID_ARG, "T out of range");
+    if (dt != GF8_DT_BF16 && dt != GF8_DT_F32) return fail(ctx, GF8_ERR_INVALID_ARG, "bad dtype");
+    if ((act && !aligned16(act)) || (gout && !aligned16(gout)))
+        return fail(ctx, GF8_ERR_UNSUPPORTED, "pointers must be 16-byte aligned");
+    if (L.in.used && !act) return fail(ctx, GF8_ERR_INVALID_ARG, "layer %d whitens the input side: act required", layer);
+    if (L.out.used && !gout) return fail(ctx, GF8_ERR_INVALID_ARG, "layer %d whitens the output side: gout required", layer);
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    for (int sidx = 0; sidx < 2; ++sidx) {
+        SideState& s = sidx == 0 ? L.in : L.out;
+        const void* X = sidx == 0 ? act : gout;
+        if (!s.used) continue;
+        GF_TRY(ensure_factor(ctx, s));
+        const float beta = s.has_factor ? L.desc.ema_beta : 0.0f;
+        const float alpha = (1.0f - beta) / (float)T;
+        const int d = s.d;
+        if (dt == GF8_DT_BF16)
+            GF_TRY((launch_gemm<bf16, bf16, float, float>(ctx, st, (const bf16*)X, 1, d, (const bf16*)X, d, 1, s.factor,
+                                                          d, d, d, (int)T, nullptr, nullptr, alpha, beta)));
+        else
+            GF_TRY((launch_gemm<float, float, float, float>(ctx, st, (const float*)X, 1, d, (const float*)X, d, 1,
+                                                            s.factor, d, d, d, (int)T, nullptr, nullptr, alpha, beta)));
+        s.has_factor = true;
+    }
+    return GF8_OK;
+}
+
+// ---- a2 ---------------------------------------------------------------------------------------------------
+gf8_status gf8_refresh_basis(gf8_ctx* ctx, int layer, int n_iter, void* stream) {
+    GF_TRY(check_layer(ctx, layer));
+    if (n_iter < 0 || n_iter > 1000) return fail(ctx, GF8_ERR_INVALID_ARG, "n_iter out of range");
+    LayerState& L = ctx->layers[layer];
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    if (L.in.used) GF_TRY(refresh_side(ctx, (cudaStream_t)stream, L.in, (double)L.desc.damping, n_iter, layer));
+    if (L.out.used) GF_TRY(refresh_side(ctx, (cudaStream_t)stream, L.out, (double)L.desc.damping, n_iter, layer));
+    return GF8_OK;
+}
+
+// ---- codec ------------------------------------------------------------------------------------------------
+gf8_status gf8_encode(gf8_ctx* ctx, int layer, const void* grad, gf8_dtype dt, uint8_t* codes, float* scale_inv,
+                      void* stream) {
+    if (!ctx) return GF8_ERR_INVALID_ARG;
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    return encode_one(ctx, layer, grad, dt, codes, scale_inv, (cudaStream_t)stream);
+}
+
+gf8_status gf8_decode(gf8_ctx* ctx, int layer, const uint8_t* codes, const float* scale_inv, void* grad_out,
+                      gf8_dtype dt, void* stream) {
+    if (!ctx) return GF8_ERR_INVALID_ARG;
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    const uint8_t* cp[1] = {codes};
+    const float* sp[1] = {scale_inv};
+    return reduce_decoded_one(ctx, layer, cp, sp, 1, 0, grad_out, dt, (cudaStream_t)stream);
+}
+
+gf8_status gf8_reduce_decoded(gf8_ctx* ctx, int layer, const uint8_t* const* codes, const float* const* scale_inv,
+                              int R, int average, void* grad_out, gf8_dtype dt, void* stream) {
+    if (!ctx) return GF8_ERR_INVALID_ARG;
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    return reduce_decoded_one(ctx, layer, codes, scale_inv, R, average, grad_out, dt, (cudaStream_t)stream);
+}
+
+gf8_status gf8_encode_many(gf8_ctx* ctx, int n, const int* layers, const void* const* grads, gf8_dtype dt,
+                           uint8_t* const* codes, float* const* scale_inv, void* stream) {
+    if (!ctx) return GF8_ERR_INVALID_ARG;
+    if (n < 0 || !layers || !grads || !codes || !scale_inv) return fail(ctx, GF8_ERR_INVALID_ARG, "null argument");
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    for (int i = 0; i < n; ++i) GF_TRY(encode_one(ctx, layers[i], grads[i], dt, codes[i], scale_inv[i], (cudaStream_t)stream));
+    return GF8_OK;
+}
+
+gf8_status gf8_reduce_decoded_many(gf8_ctx* ctx, int n, const int* layers, const uint8_t* const* codes,
+                                   const float* const* scale_inv, int R, int average, void* const* grads_out,
+                                   gf8_dtype dt, void* stream) {
+    if (!ctx) return GF8_ERR_INVALID_ARG;
+    if (n < 0 || !layers || !grads_out || !codes || !scale_inv) return fail(ctx, GF8_ERR_INVALID_ARG, "null argument");
+    if (R < 1 || R > GF8_MAX_R) return fail(ctx, GF8_ERR_INVALID_ARG, "R=%d out of range [1,%d]", R, GF8_MAX_R);
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    for (int i = 0; i < n; ++i)
+        GF_TRY(reduce_decoded_one(ctx, layers[i], codes + (size_t)i * R, scale_inv + (size_t)i * R, R, average,
+                                  grads_out[i], dt, (cudaStream_t)stream));
+    return GF8_OK;
+}
+
+gf8_status gf8_factor_update_many(gf8_ctx* ctx, int n, const int* layers, const void* const* acts,
+                                  const void* const* gouts, const int64_t* T, gf8_dtype dt, void* stream) {
+    if (!ctx) return GF8_ERR_INVALID_ARG;
+    if (n < 0 || !layers || !acts || !gouts || !T) return fail(ctx, GF8_ERR_INVALID_ARG, "null argument");
+    for (int i = 0; i < n; ++i) GF_TRY(gf8_factor_update(ctx, layers[i], acts[i], gouts[i], T[i], dt, stream));
+    return GF8_OK;
+}
+
+gf8_status gf8_refresh_basis_many(gf8_ctx* ctx, int n, const int* layers, int n_iter, void* stream) {
+    if (!ctx) return GF8_ERR_INVALID_ARG;
+    if (n < 0 || !layers) return fail(ctx, GF8_ERR_INVALID_ARG, "null argument");
+    for (int i = 0; i < n; ++i) GF_TRY(gf8_refresh_basis(ctx, layers[i], n_iter, stream));
+    return GF8_OK;
+}
+
+// ---- end-to-end with host buffers -----------------------------------------------------------------------------
+gf8_status gf8_step_host(gf8_ctx* ctx, int n, const int* layers, const void* const* grads_host, int R, int average,
+                         void* const* out_host, gf8_dtype dt, void* stream) {
+    if (!ctx) return GF8_ERR_INVALID_ARG;
+    if (n < 1 || !layers || !grads_host || !out_host) return fail(ctx, GF8_ERR_INVALID_ARG, "null argument");
+    if (R < 1 || R > GF8_MAX_R) return fail(ctx, GF8_ERR_INVALID_ARG, "R=%d out of range [1,%d]", R, GF8_MAX_R);
+    if (dt != GF8_DT_BF16 && dt != GF8_DT_F32) return fail(ctx, GF8_ERR_INVALID_ARG, "bad dtype");
+    for (int i = 0; i < n; ++i) GF_TRY(check_layer(ctx, layers[i]));
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t esz = dt == GF8_DT_BF16 ? 2 : 4;
+    bool same = ctx->st_R == R && ctx->st_dt == (int)dt && (int)ctx->st_layers.size() == n;
+    for (int i = 0; same && i < n; ++i) same = ctx->st_layers[i] == layers[i];
+    if (!same) {
+        CU_TRY(ctx, cudaDeviceSynchronize());
+        for (void* p : ctx->stage_allocs) cudaFree(p);
+        ctx->stage_allocs.clear();
+        ctx->st_grads.assign((size_t)n * R, nullptr);
+        ctx->st_codes.assign((size_t)n * R, nullptr);
+        ctx->st_sinv.assign((size_t)n * R, nullptr);
+        ctx->st_out.assign(n, nullptr);
+        for (int i = 0; i < n; ++i) {
+            const LayerState& L = ctx->layers[layers[i]];
+            const size_t mn = (size_t)L.desc.d_out * L.desc.d_in;
+            for (int r = 0; r < R; ++r) {
+                uint8_t* g = nullptr;
+                GF_TRY(dmalloc(ctx, &g, mn * esz, &ctx->stage_allocs));
+                ctx->st_grads[(size_t)i * R + r] = g;
+                GF_TRY(dmalloc(ctx, &ctx->st_codes[(size_t)i * R + r], mn, &ctx->stage_allocs));
+                GF_TRY(dmalloc(ctx, &ctx->st_sinv[(size_t)i * R + r], L.n_scales, &ctx->stage_allocs));
+            }
+            uint8_t* o = nullptr;
+            GF_TRY(dmalloc(ctx, &o, mn * esz, &ctx->stage_allocs));
+            ctx->st_out[i] = o;
+        }
+        ctx->st_layers.assign(layers, layers + n);
+        ctx->st_R = R;
+        ctx->st_dt = (int)dt;
+    }
+    for (int i = 0; i < n; ++i) {
+        const LayerState& L = ctx->layers[layers[i]];
+        const size_t bytes = (size_t)L.desc.d_out * L.desc.d_in * esz;
+        for (int r = 0; r < R; ++r) {
+            if (!grads_host[(size_t)i * R + r]) return fail(ctx, GF8_ERR_INVALID_ARG, "null host gradient");
+            CU_TRY(ctx, cudaMemcpyAsync(ctx->st_grads[(size_t)i * R + r], grads_host[(size_t)i * R + r], bytes,
+                                        cudaMemcpyHostToDevice, st));
+        }
+    }
+    for (int r = 0; r < R; ++r)
+        for (int i = 0; i < n; ++i)
+            GF_TRY(encode_one(ctx, layers[i], ctx->st_grads[(size_t)i * R + r], dt, ctx->st_codes[(size_t)i * R + r],
+                              ctx->st_sinv[(size_t)i * R + r], st));
+    for (int i = 0; i < n; ++i) {
+        GF_TRY(reduce_decoded_one(ctx, layers[i], (const uint8_t* const*)&ctx->st_codes[(size_t)i * R],
+                                  (const float* const*)&ctx->st_sinv[(size_t)i * R], R, average, ctx->st_out[i], dt, st));
+        const LayerState& L = ctx->layers[layers[i]];
+        if (!out_host[i]) return fail(ctx, GF8_ERR_INVALID_ARG, "null host output");
+        CU_TRY(ctx, cudaMemcpyAsync(out_host[i], ctx->st_out[i], (size_t)L.desc.d_out * L.desc.d_in * esz,
+                                    cudaMemcpyDeviceToHost, st));
+    }
+    return GF8_OK;
+}
+
+// ---- state access ---------------------------------------------------------------------------------------------
+gf8_status gf8_get_factor(gf8_ctx* ctx, int layer, int side, float* f, void* stream) {
+    GF_TRY(check_layer(ctx, layer));
+    SideState* s = side_of(ctx, ctx->layers[layer], side);
+    if (!s) return fail(ctx, GF8_ERR_INVALID_ARG, "layer %d does not use side %d", layer, side);
+    if (!f) return fail(ctx, GF8_ERR_INVALID_ARG, "null pointer");
+    if (!s->has_factor) return fail(ctx, GF8_ERR_BAD_STATE, "layer %d: no factor yet", layer);
+    CU_TRY(ctx, cudaMemcpyAsync(f, s->factor, sizeof(float) * (size_t)s->d * s->d, cudaMemcpyDeviceToDevice,
+                                (cudaStream_t)stream));
+    return GF8_OK;
+}
+
+gf8_status gf8_set_factor(gf8_ctx* ctx, int layer, int side, const float* f, void* stream) {
+    GF_TRY(check_layer(ctx, layer));
+    SideState* s = side_of(ctx, ctx->layers[layer], side);
+    if (!s) return fail(ctx, GF8_ERR_INVALID_ARG, "layer %d does not use side %d", layer, side);
+    if (!f) return fail(ctx, GF8_ERR_INVALID_ARG, "null pointer");
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    GF_TRY(ensure_factor(ctx, *s));
+    CU_TRY(ctx, cudaMemcpyAsync(s->factor, f, sizeof(float) * (size_t)s->d * s->d, cudaMemcpyDeviceToDevice,
+                                (cudaStream_t)stream));
+    s->has_factor = true;
+    return GF8_OK;
+}
+
+gf8_status gf8_get_basis(gf8_ctx* ctx, int layer, int side, float* U, float* mu, float* rho_host, void* stream) {
+    GF_TRY(check_layer(ctx, layer));
+    SideState* s = side_of(ctx, ctx->layers[layer], side);
+    if (!s) return fail(ctx, GF8_ERR_INVALID_ARG, "layer %d does not use side %d", layer, side);
+    if (!s->has_basis) return fail(ctx, GF8_ERR_BAD_STATE, "layer %d: no basis yet", layer);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (U) CU_TRY(ctx, cudaMemcpyAsync(U, s->U, sizeof(float) * (size_t)s->d * s->k, cudaMemcpyDeviceToDevice, st));
+    if (mu) CU_TRY(ctx, cudaMemcpyAsync(mu, s->mu, sizeof(float) * (size_t)s->k, cudaMemcpyDeviceToDevice, st));
+    if (rho_host) {
+        CU_TRY(ctx, cudaMemcpyAsync(rho_host, s->rho, sizeof(float), cudaMemcpyDeviceToHost, st));
+        CU_TRY(ctx, cudaStreamSynchronize(st));
+    }
+    return GF8_OK;
+}
+
+gf8_status gf8_set_basis(gf8_ctx* ctx, int layer, int side, const float* U, const float* mu, float rho, void* stream) {
+    GF_TRY(check_layer(ctx, layer));
+    LayerState& L = ctx->layers[layer];
+    SideState* s = side_of(ctx, L, side);
+    if (!s) return fail(ctx, GF8_ERR_INVALID_ARG, "layer %d does not use side %d", layer, side);
+    if (!U) return fail(ctx, GF8_ERR_INVALID_ARG, "null pointer");
+    if (mu && !(rho > 0.0f)) return fail(ctx, GF8_ERR_INVALID_ARG, "rho must be positive");
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    CU_TRY(ctx, cudaMemcpyAsync(s->U, U, sizeof(float) * (size_t)s->d * s->k, cudaMemcpyDeviceToDevice, st));
+    s->has_start = true;
+    if (mu) {
+        multipliers_kernel<<<1, 256, 0, st>>>(nullptr, s->d, s->k, nullptr, mu, (double)L.desc.damping, (double)rho,
+                                              s->mu, s->e, s->ebar, s->rho);
+        LAUNCH_CHECK(ctx);
+        s->has_basis = true;
+    } else {
+        s->has_basis = false;
+    }
+    return GF8_OK;
+}
+
+gf8_status gf8_whiten_f32(gf8_ctx* ctx, int layer, const void* grad, gf8_dtype dt, float* out, void* stream) {
+    GF_TRY(check_layer(ctx, layer));
+    LayerState& L = ctx->layers[layer];
+    if (!grad || !out) return fail(ctx, GF8_ERR_INVALID_ARG, "null pointer");
+    if (!aligned16(grad) || !aligned16(out)) return fail(ctx, GF8_ERR_UNSUPPORTED, "pointers must be 16-byte aligned");
+    if (dt != GF8_DT_BF16 && dt != GF8_DT_F32) return fail(ctx, GF8_ERR_INVALID_ARG, "bad dtype");
+    GF_TRY(check_basis(ctx, L, layer));
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    if (dt == GF8_DT_BF16) return transform_simt<bf16>(ctx, st, L, (const bf16*)grad, out, false);
+    if ((const void*)grad == (const void*)out) return fail(ctx, GF8_ERR_INVALID_ARG, "in-place whiten tap not allowed");
+    return transform_simt<float>(ctx, st, L, (const float*)grad, out, false);
+}
+
+gf8_status gf8_quantize_f32(gf8_ctx* ctx, int fmt, int scaling, const float* in, int64_t m, int64_t n, uint8_t* codes,
+                            float* scale_inv, void* stream) {
+    if (!ctx) return GF8_ERR_INVALID_ARG;
+    if (!in || !codes || !scale_inv) return fail(ctx, GF8_ERR_INVALID_ARG, "null pointer");
+    if (fmt < 0 || fmt > 1 || scaling < 0 || scaling > 1 || m < 1 || n < 1) return fail(ctx, GF8_ERR_INVALID_ARG, "bad argument");
+    if (n % 16 || (m * n) % 16) return fail(ctx, GF8_ERR_UNSUPPORTED, "n must be a multiple of 16");
+    if (!aligned16(in) || !aligned16(codes)) return fail(ctx, GF8_ERR_UNSUPPORTED, "pointers must be 16-byte aligned");
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    const size_t ns = n_scales_of(scaling, m, n);
+    if (ns > ctx->tap_cap) {
+        GF_TRY(dmalloc(ctx, &ctx->tap_amax, ns));
+        GF_TRY(dmalloc(ctx, &ctx->tap_scale, ns));
+        ctx->tap_cap = ns;
+    }
+    return quantize_dev<float>(ctx, (cudaStream_t)stream, in, m, n, fmt, scaling, ctx->tap_amax, ctx->tap_scale, codes,
+                               scale_inv);
+}
+
+gf8_status gf8_reduce_f32(gf8_ctx* ctx, int fmt, int scaling, const uint8_t* const* codes, const float* const* scale_inv,
+                          int R, int average, int64_t m, int64_t n, float* out, void* stream) {
+    if (!ctx) return GF8_ERR_INVALID_ARG;
+    if (!codes || !scale_inv || !out) return fail(ctx, GF8_ERR_INVALID_ARG, "null pointer");
+    if (R < 1 || R > GF8_MAX_R) return fail(ctx, GF8_ERR_INVALID_ARG, "R=%d out of range [1,%d]", R, GF8_MAX_R);
+    if (fmt < 0 || fmt > 1 || scaling < 0 || scaling > 1 || m < 1 || n < 1) return fail(ctx, GF8_ERR_INVALID_ARG, "bad argument");
+    if (n % 16) return fail(ctx, GF8_ERR_UNSUPPORTED, "n must be a multiple of 16");
+    for (int r = 0; r < R; ++r)
+        if (!codes[r] || !scale_inv[r] || !aligned16(codes[r])) return fail(ctx, GF8_ERR_INVALID_ARG, "bad payload pointer");
+    if (!aligned16(out)) return fail(ctx, GF8_ERR_UNSUPPORTED, "pointers must be 16-byte aligned");
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    return reduce_dev<float>(ctx, (cudaStream_t)stream, codes, scale_inv, R, average, m, n, fmt, scaling, out);
+}
+
+}  // extern "C"

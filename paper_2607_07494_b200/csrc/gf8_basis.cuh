@@ -1,0 +1,207 @@
+// gf8_basis.cuh -- the small dense pieces of a2 basis refresh (Eq. 24; S5):
+//   CholeskyQR orthonormalisation in FP64, the single-CTA Jacobi eigensolve of the k x k Rayleigh-Ritz
+//   matrix, and the multipliers (rho, e, ebar).  No host eigensolver, no host synchronisation.
+#pragma once
+#include "gf8_common.cuh"
+
+namespace gf8 {
+
+// ---- Cholesky of a k x k SPD Gram matrix, in place, upper factor R (G = R^T R), one CTA -----------
+// G row-major in global memory (k <= 512); only the upper triangle is read and written.
+__global__ void __launch_bounds__(1024) cholesky_upper_kernel(double* __restrict__ G, int k) {
+    __shared__ double s_diag;
+    for (int j = 0; j < k; ++j) {
+        if (threadIdx.x == 0) {
+            double d = G[(int64_t)j * k + j];
+            // Breakdown guard: a non-positive pivot (rank-deficient start basis) becomes a tiny one,
+            // so the column is kept finite and the second CholeskyQR pass re-orthonormalises it.
+            if (!(d > 0.0)) d = 1e-300;
+            s_diag = sqrt(d);
+            G[(int64_t)j * k + j] = s_diag;
+        }
+        __syncthreads();
+        const double rjj = s_diag;
+        for (int l = j + 1 + threadIdx.x; l < k; l += blockDim.x) G[(int64_t)j * k + l] /= rjj;
+        __syncthreads();
+        // trailing update of the upper triangle: G[i][l] -= R[j][i] * R[j][l], j < i <= l
+        const int rem = k - j - 1;
+        for (int idx = threadIdx.x; idx < rem * rem; idx += blockDim.x) {
+            const int i = j + 1 + idx / rem, l = j + 1 + idx % rem;
+            if (l >= i) G[(int64_t)i * k + l] -= G[(int64_t)j * k + i] * G[(int64_t)j * k + l];
+        }
+        __syncthreads();
+    }
+}
+
+// ---- V <- V R^-1 (R upper triangular), one thread per row of V (d x k, FP64, in place) -----------
+__global__ void __launch_bounds__(128) trisolve_rows_kernel(double* __restrict__ V, const double* __restrict__ Rm,
+                                                            int d, int k) {
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= d) return;
+    double* v = V + (int64_t)r * k;
+    for (int j = 0; j < k; ++j) {
+        double x = v[j];
+        for (int i = 0; i < j; ++i) x -= v[i] * Rm[(int64_t)i * k + j];
+        v[j] = x / Rm[(int64_t)j * k + j];
+    }
+}
+
+// ---- Single-CTA parallel-order two-sided Jacobi on a symmetric k x k matrix (FP64) ----------------
+// B (k x k) is overwritten; Z receives the eigenvectors (columns).  If the two matrices fit in
+// dynamic shared memory (use_smem) they are staged there, otherwise the CTA works on global / L2.
+// Round-robin ordering: k-1 rounds of k/2 disjoint rotations per sweep.  Output: mu sorted
+// descending, Zs = Z with its columns permuted into that order.
+__global__ void __launch_bounds__(1024) jacobi_kernel(double* __restrict__ Bg, double* __restrict__ Zg, int k,
+                                                      int use_smem, double* __restrict__ mu_sorted,
+                                                      double* __restrict__ Zs, int max_sweeps) {
+    extern __shared__ double s_dyn[];
+    __shared__ double s_c[256], s_s[256];
+    __shared__ int s_p[256], s_q[256];
+    __shared__ double s_red[64];
+    __shared__ int s_done;
+    const int tid = threadIdx.x, nt = blockDim.x;
+    double* B = use_smem ? s_dyn : Bg;
+    double* Z = use_smem ? s_dyn + (size_t)k * k : Zg;
+    // load + symmetrise; Z = I
+    for (int idx = tid; idx < k * k; idx += nt) {
+        const int i = idx / k, j = idx % k;
+        if (use_smem) B[idx] = 0.5 * (Bg[(int64_t)i * k + j] + Bg[(int64_t)j * k + i]);
+        Z[idx] = (i == j) ? 1.0 : 0.0;
+    }
+    __syncthreads();
+    if (!use_smem) {                    // in-place symmetrisation on global memory
+        for (int idx = tid; idx < k * k; idx += nt) {
+            const int i = idx / k, j = idx % k;
+            if (i < j) {
+                const double v = 0.5 * (B[(int64_t)i * k + j] + B[(int64_t)j * k + i]);
+                B[(int64_t)i * k + j] = v;
+                B[(int64_t)j * k + i] = v;
+            }
+        }
+        __syncthreads();
+    }
+    const int ke = (k + 1) & ~1;        // players (one dummy when k is odd)
+    const int half = ke / 2;
+    for (int sweep = 0; sweep < max_sweeps; ++sweep) {
+        // convergence: off(B) <= 1e-14 ||B||_F
+        double off = 0.0, fro = 0.0;
+        for (int idx = tid; idx < k * k; idx += nt) {
+            const double v = B[idx];
+            fro += v * v;
+            if (idx / k != idx % k) off += v * v;
+        }
+        for (int o = 16; o > 0; o >>= 1) {
+            off += __shfl_xor_sync(0xFFFFFFFFu, off, o);
+            fro += __shfl_xor_sync(0xFFFFFFFFu, fro, o);
+        }
+        if ((tid & 31) == 0) { s_red[tid >> 5] = off; s_red[32 + (tid >> 5)] = fro; }
+        __syncthreads();
+        if (tid == 0) {
+            double o2 = 0, f2 = 0;
+            for (int w = 0; w < (nt + 31) / 32; ++w) { o2 += s_red[w]; f2 += s_red[32 + w]; }
+            s_done = (sqrt(o2) <= 1e-14 * sqrt(f2)) ? 1 : 0;
+        }
+        __syncthreads();
+        if (s_done) break;
+        for (int round = 0; round < ke - 1; ++round) {
+            // pairs of this round + rotation angles
+            for (int i = tid; i < half; i += nt) {
+                int p, q;
+                if (i == 0) { p = ke - 1; q = round; }
+                else { p = (round + i) % (ke - 1); q = (round - i + (ke - 1)) % (ke - 1); }
+                if (p > q) { const int t = p; p = q; q = t; }
+                double c = 1.0, s = 0.0;
+                if (q < k) {
+                    const double bpq = B[(int64_t)p * k + q];
+                    if (bpq != 0.0) {
+                        const double tau = (B[(int64_t)q * k + q] - B[(int64_t)p * k + p]) / (2.0 * bpq);
+                        const double t = (tau >= 0 ? 1.0 : -1.0) / (fabs(tau) + sqrt(1.0 + tau * tau));
+                        c = 1.0 / sqrt(1.0 + t * t);
+                        s = t * c;
+                    }
+                } else { q = -1; }
+                s_p[i] = p; s_q[i] = q; s_c[i] = c; s_s[i] = s;
+            }
+            __syncthreads();
+            // B <- B J and Z <- Z J  (columns p, q of every row)
+            for (int idx = tid; idx < half * k; idx += nt) {
+                const int i = idx / k, r = idx % k;
+                const int p = s_p[i], q = s_q[i];
+                if (q < 0) continue;
+                const double c = s_c[i], s = s_s[i];
+                const double bp = B[(int64_t)r * k + p], bq = B[(int64_t)r * k + q];
+                B[(int64_t)r * k + p] = c * bp - s * bq;
+                B[(int64_t)r * k + q] = s * bp + c * bq;
+                const double zp = Z[(int64_t)r * k + p], zq = Z[(int64_t)r * k + q];
+                Z[(int64_t)r * k + p] = c * zp - s * zq;
+                Z[(int64_t)r * k + q] = s * zp + c * zq;
+            }
+            __syncthreads();
+            // B <- J^T B  (rows p, q of every column)
+            for (int idx = tid; idx < half * k; idx += nt) {
+                const int i = idx / k, j = idx % k;
+                const int p = s_p[i], q = s_q[i];
+                if (q < 0) continue;
+                const double c = s_c[i], s = s_s[i];
+                const double bp = B[(int64_t)p * k + j], bq = B[(int64_t)q * k + j];
+                B[(int64_t)p * k + j] = c * bp - s * bq;
+                B[(int64_t)q * k + j] = s * bp + c * bq;
+            }
+            __syncthreads();
+        }
+    }
+    // rank sort (descending, ties by index) and permuted eigenvector output
+    for (int i = tid; i < k; i += nt) {
+        const double mi = B[(int64_t)i * k + i];
+        int rank = 0;
+        for (int j = 0; j < k; ++j) {
+            const double mj = B[(int64_t)j * k + j];
+            rank += (mj > mi) || (mj == mi && j < i);
+        }
+        mu_sorted[rank] = mi;
+        // column i of Z goes to column `rank` of Zs
+        for (int r = 0; r < k; ++r) Zs[(int64_t)r * k + rank] = Z[(int64_t)r * k + i];
+    }
+}
+
+// ---- trace(A) in FP64 and the multipliers (S2, S3) ---------------------------------------
+//   rho = max(0, (tr A - sum mu) / (d - k)) + lam   (k == d: rho = mu_k + lam)
+//   D_i = sqrt(rho / (mu_i + lam)),  e_i = D_i - 1,  ebar_i = 1/D_i - 1
+// One CTA.  If `trace_from` is null, rho_in is used as given (gf8_set_basis).
+__global__ void __launch_bounds__(256) multipliers_kernel(const float* __restrict__ factor, int d, int k,
+                                                          const double* __restrict__ mu64, const float* __restrict__ mu32,
+                                                          double lam, double rho_in, float* __restrict__ mu_out,
+                                                          float* __restrict__ e, float* __restrict__ ebar,
+                                                          float* __restrict__ rho_out) {
+    __shared__ double s_part[256];
+    __shared__ double s_rho;
+    double tr = 0.0, sm = 0.0;
+    if (factor) for (int i = threadIdx.x; i < d; i += blockDim.x) tr += (double)factor[(int64_t)i * d + i];
+    for (int i = threadIdx.x; i < k; i += blockDim.x) {
+        const double m = mu64 ? fmax(mu64[i], 0.0) : (double)mu32[i];
+        sm += m;
+    }
+    s_part[threadIdx.x] = tr - sm;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int i = 0; i < blockDim.x; ++i) t += s_part[i];
+        double rho;
+        if (!factor) rho = rho_in;
+        else if (k < d) rho = fmax(0.0, t / (double)(d - k)) + lam;
+        else rho = (mu64 ? fmax(mu64[k - 1], 0.0) : (double)mu32[k - 1]) + lam;
+        s_rho = rho;
+        *rho_out = (float)rho;
+    }
+    __syncthreads();
+    const double rho = s_rho;
+    for (int i = threadIdx.x; i < k; i += blockDim.x) {
+        const double m = mu64 ? fmax(mu64[i], 0.0) : (double)mu32[i];
+        const double D = sqrt(rho / (m + lam));
+        mu_out[i] = (float)m;
+        e[i] = (float)(D - 1.0);
+        ebar[i] = (float)(1.0 / D - 1.0);
+    }
+}
+
+}  // namespace gf8

@@ -1,0 +1,277 @@
+"""Parity gates G1-G7: the CUDA path (through the C ABI) against the CPU oracle on the same seeded
+inputs, element by element.  Upstream state is handed across so each stage is isolated
+(DESIGN.md "Parity gates").  Sizes span several 64/128-wide tiles plus a ragged tail and finish
+on the oracle in seconds."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2607_07494_b200 import gf8, synth
+from tests._util import Case, bf16_bits, bf16_ordinal, code_mismatch, relfro, to_np64
+
+pytestmark = pytest.mark.gpu
+
+TOL_EXACT = 1e-4          # north_star: transform within 1e-4 relative Frobenius in FP32
+MISMATCH_FRAC = 1e-4      # north_star: <= 1e-4 of FP8 codes differ, never by more than one step
+
+
+@pytest.fixture(scope="module")
+def ctx0():
+    return gf8.create([gf8.Layer(256, 256, gf8.SIDE_NONE)])
+
+
+def _dev(a, dtype=None):
+    t = torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    return t.to(dtype) if dtype is not None else t
+
+
+# ---- G1: quantizer, bit-exact -------------------------------------------------------------------------
+@pytest.mark.parametrize("fmt", [gf8.E4M3, gf8.E5M2])
+@pytest.mark.parametrize("scaling", [gf8.SCALE_TENSOR, gf8.SCALE_BLOCK128])
+@pytest.mark.parametrize("shape", [(256, 256), (208, 336), (1, 16), (515, 1040)])
+def test_g1_quantizer_bit_exact(ctx0, fmt, scaling, shape):
+    rng = np.random.default_rng(hash((fmt, scaling, shape)) % 2**32)
+    m, n = shape
+    x = (rng.normal(0, 1, (m, n)) * np.exp(rng.normal(0, 3, (m, n)))).astype(np.float32)
+    x[rng.integers(0, m), rng.integers(0, n)] = 0.0
+    x[rng.integers(0, m), rng.integers(0, n)] = -0.0
+    oc, os_ = oracle.quantize(x, fmt, scaling)
+    gc, gs = ctx0.quantize_f32(_dev(x), fmt, scaling)
+    assert np.array_equal(gs.cpu().numpy().view(np.uint32), os_.view(np.uint32))
+    assert np.array_equal(gc.cpu().numpy(), oc)
+
+
+@pytest.mark.parametrize("fmt", [gf8.E4M3, gf8.E5M2])
+def test_g1_quantizer_edge_values(ctx0, fmt):
+    tab = oracle.fp8_table(fmt)
+    pos = tab[:128][np.isfinite(tab[:128])]
+    mids = 0.5 * (pos[:-1] + pos[1:])
+    fmax = oracle.fp8_max(fmt)
+    # every representable value, every rounding midpoint and its two FP32 neighbours, with amax == fmax
+    # so that scale == 1 and the cast is exercised exactly at its decision points
+    v = np.concatenate([pos, mids, np.nextafter(mids.astype(np.float32), np.float32(0)),
+                        np.nextafter(mids.astype(np.float32), np.float32(np.inf))]).astype(np.float32)
+    v = np.concatenate([v, -v, [fmax, -fmax]]).astype(np.float32)
+    v = np.concatenate([v, np.zeros((-len(v)) % 16, np.float32)]).reshape(1, -1)
+    oc, os_ = oracle.quantize(v, fmt)
+    gc, gs = ctx0.quantize_f32(_dev(v), fmt)
+    assert os_[0] == 1.0 and gs.item() == 1.0
+    assert np.array_equal(gc.cpu().numpy(), oc)
+    # degenerate tensors (S13): zeros; amax so small that fmax/amax overflows; non-finite input
+    for x in [np.zeros((16, 32), np.float32), np.full((2, 16), 1e-44, np.float32),
+              np.array([[1.0, np.nan, -np.inf, 3.0] * 4], np.float32)]:
+        oc, os_ = oracle.quantize(x, fmt)
+        gc, gs = ctx0.quantize_f32(_dev(x), fmt)
+        assert np.array_equal(gs.cpu().numpy(), os_)
+        g, o = gc.cpu().numpy(), oc
+        nan_o = np.isnan(tab[o])
+        assert np.array_equal(np.isnan(tab[g]), nan_o) and np.array_equal(g[~nan_o], o[~nan_o])
+
+
+# ---- G4: reduce, bit-exact ------------------------------------------------------------------------------
+@pytest.mark.parametrize("fmt", [gf8.E4M3, gf8.E5M2])
+@pytest.mark.parametrize("scaling", [gf8.SCALE_TENSOR, gf8.SCALE_BLOCK128])
+@pytest.mark.parametrize("R,average", [(1, False), (2, True), (5, True), (16, True)])
+def test_g4_reduce_bit_exact(ctx0, fmt, scaling, R, average):
+    rng = np.random.default_rng(R * 7 + fmt)
+    m, n = 200, 272
+    pays = [oracle.quantize((rng.normal(0, 1 + r, (m, n))).astype(np.float32), fmt, scaling) for r in range(R)]
+    want = oracle.reduce([p[0] for p in pays], [p[1] for p in pays], fmt, scaling, average)
+    got = ctx0.reduce_f32([_dev(p[0]) for p in pays], [_dev(p[1]) for p in pays], fmt, scaling, average)
+    assert np.array_equal(got.cpu().numpy().view(np.uint32), want.view(np.uint32))
+
+
+# ---- G2 / G3 / G5 on whitened layers -------------------------------------------------------------------
+CASES = {
+    "config0": dict(m=256, n=256, kG=16, kA=16, side=gf8.SIDE_BOTH, dtype="f32", seed=0, T=512, q=8),
+    "ragged-bf16": dict(m=336, n=592, kG=24, kA=40, side=gf8.SIDE_BOTH, dtype="bf16", seed=1),
+    "in-only": dict(m=320, n=448, kG=0, kA=32, side=gf8.SIDE_IN, dtype="bf16", seed=2),
+    "out-only": dict(m=448, n=208, kG=16, kA=0, side=gf8.SIDE_OUT, dtype="f32", seed=3),
+    "block-e5m2": dict(m=272, n=400, kG=8, kA=8, side=gf8.SIDE_BOTH, dtype="bf16", seed=4, fmt=gf8.E5M2,
+                       scaling=gf8.SCALE_BLOCK128),
+}
+_cache = {}
+
+
+def case(name):
+    if name not in _cache:
+        _cache[name] = Case(**CASES[name])
+    return _cache[name]
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_g2_transform(name):
+    c = case(name)
+    wt = c.ctx.whiten_f32(0, c.G)
+    _, _, x = c.oracle_encode(c.G)
+    assert relfro(to_np64(wt), x) <= TOL_EXACT
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_g3_encode_end_to_end(name):
+    c = case(name)
+    for r in range(2):
+        g = c.rank_grad(r)
+        oc, os_, _ = c.oracle_encode(g)
+        gc, gs = c.ctx.encode(0, g)
+        assert np.allclose(gs.cpu().numpy(), os_, rtol=1e-5, atol=0)
+        frac, worst = code_mismatch(gc.cpu().numpy(), oc)
+        assert worst <= 1 and frac <= MISMATCH_FRAC, (frac, worst)
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_g5_reduce_decoded(name):
+    c = case(name)
+    R = 3
+    pays = [c.oracle_encode(c.rank_grad(r))[:2] for r in range(R)]           # oracle payloads, handed across
+    want = c.oracle_reduce_decoded([p[0] for p in pays], [p[1] for p in pays])
+    dc, ds = [_dev(p[0]) for p in pays], [_dev(p[1]) for p in pays]
+    got32 = c.ctx.reduce_decoded(0, dc, ds, True, dt=gf8.DT_F32)
+    assert relfro(to_np64(got32), want) <= TOL_EXACT
+    got16 = c.ctx.reduce_decoded(0, dc, ds, True, dt=gf8.DT_BF16)
+    d = np.abs(bf16_ordinal(bf16_bits(got16)) - bf16_ordinal(oracle.to_bf16_bits(want)))
+    # BF16 output within 1 ulp of the RNE-rounded oracle value (double rounding through FP32), except
+    # where the FP32 error itself spans many BF16 ulps of a near-zero element
+    small = np.abs(want) < 1e-3 * np.abs(want).max()
+    assert d[~small].max() <= 1 and (d > 1).mean() < 1e-3
+    # gf8_decode is the R = 1, no-average case
+    one = c.ctx.decode(0, dc[0], ds[0], dt=gf8.DT_F32)
+    want1 = c.oracle_reduce_decoded(pays[0][:1], [pays[0][1]], average=False)
+    assert relfro(to_np64(one), want1) <= TOL_EXACT
+
+
+def test_euclidean_layer_is_plain_fp8():
+    """side = NONE (embedding / LM head): codes and decoded values bit-exact."""
+    m, n = 400, 256
+    ctx = gf8.create([gf8.Layer(m, n, gf8.SIDE_NONE)])
+    G = synth.gradient(m, n, "cuda", 77).to(torch.bfloat16)
+    R = 4
+    grads = [synth.rank_gradient(G, r, 5).to(torch.bfloat16) for r in range(R)]
+    pays_o = [oracle.quantize(g.float().cpu().numpy()) for g in grads]
+    pays_g = [ctx.encode(0, g) for g in grads]
+    for (oc, os_), (gc, gs) in zip(pays_o, pays_g):
+        assert np.array_equal(gc.cpu().numpy(), oc) and np.array_equal(gs.cpu().numpy(), os_)
+    want = oracle.reduce([p[0] for p in pays_o], [p[1] for p in pays_o])
+    got = ctx.reduce_decoded(0, [p[0] for p in pays_g], [p[1] for p in pays_g], True, dt=gf8.DT_F32)
+    assert np.array_equal(got.cpu().numpy(), want)
+    got16 = ctx.reduce_decoded(0, [p[0] for p in pays_g], [p[1] for p in pays_g], True, dt=gf8.DT_BF16)
+    assert np.array_equal(bf16_bits(got16), oracle.to_bf16_bits(want.astype(np.float64)))
+
+
+def test_isotropic_factors_reduce_to_euclidean_on_gpu():
+    """Identity / isotropic factors => T = I => payload identical to side = NONE (north_star check)."""
+    m, n, k = 256, 320, 16
+    ctx = gf8.create([gf8.Layer(m, n, gf8.SIDE_BOTH, k, k), gf8.Layer(m, n, gf8.SIDE_NONE)])
+    ctx.set_factor(0, gf8.SIDE_IN, (2.5 * torch.eye(n, device="cuda")).contiguous())
+    ctx.set_factor(0, gf8.SIDE_OUT, (0.3 * torch.eye(m, device="cuda")).contiguous())
+    ctx.set_basis(0, gf8.SIDE_IN, synth.start_basis(n, k, "cuda", 1))
+    ctx.set_basis(0, gf8.SIDE_OUT, synth.start_basis(m, k, "cuda", 2))
+    ctx.refresh_basis(0, 2)
+    G = synth.gradient(m, n, "cuda", 5).to(torch.bfloat16)
+    c1, s1 = ctx.encode(0, G)
+    c0, s0 = ctx.encode(1, G)
+    assert torch.equal(c1, c0) and torch.equal(s1, s0)
+
+
+# ---- G6: factor accumulate --------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["config0", "ragged-bf16"])
+def test_g6_factor(name):
+    c = case(name)
+    ctx = gf8.create([c.layer])
+    ctx.factor_update(0, c.X, c.D)
+    assert relfro(to_np64(ctx.get_factor(0, gf8.SIDE_IN)), c.A) <= TOL_EXACT
+    assert relfro(to_np64(ctx.get_factor(0, gf8.SIDE_OUT)), c.Gf) <= TOL_EXACT
+
+
+def test_g6_factor_ema():
+    m, n, k, T = 128, 192, 8, 300
+    lay = gf8.Layer(m, n, gf8.SIDE_IN, k, 0, ema_beta=0.9)
+    ctx = gf8.create([lay])
+    X1 = synth.factor_samples(T, n, "cuda", 31)
+    X2 = synth.factor_samples(T + 20, n, "cuda", 32)
+    ctx.factor_update(0, X1, None)
+    ctx.factor_update(0, X2, None)
+    A = oracle.factor_accumulate(to_np64(X1))
+    A = oracle.factor_accumulate(to_np64(X2), A, 0.9)
+    assert relfro(to_np64(ctx.get_factor(0, gf8.SIDE_IN)), A) <= TOL_EXACT
+
+
+# ---- G7: basis refresh (same factor bits, same V0, same q) ------------------------------------------------
+@pytest.mark.parametrize("name,q", [("config0", 8), ("ragged-bf16", 3), ("config0", 0)])
+def test_g7_basis(name, q):
+    c = case(name)
+    ctx = gf8.create([c.layer])
+    for side, F, V0, k in ((gf8.SIDE_IN, c.A, c.V0A, c.kA), (gf8.SIDE_OUT, c.Gf, c.V0G, c.kG)):
+        f32 = torch.from_numpy(F).float().cuda().contiguous()
+        ctx.set_factor(0, side, f32)
+        ctx.set_basis(0, side, V0)
+    ctx.refresh_basis(0, q)
+    for side, F, V0, k in ((gf8.SIDE_IN, c.A, c.V0A, c.kA), (gf8.SIDE_OUT, c.Gf, c.V0G, c.kG)):
+        F32 = torch.from_numpy(F).float().double().numpy()                       # the bits the GPU holds
+        b = oracle.refresh_basis(F32, to_np64(V0), q, c.damping)
+        U, mu, rho = ctx.get_basis(0, side)
+        U, mu = to_np64(U), to_np64(mu)
+        assert np.abs(U.T @ U - np.eye(k)).max() <= 1e-5
+        lam = c.damping
+        assert np.abs(mu - b.mu).max() <= 1e-4 * (b.mu.min() + lam) and abs(rho - b.rho) <= 1e-5 * b.rho
+        D = np.sqrt(rho / (mu + lam))
+        T_gpu = np.eye(U.shape[0]) + (U * (D - 1)) @ U.T
+        T_orc = oracle.build_T(b.U, b.e)
+        assert relfro(T_gpu, T_orc) <= TOL_EXACT
+    # refreshed basis is usable by the codec and matches the oracle's codes within the G3 budget
+    g = c.rank_grad(0)
+    F32A = torch.from_numpy(c.A).float().double().numpy()
+    F32G = torch.from_numpy(c.Gf).float().double().numpy()
+    bA = oracle.refresh_basis(F32A, to_np64(c.V0A), q, c.damping)
+    bG = oracle.refresh_basis(F32G, to_np64(c.V0G), q, c.damping)
+    oc, os_, x = oracle.encode(to_np64(g), bG, bA, c.fmt, c.scaling)
+    wt = ctx.whiten_f32(0, g)
+    assert relfro(to_np64(wt), x) <= TOL_EXACT
+
+
+def test_bad_state_and_argument_errors():
+    ctx = gf8.create([gf8.Layer(256, 256, gf8.SIDE_BOTH, 8, 8)])
+    G = torch.zeros(256, 256, device="cuda")
+    with pytest.raises(gf8.Gf8Error) as e:
+        ctx.encode(0, G)                                                   # no basis yet
+    assert e.value.status == 2
+    with pytest.raises(gf8.Gf8Error) as e:
+        ctx.refresh_basis(0, 2)                                            # no factor yet
+    assert e.value.status == 2
+    with pytest.raises(gf8.Gf8Error) as e:
+        ctx.encode(3, G)
+    assert e.value.status == 1
+    codes = torch.zeros(256 * 256 + 16, dtype=torch.uint8, device="cuda")
+    ctx2 = gf8.create([gf8.Layer(256, 256, gf8.SIDE_NONE)])
+    with pytest.raises(gf8.Gf8Error) as e:                                 # misaligned codes pointer
+        ctx2.encode(0, G, codes[1:256 * 256 + 1].view(256, 256), torch.zeros(1, device="cuda"))
+    assert e.value.status == 3
+
+
+# ---- chain: whole pipeline, each side on its own upstream state (reported, loosely bounded) --------------
+def test_chain_config0_reports_metrics():
+    cfg = synth.config(0)
+    t = cfg.tensors[0]
+    lay = gf8.Layer(t.d_out, t.d_in, t.side, t.rank, t.rank, cfg.fmt, cfg.scaling, cfg.damping)
+    ctx = gf8.create([lay])
+    G = synth.tensor_gradient(cfg, t, "cuda")
+    X = synth.tensor_factor_samples(cfg, t, "in", "cuda")
+    D = synth.tensor_factor_samples(cfg, t, "out", "cuda")
+    V0A, V0G = synth.tensor_start_basis(cfg, t, "in", "cuda"), synth.tensor_start_basis(cfg, t, "out", "cuda")
+    ctx.factor_update(0, X, D)
+    ctx.set_basis(0, gf8.SIDE_IN, V0A)
+    ctx.set_basis(0, gf8.SIDE_OUT, V0G)
+    ctx.refresh_basis(0, 8)
+    grads = [synth.tensor_rank_gradient(cfg, t, G, r) for r in range(cfg.R)]
+    pays = [ctx.encode(0, g) for g in grads]
+    out = ctx.reduce_decoded(0, [p[0] for p in pays], [p[1] for p in pays], True, dt=gf8.DT_F32)
+    # oracle chain on its own state
+    bA = oracle.refresh_basis(oracle.factor_accumulate(to_np64(X)), to_np64(V0A), 8, cfg.damping)
+    bG = oracle.refresh_basis(oracle.factor_accumulate(to_np64(D)), to_np64(V0G), 8, cfg.damping)
+    po = [oracle.encode(to_np64(g), bG, bA)[:2] for g in grads]
+    want = oracle.reduce_decoded([p[0] for p in po], [p[1] for p in po], bG, bA)
+    mean = sum(to_np64(g) for g in grads) / cfg.R
+    mg, mo = oracle.metrics(to_np64(out), mean), oracle.metrics(want, mean)
+    print("chain config0  gpu:", mg, " oracle:", mo)
+    assert abs(mg["RelL2"] - mo["RelL2"]) < 0.02 * mo["RelL2"] and relfro(to_np64(out), want) < 0.02
