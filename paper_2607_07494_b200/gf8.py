@@ -175,10 +175,13 @@ class Ctx:
 
     def payload_size(self, layer):
         a, b = C.c_size_t(), C.c_size_t()
-        self._ck(lib().gf8_payload_size(self._h, layer, C.byref(a), C.byref(b)))
+        st = lib().gf8_payload_size(self._h, layer, C.byref(a), C.byref(b))
+        if st != 0:
+            raise Gf8Error(st, f"layer {layer} out of range")
         return a.value, b.value
 
     def _payload_buffers(self, layer):
+        self.payload_size(layer)                       # range check is the library's (GF8_ERR_INVALID_ARG)
         l = self.layers[layer]
         return (torch.empty((l.d_out, l.d_in), dtype=torch.uint8, device=self._tdev),
                 torch.empty((l.n_scales(),), dtype=torch.float32, device=self._tdev))
