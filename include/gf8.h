@@ -81,6 +81,9 @@ gf8_status gf8_destroy(gf8_ctx* ctx);
 gf8_status gf8_payload_size(const gf8_ctx* ctx, int layer, size_t* code_bytes, size_t* n_scales);
 const char* gf8_status_string(gf8_status s);
 const char* gf8_last_error(const gf8_ctx* ctx);
+/* Synchronises `stream` and reports asynchronous failures: GF8_ERR_CUDA if a kernel faulted or if the
+ * tensor-core engine flagged a pipeline time-out (its bounded waits drain instead of hanging the GPU). */
+gf8_status gf8_sync_check(gf8_ctx* ctx, void* stream);
 /* Number of kernels this context has launched so far (bench.py's gpu_launches). */
 int64_t gf8_launch_count(const gf8_ctx* ctx);
 

@@ -13,112 +13,10 @@
 
 using namespace gf8;
 
-namespace {
-
-struct SideState {
-    int d = 0, k = 0;
-    bool used = false;
-    float* factor = nullptr;   // d x d FP32 (lazy)
-    bool has_factor = false;   // at least one update / set
-    float* U = nullptr;        // d x k FP32 row-major
-    float* mu = nullptr;       // k
-    float* e = nullptr;        // k  encode multipliers
-    float* ebar = nullptr;     // k  decode multipliers
-    float* rho = nullptr;      // 1
-    bool has_start = false, has_basis = false;
-};
-
-struct LayerState {
-    gf8_layer_desc desc;
-    SideState in, out;         // in: A / U_A (d_in), out: Gf / U_G (d_out)
-    size_t n_scales = 1;
-    uint32_t* amax_bits = nullptr;   // n_scales
-    float* scale = nullptr;          // n_scales
-    float* P = nullptr;              // m x kA
-    float* Q = nullptr;              // kG x n
-    float* S = nullptr;              // kG x kA
-};
-
-}  // namespace
-
-struct gf8_ctx {
-    int device = 0;
-    gf8_precision precision = GF8_PREC_EXACT;
-    std::vector<LayerState> layers;
-    std::vector<void*> allocs;
-    float* wt_scratch = nullptr;     // max m*n FP32
-    // refresh scratch (FP64)
-    double *V = nullptr, *Y = nullptr, *Gm = nullptr, *Bm = nullptr, *Zm = nullptr, *Zs = nullptr, *mu64 = nullptr;
-    // tap scratch (gf8_quantize_f32 with arbitrary shapes)
-    uint32_t* tap_amax = nullptr; float* tap_scale = nullptr; size_t tap_cap = 0;
-    // host-step staging
-    std::vector<void*> stage_allocs;
-    std::vector<void*> st_grads; std::vector<uint8_t*> st_codes; std::vector<float*> st_sinv; std::vector<void*> st_out;
-    std::vector<int> st_layers; int st_R = 0; int st_dt = -1;
-    int64_t launches = 0;
-    int num_sms = 148;
-    char err[512] = {0};
-};
+#include "gf8_ctx.cuh"
+#include "gf8_fast.cuh"
 
 namespace {
-
-gf8_status fail(gf8_ctx* c, gf8_status s, const char* fmt, ...) {
-    if (c) {
-        va_list ap;
-        va_start(ap, fmt);
-        vsnprintf(c->err, sizeof(c->err), fmt, ap);
-        va_end(ap);
-    }
-    return s;
-}
-
-#define CU_TRY(ctx, expr)                                                                            \
-    do {                                                                                             \
-        cudaError_t _e = (expr);                                                                     \
-        if (_e != cudaSuccess)                                                                       \
-            return fail((ctx), GF8_ERR_CUDA, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e), \
-                        __FILE__, __LINE__);                                                         \
-    } while (0)
-
-#define GF_TRY(expr)                       \
-    do {                                   \
-        gf8_status _s = (expr);            \
-        if (_s != GF8_OK) return _s;       \
-    } while (0)
-
-#define LAUNCH_CHECK(ctx)                  \
-    do {                                   \
-        (ctx)->launches++;                 \
-        CU_TRY((ctx), cudaGetLastError()); \
-    } while (0)
-
-inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
-
-template <typename T>
-gf8_status dmalloc(gf8_ctx* c, T** p, size_t count, std::vector<void*>* track = nullptr) {
-    void* q = nullptr;
-    cudaError_t e = cudaMalloc(&q, count * sizeof(T) + 16);
-    if (e != cudaSuccess) {
-        cudaGetLastError();
-        return fail(c, GF8_ERR_NOMEM, "cudaMalloc of %zu bytes failed: %s", count * sizeof(T), cudaGetErrorString(e));
-    }
-    (track ? *track : c->allocs).push_back(q);
-    *p = static_cast<T*>(q);
-    return GF8_OK;
-}
-
-inline size_t n_scales_of(int scaling, int64_t m, int64_t n) {
-    return scaling == GF8_SCALE_TENSOR ? 1 : (size_t)((m + 127) / 128) * (size_t)((n + 127) / 128);
-}
-inline float fmax_of(int fmt) { return fmt == GF8_E4M3 ? 448.0f : 57344.0f; }
-
-inline int grid_for(gf8_ctx* c, int64_t work_items, int threads, int per_sm) {
-    int64_t blocks = (work_items + threads - 1) / threads;
-    const int64_t cap = (int64_t)c->num_sms * per_sm;
-    if (blocks > cap) blocks = cap;
-    if (blocks < 1) blocks = 1;
-    return (int)blocks;
-}
 
 // ---- GEMM launcher -------------------------------------------------------------------------------
 template <typename TA, typename TB, typename TC, typename TAcc>
@@ -177,13 +75,14 @@ gf8_status quantize_dev(gf8_ctx* c, cudaStream_t st, const T* x, int64_t m, int6
 // ---- reduce on device (a7) -----------------------------------------------------------------------------
 template <typename OutT>
 gf8_status reduce_dev(gf8_ctx* c, cudaStream_t st, const uint8_t* const* codes, const float* const* sinv, int R,
-                      int average, int64_t m, int64_t n, int fmt, int scaling, OutT* out) {
+                      int average, int64_t m, int64_t n, int fmt, int scaling, OutT* out, bf16* out16 = nullptr,
+                      bf16* out16_lo = nullptr) {
     ReducePtrs p;
     memset(&p, 0, sizeof(p));
     for (int r = 0; r < R; ++r) { p.codes[r] = codes[r]; p.sinv[r] = sinv[r]; }
     const int g = grid_for(c, m * n / 16, 256, 8);
-    if (fmt == GF8_E4M3) reduce_kernel<0, OutT><<<g, 256, 0, st>>>(p, R, average, m, n, scaling, out);
-    else reduce_kernel<1, OutT><<<g, 256, 0, st>>>(p, R, average, m, n, scaling, out);
+    if (fmt == GF8_E4M3) reduce_kernel<0, OutT><<<g, 256, 0, st>>>(p, R, average, m, n, scaling, out, out16, out16_lo);
+    else reduce_kernel<1, OutT><<<g, 256, 0, st>>>(p, R, average, m, n, scaling, out, out16, out16_lo);
     LAUNCH_CHECK(c);
     return GF8_OK;
 }
@@ -303,6 +202,7 @@ gf8_status refresh_side(gf8_ctx* c, cudaStream_t st, SideState& s, double lam, i
                                                        1.0, 0.0)));
     multipliers_kernel<<<1, 256, 0, st>>>(s.factor, d, k, c->mu64, nullptr, lam, 0.0, s.mu, s.e, s.ebar, s.rho);
     LAUNCH_CHECK(c);
+    GF_TRY(fast_pack_basis(c, st, s));
     s.has_basis = true;
     return GF8_OK;
 }
@@ -358,6 +258,160 @@ gf8_status reduce_decoded_one(gf8_ctx* c, int layer, const uint8_t* const* codes
     return GF8_OK;
 }
 
+
+// ---- FAST path: batched calls through cached plans of tensor-core items ---------------------------------------
+enum { PLAN_ENCODE = 1, PLAN_DECODE = 2, PLAN_WHITEN = 3 };
+
+inline void key_ptr(std::vector<uint64_t>& k, const void* p) { k.push_back((uint64_t)(uintptr_t)p); }
+
+// encode (PLAN_ENCODE) or the transform tap (PLAN_WHITEN: codes == nullptr, taps[i] receives FP32 W~).
+gf8_status fast_encode_many(gf8_ctx* c, int n, const int* layers, const void* const* grads, gf8_dtype dt,
+                            uint8_t* const* codes, float* const* sinv, float* const* taps, cudaStream_t st) {
+    using namespace gf8::tc;
+    const bool tap = taps != nullptr;
+    for (int i = 0; i < n; ++i) {
+        GF_TRY(check_layer(c, layers[i]));
+        LayerState& L = c->layers[layers[i]];
+        if (!grads[i] || (!tap && (!codes[i] || !sinv[i])) || (tap && !taps[i])) return fail(c, GF8_ERR_INVALID_ARG, "null pointer");
+        if (!aligned16(grads[i]) || (!tap && !aligned16(codes[i])) || (tap && !aligned16(taps[i])))
+            return fail(c, GF8_ERR_UNSUPPORTED, "pointers must be 16-byte aligned");
+        GF_TRY(check_basis(c, L, layers[i]));
+    }
+    std::vector<uint64_t> key;
+    key.push_back(tap ? PLAN_WHITEN : PLAN_ENCODE);
+    key.push_back((uint64_t)dt);
+    key.push_back((uint64_t)n);
+    for (int i = 0; i < n; ++i) {
+        key.push_back((uint64_t)layers[i]);
+        key_ptr(key, grads[i]);
+        if (tap) key_ptr(key, taps[i]); else { key_ptr(key, codes[i]); key_ptr(key, sinv[i]); }
+    }
+    Plan* p = nullptr;
+    auto found = c->plans.find(key);
+    if (found != c->plans.end()) p = found->second;
+    else {
+        p = new (std::nothrow) Plan();
+        if (!p) return fail(c, GF8_ERR_NOMEM, "host allocation failed");
+        PlanBuilder pb;
+        std::map<int, size_t> occurrence;
+        std::vector<int> tc_idx;
+        for (int i = 0; i < n; ++i) {
+            if (c->layers[layers[i]].tc_ok) tc_idx.push_back(i); else p->plain.push_back(i);
+        }
+        p->n_amax = tc_idx.size();
+        gf8_status s = GF8_OK;
+        if (p->n_amax) {
+            void* q = nullptr;
+            if (cudaMalloc(&q, p->n_amax * sizeof(uint32_t)) != cudaSuccess) { cudaGetLastError(); plan_free(p); return fail(c, GF8_ERR_NOMEM, "plan amax"); }
+            p->d_amax = (uint32_t*)q;
+        }
+        for (size_t t = 0; t < tc_idx.size() && s == GF8_OK; ++t) {
+            const int i = tc_idx[t];
+            LayerState& L = c->layers[layers[i]];
+            const int m = L.desc.d_out, nn = L.desc.d_in;
+            Slot* slot = nullptr;
+            if ((s = fast_slot(c, L, occurrence[layers[i]]++, dt == GF8_DT_F32, false, false, &slot)) != GF8_OK) break;
+            int src_map;
+            if (dt == GF8_DT_BF16) {
+                CUtensorMap mp;
+                if ((s = make_map(c, &mp, grads[i], m, nn, nn)) != GF8_OK) break;
+                src_map = pb.add_map(grads[i], mp);
+            } else {
+                p->converts.push_back({(const float*)grads[i], slot->src16, (int64_t)m * nn});
+                src_map = pb.add_map(slot->src16, slot->map_src16);
+            }
+            Final f;
+            memset(&f, 0, sizeof(f));
+            f.fmt = L.desc.fmt;
+            f.base = grads[i];
+            f.base_type = dt == GF8_DT_BF16 ? TY_BF16 : TY_F32;
+            if (tap) { f.mode = EPI_STORE; f.out = taps[i]; f.out_type = TY_F32; }
+            else {
+                f.mode = L.desc.scaling == GF8_SCALE_TENSOR ? EPI_AMAX : EPI_BLOCKCAST;
+                f.out = codes[i]; f.amax = p->d_amax + t; f.scale_inv = sinv[i];
+            }
+            add_transform(pb, L, slot, src_map, -1, false, false, f);
+        }
+        if (s == GF8_OK) s = plan_finish(c, pb, p);
+        if (s == GF8_OK) s = plan_store(c, key, p);
+        if (s != GF8_OK) { plan_free(p); return s; }
+    }
+    for (const Plan::Convert& cv : p->converts) {
+        convert_kernel<float, bf16><<<grid_for(c, cv.numel, 256, 8), 256, 0, st>>>(cv.src, cv.numel, cv.dst);
+        LAUNCH_CHECK(c);
+    }
+    if (p->n_amax) CU_TRY(c, cudaMemsetAsync(p->d_amax, 0, p->n_amax * sizeof(uint32_t), st));
+    GF_TRY(plan_run_stages(c, st, p));
+    for (int i : p->plain) {
+        if (tap) {
+            LayerState& L = c->layers[layers[i]];
+            if (dt == GF8_DT_BF16) GF_TRY(transform_simt<bf16>(c, st, L, (const bf16*)grads[i], taps[i], false));
+            else GF_TRY(transform_simt<float>(c, st, L, (const float*)grads[i], taps[i], false));
+        } else {
+            GF_TRY(encode_one(c, layers[i], grads[i], dt, codes[i], sinv[i], st));
+        }
+    }
+    return GF8_OK;
+}
+
+gf8_status fast_reduce_decoded_many(gf8_ctx* c, int n, const int* layers, const uint8_t* const* codes,
+                                    const float* const* sinv, int R, int average, void* const* outs, gf8_dtype dt,
+                                    cudaStream_t st) {
+    using namespace gf8::tc;
+    for (int i = 0; i < n; ++i) {
+        GF_TRY(check_layer(c, layers[i]));
+        if (!outs[i] || !aligned16(outs[i])) return fail(c, GF8_ERR_INVALID_ARG, "bad output pointer");
+        for (int r = 0; r < R; ++r) {
+            if (!codes[(size_t)i * R + r] || !sinv[(size_t)i * R + r]) return fail(c, GF8_ERR_INVALID_ARG, "null payload pointer");
+            if (!aligned16(codes[(size_t)i * R + r])) return fail(c, GF8_ERR_UNSUPPORTED, "pointers must be 16-byte aligned");
+        }
+        GF_TRY(check_basis(c, c->layers[layers[i]], layers[i]));
+    }
+    std::vector<uint64_t> key;
+    key.push_back(PLAN_DECODE);
+    key.push_back((uint64_t)dt);
+    key.push_back((uint64_t)n);
+    for (int i = 0; i < n; ++i) { key.push_back((uint64_t)layers[i]); key_ptr(key, outs[i]); }
+    Plan* p = nullptr;
+    auto found = c->plans.find(key);
+    if (found != c->plans.end()) p = found->second;
+    else {
+        p = new (std::nothrow) Plan();
+        if (!p) return fail(c, GF8_ERR_NOMEM, "host allocation failed");
+        PlanBuilder pb;
+        std::map<int, size_t> occurrence;
+        gf8_status s = GF8_OK;
+        for (int i = 0; i < n && s == GF8_OK; ++i) {
+            LayerState& L = c->layers[layers[i]];
+            if (!L.tc_ok) { p->plain.push_back(i); continue; }
+            Slot* slot = nullptr;
+            if ((s = fast_slot(c, L, occurrence[layers[i]]++, true, true, true, &slot)) != GF8_OK) break;
+            p->reduces.push_back({i, slot->Uhat, slot->src16, slot->src16_lo});
+            const int src_map = pb.add_map(slot->src16, slot->map_src16);
+            const int src_lo_map = pb.add_map(slot->src16_lo, slot->map_src16_lo);
+            Final f;
+            memset(&f, 0, sizeof(f));
+            f.mode = EPI_STORE; f.base = slot->Uhat; f.base_type = TY_F32;
+            f.out = outs[i]; f.out_type = dt == GF8_DT_BF16 ? TY_BF16 : TY_F32;
+            // the unwhitening multipliers ebar = 1/D - 1 amplify operand rounding, so decode runs split products
+            add_transform(pb, L, slot, src_map, src_lo_map, true, true, f);
+        }
+        if (s == GF8_OK) s = plan_finish(c, pb, p);
+        if (s == GF8_OK) s = plan_store(c, key, p);
+        if (s != GF8_OK) { plan_free(p); return s; }
+    }
+    for (const Plan::Reduce& rd : p->reduces) {
+        const int i = rd.batch_index;
+        const LayerState& L = c->layers[layers[i]];
+        GF_TRY(reduce_dev<float>(c, st, codes + (size_t)i * R, sinv + (size_t)i * R, R, average, L.desc.d_out, L.desc.d_in,
+                                 L.desc.fmt, L.desc.scaling, rd.uhat, rd.u16, rd.u16_lo));
+    }
+    GF_TRY(plan_run_stages(c, st, p));
+    for (int i : p->plain)
+        GF_TRY(reduce_decoded_one(c, layers[i], codes + (size_t)i * R, sinv + (size_t)i * R, R, average, outs[i], dt, st));
+    return GF8_OK;
+}
+
 }  // namespace
 
 // =====================================================================================================
@@ -377,6 +431,21 @@ const char* gf8_status_string(gf8_status s) {
 
 const char* gf8_last_error(const gf8_ctx* ctx) { return ctx ? ctx->err : "null context"; }
 int64_t gf8_launch_count(const gf8_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+gf8_status gf8_sync_check(gf8_ctx* ctx, void* stream) {
+    if (!ctx) return GF8_ERR_INVALID_ARG;
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    CU_TRY(ctx, cudaStreamSynchronize((cudaStream_t)stream));
+    if (ctx->d_err) {
+        int e = 0;
+        CU_TRY(ctx, cudaMemcpy(&e, ctx->d_err, sizeof(int), cudaMemcpyDeviceToHost));
+        if (e) {
+            cudaMemset(ctx->d_err, 0, sizeof(int));
+            return fail(ctx, GF8_ERR_CUDA, "tensor-core pipeline time-out (error flag %d)", e);
+        }
+    }
+    return GF8_OK;
+}
 
 gf8_status gf8_create(gf8_ctx** out, int device, const gf8_layer_desc* layers, int n_layers, gf8_precision precision) {
     if (!out || !layers || n_layers < 1) return GF8_ERR_INVALID_ARG;
@@ -412,12 +481,15 @@ gf8_status gf8_create(gf8_ctx** out, int device, const gf8_layer_desc* layers, i
         if ((s = dmalloc(c, &L.scale, L.n_scales)) != GF8_OK) break;
         if (L.desc.side != GF8_SIDE_NONE) max_mn = std::max(max_mn, (size_t)m * n);
         auto init_side = [&](SideState& sd, int d, int k) -> gf8_status {
-            sd.used = true; sd.d = d; sd.k = k;
+            sd.used = true; sd.d = d; sd.k = k; sd.kp = pad64(k);
             gf8_status r;
             if ((r = dmalloc(c, &sd.U, (size_t)d * k)) != GF8_OK) return r;
             if ((r = dmalloc(c, &sd.mu, (size_t)k)) != GF8_OK) return r;
-            if ((r = dmalloc(c, &sd.e, (size_t)k)) != GF8_OK) return r;
-            if ((r = dmalloc(c, &sd.ebar, (size_t)k)) != GF8_OK) return r;
+            // multipliers are zero-padded to kp entries (the FAST path's padded rank columns contribute 0)
+            if ((r = dmalloc(c, &sd.e, (size_t)sd.kp)) != GF8_OK) return r;
+            if ((r = dmalloc(c, &sd.ebar, (size_t)sd.kp)) != GF8_OK) return r;
+            if (cudaMemset(sd.e, 0, sizeof(float) * sd.kp) != cudaSuccess || cudaMemset(sd.ebar, 0, sizeof(float) * sd.kp) != cudaSuccess)
+                return GF8_ERR_CUDA;
             if ((r = dmalloc(c, &sd.rho, (size_t)1)) != GF8_OK) return r;
             max_dk = std::max(max_dk, (size_t)d * k);
             max_k = std::max(max_k, (size_t)k);
@@ -433,6 +505,7 @@ gf8_status gf8_create(gf8_ctx** out, int device, const gf8_layer_desc* layers, i
         }
         if (L.desc.side == GF8_SIDE_BOTH)
             if ((s = dmalloc(c, &L.S, (size_t)L.desc.rank_out * L.desc.rank_in)) != GF8_OK) break;
+        if ((s = fast_init_layer(c, L)) != GF8_OK) break;
     }
     if (s == GF8_OK && max_mn) s = dmalloc(c, &c->wt_scratch, max_mn);
     if (s == GF8_OK && max_dk) {
@@ -452,6 +525,9 @@ gf8_status gf8_destroy(gf8_ctx* ctx) {
     cudaDeviceSynchronize();
     for (void* p : ctx->allocs) cudaFree(p);
     for (void* p : ctx->stage_allocs) cudaFree(p);
+    for (Plan* p : ctx->plan_order) plan_free(p);
+    for (LayerState& L : ctx->layers)
+        for (Slot* sl : L.slots) delete sl;
     delete ctx;
     return GF8_OK;
 }
@@ -512,6 +588,10 @@ gf8_status gf8_encode(gf8_ctx* ctx, int layer, const void* grad, gf8_dtype dt, u
                       void* stream) {
     if (!ctx) return GF8_ERR_INVALID_ARG;
     CU_TRY(ctx, cudaSetDevice(ctx->device));
+    if (ctx->precision == GF8_PREC_FAST) {
+        if (dt != GF8_DT_BF16 && dt != GF8_DT_F32) return fail(ctx, GF8_ERR_INVALID_ARG, "bad dtype");
+        return fast_encode_many(ctx, 1, &layer, &grad, dt, &codes, &scale_inv, nullptr, (cudaStream_t)stream);
+    }
     return encode_one(ctx, layer, grad, dt, codes, scale_inv, (cudaStream_t)stream);
 }
 
@@ -521,6 +601,11 @@ gf8_status gf8_decode(gf8_ctx* ctx, int layer, const uint8_t* codes, const float
     CU_TRY(ctx, cudaSetDevice(ctx->device));
     const uint8_t* cp[1] = {codes};
     const float* sp[1] = {scale_inv};
+    if (ctx->precision == GF8_PREC_FAST) {
+        if (!codes || !scale_inv || !grad_out) return fail(ctx, GF8_ERR_INVALID_ARG, "null pointer");
+        if (dt != GF8_DT_BF16 && dt != GF8_DT_F32) return fail(ctx, GF8_ERR_INVALID_ARG, "bad dtype");
+        return fast_reduce_decoded_many(ctx, 1, &layer, cp, sp, 1, 0, &grad_out, dt, (cudaStream_t)stream);
+    }
     return reduce_decoded_one(ctx, layer, cp, sp, 1, 0, grad_out, dt, (cudaStream_t)stream);
 }
 
@@ -528,6 +613,12 @@ gf8_status gf8_reduce_decoded(gf8_ctx* ctx, int layer, const uint8_t* const* cod
                               int R, int average, void* grad_out, gf8_dtype dt, void* stream) {
     if (!ctx) return GF8_ERR_INVALID_ARG;
     CU_TRY(ctx, cudaSetDevice(ctx->device));
+    if (ctx->precision == GF8_PREC_FAST) {
+        if (!codes || !scale_inv || !grad_out) return fail(ctx, GF8_ERR_INVALID_ARG, "null pointer");
+        if (R < 1 || R > GF8_MAX_R) return fail(ctx, GF8_ERR_INVALID_ARG, "R=%d out of range [1,%d]", R, GF8_MAX_R);
+        if (dt != GF8_DT_BF16 && dt != GF8_DT_F32) return fail(ctx, GF8_ERR_INVALID_ARG, "bad dtype");
+        return fast_reduce_decoded_many(ctx, 1, &layer, codes, scale_inv, R, average, &grad_out, dt, (cudaStream_t)stream);
+    }
     return reduce_decoded_one(ctx, layer, codes, scale_inv, R, average, grad_out, dt, (cudaStream_t)stream);
 }
 
@@ -536,6 +627,9 @@ gf8_status gf8_encode_many(gf8_ctx* ctx, int n, const int* layers, const void* c
     if (!ctx) return GF8_ERR_INVALID_ARG;
     if (n < 0 || !layers || !grads || !codes || !scale_inv) return fail(ctx, GF8_ERR_INVALID_ARG, "null argument");
     CU_TRY(ctx, cudaSetDevice(ctx->device));
+    if (dt != GF8_DT_BF16 && dt != GF8_DT_F32) return fail(ctx, GF8_ERR_INVALID_ARG, "bad dtype");
+    if (ctx->precision == GF8_PREC_FAST)
+        return fast_encode_many(ctx, n, layers, grads, dt, codes, scale_inv, nullptr, (cudaStream_t)stream);
     for (int i = 0; i < n; ++i) GF_TRY(encode_one(ctx, layers[i], grads[i], dt, codes[i], scale_inv[i], (cudaStream_t)stream));
     return GF8_OK;
 }
@@ -547,6 +641,9 @@ gf8_status gf8_reduce_decoded_many(gf8_ctx* ctx, int n, const int* layers, const
     if (n < 0 || !layers || !grads_out || !codes || !scale_inv) return fail(ctx, GF8_ERR_INVALID_ARG, "null argument");
     if (R < 1 || R > GF8_MAX_R) return fail(ctx, GF8_ERR_INVALID_ARG, "R=%d out of range [1,%d]", R, GF8_MAX_R);
     CU_TRY(ctx, cudaSetDevice(ctx->device));
+    if (dt != GF8_DT_BF16 && dt != GF8_DT_F32) return fail(ctx, GF8_ERR_INVALID_ARG, "bad dtype");
+    if (ctx->precision == GF8_PREC_FAST)
+        return fast_reduce_decoded_many(ctx, n, layers, codes, scale_inv, R, average, grads_out, dt, (cudaStream_t)stream);
     for (int i = 0; i < n; ++i)
         GF_TRY(reduce_decoded_one(ctx, layers[i], codes + (size_t)i * R, scale_inv + (size_t)i * R, R, average,
                                   grads_out[i], dt, (cudaStream_t)stream));
@@ -616,13 +713,16 @@ gf8_status gf8_step_host(gf8_ctx* ctx, int n, const int* layers, const void* con
                                         cudaMemcpyHostToDevice, st));
         }
     }
-    for (int r = 0; r < R; ++r)
+    {
+        std::vector<int> lay((size_t)n * R);
         for (int i = 0; i < n; ++i)
-            GF_TRY(encode_one(ctx, layers[i], ctx->st_grads[(size_t)i * R + r], dt, ctx->st_codes[(size_t)i * R + r],
-                              ctx->st_sinv[(size_t)i * R + r], st));
+            for (int r = 0; r < R; ++r) lay[(size_t)i * R + r] = layers[i];
+        GF_TRY(gf8_encode_many(ctx, n * R, lay.data(), ctx->st_grads.data(), dt, ctx->st_codes.data(), ctx->st_sinv.data(),
+                               stream));
+        GF_TRY(gf8_reduce_decoded_many(ctx, n, layers, (const uint8_t* const*)ctx->st_codes.data(),
+                                       (const float* const*)ctx->st_sinv.data(), R, average, ctx->st_out.data(), dt, stream));
+    }
     for (int i = 0; i < n; ++i) {
-        GF_TRY(reduce_decoded_one(ctx, layers[i], (const uint8_t* const*)&ctx->st_codes[(size_t)i * R],
-                                  (const float* const*)&ctx->st_sinv[(size_t)i * R], R, average, ctx->st_out[i], dt, st));
         const LayerState& L = ctx->layers[layers[i]];
         if (!out_host[i]) return fail(ctx, GF8_ERR_INVALID_ARG, "null host output");
         CU_TRY(ctx, cudaMemcpyAsync(out_host[i], ctx->st_out[i], (size_t)L.desc.d_out * L.desc.d_in * esz,
@@ -686,6 +786,7 @@ gf8_status gf8_set_basis(gf8_ctx* ctx, int layer, int side, const float* U, cons
         multipliers_kernel<<<1, 256, 0, st>>>(nullptr, s->d, s->k, nullptr, mu, (double)L.desc.damping, (double)rho,
                                               s->mu, s->e, s->ebar, s->rho);
         LAUNCH_CHECK(ctx);
+        GF_TRY(fast_pack_basis(ctx, st, *s));
         s->has_basis = true;
     } else {
         s->has_basis = false;
@@ -702,8 +803,10 @@ gf8_status gf8_whiten_f32(gf8_ctx* ctx, int layer, const void* grad, gf8_dtype d
     GF_TRY(check_basis(ctx, L, layer));
     CU_TRY(ctx, cudaSetDevice(ctx->device));
     cudaStream_t st = (cudaStream_t)stream;
-    if (dt == GF8_DT_BF16) return transform_simt<bf16>(ctx, st, L, (const bf16*)grad, out, false);
     if ((const void*)grad == (const void*)out) return fail(ctx, GF8_ERR_INVALID_ARG, "in-place whiten tap not allowed");
+    if (ctx->precision == GF8_PREC_FAST && L.tc_ok)
+        return fast_encode_many(ctx, 1, &layer, &grad, dt, nullptr, nullptr, &out, st);
+    if (dt == GF8_DT_BF16) return transform_simt<bf16>(ctx, st, L, (const bf16*)grad, out, false);
     return transform_simt<float>(ctx, st, L, (const float*)grad, out, false);
 }
 

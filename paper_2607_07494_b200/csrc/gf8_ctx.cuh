@@ -1,0 +1,150 @@
+// gf8_ctx.cuh -- internal: the context behind the opaque gf8_ctx of include/gf8.h, and small host helpers.
+#pragma once
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <new>
+#include <vector>
+
+#include <cuda.h>
+
+#include "../../include/gf8.h"
+#include "gf8_common.cuh"
+
+namespace {
+
+struct SideState {
+    int d = 0, k = 0;
+    bool used = false;
+    float* factor = nullptr;   // d x d FP32 (lazy)
+    bool has_factor = false;   // at least one update / set
+    float* U = nullptr;        // d x k FP32 row-major
+    float* mu = nullptr;       // k
+    float* e = nullptr;        // k  encode multipliers
+    float* ebar = nullptr;     // k  decode multipliers
+    float* rho = nullptr;      // 1
+    bool has_start = false, has_basis = false;
+    // FAST path (tensor cores): rank padded to a multiple of 64, BF16 copies of the basis, TMA maps
+    int kp = 0;
+    gf8::bf16* U16 = nullptr;  // d x kp   (zero-padded columns)
+    gf8::bf16* Ut16 = nullptr; // kp x d
+    gf8::bf16 *U16_lo = nullptr, *Ut16_lo = nullptr;   // BF16 residuals U - bf16(U) (split-operand products)
+    CUtensorMap map_U16, map_Ut16, map_U16_lo, map_Ut16_lo;
+};
+
+// Per (layer, occurrence-in-batch) scratch of the FAST path; buffers and their TMA maps are static.
+struct Slot {
+    gf8::bf16* Pp = nullptr;   // m x kpA   P' = (src U_A) E_A
+    float* Qt = nullptr;       // n x kpG   Q^T
+    gf8::bf16* Qpt = nullptr;  // n x kpG   Q'^T
+    gf8::bf16* SEA = nullptr;  // kpG x kpA S E_A
+    gf8::bf16 *Pp_lo = nullptr, *Qpt_lo = nullptr, *SEA_lo = nullptr;   // residuals, lazy (split products)
+    CUtensorMap map_Pp, map_Qpt, map_SEA, map_Pp_lo, map_Qpt_lo, map_SEA_lo;
+    float* Uhat = nullptr;     // m x n FP32 reduced payload (decode), lazy
+    gf8::bf16* src16 = nullptr;// m x n BF16 copy of an FP32 source (decode, FP32 gradients), lazy
+    gf8::bf16* src16_lo = nullptr;
+    CUtensorMap map_src16, map_src16_lo;
+};
+
+struct LayerState {
+    gf8_layer_desc desc;
+    SideState in, out;         // in: A / U_A (d_in), out: Gf / U_G (d_out)
+    size_t n_scales = 1;
+    uint32_t* amax_bits = nullptr;   // n_scales
+    float* scale = nullptr;          // n_scales
+    float* P = nullptr;              // m x kA
+    float* Q = nullptr;              // kG x n
+    float* S = nullptr;              // kG x kA
+    bool tc_ok = false;              // FAST path eligible (tensor-core engine)
+    std::vector<Slot*> slots;
+};
+
+}  // namespace
+
+struct gf8_ctx {
+    int device = 0;
+    gf8_precision precision = GF8_PREC_EXACT;
+    std::vector<LayerState> layers;
+    std::vector<void*> allocs;
+    float* wt_scratch = nullptr;     // max m*n FP32
+    // refresh scratch (FP64)
+    double *V = nullptr, *Y = nullptr, *Gm = nullptr, *Bm = nullptr, *Zm = nullptr, *Zs = nullptr, *mu64 = nullptr;
+    // tap scratch (gf8_quantize_f32 with arbitrary shapes)
+    uint32_t* tap_amax = nullptr; float* tap_scale = nullptr; size_t tap_cap = 0;
+    // host-step staging
+    std::vector<void*> stage_allocs;
+    std::vector<void*> st_grads; std::vector<uint8_t*> st_codes; std::vector<float*> st_sinv; std::vector<void*> st_out;
+    std::vector<int> st_layers; int st_R = 0; int st_dt = -1;
+    // FAST path: cached launch plans (device item lists + tensor maps), error flag, driver entry point
+    std::map<std::vector<uint64_t>, struct Plan*> plans;
+    std::vector<struct Plan*> plan_order;
+    int* d_err = nullptr;
+    void* encode_tiled = nullptr;    // cuTensorMapEncodeTiled, resolved at run time (no link-time libcuda)
+    bool tc_attr_set = false;
+    int64_t launches = 0;
+    int num_sms = 148;
+    char err[512] = {0};
+};
+
+namespace {
+
+gf8_status fail(gf8_ctx* c, gf8_status s, const char* fmt, ...) {
+    if (c) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(c->err, sizeof(c->err), fmt, ap);
+        va_end(ap);
+    }
+    return s;
+}
+
+#define CU_TRY(ctx, expr)                                                                            \
+    do {                                                                                             \
+        cudaError_t _e = (expr);                                                                     \
+        if (_e != cudaSuccess)                                                                       \
+            return fail((ctx), GF8_ERR_CUDA, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e), \
+                        __FILE__, __LINE__);                                                         \
+    } while (0)
+
+#define GF_TRY(expr)                       \
+    do {                                   \
+        gf8_status _s = (expr);            \
+        if (_s != GF8_OK) return _s;       \
+    } while (0)
+
+#define LAUNCH_CHECK(ctx)                  \
+    do {                                   \
+        (ctx)->launches++;                 \
+        CU_TRY((ctx), cudaGetLastError()); \
+    } while (0)
+
+inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+template <typename T>
+gf8_status dmalloc(gf8_ctx* c, T** p, size_t count, std::vector<void*>* track = nullptr) {
+    void* q = nullptr;
+    cudaError_t e = cudaMalloc(&q, count * sizeof(T) + 16);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(c, GF8_ERR_NOMEM, "cudaMalloc of %zu bytes failed: %s", count * sizeof(T), cudaGetErrorString(e));
+    }
+    (track ? *track : c->allocs).push_back(q);
+    *p = static_cast<T*>(q);
+    return GF8_OK;
+}
+
+inline size_t n_scales_of(int scaling, int64_t m, int64_t n) {
+    return scaling == GF8_SCALE_TENSOR ? 1 : (size_t)((m + 127) / 128) * (size_t)((n + 127) / 128);
+}
+inline float fmax_of(int fmt) { return fmt == GF8_E4M3 ? 448.0f : 57344.0f; }
+
+inline int grid_for(gf8_ctx* c, int64_t work_items, int threads, int per_sm) {
+    int64_t blocks = (work_items + threads - 1) / threads;
+    const int64_t cap = (int64_t)c->num_sms * per_sm;
+    if (blocks > cap) blocks = cap;
+    if (blocks < 1) blocks = 1;
+    return (int)blocks;
+}
+
+}  // namespace

@@ -1,0 +1,367 @@
+// gf8_fast.cuh -- host side of the FAST (tensor-core) path: TMA maps, per-slot scratch, cached launch
+// plans, and the stage sequence that turns encode / reduce_decoded / whiten into lists of tc::Item.
+// Included by gf8_api.cu after gf8_ctx.cuh.  Arithmetic lives in gf8_tc.cuh; nothing here computes.
+#pragma once
+#include <algorithm>
+
+#include "gf8_ctx.cuh"
+#include "gf8_tc.cuh"
+
+// A cached launch plan: everything a batched call needs on the device, built on first use of a given
+// argument list (steady-state training calls repeat the same pointers every step).
+struct Plan {
+    CUtensorMap* d_maps = nullptr;
+    gf8::tc::Item* d_items = nullptr;
+    int stage_off[6] = {0, 0, 0, 0, 0, 0}, stage_cnt[6] = {0, 0, 0, 0, 0, 0};
+    uint32_t* d_amax = nullptr;          // one word per TC problem (per-tensor scaling)
+    size_t n_amax = 0;
+    struct Convert { const float* src; gf8::bf16* dst; int64_t numel; };
+    std::vector<Convert> converts;       // FP32 gradient -> BF16 MMA operand copies
+    std::vector<int> plain;              // batch indices served by the per-problem (non-TC) path
+    struct Reduce { int batch_index; float* uhat; gf8::bf16 *u16, *u16_lo; };
+    std::vector<Reduce> reduces;         // decode: payload reduction into the slot before the stages
+};
+
+namespace {
+
+using gf8::bf16;
+using gf8::tc::Item;
+
+constexpr int FAST_MAX_KP = 256;
+constexpr size_t FAST_MAX_PLANS = 64;
+
+inline int pad64(int k) { return (k + 63) / 64 * 64; }
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+gf8_status fast_init(gf8_ctx* c) {
+    if (c->encode_tiled) return GF8_OK;
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    CU_TRY(c, cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q));
+    if (!fn || q != cudaDriverEntryPointSuccess) return fail(c, GF8_ERR_CUDA, "cuTensorMapEncodeTiled not available");
+    c->encode_tiled = fn;
+    GF_TRY(dmalloc(c, &c->d_err, 1));
+    CU_TRY(c, cudaMemset(c->d_err, 0, sizeof(int)));
+    CU_TRY(c, cudaFuncSetAttribute(gf8::tc::tc_items_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   gf8::tc::SMEM_BYTES));
+    return GF8_OK;
+}
+
+// BF16 row-major matrix [rows][cols] (leading dimension ld elements) -> TMA map, 64 x 64 boxes, 128 B swizzle,
+// out-of-bounds elements read as zero.
+gf8_status make_map(gf8_ctx* c, CUtensorMap* out, const void* ptr, uint64_t rows, uint64_t cols, uint64_t ld) {
+    const cuuint64_t gdim[2] = {cols, rows};
+    const cuuint64_t gstride[1] = {ld * 2};
+    const cuuint32_t box[2] = {64, 64};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = ((EncodeTiledFn)c->encode_tiled)(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), gdim,
+                                                        gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                                        CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(c, GF8_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d) for %llu x %llu", (int)r,
+                                       (unsigned long long)rows, (unsigned long long)cols);
+    return GF8_OK;
+}
+
+// U (d x k FP32) -> U16 (d x kp BF16, zero-padded) and its transpose Ut16 (kp x d).
+__global__ void pack_basis_kernel(const float* __restrict__ U, int d, int k, int kp, bf16* __restrict__ U16,
+                                  bf16* __restrict__ Ut16, bf16* __restrict__ U16_lo, bf16* __restrict__ Ut16_lo) {
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < (int64_t)d * kp;
+         idx += (int64_t)gridDim.x * blockDim.x) {
+        const int i = (int)(idx / kp), col = (int)(idx % kp);
+        const float x = col < k ? U[(int64_t)i * k + col] : 0.0f;
+        const bf16 v = __float2bfloat16_rn(x);
+        const bf16 lo = __float2bfloat16_rn(x - __bfloat162float(v));
+        U16[idx] = v;
+        Ut16[(int64_t)col * d + i] = v;
+        U16_lo[idx] = lo;
+        Ut16_lo[(int64_t)col * d + i] = lo;
+    }
+}
+
+gf8_status fast_pack_basis(gf8_ctx* c, cudaStream_t st, SideState& s) {
+    if (!s.U16) return GF8_OK;
+    pack_basis_kernel<<<grid_for(c, (int64_t)s.d * s.kp, 256, 4), 256, 0, st>>>(s.U, s.d, s.k, s.kp, s.U16, s.Ut16,
+                                                                                s.U16_lo, s.Ut16_lo);
+    LAUNCH_CHECK(c);
+    return GF8_OK;
+}
+
+// Called from gf8_create for every layer: decides eligibility and allocates the BF16 basis copies.
+gf8_status fast_init_layer(gf8_ctx* c, LayerState& L) {
+    L.tc_ok = false;
+    if (c->precision != GF8_PREC_FAST || L.desc.side == GF8_SIDE_NONE) return GF8_OK;
+    if (L.desc.d_out < 64 || L.desc.d_in < 64) return GF8_OK;
+    if ((L.in.used && pad64(L.in.k) > FAST_MAX_KP) || (L.out.used && pad64(L.out.k) > FAST_MAX_KP)) return GF8_OK;
+    GF_TRY(fast_init(c));
+    for (SideState* s : {&L.in, &L.out}) {
+        if (!s->used) continue;
+        GF_TRY(dmalloc(c, &s->U16, (size_t)s->d * s->kp));
+        GF_TRY(dmalloc(c, &s->Ut16, (size_t)s->kp * s->d));
+        GF_TRY(make_map(c, &s->map_U16, s->U16, s->d, s->kp, s->kp));
+        GF_TRY(make_map(c, &s->map_Ut16, s->Ut16, s->kp, s->d, s->d));
+        GF_TRY(dmalloc(c, &s->U16_lo, (size_t)s->d * s->kp));
+        GF_TRY(dmalloc(c, &s->Ut16_lo, (size_t)s->kp * s->d));
+        GF_TRY(make_map(c, &s->map_U16_lo, s->U16_lo, s->d, s->kp, s->kp));
+        GF_TRY(make_map(c, &s->map_Ut16_lo, s->Ut16_lo, s->kp, s->d, s->d));
+    }
+    L.tc_ok = true;
+    return GF8_OK;
+}
+
+gf8_status fast_slot(gf8_ctx* c, LayerState& L, size_t idx, bool need_src16, bool need_uhat, bool need_split,
+                     Slot** out) {
+    while (L.slots.size() <= idx) L.slots.push_back(nullptr);
+    const size_t m = L.desc.d_out, n = L.desc.d_in;
+    const size_t kpA = L.in.used ? L.in.kp : 0, kpG = L.out.used ? L.out.kp : 0;
+    if (!L.slots[idx]) {
+        Slot* s = new (std::nothrow) Slot();
+        if (!s) return fail(c, GF8_ERR_NOMEM, "host allocation failed");
+        L.slots[idx] = s;
+        if (kpA) {
+            GF_TRY(dmalloc(c, &s->Pp, m * kpA));
+            GF_TRY(make_map(c, &s->map_Pp, s->Pp, m, kpA, kpA));
+        }
+        if (kpG) {
+            GF_TRY(dmalloc(c, &s->Qt, n * kpG));
+            GF_TRY(dmalloc(c, &s->Qpt, n * kpG));
+            GF_TRY(make_map(c, &s->map_Qpt, s->Qpt, n, kpG, kpG));
+        }
+        if (kpA && kpG) {
+            GF_TRY(dmalloc(c, &s->SEA, kpG * kpA));
+            GF_TRY(make_map(c, &s->map_SEA, s->SEA, kpG, kpA, kpA));
+        }
+    }
+    Slot* s = L.slots[idx];
+    if (need_src16 && !s->src16) {
+        GF_TRY(dmalloc(c, &s->src16, m * n));
+        GF_TRY(make_map(c, &s->map_src16, s->src16, m, n, n));
+    }
+    if (need_uhat && !s->Uhat) GF_TRY(dmalloc(c, &s->Uhat, m * n));
+    if (need_split && !s->src16_lo) {
+        GF_TRY(dmalloc(c, &s->src16_lo, m * n));
+        GF_TRY(make_map(c, &s->map_src16_lo, s->src16_lo, m, n, n));
+        if (kpA) {
+            GF_TRY(dmalloc(c, &s->Pp_lo, m * kpA));
+            GF_TRY(make_map(c, &s->map_Pp_lo, s->Pp_lo, m, kpA, kpA));
+        }
+        if (kpG) {
+            GF_TRY(dmalloc(c, &s->Qpt_lo, n * kpG));
+            GF_TRY(make_map(c, &s->map_Qpt_lo, s->Qpt_lo, n, kpG, kpG));
+        }
+        if (kpA && kpG) {
+            GF_TRY(dmalloc(c, &s->SEA_lo, kpG * kpA));
+            GF_TRY(make_map(c, &s->map_SEA_lo, s->SEA_lo, kpG, kpA, kpA));
+        }
+    }
+    *out = s;
+    return GF8_OK;
+}
+
+
+// ---- plan builder ------------------------------------------------------------------------------------
+struct PlanBuilder {
+    std::vector<CUtensorMap> maps;
+    std::map<const void*, int> map_index;      // buffer -> index (static maps are shared by all problems)
+    std::vector<Item> stage[6];
+    int add_map(const void* key, const CUtensorMap& m) {
+        auto it = map_index.find(key);
+        if (it != map_index.end()) return it->second;
+        maps.push_back(m);
+        map_index[key] = (int)maps.size() - 1;
+        return (int)maps.size() - 1;
+    }
+};
+
+struct Final {                  // what the last stage of a transform does with W~ (or Wg^)
+    int mode;                   // EPI_AMAX (+ EPI_CAST), EPI_BLOCKCAST or EPI_STORE
+    int fmt;
+    const void* base; int base_type;
+    void* out; int out_type;
+    uint32_t* amax; float* scale_inv;
+};
+
+inline Item blank_item() {
+    Item it;
+    memset(&it, 0, sizeof(it));
+    return it;
+}
+
+// Stages of out = T_G src T_A (inverse: T^-1) in the low-rank form; src_map indexes the BF16 source.
+// split: every BF16 operand x is carried as hi + lo (x_hi = bf16(x), x_lo = bf16(x - x_hi)) and each product
+// expands to hi*hi + lo*hi + hi*lo, which brings the tensor-core result to ~FP32 accuracy at 3x the MMAs.
+// src_lo_map < 0 means the source is exactly BF16 (a BF16 gradient) and needs no residual.
+void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src_lo_map, bool inverse, bool split,
+                   const Final& f) {
+    using namespace gf8::tc;
+    const int m = L.desc.d_out, n = L.desc.d_in;
+    const bool useA = L.in.used, useG = L.out.used;
+    const int kpA = useA ? L.in.kp : 0, kpG = useG ? L.out.kp : 0;
+    const float* eA = inverse ? L.in.ebar : L.in.e;
+    const float* eG = inverse ? L.out.ebar : L.out.e;
+    struct MapPair { int hi, lo; };
+    auto pair = [&](bool use, const void* bh, const CUtensorMap& mh, const void* bl, const CUtensorMap& ml) {
+        MapPair r{-1, -1};
+        if (use) { r.hi = pb.add_map(bh, mh); if (split) r.lo = pb.add_map(bl, ml); }
+        return r;
+    };
+    const MapPair mUA = pair(useA, L.in.U16, L.in.map_U16, L.in.U16_lo, L.in.map_U16_lo);
+    const MapPair mUAt = pair(useA, L.in.Ut16, L.in.map_Ut16, L.in.Ut16_lo, L.in.map_Ut16_lo);
+    const MapPair mUG = pair(useG, L.out.U16, L.out.map_U16, L.out.U16_lo, L.out.map_U16_lo);
+    const MapPair mUGt = pair(useG, L.out.Ut16, L.out.map_Ut16, L.out.Ut16_lo, L.out.map_Ut16_lo);
+    const MapPair mPp = pair(useA, s->Pp, s->map_Pp, s->Pp_lo, s->map_Pp_lo);
+    const MapPair mQpt = pair(useG, s->Qpt, s->map_Qpt, s->Qpt_lo, s->map_Qpt_lo);
+    const MapPair mSEA = pair(useA && useG, s->SEA, s->map_SEA, s->SEA_lo, s->map_SEA_lo);
+    const MapPair mSrc{src_map, src_lo_map};
+    // append the product A * B^T (hi*hi [+ lo*hi + hi*lo]) to an item
+    auto add_product = [&](Item& it, int& seg, MapPair a, MapPair b, int atoms, int a_c0, int a_r0, int b_c0, int b_r0) {
+        auto one = [&](int ma, int mb) {
+            it.map_a[seg] = ma; it.map_b[seg] = mb; it.atoms[seg] = atoms;
+            it.a_c0[seg] = a_c0; it.a_r0[seg] = a_r0; it.b_c0[seg] = b_c0; it.b_r0[seg] = b_r0;
+            ++seg;
+        };
+        one(a.hi, b.hi);
+        if (a.lo >= 0) one(a.lo, b.hi);
+        if (b.lo >= 0) one(a.hi, b.lo);
+    };
+    if (useA)      // P' = (src U_A) E_A : row panels
+        for (int i0 = 0; i0 < m; i0 += 128) {
+            Item it = blank_item();
+            int seg = 0;
+            add_product(it, seg, mSrc, mUAt, (n + 63) / 64, 0, i0, 0, 0);
+            it.N = kpA;
+            it.mode = EPI_STORE; it.out = s->Pp; it.out_lo = split ? s->Pp_lo : nullptr; it.out_ld = kpA;
+            it.out_type = TY_BF16; it.colscale = eA;
+            it.row0 = i0; it.rows = std::min(128, m - i0); it.cols = kpA;
+            pb.stage[0].push_back(it);
+        }
+    if (useG) {    // Q^T = src^T U_G : column panels (A is MN-major)
+        for (int j0 = 0; j0 < n; j0 += 128) {
+            Item it = blank_item();
+            int seg = 0;
+            add_product(it, seg, mSrc, mUGt, (m + 63) / 64, j0, 0, 0, 0);
+            it.a_mn = 1; it.N = kpG;
+            it.mode = EPI_STORE; it.row0 = j0; it.rows = std::min(128, n - j0); it.cols = kpG;
+            if (useA) { it.out = s->Qt; it.out_ld = kpG; it.out_type = TY_F32; }
+            else {
+                it.out = s->Qpt; it.out_lo = split ? s->Qpt_lo : nullptr; it.out_ld = kpG; it.out_type = TY_BF16;
+                it.colscale = eG;
+            }
+            pb.stage[1].push_back(it);
+        }
+        if (useA) {
+            // (S E_A)^T = P'^T U_G, stored transposed as SEA[g][a]
+            for (int a0 = 0; a0 < kpA; a0 += 128) {
+                Item it = blank_item();
+                int seg = 0;
+                add_product(it, seg, mPp, mUGt, (m + 63) / 64, a0, 0, 0, 0);
+                it.a_mn = 1; it.N = kpG;
+                it.mode = EPI_STORE_T; it.out = s->SEA; it.out_lo = split ? s->SEA_lo : nullptr; it.out_ld = kpA;
+                it.out_type = TY_BF16;
+                it.row0 = a0; it.rows = std::min(128, kpA - a0); it.cols = kpG;
+                pb.stage[1].push_back(it);
+            }
+            // Q'^T = (Q^T + U_A (S E_A)^T) E_G
+            for (int j0 = 0; j0 < n; j0 += 128) {
+                Item it = blank_item();
+                int seg = 0;
+                add_product(it, seg, mUA, mSEA, kpA / 64, 0, j0, 0, 0);
+                it.N = kpG;
+                it.mode = EPI_STORE; it.base = s->Qt; it.base_ld = kpG; it.base_type = TY_F32;
+                it.out = s->Qpt; it.out_lo = split ? s->Qpt_lo : nullptr; it.out_ld = kpG; it.out_type = TY_BF16;
+                it.colscale = eG;
+                it.row0 = j0; it.rows = std::min(128, n - j0); it.cols = kpG;
+                pb.stage[2].push_back(it);
+            }
+        }
+    }
+    // rank-(kA + kG) update of the streamed base tile
+    const int tiles_n = (n + 127) / 128;
+    for (int i0 = 0; i0 < m; i0 += 128)
+        for (int j0 = 0; j0 < n; j0 += 128) {
+            Item it = blank_item();
+            int seg = 0;
+            if (useA) add_product(it, seg, mPp, mUA, kpA / 64, 0, i0, 0, j0);
+            if (useG) add_product(it, seg, mUG, mQpt, kpG / 64, 0, i0, 0, j0);
+            it.N = 128; it.fmt = f.fmt;
+            it.base = f.base; it.base_ld = n; it.base_type = f.base_type;
+            it.row0 = i0; it.col0 = j0; it.rows = std::min(128, m - i0); it.cols = std::min(128, n - j0);
+            it.mode = f.mode;
+            if (f.mode == EPI_AMAX) {
+                it.amax = f.amax;
+                pb.stage[3].push_back(it);
+                it.mode = EPI_CAST; it.out = f.out; it.out_ld = n; it.scale_inv_out = f.scale_inv;
+                it.write_scale = (i0 == 0 && j0 == 0) ? 1 : 0;
+                pb.stage[4].push_back(it);
+            } else if (f.mode == EPI_BLOCKCAST) {
+                it.out = f.out; it.out_ld = n;
+                it.scale_inv_out = f.scale_inv + (size_t)(i0 / 128) * tiles_n + j0 / 128;
+                pb.stage[3].push_back(it);
+            } else {
+                it.out = f.out; it.out_ld = n; it.out_type = f.out_type;
+                pb.stage[3].push_back(it);
+            }
+        }
+}
+
+void plan_free(Plan* p) {
+    if (!p) return;
+    cudaFree(p->d_maps);
+    cudaFree(p->d_items);
+    cudaFree(p->d_amax);
+    delete p;
+}
+
+// Upload the builder's maps and items (longest contractions first within a stage: CTAs take items round-robin).
+gf8_status plan_finish(gf8_ctx* c, PlanBuilder& pb, Plan* p) {
+    std::vector<Item> all;
+    for (int s = 0; s < 6; ++s) {
+        std::stable_sort(pb.stage[s].begin(), pb.stage[s].end(), [](const Item& a, const Item& b) {
+            int ta = 0, tb = 0;
+            for (int g = 0; g < gf8::tc::NSEG; ++g) { ta += a.atoms[g]; tb += b.atoms[g]; }
+            return ta > tb;
+        });
+        p->stage_off[s] = (int)all.size();
+        p->stage_cnt[s] = (int)pb.stage[s].size();
+        all.insert(all.end(), pb.stage[s].begin(), pb.stage[s].end());
+    }
+    if (all.empty()) return GF8_OK;
+    void* q = nullptr;
+    if (cudaMalloc(&q, pb.maps.size() * sizeof(CUtensorMap)) != cudaSuccess) { cudaGetLastError(); return fail(c, GF8_ERR_NOMEM, "plan maps"); }
+    p->d_maps = (CUtensorMap*)q;
+    if (cudaMalloc(&q, all.size() * sizeof(Item)) != cudaSuccess) { cudaGetLastError(); return fail(c, GF8_ERR_NOMEM, "plan items"); }
+    p->d_items = (Item*)q;
+    CU_TRY(c, cudaMemcpy(p->d_maps, pb.maps.data(), pb.maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice));
+    CU_TRY(c, cudaMemcpy(p->d_items, all.data(), all.size() * sizeof(Item), cudaMemcpyHostToDevice));
+    return GF8_OK;
+}
+
+gf8_status plan_store(gf8_ctx* c, const std::vector<uint64_t>& key, Plan* p) {
+    if (c->plan_order.size() >= FAST_MAX_PLANS) {
+        CU_TRY(c, cudaDeviceSynchronize());
+        Plan* old = c->plan_order.front();
+        c->plan_order.erase(c->plan_order.begin());
+        for (auto it = c->plans.begin(); it != c->plans.end(); ++it)
+            if (it->second == old) { c->plans.erase(it); break; }
+        plan_free(old);
+    }
+    c->plans[key] = p;
+    c->plan_order.push_back(p);
+    return GF8_OK;
+}
+
+gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, const Plan* p) {
+    for (int s = 0; s < 6; ++s) {
+        if (!p->stage_cnt[s]) continue;
+        const int grid = std::min(p->stage_cnt[s], c->num_sms);
+        gf8::tc::tc_items_kernel<<<grid, gf8::tc::THREADS, gf8::tc::SMEM_BYTES, st>>>(p->d_items + p->stage_off[s],
+                                                                                  p->stage_cnt[s], p->d_maps, c->d_err);
+        LAUNCH_CHECK(c);
+    }
+    return GF8_OK;
+}
+
+}  // namespace

@@ -141,7 +141,8 @@ struct ReducePtrs {
 // OutT = float (scratch / FP32 output) or bf16 (Euclidean tensors decoded straight to BF16).
 template <int FMT, typename OutT>
 __global__ void __launch_bounds__(256) reduce_kernel(const __grid_constant__ ReducePtrs p, int R, int average,
-                                                     int64_t m, int64_t n, int scaling, OutT* __restrict__ out) {
+                                                     int64_t m, int64_t n, int scaling, OutT* __restrict__ out,
+                                                     bf16* __restrict__ out16 = nullptr, bf16* __restrict__ out16_lo = nullptr) {
     const int64_t ngroups = m * n / 16;
     const int64_t bn = (n + 127) / 128;
     const float invR = __fdiv_rn(1.0f, (float)R);
@@ -171,6 +172,28 @@ __global__ void __launch_bounds__(256) reduce_kernel(const __grid_constant__ Red
             for (int u = 0; u < 4; ++u)
                 st_stream(o + u, make_uint4(__float_as_uint(acc[4 * u]), __float_as_uint(acc[4 * u + 1]),
                                             __float_as_uint(acc[4 * u + 2]), __float_as_uint(acc[4 * u + 3])));
+            if (out16) {      // BF16 copy: the tensor-core operand of the unwhitening projections (FAST path)
+                uint32_t w[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    const __nv_bfloat162 h = __floats2bfloat162_rn(acc[2 * u], acc[2 * u + 1]);
+                    w[u] = *reinterpret_cast<const uint32_t*>(&h);
+                }
+                uint4* o2 = reinterpret_cast<uint4*>(out16 + e0);
+                o2[0] = make_uint4(w[0], w[1], w[2], w[3]);
+                o2[1] = make_uint4(w[4], w[5], w[6], w[7]);
+                if (out16_lo) {   // residual acc - bf16(acc): hi + lo carries ~16 mantissa bits into the MMAs
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) {
+                        const float2 hi = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&w[u]));
+                        const __nv_bfloat162 h = __floats2bfloat162_rn(acc[2 * u] - hi.x, acc[2 * u + 1] - hi.y);
+                        w[u] = *reinterpret_cast<const uint32_t*>(&h);
+                    }
+                    uint4* o3 = reinterpret_cast<uint4*>(out16_lo + e0);
+                    o3[0] = make_uint4(w[0], w[1], w[2], w[3]);
+                    o3[1] = make_uint4(w[4], w[5], w[6], w[7]);
+                }
+            }
         } else {
             uint32_t w[8];
 #pragma unroll

@@ -1,0 +1,399 @@
+// gf8_tc.cuh -- the tensor-core engine of the FAST path (sm_100a): one persistent, warp-specialised
+// kernel that runs a list of "items", each a 128 x N BF16 contraction with FP32 accumulation in TMEM
+//
+//     acc[128][N] = sum over K-atoms t of  A_t[128][64] * B_t[N][64]^T          (tcgen05.mma, kind::f16)
+//
+// followed by a fused epilogue (add the streamed base tile, column multipliers, amax, FP8 cast ...).
+// Every dense contraction of the codec is an instance (PAPER.md:158 Eq. 14, :250 Eq. 22, :172 Eq. 17 in the
+// low-rank form of DESIGN.md "Transform"):
+//     P' = (Wg U_A) E_A        A = Wg   (K-major),  B = U_A^T        -> BF16 panel
+//     Q^T = Wg^T U_G           A = Wg   (MN-major), B = U_G^T        -> FP32 / BF16 panel
+//     (S E_A)^T = P'^T U_G     A = P'   (MN-major), B = U_G^T        -> BF16, stored transposed
+//     Q'^T = (Q^T + U_A (S E_A)^T) E_G                               -> BF16 panel
+//     W~ = Wg + [P' | U_G] [U_A | Q'^T]^T   (rank-2k update)         -> amax / FP8 codes / BF16 / FP32
+// Operands are staged by TMA (cp.async.bulk.tensor, 64 x 64 BF16 boxes, 128-byte swizzle) through a
+// 4-stage mbarrier ring; one elected thread issues the MMAs; accumulators are double-buffered in TMEM
+// so the epilogue of item i overlaps the MMAs of item i+1.  Warps 0-3: epilogue (TMEM lane quarter =
+// warp index), warp 4: TMA producer, warp 5: TMEM allocation + MMA issue.
+#pragma once
+#include <cuda.h>
+
+#include "gf8_common.cuh"
+#include "gf8_quant.cuh"
+
+namespace gf8 {
+namespace tc {
+
+constexpr int STAGES = 4;
+constexpr int A_BYTES = 128 * 64 * 2;            // one K-atom of A: 128 x 64 BF16
+constexpr int B_BYTES = 256 * 64 * 2;            // one K-atom of B: up to 256 x 64 BF16
+constexpr int STAGE_BYTES = A_BYTES + B_BYTES;   // 48 KB
+constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 256 /*barriers*/;
+constexpr int THREADS = 192;
+constexpr int TMEM_COLS = 512;                   // two accumulators of up to 256 columns
+constexpr int NSEG = 6;                          // operand segments per item (hi/lo split products)
+
+enum Epi : int32_t {
+    EPI_STORE = 0,       // out = (base + acc) * colscale           (BF16 or FP32)
+    EPI_STORE_T = 1,     // out[c][r] = acc * colscale  (BF16, transposed store; the small S matrix)
+    EPI_AMAX = 2,        // atomicMax(amax, max |base + acc|)        (a5, per-tensor scale)
+    EPI_CAST = 3,        // codes = fp8((base + acc) * scale(amax))  (a6)
+    EPI_BLOCKCAST = 4    // per-128x128-block amax + scale + cast in one pass (a5 + a6)
+};
+enum Ty : int32_t { TY_NONE = 0, TY_BF16 = 1, TY_F32 = 2 };
+
+struct __align__(16) Item {
+    int32_t map_a[NSEG], map_b[NSEG];   // tensor-map indices (into the plan's CUtensorMap array) per segment
+    int32_t atoms[NSEG];                // K-atoms (64 wide) per segment; 0 = unused
+    int32_t a_c0[NSEG], a_r0[NSEG];     // first box of A: (col, row) in its matrix
+    int32_t b_c0[NSEG], b_r0[NSEG];     // first box of B
+    int32_t a_mn;                 // 1: A is MN-major (the 128 "M" elements are contiguous in memory)
+    int32_t N;                    // accumulator columns: multiple of 64, <= 256
+    int32_t mode, fmt;
+    int32_t row0, col0, rows, cols;   // output tile origin and valid extent (rows <= 128, cols <= N)
+    int32_t base_type, out_type;
+    int32_t write_scale, pad0;
+    int64_t base_ld, out_ld;
+    const void* base;
+    void* out;
+    void* out_lo;                 // EPI_STORE / EPI_STORE_T with BF16 output: optional residual v - bf16(v) (split operands)
+    const float* colscale;        // indexed by tile column c (already offset), or null
+    uint32_t* amax;               // EPI_AMAX: target; EPI_CAST: source
+    float* scale_inv_out;         // EPI_CAST (write_scale) / EPI_BLOCKCAST: where scale_inv goes
+};
+
+// ---- PTX wrappers ------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}" ::"r"(bar), "r"(bytes)
+                 : "memory");
+}
+// Bounded spin: a broken pipeline sets *err and lets the kernel drain instead of hanging the GPU.
+__device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity, int* err) {
+    uint32_t done = 0;
+    for (uint32_t spin = 0; spin < (1u << 26); ++spin) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+        if (done) return true;
+        if ((spin & 0xFFFF) == 0xFFFF && *(volatile int*)err) return false;
+    }
+    atomicExch(err, 1);
+    return false;
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c, int r, uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+        ::"r"(dst), "l"(map), "r"(bar), "r"(c), "r"(r) : "memory");
+}
+__device__ __forceinline__ void tmap_acquire(const CUtensorMap* map) {
+    asm volatile("fence.proxy.tensormap::generic.acquire.gpu [%0], 128;" ::"l"(map) : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tc_mma_bf16(uint32_t tmem_d, uint64_t desc_a, uint64_t desc_b, uint32_t idesc,
+                                            uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+        ::"r"(tmem_d), "l"(desc_a), "l"(desc_b), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t* v) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+        : "r"(taddr) : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+// Shared-memory matrix descriptor (SWIZZLE_128B, version 1).  lbo / sbo in bytes.
+__device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo, uint32_t sbo) {
+    return (uint64_t)((addr >> 4) & 0x3FFFu) | ((uint64_t)((lbo >> 4) & 0x3FFFu) << 16) |
+           ((uint64_t)((sbo >> 4) & 0x3FFFu) << 32) | (1ull << 46) | (2ull << 61);
+}
+// Instruction descriptor: D = F32, A = B = BF16, M = 128, N, A major-ness; B always K-major.
+__device__ __forceinline__ uint32_t instr_desc(int N, int a_mn) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)a_mn << 15) | ((uint32_t)(N >> 3) << 17) | ((128u >> 4) << 24);
+}
+
+// ---- epilogue helpers ---------------------------------------------------------------------------------
+// 16 consecutive elements of the base tile row as floats (zero when there is no base).
+__device__ __forceinline__ void load_base16(const Item& it, int64_t off, float* b) {
+    if (it.base_type == TY_BF16) {
+        const uint4* p = reinterpret_cast<const uint4*>(reinterpret_cast<const bf16*>(it.base) + off);
+        const uint4 x = __ldg(p), y = __ldg(p + 1);
+        unpack_bf16x8(x, b);
+        unpack_bf16x8(y, b + 8);
+    } else if (it.base_type == TY_F32) {
+        const float4* p = reinterpret_cast<const float4*>(reinterpret_cast<const float*>(it.base) + off);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const float4 x = __ldg(p + u);
+            b[4 * u] = x.x; b[4 * u + 1] = x.y; b[4 * u + 2] = x.z; b[4 * u + 3] = x.w;
+        }
+    } else {
+#pragma unroll
+        for (int u = 0; u < 16; ++u) b[u] = 0.0f;
+    }
+}
+
+template <int FMT>
+__device__ __forceinline__ void store_codes16(uint8_t* p, const float* v, float s) {
+    uint4 o;
+    o.x = f32x4_to_fp8x4<FMT>(__fmul_rn(v[0], s), __fmul_rn(v[1], s), __fmul_rn(v[2], s), __fmul_rn(v[3], s));
+    o.y = f32x4_to_fp8x4<FMT>(__fmul_rn(v[4], s), __fmul_rn(v[5], s), __fmul_rn(v[6], s), __fmul_rn(v[7], s));
+    o.z = f32x4_to_fp8x4<FMT>(__fmul_rn(v[8], s), __fmul_rn(v[9], s), __fmul_rn(v[10], s), __fmul_rn(v[11], s));
+    o.w = f32x4_to_fp8x4<FMT>(__fmul_rn(v[12], s), __fmul_rn(v[13], s), __fmul_rn(v[14], s), __fmul_rn(v[15], s));
+    *reinterpret_cast<uint4*>(p) = o;
+}
+
+// One accumulator tile -> global memory.  Thread = one row (TMEM lane), 16 columns per tcgen05.ld.
+__device__ __forceinline__ void epilogue(const Item& it, uint32_t tmem_acc, int warp, int lane, uint32_t* s_red) {
+    const int r = warp * 32 + lane;
+    const bool row_ok = r < it.rows;
+    const int64_t grow = it.row0 + r;
+    const uint32_t taddr = tmem_acc + ((uint32_t)(warp * 32) << 16);
+    uint32_t a[16];
+    float v[16];
+    if (it.mode == EPI_BLOCKCAST) {
+        // pass 1: block amax over the 128 x 128 tile (all four epilogue warps)
+        uint32_t loc = 0;
+        for (int c0 = 0; c0 < it.cols; c0 += 16) {
+            tmem_ld16(taddr + c0, a);
+            if (row_ok) {
+                load_base16(it, grow * it.base_ld + it.col0 + c0, v);
+#pragma unroll
+                for (int u = 0; u < 16; ++u) loc = max(loc, __float_as_uint(v[u] + __uint_as_float(a[u])) & 0x7FFFFFFFu);
+            }
+        }
+        loc = warp_max_u32(loc);
+        if (lane == 0) s_red[warp] = loc;
+        asm volatile("bar.sync 1, 128;" ::: "memory");
+        const uint32_t bits = max(max(s_red[0], s_red[1]), max(s_red[2], s_red[3]));
+        asm volatile("bar.sync 1, 128;" ::: "memory");
+        float s, si;
+        scales_from_amax(bits, it.fmt == 0 ? 448.0f : 57344.0f, s, si);
+        if (r == 0) *it.scale_inv_out = si;
+        for (int c0 = 0; c0 < it.cols; c0 += 16) {
+            tmem_ld16(taddr + c0, a);
+            if (row_ok) {
+                load_base16(it, grow * it.base_ld + it.col0 + c0, v);
+#pragma unroll
+                for (int u = 0; u < 16; ++u) v[u] += __uint_as_float(a[u]);
+                uint8_t* p = reinterpret_cast<uint8_t*>(it.out) + grow * it.out_ld + it.col0 + c0;
+                if (it.fmt == 0) store_codes16<0>(p, v, s); else store_codes16<1>(p, v, s);
+            }
+        }
+        return;
+    }
+    float scale = 1.0f;
+    if (it.mode == EPI_CAST) {
+        float si;
+        scales_from_amax(*reinterpret_cast<volatile uint32_t*>(it.amax), it.fmt == 0 ? 448.0f : 57344.0f, scale, si);
+        if (it.write_scale && r == 0) *it.scale_inv_out = si;
+    }
+    uint32_t loc = 0;
+    for (int c0 = 0; c0 < it.cols; c0 += 16) {
+        tmem_ld16(taddr + c0, a);                 // warp-collective: every lane executes it
+        if (!row_ok) continue;
+        if (it.mode == EPI_STORE_T) {
+            bf16* o = reinterpret_cast<bf16*>(it.out);
+#pragma unroll
+            for (int u = 0; u < 16; ++u) {
+                const float cs = it.colscale ? __ldg(it.colscale + c0 + u) : 1.0f;
+                const float x = __uint_as_float(a[u]) * cs;
+                const bf16 hi = __float2bfloat16_rn(x);
+                o[(int64_t)(it.col0 + c0 + u) * it.out_ld + grow] = hi;
+                if (it.out_lo)
+                    reinterpret_cast<bf16*>(it.out_lo)[(int64_t)(it.col0 + c0 + u) * it.out_ld + grow] =
+                        __float2bfloat16_rn(x - __bfloat162float(hi));
+            }
+            continue;
+        }
+        load_base16(it, grow * it.base_ld + it.col0 + c0, v);
+#pragma unroll
+        for (int u = 0; u < 16; ++u) v[u] += __uint_as_float(a[u]);
+        if (it.mode == EPI_AMAX) {
+#pragma unroll
+            for (int u = 0; u < 16; ++u) loc = max(loc, __float_as_uint(v[u]) & 0x7FFFFFFFu);
+        } else if (it.mode == EPI_CAST) {
+            uint8_t* p = reinterpret_cast<uint8_t*>(it.out) + grow * it.out_ld + it.col0 + c0;
+            if (it.fmt == 0) store_codes16<0>(p, v, scale); else store_codes16<1>(p, v, scale);
+        } else {   // EPI_STORE
+            if (it.colscale) {
+#pragma unroll
+                for (int u = 0; u < 16; ++u) v[u] *= __ldg(it.colscale + c0 + u);
+            }
+            const int64_t off = grow * it.out_ld + it.col0 + c0;
+            if (it.out_type == TY_F32) {
+                float4* o = reinterpret_cast<float4*>(reinterpret_cast<float*>(it.out) + off);
+#pragma unroll
+                for (int u = 0; u < 4; ++u) o[u] = make_float4(v[4 * u], v[4 * u + 1], v[4 * u + 2], v[4 * u + 3]);
+            } else {
+                uint32_t w[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    const __nv_bfloat162 h = __floats2bfloat162_rn(v[2 * u], v[2 * u + 1]);
+                    w[u] = *reinterpret_cast<const uint32_t*>(&h);
+                }
+                uint4* o = reinterpret_cast<uint4*>(reinterpret_cast<bf16*>(it.out) + off);
+                o[0] = make_uint4(w[0], w[1], w[2], w[3]);
+                o[1] = make_uint4(w[4], w[5], w[6], w[7]);
+                if (it.out_lo) {
+#pragma unroll
+                    for (int u = 0; u < 8; ++u) {
+                        const float2 hi = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&w[u]));
+                        const __nv_bfloat162 h = __floats2bfloat162_rn(v[2 * u] - hi.x, v[2 * u + 1] - hi.y);
+                        w[u] = *reinterpret_cast<const uint32_t*>(&h);
+                    }
+                    uint4* o2 = reinterpret_cast<uint4*>(reinterpret_cast<bf16*>(it.out_lo) + off);
+                    o2[0] = make_uint4(w[0], w[1], w[2], w[3]);
+                    o2[1] = make_uint4(w[4], w[5], w[6], w[7]);
+                }
+            }
+        }
+    }
+    if (it.mode == EPI_AMAX) {
+        loc = warp_max_u32(loc);
+        if (lane == 0 && loc != 0u) atomicMax(it.amax, loc);
+    }
+}
+
+// ---- the kernel ------------------------------------------------------------------------------------------
+// Persistent: CTA b runs items b, b + gridDim.x, ...  `err` is set (and the kernel drains) if a barrier
+// wait times out, so a pipeline bug cannot hang the GPU.
+__global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __restrict__ items, int n_items,
+                                                              const CUtensorMap* __restrict__ maps, int* err) {
+    extern __shared__ uint8_t smem_raw[];
+    const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;          // 1024-byte aligned (swizzle atoms)
+    const uint32_t bars = smem0 + STAGES * STAGE_BYTES;                     // full[4] empty[4] tfull[2] tempty[2]
+    uint8_t* gen0 = smem_raw + (smem0 - smem_u32(smem_raw));
+    uint32_t* s_tmem = reinterpret_cast<uint32_t*>(gen0 + STAGES * STAGE_BYTES + 128);
+    uint32_t* s_red = s_tmem + 4;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    auto full_bar = [&](int s) { return bars + 8u * s; };
+    auto empty_bar = [&](int s) { return bars + 8u * (STAGES + s); };
+    auto tfull_bar = [&](int a) { return bars + 8u * (2 * STAGES + a); };
+    auto tempty_bar = [&](int a) { return bars + 8u * (2 * STAGES + 2 + a); };
+
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+        for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), 4); }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 5) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(s_tmem)), "r"(TMEM_COLS)
+                     : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(s_tmem);
+
+    if (warp == 4) {
+        // ===== TMA producer (one lane) =====
+        if (lane == 0) {
+            uint32_t stage = 0, phase = 0;
+            bool ok = true;
+            for (int i = blockIdx.x; i < n_items && ok; i += gridDim.x) {
+                const Item& it = items[i];
+                const int nb = it.N >> 6;
+                const uint32_t tx = A_BYTES + (uint32_t)it.N * 128u;
+                for (int seg = 0; seg < NSEG && ok; ++seg) {
+                    const int na = it.atoms[seg];
+                    if (na <= 0) continue;
+                    const CUtensorMap* ma = maps + it.map_a[seg];
+                    const CUtensorMap* mb = maps + it.map_b[seg];
+                    tmap_acquire(ma);
+                    tmap_acquire(mb);
+                    for (int t = 0; t < na; ++t) {
+                        if (!(ok = mbar_wait(empty_bar(stage), phase ^ 1u, err))) break;
+                        const uint32_t sa = smem0 + stage * STAGE_BYTES, sb = sa + A_BYTES;
+                        mbar_expect_tx(full_bar(stage), tx);
+                        if (it.a_mn) {
+                            tma_load_2d(sa, ma, it.a_c0[seg], it.a_r0[seg] + 64 * t, full_bar(stage));
+                            tma_load_2d(sa + 8192, ma, it.a_c0[seg] + 64, it.a_r0[seg] + 64 * t, full_bar(stage));
+                        } else {
+                            tma_load_2d(sa, ma, it.a_c0[seg] + 64 * t, it.a_r0[seg], full_bar(stage));
+                            tma_load_2d(sa + 8192, ma, it.a_c0[seg] + 64 * t, it.a_r0[seg] + 64, full_bar(stage));
+                        }
+                        for (int b = 0; b < nb; ++b)
+                            tma_load_2d(sb + 8192 * b, mb, it.b_c0[seg] + 64 * t, it.b_r0[seg] + 64 * b, full_bar(stage));
+                        if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                    }
+                }
+            }
+        }
+    } else if (warp == 5) {
+        // ===== MMA issuer (one lane) =====
+        if (lane == 0) {
+            uint32_t stage = 0, phase = 0, n_done = 0;
+            bool ok = true;
+            for (int i = blockIdx.x; i < n_items && ok; i += gridDim.x, ++n_done) {
+                const Item& it = items[i];
+                const uint32_t acc = n_done & 1u, aphase = (n_done >> 1) & 1u;
+                if (!(ok = mbar_wait(tempty_bar(acc), aphase ^ 1u, err))) break;
+                tc_fence_after();
+                const uint32_t d = tmem_base + acc * 256u;
+                const uint32_t idesc = instr_desc(it.N, it.a_mn);
+                int total = 0;
+#pragma unroll
+                for (int seg = 0; seg < NSEG; ++seg) total += it.atoms[seg];
+                for (int t = 0; t < total; ++t) {
+                    if (!(ok = mbar_wait(full_bar(stage), phase, err))) break;
+                    tc_fence_after();
+                    const uint32_t sa = smem0 + stage * STAGE_BYTES, sb = sa + A_BYTES;
+#pragma unroll
+                    for (int kk = 0; kk < 4; ++kk) {
+                        const uint64_t da = it.a_mn ? smem_desc(sa + 2048u * kk, 8192u, 1024u)
+                                                    : smem_desc(sa + 32u * kk, 16u, 1024u);
+                        const uint64_t db = smem_desc(sb + 32u * kk, 16u, 1024u);
+                        tc_mma_bf16(d, da, db, idesc, (t | kk) ? 1u : 0u);
+                    }
+                    tc_commit(empty_bar(stage));          // frees the smem stage when these MMAs retire
+                    if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                }
+                tc_commit(tfull_bar(acc));                // accumulator complete -> epilogue
+            }
+        }
+    } else {
+        // ===== epilogue warps 0..3 =====
+        uint32_t n_done = 0;
+        bool ok = true;
+        for (int i = blockIdx.x; i < n_items && ok; i += gridDim.x, ++n_done) {
+            const Item& it = items[i];
+            const uint32_t acc = n_done & 1u, aphase = (n_done >> 1) & 1u;
+            ok = mbar_wait(tfull_bar(acc), aphase, err);
+            ok = __all_sync(0xFFFFFFFFu, ok);
+            if (!ok) break;
+            tc_fence_after();
+            epilogue(it, tmem_base + acc * 256u, warp, lane, s_red);
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(tempty_bar(acc));
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 5) {
+        tc_fence_after();
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
+    }
+}
+
+}  // namespace tc
+}  // namespace gf8

@@ -23,6 +23,7 @@ MAX_RANK, MAX_R = 512, 64
 
 EXPORTS = [
     "gf8_create", "gf8_destroy", "gf8_payload_size", "gf8_status_string", "gf8_last_error", "gf8_launch_count",
+    "gf8_sync_check",
     "gf8_factor_update", "gf8_refresh_basis", "gf8_encode", "gf8_decode", "gf8_reduce_decoded",
     "gf8_encode_many", "gf8_reduce_decoded_many", "gf8_factor_update_many", "gf8_refresh_basis_many",
     "gf8_step_host", "gf8_get_factor", "gf8_set_factor", "gf8_get_basis", "gf8_set_basis",
@@ -79,6 +80,7 @@ def lib():
         L.gf8_last_error.argtypes = [vp]
         L.gf8_launch_count.restype = i64
         L.gf8_launch_count.argtypes = [vp]
+        L.gf8_sync_check.argtypes = [vp, vp]
         L.gf8_factor_update.argtypes = [vp, i32, vp, vp, i64, i32, vp]
         L.gf8_refresh_basis.argtypes = [vp, i32, i32, vp]
         L.gf8_encode.argtypes = [vp, i32, vp, i32, vp, vp, vp]
@@ -172,6 +174,10 @@ class Ctx:
 
     def launch_count(self) -> int:
         return int(lib().gf8_launch_count(self._h))
+
+    def sync_check(self):
+        """Synchronise the current stream and raise if a kernel reported an asynchronous failure."""
+        self._ck(lib().gf8_sync_check(self._h, _stream()))
 
     def payload_size(self, layer):
         a, b = C.c_size_t(), C.c_size_t()

@@ -141,6 +141,89 @@ def test_g5_reduce_decoded(name):
     assert relfro(to_np64(one), want1) <= TOL_EXACT
 
 
+# ---- the same gates on the FAST (BF16 tensor-core, tcgen05) path: north_star's 2e-3 tier ------------------
+TOL_FAST = 2e-3
+FAST_CASES = dict(CASES)
+FAST_CASES.update({
+    "llama600m-q": dict(m=1536, n=1536, kG=64, kA=64, side=gf8.SIDE_BOTH, dtype="bf16", seed=5, T=4096, q=2),
+    "wide-k96": dict(m=640, n=1168, kG=96, kA=80, side=gf8.SIDE_BOTH, dtype="bf16", seed=6, q=2),
+    "in-only-block": dict(m=384, n=528, kG=0, kA=32, side=gf8.SIDE_IN, dtype="bf16", seed=7, scaling=gf8.SCALE_BLOCK128),
+})
+_fcache = {}
+
+
+def fcase(name):
+    if name not in _fcache:
+        _fcache[name] = Case(precision=gf8.PREC_FAST, **FAST_CASES[name])
+    return _fcache[name]
+
+
+@pytest.mark.parametrize("name", list(FAST_CASES))
+def test_fast_g2_transform(name):
+    c = fcase(name)
+    wt = c.ctx.whiten_f32(0, c.G)
+    c.ctx.sync_check()
+    _, _, x = c.oracle_encode(c.G)
+    assert relfro(to_np64(wt), x) <= TOL_FAST
+
+
+@pytest.mark.parametrize("name", list(FAST_CASES))
+def test_fast_g3_encode_self_consistent(name):
+    """FAST replaces G3 by self-consistency: the fused encode's codes and scales are bit-identical to the
+    ORACLE quantizer applied to the GPU's own tapped W~, and stay close to the oracle's."""
+    c = fcase(name)
+    g = c.rank_grad(1)
+    wt = c.ctx.whiten_f32(0, g)
+    gc, gs = c.ctx.encode(0, g)
+    c.ctx.sync_check()
+    oc, os_ = oracle.quantize(wt.cpu().numpy(), c.fmt, c.scaling)
+    assert np.array_equal(gc.cpu().numpy(), oc) and np.array_equal(gs.cpu().numpy(), os_)
+    rc, rs, _ = c.oracle_encode(g)
+    assert np.allclose(gs.cpu().numpy(), rs, rtol=5e-3, atol=0)
+    # BF16-tier transform error flips codes near rounding boundaries; in value space the payload stays close
+    tab = oracle.fp8_table(c.fmt)
+    frac, _ = code_mismatch(gc.cpu().numpy(), rc)
+    assert frac <= 0.2 and relfro(tab[gc.cpu().numpy()], tab[rc]) <= 2e-2, frac
+
+
+@pytest.mark.parametrize("name", list(FAST_CASES))
+def test_fast_g5_reduce_decoded(name):
+    c = fcase(name)
+    R = 3
+    pays = [c.oracle_encode(c.rank_grad(r))[:2] for r in range(R)]
+    want = c.oracle_reduce_decoded([p[0] for p in pays], [p[1] for p in pays])
+    dc, ds = [_dev(p[0]) for p in pays], [_dev(p[1]) for p in pays]
+    got32 = c.ctx.reduce_decoded(0, dc, ds, True, dt=gf8.DT_F32)
+    c.ctx.sync_check()
+    assert relfro(to_np64(got32), want) <= TOL_FAST
+    got16 = c.ctx.reduce_decoded(0, dc, ds, True, dt=gf8.DT_BF16)
+    assert relfro(to_np64(got16), want) <= 2 * TOL_FAST
+    one = c.ctx.decode(0, dc[0], ds[0], dt=gf8.DT_F32)
+    want1 = c.oracle_reduce_decoded(pays[0][:1], [pays[0][1]], average=False)
+    assert relfro(to_np64(one), want1) <= TOL_FAST
+
+
+def test_fast_batched_matches_single_calls():
+    """encode_many / reduce_decoded_many with repeated layer ids (R ranks in one launch set) give the
+    same bytes as one call per payload."""
+    c = fcase("ragged-bf16")
+    R = 3
+    gs = [c.rank_grad(r) for r in range(R)]
+    single = [c.ctx.encode(0, g) for g in gs]
+    single = [(a.clone(), b.clone()) for a, b in single]
+    codes = [torch.empty_like(single[0][0]) for _ in range(R)]
+    sinvs = [torch.empty_like(single[0][1]) for _ in range(R)]
+    c.ctx.encode_many([0] * R, gs, codes, sinvs)
+    c.ctx.sync_check()
+    for r in range(R):
+        assert torch.equal(codes[r], single[r][0]) and torch.equal(sinvs[r], single[r][1])
+    out1 = c.ctx.reduce_decoded(0, codes, sinvs, True, dt=gf8.DT_BF16).clone()
+    outs = [torch.empty_like(out1)]
+    c.ctx.reduce_decoded_many([0], codes, sinvs, R, outs, average=True)
+    c.ctx.sync_check()
+    assert torch.equal(outs[0], out1)
+
+
 def test_euclidean_layer_is_plain_fp8():
     """side = NONE (embedding / LM head): codes and decoded values bit-exact."""
     m, n = 400, 256
