@@ -210,13 +210,25 @@ def run_gf8(args):
             for t in cfg.tensors]
     codes_flat = [codes[r][i] for i in ids for r in range(R)]
     sinvs_flat = [sinvs[r][i] for i in ids for r in range(R)]
+    # one batched call encodes every (tensor, rank) payload: pointer tables are marshalled once, as a training
+    # loop that reuses its gradient buffers would
+    dtc = gf8.DT_BF16 if cfg.dtype == "bf16" else gf8.DT_F32
+    a_ids_all = gf8.int_array([i for i in ids for _ in range(R)])
+    a_ids = gf8.int_array(ids)
+    a_grads = gf8.ptr_array([grads[r][i] for i in ids for r in range(R)])
+    a_codes, a_sinvs, a_outs = gf8.ptr_array(codes_flat), gf8.ptr_array(sinvs_flat), gf8.ptr_array(outs)
     torch.cuda.synchronize()
     gen_s = time.perf_counter() - t_gen0
 
+    def encode_all():
+        ctx.encode_many(a_ids_all, a_grads, a_codes, a_sinvs, dt=dtc)
+
+    def reduce_all():
+        ctx.reduce_decoded_many(a_ids, a_codes, a_sinvs, R, a_outs, average=True, dt=dtc)
+
     def step():
-        for r in range(R):
-            ctx.encode_many(ids, grads[r], codes[r], sinvs[r])
-        ctx.reduce_decoded_many(ids, codes_flat, sinvs_flat, R, outs, average=True)
+        encode_all()
+        reduce_all()
 
     def barrier():
         if world > 1:
@@ -235,13 +247,13 @@ def run_gf8(args):
     e0.record()
     for s in range(args.steps):
         seg[s][0].record()
-        for r in range(R):
-            ctx.encode_many(ids, grads[r], codes[r], sinvs[r])
+        encode_all()
         seg[s][1].record()
-        ctx.reduce_decoded_many(ids, codes_flat, sinvs_flat, R, outs, average=True)
+        reduce_all()
         seg[s][2].record()
     e1.record()
     barrier()
+    ctx.sync_check()
     clocks = sampler.stop()
     launches = ctx.launch_count() - l0
     ms = e0.elapsed_time(e1)
@@ -281,7 +293,7 @@ def run_gf8(args):
     # ---- e2e: the same step through gf8_step_host with pinned HOST buffers (H2D + D2H inside the timed region)
     e2e = None
     if not args.no_e2e:
-        del codes, sinvs, codes_flat, sinvs_flat
+        del codes, sinvs, codes_flat, sinvs_flat, a_codes, a_sinvs, a_grads
         hg = [g.cpu().pin_memory() for i in ids for g in [grads[r][i] for r in range(R)]]
         ho = [torch.empty_like(o, device="cpu").pin_memory() for o in outs]
         del grads

@@ -325,10 +325,18 @@ gf8_status fast_encode_many(gf8_ctx* c, int n, const int* layers, const void* co
             f.fmt = L.desc.fmt;
             f.base = grads[i];
             f.base_type = dt == GF8_DT_BF16 ? TY_BF16 : TY_F32;
+            f.base_map[0] = dt == GF8_DT_BF16 ? src_map : -1;      // BF16 gradients stream through TMA
+            f.base_map[1] = -1;
+            f.out_map = -1;
             if (tap) { f.mode = EPI_STORE; f.out = taps[i]; f.out_type = TY_F32; }
             else {
                 f.mode = L.desc.scaling == GF8_SCALE_TENSOR ? EPI_AMAX : EPI_BLOCKCAST;
                 f.out = codes[i]; f.amax = p->d_amax + t; f.scale_inv = sinv[i];
+                if (dt == GF8_DT_BF16) {
+                    CUtensorMap mc;
+                    if ((s = make_map_u8(c, &mc, codes[i], m, nn)) != GF8_OK) break;
+                    f.out_map = pb.add_map(codes[i], mc);
+                }
             }
             add_transform(pb, L, slot, src_map, -1, false, false, f);
         }
@@ -385,14 +393,24 @@ gf8_status fast_reduce_decoded_many(gf8_ctx* c, int n, const int* layers, const 
             LayerState& L = c->layers[layers[i]];
             if (!L.tc_ok) { p->plain.push_back(i); continue; }
             Slot* slot = nullptr;
-            if ((s = fast_slot(c, L, occurrence[layers[i]]++, true, true, true, &slot)) != GF8_OK) break;
-            p->reduces.push_back({i, slot->Uhat, slot->src16, slot->src16_lo});
+            if ((s = fast_slot(c, L, occurrence[layers[i]]++, true, false, true, &slot)) != GF8_OK) break;
+            p->reduces.push_back({i, nullptr, slot->src16, slot->src16_lo});
             const int src_map = pb.add_map(slot->src16, slot->map_src16);
             const int src_lo_map = pb.add_map(slot->src16_lo, slot->map_src16_lo);
             Final f;
             memset(&f, 0, sizeof(f));
-            f.mode = EPI_STORE; f.base = slot->Uhat; f.base_type = TY_F32;
+            // the reduced payload U^ is carried as hi + lo BF16 (16 mantissa bits): the same two tiles feed the
+            // projections as operands and the update as its streamed base
+            f.mode = EPI_STORE; f.base = nullptr; f.base_type = TY_BF16;
+            f.base_map[0] = src_map; f.base_map[1] = src_lo_map;
             f.out = outs[i]; f.out_type = dt == GF8_DT_BF16 ? TY_BF16 : TY_F32;
+            f.out_map = -1;
+            if (dt == GF8_DT_BF16) {
+                const LayerState& Lc = L;
+                CUtensorMap mo;
+                if ((s = make_map(c, &mo, outs[i], Lc.desc.d_out, Lc.desc.d_in, Lc.desc.d_in)) != GF8_OK) break;
+                f.out_map = pb.add_map(outs[i], mo);
+            }
             // the unwhitening multipliers ebar = 1/D - 1 amplify operand rounding, so decode runs split products
             add_transform(pb, L, slot, src_map, src_lo_map, true, true, f);
         }

@@ -13,6 +13,7 @@ struct Plan {
     CUtensorMap* d_maps = nullptr;
     gf8::tc::Item* d_items = nullptr;
     int stage_off[6] = {0, 0, 0, 0, 0, 0}, stage_cnt[6] = {0, 0, 0, 0, 0, 0};
+    int stage_base[6] = {0, 0, 0, 0, 0, 0};  // streamed base tiles per item in that stage's launch (0, 1 or 2)
     uint32_t* d_amax = nullptr;          // one word per TC problem (per-tensor scaling)
     size_t n_amax = 0;
     struct Convert { const float* src; gf8::bf16* dst; int64_t numel; };
@@ -27,7 +28,7 @@ namespace {
 using gf8::bf16;
 using gf8::tc::Item;
 
-constexpr int FAST_MAX_KP = 256;
+constexpr int FAST_MAX_KP = 256;   // two 128-column accumulator chunks per panel
 constexpr size_t FAST_MAX_PLANS = 64;
 
 inline int pad64(int k) { return (k + 63) / 64 * 64; }
@@ -62,6 +63,21 @@ gf8_status make_map(gf8_ctx* c, CUtensorMap* out, const void* ptr, uint64_t rows
                                                         CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                                                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(c, GF8_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d) for %llu x %llu", (int)r,
+                                       (unsigned long long)rows, (unsigned long long)cols);
+    return GF8_OK;
+}
+
+// FP8 code matrix [rows][cols] bytes -> TMA store map, 128 x 128 boxes (one update tile), 128 B swizzle.
+gf8_status make_map_u8(gf8_ctx* c, CUtensorMap* out, const void* ptr, uint64_t rows, uint64_t cols) {
+    const cuuint64_t gdim[2] = {cols, rows};
+    const cuuint64_t gstride[1] = {cols};
+    const cuuint32_t box[2] = {128, 128};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = ((EncodeTiledFn)c->encode_tiled)(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(ptr), gdim,
+                                                        gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                                        CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                                                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(c, GF8_ERR_CUDA, "cuTensorMapEncodeTiled (u8) failed (%d) for %llu x %llu", (int)r,
                                        (unsigned long long)rows, (unsigned long long)cols);
     return GF8_OK;
 }
@@ -182,11 +198,14 @@ struct Final {                  // what the last stage of a transform does with 
     const void* base; int base_type;
     void* out; int out_type;
     uint32_t* amax; float* scale_inv;
+    int base_map[2];            // TMA-streamed base tile(s) (hi [+ lo]); -1: base read straight from global memory
+    int out_map;                // TMA store map of the output (codes or BF16); -1: direct stores
 };
 
 inline Item blank_item() {
     Item it;
     memset(&it, 0, sizeof(it));
+    it.base_map[0] = it.base_map[1] = it.out_map = -1;
     return it;
 }
 
@@ -227,55 +246,60 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
         if (a.lo >= 0) one(a.lo, b.hi);
         if (b.lo >= 0) one(a.hi, b.lo);
     };
+    // panels wider than 128 basis columns are cut into 128-column accumulator chunks (nc)
     if (useA)      // P' = (src U_A) E_A : row panels
-        for (int i0 = 0; i0 < m; i0 += 128) {
-            Item it = blank_item();
-            int seg = 0;
-            add_product(it, seg, mSrc, mUAt, (n + 63) / 64, 0, i0, 0, 0);
-            it.N = kpA;
-            it.mode = EPI_STORE; it.out = s->Pp; it.out_lo = split ? s->Pp_lo : nullptr; it.out_ld = kpA;
-            it.out_type = TY_BF16; it.colscale = eA;
-            it.row0 = i0; it.rows = std::min(128, m - i0); it.cols = kpA;
-            pb.stage[0].push_back(it);
-        }
-    if (useG) {    // Q^T = src^T U_G : column panels (A is MN-major)
-        for (int j0 = 0; j0 < n; j0 += 128) {
-            Item it = blank_item();
-            int seg = 0;
-            add_product(it, seg, mSrc, mUGt, (m + 63) / 64, j0, 0, 0, 0);
-            it.a_mn = 1; it.N = kpG;
-            it.mode = EPI_STORE; it.row0 = j0; it.rows = std::min(128, n - j0); it.cols = kpG;
-            if (useA) { it.out = s->Qt; it.out_ld = kpG; it.out_type = TY_F32; }
-            else {
-                it.out = s->Qpt; it.out_lo = split ? s->Qpt_lo : nullptr; it.out_ld = kpG; it.out_type = TY_BF16;
-                it.colscale = eG;
-            }
-            pb.stage[1].push_back(it);
-        }
-        if (useA) {
-            // (S E_A)^T = P'^T U_G, stored transposed as SEA[g][a]
-            for (int a0 = 0; a0 < kpA; a0 += 128) {
+        for (int i0 = 0; i0 < m; i0 += 128)
+            for (int nc = 0; nc < kpA; nc += 128) {
                 Item it = blank_item();
                 int seg = 0;
-                add_product(it, seg, mPp, mUGt, (m + 63) / 64, a0, 0, 0, 0);
-                it.a_mn = 1; it.N = kpG;
-                it.mode = EPI_STORE_T; it.out = s->SEA; it.out_lo = split ? s->SEA_lo : nullptr; it.out_ld = kpA;
-                it.out_type = TY_BF16;
-                it.row0 = a0; it.rows = std::min(128, kpA - a0); it.cols = kpG;
+                add_product(it, seg, mSrc, mUAt, (n + 63) / 64, 0, i0, 0, nc);
+                it.N = std::min(128, kpA - nc);
+                it.mode = EPI_STORE; it.out = s->Pp; it.out_lo = split ? s->Pp_lo : nullptr; it.out_ld = kpA;
+                it.out_type = TY_BF16; it.colscale = eA + nc;
+                it.row0 = i0; it.col0 = nc; it.rows = std::min(128, m - i0); it.cols = it.N;
+                pb.stage[0].push_back(it);
+            }
+    if (useG) {    // Q^T = src^T U_G : column panels (A is MN-major)
+        for (int j0 = 0; j0 < n; j0 += 128)
+            for (int nc = 0; nc < kpG; nc += 128) {
+                Item it = blank_item();
+                int seg = 0;
+                add_product(it, seg, mSrc, mUGt, (m + 63) / 64, j0, 0, 0, nc);
+                it.a_mn = 1; it.N = std::min(128, kpG - nc);
+                it.mode = EPI_STORE; it.row0 = j0; it.col0 = nc; it.rows = std::min(128, n - j0); it.cols = it.N;
+                if (useA) { it.out = s->Qt; it.out_ld = kpG; it.out_type = TY_F32; }
+                else {
+                    it.out = s->Qpt; it.out_lo = split ? s->Qpt_lo : nullptr; it.out_ld = kpG; it.out_type = TY_BF16;
+                    it.colscale = eG + nc;
+                }
                 pb.stage[1].push_back(it);
             }
+        if (useA) {
+            // (S E_A)^T = P'^T U_G, stored transposed as SEA[g][a]
+            for (int a0 = 0; a0 < kpA; a0 += 128)
+                for (int nc = 0; nc < kpG; nc += 128) {
+                    Item it = blank_item();
+                    int seg = 0;
+                    add_product(it, seg, mPp, mUGt, (m + 63) / 64, a0, 0, 0, nc);
+                    it.a_mn = 1; it.N = std::min(128, kpG - nc);
+                    it.mode = EPI_STORE_T; it.out = s->SEA; it.out_lo = split ? s->SEA_lo : nullptr; it.out_ld = kpA;
+                    it.out_type = TY_BF16;
+                    it.row0 = a0; it.col0 = nc; it.rows = std::min(128, kpA - a0); it.cols = it.N;
+                    pb.stage[1].push_back(it);
+                }
             // Q'^T = (Q^T + U_A (S E_A)^T) E_G
-            for (int j0 = 0; j0 < n; j0 += 128) {
-                Item it = blank_item();
-                int seg = 0;
-                add_product(it, seg, mUA, mSEA, kpA / 64, 0, j0, 0, 0);
-                it.N = kpG;
-                it.mode = EPI_STORE; it.base = s->Qt; it.base_ld = kpG; it.base_type = TY_F32;
-                it.out = s->Qpt; it.out_lo = split ? s->Qpt_lo : nullptr; it.out_ld = kpG; it.out_type = TY_BF16;
-                it.colscale = eG;
-                it.row0 = j0; it.rows = std::min(128, n - j0); it.cols = kpG;
-                pb.stage[2].push_back(it);
-            }
+            for (int j0 = 0; j0 < n; j0 += 128)
+                for (int nc = 0; nc < kpG; nc += 128) {
+                    Item it = blank_item();
+                    int seg = 0;
+                    add_product(it, seg, mUA, mSEA, kpA / 64, 0, j0, 0, nc);
+                    it.N = std::min(128, kpG - nc);
+                    it.mode = EPI_STORE; it.base = s->Qt; it.base_ld = kpG; it.base_type = TY_F32;
+                    it.out = s->Qpt; it.out_lo = split ? s->Qpt_lo : nullptr; it.out_ld = kpG; it.out_type = TY_BF16;
+                    it.colscale = eG + nc;
+                    it.row0 = j0; it.col0 = nc; it.rows = std::min(128, n - j0); it.cols = it.N;
+                    pb.stage[2].push_back(it);
+                }
         }
     }
     // rank-(kA + kG) update of the streamed base tile
@@ -290,18 +314,19 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
             it.base = f.base; it.base_ld = n; it.base_type = f.base_type;
             it.row0 = i0; it.col0 = j0; it.rows = std::min(128, m - i0); it.cols = std::min(128, n - j0);
             it.mode = f.mode;
+            it.base_map[0] = f.base_map[0]; it.base_map[1] = f.base_map[1];
             if (f.mode == EPI_AMAX) {
                 it.amax = f.amax;
                 pb.stage[3].push_back(it);
-                it.mode = EPI_CAST; it.out = f.out; it.out_ld = n; it.scale_inv_out = f.scale_inv;
+                it.mode = EPI_CAST; it.out = f.out; it.out_ld = n; it.scale_inv_out = f.scale_inv; it.out_map = f.out_map;
                 it.write_scale = (i0 == 0 && j0 == 0) ? 1 : 0;
                 pb.stage[4].push_back(it);
             } else if (f.mode == EPI_BLOCKCAST) {
-                it.out = f.out; it.out_ld = n;
+                it.out = f.out; it.out_ld = n; it.out_map = f.out_map;
                 it.scale_inv_out = f.scale_inv + (size_t)(i0 / 128) * tiles_n + j0 / 128;
                 pb.stage[3].push_back(it);
             } else {
-                it.out = f.out; it.out_ld = n; it.out_type = f.out_type;
+                it.out = f.out; it.out_ld = n; it.out_type = f.out_type; it.out_map = f.out_map;
                 pb.stage[3].push_back(it);
             }
         }
@@ -326,6 +351,8 @@ gf8_status plan_finish(gf8_ctx* c, PlanBuilder& pb, Plan* p) {
         });
         p->stage_off[s] = (int)all.size();
         p->stage_cnt[s] = (int)pb.stage[s].size();
+        for (const Item& it : pb.stage[s])
+            p->stage_base[s] = std::max(p->stage_base[s], (it.base_map[0] >= 0 ? 1 : 0) + (it.base_map[1] >= 0 ? 1 : 0));
         all.insert(all.end(), pb.stage[s].begin(), pb.stage[s].end());
     }
     if (all.empty()) return GF8_OK;
@@ -357,8 +384,9 @@ gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, const Plan* p) {
     for (int s = 0; s < 6; ++s) {
         if (!p->stage_cnt[s]) continue;
         const int grid = std::min(p->stage_cnt[s], c->num_sms);
-        gf8::tc::tc_items_kernel<<<grid, gf8::tc::THREADS, gf8::tc::SMEM_BYTES, st>>>(p->d_items + p->stage_off[s],
-                                                                                  p->stage_cnt[s], p->d_maps, c->d_err);
+        const int n_base = p->stage_base[s], n_stages = gf8::tc::MAX_STAGES - 2 * n_base;
+        gf8::tc::tc_items_kernel<<<grid, gf8::tc::THREADS, gf8::tc::SMEM_BYTES, st>>>(
+            p->d_items + p->stage_off[s], p->stage_cnt[s], p->d_maps, c->d_err, n_stages, n_base);
         LAUNCH_CHECK(c);
     }
     return GF8_OK;

@@ -167,11 +167,13 @@ __global__ void __launch_bounds__(256) reduce_kernel(const __grid_constant__ Red
             for (int u = 0; u < 16; ++u) acc[u] = __fmul_rn(acc[u], invR);
         }
         if (sizeof(OutT) == 4) {
-            uint4* o = reinterpret_cast<uint4*>(reinterpret_cast<float*>(out) + e0);
+            if (out) {
+                uint4* o = reinterpret_cast<uint4*>(reinterpret_cast<float*>(out) + e0);
 #pragma unroll
-            for (int u = 0; u < 4; ++u)
-                st_stream(o + u, make_uint4(__float_as_uint(acc[4 * u]), __float_as_uint(acc[4 * u + 1]),
-                                            __float_as_uint(acc[4 * u + 2]), __float_as_uint(acc[4 * u + 3])));
+                for (int u = 0; u < 4; ++u)
+                    st_stream(o + u, make_uint4(__float_as_uint(acc[4 * u]), __float_as_uint(acc[4 * u + 1]),
+                                                __float_as_uint(acc[4 * u + 2]), __float_as_uint(acc[4 * u + 3])));
+            }
             if (out16) {      // BF16 copy: the tensor-core operand of the unwhitening projections (FAST path)
                 uint32_t w[8];
 #pragma unroll

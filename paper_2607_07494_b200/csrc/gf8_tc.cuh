@@ -11,10 +11,12 @@
 //     (S E_A)^T = P'^T U_G     A = P'   (MN-major), B = U_G^T        -> BF16, stored transposed
 //     Q'^T = (Q^T + U_A (S E_A)^T) E_G                               -> BF16 panel
 //     W~ = Wg + [P' | U_G] [U_A | Q'^T]^T   (rank-2k update)         -> amax / FP8 codes / BF16 / FP32
-// Operands are staged by TMA (cp.async.bulk.tensor, 64 x 64 BF16 boxes, 128-byte swizzle) through a
-// 4-stage mbarrier ring; one elected thread issues the MMAs; accumulators are double-buffered in TMEM
-// so the epilogue of item i overlaps the MMAs of item i+1.  Warps 0-3: epilogue (TMEM lane quarter =
-// warp index), warp 4: TMA producer, warp 5: TMEM allocation + MMA issue.
+// Operands are staged by TMA (cp.async.bulk.tensor, 64 x 64 BF16 boxes, 128-byte swizzle) through an
+// mbarrier ring of 32 KB stages; one elected thread issues the MMAs; accumulators are double-buffered in
+// TMEM so the epilogue of item i overlaps the MMAs of item i+1.  The streamed base tile of the rank-2k
+// update (the gradient itself: the HBM-bound traffic) is also fetched by TMA, double-buffered, and the
+// FP8 / BF16 output tile leaves through a TMA store, so every HBM access is a full-line bulk transfer.
+// Warps 0-3: epilogue (TMEM lane quarter = warp index), warp 4: TMA producer, warp 5: TMEM alloc + MMA issue.
 #pragma once
 #include <cuda.h>
 
@@ -24,13 +26,15 @@
 namespace gf8 {
 namespace tc {
 
-constexpr int STAGES = 4;
+constexpr int MAX_STAGES = 7;
 constexpr int A_BYTES = 128 * 64 * 2;            // one K-atom of A: 128 x 64 BF16
-constexpr int B_BYTES = 256 * 64 * 2;            // one K-atom of B: up to 256 x 64 BF16
-constexpr int STAGE_BYTES = A_BYTES + B_BYTES;   // 48 KB
-constexpr int SMEM_BYTES = STAGES * STAGE_BYTES + 1024 /*alignment slack*/ + 256 /*barriers*/;
+constexpr int B_BYTES = 128 * 64 * 2;            // one K-atom of B: up to 128 x 64 BF16
+constexpr int STAGE_BYTES = A_BYTES + B_BYTES;   // 32 KB
+constexpr int TILE_BYTES = 128 * 128 * 2;        // one streamed 128 x 128 BF16 base tile (two 64-column halves)
+constexpr int DATA_BYTES = MAX_STAGES * STAGE_BYTES;   // 224 KB, split at launch into ring stages + base tiles
+constexpr int SMEM_BYTES = DATA_BYTES + 1024 /*alignment slack*/ + 512 /*barriers*/;
 constexpr int THREADS = 192;
-constexpr int TMEM_COLS = 512;                   // two accumulators of up to 256 columns
+constexpr int TMEM_COLS = 256;                   // two accumulators of up to 128 columns
 constexpr int NSEG = 6;                          // operand segments per item (hi/lo split products)
 
 enum Epi : int32_t {
@@ -48,11 +52,12 @@ struct __align__(16) Item {
     int32_t a_c0[NSEG], a_r0[NSEG];     // first box of A: (col, row) in its matrix
     int32_t b_c0[NSEG], b_r0[NSEG];     // first box of B
     int32_t a_mn;                 // 1: A is MN-major (the 128 "M" elements are contiguous in memory)
-    int32_t N;                    // accumulator columns: multiple of 64, <= 256
+    int32_t N;                    // accumulator columns: multiple of 64, <= 128
     int32_t mode, fmt;
     int32_t row0, col0, rows, cols;   // output tile origin and valid extent (rows <= 128, cols <= N)
     int32_t base_type, out_type;
-    int32_t write_scale, pad0;
+    int32_t write_scale, out_map; // out_map >= 0: the output tile leaves through a TMA store from shared memory
+    int32_t base_map[2];          // >= 0: the base tile (hi [+ lo]) is streamed by TMA into shared memory
     int64_t base_ld, out_ld;
     const void* base;
     void* out;
@@ -272,26 +277,184 @@ __device__ __forceinline__ void epilogue(const Item& it, uint32_t tmem_acc, int 
     }
 }
 
+// ---- tile epilogue: base tile(s) in shared memory (TMA, 128 B swizzle), output through a TMA store ------------
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap* map, uint32_t src, int c, int r) {
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];"
+                 ::"l"(map), "r"(src), "r"(c), "r"(r) : "memory");
+}
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void sts128(uint32_t addr, const uint4& v) {
+    asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+// v[16] = base(hi [+ lo]) columns [c0, c0+16) of row r of the staged tile + accumulator.
+// Tile layout: half h (64 columns) at h * 16 KB, row r at r * 128 B, 16-byte chunk q at (q ^ (r & 7)) * 16.
+__device__ __forceinline__ void tile_values16(uint32_t tile, int n_base, int r, int c0, const uint32_t* a, float* v) {
+    const uint32_t row = tile + (uint32_t)(c0 >> 6) * 16384u + (uint32_t)r * 128u;
+    const uint32_t q = (uint32_t)(c0 & 63) >> 3;
+    const uint4 x = lds128(row + (((q) ^ (uint32_t)(r & 7)) << 4));
+    const uint4 y = lds128(row + (((q + 1) ^ (uint32_t)(r & 7)) << 4));
+    unpack_bf16x8(x, v);
+    unpack_bf16x8(y, v + 8);
+    if (n_base > 1) {
+        float w[16];
+        const uint4 x2 = lds128(row + TILE_BYTES + (((q) ^ (uint32_t)(r & 7)) << 4));
+        const uint4 y2 = lds128(row + TILE_BYTES + (((q + 1) ^ (uint32_t)(r & 7)) << 4));
+        unpack_bf16x8(x2, w);
+        unpack_bf16x8(y2, w + 8);
+#pragma unroll
+        for (int u = 0; u < 16; ++u) v[u] += w[u];
+    }
+#pragma unroll
+    for (int u = 0; u < 16; ++u) v[u] += __uint_as_float(a[u]);
+}
+
+template <int FMT>
+__device__ __forceinline__ uint4 codes16(const float* v, float s) {
+    uint4 o;
+    o.x = f32x4_to_fp8x4<FMT>(__fmul_rn(v[0], s), __fmul_rn(v[1], s), __fmul_rn(v[2], s), __fmul_rn(v[3], s));
+    o.y = f32x4_to_fp8x4<FMT>(__fmul_rn(v[4], s), __fmul_rn(v[5], s), __fmul_rn(v[6], s), __fmul_rn(v[7], s));
+    o.z = f32x4_to_fp8x4<FMT>(__fmul_rn(v[8], s), __fmul_rn(v[9], s), __fmul_rn(v[10], s), __fmul_rn(v[11], s));
+    o.w = f32x4_to_fp8x4<FMT>(__fmul_rn(v[12], s), __fmul_rn(v[13], s), __fmul_rn(v[14], s), __fmul_rn(v[15], s));
+    return o;
+}
+
+// Returns true if a TMA store was issued from `tile` (the caller must wait for its smem reads before reuse).
+__device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc, uint32_t tile, int n_base, int warp,
+                                              int lane, uint32_t* s_red, const CUtensorMap* maps) {
+    const int r = warp * 32 + lane;
+    const uint32_t taddr = tmem_acc + ((uint32_t)(warp * 32) << 16);
+    uint32_t a[16];
+    float v[16];
+    float scale = 1.0f;
+    if (it.mode == EPI_BLOCKCAST) {
+        uint32_t loc = 0;
+        for (int c0 = 0; c0 < 128; c0 += 16) {
+            tmem_ld16(taddr + c0, a);
+            tile_values16(tile, n_base, r, c0, a, v);
+#pragma unroll
+            for (int u = 0; u < 16; ++u) loc = max(loc, __float_as_uint(v[u]) & 0x7FFFFFFFu);
+        }
+        loc = warp_max_u32(loc);
+        if (lane == 0) s_red[warp] = loc;
+        asm volatile("bar.sync 1, 128;" ::: "memory");
+        const uint32_t bits = max(max(s_red[0], s_red[1]), max(s_red[2], s_red[3]));
+        asm volatile("bar.sync 1, 128;" ::: "memory");
+        float si;
+        scales_from_amax(bits, it.fmt == 0 ? 448.0f : 57344.0f, scale, si);
+        if (r == 0) *it.scale_inv_out = si;
+    } else if (it.mode == EPI_CAST) {
+        float si;
+        scales_from_amax(*reinterpret_cast<volatile uint32_t*>(it.amax), it.fmt == 0 ? 448.0f : 57344.0f, scale, si);
+        if (it.write_scale && r == 0) *it.scale_inv_out = si;
+    }
+    if (it.mode == EPI_AMAX) {
+        uint32_t loc = 0;
+        for (int c0 = 0; c0 < 128; c0 += 16) {
+            tmem_ld16(taddr + c0, a);
+            tile_values16(tile, n_base, r, c0, a, v);
+#pragma unroll
+            for (int u = 0; u < 16; ++u) loc = max(loc, __float_as_uint(v[u]) & 0x7FFFFFFFu);
+        }
+        loc = warp_max_u32(loc);
+        if (lane == 0 && loc != 0u) atomicMax(it.amax, loc);
+        return false;
+    }
+    if (it.mode == EPI_CAST || it.mode == EPI_BLOCKCAST) {
+        // 128 codes of this row, then written over the (consumed) first half of the row's base data:
+        // a dense 128 x 128-byte tile in the store map's 128 B swizzle
+        uint4 cd[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+            tmem_ld16(taddr + 16 * q, a);
+            tile_values16(tile, n_base, r, 16 * q, a, v);
+            cd[q] = it.fmt == 0 ? codes16<0>(v, scale) : codes16<1>(v, scale);
+        }
+        __syncwarp();
+#pragma unroll
+        for (int q = 0; q < 8; ++q) sts128(tile + (uint32_t)r * 128u + (((uint32_t)q ^ (uint32_t)(r & 7)) << 4), cd[q]);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        asm volatile("bar.sync 1, 128;" ::: "memory");
+        if (r == 0) {
+            tma_store_2d(maps + it.out_map, tile, it.col0, it.row0);
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        }
+        return true;
+    }
+    // EPI_STORE, BF16 output in place of the hi tile (same layout), or FP32 output straight to global memory
+    if (it.out_type == TY_BF16) {
+        for (int c0 = 0; c0 < 128; c0 += 16) {
+            tmem_ld16(taddr + c0, a);
+            tile_values16(tile, n_base, r, c0, a, v);
+            uint32_t w[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const __nv_bfloat162 h = __floats2bfloat162_rn(v[2 * u], v[2 * u + 1]);
+                w[u] = *reinterpret_cast<const uint32_t*>(&h);
+            }
+            const uint32_t row = tile + (uint32_t)(c0 >> 6) * 16384u + (uint32_t)r * 128u;
+            const uint32_t q = (uint32_t)(c0 & 63) >> 3;
+            sts128(row + ((q ^ (uint32_t)(r & 7)) << 4), make_uint4(w[0], w[1], w[2], w[3]));
+            sts128(row + (((q + 1) ^ (uint32_t)(r & 7)) << 4), make_uint4(w[4], w[5], w[6], w[7]));
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        asm volatile("bar.sync 1, 128;" ::: "memory");
+        if (r == 0) {
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int g = 0; g < 2; ++g)
+                    tma_store_2d(maps + it.out_map, tile + h * 16384u + g * 8192u, it.col0 + 64 * h, it.row0 + 64 * g);
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        }
+        return true;
+    }
+    const bool row_ok = r < it.rows;
+    for (int c0 = 0; c0 < it.cols; c0 += 16) {
+        tmem_ld16(taddr + c0, a);
+        tile_values16(tile, n_base, r, c0, a, v);
+        if (!row_ok) continue;
+        float4* o = reinterpret_cast<float4*>(reinterpret_cast<float*>(it.out) + (int64_t)(it.row0 + r) * it.out_ld + it.col0 + c0);
+#pragma unroll
+        for (int u = 0; u < 4; ++u) o[u] = make_float4(v[4 * u], v[4 * u + 1], v[4 * u + 2], v[4 * u + 3]);
+    }
+    return false;
+}
+
 // ---- the kernel ------------------------------------------------------------------------------------------
-// Persistent: CTA b runs items b, b + gridDim.x, ...  `err` is set (and the kernel drains) if a barrier
-// wait times out, so a pipeline bug cannot hang the GPU.
+// Persistent: CTA b runs items b, b + gridDim.x, ...  The 224 KB of data shared memory is split at launch into
+// `n_stages` operand ring stages (32 KB) and 2 x `n_base` streamed base tiles (32 KB; double-buffered like the
+// TMEM accumulators).  `err` is set (and the kernel drains) if a barrier wait times out, so a pipeline bug
+// cannot hang the GPU.
 __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __restrict__ items, int n_items,
-                                                              const CUtensorMap* __restrict__ maps, int* err) {
+                                                              const CUtensorMap* __restrict__ maps, int* err,
+                                                              int n_stages, int n_base) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;          // 1024-byte aligned (swizzle atoms)
-    const uint32_t bars = smem0 + STAGES * STAGE_BYTES;                     // full[4] empty[4] tfull[2] tempty[2]
+    const uint32_t base0 = smem0 + (uint32_t)n_stages * STAGE_BYTES;        // base tiles: [acc][n_base] x 32 KB
+    const uint32_t bars = smem0 + DATA_BYTES;      // full[7] empty[7] tfull[2] tempty[2] bfull[2] bempty[2]
     uint8_t* gen0 = smem_raw + (smem0 - smem_u32(smem_raw));
-    uint32_t* s_tmem = reinterpret_cast<uint32_t*>(gen0 + STAGES * STAGE_BYTES + 128);
+    uint32_t* s_tmem = reinterpret_cast<uint32_t*>(gen0 + DATA_BYTES + 192);
     uint32_t* s_red = s_tmem + 4;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     auto full_bar = [&](int s) { return bars + 8u * s; };
-    auto empty_bar = [&](int s) { return bars + 8u * (STAGES + s); };
-    auto tfull_bar = [&](int a) { return bars + 8u * (2 * STAGES + a); };
-    auto tempty_bar = [&](int a) { return bars + 8u * (2 * STAGES + 2 + a); };
+    auto empty_bar = [&](int s) { return bars + 8u * (MAX_STAGES + s); };
+    auto tfull_bar = [&](int a) { return bars + 8u * (2 * MAX_STAGES + a); };
+    auto tempty_bar = [&](int a) { return bars + 8u * (2 * MAX_STAGES + 2 + a); };
+    auto bfull_bar = [&](int a) { return bars + 8u * (2 * MAX_STAGES + 4 + a); };
+    auto bempty_bar = [&](int a) { return bars + 8u * (2 * MAX_STAGES + 6 + a); };
+    auto base_tile = [&](uint32_t a) { return base0 + a * (uint32_t)n_base * TILE_BYTES; };
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-        for (int a = 0; a < 2; ++a) { mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), 4); }
+        for (int s = 0; s < MAX_STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+        for (int a = 0; a < 2; ++a) {
+            mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), 4);
+            mbar_init(bfull_bar(a), 1); mbar_init(bempty_bar(a), 1);
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == 5) {
@@ -307,11 +470,33 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
     if (warp == 4) {
         // ===== TMA producer (one lane) =====
         if (lane == 0) {
-            uint32_t stage = 0, phase = 0;
+            uint32_t stage = 0, phase = 0, n_done = 0;
             bool ok = true;
-            for (int i = blockIdx.x; i < n_items && ok; i += gridDim.x) {
+            for (int i = blockIdx.x; i < n_items && ok; i += gridDim.x, ++n_done) {
                 const Item& it = items[i];
-                const int nb = it.N >> 6;
+                if (n_base > 0) {
+                    // the item's base tile(s): hi [+ lo], each 2 halves x 2 row groups of 64 x 64 boxes
+                    const uint32_t acc = n_done & 1u, aphase = (n_done >> 1) & 1u;
+                    if (!(ok = mbar_wait(bempty_bar(acc), aphase ^ 1u, err))) break;
+                    int nb = 0;
+                    for (int b = 0; b < 2; ++b) nb += (it.base_map[b] >= 0) ? 1 : 0;
+                    if (nb == 0) mbar_arrive(bfull_bar(acc));
+                    else {
+                        mbar_expect_tx(bfull_bar(acc), (uint32_t)nb * TILE_BYTES);
+                        for (int b = 0; b < nb; ++b) {
+                            const CUtensorMap* mp = maps + it.base_map[b];
+                            tmap_acquire(mp);
+                            const uint32_t dst = base_tile(acc) + (uint32_t)b * TILE_BYTES;
+#pragma unroll
+                            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                                for (int g = 0; g < 2; ++g)
+                                    tma_load_2d(dst + h * 16384u + g * 8192u, mp, it.col0 + 64 * h, it.row0 + 64 * g,
+                                                bfull_bar(acc));
+                        }
+                    }
+                }
+                const int nbx = it.N >> 6;
                 const uint32_t tx = A_BYTES + (uint32_t)it.N * 128u;
                 for (int seg = 0; seg < NSEG && ok; ++seg) {
                     const int na = it.atoms[seg];
@@ -331,9 +516,9 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                             tma_load_2d(sa, ma, it.a_c0[seg] + 64 * t, it.a_r0[seg], full_bar(stage));
                             tma_load_2d(sa + 8192, ma, it.a_c0[seg] + 64 * t, it.a_r0[seg] + 64, full_bar(stage));
                         }
-                        for (int b = 0; b < nb; ++b)
+                        for (int b = 0; b < nbx; ++b)
                             tma_load_2d(sb + 8192 * b, mb, it.b_c0[seg] + 64 * t, it.b_r0[seg] + 64 * b, full_bar(stage));
-                        if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                        if (++stage == (uint32_t)n_stages) { stage = 0; phase ^= 1u; }
                     }
                 }
             }
@@ -348,7 +533,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 const uint32_t acc = n_done & 1u, aphase = (n_done >> 1) & 1u;
                 if (!(ok = mbar_wait(tempty_bar(acc), aphase ^ 1u, err))) break;
                 tc_fence_after();
-                const uint32_t d = tmem_base + acc * 256u;
+                const uint32_t d = tmem_base + acc * 128u;
                 const uint32_t idesc = instr_desc(it.N, it.a_mn);
                 int total = 0;
 #pragma unroll
@@ -365,7 +550,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                         tc_mma_bf16(d, da, db, idesc, (t | kk) ? 1u : 0u);
                     }
                     tc_commit(empty_bar(stage));          // frees the smem stage when these MMAs retire
-                    if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                    if (++stage == (uint32_t)n_stages) { stage = 0; phase ^= 1u; }
                 }
                 tc_commit(tfull_bar(acc));                // accumulator complete -> epilogue
             }
@@ -375,17 +560,29 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
         uint32_t n_done = 0;
         bool ok = true;
         for (int i = blockIdx.x; i < n_items && ok; i += gridDim.x, ++n_done) {
-            const Item& it = items[i];
+            const Item it = items[i];
             const uint32_t acc = n_done & 1u, aphase = (n_done >> 1) & 1u;
-            ok = mbar_wait(tfull_bar(acc), aphase, err);
+            if (n_base > 0) ok = mbar_wait(bfull_bar(acc), aphase, err);
+            ok = ok && mbar_wait(tfull_bar(acc), aphase, err);
             ok = __all_sync(0xFFFFFFFFu, ok);
             if (!ok) break;
             tc_fence_after();
-            epilogue(it, tmem_base + acc * 256u, warp, lane, s_red);
+            bool stored = false;
+            if (it.base_map[0] >= 0) stored = epilogue_tile(it, tmem_base + acc * 128u, base_tile(acc), it.base_map[1] >= 0 ? 2 : 1,
+                                                            warp, lane, s_red, maps);
+            else epilogue(it, tmem_base + acc * 128u, warp, lane, s_red);
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive(tempty_bar(acc));
+            if (n_base > 0) {
+                asm volatile("bar.sync 1, 128;" ::: "memory");          // every epilogue thread is done with the tile
+                if (threadIdx.x == 0) {
+                    if (stored) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+                    mbar_arrive(bempty_bar(acc));
+                }
+            }
         }
+        if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     }
     tc_fence_before();
     __syncthreads();

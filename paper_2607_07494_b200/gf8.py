@@ -126,11 +126,25 @@ def _ptr(t: Optional[torch.Tensor]):
     return C.c_void_p(t.data_ptr())
 
 
-def _ptr_array(ts: Sequence[Optional[torch.Tensor]]):
+def _ptr_array(ts):
+    """ctypes array of device (or host) pointers; an array made earlier by ptr_array() passes through, so a
+    training loop that reuses its buffers marshals them once."""
+    if isinstance(ts, C.Array):
+        return ts
     arr = (C.c_void_p * len(ts))()
     for i, t in enumerate(ts):
         arr[i] = None if t is None else t.data_ptr()
     return arr
+
+
+def ptr_array(ts: Sequence[Optional[torch.Tensor]]):
+    for t in ts:
+        assert t is None or t.is_contiguous(), "gf8 takes contiguous row-major tensors"
+    return _ptr_array(list(ts))
+
+
+def int_array(xs):
+    return xs if isinstance(xs, C.Array) else (C.c_int * len(xs))(*xs)
 
 
 def _stream():
@@ -235,17 +249,19 @@ class Ctx:
                                           1 if average else 0, _ptr(out), _dt(out), _stream()))
         return out
 
-    def encode_many(self, layers, grads, codes, scale_invs):
+    def encode_many(self, layers, grads, codes, scale_invs, dt=None):
         n = len(layers)
-        self._ck(lib().gf8_encode_many(self._h, n, (C.c_int * n)(*layers), _ptr_array(grads), _dt(grads[0]),
+        dt = dt if dt is not None else _dt(grads[0])
+        self._ck(lib().gf8_encode_many(self._h, n, int_array(layers), _ptr_array(grads), dt,
                                        _ptr_array(codes), _ptr_array(scale_invs), _stream()))
 
-    def reduce_decoded_many(self, layers, codes, scale_invs, R, outs, average=True):
+    def reduce_decoded_many(self, layers, codes, scale_invs, R, outs, average=True, dt=None):
         """codes / scale_invs: flat lists of n*R tensors, index [i*R + r]."""
         n = len(layers)
-        self._ck(lib().gf8_reduce_decoded_many(self._h, n, (C.c_int * n)(*layers), _ptr_array(codes),
+        dt = dt if dt is not None else _dt(outs[0])
+        self._ck(lib().gf8_reduce_decoded_many(self._h, n, int_array(layers), _ptr_array(codes),
                                                _ptr_array(scale_invs), R, 1 if average else 0, _ptr_array(outs),
-                                               _dt(outs[0]), _stream()))
+                                               dt, _stream()))
 
     def step_host(self, layers, grads_host, R, outs_host, average=True):
         """grads_host: flat list of n*R pinned CPU tensors [i*R + r]; outs_host: n pinned CPU tensors."""
