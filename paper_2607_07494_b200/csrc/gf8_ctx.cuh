@@ -80,6 +80,7 @@ struct gf8_ctx {
     std::map<std::vector<uint64_t>, struct Plan*> plans;
     std::vector<struct Plan*> plan_order;
     int* d_err = nullptr;
+    long long* d_prof = nullptr;     // debug profile of the TC kernel (GF8_TC_DBG & 4)
     void* encode_tiled = nullptr;    // cuTensorMapEncodeTiled, resolved at run time (no link-time libcuda)
     bool tc_attr_set = false;
     int64_t launches = 0;

@@ -45,6 +45,7 @@ gf8_status fast_init(gf8_ctx* c) {
     if (!fn || q != cudaDriverEntryPointSuccess) return fail(c, GF8_ERR_CUDA, "cuTensorMapEncodeTiled not available");
     c->encode_tiled = fn;
     GF_TRY(dmalloc(c, &c->d_err, 1));
+    GF_TRY(dmalloc(c, &c->d_prof, (size_t)c->num_sms * 18 + 64));
     CU_TRY(c, cudaMemset(c->d_err, 0, sizeof(int)));
     CU_TRY(c, cudaFuncSetAttribute(gf8::tc::tc_items_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                    gf8::tc::SMEM_BYTES));
@@ -384,9 +385,26 @@ gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, const Plan* p) {
     for (int s = 0; s < 6; ++s) {
         if (!p->stage_cnt[s]) continue;
         const int grid = std::min(p->stage_cnt[s], c->num_sms);
-        const int n_base = p->stage_base[s], n_stages = gf8::tc::MAX_STAGES - 2 * n_base;
+        const int n_base = p->stage_base[s];
+        // shared-memory split: update stages keep a short operand ring (their operands are L2-resident) and give
+        // the rest to base tiles in flight (the HBM stream); panel stages give everything to the operand ring
+        int n_stages = n_base ? 3 : gf8::tc::MAX_STAGES, dbg = 0, only = -1;
+        const int n_bslots = n_base ? (gf8::tc::MAX_STAGES - n_stages) / n_base : 1;
+        if (const char* e = getenv("GF8_TC_DBG")) dbg = atoi(e);
+        if (const char* e = getenv("GF8_TC_ONLY")) only = atoi(e);
+        if (only >= 0 && only != s) continue;
         gf8::tc::tc_items_kernel<<<grid, gf8::tc::THREADS, gf8::tc::SMEM_BYTES, st>>>(
-            p->d_items + p->stage_off[s], p->stage_cnt[s], p->d_maps, c->d_err, n_stages, n_base);
+            p->d_items + p->stage_off[s], p->stage_cnt[s], p->d_maps, c->d_err, n_stages, n_base, n_bslots, dbg, (dbg & 4) ? c->d_prof : nullptr);
+        if (dbg & 4) {
+            std::vector<long long> h((size_t)c->num_sms * 18);
+            cudaMemcpy(h.data(), c->d_prof, h.size() * sizeof(long long), cudaMemcpyDeviceToHost);
+            const char* roles[3] = {"epilogue", "producer", "mma"};
+            for (int r = 0; r < 3; ++r) {
+                double a[6] = {0, 0, 0, 0, 0, 0};
+                for (int b = 0; b < grid; ++b) for (int q = 0; q < 6; ++q) a[q] += (double)h[((size_t)b * 3 + r) * 6 + q] / grid;
+                fprintf(stderr, "stage %d %-8s waits[0..2] %.0f %.0f %.0f  work %.0f  post %.0f  total %.0f cycles (avg/CTA)\n", s, roles[r], a[0], a[1], a[2], a[3], a[4], a[5]);
+            }
+        }
         LAUNCH_CHECK(c);
     }
     return GF8_OK;

@@ -16,7 +16,8 @@
 // TMEM so the epilogue of item i overlaps the MMAs of item i+1.  The streamed base tile of the rank-2k
 // update (the gradient itself: the HBM-bound traffic) is also fetched by TMA, double-buffered, and the
 // FP8 / BF16 output tile leaves through a TMA store, so every HBM access is a full-line bulk transfer.
-// Warps 0-3: epilogue (TMEM lane quarter = warp index), warp 4: TMA producer, warp 5: TMEM alloc + MMA issue.
+// Warps 0-7: epilogue (TMEM lane quarter = warp & 3, column half = warp >> 2), warp 8: item fetch + TMA
+// producer, warp 9: TMEM allocation + MMA issue.
 #pragma once
 #include <cuda.h>
 
@@ -32,8 +33,11 @@ constexpr int B_BYTES = 128 * 64 * 2;            // one K-atom of B: up to 128 x
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;   // 32 KB
 constexpr int TILE_BYTES = 128 * 128 * 2;        // one streamed 128 x 128 BF16 base tile (two 64-column halves)
 constexpr int DATA_BYTES = MAX_STAGES * STAGE_BYTES;   // 224 KB, split at launch into ring stages + base tiles
-constexpr int SMEM_BYTES = DATA_BYTES + 1024 /*alignment slack*/ + 512 /*barriers*/;
-constexpr int THREADS = 192;
+constexpr int SMEM_BYTES = DATA_BYTES + 1024 /*alignment slack*/ + 1536 /*barriers, item ring*/;
+constexpr int EPI_WARPS = 8, PRODUCER_WARP = 8, MMA_WARP = 9;
+constexpr int THREADS = 32 * (EPI_WARPS + 2);
+constexpr int ITEM_SLOTS = 4;                    // shared-memory ring of item descriptors
+constexpr int MAX_BASE_SLOTS = 4;                // streamed base tiles in flight (ring, decoupled from TMEM)
 constexpr int TMEM_COLS = 256;                   // two accumulators of up to 128 columns
 constexpr int NSEG = 6;                          // operand segments per item (hi/lo split products)
 
@@ -66,6 +70,9 @@ struct __align__(16) Item {
     uint32_t* amax;               // EPI_AMAX: target; EPI_CAST: source
     float* scale_inv_out;         // EPI_CAST (write_scale) / EPI_BLOCKCAST: where scale_inv goes
 };
+
+constexpr int ITEM_BYTES = (int)sizeof(Item);
+static_assert(ITEM_BYTES % 16 == 0 && 352 + ITEM_SLOTS * ITEM_BYTES <= 1536, "item ring must fit its shared-memory slice");
 
 // ---- PTX wrappers ------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -135,6 +142,8 @@ __device__ __forceinline__ uint32_t instr_desc(int N, int a_mn) {
 }
 
 // ---- epilogue helpers ---------------------------------------------------------------------------------
+// Eight epilogue warps: warp w reads TMEM lanes 32 (w & 3) .. +31 (one accumulator row per thread) and the
+// column half (w >> 2) of the tile, so every SM sub-partition holds two epilogue warps.
 // 16 consecutive elements of the base tile row as floats (zero when there is no base).
 __device__ __forceinline__ void load_base16(const Item& it, int64_t off, float* b) {
     if (it.base_type == TY_BF16) {
@@ -156,27 +165,43 @@ __device__ __forceinline__ void load_base16(const Item& it, int64_t off, float* 
 }
 
 template <int FMT>
-__device__ __forceinline__ void store_codes16(uint8_t* p, const float* v, float s) {
+__device__ __forceinline__ uint4 codes16(const float* v, float s) {
     uint4 o;
     o.x = f32x4_to_fp8x4<FMT>(__fmul_rn(v[0], s), __fmul_rn(v[1], s), __fmul_rn(v[2], s), __fmul_rn(v[3], s));
     o.y = f32x4_to_fp8x4<FMT>(__fmul_rn(v[4], s), __fmul_rn(v[5], s), __fmul_rn(v[6], s), __fmul_rn(v[7], s));
     o.z = f32x4_to_fp8x4<FMT>(__fmul_rn(v[8], s), __fmul_rn(v[9], s), __fmul_rn(v[10], s), __fmul_rn(v[11], s));
     o.w = f32x4_to_fp8x4<FMT>(__fmul_rn(v[12], s), __fmul_rn(v[13], s), __fmul_rn(v[14], s), __fmul_rn(v[15], s));
-    *reinterpret_cast<uint4*>(p) = o;
+    return o;
 }
 
-// One accumulator tile -> global memory.  Thread = one row (TMEM lane), 16 columns per tcgen05.ld.
+__device__ __forceinline__ void epi_sync() { asm volatile("bar.sync 1, 256;" ::: "memory"); }
+
+__device__ __forceinline__ uint32_t epi_block_max(uint32_t loc, int warp, int lane, uint32_t* s_red) {
+    loc = warp_max_u32(loc);
+    if (lane == 0) s_red[warp] = loc;
+    epi_sync();
+    uint32_t bits = 0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) bits = max(bits, s_red[w]);
+    epi_sync();
+    return bits;
+}
+
+// One accumulator tile -> global memory with the base (if any) read straight from global memory: the small
+// panels (P', Q^T, S, Q'^T) and FP32 gradients.  Thread = one row, 16 columns per tcgen05.ld.
 __device__ __forceinline__ void epilogue(const Item& it, uint32_t tmem_acc, int warp, int lane, uint32_t* s_red) {
-    const int r = warp * 32 + lane;
+    const int r = (warp & 3) * 32 + lane, half = warp >> 2;
     const bool row_ok = r < it.rows;
     const int64_t grow = it.row0 + r;
-    const uint32_t taddr = tmem_acc + ((uint32_t)(warp * 32) << 16);
+    const uint32_t taddr = tmem_acc + ((uint32_t)((warp & 3) * 32) << 16);
+    const int nch = it.cols >> 4;
+    const int cb = half ? ((nch + 1) >> 1) << 4 : 0, ce = half ? nch << 4 : ((nch + 1) >> 1) << 4;
     uint32_t a[16];
     float v[16];
+    float scale = 1.0f;
     if (it.mode == EPI_BLOCKCAST) {
-        // pass 1: block amax over the 128 x 128 tile (all four epilogue warps)
         uint32_t loc = 0;
-        for (int c0 = 0; c0 < it.cols; c0 += 16) {
+        for (int c0 = cb; c0 < ce; c0 += 16) {
             tmem_ld16(taddr + c0, a);
             if (row_ok) {
                 load_base16(it, grow * it.base_ld + it.col0 + c0, v);
@@ -184,34 +209,17 @@ __device__ __forceinline__ void epilogue(const Item& it, uint32_t tmem_acc, int 
                 for (int u = 0; u < 16; ++u) loc = max(loc, __float_as_uint(v[u] + __uint_as_float(a[u])) & 0x7FFFFFFFu);
             }
         }
-        loc = warp_max_u32(loc);
-        if (lane == 0) s_red[warp] = loc;
-        asm volatile("bar.sync 1, 128;" ::: "memory");
-        const uint32_t bits = max(max(s_red[0], s_red[1]), max(s_red[2], s_red[3]));
-        asm volatile("bar.sync 1, 128;" ::: "memory");
-        float s, si;
-        scales_from_amax(bits, it.fmt == 0 ? 448.0f : 57344.0f, s, si);
-        if (r == 0) *it.scale_inv_out = si;
-        for (int c0 = 0; c0 < it.cols; c0 += 16) {
-            tmem_ld16(taddr + c0, a);
-            if (row_ok) {
-                load_base16(it, grow * it.base_ld + it.col0 + c0, v);
-#pragma unroll
-                for (int u = 0; u < 16; ++u) v[u] += __uint_as_float(a[u]);
-                uint8_t* p = reinterpret_cast<uint8_t*>(it.out) + grow * it.out_ld + it.col0 + c0;
-                if (it.fmt == 0) store_codes16<0>(p, v, s); else store_codes16<1>(p, v, s);
-            }
-        }
-        return;
-    }
-    float scale = 1.0f;
-    if (it.mode == EPI_CAST) {
+        const uint32_t bits = epi_block_max(loc, warp, lane, s_red);
+        float si;
+        scales_from_amax(bits, it.fmt == 0 ? 448.0f : 57344.0f, scale, si);
+        if (r == 0 && half == 0) *it.scale_inv_out = si;
+    } else if (it.mode == EPI_CAST) {
         float si;
         scales_from_amax(*reinterpret_cast<volatile uint32_t*>(it.amax), it.fmt == 0 ? 448.0f : 57344.0f, scale, si);
-        if (it.write_scale && r == 0) *it.scale_inv_out = si;
+        if (it.write_scale && r == 0 && half == 0) *it.scale_inv_out = si;
     }
     uint32_t loc = 0;
-    for (int c0 = 0; c0 < it.cols; c0 += 16) {
+    for (int c0 = cb; c0 < ce; c0 += 16) {
         tmem_ld16(taddr + c0, a);                 // warp-collective: every lane executes it
         if (!row_ok) continue;
         if (it.mode == EPI_STORE_T) {
@@ -234,9 +242,9 @@ __device__ __forceinline__ void epilogue(const Item& it, uint32_t tmem_acc, int 
         if (it.mode == EPI_AMAX) {
 #pragma unroll
             for (int u = 0; u < 16; ++u) loc = max(loc, __float_as_uint(v[u]) & 0x7FFFFFFFu);
-        } else if (it.mode == EPI_CAST) {
+        } else if (it.mode == EPI_CAST || it.mode == EPI_BLOCKCAST) {
             uint8_t* p = reinterpret_cast<uint8_t*>(it.out) + grow * it.out_ld + it.col0 + c0;
-            if (it.fmt == 0) store_codes16<0>(p, v, scale); else store_codes16<1>(p, v, scale);
+            *reinterpret_cast<uint4*>(p) = it.fmt == 0 ? codes16<0>(v, scale) : codes16<1>(v, scale);
         } else {   // EPI_STORE
             if (it.colscale) {
 #pragma unroll
@@ -313,73 +321,55 @@ __device__ __forceinline__ void tile_values16(uint32_t tile, int n_base, int r, 
     for (int u = 0; u < 16; ++u) v[u] += __uint_as_float(a[u]);
 }
 
-template <int FMT>
-__device__ __forceinline__ uint4 codes16(const float* v, float s) {
-    uint4 o;
-    o.x = f32x4_to_fp8x4<FMT>(__fmul_rn(v[0], s), __fmul_rn(v[1], s), __fmul_rn(v[2], s), __fmul_rn(v[3], s));
-    o.y = f32x4_to_fp8x4<FMT>(__fmul_rn(v[4], s), __fmul_rn(v[5], s), __fmul_rn(v[6], s), __fmul_rn(v[7], s));
-    o.z = f32x4_to_fp8x4<FMT>(__fmul_rn(v[8], s), __fmul_rn(v[9], s), __fmul_rn(v[10], s), __fmul_rn(v[11], s));
-    o.w = f32x4_to_fp8x4<FMT>(__fmul_rn(v[12], s), __fmul_rn(v[13], s), __fmul_rn(v[14], s), __fmul_rn(v[15], s));
-    return o;
-}
-
-// Returns true if a TMA store was issued from `tile` (the caller must wait for its smem reads before reuse).
+// Returns true if a TMA store was issued from `tile` (the caller waits for its smem reads before reuse).
+// Each warp covers 32 rows x 64 columns (its half) as four 16-column chunks.
 __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc, uint32_t tile, int n_base, int warp,
                                               int lane, uint32_t* s_red, const CUtensorMap* maps) {
-    const int r = warp * 32 + lane;
-    const uint32_t taddr = tmem_acc + ((uint32_t)(warp * 32) << 16);
+    const int r = (warp & 3) * 32 + lane, half = warp >> 2, cbase = half * 64;
+    const uint32_t taddr = tmem_acc + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)cbase;
     uint32_t a[16];
     float v[16];
     float scale = 1.0f;
-    if (it.mode == EPI_BLOCKCAST) {
+    if (it.mode == EPI_BLOCKCAST || it.mode == EPI_AMAX) {
         uint32_t loc = 0;
-        for (int c0 = 0; c0 < 128; c0 += 16) {
-            tmem_ld16(taddr + c0, a);
-            tile_values16(tile, n_base, r, c0, a, v);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            tmem_ld16(taddr + 16 * q, a);
+            tile_values16(tile, n_base, r, cbase + 16 * q, a, v);
 #pragma unroll
             for (int u = 0; u < 16; ++u) loc = max(loc, __float_as_uint(v[u]) & 0x7FFFFFFFu);
         }
-        loc = warp_max_u32(loc);
-        if (lane == 0) s_red[warp] = loc;
-        asm volatile("bar.sync 1, 128;" ::: "memory");
-        const uint32_t bits = max(max(s_red[0], s_red[1]), max(s_red[2], s_red[3]));
-        asm volatile("bar.sync 1, 128;" ::: "memory");
+        if (it.mode == EPI_AMAX) {
+            loc = warp_max_u32(loc);
+            if (lane == 0 && loc != 0u) atomicMax(it.amax, loc);
+            return false;
+        }
+        const uint32_t bits = epi_block_max(loc, warp, lane, s_red);
         float si;
         scales_from_amax(bits, it.fmt == 0 ? 448.0f : 57344.0f, scale, si);
-        if (r == 0) *it.scale_inv_out = si;
+        if (r == 0 && half == 0) *it.scale_inv_out = si;
     } else if (it.mode == EPI_CAST) {
         float si;
         scales_from_amax(*reinterpret_cast<volatile uint32_t*>(it.amax), it.fmt == 0 ? 448.0f : 57344.0f, scale, si);
-        if (it.write_scale && r == 0) *it.scale_inv_out = si;
-    }
-    if (it.mode == EPI_AMAX) {
-        uint32_t loc = 0;
-        for (int c0 = 0; c0 < 128; c0 += 16) {
-            tmem_ld16(taddr + c0, a);
-            tile_values16(tile, n_base, r, c0, a, v);
-#pragma unroll
-            for (int u = 0; u < 16; ++u) loc = max(loc, __float_as_uint(v[u]) & 0x7FFFFFFFu);
-        }
-        loc = warp_max_u32(loc);
-        if (lane == 0 && loc != 0u) atomicMax(it.amax, loc);
-        return false;
+        if (it.write_scale && r == 0 && half == 0) *it.scale_inv_out = si;
     }
     if (it.mode == EPI_CAST || it.mode == EPI_BLOCKCAST) {
-        // 128 codes of this row, then written over the (consumed) first half of the row's base data:
-        // a dense 128 x 128-byte tile in the store map's 128 B swizzle
-        uint4 cd[8];
+        // 64 codes of this row half; the 128 x 128-byte code tile then overwrites the (consumed) first half of
+        // the base tile in the store map's 128 B swizzle
+        uint4 cd[4];
 #pragma unroll
-        for (int q = 0; q < 8; ++q) {
+        for (int q = 0; q < 4; ++q) {
             tmem_ld16(taddr + 16 * q, a);
-            tile_values16(tile, n_base, r, 16 * q, a, v);
+            tile_values16(tile, n_base, r, cbase + 16 * q, a, v);
             cd[q] = it.fmt == 0 ? codes16<0>(v, scale) : codes16<1>(v, scale);
         }
-        __syncwarp();
+        epi_sync();                               // every thread has read its base data
 #pragma unroll
-        for (int q = 0; q < 8; ++q) sts128(tile + (uint32_t)r * 128u + (((uint32_t)q ^ (uint32_t)(r & 7)) << 4), cd[q]);
+        for (int q = 0; q < 4; ++q)
+            sts128(tile + (uint32_t)r * 128u + (((uint32_t)(4 * half + q) ^ (uint32_t)(r & 7)) << 4), cd[q]);
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        asm volatile("bar.sync 1, 128;" ::: "memory");
-        if (r == 0) {
+        epi_sync();
+        if (threadIdx.x == 0) {
             tma_store_2d(maps + it.out_map, tile, it.col0, it.row0);
             asm volatile("cp.async.bulk.commit_group;" ::: "memory");
         }
@@ -387,8 +377,10 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
     }
     // EPI_STORE, BF16 output in place of the hi tile (same layout), or FP32 output straight to global memory
     if (it.out_type == TY_BF16) {
-        for (int c0 = 0; c0 < 128; c0 += 16) {
-            tmem_ld16(taddr + c0, a);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int c0 = cbase + 16 * q;
+            tmem_ld16(taddr + 16 * q, a);
             tile_values16(tile, n_base, r, c0, a, v);
             uint32_t w[8];
 #pragma unroll
@@ -396,14 +388,13 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
                 const __nv_bfloat162 h = __floats2bfloat162_rn(v[2 * u], v[2 * u + 1]);
                 w[u] = *reinterpret_cast<const uint32_t*>(&h);
             }
-            const uint32_t row = tile + (uint32_t)(c0 >> 6) * 16384u + (uint32_t)r * 128u;
-            const uint32_t q = (uint32_t)(c0 & 63) >> 3;
-            sts128(row + ((q ^ (uint32_t)(r & 7)) << 4), make_uint4(w[0], w[1], w[2], w[3]));
-            sts128(row + (((q + 1) ^ (uint32_t)(r & 7)) << 4), make_uint4(w[4], w[5], w[6], w[7]));
+            const uint32_t row = tile + (uint32_t)half * 16384u + (uint32_t)r * 128u;
+            sts128(row + (((uint32_t)(2 * q) ^ (uint32_t)(r & 7)) << 4), make_uint4(w[0], w[1], w[2], w[3]));
+            sts128(row + (((uint32_t)(2 * q + 1) ^ (uint32_t)(r & 7)) << 4), make_uint4(w[4], w[5], w[6], w[7]));
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        asm volatile("bar.sync 1, 128;" ::: "memory");
-        if (r == 0) {
+        epi_sync();
+        if (threadIdx.x == 0) {
 #pragma unroll
             for (int h = 0; h < 2; ++h)
 #pragma unroll
@@ -414,10 +405,12 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
         return true;
     }
     const bool row_ok = r < it.rows;
-    for (int c0 = 0; c0 < it.cols; c0 += 16) {
-        tmem_ld16(taddr + c0, a);
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        const int c0 = cbase + 16 * q;
+        tmem_ld16(taddr + 16 * q, a);
         tile_values16(tile, n_base, r, c0, a, v);
-        if (!row_ok) continue;
+        if (!row_ok || c0 >= it.cols) continue;
         float4* o = reinterpret_cast<float4*>(reinterpret_cast<float*>(it.out) + (int64_t)(it.row0 + r) * it.out_ld + it.col0 + c0);
 #pragma unroll
         for (int u = 0; u < 4; ++u) o[u] = make_float4(v[4 * u], v[4 * u + 1], v[4 * u + 2], v[4 * u + 3]);
@@ -428,36 +421,43 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
 // ---- the kernel ------------------------------------------------------------------------------------------
 // Persistent: CTA b runs items b, b + gridDim.x, ...  The 224 KB of data shared memory is split at launch into
 // `n_stages` operand ring stages (32 KB) and 2 x `n_base` streamed base tiles (32 KB; double-buffered like the
-// TMEM accumulators).  `err` is set (and the kernel drains) if a barrier wait times out, so a pipeline bug
-// cannot hang the GPU.
+// TMEM accumulators).  The producer warp copies each item descriptor into a 4-slot shared-memory ring one item
+// ahead, so no role waits on a global load.  `err` is set (and the kernel drains) if a barrier wait times out,
+// so a pipeline bug cannot hang the GPU.
 __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __restrict__ items, int n_items,
                                                               const CUtensorMap* __restrict__ maps, int* err,
-                                                              int n_stages, int n_base) {
+                                                              int n_stages, int n_base, int n_bslots, int dbg,
+                                                              long long* __restrict__ prof) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;          // 1024-byte aligned (swizzle atoms)
     const uint32_t base0 = smem0 + (uint32_t)n_stages * STAGE_BYTES;        // base tiles: [acc][n_base] x 32 KB
-    const uint32_t bars = smem0 + DATA_BYTES;      // full[7] empty[7] tfull[2] tempty[2] bfull[2] bempty[2]
+    const uint32_t bars = smem0 + DATA_BYTES;
     uint8_t* gen0 = smem_raw + (smem0 - smem_u32(smem_raw));
-    uint32_t* s_tmem = reinterpret_cast<uint32_t*>(gen0 + DATA_BYTES + 192);
+    uint32_t* s_tmem = reinterpret_cast<uint32_t*>(gen0 + DATA_BYTES + 288);
     uint32_t* s_red = s_tmem + 4;
+    uint8_t* s_items = gen0 + DATA_BYTES + 352;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     auto full_bar = [&](int s) { return bars + 8u * s; };
     auto empty_bar = [&](int s) { return bars + 8u * (MAX_STAGES + s); };
     auto tfull_bar = [&](int a) { return bars + 8u * (2 * MAX_STAGES + a); };
     auto tempty_bar = [&](int a) { return bars + 8u * (2 * MAX_STAGES + 2 + a); };
     auto bfull_bar = [&](int a) { return bars + 8u * (2 * MAX_STAGES + 4 + a); };
-    auto bempty_bar = [&](int a) { return bars + 8u * (2 * MAX_STAGES + 6 + a); };
-    auto base_tile = [&](uint32_t a) { return base0 + a * (uint32_t)n_base * TILE_BYTES; };
+    auto bempty_bar = [&](int a) { return bars + 8u * (2 * MAX_STAGES + 4 + MAX_BASE_SLOTS + a); };
+    auto ifull_bar = [&](int s) { return bars + 8u * (2 * MAX_STAGES + 4 + 2 * MAX_BASE_SLOTS + s); };
+    auto iempty_bar = [&](int s) { return bars + 8u * (2 * MAX_STAGES + 4 + 2 * MAX_BASE_SLOTS + ITEM_SLOTS + s); };
+    auto base_tile = [&](uint32_t b) { return base0 + b * (uint32_t)n_base * TILE_BYTES; };
+    auto item_slot = [&](uint32_t s) { return reinterpret_cast<const Item*>(s_items + s * ITEM_BYTES); };
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < MAX_STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
         for (int a = 0; a < 2; ++a) {
-            mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), 4);
-            mbar_init(bfull_bar(a), 1); mbar_init(bempty_bar(a), 1);
+            mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), EPI_WARPS);
         }
+        for (int b = 0; b < MAX_BASE_SLOTS; ++b) { mbar_init(bfull_bar(b), 1); mbar_init(bempty_bar(b), 1); }
+        for (int s = 0; s < ITEM_SLOTS; ++s) { mbar_init(ifull_bar(s), 1); mbar_init(iempty_bar(s), EPI_WARPS + 1); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (warp == 5) {
+    if (warp == MMA_WARP) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(s_tmem)), "r"(TMEM_COLS)
                      : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
@@ -467,87 +467,108 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
     tc_fence_after();
     const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(s_tmem);
 
-    if (warp == 4) {
-        // ===== TMA producer (one lane) =====
-        if (lane == 0) {
-            uint32_t stage = 0, phase = 0, n_done = 0;
-            bool ok = true;
-            for (int i = blockIdx.x; i < n_items && ok; i += gridDim.x, ++n_done) {
-                const Item& it = items[i];
+    // optional profile (prof != nullptr): cycles each role spends in each kind of wait, per CTA
+    long long pw[6] = {0, 0, 0, 0, 0, 0};
+    const long long t_start = clock64();
+#define TWAIT(slot, expr) ([&]() { const long long _t0 = prof ? clock64() : 0; const bool _r = (expr); if (prof) pw[slot] += clock64() - _t0; return _r; })()
+    if (warp == PRODUCER_WARP) {
+        // ===== item fetch (whole warp) + TMA producer (lane 0) =====
+        constexpr int NCHUNK = ITEM_BYTES / 16;
+        uint32_t stage = 0, phase = 0, n_done = 0;
+        int ok = 1;
+        uint4 nxt = make_uint4(0, 0, 0, 0);
+        if ((int)blockIdx.x < n_items && lane < NCHUNK) nxt = __ldg(reinterpret_cast<const uint4*>(items + blockIdx.x) + lane);
+        for (int i = blockIdx.x; i < n_items && ok; i += gridDim.x, ++n_done) {
+            const uint32_t slot = n_done % ITEM_SLOTS, iphase = (n_done / ITEM_SLOTS) & 1u;
+            if (lane == 0) ok = TWAIT(0, mbar_wait(iempty_bar(slot), iphase ^ 1u, err)) ? 1 : 0;
+            ok = __shfl_sync(0xFFFFFFFFu, ok, 0);
+            if (!ok) break;
+            if (lane < NCHUNK) reinterpret_cast<uint4*>(s_items + slot * ITEM_BYTES)[lane] = nxt;
+            __syncwarp();
+            if (lane == 0) mbar_arrive(ifull_bar(slot));
+            if (i + (int)gridDim.x < n_items && lane < NCHUNK)
+                nxt = __ldg(reinterpret_cast<const uint4*>(items + i + gridDim.x) + lane);
+            if (lane == 0) {
+                const Item& it = *item_slot(slot);
                 if (n_base > 0) {
                     // the item's base tile(s): hi [+ lo], each 2 halves x 2 row groups of 64 x 64 boxes
-                    const uint32_t acc = n_done & 1u, aphase = (n_done >> 1) & 1u;
-                    if (!(ok = mbar_wait(bempty_bar(acc), aphase ^ 1u, err))) break;
-                    int nb = 0;
-                    for (int b = 0; b < 2; ++b) nb += (it.base_map[b] >= 0) ? 1 : 0;
-                    if (nb == 0) mbar_arrive(bfull_bar(acc));
-                    else {
-                        mbar_expect_tx(bfull_bar(acc), (uint32_t)nb * TILE_BYTES);
-                        for (int b = 0; b < nb; ++b) {
-                            const CUtensorMap* mp = maps + it.base_map[b];
-                            tmap_acquire(mp);
-                            const uint32_t dst = base_tile(acc) + (uint32_t)b * TILE_BYTES;
+                    const uint32_t acc = n_done % (uint32_t)n_bslots, aphase = (n_done / (uint32_t)n_bslots) & 1u;
+                    ok = TWAIT(1, mbar_wait(bempty_bar(acc), aphase ^ 1u, err)) ? 1 : 0;
+                    if (ok) {
+                        int nb = 0;
+                        for (int b = 0; b < 2; ++b) nb += (it.base_map[b] >= 0) ? 1 : 0;
+                        if (nb == 0) mbar_arrive(bfull_bar(acc));
+                        else {
+                            mbar_expect_tx(bfull_bar(acc), (uint32_t)nb * TILE_BYTES);
+                            for (int b = 0; b < nb; ++b) {
+                                const CUtensorMap* mp = maps + it.base_map[b];
+                                if (!(dbg & 2)) tmap_acquire(mp);
+                                const uint32_t dst = base_tile(acc) + (uint32_t)b * TILE_BYTES;
 #pragma unroll
-                            for (int h = 0; h < 2; ++h)
+                                for (int h = 0; h < 2; ++h)
 #pragma unroll
-                                for (int g = 0; g < 2; ++g)
-                                    tma_load_2d(dst + h * 16384u + g * 8192u, mp, it.col0 + 64 * h, it.row0 + 64 * g,
-                                                bfull_bar(acc));
+                                    for (int g = 0; g < 2; ++g)
+                                        tma_load_2d(dst + h * 16384u + g * 8192u, mp, it.col0 + 64 * h, it.row0 + 64 * g,
+                                                    bfull_bar(acc));
+                            }
                         }
                     }
                 }
-                const int nbx = it.N >> 6;
+                const int nbx = it.N >> 6, a_mn = it.a_mn;
                 const uint32_t tx = A_BYTES + (uint32_t)it.N * 128u;
                 for (int seg = 0; seg < NSEG && ok; ++seg) {
                     const int na = it.atoms[seg];
                     if (na <= 0) continue;
                     const CUtensorMap* ma = maps + it.map_a[seg];
                     const CUtensorMap* mb = maps + it.map_b[seg];
-                    tmap_acquire(ma);
-                    tmap_acquire(mb);
+                    if (!(dbg & 2)) { tmap_acquire(ma); tmap_acquire(mb); }
+                    const int ac = it.a_c0[seg], ar = it.a_r0[seg], bc = it.b_c0[seg], br = it.b_r0[seg];
                     for (int t = 0; t < na; ++t) {
-                        if (!(ok = mbar_wait(empty_bar(stage), phase ^ 1u, err))) break;
+                        if (!TWAIT(2, mbar_wait(empty_bar(stage), phase ^ 1u, err))) { ok = 0; break; }
                         const uint32_t sa = smem0 + stage * STAGE_BYTES, sb = sa + A_BYTES;
                         mbar_expect_tx(full_bar(stage), tx);
-                        if (it.a_mn) {
-                            tma_load_2d(sa, ma, it.a_c0[seg], it.a_r0[seg] + 64 * t, full_bar(stage));
-                            tma_load_2d(sa + 8192, ma, it.a_c0[seg] + 64, it.a_r0[seg] + 64 * t, full_bar(stage));
+                        if (a_mn) {
+                            tma_load_2d(sa, ma, ac, ar + 64 * t, full_bar(stage));
+                            tma_load_2d(sa + 8192, ma, ac + 64, ar + 64 * t, full_bar(stage));
                         } else {
-                            tma_load_2d(sa, ma, it.a_c0[seg] + 64 * t, it.a_r0[seg], full_bar(stage));
-                            tma_load_2d(sa + 8192, ma, it.a_c0[seg] + 64 * t, it.a_r0[seg] + 64, full_bar(stage));
+                            tma_load_2d(sa, ma, ac + 64 * t, ar, full_bar(stage));
+                            tma_load_2d(sa + 8192, ma, ac + 64 * t, ar + 64, full_bar(stage));
                         }
-                        for (int b = 0; b < nbx; ++b)
-                            tma_load_2d(sb + 8192 * b, mb, it.b_c0[seg] + 64 * t, it.b_r0[seg] + 64 * b, full_bar(stage));
+                        for (int b = 0; b < nbx; ++b) tma_load_2d(sb + 8192 * b, mb, bc + 64 * t, br + 64 * b, full_bar(stage));
                         if (++stage == (uint32_t)n_stages) { stage = 0; phase ^= 1u; }
                     }
                 }
             }
+            ok = __shfl_sync(0xFFFFFFFFu, ok, 0);
         }
-    } else if (warp == 5) {
+    } else if (warp == MMA_WARP) {
         // ===== MMA issuer (one lane) =====
         if (lane == 0) {
             uint32_t stage = 0, phase = 0, n_done = 0;
             bool ok = true;
             for (int i = blockIdx.x; i < n_items && ok; i += gridDim.x, ++n_done) {
-                const Item& it = items[i];
-                const uint32_t acc = n_done & 1u, aphase = (n_done >> 1) & 1u;
-                if (!(ok = mbar_wait(tempty_bar(acc), aphase ^ 1u, err))) break;
-                tc_fence_after();
-                const uint32_t d = tmem_base + acc * 128u;
-                const uint32_t idesc = instr_desc(it.N, it.a_mn);
+                const uint32_t slot = n_done % ITEM_SLOTS, iphase = (n_done / ITEM_SLOTS) & 1u;
+                if (!(ok = TWAIT(0, mbar_wait(ifull_bar(slot), iphase, err)))) break;
+                const Item& it = *item_slot(slot);
+                const int a_mn = it.a_mn;
+                const uint32_t idesc = instr_desc(it.N, a_mn);
                 int total = 0;
 #pragma unroll
                 for (int seg = 0; seg < NSEG; ++seg) total += it.atoms[seg];
+                mbar_arrive(iempty_bar(slot));
+                const uint32_t acc = n_done & 1u, aphase = (n_done >> 1) & 1u;
+                if (!(ok = TWAIT(1, mbar_wait(tempty_bar(acc), aphase ^ 1u, err)))) break;
+                tc_fence_after();
+                const uint32_t d = tmem_base + acc * 128u;
                 for (int t = 0; t < total; ++t) {
-                    if (!(ok = mbar_wait(full_bar(stage), phase, err))) break;
+                    if (!(ok = TWAIT(2, mbar_wait(full_bar(stage), phase, err)))) break;
                     tc_fence_after();
                     const uint32_t sa = smem0 + stage * STAGE_BYTES, sb = sa + A_BYTES;
 #pragma unroll
                     for (int kk = 0; kk < 4; ++kk) {
-                        const uint64_t da = it.a_mn ? smem_desc(sa + 2048u * kk, 8192u, 1024u)
-                                                    : smem_desc(sa + 32u * kk, 16u, 1024u);
+                        const uint64_t da = a_mn ? smem_desc(sa + 2048u * kk, 8192u, 1024u) : smem_desc(sa + 32u * kk, 16u, 1024u);
                         const uint64_t db = smem_desc(sb + 32u * kk, 16u, 1024u);
-                        tc_mma_bf16(d, da, db, idesc, (t | kk) ? 1u : 0u);
+                        if (!(dbg & 1)) tc_mma_bf16(d, da, db, idesc, (t | kk) ? 1u : 0u);
                     }
                     tc_commit(empty_bar(stage));          // frees the smem stage when these MMAs retire
                     if (++stage == (uint32_t)n_stages) { stage = 0; phase ^= 1u; }
@@ -556,37 +577,51 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
             }
         }
     } else {
-        // ===== epilogue warps 0..3 =====
+        // ===== epilogue warps 0..7 =====
         uint32_t n_done = 0;
         bool ok = true;
         for (int i = blockIdx.x; i < n_items && ok; i += gridDim.x, ++n_done) {
-            const Item it = items[i];
+            const uint32_t slot = n_done % ITEM_SLOTS, iphase = (n_done / ITEM_SLOTS) & 1u;
             const uint32_t acc = n_done & 1u, aphase = (n_done >> 1) & 1u;
-            if (n_base > 0) ok = mbar_wait(bfull_bar(acc), aphase, err);
-            ok = ok && mbar_wait(tfull_bar(acc), aphase, err);
+            const uint32_t bs = n_base > 0 ? n_done % (uint32_t)n_bslots : 0u, bphase = n_base > 0 ? (n_done / (uint32_t)n_bslots) & 1u : 0u;
+            ok = TWAIT(0, mbar_wait(ifull_bar(slot), iphase, err));
+            if (ok && n_base > 0) ok = TWAIT(1, mbar_wait(bfull_bar(bs), bphase, err));
+            ok = ok && TWAIT(2, mbar_wait(tfull_bar(acc), aphase, err));
+            const long long t_e0 = prof ? clock64() : 0;
             ok = __all_sync(0xFFFFFFFFu, ok);
             if (!ok) break;
             tc_fence_after();
+            const Item& it = *item_slot(slot);
             bool stored = false;
-            if (it.base_map[0] >= 0) stored = epilogue_tile(it, tmem_base + acc * 128u, base_tile(acc), it.base_map[1] >= 0 ? 2 : 1,
-                                                            warp, lane, s_red, maps);
-            else epilogue(it, tmem_base + acc * 128u, warp, lane, s_red);
+            if (it.base_map[0] >= 0)
+                stored = epilogue_tile(it, tmem_base + acc * 128u, base_tile(bs), it.base_map[1] >= 0 ? 2 : 1, warp, lane, s_red, maps);
+            else
+                epilogue(it, tmem_base + acc * 128u, warp, lane, s_red);
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(tempty_bar(acc));
+            if (prof) pw[3] += clock64() - t_e0;
+            const long long t_p0 = prof ? clock64() : 0;
+            if (lane == 0) { mbar_arrive(tempty_bar(acc)); mbar_arrive(iempty_bar(slot)); }
             if (n_base > 0) {
-                asm volatile("bar.sync 1, 128;" ::: "memory");          // every epilogue thread is done with the tile
+                epi_sync();                                   // every epilogue thread is done with the tile
                 if (threadIdx.x == 0) {
                     if (stored) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-                    mbar_arrive(bempty_bar(acc));
+                    mbar_arrive(bempty_bar(bs));
                 }
             }
+            if (prof) pw[4] += clock64() - t_p0;
         }
         if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     }
+#undef TWAIT
+    if (prof && lane == 0 && (warp == 0 || warp == PRODUCER_WARP || warp == MMA_WARP)) {
+        const int role = warp == 0 ? 0 : (warp == PRODUCER_WARP ? 1 : 2);
+        pw[5] = clock64() - t_start;
+        for (int q = 0; q < 6; ++q) prof[((size_t)blockIdx.x * 3 + role) * 6 + q] = pw[q];
+    }
     tc_fence_before();
     __syncthreads();
-    if (warp == 5) {
+    if (warp == MMA_WARP) {
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
     }
