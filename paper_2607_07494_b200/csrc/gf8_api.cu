@@ -313,8 +313,8 @@ gf8_status fast_encode_many(gf8_ctx* c, int n, const int* layers, const void* co
             if ((s = fast_slot(c, L, occurrence[layers[i]]++, dt == GF8_DT_F32, false, false, &slot)) != GF8_OK) break;
             int src_map;
             if (dt == GF8_DT_BF16) {
-                CUtensorMap mp;
-                if ((s = make_map(c, &mp, grads[i], m, nn, nn)) != GF8_OK) break;
+                CUtensorMap mp[2];
+                if ((s = make_map(c, mp, grads[i], m, nn, nn)) != GF8_OK) break;
                 src_map = pb.add_map(grads[i], mp);
             } else {
                 p->converts.push_back({(const float*)grads[i], slot->src16, (int64_t)m * nn});
@@ -335,7 +335,7 @@ gf8_status fast_encode_many(gf8_ctx* c, int n, const int* layers, const void* co
                 if (dt == GF8_DT_BF16) {
                     CUtensorMap mc;
                     if ((s = make_map_u8(c, &mc, codes[i], m, nn)) != GF8_OK) break;
-                    f.out_map = pb.add_map(codes[i], mc);
+                    f.out_map = pb.add_single(codes[i], mc);
                 }
             }
             add_transform(pb, L, slot, src_map, -1, false, false, f);
@@ -407,9 +407,9 @@ gf8_status fast_reduce_decoded_many(gf8_ctx* c, int n, const int* layers, const 
             f.out_map = -1;
             if (dt == GF8_DT_BF16) {
                 const LayerState& Lc = L;
-                CUtensorMap mo;
-                if ((s = make_map(c, &mo, outs[i], Lc.desc.d_out, Lc.desc.d_in, Lc.desc.d_in)) != GF8_OK) break;
-                f.out_map = pb.add_map(outs[i], mo);
+                CUtensorMap mo[2];
+                if ((s = make_map(c, mo, outs[i], Lc.desc.d_out, Lc.desc.d_in, Lc.desc.d_in)) != GF8_OK) break;
+                f.out_map = pb.add_map(outs[i], mo) + 1;           // 128-row boxes
             }
             // the unwhitening multipliers ebar = 1/D - 1 amplify operand rounding, so decode runs split products
             add_transform(pb, L, slot, src_map, src_lo_map, true, true, f);

@@ -30,7 +30,8 @@ struct SideState {
     gf8::bf16* U16 = nullptr;  // d x kp   (zero-padded columns)
     gf8::bf16* Ut16 = nullptr; // kp x d
     gf8::bf16 *U16_lo = nullptr, *Ut16_lo = nullptr;   // BF16 residuals U - bf16(U) (split-operand products)
-    CUtensorMap map_U16, map_Ut16, map_U16_lo, map_Ut16_lo;
+    // every TMA map exists for 64-row boxes [0] and 128-row boxes [1] (64 columns = one 128 B swizzle span)
+    CUtensorMap map_U16[2], map_Ut16[2], map_U16_lo[2], map_Ut16_lo[2];
 };
 
 // Per (layer, occurrence-in-batch) scratch of the FAST path; buffers and their TMA maps are static.
@@ -40,11 +41,11 @@ struct Slot {
     gf8::bf16* Qpt = nullptr;  // n x kpG   Q'^T
     gf8::bf16* SEA = nullptr;  // kpG x kpA S E_A
     gf8::bf16 *Pp_lo = nullptr, *Qpt_lo = nullptr, *SEA_lo = nullptr;   // residuals, lazy (split products)
-    CUtensorMap map_Pp, map_Qpt, map_SEA, map_Pp_lo, map_Qpt_lo, map_SEA_lo;
+    CUtensorMap map_Pp[2], map_Qpt[2], map_SEA[2], map_Pp_lo[2], map_Qpt_lo[2], map_SEA_lo[2];
     float* Uhat = nullptr;     // m x n FP32 reduced payload (decode), lazy
     gf8::bf16* src16 = nullptr;// m x n BF16 copy of an FP32 source (decode, FP32 gradients), lazy
     gf8::bf16* src16_lo = nullptr;
-    CUtensorMap map_src16, map_src16_lo;
+    CUtensorMap map_src16[2], map_src16_lo[2];
 };
 
 struct LayerState {

@@ -14,6 +14,7 @@ struct Plan {
     gf8::tc::Item* d_items = nullptr;
     int stage_off[6] = {0, 0, 0, 0, 0, 0}, stage_cnt[6] = {0, 0, 0, 0, 0, 0};
     int stage_base[6] = {0, 0, 0, 0, 0, 0};  // streamed base tiles per item in that stage's launch (0, 1 or 2)
+    int runs = 0;                        // launches so far: the first one acquires its tensor maps with proxy fences
     uint32_t* d_amax = nullptr;          // one word per TC problem (per-tensor scaling)
     size_t n_amax = 0;
     struct Convert { const float* src; gf8::bf16* dst; int64_t numel; };
@@ -54,10 +55,10 @@ gf8_status fast_init(gf8_ctx* c) {
 
 // BF16 row-major matrix [rows][cols] (leading dimension ld elements) -> TMA map, 64 x 64 boxes, 128 B swizzle,
 // out-of-bounds elements read as zero.
-gf8_status make_map(gf8_ctx* c, CUtensorMap* out, const void* ptr, uint64_t rows, uint64_t cols, uint64_t ld) {
+gf8_status make_map1(gf8_ctx* c, CUtensorMap* out, const void* ptr, uint64_t rows, uint64_t cols, uint64_t ld, uint32_t box_rows) {
     const cuuint64_t gdim[2] = {cols, rows};
     const cuuint64_t gstride[1] = {ld * 2};
-    const cuuint32_t box[2] = {64, 64};
+    const cuuint32_t box[2] = {64, box_rows};
     const cuuint32_t estr[2] = {1, 1};
     const CUresult r = ((EncodeTiledFn)c->encode_tiled)(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), gdim,
                                                         gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
@@ -66,6 +67,12 @@ gf8_status make_map(gf8_ctx* c, CUtensorMap* out, const void* ptr, uint64_t rows
     if (r != CUDA_SUCCESS) return fail(c, GF8_ERR_CUDA, "cuTensorMapEncodeTiled failed (%d) for %llu x %llu", (int)r,
                                        (unsigned long long)rows, (unsigned long long)cols);
     return GF8_OK;
+}
+
+// Both box heights of a BF16 matrix: out[0] = 64-row boxes, out[1] = 128-row boxes.
+gf8_status make_map(gf8_ctx* c, CUtensorMap* out, const void* ptr, uint64_t rows, uint64_t cols, uint64_t ld) {
+    GF_TRY(make_map1(c, &out[0], ptr, rows, cols, ld, 64));
+    return make_map1(c, &out[1], ptr, rows, cols, ld, 128);
 }
 
 // FP8 code matrix [rows][cols] bytes -> TMA store map, 128 x 128 boxes (one update tile), 128 B swizzle.
@@ -118,12 +125,12 @@ gf8_status fast_init_layer(gf8_ctx* c, LayerState& L) {
         if (!s->used) continue;
         GF_TRY(dmalloc(c, &s->U16, (size_t)s->d * s->kp));
         GF_TRY(dmalloc(c, &s->Ut16, (size_t)s->kp * s->d));
-        GF_TRY(make_map(c, &s->map_U16, s->U16, s->d, s->kp, s->kp));
-        GF_TRY(make_map(c, &s->map_Ut16, s->Ut16, s->kp, s->d, s->d));
+        GF_TRY(make_map(c, s->map_U16, s->U16, s->d, s->kp, s->kp));
+        GF_TRY(make_map(c, s->map_Ut16, s->Ut16, s->kp, s->d, s->d));
         GF_TRY(dmalloc(c, &s->U16_lo, (size_t)s->d * s->kp));
         GF_TRY(dmalloc(c, &s->Ut16_lo, (size_t)s->kp * s->d));
-        GF_TRY(make_map(c, &s->map_U16_lo, s->U16_lo, s->d, s->kp, s->kp));
-        GF_TRY(make_map(c, &s->map_Ut16_lo, s->Ut16_lo, s->kp, s->d, s->d));
+        GF_TRY(make_map(c, s->map_U16_lo, s->U16_lo, s->d, s->kp, s->kp));
+        GF_TRY(make_map(c, s->map_Ut16_lo, s->Ut16_lo, s->kp, s->d, s->d));
     }
     L.tc_ok = true;
     return GF8_OK;
@@ -140,38 +147,38 @@ gf8_status fast_slot(gf8_ctx* c, LayerState& L, size_t idx, bool need_src16, boo
         L.slots[idx] = s;
         if (kpA) {
             GF_TRY(dmalloc(c, &s->Pp, m * kpA));
-            GF_TRY(make_map(c, &s->map_Pp, s->Pp, m, kpA, kpA));
+            GF_TRY(make_map(c, s->map_Pp, s->Pp, m, kpA, kpA));
         }
         if (kpG) {
             GF_TRY(dmalloc(c, &s->Qt, n * kpG));
             GF_TRY(dmalloc(c, &s->Qpt, n * kpG));
-            GF_TRY(make_map(c, &s->map_Qpt, s->Qpt, n, kpG, kpG));
+            GF_TRY(make_map(c, s->map_Qpt, s->Qpt, n, kpG, kpG));
         }
         if (kpA && kpG) {
             GF_TRY(dmalloc(c, &s->SEA, kpG * kpA));
-            GF_TRY(make_map(c, &s->map_SEA, s->SEA, kpG, kpA, kpA));
+            GF_TRY(make_map(c, s->map_SEA, s->SEA, kpG, kpA, kpA));
         }
     }
     Slot* s = L.slots[idx];
     if (need_src16 && !s->src16) {
         GF_TRY(dmalloc(c, &s->src16, m * n));
-        GF_TRY(make_map(c, &s->map_src16, s->src16, m, n, n));
+        GF_TRY(make_map(c, s->map_src16, s->src16, m, n, n));
     }
     if (need_uhat && !s->Uhat) GF_TRY(dmalloc(c, &s->Uhat, m * n));
     if (need_split && !s->src16_lo) {
         GF_TRY(dmalloc(c, &s->src16_lo, m * n));
-        GF_TRY(make_map(c, &s->map_src16_lo, s->src16_lo, m, n, n));
+        GF_TRY(make_map(c, s->map_src16_lo, s->src16_lo, m, n, n));
         if (kpA) {
             GF_TRY(dmalloc(c, &s->Pp_lo, m * kpA));
-            GF_TRY(make_map(c, &s->map_Pp_lo, s->Pp_lo, m, kpA, kpA));
+            GF_TRY(make_map(c, s->map_Pp_lo, s->Pp_lo, m, kpA, kpA));
         }
         if (kpG) {
             GF_TRY(dmalloc(c, &s->Qpt_lo, n * kpG));
-            GF_TRY(make_map(c, &s->map_Qpt_lo, s->Qpt_lo, n, kpG, kpG));
+            GF_TRY(make_map(c, s->map_Qpt_lo, s->Qpt_lo, n, kpG, kpG));
         }
         if (kpA && kpG) {
             GF_TRY(dmalloc(c, &s->SEA_lo, kpG * kpA));
-            GF_TRY(make_map(c, &s->map_SEA_lo, s->SEA_lo, kpG, kpA, kpA));
+            GF_TRY(make_map(c, s->map_SEA_lo, s->SEA_lo, kpG, kpA, kpA));
         }
     }
     *out = s;
@@ -184,7 +191,16 @@ struct PlanBuilder {
     std::vector<CUtensorMap> maps;
     std::map<const void*, int> map_index;      // buffer -> index (static maps are shared by all problems)
     std::vector<Item> stage[6];
-    int add_map(const void* key, const CUtensorMap& m) {
+    // registers both box heights of a buffer; returns the index of the 64-row-box map, +1 is the 128-row-box map
+    int add_map(const void* key, const CUtensorMap* m2) {
+        auto it = map_index.find(key);
+        if (it != map_index.end()) return it->second;
+        maps.push_back(m2[0]);
+        maps.push_back(m2[1]);
+        map_index[key] = (int)maps.size() - 2;
+        return (int)maps.size() - 2;
+    }
+    int add_single(const void* key, const CUtensorMap& m) {
         auto it = map_index.find(key);
         if (it != map_index.end()) return it->second;
         maps.push_back(m);
@@ -223,7 +239,7 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
     const float* eA = inverse ? L.in.ebar : L.in.e;
     const float* eG = inverse ? L.out.ebar : L.out.e;
     struct MapPair { int hi, lo; };
-    auto pair = [&](bool use, const void* bh, const CUtensorMap& mh, const void* bl, const CUtensorMap& ml) {
+    auto pair = [&](bool use, const void* bh, const CUtensorMap* mh, const void* bl, const CUtensorMap* ml) {
         MapPair r{-1, -1};
         if (use) { r.hi = pb.add_map(bh, mh); if (split) r.lo = pb.add_map(bl, ml); }
         return r;
@@ -237,9 +253,12 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
     const MapPair mSEA = pair(useA && useG, s->SEA, s->map_SEA, s->SEA_lo, s->map_SEA_lo);
     const MapPair mSrc{src_map, src_lo_map};
     // append the product A * B^T (hi*hi [+ lo*hi + hi*lo]) to an item
+    // (map indices point at the 64-row-box map of a buffer; +1 is its 128-row-box map: a K-major A atom and a
+    //  128-row B atom are one box each, an MN-major A atom is two 64 x 64 boxes)
     auto add_product = [&](Item& it, int& seg, MapPair a, MapPair b, int atoms, int a_c0, int a_r0, int b_c0, int b_r0) {
+        const int ao = it.a_mn ? 0 : 1, bo = it.N == 128 ? 1 : 0;
         auto one = [&](int ma, int mb) {
-            it.map_a[seg] = ma; it.map_b[seg] = mb; it.atoms[seg] = atoms;
+            it.map_a[seg] = ma + ao; it.map_b[seg] = mb + bo; it.atoms[seg] = atoms;
             it.a_c0[seg] = a_c0; it.a_r0[seg] = a_r0; it.b_c0[seg] = b_c0; it.b_r0[seg] = b_r0;
             ++seg;
         };
@@ -253,8 +272,8 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
             for (int nc = 0; nc < kpA; nc += 128) {
                 Item it = blank_item();
                 int seg = 0;
-                add_product(it, seg, mSrc, mUAt, (n + 63) / 64, 0, i0, 0, nc);
                 it.N = std::min(128, kpA - nc);
+                add_product(it, seg, mSrc, mUAt, (n + 63) / 64, 0, i0, 0, nc);
                 it.mode = EPI_STORE; it.out = s->Pp; it.out_lo = split ? s->Pp_lo : nullptr; it.out_ld = kpA;
                 it.out_type = TY_BF16; it.colscale = eA + nc;
                 it.row0 = i0; it.col0 = nc; it.rows = std::min(128, m - i0); it.cols = it.N;
@@ -265,8 +284,8 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
             for (int nc = 0; nc < kpG; nc += 128) {
                 Item it = blank_item();
                 int seg = 0;
-                add_product(it, seg, mSrc, mUGt, (m + 63) / 64, j0, 0, 0, nc);
                 it.a_mn = 1; it.N = std::min(128, kpG - nc);
+                add_product(it, seg, mSrc, mUGt, (m + 63) / 64, j0, 0, 0, nc);
                 it.mode = EPI_STORE; it.row0 = j0; it.col0 = nc; it.rows = std::min(128, n - j0); it.cols = it.N;
                 if (useA) { it.out = s->Qt; it.out_ld = kpG; it.out_type = TY_F32; }
                 else {
@@ -281,8 +300,8 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
                 for (int nc = 0; nc < kpG; nc += 128) {
                     Item it = blank_item();
                     int seg = 0;
-                    add_product(it, seg, mPp, mUGt, (m + 63) / 64, a0, 0, 0, nc);
                     it.a_mn = 1; it.N = std::min(128, kpG - nc);
+                    add_product(it, seg, mPp, mUGt, (m + 63) / 64, a0, 0, 0, nc);
                     it.mode = EPI_STORE_T; it.out = s->SEA; it.out_lo = split ? s->SEA_lo : nullptr; it.out_ld = kpA;
                     it.out_type = TY_BF16;
                     it.row0 = a0; it.col0 = nc; it.rows = std::min(128, kpA - a0); it.cols = it.N;
@@ -293,8 +312,8 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
                 for (int nc = 0; nc < kpG; nc += 128) {
                     Item it = blank_item();
                     int seg = 0;
-                    add_product(it, seg, mUA, mSEA, kpA / 64, 0, j0, 0, nc);
                     it.N = std::min(128, kpG - nc);
+                    add_product(it, seg, mUA, mSEA, kpA / 64, 0, j0, 0, nc);
                     it.mode = EPI_STORE; it.base = s->Qt; it.base_ld = kpG; it.base_type = TY_F32;
                     it.out = s->Qpt; it.out_lo = split ? s->Qpt_lo : nullptr; it.out_ld = kpG; it.out_type = TY_BF16;
                     it.colscale = eG + nc;
@@ -309,13 +328,14 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
         for (int j0 = 0; j0 < n; j0 += 128) {
             Item it = blank_item();
             int seg = 0;
+            it.N = 128; it.fmt = f.fmt;
             if (useA) add_product(it, seg, mPp, mUA, kpA / 64, 0, i0, 0, j0);
             if (useG) add_product(it, seg, mUG, mQpt, kpG / 64, 0, i0, 0, j0);
-            it.N = 128; it.fmt = f.fmt;
             it.base = f.base; it.base_ld = n; it.base_type = f.base_type;
             it.row0 = i0; it.col0 = j0; it.rows = std::min(128, m - i0); it.cols = std::min(128, n - j0);
             it.mode = f.mode;
-            it.base_map[0] = f.base_map[0]; it.base_map[1] = f.base_map[1];
+            it.base_map[0] = f.base_map[0] >= 0 ? f.base_map[0] + 1 : -1;      // 128-row boxes
+            it.base_map[1] = f.base_map[1] >= 0 ? f.base_map[1] + 1 : -1;
             if (f.mode == EPI_AMAX) {
                 it.amax = f.amax;
                 pb.stage[3].push_back(it);
@@ -381,7 +401,8 @@ gf8_status plan_store(gf8_ctx* c, const std::vector<uint64_t>& key, Plan* p) {
     return GF8_OK;
 }
 
-gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, const Plan* p) {
+gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
+    const bool first_run = p->runs++ == 0;
     for (int s = 0; s < 6; ++s) {
         if (!p->stage_cnt[s]) continue;
         const int grid = std::min(p->stage_cnt[s], c->num_sms);
@@ -391,6 +412,7 @@ gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, const Plan* p) {
         int n_stages = n_base ? 3 : gf8::tc::MAX_STAGES, dbg = 0, only = -1;
         const int n_bslots = n_base ? (gf8::tc::MAX_STAGES - n_stages) / n_base : 1;
         if (const char* e = getenv("GF8_TC_DBG")) dbg = atoi(e);
+        if (!first_run) dbg |= 2;        // tensor maps are written once by the host before the plan's first launch
         if (const char* e = getenv("GF8_TC_ONLY")) only = atoi(e);
         if (only >= 0 && only != s) continue;
         gf8::tc::tc_items_kernel<<<grid, gf8::tc::THREADS, gf8::tc::SMEM_BYTES, st>>>(

@@ -16,8 +16,8 @@
 // TMEM so the epilogue of item i overlaps the MMAs of item i+1.  The streamed base tile of the rank-2k
 // update (the gradient itself: the HBM-bound traffic) is also fetched by TMA, double-buffered, and the
 // FP8 / BF16 output tile leaves through a TMA store, so every HBM access is a full-line bulk transfer.
-// Warps 0-7: epilogue (TMEM lane quarter = warp & 3, column half = warp >> 2), warp 8: item fetch + TMA
-// producer, warp 9: TMEM allocation + MMA issue.
+// Warps 0-7: epilogue (TMEM lane quarter = warp & 3, column half = warp >> 2), warp 8: item fetch + base-tile
+// TMA producer, warps 9 / 10: A / B operand TMA producers, warp 11: TMEM allocation + MMA issue.
 #pragma once
 #include <cuda.h>
 
@@ -34,8 +34,8 @@ constexpr int STAGE_BYTES = A_BYTES + B_BYTES;   // 32 KB
 constexpr int TILE_BYTES = 128 * 128 * 2;        // one streamed 128 x 128 BF16 base tile (two 64-column halves)
 constexpr int DATA_BYTES = MAX_STAGES * STAGE_BYTES;   // 224 KB, split at launch into ring stages + base tiles
 constexpr int SMEM_BYTES = DATA_BYTES + 1024 /*alignment slack*/ + 1536 /*barriers, item ring*/;
-constexpr int EPI_WARPS = 8, PRODUCER_WARP = 8, MMA_WARP = 9;
-constexpr int THREADS = 32 * (EPI_WARPS + 2);
+constexpr int EPI_WARPS = 8, PRODUCER_WARP = 8, OPERAND_WARP = 9, MMA_WARP = 11;
+constexpr int THREADS = 32 * (EPI_WARPS + 4);
 constexpr int ITEM_SLOTS = 4;                    // shared-memory ring of item descriptors
 constexpr int MAX_BASE_SLOTS = 4;                // streamed base tiles in flight (ring, decoupled from TMEM)
 constexpr int TMEM_COLS = 256;                   // two accumulators of up to 128 columns
@@ -130,6 +130,19 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t* v) {
         : "r"(taddr) : "memory");
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
+
+// 32 columns of this thread's TMEM lane; the caller waits (tmem_wait) before using v.
+__device__ __forceinline__ void tmem_ld32_nowait(uint32_t taddr, uint32_t* v) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,"
+        "%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+          "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+          "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // Shared-memory matrix descriptor (SWIZZLE_128B, version 1).  lbo / sbo in bytes.
 __device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo, uint32_t sbo) {
@@ -321,47 +334,73 @@ __device__ __forceinline__ void tile_values16(uint32_t tile, int n_base, int r, 
     for (int u = 0; u < 16; ++u) v[u] += __uint_as_float(a[u]);
 }
 
+// v[32] = base(hi [+ lo]) + accumulator for columns [32 g, 32 g + 32) of this warp's 64-column half: the TMEM
+// load and the shared-memory loads are all issued before the single wait.  `row` = this row's 128 B of the half.
+__device__ __forceinline__ void tile_values32(uint32_t taddr, uint32_t row, int n_base, int r, int g, float* v) {
+    uint32_t a[32];
+    tmem_ld32_nowait(taddr + 32u * g, a);
+    uint4 b[4];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) b[j] = lds128(row + (((uint32_t)(4 * g + j) ^ (uint32_t)(r & 7)) << 4));
+#pragma unroll
+    for (int j = 0; j < 4; ++j) unpack_bf16x8(b[j], v + 8 * j);
+    if (n_base > 1) {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) b[j] = lds128(row + TILE_BYTES + (((uint32_t)(4 * g + j) ^ (uint32_t)(r & 7)) << 4));
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            float w[8];
+            unpack_bf16x8(b[j], w);
+#pragma unroll
+            for (int u = 0; u < 8; ++u) v[8 * j + u] += w[u];
+        }
+    }
+    tmem_wait();
+#pragma unroll
+    for (int u = 0; u < 32; ++u) v[u] += __uint_as_float(a[u]);
+}
+
 // Returns true if a TMA store was issued from `tile` (the caller waits for its smem reads before reuse).
 // Each warp covers 32 rows x 64 columns (its half) as four 16-column chunks.
 __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc, uint32_t tile, int n_base, int warp,
-                                              int lane, uint32_t* s_red, const CUtensorMap* maps) {
+                                              int lane, uint32_t* s_red, const CUtensorMap* maps, uint32_t amax_bits) {
     const int r = (warp & 3) * 32 + lane, half = warp >> 2, cbase = half * 64;
     const uint32_t taddr = tmem_acc + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)cbase;
-    uint32_t a[16];
-    float v[16];
+    const uint32_t row = tile + (uint32_t)half * 16384u + (uint32_t)r * 128u;
+    const int mode = it.mode, fmt = it.fmt;
+    float v[32];
     float scale = 1.0f;
-    if (it.mode == EPI_BLOCKCAST || it.mode == EPI_AMAX) {
+    if (mode == EPI_BLOCKCAST || mode == EPI_AMAX) {
         uint32_t loc = 0;
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            tmem_ld16(taddr + 16 * q, a);
-            tile_values16(tile, n_base, r, cbase + 16 * q, a, v);
+        for (int g = 0; g < 2; ++g) {
+            tile_values32(taddr, row, n_base, r, g, v);
 #pragma unroll
-            for (int u = 0; u < 16; ++u) loc = max(loc, __float_as_uint(v[u]) & 0x7FFFFFFFu);
+            for (int u = 0; u < 32; ++u) loc = max(loc, __float_as_uint(v[u]) & 0x7FFFFFFFu);
         }
-        if (it.mode == EPI_AMAX) {
+        if (mode == EPI_AMAX) {
             loc = warp_max_u32(loc);
             if (lane == 0 && loc != 0u) atomicMax(it.amax, loc);
             return false;
         }
         const uint32_t bits = epi_block_max(loc, warp, lane, s_red);
         float si;
-        scales_from_amax(bits, it.fmt == 0 ? 448.0f : 57344.0f, scale, si);
+        scales_from_amax(bits, fmt == 0 ? 448.0f : 57344.0f, scale, si);
         if (r == 0 && half == 0) *it.scale_inv_out = si;
-    } else if (it.mode == EPI_CAST) {
+    } else if (mode == EPI_CAST) {
         float si;
-        scales_from_amax(*reinterpret_cast<volatile uint32_t*>(it.amax), it.fmt == 0 ? 448.0f : 57344.0f, scale, si);
+        scales_from_amax(amax_bits, fmt == 0 ? 448.0f : 57344.0f, scale, si);
         if (it.write_scale && r == 0 && half == 0) *it.scale_inv_out = si;
     }
-    if (it.mode == EPI_CAST || it.mode == EPI_BLOCKCAST) {
+    if (mode == EPI_CAST || mode == EPI_BLOCKCAST) {
         // 64 codes of this row half; the 128 x 128-byte code tile then overwrites the (consumed) first half of
         // the base tile in the store map's 128 B swizzle
         uint4 cd[4];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            tmem_ld16(taddr + 16 * q, a);
-            tile_values16(tile, n_base, r, cbase + 16 * q, a, v);
-            cd[q] = it.fmt == 0 ? codes16<0>(v, scale) : codes16<1>(v, scale);
+        for (int g = 0; g < 2; ++g) {
+            tile_values32(taddr, row, n_base, r, g, v);
+            cd[2 * g] = fmt == 0 ? codes16<0>(v, scale) : codes16<1>(v, scale);
+            cd[2 * g + 1] = fmt == 0 ? codes16<0>(v + 16, scale) : codes16<1>(v + 16, scale);
         }
         epi_sync();                               // every thread has read its base data
 #pragma unroll
@@ -378,42 +417,41 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
     // EPI_STORE, BF16 output in place of the hi tile (same layout), or FP32 output straight to global memory
     if (it.out_type == TY_BF16) {
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const int c0 = cbase + 16 * q;
-            tmem_ld16(taddr + 16 * q, a);
-            tile_values16(tile, n_base, r, c0, a, v);
-            uint32_t w[8];
+        for (int g = 0; g < 2; ++g) {
+            tile_values32(taddr, row, n_base, r, g, v);
 #pragma unroll
-            for (int u = 0; u < 8; ++u) {
-                const __nv_bfloat162 h = __floats2bfloat162_rn(v[2 * u], v[2 * u + 1]);
-                w[u] = *reinterpret_cast<const uint32_t*>(&h);
+            for (int j = 0; j < 4; ++j) {
+                uint32_t w[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const __nv_bfloat162 h = __floats2bfloat162_rn(v[8 * j + 2 * u], v[8 * j + 2 * u + 1]);
+                    w[u] = *reinterpret_cast<const uint32_t*>(&h);
+                }
+                sts128(row + (((uint32_t)(4 * g + j) ^ (uint32_t)(r & 7)) << 4), make_uint4(w[0], w[1], w[2], w[3]));
             }
-            const uint32_t row = tile + (uint32_t)half * 16384u + (uint32_t)r * 128u;
-            sts128(row + (((uint32_t)(2 * q) ^ (uint32_t)(r & 7)) << 4), make_uint4(w[0], w[1], w[2], w[3]));
-            sts128(row + (((uint32_t)(2 * q + 1) ^ (uint32_t)(r & 7)) << 4), make_uint4(w[4], w[5], w[6], w[7]));
         }
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         epi_sync();
         if (threadIdx.x == 0) {
 #pragma unroll
-            for (int h = 0; h < 2; ++h)
-#pragma unroll
-                for (int g = 0; g < 2; ++g)
-                    tma_store_2d(maps + it.out_map, tile + h * 16384u + g * 8192u, it.col0 + 64 * h, it.row0 + 64 * g);
+            for (int h = 0; h < 2; ++h) tma_store_2d(maps + it.out_map, tile + h * 16384u, it.col0 + 64 * h, it.row0);
             asm volatile("cp.async.bulk.commit_group;" ::: "memory");
         }
         return true;
     }
     const bool row_ok = r < it.rows;
 #pragma unroll
-    for (int q = 0; q < 4; ++q) {
-        const int c0 = cbase + 16 * q;
-        tmem_ld16(taddr + 16 * q, a);
-        tile_values16(tile, n_base, r, c0, a, v);
-        if (!row_ok || c0 >= it.cols) continue;
-        float4* o = reinterpret_cast<float4*>(reinterpret_cast<float*>(it.out) + (int64_t)(it.row0 + r) * it.out_ld + it.col0 + c0);
+    for (int g = 0; g < 2; ++g) {
+        tile_values32(taddr, row, n_base, r, g, v);
 #pragma unroll
-        for (int u = 0; u < 4; ++u) o[u] = make_float4(v[4 * u], v[4 * u + 1], v[4 * u + 2], v[4 * u + 3]);
+        for (int q = 0; q < 2; ++q) {
+            const int c0 = cbase + 32 * g + 16 * q;
+            if (!row_ok || c0 >= it.cols) continue;
+            float4* o = reinterpret_cast<float4*>(reinterpret_cast<float*>(it.out) + (int64_t)(it.row0 + r) * it.out_ld + it.col0 + c0);
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                o[u] = make_float4(v[16 * q + 4 * u], v[16 * q + 4 * u + 1], v[16 * q + 4 * u + 2], v[16 * q + 4 * u + 3]);
+        }
     }
     return false;
 }
@@ -449,12 +487,12 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
     auto item_slot = [&](uint32_t s) { return reinterpret_cast<const Item*>(s_items + s * ITEM_BYTES); };
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < MAX_STAGES; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+        for (int s = 0; s < MAX_STAGES; ++s) { mbar_init(full_bar(s), 2); mbar_init(empty_bar(s), 1); }
         for (int a = 0; a < 2; ++a) {
             mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), EPI_WARPS);
         }
         for (int b = 0; b < MAX_BASE_SLOTS; ++b) { mbar_init(bfull_bar(b), 1); mbar_init(bempty_bar(b), 1); }
-        for (int s = 0; s < ITEM_SLOTS; ++s) { mbar_init(ifull_bar(s), 1); mbar_init(iempty_bar(s), EPI_WARPS + 1); }
+        for (int s = 0; s < ITEM_SLOTS; ++s) { mbar_init(ifull_bar(s), 1); mbar_init(iempty_bar(s), EPI_WARPS + 3); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == MMA_WARP) {
@@ -506,40 +544,51 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                                 const uint32_t dst = base_tile(acc) + (uint32_t)b * TILE_BYTES;
 #pragma unroll
                                 for (int h = 0; h < 2; ++h)
-#pragma unroll
-                                    for (int g = 0; g < 2; ++g)
-                                        tma_load_2d(dst + h * 16384u + g * 8192u, mp, it.col0 + 64 * h, it.row0 + 64 * g,
-                                                    bfull_bar(acc));
+                                    tma_load_2d(dst + h * 16384u, mp, it.col0 + 64 * h, it.row0, bfull_bar(acc));
                             }
                         }
                     }
                 }
-                const int nbx = it.N >> 6, a_mn = it.a_mn;
-                const uint32_t tx = A_BYTES + (uint32_t)it.N * 128u;
+            }
+            ok = __shfl_sync(0xFFFFFFFFu, ok, 0);
+        }
+    } else if (warp == OPERAND_WARP || warp == OPERAND_WARP + 1) {
+        // ===== operand TMA producers (one lane each): warp 9 streams the A K-atoms, warp 10 the B K-atoms =====
+        // (a TMA issue costs ~200 cycles of the issuing thread, so the two operands get a thread each)
+        if (lane == 0) {
+            const bool is_b = warp != OPERAND_WARP;
+            uint32_t stage = 0, phase = 0, n_done = 0;
+            bool ok = true;
+            for (int i = blockIdx.x; i < n_items && ok; i += gridDim.x, ++n_done) {
+                const uint32_t slot = n_done % ITEM_SLOTS, iphase = (n_done / ITEM_SLOTS) & 1u;
+                if (!(ok = TWAIT(3, mbar_wait(ifull_bar(slot), iphase, err)))) break;
+                const Item& it = *item_slot(slot);
+                const int a_mn = it.a_mn;
+                const uint32_t tx = is_b ? (uint32_t)it.N * 128u : (uint32_t)A_BYTES;
+#pragma unroll 1
                 for (int seg = 0; seg < NSEG && ok; ++seg) {
                     const int na = it.atoms[seg];
                     if (na <= 0) continue;
-                    const CUtensorMap* ma = maps + it.map_a[seg];
-                    const CUtensorMap* mb = maps + it.map_b[seg];
-                    if (!(dbg & 2)) { tmap_acquire(ma); tmap_acquire(mb); }
-                    const int ac = it.a_c0[seg], ar = it.a_r0[seg], bc = it.b_c0[seg], br = it.b_r0[seg];
+                    const CUtensorMap* mp = maps + (is_b ? it.map_b[seg] : it.map_a[seg]);
+                    const int c0 = is_b ? it.b_c0[seg] : it.a_c0[seg], r0 = is_b ? it.b_r0[seg] : it.a_r0[seg];
+                    if (!(dbg & 2)) tmap_acquire(mp);
                     for (int t = 0; t < na; ++t) {
-                        if (!TWAIT(2, mbar_wait(empty_bar(stage), phase ^ 1u, err))) { ok = 0; break; }
-                        const uint32_t sa = smem0 + stage * STAGE_BYTES, sb = sa + A_BYTES;
+                        if (!TWAIT(2, mbar_wait(empty_bar(stage), phase ^ 1u, err))) { ok = false; break; }
+                        const uint32_t sa = smem0 + stage * STAGE_BYTES;
                         mbar_expect_tx(full_bar(stage), tx);
-                        if (a_mn) {
-                            tma_load_2d(sa, ma, ac, ar + 64 * t, full_bar(stage));
-                            tma_load_2d(sa + 8192, ma, ac + 64, ar + 64 * t, full_bar(stage));
-                        } else {
-                            tma_load_2d(sa, ma, ac + 64 * t, ar, full_bar(stage));
-                            tma_load_2d(sa + 8192, ma, ac + 64 * t, ar + 64, full_bar(stage));
+                        if (is_b) {               // N rows x 64 columns, one box
+                            tma_load_2d(sa + A_BYTES, mp, c0 + 64 * t, r0, full_bar(stage));
+                        } else if (a_mn) {        // two 64 x 64 boxes: 64 K-rows of 128 contiguous M elements
+                            tma_load_2d(sa, mp, c0, r0 + 64 * t, full_bar(stage));
+                            tma_load_2d(sa + 8192, mp, c0 + 64, r0 + 64 * t, full_bar(stage));
+                        } else {                  // one 128-row x 64-column box
+                            tma_load_2d(sa, mp, c0 + 64 * t, r0, full_bar(stage));
                         }
-                        for (int b = 0; b < nbx; ++b) tma_load_2d(sb + 8192 * b, mb, bc + 64 * t, br + 64 * b, full_bar(stage));
                         if (++stage == (uint32_t)n_stages) { stage = 0; phase ^= 1u; }
                     }
                 }
+                mbar_arrive(iempty_bar(slot));
             }
-            ok = __shfl_sync(0xFFFFFFFFu, ok, 0);
         }
     } else if (warp == MMA_WARP) {
         // ===== MMA issuer (one lane) =====
@@ -579,12 +628,16 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
     } else {
         // ===== epilogue warps 0..7 =====
         uint32_t n_done = 0;
+        int pending_slot = -1;
         bool ok = true;
         for (int i = blockIdx.x; i < n_items && ok; i += gridDim.x, ++n_done) {
             const uint32_t slot = n_done % ITEM_SLOTS, iphase = (n_done / ITEM_SLOTS) & 1u;
             const uint32_t acc = n_done & 1u, aphase = (n_done >> 1) & 1u;
             const uint32_t bs = n_base > 0 ? n_done % (uint32_t)n_bslots : 0u, bphase = n_base > 0 ? (n_done / (uint32_t)n_bslots) & 1u : 0u;
             ok = TWAIT(0, mbar_wait(ifull_bar(slot), iphase, err));
+            // the tensor's amax (EPI_CAST) is fetched before the data waits, so its latency hides behind them
+            uint32_t amax_bits = 0;
+            if (ok && item_slot(slot)->mode == EPI_CAST) amax_bits = *reinterpret_cast<volatile uint32_t*>(item_slot(slot)->amax);
             if (ok && n_base > 0) ok = TWAIT(1, mbar_wait(bfull_bar(bs), bphase, err));
             ok = ok && TWAIT(2, mbar_wait(tfull_bar(acc), aphase, err));
             const long long t_e0 = prof ? clock64() : 0;
@@ -594,7 +647,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
             const Item& it = *item_slot(slot);
             bool stored = false;
             if (it.base_map[0] >= 0)
-                stored = epilogue_tile(it, tmem_base + acc * 128u, base_tile(bs), it.base_map[1] >= 0 ? 2 : 1, warp, lane, s_red, maps);
+                stored = epilogue_tile(it, tmem_base + acc * 128u, base_tile(bs), it.base_map[1] >= 0 ? 2 : 1, warp, lane, s_red, maps, amax_bits);
             else
                 epilogue(it, tmem_base + acc * 128u, warp, lane, s_red);
             tc_fence_before();
@@ -603,19 +656,27 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
             const long long t_p0 = prof ? clock64() : 0;
             if (lane == 0) { mbar_arrive(tempty_bar(acc)); mbar_arrive(iempty_bar(slot)); }
             if (n_base > 0) {
-                epi_sync();                                   // every epilogue thread is done with the tile
+                // the base slot goes back to the producer once every epilogue thread is done with it and the TMA
+                // store issued from it (if any) has read it.  That store wait is deferred by one item, so it
+                // overlaps the next tile instead of stalling this warp.
+                if (threadIdx.x == 0 && pending_slot >= 0) {
+                    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+                    mbar_arrive(bempty_bar(pending_slot));
+                    pending_slot = -1;
+                }
+                epi_sync();
                 if (threadIdx.x == 0) {
-                    if (stored) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-                    mbar_arrive(bempty_bar(bs));
+                    if (stored) pending_slot = (int)bs;
+                    else mbar_arrive(bempty_bar(bs));
                 }
             }
             if (prof) pw[4] += clock64() - t_p0;
         }
-        if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+        if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // (pending slot: kernel ends)
     }
 #undef TWAIT
-    if (prof && lane == 0 && (warp == 0 || warp == PRODUCER_WARP || warp == MMA_WARP)) {
-        const int role = warp == 0 ? 0 : (warp == PRODUCER_WARP ? 1 : 2);
+    if (prof && lane == 0 && (warp == 0 || warp == OPERAND_WARP || warp == MMA_WARP)) {
+        const int role = warp == 0 ? 0 : (warp == OPERAND_WARP ? 1 : 2);
         pw[5] = clock64() - t_start;
         for (int q = 0; q < 6; ++q) prof[((size_t)blockIdx.x * 3 + role) * 6 + q] = pw[q];
     }
