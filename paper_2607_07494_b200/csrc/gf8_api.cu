@@ -298,7 +298,7 @@ gf8_status fast_encode_many(gf8_ctx* c, int n, const int* layers, const void* co
         for (int i = 0; i < n; ++i) {
             if (c->layers[layers[i]].tc_ok) tc_idx.push_back(i); else p->plain.push_back(i);
         }
-        p->n_amax = tc_idx.size();
+        p->n_amax = 2 * tc_idx.size();           // per TC problem: amax word + parked-tile counter
         gf8_status s = GF8_OK;
         if (p->n_amax) {
             void* q = nullptr;
@@ -331,7 +331,7 @@ gf8_status fast_encode_many(gf8_ctx* c, int n, const int* layers, const void* co
             if (tap) { f.mode = EPI_STORE; f.out = taps[i]; f.out_type = TY_F32; }
             else {
                 f.mode = L.desc.scaling == GF8_SCALE_TENSOR ? EPI_AMAX : EPI_BLOCKCAST;
-                f.out = codes[i]; f.amax = p->d_amax + t; f.scale_inv = sinv[i];
+                f.out = codes[i]; f.amax = p->d_amax + 2 * t; f.done = p->d_amax + 2 * t + 1; f.scale_inv = sinv[i];
                 if (dt == GF8_DT_BF16) {
                     CUtensorMap mc;
                     if ((s = make_map_u8(c, &mc, codes[i], m, nn)) != GF8_OK) break;

@@ -215,6 +215,7 @@ struct Final {                  // what the last stage of a transform does with 
     const void* base; int base_type;
     void* out; int out_type;
     uint32_t* amax; float* scale_inv;
+    uint32_t* done;             // fused update: the tensor's parked-tile counter (next to its amax word)
     int base_map[2];            // TMA-streamed base tile(s) (hi [+ lo]); -1: base read straight from global memory
     int out_map;                // TMA store map of the output (codes or BF16); -1: direct stores
 };
@@ -231,7 +232,7 @@ inline Item blank_item() {
 // expands to hi*hi + lo*hi + hi*lo, which brings the tensor-core result to ~FP32 accuracy at 3x the MMAs.
 // src_lo_map < 0 means the source is exactly BF16 (a BF16 gradient) and needs no residual.
 void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src_lo_map, bool inverse, bool split,
-                   const Final& f) {
+                   const Final& f, int c_num_sms = 148) {
     using namespace gf8::tc;
     const int m = L.desc.d_out, n = L.desc.d_in;
     const bool useA = L.in.used, useG = L.out.used;
@@ -336,7 +337,16 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
             it.mode = f.mode;
             it.base_map[0] = f.base_map[0] >= 0 ? f.base_map[0] + 1 : -1;      // 128-row boxes
             it.base_map[1] = f.base_map[1] >= 0 ? f.base_map[1] + 1 : -1;
-            if (f.mode == EPI_AMAX) {
+            const int n_tiles = ((m + 127) / 128) * tiles_n;
+            if (f.mode == EPI_AMAX && f.done && f.out_map >= 0 && it.base_map[0] >= 0 && n_tiles <= gf8::tc::FUSE_LAG * c_num_sms &&
+                getenv("GF8_TC_FUSE")) {
+                // fused update (opt-in, GF8_TC_FUSE=1): one pass parks the FP32 tile in TMEM, the cast
+                // follows when the tensor amax is complete.  It needs every CTA of the launch co-resident.
+                it.amax = f.amax; it.out = f.out; it.out_ld = n; it.scale_inv_out = f.scale_inv; it.out_map = f.out_map;
+                it.write_scale = (i0 == 0 && j0 == 0) ? 1 : 0;
+                it.base = f.done; it.base_ld = n_tiles;
+                pb.stage[5].push_back(it);
+            } else if (f.mode == EPI_AMAX) {
                 it.amax = f.amax;
                 pb.stage[3].push_back(it);
                 it.mode = EPI_CAST; it.out = f.out; it.out_ld = n; it.scale_inv_out = f.scale_inv; it.out_map = f.out_map;
@@ -409,14 +419,17 @@ gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
         const int n_base = p->stage_base[s];
         // shared-memory split: update stages keep a short operand ring (their operands are L2-resident) and give
         // the rest to base tiles in flight (the HBM stream); panel stages give everything to the operand ring
+        const int fuse = s == 5 ? 1 : 0;
         int n_stages = n_base ? 3 : gf8::tc::MAX_STAGES, dbg = 0, only = -1;
-        const int n_bslots = n_base ? (gf8::tc::MAX_STAGES - n_stages) / n_base : 1;
+        // (the fused stage gives one base slot's worth of shared memory to its two code-tile staging buffers)
+        const int n_bslots = fuse ? 3 : (n_base ? (gf8::tc::MAX_STAGES - n_stages) / n_base : 1);
+        if (fuse && grid < c->num_sms && p->stage_cnt[s] > grid) return fail(c, GF8_ERR_BAD_STATE, "fused stage needs a full grid");
         if (const char* e = getenv("GF8_TC_DBG")) dbg = atoi(e);
         if (!first_run) dbg |= 2;        // tensor maps are written once by the host before the plan's first launch
         if (const char* e = getenv("GF8_TC_ONLY")) only = atoi(e);
         if (only >= 0 && only != s) continue;
         gf8::tc::tc_items_kernel<<<grid, gf8::tc::THREADS, gf8::tc::SMEM_BYTES, st>>>(
-            p->d_items + p->stage_off[s], p->stage_cnt[s], p->d_maps, c->d_err, n_stages, n_base, n_bslots, dbg, (dbg & 4) ? c->d_prof : nullptr);
+            p->d_items + p->stage_off[s], p->stage_cnt[s], p->d_maps, c->d_err, n_stages, n_base, n_bslots, fuse, dbg, (dbg & 4) ? c->d_prof : nullptr);
         if (dbg & 4) {
             std::vector<long long> h((size_t)c->num_sms * 18);
             cudaMemcpy(h.data(), c->d_prof, h.size() * sizeof(long long), cudaMemcpyDeviceToHost);

@@ -33,12 +33,16 @@ constexpr int B_BYTES = 128 * 64 * 2;            // one K-atom of B: up to 128 x
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;   // 32 KB
 constexpr int TILE_BYTES = 128 * 128 * 2;        // one streamed 128 x 128 BF16 base tile (two 64-column halves)
 constexpr int DATA_BYTES = MAX_STAGES * STAGE_BYTES;   // 224 KB, split at launch into ring stages + base tiles
-constexpr int SMEM_BYTES = DATA_BYTES + 1024 /*alignment slack*/ + 1536 /*barriers, item ring*/;
-constexpr int EPI_WARPS = 8, PRODUCER_WARP = 8, OPERAND_WARP = 9, MMA_WARP = 11;
-constexpr int THREADS = 32 * (EPI_WARPS + 4);
+constexpr int MISC_BYTES = 2048;                 // barriers, TMEM address, reductions, parked-tile info, item ring
+constexpr int SMEM_BYTES = DATA_BYTES + 1024 /*alignment slack*/ + MISC_BYTES;
+constexpr int EPI_WARPS = 8, PRODUCER_WARP = 8, OPERAND_WARP = 9, MMA_WARP = 11, SYNC_WARP = 12;
+constexpr int THREADS = 32 * (EPI_WARPS + 5);
 constexpr int ITEM_SLOTS = 4;                    // shared-memory ring of item descriptors
 constexpr int MAX_BASE_SLOTS = 4;                // streamed base tiles in flight (ring, decoupled from TMEM)
-constexpr int TMEM_COLS = 256;                   // two accumulators of up to 128 columns
+constexpr int TMEM_COLS = 512;                   // four 128-column accumulator slots
+constexpr int FUSE_LAG = 2;                      // fused update: tiles parked in TMEM while the tensor amax completes
+                                                 // (2 parked + 1 in the epilogue + 1 under the MMAs = 4 slots)
+constexpr int CODE_TILE_BYTES = 128 * 128;       // staging of one 128 x 128 FP8 code tile
 constexpr int NSEG = 6;                          // operand segments per item (hi/lo split products)
 
 enum Epi : int32_t {
@@ -71,8 +75,16 @@ struct __align__(16) Item {
     float* scale_inv_out;         // EPI_CAST (write_scale) / EPI_BLOCKCAST: where scale_inv goes
 };
 
+// What the fused update keeps about a tile parked in TMEM until its tensor's amax is complete.
+struct Parked {
+    int32_t out_map, col0, row0, fmt, write_scale, total;
+    uint32_t* amax;
+    float* scale_inv_out;
+    uint32_t* done;
+};
+
 constexpr int ITEM_BYTES = (int)sizeof(Item);
-static_assert(ITEM_BYTES % 16 == 0 && 352 + ITEM_SLOTS * ITEM_BYTES <= 1536, "item ring must fit its shared-memory slice");
+static_assert(ITEM_BYTES % 16 == 0 && 656 + ITEM_SLOTS * ITEM_BYTES <= MISC_BYTES, "item ring must fit its shared-memory slice");
 
 // ---- PTX wrappers ------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -142,6 +154,17 @@ __device__ __forceinline__ void tmem_ld32_nowait(uint32_t taddr, uint32_t* v) {
           "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
         : "r"(taddr) : "memory");
 }
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t* v) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,"
+        "%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};"
+        ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]),
+          "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]),
+          "r"(v[16]), "r"(v[17]), "r"(v[18]), "r"(v[19]), "r"(v[20]), "r"(v[21]), "r"(v[22]), "r"(v[23]),
+          "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]), "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31])
+        : "memory");
+}
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // Shared-memory matrix descriptor (SWIZZLE_128B, version 1).  lbo / sbo in bytes.
@@ -464,31 +487,37 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
 // so a pipeline bug cannot hang the GPU.
 __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __restrict__ items, int n_items,
                                                               const CUtensorMap* __restrict__ maps, int* err,
-                                                              int n_stages, int n_base, int n_bslots, int dbg,
+                                                              int n_stages, int n_base, int n_bslots, int fuse, int dbg,
                                                               long long* __restrict__ prof) {
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;          // 1024-byte aligned (swizzle atoms)
     const uint32_t base0 = smem0 + (uint32_t)n_stages * STAGE_BYTES;        // base tiles: [acc][n_base] x 32 KB
     const uint32_t bars = smem0 + DATA_BYTES;
     uint8_t* gen0 = smem_raw + (smem0 - smem_u32(smem_raw));
-    uint32_t* s_tmem = reinterpret_cast<uint32_t*>(gen0 + DATA_BYTES + 288);
+    uint32_t* s_tmem = reinterpret_cast<uint32_t*>(gen0 + DATA_BYTES + 384);
     uint32_t* s_red = s_tmem + 4;
-    uint8_t* s_items = gen0 + DATA_BYTES + 352;
+    Parked* s_park = reinterpret_cast<Parked*>(gen0 + DATA_BYTES + 464);
+    uint8_t* s_items = gen0 + DATA_BYTES + 656;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     auto full_bar = [&](int s) { return bars + 8u * s; };
     auto empty_bar = [&](int s) { return bars + 8u * (MAX_STAGES + s); };
     auto tfull_bar = [&](int a) { return bars + 8u * (2 * MAX_STAGES + a); };
-    auto tempty_bar = [&](int a) { return bars + 8u * (2 * MAX_STAGES + 2 + a); };
-    auto bfull_bar = [&](int a) { return bars + 8u * (2 * MAX_STAGES + 4 + a); };
-    auto bempty_bar = [&](int a) { return bars + 8u * (2 * MAX_STAGES + 4 + MAX_BASE_SLOTS + a); };
-    auto ifull_bar = [&](int s) { return bars + 8u * (2 * MAX_STAGES + 4 + 2 * MAX_BASE_SLOTS + s); };
-    auto iempty_bar = [&](int s) { return bars + 8u * (2 * MAX_STAGES + 4 + 2 * MAX_BASE_SLOTS + ITEM_SLOTS + s); };
+    auto tempty_bar = [&](int a) { return bars + 8u * (2 * MAX_STAGES + 4 + a); };
+    auto bfull_bar = [&](int a) { return bars + 8u * (2 * MAX_STAGES + 8 + a); };
+    auto bempty_bar = [&](int a) { return bars + 8u * (2 * MAX_STAGES + 8 + MAX_BASE_SLOTS + a); };
+    auto ifull_bar = [&](int s) { return bars + 8u * (2 * MAX_STAGES + 8 + 2 * MAX_BASE_SLOTS + s); };
+    auto iempty_bar = [&](int s) { return bars + 8u * (2 * MAX_STAGES + 8 + 2 * MAX_BASE_SLOTS + ITEM_SLOTS + s); };
+    auto parked_bar = [&](int a) { return bars + 8u * (2 * MAX_STAGES + 8 + 2 * MAX_BASE_SLOTS + 2 * ITEM_SLOTS + a); };
+    auto sready_bar = [&](int a) { return bars + 8u * (2 * MAX_STAGES + 8 + 2 * MAX_BASE_SLOTS + 2 * ITEM_SLOTS + 4 + a); };
+    float* s_scale = reinterpret_cast<float*>(s_red + 8);     // fused update: scale of each parked tile's tensor
+    const uint32_t n_acc = fuse ? 4u : 2u;           // TMEM accumulator slots in rotation
     auto base_tile = [&](uint32_t b) { return base0 + b * (uint32_t)n_base * TILE_BYTES; };
     auto item_slot = [&](uint32_t s) { return reinterpret_cast<const Item*>(s_items + s * ITEM_BYTES); };
 
     if (threadIdx.x == 0) {
         for (int s = 0; s < MAX_STAGES; ++s) { mbar_init(full_bar(s), 2); mbar_init(empty_bar(s), 1); }
-        for (int a = 0; a < 2; ++a) {
+        for (int a = 0; a < 4; ++a) {
+            mbar_init(parked_bar(a), 1); mbar_init(sready_bar(a), 1);
             mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), EPI_WARPS);
         }
         for (int b = 0; b < MAX_BASE_SLOTS; ++b) { mbar_init(bfull_bar(b), 1); mbar_init(bempty_bar(b), 1); }
@@ -605,7 +634,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
 #pragma unroll
                 for (int seg = 0; seg < NSEG; ++seg) total += it.atoms[seg];
                 mbar_arrive(iempty_bar(slot));
-                const uint32_t acc = n_done & 1u, aphase = (n_done >> 1) & 1u;
+                const uint32_t acc = n_done % n_acc, aphase = (n_done / n_acc) & 1u;
                 if (!(ok = TWAIT(1, mbar_wait(tempty_bar(acc), aphase ^ 1u, err)))) break;
                 tc_fence_after();
                 const uint32_t d = tmem_base + acc * 128u;
@@ -625,6 +654,132 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 tc_commit(tfull_bar(acc));                // accumulator complete -> epilogue
             }
         }
+    } else if (warp == SYNC_WARP) {
+        // ===== fused update: grid-level bookkeeping off the epilogue's critical path (one lane) =====
+        // add(n): tile n is parked -> bump its tensor's counter.  resolve(n - FUSE_LAG): wait until that tensor's
+        // counter is complete, read its amax, publish the scale in shared memory and release cast(n - FUSE_LAG).
+        // Lane a serves TMEM slot a (tiles n = a, a + 4, ...): bump (release) then poll (acquire), so the four
+        // slots' round trips to L2 overlap and no lane's wait holds back another tile's bump.
+        if (fuse && lane < 4) {
+            uint32_t my_items = 0;
+            for (int i = blockIdx.x; i < n_items; i += gridDim.x) ++my_items;
+            for (uint32_t n = (uint32_t)lane; n < my_items; n += 4) {
+                const uint32_t acc = n & 3u;
+                if (!mbar_wait(parked_bar(acc), (n >> 2) & 1u, err)) break;
+                const Parked pk = s_park[acc];
+                asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(pk.done) : "memory");
+                uint32_t spin = 0, seen = 0;
+                bool bad = false;
+                for (;;) {
+                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(pk.done) : "memory");
+                    if (seen >= (uint32_t)pk.total) break;
+                    if (++spin > (1u << 22) || ((spin & 0x3FF) == 0 && *reinterpret_cast<volatile int*>(err))) { bad = true; break; }
+                    __nanosleep(32);
+                }
+                if (bad) { atomicExch(err, 2); break; }
+                float scale, si;
+                scales_from_amax(*reinterpret_cast<volatile uint32_t*>(pk.amax), pk.fmt == 0 ? 448.0f : 57344.0f, scale, si);
+                if (pk.write_scale) *pk.scale_inv_out = si;
+                s_scale[acc] = scale;
+                mbar_arrive(sready_bar(acc));
+            }
+        }
+    } else if (fuse) {
+        // ===== epilogue warps 0..7, FUSED update (a4 + a5 + a6 in one pass over the gradient) =====
+        // park(n): W~ tile = base + acc, its amax goes to the tensor's amax word, the FP32 tile is written back into
+        // its TMEM slot and the tensor's done-counter is bumped.  cast(n - FUSE_LAG): once the counter says every
+        // tile of that tensor is parked (spin on a global word; deadlock-free because a tensor's tiles are contiguous
+        // in the item list, all CTAs are co-resident and FUSE_LAG >= ceil(tiles / grid)), the parked tile is read
+        // back, scaled, cast and stored.  Four TMEM slots hold three parked tiles plus the one being computed.
+        const int r = (warp & 3) * 32 + lane, half = warp >> 2;
+        const uint32_t lane_off = ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(half * 64);
+        const uint32_t code0 = base0 + (uint32_t)n_bslots * (uint32_t)n_base * TILE_BYTES;   // two code-tile buffers
+        uint32_t my_items = 0;
+        for (int i = blockIdx.x; i < n_items; i += gridDim.x) ++my_items;
+        bool ok = true;
+        auto cast_one = [&](uint32_t j) -> bool {
+            const uint32_t acc = j & 3u;
+            // the sync warp has seen the tensor's last tile parked and left its scale in shared memory
+            if (!mbar_wait(sready_bar(acc), (j >> 2) & 1u, err)) return false;
+            if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");   // staging buffer j & 1 is free
+            epi_sync();
+            const Parked pk = s_park[acc];
+            const float scale = s_scale[acc];
+            const uint32_t taddr = tmem_base + acc * 128u + lane_off;
+            uint4 cd[4];
+#pragma unroll
+            for (int g = 0; g < 2; ++g) {
+                uint32_t a[32];
+                tmem_ld32_nowait(taddr + 32u * g, a);
+                tmem_wait();
+                float v[32];
+#pragma unroll
+                for (int u = 0; u < 32; ++u) v[u] = __uint_as_float(a[u]);
+                cd[2 * g] = pk.fmt == 0 ? codes16<0>(v, scale) : codes16<1>(v, scale);
+                cd[2 * g + 1] = pk.fmt == 0 ? codes16<0>(v + 16, scale) : codes16<1>(v + 16, scale);
+            }
+            const uint32_t tile = code0 + (j & 1u) * CODE_TILE_BYTES;
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                sts128(tile + (uint32_t)r * 128u + (((uint32_t)(4 * half + q) ^ (uint32_t)(r & 7)) << 4), cd[q]);
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            tc_fence_before();
+            epi_sync();
+            if (threadIdx.x == 0) {
+                tma_store_2d(maps + pk.out_map, tile, pk.col0, pk.row0);
+                asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(tempty_bar(acc));
+            return true;
+        };
+        for (uint32_t n = 0; n < my_items && ok; ++n) {
+            const uint32_t slot = n % ITEM_SLOTS, iphase = (n / ITEM_SLOTS) & 1u;
+            const uint32_t acc = n & 3u, aphase = (n >> 2) & 1u;
+            const uint32_t bs = n % (uint32_t)n_bslots, bphase = (n / (uint32_t)n_bslots) & 1u;
+            ok = TWAIT(0, mbar_wait(ifull_bar(slot), iphase, err));
+            ok = ok && TWAIT(1, mbar_wait(bfull_bar(bs), bphase, err));
+            ok = ok && TWAIT(2, mbar_wait(tfull_bar(acc), aphase, err));
+            ok = __all_sync(0xFFFFFFFFu, ok);
+            if (!ok) break;
+            tc_fence_after();
+            const long long t_e0 = prof ? clock64() : 0;
+            const Item& it = *item_slot(slot);
+            const uint32_t taddr = tmem_base + acc * 128u + lane_off;
+            const uint32_t row = base_tile(bs) + (uint32_t)half * 16384u + (uint32_t)r * 128u;
+            uint32_t loc = 0;
+#pragma unroll
+            for (int g = 0; g < 2; ++g) {
+                float v[32];
+                tile_values32(taddr, row, 1, r, g, v);
+                uint32_t w[32];
+#pragma unroll
+                for (int u = 0; u < 32; ++u) { w[u] = __float_as_uint(v[u]); loc = max(loc, w[u] & 0x7FFFFFFFu); }
+                tmem_st32(taddr + 32u * g, w);
+            }
+            tmem_wait_st();
+            loc = warp_max_u32(loc);
+            if (lane == 0 && loc != 0u) atomicMax(it.amax, loc);
+            if (threadIdx.x == 0) {
+                Parked pk;
+                pk.out_map = it.out_map; pk.col0 = it.col0; pk.row0 = it.row0; pk.fmt = it.fmt;
+                pk.write_scale = it.write_scale; pk.total = (int32_t)it.base_ld;
+                pk.amax = it.amax; pk.scale_inv_out = it.scale_inv_out;
+                pk.done = reinterpret_cast<uint32_t*>(const_cast<void*>(it.base));
+                s_park[acc] = pk;
+            }
+            tc_fence_before();
+            epi_sync();                       // base tile consumed, amax atomics issued, parked info visible
+            if (threadIdx.x == 0) { mbar_arrive(parked_bar(acc)); mbar_arrive(bempty_bar(bs)); }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(iempty_bar(slot));
+            if (prof) pw[3] += clock64() - t_e0;
+            const long long t_p0 = prof ? clock64() : 0;
+            if (n >= (uint32_t)FUSE_LAG) ok = cast_one(n - FUSE_LAG);
+            if (prof) pw[4] += clock64() - t_p0;
+        }
+        for (uint32_t j = my_items > (uint32_t)FUSE_LAG ? my_items - FUSE_LAG : 0u; j < my_items && ok; ++j) ok = cast_one(j);
+        if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     } else {
         // ===== epilogue warps 0..7 =====
         uint32_t n_done = 0;
@@ -632,7 +787,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
         bool ok = true;
         for (int i = blockIdx.x; i < n_items && ok; i += gridDim.x, ++n_done) {
             const uint32_t slot = n_done % ITEM_SLOTS, iphase = (n_done / ITEM_SLOTS) & 1u;
-            const uint32_t acc = n_done & 1u, aphase = (n_done >> 1) & 1u;
+            const uint32_t acc = n_done % n_acc, aphase = (n_done / n_acc) & 1u;
             const uint32_t bs = n_base > 0 ? n_done % (uint32_t)n_bslots : 0u, bphase = n_base > 0 ? (n_done / (uint32_t)n_bslots) & 1u : 0u;
             ok = TWAIT(0, mbar_wait(ifull_bar(slot), iphase, err));
             // the tensor's amax (EPI_CAST) is fetched before the data waits, so its latency hides behind them

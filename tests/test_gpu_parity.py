@@ -224,6 +224,22 @@ def test_fast_batched_matches_single_calls():
     assert torch.equal(outs[0], out1)
 
 
+def test_fast_fused_update_matches_two_pass(monkeypatch):
+    """The opt-in fused update (W~ tiles parked in TMEM across the tensor-wide amax, GF8_TC_FUSE=1) produces the
+    same codes and scales as the default amax pass + cast pass."""
+    c = fcase("llama600m-q")
+    gs = [c.rank_grad(r) for r in range(4)]
+    ref = [tuple(t.clone() for t in c.ctx.encode(0, g)) for g in gs]
+    monkeypatch.setenv("GF8_TC_FUSE", "1")
+    gs2 = [g.clone() for g in gs]                       # new pointers -> a new (fused) plan
+    codes = [torch.empty_like(ref[0][0]) for _ in gs2]
+    sinvs = [torch.empty_like(ref[0][1]) for _ in gs2]
+    c.ctx.encode_many([0] * len(gs2), gs2, codes, sinvs)
+    c.ctx.sync_check()
+    for r in range(len(gs2)):
+        assert torch.equal(codes[r], ref[r][0]) and torch.equal(sinvs[r], ref[r][1])
+
+
 def test_euclidean_layer_is_plain_fp8():
     """side = NONE (embedding / LM head): codes and decoded values bit-exact."""
     m, n = 400, 256
