@@ -119,6 +119,13 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map
         "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
         ::"r"(dst), "l"(map), "r"(bar), "r"(c), "r"(r) : "memory");
 }
+// One lane of a converged warp (the role loops stay warp-uniform, so their operands live in uniform registers
+// and the TMA / MMA issues need no per-thread waterfall).
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+    return pred != 0;
+}
 __device__ __forceinline__ void tmap_acquire(const CUtensorMap* map) {
     asm volatile("fence.proxy.tensormap::generic.acquire.gpu [%0], 128;" ::"l"(map) : "memory");
 }
@@ -555,36 +562,37 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
             if (lane == 0) mbar_arrive(ifull_bar(slot));
             if (i + (int)gridDim.x < n_items && lane < NCHUNK)
                 nxt = __ldg(reinterpret_cast<const uint4*>(items + i + gridDim.x) + lane);
-            if (lane == 0) {
+            if (n_base > 0) {
+                // the item's base tile(s): hi [+ lo], each two 64-column halves of 128 rows (converged warp, one
+                // elected lane issues)
                 const Item& it = *item_slot(slot);
-                if (n_base > 0) {
-                    // the item's base tile(s): hi [+ lo], each 2 halves x 2 row groups of 64 x 64 boxes
-                    const uint32_t acc = n_done % (uint32_t)n_bslots, aphase = (n_done / (uint32_t)n_bslots) & 1u;
-                    ok = TWAIT(1, mbar_wait(bempty_bar(acc), aphase ^ 1u, err)) ? 1 : 0;
-                    if (ok) {
-                        int nb = 0;
-                        for (int b = 0; b < 2; ++b) nb += (it.base_map[b] >= 0) ? 1 : 0;
+                const uint32_t acc = n_done % (uint32_t)n_bslots, aphase = (n_done / (uint32_t)n_bslots) & 1u;
+                ok = TWAIT(1, mbar_wait(bempty_bar(acc), aphase ^ 1u, err)) ? 1 : 0;
+                if (ok) {
+                    const int bm0 = it.base_map[0], bm1 = it.base_map[1], col0 = it.col0, row0 = it.row0;
+                    const int nb = (bm0 >= 0 ? 1 : 0) + (bm1 >= 0 ? 1 : 0);
+                    if (elect_one()) {
                         if (nb == 0) mbar_arrive(bfull_bar(acc));
                         else {
                             mbar_expect_tx(bfull_bar(acc), (uint32_t)nb * TILE_BYTES);
                             for (int b = 0; b < nb; ++b) {
-                                const CUtensorMap* mp = maps + it.base_map[b];
+                                const CUtensorMap* mp = maps + (b ? bm1 : bm0);
                                 if (!(dbg & 2)) tmap_acquire(mp);
                                 const uint32_t dst = base_tile(acc) + (uint32_t)b * TILE_BYTES;
 #pragma unroll
-                                for (int h = 0; h < 2; ++h)
-                                    tma_load_2d(dst + h * 16384u, mp, it.col0 + 64 * h, it.row0, bfull_bar(acc));
+                                for (int h = 0; h < 2; ++h) tma_load_2d(dst + h * 16384u, mp, col0 + 64 * h, row0, bfull_bar(acc));
                             }
                         }
                     }
+                    __syncwarp();
                 }
             }
             ok = __shfl_sync(0xFFFFFFFFu, ok, 0);
         }
     } else if (warp == OPERAND_WARP || warp == OPERAND_WARP + 1) {
         // ===== operand TMA producers (one lane each): warp 9 streams the A K-atoms, warp 10 the B K-atoms =====
-        // (a TMA issue costs ~200 cycles of the issuing thread, so the two operands get a thread each)
-        if (lane == 0) {
+        // (a TMA issue costs ~200 cycles of the issuing thread, so the two operands get a warp each)
+        {
             const bool is_b = warp != OPERAND_WARP;
             uint32_t stage = 0, phase = 0, n_done = 0;
             bool ok = true;
@@ -600,28 +608,33 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                     if (na <= 0) continue;
                     const CUtensorMap* mp = maps + (is_b ? it.map_b[seg] : it.map_a[seg]);
                     const int c0 = is_b ? it.b_c0[seg] : it.a_c0[seg], r0 = is_b ? it.b_r0[seg] : it.a_r0[seg];
-                    if (!(dbg & 2)) tmap_acquire(mp);
+                    if (!(dbg & 2) && elect_one()) tmap_acquire(mp);
+                    __syncwarp();
                     for (int t = 0; t < na; ++t) {
                         if (!TWAIT(2, mbar_wait(empty_bar(stage), phase ^ 1u, err))) { ok = false; break; }
                         const uint32_t sa = smem0 + stage * STAGE_BYTES;
-                        mbar_expect_tx(full_bar(stage), tx);
-                        if (is_b) {               // N rows x 64 columns, one box
-                            tma_load_2d(sa + A_BYTES, mp, c0 + 64 * t, r0, full_bar(stage));
-                        } else if (a_mn) {        // two 64 x 64 boxes: 64 K-rows of 128 contiguous M elements
-                            tma_load_2d(sa, mp, c0, r0 + 64 * t, full_bar(stage));
-                            tma_load_2d(sa + 8192, mp, c0 + 64, r0 + 64 * t, full_bar(stage));
-                        } else {                  // one 128-row x 64-column box
-                            tma_load_2d(sa, mp, c0 + 64 * t, r0, full_bar(stage));
+                        if (elect_one()) {
+                            mbar_expect_tx(full_bar(stage), tx);
+                            if (is_b) {               // N rows x 64 columns, one box
+                                tma_load_2d(sa + A_BYTES, mp, c0 + 64 * t, r0, full_bar(stage));
+                            } else if (a_mn) {        // two 64 x 64 boxes: 64 K-rows of 128 contiguous M elements
+                                tma_load_2d(sa, mp, c0, r0 + 64 * t, full_bar(stage));
+                                tma_load_2d(sa + 8192, mp, c0 + 64, r0 + 64 * t, full_bar(stage));
+                            } else {                  // one 128-row x 64-column box
+                                tma_load_2d(sa, mp, c0 + 64 * t, r0, full_bar(stage));
+                            }
                         }
+                        __syncwarp();
                         if (++stage == (uint32_t)n_stages) { stage = 0; phase ^= 1u; }
                     }
                 }
-                mbar_arrive(iempty_bar(slot));
+                __syncwarp();
+                if (elect_one()) mbar_arrive(iempty_bar(slot));
             }
         }
     } else if (warp == MMA_WARP) {
-        // ===== MMA issuer (one lane) =====
-        if (lane == 0) {
+        // ===== MMA issuer (converged warp, one elected lane issues) =====
+        {
             uint32_t stage = 0, phase = 0, n_done = 0;
             bool ok = true;
             for (int i = blockIdx.x; i < n_items && ok; i += gridDim.x, ++n_done) {
@@ -633,7 +646,8 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 int total = 0;
 #pragma unroll
                 for (int seg = 0; seg < NSEG; ++seg) total += it.atoms[seg];
-                mbar_arrive(iempty_bar(slot));
+                __syncwarp();
+                if (elect_one()) mbar_arrive(iempty_bar(slot));
                 const uint32_t acc = n_done % n_acc, aphase = (n_done / n_acc) & 1u;
                 if (!(ok = TWAIT(1, mbar_wait(tempty_bar(acc), aphase ^ 1u, err)))) break;
                 tc_fence_after();
@@ -642,16 +656,20 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                     if (!(ok = TWAIT(2, mbar_wait(full_bar(stage), phase, err)))) break;
                     tc_fence_after();
                     const uint32_t sa = smem0 + stage * STAGE_BYTES, sb = sa + A_BYTES;
+                    if (elect_one()) {
 #pragma unroll
-                    for (int kk = 0; kk < 4; ++kk) {
-                        const uint64_t da = a_mn ? smem_desc(sa + 2048u * kk, 8192u, 1024u) : smem_desc(sa + 32u * kk, 16u, 1024u);
-                        const uint64_t db = smem_desc(sb + 32u * kk, 16u, 1024u);
-                        if (!(dbg & 1)) tc_mma_bf16(d, da, db, idesc, (t | kk) ? 1u : 0u);
+                        for (int kk = 0; kk < 4; ++kk) {
+                            const uint64_t da = a_mn ? smem_desc(sa + 2048u * kk, 8192u, 1024u) : smem_desc(sa + 32u * kk, 16u, 1024u);
+                            const uint64_t db = smem_desc(sb + 32u * kk, 16u, 1024u);
+                            if (!(dbg & 1)) tc_mma_bf16(d, da, db, idesc, (t | kk) ? 1u : 0u);
+                        }
+                        tc_commit(empty_bar(stage));      // frees the smem stage when these MMAs retire
                     }
-                    tc_commit(empty_bar(stage));          // frees the smem stage when these MMAs retire
+                    __syncwarp();
                     if (++stage == (uint32_t)n_stages) { stage = 0; phase ^= 1u; }
                 }
-                tc_commit(tfull_bar(acc));                // accumulator complete -> epilogue
+                if (ok && elect_one()) tc_commit(tfull_bar(acc));   // accumulator complete -> epilogue
+                __syncwarp();
             }
         }
     } else if (warp == SYNC_WARP) {
