@@ -186,6 +186,14 @@ def run_gf8(args):
     for i, t in enumerate(cfg.tensors):
         if t.side == synth.SIDE_NONE:
             continue
+        if args.synthetic_basis:
+            # profiling aid: seeded orthonormal bases with the configs' i^-2 Ritz values handed to the library,
+            # instead of running a1 + a2 (thousands of small launches) before the timed region
+            for side, d in ((gf8.SIDE_IN, t.d_in), (gf8.SIDE_OUT, t.d_out)):
+                U = synth.rand_orthonormal(d, t.rank, dev, cfg.index, t.layer, t.matrix, 41 + side).contiguous()
+                mu = torch.arange(1, t.rank + 1, device=dev, dtype=torch.float32) ** -2.0
+                ctx.set_basis(i, side, U, mu, 1.0 / t.rank / d + cfg.damping)
+            continue
         X = synth.tensor_factor_samples(cfg, t, "in", dev)
         D = synth.tensor_factor_samples(cfg, t, "out", dev)
         ctx.set_basis(i, gf8.SIDE_IN, synth.tensor_start_basis(cfg, t, "in", dev))
@@ -273,7 +281,8 @@ def run_gf8(args):
     red_bytes = n_el * (R + esz)
     enc_gbs = enc_bytes / (enc_ms * 1e-3) / 1e9
     red_gbs = red_bytes / (red_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "gf8_encode_many (a3-a6), all R ranks", "achieved": enc_gbs, "peak": hbm_peak,
+    roofline = {"bound": "hbm", "kernel": "gf8::tc::tc_items_kernel — the 5 launches of one gf8_encode_many call over all R ranks (a3-a6; 98 % of "
+                          "the call, profiles/r01_launches.md) + the Euclidean tensors' streaming kernels", "achieved": enc_gbs, "peak": hbm_peak,
                 "unit": "GB/s", "frac": enc_gbs / hbm_peak, "traffic": None, "peak_source": which,
                 "algorithmic_bytes_per_launch": enc_bytes, "ms_per_launch": enc_ms,
                 "reduce_decoded": {"achieved": red_gbs, "frac": red_gbs / hbm_peak, "ms": red_ms,
@@ -283,7 +292,7 @@ def run_gf8(args):
                              "frac_of_nominal_8TBps": (enc_bytes + red_bytes) / (ms_step * 1e-3) / 1e9 / 8000.0},
                 "tensor_flops_per_step": (R + 1) * wh_el * 8 * (cfg.tensors[0].rank if cfg.tensors[0].side else 0),
                 }
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    tp = os.path.join(ROOT, "profiles", "r01_traffic.json.txt")
     if os.path.exists(tp):
         try:
             roofline["traffic"] = json.load(open(tp)).get("encode_dram_bytes_per_launch")
@@ -328,7 +337,8 @@ def run_gf8(args):
                                        f"simulated ranks, k={cfg.tensors[0].rank} side BOTH, embedding+LM head Euclidean, "
                                        f"E4M3 per-tensor scale", "precision": args.precision, "layers": args.layers or 24,
                            "l2": "inputs larger than L2 (per-step working set %.1f GB)" % ((R * n_el * (esz + 1) + n_el * esz) / 1e9),
-                           "replicas": "independent replica per GPU, no collective" if world > 1 else "single GPU"},
+                           "replicas": "independent replica per GPU, no collective" if world > 1 else "single GPU",
+                           "geometry": "synthetic bases (set_basis)" if args.synthetic_basis else "factor_update + refresh_basis"},
                 "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
                 "clocks": clocks, "encode_ms": enc_ms, "reduce_decoded_ms": red_ms, "geometry_ms": geo_ms,
                 "setup_s": gen_s}
@@ -350,6 +360,8 @@ def main():
     ap.add_argument("--precision", default="fast", choices=["fast", "exact"])
     ap.add_argument("--refresh-iters", type=int, default=2)
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--synthetic-basis", action="store_true",
+                    help="hand seeded orthonormal bases to the library instead of running factor update + refresh")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
