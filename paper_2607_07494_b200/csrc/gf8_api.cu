@@ -155,6 +155,15 @@ gf8_status ensure_factor(gf8_ctx* c, SideState& s) {
     return dmalloc(c, &s.factor, (size_t)s.d * s.d);
 }
 
+__global__ void fill_kernel(float* p, float v, int n) {
+    if ((int)threadIdx.x < n) p[threadIdx.x] = v;
+}
+// F <- beta F + C
+__global__ void axpby_kernel(float* __restrict__ F, const float* __restrict__ C, float beta, int64_t n) {
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        F[i] = fmaf(beta, F[i], C[i]);
+}
+
 __global__ void widen_kernel(const float* __restrict__ in, int64_t n, double* __restrict__ out) {
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
         out[i] = (double)in[i];
@@ -260,7 +269,7 @@ gf8_status reduce_decoded_one(gf8_ctx* c, int layer, const uint8_t* const* codes
 
 
 // ---- FAST path: batched calls through cached plans of tensor-core items ---------------------------------------
-enum { PLAN_ENCODE = 1, PLAN_DECODE = 2, PLAN_WHITEN = 3 };
+enum { PLAN_ENCODE = 1, PLAN_DECODE = 2, PLAN_WHITEN = 3, PLAN_FACTOR = 4 };
 
 inline void key_ptr(std::vector<uint64_t>& k, const void* p) { k.push_back((uint64_t)(uintptr_t)p); }
 
@@ -430,6 +439,59 @@ gf8_status fast_reduce_decoded_many(gf8_ctx* c, int n, const int* layers, const 
     return GF8_OK;
 }
 
+
+// ---- a1 on the tensor cores: C = alpha X^T X (d x d FP32) for BF16 samples X [T][d] (Eq. 4) -----------
+// Both MMA operands are MN-major views of X (64-row boxes): 128 x 128 output tiles, K = T streamed in 64-row atoms.
+// BF16 products are exact in FP32, so only the accumulation order differs from the FP32 reference (gate G6).
+gf8_status fast_factor_gemm(gf8_ctx* c, cudaStream_t st, const void* X, int64_t T, int d, float alpha, float beta,
+                            float* factor) {
+    using namespace gf8::tc;
+    GF_TRY(fast_init(c));
+    if (!c->fac_alpha) {
+        GF_TRY(dmalloc(c, &c->fac_alpha, 128));
+    }
+    if (beta != 0.0f && c->fac_tmp_cap < (size_t)d * d) {
+        GF_TRY(dmalloc(c, &c->fac_tmp, (size_t)d * d));
+        c->fac_tmp_cap = (size_t)d * d;
+    }
+    std::vector<uint64_t> key = {PLAN_FACTOR, (uint64_t)(uintptr_t)X, (uint64_t)T, (uint64_t)d,
+                                 (uint64_t)(uintptr_t)(beta != 0.0f ? c->fac_tmp : factor)};
+    Plan* p = nullptr;
+    auto found = c->plans.find(key);
+    if (found != c->plans.end()) p = found->second;
+    else {
+        p = new (std::nothrow) Plan();
+        if (!p) return fail(c, GF8_ERR_NOMEM, "host allocation failed");
+        PlanBuilder pb;
+        CUtensorMap mx[2];
+        gf8_status s = make_map(c, mx, X, (uint64_t)T, (uint64_t)d, (uint64_t)d);
+        if (s == GF8_OK) {
+            const int mi = pb.add_map(X, mx);
+            float* out = beta != 0.0f ? c->fac_tmp : factor;
+            for (int i0 = 0; i0 < d; i0 += 128)
+                for (int j0 = 0; j0 < d; j0 += 128) {
+                    Item it = blank_item();
+                    it.map_a[0] = mi; it.map_b[0] = mi; it.atoms[0] = (int)((T + 63) / 64);
+                    it.a_c0[0] = i0; it.b_c0[0] = j0; it.a_mn = 1; it.b_mn = 1; it.N = 128;
+                    it.mode = EPI_STORE; it.out = out; it.out_ld = d; it.out_type = TY_F32; it.colscale = c->fac_alpha;
+                    it.row0 = i0; it.col0 = j0; it.rows = std::min(128, d - i0); it.cols = std::min(128, d - j0);
+                    pb.stage[0].push_back(it);
+                }
+            s = plan_finish(c, pb, p);
+        }
+        if (s == GF8_OK) s = plan_store(c, key, p);
+        if (s != GF8_OK) { plan_free(p); return s; }
+    }
+    fill_kernel<<<1, 128, 0, st>>>(c->fac_alpha, alpha, 128);
+    LAUNCH_CHECK(c);
+    GF_TRY(plan_run_stages(c, st, p));
+    if (beta != 0.0f) {
+        axpby_kernel<<<grid_for(c, (int64_t)d * d, 256, 8), 256, 0, st>>>(factor, c->fac_tmp, beta, (int64_t)d * d);
+        LAUNCH_CHECK(c);
+    }
+    return GF8_OK;
+}
+
 }  // namespace
 
 // =====================================================================================================
@@ -579,7 +641,9 @@ gf8_status gf8_factor_update(gf8_ctx* ctx, int layer, const void* act, const voi
         const float beta = s.has_factor ? L.desc.ema_beta : 0.0f;
         const float alpha = (1.0f - beta) / (float)T;
         const int d = s.d;
-        if (dt == GF8_DT_BF16)
+        if (dt == GF8_DT_BF16 && ctx->precision == GF8_PREC_FAST && d >= 128)
+            GF_TRY(fast_factor_gemm(ctx, st, X, T, d, alpha, beta, s.factor));
+        else if (dt == GF8_DT_BF16)
             GF_TRY((launch_gemm<bf16, bf16, float, float>(ctx, st, (const bf16*)X, 1, d, (const bf16*)X, d, 1, s.factor,
                                                           d, d, d, (int)T, nullptr, nullptr, alpha, beta)));
         else

@@ -81,6 +81,9 @@ struct gf8_ctx {
     std::map<std::vector<uint64_t>, struct Plan*> plans;
     std::vector<struct Plan*> plan_order;
     int* d_err = nullptr;
+    float* fac_alpha = nullptr;      // 128 copies of the factor GEMM's scale (its epilogue's column multipliers)
+    float* fac_tmp = nullptr;        // d x d scratch of the EMA form of the factor update
+    size_t fac_tmp_cap = 0;
     long long* d_prof = nullptr;     // debug profile of the TC kernel (GF8_TC_DBG & 4)
     void* encode_tiled = nullptr;    // cuTensorMapEncodeTiled, resolved at run time (no link-time libcuda)
     bool tc_attr_set = false;

@@ -66,6 +66,7 @@ struct __align__(16) Item {
     int32_t base_type, out_type;
     int32_t write_scale, out_map; // out_map >= 0: the output tile leaves through a TMA store from shared memory
     int32_t base_map[2];          // >= 0: the base tile (hi [+ lo]) is streamed by TMA into shared memory
+    int32_t b_mn, pad1;           // 1: B is MN-major too (the factor GEMM X^T X reads both operands from X)
     int64_t base_ld, out_ld;
     const void* base;
     void* out;
@@ -179,9 +180,10 @@ __device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo, uint3
     return (uint64_t)((addr >> 4) & 0x3FFFu) | ((uint64_t)((lbo >> 4) & 0x3FFFu) << 16) |
            ((uint64_t)((sbo >> 4) & 0x3FFFu) << 32) | (1ull << 46) | (2ull << 61);
 }
-// Instruction descriptor: D = F32, A = B = BF16, M = 128, N, A major-ness; B always K-major.
-__device__ __forceinline__ uint32_t instr_desc(int N, int a_mn) {
-    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)a_mn << 15) | ((uint32_t)(N >> 3) << 17) | ((128u >> 4) << 24);
+// Instruction descriptor: D = F32, A = B = BF16, M = 128, N, A / B major-ness (0 = K-major, 1 = MN-major).
+__device__ __forceinline__ uint32_t instr_desc(int N, int a_mn, int b_mn) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)a_mn << 15) | ((uint32_t)b_mn << 16) | ((uint32_t)(N >> 3) << 17) |
+           ((128u >> 4) << 24);
 }
 
 // ---- epilogue helpers ---------------------------------------------------------------------------------
@@ -600,7 +602,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 const uint32_t slot = n_done % ITEM_SLOTS, iphase = (n_done / ITEM_SLOTS) & 1u;
                 if (!(ok = TWAIT(3, mbar_wait(ifull_bar(slot), iphase, err)))) break;
                 const Item& it = *item_slot(slot);
-                const int a_mn = it.a_mn;
+                const int a_mn = it.a_mn, b_mn = it.b_mn, nbx = it.N >> 6;
                 const uint32_t tx = is_b ? (uint32_t)it.N * 128u : (uint32_t)A_BYTES;
 #pragma unroll 1
                 for (int seg = 0; seg < NSEG && ok; ++seg) {
@@ -615,7 +617,10 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                         const uint32_t sa = smem0 + stage * STAGE_BYTES;
                         if (elect_one()) {
                             mbar_expect_tx(full_bar(stage), tx);
-                            if (is_b) {               // N rows x 64 columns, one box
+                            if (is_b && b_mn) {       // N / 64 boxes of 64 K-rows x 64 contiguous N elements
+                                for (int h = 0; h < nbx; ++h)
+                                    tma_load_2d(sa + A_BYTES + 8192u * h, mp, c0 + 64 * h, r0 + 64 * t, full_bar(stage));
+                            } else if (is_b) {        // N rows x 64 columns, one box
                                 tma_load_2d(sa + A_BYTES, mp, c0 + 64 * t, r0, full_bar(stage));
                             } else if (a_mn) {        // two 64 x 64 boxes: 64 K-rows of 128 contiguous M elements
                                 tma_load_2d(sa, mp, c0, r0 + 64 * t, full_bar(stage));
@@ -641,8 +646,8 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 const uint32_t slot = n_done % ITEM_SLOTS, iphase = (n_done / ITEM_SLOTS) & 1u;
                 if (!(ok = TWAIT(0, mbar_wait(ifull_bar(slot), iphase, err)))) break;
                 const Item& it = *item_slot(slot);
-                const int a_mn = it.a_mn;
-                const uint32_t idesc = instr_desc(it.N, a_mn);
+                const int a_mn = it.a_mn, b_mn = it.b_mn;
+                const uint32_t idesc = instr_desc(it.N, a_mn, b_mn);
                 int total = 0;
 #pragma unroll
                 for (int seg = 0; seg < NSEG; ++seg) total += it.atoms[seg];
@@ -660,7 +665,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
 #pragma unroll
                         for (int kk = 0; kk < 4; ++kk) {
                             const uint64_t da = a_mn ? smem_desc(sa + 2048u * kk, 8192u, 1024u) : smem_desc(sa + 32u * kk, 16u, 1024u);
-                            const uint64_t db = smem_desc(sb + 32u * kk, 16u, 1024u);
+                            const uint64_t db = b_mn ? smem_desc(sb + 2048u * kk, 8192u, 1024u) : smem_desc(sb + 32u * kk, 16u, 1024u);
                             if (!(dbg & 1)) tc_mma_bf16(d, da, db, idesc, (t | kk) ? 1u : 0u);
                         }
                         tc_commit(empty_bar(stage));      // frees the smem stage when these MMAs retire

@@ -240,6 +240,27 @@ def test_fast_fused_update_matches_two_pass(monkeypatch):
         assert torch.equal(codes[r], ref[r][0]) and torch.equal(sinvs[r], ref[r][1])
 
 
+@pytest.mark.parametrize("name", ["ragged-bf16", "wide-k96"])
+def test_fast_g6_factor_on_tensor_cores(name):
+    """a1 on the tcgen05 engine (BF16 samples, both MMA operands MN-major views of X): BF16 products are exact in
+    FP32, so the factor stays within the FP32-accumulation tier of G6; the EMA form goes through the same GEMM."""
+    c = fcase(name)
+    c.ctx.factor_update(0, c.X, c.D)
+    c.ctx.sync_check()
+    assert relfro(to_np64(c.ctx.get_factor(0, gf8.SIDE_IN)), c.A) <= TOL_EXACT
+    assert relfro(to_np64(c.ctx.get_factor(0, gf8.SIDE_OUT)), c.Gf) <= TOL_EXACT
+    f = c.ctx.get_factor(0, gf8.SIDE_IN)
+    assert torch.equal(f, f.t())                      # X^T X: tile (i, j) and tile (j, i) sum the same products
+    lay = gf8.Layer(c.m, c.n, c.side, c.kA, c.kG, c.fmt, c.scaling, c.damping, 0.75)
+    ctx = gf8.create([lay], gf8.PREC_FAST)
+    X2 = synth.factor_samples(c.X.shape[0], c.n, "cuda", 123, 1).to(torch.bfloat16)
+    ctx.factor_update(0, c.X, c.D)
+    ctx.factor_update(0, X2, c.D)
+    ctx.sync_check()
+    want = oracle.factor_accumulate(to_np64(X2), oracle.factor_accumulate(to_np64(c.X)), 0.75)
+    assert relfro(to_np64(ctx.get_factor(0, gf8.SIDE_IN)), want) <= TOL_EXACT
+
+
 def test_euclidean_layer_is_plain_fp8():
     """side = NONE (embedding / LM head): codes and decoded values bit-exact."""
     m, n = 400, 256
