@@ -169,47 +169,58 @@ __global__ void widen_kernel(const float* __restrict__ in, int64_t n, double* __
         out[i] = (double)in[i];
 }
 
+gf8_status alloc_refresh_scratch(gf8_ctx* c, RefreshScratch& r) {
+    if (r.V) return GF8_OK;
+    GF_TRY(dmalloc(c, &r.V, c->rs_dk));
+    GF_TRY(dmalloc(c, &r.Y, c->rs_dk));
+    GF_TRY(dmalloc(c, &r.Gm, c->rs_k * c->rs_k));
+    GF_TRY(dmalloc(c, &r.Bm, c->rs_k * c->rs_k));
+    GF_TRY(dmalloc(c, &r.Zm, c->rs_k * c->rs_k));
+    GF_TRY(dmalloc(c, &r.Zs, c->rs_k * c->rs_k));
+    return dmalloc(c, &r.mu64, c->rs_k);
+}
+
 // CholeskyQR in FP64, applied twice (V d x k, in place).
-gf8_status orthonormalise(gf8_ctx* c, cudaStream_t st, double* V, int d, int k) {
+gf8_status orthonormalise(gf8_ctx* c, cudaStream_t st, RefreshScratch& rs, double* V, int d, int k) {
     for (int pass = 0; pass < 2; ++pass) {
-        GF_TRY((launch_gemm<double, double, double, double>(c, st, V, 1, k, V, k, 1, c->Gm, k, k, k, d, nullptr, nullptr,
+        GF_TRY((launch_gemm<double, double, double, double>(c, st, V, 1, k, V, k, 1, rs.Gm, k, k, k, d, nullptr, nullptr,
                                                             1.0, 0.0, pick_splits(c, k, k, d))));
-        cholesky_upper_kernel<<<1, 1024, 0, st>>>(c->Gm, k);
+        cholesky_upper_kernel<<<1, 1024, 0, st>>>(rs.Gm, k);
         LAUNCH_CHECK(c);
-        trisolve_rows_kernel<<<(d + 127) / 128, 128, 0, st>>>(V, c->Gm, d, k);
+        trisolve_rows_kernel<<<(d + 127) / 128, 128, 0, st>>>(V, rs.Gm, d, k);
         LAUNCH_CHECK(c);
     }
     return GF8_OK;
 }
 
-gf8_status refresh_side(gf8_ctx* c, cudaStream_t st, SideState& s, double lam, int n_iter, int layer) {
+gf8_status refresh_side(gf8_ctx* c, cudaStream_t st, RefreshScratch& rs, SideState& s, double lam, int n_iter, int layer) {
     if (!s.has_factor) return fail(c, GF8_ERR_BAD_STATE, "layer %d: no factor accumulated yet", layer);
     if (!s.has_start) return fail(c, GF8_ERR_BAD_STATE, "layer %d: no start basis (gf8_set_basis first)", layer);
     const int d = s.d, k = s.k;
-    double *V = c->V, *Y = c->Y;
+    double *V = rs.V, *Y = rs.Y;
     widen_kernel<<<grid_for(c, (int64_t)d * k, 256, 4), 256, 0, st>>>(s.U, (int64_t)d * k, V);
     LAUNCH_CHECK(c);
-    GF_TRY(orthonormalise(c, st, V, d, k));
+    GF_TRY(orthonormalise(c, st, rs, V, d, k));
     for (int it = 0; it < n_iter; ++it) {
         GF_TRY((launch_gemm<float, double, double, double>(c, st, s.factor, d, 1, V, k, 1, Y, k, d, k, d, nullptr,
                                                            nullptr, 1.0, 0.0, pick_splits(c, d, k, d))));
         double* t = V; V = Y; Y = t;
-        GF_TRY(orthonormalise(c, st, V, d, k));
+        GF_TRY(orthonormalise(c, st, rs, V, d, k));
     }
     // Rayleigh-Ritz: Y = A V, B = V^T Y
     GF_TRY((launch_gemm<float, double, double, double>(c, st, s.factor, d, 1, V, k, 1, Y, k, d, k, d, nullptr, nullptr,
                                                        1.0, 0.0, pick_splits(c, d, k, d))));
-    GF_TRY((launch_gemm<double, double, double, double>(c, st, V, 1, k, Y, k, 1, c->Bm, k, k, k, d, nullptr, nullptr,
+    GF_TRY((launch_gemm<double, double, double, double>(c, st, V, 1, k, Y, k, 1, rs.Bm, k, k, k, d, nullptr, nullptr,
                                                         1.0, 0.0, pick_splits(c, k, k, d))));
     const size_t smem = 2 * (size_t)k * k * sizeof(double);
     const int use_smem = smem <= 200 * 1024 ? 1 : 0;
     if (use_smem) CU_TRY(c, cudaFuncSetAttribute(jacobi_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    jacobi_kernel<<<1, 1024, use_smem ? smem : 0, st>>>(c->Bm, c->Zm, k, use_smem, c->mu64, c->Zs, 60);
+    jacobi_kernel<<<1, 1024, use_smem ? smem : 0, st>>>(rs.Bm, rs.Zm, k, use_smem, rs.mu64, rs.Zs, 60);
     LAUNCH_CHECK(c);
     // U = V Zs (FP32 out)
-    GF_TRY((launch_gemm<double, double, float, double>(c, st, V, k, 1, c->Zs, k, 1, s.U, k, d, k, k, nullptr, nullptr,
+    GF_TRY((launch_gemm<double, double, float, double>(c, st, V, k, 1, rs.Zs, k, 1, s.U, k, d, k, k, nullptr, nullptr,
                                                        1.0, 0.0)));
-    multipliers_kernel<<<1, 256, 0, st>>>(s.factor, d, k, c->mu64, nullptr, lam, 0.0, s.mu, s.e, s.ebar, s.rho);
+    multipliers_kernel<<<1, 256, 0, st>>>(s.factor, d, k, rs.mu64, nullptr, lam, 0.0, s.mu, s.e, s.ebar, s.rho);
     LAUNCH_CHECK(c);
     GF_TRY(fast_pack_basis(c, st, s));
     s.has_basis = true;
@@ -456,9 +467,11 @@ gf8_status fast_factor_gemm(gf8_ctx* c, cudaStream_t st, const void* X, int64_t 
     }
     std::vector<uint64_t> key = {PLAN_FACTOR, (uint64_t)(uintptr_t)X, (uint64_t)T, (uint64_t)d,
                                  (uint64_t)(uintptr_t)(beta != 0.0f ? c->fac_tmp : factor)};
+    // factor plans live in their own small cache: sample buffers change from refresh to refresh and must not
+    // evict the per-step encode / decode plans
     Plan* p = nullptr;
-    auto found = c->plans.find(key);
-    if (found != c->plans.end()) p = found->second;
+    auto found = c->fac_plans.find(key);
+    if (found != c->fac_plans.end()) p = found->second;
     else {
         p = new (std::nothrow) Plan();
         if (!p) return fail(c, GF8_ERR_NOMEM, "host allocation failed");
@@ -479,8 +492,13 @@ gf8_status fast_factor_gemm(gf8_ctx* c, cudaStream_t st, const void* X, int64_t 
                 }
             s = plan_finish(c, pb, p);
         }
-        if (s == GF8_OK) s = plan_store(c, key, p);
         if (s != GF8_OK) { plan_free(p); return s; }
+        if (c->fac_plans.size() >= 32) {
+            CU_TRY(c, cudaDeviceSynchronize());
+            for (auto& kv : c->fac_plans) plan_free(kv.second);
+            c->fac_plans.clear();
+        }
+        c->fac_plans[key] = p;
     }
     fill_kernel<<<1, 128, 0, st>>>(c->fac_alpha, alpha, 128);
     LAUNCH_CHECK(c);
@@ -589,10 +607,8 @@ gf8_status gf8_create(gf8_ctx** out, int device, const gf8_layer_desc* layers, i
     }
     if (s == GF8_OK && max_mn) s = dmalloc(c, &c->wt_scratch, max_mn);
     if (s == GF8_OK && max_dk) {
-        if ((s = dmalloc(c, &c->V, max_dk)) == GF8_OK && (s = dmalloc(c, &c->Y, max_dk)) == GF8_OK &&
-            (s = dmalloc(c, &c->Gm, max_k * max_k)) == GF8_OK && (s = dmalloc(c, &c->Bm, max_k * max_k)) == GF8_OK &&
-            (s = dmalloc(c, &c->Zm, max_k * max_k)) == GF8_OK && (s = dmalloc(c, &c->Zs, max_k * max_k)) == GF8_OK)
-            s = dmalloc(c, &c->mu64, max_k);
+        c->rs_dk = max_dk; c->rs_k = max_k;
+        s = alloc_refresh_scratch(c, c->rs[0]);
     }
     if (s != GF8_OK) { gf8_destroy(c); return s; }
     *out = c;
@@ -605,7 +621,13 @@ gf8_status gf8_destroy(gf8_ctx* ctx) {
     cudaDeviceSynchronize();
     for (void* p : ctx->allocs) cudaFree(p);
     for (void* p : ctx->stage_allocs) cudaFree(p);
+    for (int q = 0; q < GF8_REFRESH_STREAMS; ++q) {
+        if (ctx->rs_stream[q]) cudaStreamDestroy(ctx->rs_stream[q]);
+        if (ctx->rs_ev[q]) cudaEventDestroy(ctx->rs_ev[q]);
+    }
+    if (ctx->rs_fork) cudaEventDestroy(ctx->rs_fork);
     for (Plan* p : ctx->plan_order) plan_free(p);
+    for (auto& kv : ctx->fac_plans) plan_free(kv.second);
     for (LayerState& L : ctx->layers)
         for (Slot* sl : L.slots) delete sl;
     delete ctx;
@@ -660,8 +682,8 @@ gf8_status gf8_refresh_basis(gf8_ctx* ctx, int layer, int n_iter, void* stream) 
     if (n_iter < 0 || n_iter > 1000) return fail(ctx, GF8_ERR_INVALID_ARG, "n_iter out of range");
     LayerState& L = ctx->layers[layer];
     CU_TRY(ctx, cudaSetDevice(ctx->device));
-    if (L.in.used) GF_TRY(refresh_side(ctx, (cudaStream_t)stream, L.in, (double)L.desc.damping, n_iter, layer));
-    if (L.out.used) GF_TRY(refresh_side(ctx, (cudaStream_t)stream, L.out, (double)L.desc.damping, n_iter, layer));
+    if (L.in.used) GF_TRY(refresh_side(ctx, (cudaStream_t)stream, ctx->rs[0], L.in, (double)L.desc.damping, n_iter, layer));
+    if (L.out.used) GF_TRY(refresh_side(ctx, (cudaStream_t)stream, ctx->rs[0], L.out, (double)L.desc.damping, n_iter, layer));
     return GF8_OK;
 }
 
@@ -743,7 +765,35 @@ gf8_status gf8_factor_update_many(gf8_ctx* ctx, int n, const int* layers, const 
 gf8_status gf8_refresh_basis_many(gf8_ctx* ctx, int n, const int* layers, int n_iter, void* stream) {
     if (!ctx) return GF8_ERR_INVALID_ARG;
     if (n < 0 || !layers) return fail(ctx, GF8_ERR_INVALID_ARG, "null argument");
-    for (int i = 0; i < n; ++i) GF_TRY(gf8_refresh_basis(ctx, layers[i], n_iter, stream));
+    if (n_iter < 0 || n_iter > 1000) return fail(ctx, GF8_ERR_INVALID_ARG, "n_iter out of range");
+    for (int i = 0; i < n; ++i) GF_TRY(check_layer(ctx, layers[i]));
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    // The refresh of one factor is a chain of small, latency-bound launches (CholeskyQR, a single-CTA Jacobi, skinny
+    // products): independent factors run concurrently on the context's side streams, each with its own scratch.
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!ctx->rs_ev[0]) {
+        for (int q = 0; q < GF8_REFRESH_STREAMS; ++q) {
+            CU_TRY(ctx, cudaStreamCreateWithFlags(&ctx->rs_stream[q], cudaStreamNonBlocking));
+            CU_TRY(ctx, cudaEventCreateWithFlags(&ctx->rs_ev[q], cudaEventDisableTiming));
+        }
+        CU_TRY(ctx, cudaEventCreateWithFlags(&ctx->rs_fork, cudaEventDisableTiming));
+    }
+    for (int q = 0; q < GF8_REFRESH_STREAMS; ++q) GF_TRY(alloc_refresh_scratch(ctx, ctx->rs[q]));
+    CU_TRY(ctx, cudaEventRecord(ctx->rs_fork, st));
+    for (int q = 0; q < GF8_REFRESH_STREAMS; ++q) CU_TRY(ctx, cudaStreamWaitEvent(ctx->rs_stream[q], ctx->rs_fork, 0));
+    int job = 0;
+    for (int i = 0; i < n; ++i) {
+        LayerState& L = ctx->layers[layers[i]];
+        for (SideState* sd : {&L.in, &L.out}) {
+            if (!sd->used) continue;
+            const int q = job++ % GF8_REFRESH_STREAMS;
+            GF_TRY(refresh_side(ctx, ctx->rs_stream[q], ctx->rs[q], *sd, (double)L.desc.damping, n_iter, layers[i]));
+        }
+    }
+    for (int q = 0; q < GF8_REFRESH_STREAMS; ++q) {
+        CU_TRY(ctx, cudaEventRecord(ctx->rs_ev[q], ctx->rs_stream[q]));
+        CU_TRY(ctx, cudaStreamWaitEvent(st, ctx->rs_ev[q], 0));
+    }
     return GF8_OK;
 }
 

@@ -63,14 +63,23 @@ struct LayerState {
 
 }  // namespace
 
+constexpr int GF8_REFRESH_STREAMS = 16;
+struct RefreshScratch {
+    double *V = nullptr, *Y = nullptr, *Gm = nullptr, *Bm = nullptr, *Zm = nullptr, *Zs = nullptr, *mu64 = nullptr;
+};
+
 struct gf8_ctx {
     int device = 0;
     gf8_precision precision = GF8_PREC_EXACT;
     std::vector<LayerState> layers;
     std::vector<void*> allocs;
     float* wt_scratch = nullptr;     // max m*n FP32
-    // refresh scratch (FP64)
-    double *V = nullptr, *Y = nullptr, *Gm = nullptr, *Bm = nullptr, *Zm = nullptr, *Zs = nullptr, *mu64 = nullptr;
+    // refresh scratch (FP64): one set per concurrent refresh stream (gf8_refresh_basis_many); set 0 serves single calls
+    RefreshScratch rs[GF8_REFRESH_STREAMS];
+    size_t rs_dk = 0, rs_k = 0;
+    cudaStream_t rs_stream[GF8_REFRESH_STREAMS] = {};
+    cudaEvent_t rs_ev[GF8_REFRESH_STREAMS] = {};
+    cudaEvent_t rs_fork = nullptr;
     // tap scratch (gf8_quantize_f32 with arbitrary shapes)
     uint32_t* tap_amax = nullptr; float* tap_scale = nullptr; size_t tap_cap = 0;
     // host-step staging
@@ -80,6 +89,7 @@ struct gf8_ctx {
     // FAST path: cached launch plans (device item lists + tensor maps), error flag, driver entry point
     std::map<std::vector<uint64_t>, struct Plan*> plans;
     std::vector<struct Plan*> plan_order;
+    std::map<std::vector<uint64_t>, struct Plan*> fac_plans;   // factor-GEMM plans (keyed by the sample buffer)
     int* d_err = nullptr;
     float* fac_alpha = nullptr;      // 128 copies of the factor GEMM's scale (its epilogue's column multipliers)
     float* fac_tmp = nullptr;        // d x d scratch of the EMA form of the factor update

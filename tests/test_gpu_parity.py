@@ -261,6 +261,29 @@ def test_fast_g6_factor_on_tensor_cores(name):
     assert relfro(to_np64(ctx.get_factor(0, gf8.SIDE_IN)), want) <= TOL_EXACT
 
 
+def test_refresh_basis_many_matches_single_calls():
+    """gf8_refresh_basis_many (independent factors on concurrent streams, own scratch each) == one call per layer."""
+    shapes = [(256, 384, 16), (320, 256, 24), (384, 448, 8), (256, 256, 32)]
+    lays = [gf8.Layer(m, n, gf8.SIDE_BOTH, k, k) for m, n, k in shapes]
+    ctxs = [gf8.create(lays), gf8.create(lays)]
+    for i, (m, n, k) in enumerate(shapes):
+        X = synth.factor_samples(1024, n, "cuda", 31, i)
+        D = synth.factor_samples(1024, m, "cuda", 32, i)
+        for c in ctxs:
+            c.factor_update(i, X, D)
+            c.set_basis(i, gf8.SIDE_IN, synth.start_basis(n, k, "cuda", 33, i))
+            c.set_basis(i, gf8.SIDE_OUT, synth.start_basis(m, k, "cuda", 34, i))
+    for i in range(len(shapes)):
+        ctxs[0].refresh_basis(i, 3)
+    ctxs[1].refresh_basis_many(list(range(len(shapes))), 3)
+    torch.cuda.synchronize()
+    for i in range(len(shapes)):
+        for side in (gf8.SIDE_IN, gf8.SIDE_OUT):
+            U0, mu0, rho0 = ctxs[0].get_basis(i, side)
+            U1, mu1, rho1 = ctxs[1].get_basis(i, side)
+            assert torch.equal(U0, U1) and torch.equal(mu0, mu1) and rho0 == rho1
+
+
 def test_euclidean_layer_is_plain_fp8():
     """side = NONE (embedding / LM head): codes and decoded values bit-exact."""
     m, n = 400, 256
