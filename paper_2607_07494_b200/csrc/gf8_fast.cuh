@@ -420,9 +420,13 @@ gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
         // shared-memory split: update stages keep a short operand ring (their operands are L2-resident) and give
         // the rest to base tiles in flight (the HBM stream); panel stages give everything to the operand ring
         const int fuse = s == 5 ? 1 : 0;
-        int n_stages = n_base ? 3 : gf8::tc::MAX_STAGES, dbg = 0, only = -1;
+        // Bytes in flight per SM are what hides the load latency (Little's law), so the 7 x 32 KB are split in
+        // proportion to what a tile needs: an encode update tile loads 64 KB of operands + 32 KB of base.
+        int n_stages = n_base ? (fuse ? 3 : 5) : gf8::tc::MAX_STAGES, dbg = 0, only = -1;
+        if (const char* e = getenv("GF8_TC_RING")) n_stages = std::max(2, std::min(6, atoi(e)));
         // (the fused stage gives one base slot's worth of shared memory to its two code-tile staging buffers)
-        const int n_bslots = fuse ? 3 : (n_base ? (gf8::tc::MAX_STAGES - n_stages) / n_base : 1);
+        const int n_bslots = fuse ? 3 : (n_base ? std::max(1, (gf8::tc::MAX_STAGES - n_stages) / n_base) : 1);
+        if (n_base && !fuse && n_stages + n_bslots * n_base > gf8::tc::MAX_STAGES) n_stages = gf8::tc::MAX_STAGES - n_bslots * n_base;
         if (fuse && grid < c->num_sms && p->stage_cnt[s] > grid) return fail(c, GF8_ERR_BAD_STATE, "fused stage needs a full grid");
         if (const char* e = getenv("GF8_TC_DBG")) dbg = atoi(e);
         if (!first_run) dbg |= 2;        // tensor maps are written once by the host before the plan's first launch

@@ -519,7 +519,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
     auto parked_bar = [&](int a) { return bars + 8u * (2 * MAX_STAGES + 8 + 2 * MAX_BASE_SLOTS + 2 * ITEM_SLOTS + a); };
     auto sready_bar = [&](int a) { return bars + 8u * (2 * MAX_STAGES + 8 + 2 * MAX_BASE_SLOTS + 2 * ITEM_SLOTS + 4 + a); };
     float* s_scale = reinterpret_cast<float*>(s_red + 8);     // fused update: scale of each parked tile's tensor
-    const uint32_t n_acc = fuse ? 4u : 2u;           // TMEM accumulator slots in rotation
+    const uint32_t n_acc = 4u;                       // TMEM accumulator slots in rotation (4 x 128 columns)
     auto base_tile = [&](uint32_t b) { return base0 + b * (uint32_t)n_base * TILE_BYTES; };
     auto item_slot = [&](uint32_t s) { return reinterpret_cast<const Item*>(s_items + s * ITEM_BYTES); };
 
