@@ -12,8 +12,10 @@
 struct Plan {
     CUtensorMap* d_maps = nullptr;
     gf8::tc::Item* d_items = nullptr;
-    int stage_off[6] = {0, 0, 0, 0, 0, 0}, stage_cnt[6] = {0, 0, 0, 0, 0, 0};
-    int stage_base[6] = {0, 0, 0, 0, 0, 0};  // streamed base tiles per item in that stage's launch (0, 1 or 2)
+    // stages: 0 P', 1 Q^T (+S), 2 Q'^T, 3 update tiles (amax / block cast / store), 4 update tiles (cast),
+    //         5 update strips (amax / block cast), 6 update strips (cast), 7 fused update (opt-in)
+    int stage_off[8] = {0, 0, 0, 0, 0, 0, 0, 0}, stage_cnt[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    int stage_base[8] = {0, 0, 0, 0, 0, 0, 0, 0};  // streamed base tiles per item in that stage's launch (0, 1 or 2)
     int runs = 0;                        // launches so far: the first one acquires its tensor maps with proxy fences
     uint32_t* d_amax = nullptr;          // one word per TC problem (per-tensor scaling)
     size_t n_amax = 0;
@@ -190,7 +192,7 @@ gf8_status fast_slot(gf8_ctx* c, LayerState& L, size_t idx, bool need_src16, boo
 struct PlanBuilder {
     std::vector<CUtensorMap> maps;
     std::map<const void*, int> map_index;      // buffer -> index (static maps are shared by all problems)
-    std::vector<Item> stage[6];
+    std::vector<Item> stage[8];
     // registers both box heights of a buffer; returns the index of the 64-row-box map, +1 is the 128-row-box map
     int add_map(const void* key, const CUtensorMap* m2) {
         auto it = map_index.find(key);
@@ -325,6 +327,31 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
     }
     // rank-(kA + kG) update of the streamed base tile
     const int tiles_n = (n + 127) / 128;
+    // Strip items (encode, K = kpA + kpG <= 128): one item = up to 256 rows x all columns; its A tiles [P' | U_G] stay
+    // resident in shared memory and every B K-atom [U_A | Q'^T] serves both row blocks, which halves the bytes TMA has
+    // to bring in per output tile (96 KB -> 48 KB) and amortises the per-item hand-shakes over 2 x n / 128 tiles.
+    if (!split && kpA + kpG <= 128 && f.base_map[0] >= 0 && f.base_map[1] < 0 && f.out_map >= 0 &&
+        (f.mode == EPI_AMAX || f.mode == EPI_BLOCKCAST) && !getenv("GF8_TC_NOSTRIP") && !getenv("GF8_TC_FUSE")) {
+        for (int i0 = 0; i0 < m; i0 += 256) {
+            Item it = blank_item();
+            int seg = 0;
+            it.N = 128; it.fmt = f.fmt; it.strip = 1;
+            if (useA) add_product(it, seg, mPp, mUA, kpA / 64, 0, i0, 0, 0);
+            if (useG) add_product(it, seg, mUG, mQpt, kpG / 64, 0, i0, 0, 0);
+            it.base_type = f.base_type; it.base_map[0] = f.base_map[0] + 1;
+            it.row0 = i0; it.col0 = 0; it.rows = std::min(256, m - i0); it.cols = n;
+            it.mode = f.mode; it.out = f.out; it.out_ld = n; it.out_map = f.out_map; it.scale_inv_out = f.scale_inv;
+            if (f.mode == EPI_AMAX) {
+                it.amax = f.amax;
+                pb.stage[5].push_back(it);
+                it.mode = EPI_CAST; it.write_scale = i0 == 0 ? 1 : 0;
+                pb.stage[6].push_back(it);
+            } else {
+                pb.stage[5].push_back(it);
+            }
+        }
+        return;
+    }
     for (int i0 = 0; i0 < m; i0 += 128)
         for (int j0 = 0; j0 < n; j0 += 128) {
             Item it = blank_item();
@@ -345,7 +372,7 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
                 it.amax = f.amax; it.out = f.out; it.out_ld = n; it.scale_inv_out = f.scale_inv; it.out_map = f.out_map;
                 it.write_scale = (i0 == 0 && j0 == 0) ? 1 : 0;
                 it.base = f.done; it.base_ld = n_tiles;
-                pb.stage[5].push_back(it);
+                pb.stage[7].push_back(it);
             } else if (f.mode == EPI_AMAX) {
                 it.amax = f.amax;
                 pb.stage[3].push_back(it);
@@ -374,10 +401,12 @@ void plan_free(Plan* p) {
 // Upload the builder's maps and items (longest contractions first within a stage: CTAs take items round-robin).
 gf8_status plan_finish(gf8_ctx* c, PlanBuilder& pb, Plan* p) {
     std::vector<Item> all;
-    for (int s = 0; s < 6; ++s) {
+    for (int s = 0; s < 8; ++s) {
         std::stable_sort(pb.stage[s].begin(), pb.stage[s].end(), [](const Item& a, const Item& b) {
-            int ta = 0, tb = 0;
+            int64_t ta = 0, tb = 0;
             for (int g = 0; g < gf8::tc::NSEG; ++g) { ta += a.atoms[g]; tb += b.atoms[g]; }
+            if (a.strip) ta *= (int64_t)((a.rows + 127) / 128) * ((a.cols + 127) / 128);
+            if (b.strip) tb *= (int64_t)((b.rows + 127) / 128) * ((b.cols + 127) / 128);
             return ta > tb;
         });
         p->stage_off[s] = (int)all.size();
@@ -413,17 +442,16 @@ gf8_status plan_store(gf8_ctx* c, const std::vector<uint64_t>& key, Plan* p) {
 
 gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
     const bool first_run = p->runs++ == 0;
-    for (int s = 0; s < 6; ++s) {
+    for (int s = 0; s < 8; ++s) {
         if (!p->stage_cnt[s]) continue;
         const int grid = std::min(p->stage_cnt[s], c->num_sms);
         const int n_base = p->stage_base[s];
         // shared-memory split: update stages keep a short operand ring (their operands are L2-resident) and give
         // the rest to base tiles in flight (the HBM stream); panel stages give everything to the operand ring
-        const int fuse = s == 5 ? 1 : 0;
-        // Bytes in flight per SM are what hides the load latency (Little's law), so the 7 x 32 KB are split in
-        // proportion to what a tile needs: an encode update tile loads 64 KB of operands + 32 KB of base.
-        int n_stages = n_base ? (fuse ? 3 : 5) : gf8::tc::MAX_STAGES, dbg = 0, only = -1;
-        if (const char* e = getenv("GF8_TC_RING")) n_stages = std::max(2, std::min(6, atoi(e)));
+        const int fuse = s == 7 ? 1 : 0, strip = (s == 5 || s == 6) ? 1 : 0, kmode = fuse ? 1 : (strip ? 2 : 0);
+        // shared-memory split of the tile-mode update stages: 3 operand stages + the rest as base tiles in flight
+        int n_stages = n_base ? (strip ? 4 : 3) : gf8::tc::MAX_STAGES, dbg = 0, only = -1;
+        // (strip stages: 64 KB of resident A tiles + 4 x 16 KB of B atoms = the first four 32 KB units, then 3 base slots)
         // (the fused stage gives one base slot's worth of shared memory to its two code-tile staging buffers)
         const int n_bslots = fuse ? 3 : (n_base ? std::max(1, (gf8::tc::MAX_STAGES - n_stages) / n_base) : 1);
         if (n_base && !fuse && n_stages + n_bslots * n_base > gf8::tc::MAX_STAGES) n_stages = gf8::tc::MAX_STAGES - n_bslots * n_base;
@@ -433,7 +461,7 @@ gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
         if (const char* e = getenv("GF8_TC_ONLY")) only = atoi(e);
         if (only >= 0 && only != s) continue;
         gf8::tc::tc_items_kernel<<<grid, gf8::tc::THREADS, gf8::tc::SMEM_BYTES, st>>>(
-            p->d_items + p->stage_off[s], p->stage_cnt[s], p->d_maps, c->d_err, n_stages, n_base, n_bslots, fuse, dbg, (dbg & 4) ? c->d_prof : nullptr);
+            p->d_items + p->stage_off[s], p->stage_cnt[s], p->d_maps, c->d_err, n_stages, n_base, n_bslots, kmode, dbg, (dbg & 4) ? c->d_prof : nullptr);
         if (dbg & 4) {
             std::vector<long long> h((size_t)c->num_sms * 18);
             cudaMemcpy(h.data(), c->d_prof, h.size() * sizeof(long long), cudaMemcpyDeviceToHost);

@@ -43,6 +43,8 @@ constexpr int TMEM_COLS = 512;                   // four 128-column accumulator 
 constexpr int FUSE_LAG = 2;                      // fused update: tiles parked in TMEM while the tensor amax completes
                                                  // (2 parked + 1 in the epilogue + 1 under the MMAs = 4 slots)
 constexpr int CODE_TILE_BYTES = 128 * 128;       // staging of one 128 x 128 FP8 code tile
+constexpr int STRIP_L_BYTES = 4 * A_BYTES;       // strip mode: resident A tiles, [row block 0/1][K-atom 0/1]
+constexpr int STRIP_RING = 4;                    // strip mode: ring of 16 KB B K-atoms
 constexpr int NSEG = 6;                          // operand segments per item (hi/lo split products)
 
 enum Epi : int32_t {
@@ -66,7 +68,8 @@ struct __align__(16) Item {
     int32_t base_type, out_type;
     int32_t write_scale, out_map; // out_map >= 0: the output tile leaves through a TMA store from shared memory
     int32_t base_map[2];          // >= 0: the base tile (hi [+ lo]) is streamed by TMA into shared memory
-    int32_t b_mn, pad1;           // 1: B is MN-major too (the factor GEMM X^T X reads both operands from X)
+    int32_t b_mn;                 // 1: B is MN-major too (the factor GEMM X^T X reads both operands from X)
+    int32_t strip;                // 1: strip item of the update (up to 256 rows x all columns; see tc_items_kernel)
     int64_t base_ld, out_ld;
     const void* base;
     void* out;
@@ -395,7 +398,10 @@ __device__ __forceinline__ void tile_values32(uint32_t taddr, uint32_t row, int 
 // Returns true if a TMA store was issued from `tile` (the caller waits for its smem reads before reuse).
 // Each warp covers 32 rows x 64 columns (its half) as four 16-column chunks.
 __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc, uint32_t tile, int n_base, int warp,
-                                              int lane, uint32_t* s_red, const CUtensorMap* maps, uint32_t amax_bits) {
+                                              int lane, uint32_t* s_red, const CUtensorMap* maps, uint32_t amax_bits,
+                                              int row0, int col0, bool write_scale, float* sinv_out, uint32_t* run_max) {
+    // (row0, col0) = the tile's origin: the item's own for tile items, a tile of the strip for strip items;
+    // run_max != null: EPI_AMAX accumulates into the caller's per-thread running maximum (one atomic per strip)
     const int r = (warp & 3) * 32 + lane, half = warp >> 2, cbase = half * 64;
     const uint32_t taddr = tmem_acc + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)cbase;
     const uint32_t row = tile + (uint32_t)half * 16384u + (uint32_t)r * 128u;
@@ -411,6 +417,7 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
             for (int u = 0; u < 32; ++u) loc = max(loc, __float_as_uint(v[u]) & 0x7FFFFFFFu);
         }
         if (mode == EPI_AMAX) {
+            if (run_max) { *run_max = max(*run_max, loc); return false; }
             loc = warp_max_u32(loc);
             if (lane == 0 && loc != 0u) atomicMax(it.amax, loc);
             return false;
@@ -418,11 +425,11 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
         const uint32_t bits = epi_block_max(loc, warp, lane, s_red);
         float si;
         scales_from_amax(bits, fmt == 0 ? 448.0f : 57344.0f, scale, si);
-        if (r == 0 && half == 0) *it.scale_inv_out = si;
+        if (r == 0 && half == 0) *sinv_out = si;
     } else if (mode == EPI_CAST) {
         float si;
         scales_from_amax(amax_bits, fmt == 0 ? 448.0f : 57344.0f, scale, si);
-        if (it.write_scale && r == 0 && half == 0) *it.scale_inv_out = si;
+        if (write_scale && r == 0 && half == 0) *sinv_out = si;
     }
     if (mode == EPI_CAST || mode == EPI_BLOCKCAST) {
         // 64 codes of this row half; the 128 x 128-byte code tile then overwrites the (consumed) first half of
@@ -441,7 +448,7 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         epi_sync();
         if (threadIdx.x == 0) {
-            tma_store_2d(maps + it.out_map, tile, it.col0, it.row0);
+            tma_store_2d(maps + it.out_map, tile, col0, row0);
             asm volatile("cp.async.bulk.commit_group;" ::: "memory");
         }
         return true;
@@ -466,7 +473,7 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
         epi_sync();
         if (threadIdx.x == 0) {
 #pragma unroll
-            for (int h = 0; h < 2; ++h) tma_store_2d(maps + it.out_map, tile + h * 16384u, it.col0 + 64 * h, it.row0);
+            for (int h = 0; h < 2; ++h) tma_store_2d(maps + it.out_map, tile + h * 16384u, col0 + 64 * h, row0);
             asm volatile("cp.async.bulk.commit_group;" ::: "memory");
         }
         return true;
@@ -479,7 +486,7 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
         for (int q = 0; q < 2; ++q) {
             const int c0 = cbase + 32 * g + 16 * q;
             if (!row_ok || c0 >= it.cols) continue;
-            float4* o = reinterpret_cast<float4*>(reinterpret_cast<float*>(it.out) + (int64_t)(it.row0 + r) * it.out_ld + it.col0 + c0);
+            float4* o = reinterpret_cast<float4*>(reinterpret_cast<float*>(it.out) + (int64_t)(row0 + r) * it.out_ld + col0 + c0);
 #pragma unroll
             for (int u = 0; u < 4; ++u)
                 o[u] = make_float4(v[16 * q + 4 * u], v[16 * q + 4 * u + 1], v[16 * q + 4 * u + 2], v[16 * q + 4 * u + 3]);
@@ -496,9 +503,11 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
 // so a pipeline bug cannot hang the GPU.
 __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __restrict__ items, int n_items,
                                                               const CUtensorMap* __restrict__ maps, int* err,
-                                                              int n_stages, int n_base, int n_bslots, int fuse, int dbg,
+                                                              int n_stages, int n_base, int n_bslots, int kmode, int dbg,
                                                               long long* __restrict__ prof) {
     extern __shared__ uint8_t smem_raw[];
+    const int fuse = kmode == 1 ? 1 : 0;           // kmode: 0 = tile items, 1 = fused update (TMEM-parked), 2 = strip items
+    const bool strip = kmode == 2;
     const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;          // 1024-byte aligned (swizzle atoms)
     const uint32_t base0 = smem0 + (uint32_t)n_stages * STAGE_BYTES;        // base tiles: [acc][n_base] x 32 KB
     const uint32_t bars = smem0 + DATA_BYTES;
@@ -524,7 +533,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
     auto item_slot = [&](uint32_t s) { return reinterpret_cast<const Item*>(s_items + s * ITEM_BYTES); };
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < MAX_STAGES; ++s) { mbar_init(full_bar(s), 2); mbar_init(empty_bar(s), 1); }
+        for (int s = 0; s < MAX_STAGES; ++s) { mbar_init(full_bar(s), strip ? 1 : 2); mbar_init(empty_bar(s), 1); }
         for (int a = 0; a < 4; ++a) {
             mbar_init(parked_bar(a), 1); mbar_init(sready_bar(a), 1);
             mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), EPI_WARPS);
@@ -550,7 +559,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
     if (warp == PRODUCER_WARP) {
         // ===== item fetch (whole warp) + TMA producer (lane 0) =====
         constexpr int NCHUNK = ITEM_BYTES / 16;
-        uint32_t stage = 0, phase = 0, n_done = 0;
+        uint32_t stage = 0, phase = 0, n_done = 0, b_count = 0;
         int ok = 1;
         uint4 nxt = make_uint4(0, 0, 0, 0);
         if ((int)blockIdx.x < n_items && lane < NCHUNK) nxt = __ldg(reinterpret_cast<const uint4*>(items + blockIdx.x) + lane);
@@ -564,7 +573,24 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
             if (lane == 0) mbar_arrive(ifull_bar(slot));
             if (i + (int)gridDim.x < n_items && lane < NCHUNK)
                 nxt = __ldg(reinterpret_cast<const uint4*>(items + i + gridDim.x) + lane);
-            if (n_base > 0) {
+            if (strip) {
+                // strip item: one base tile per (column tile, row block), in the order the epilogue consumes them
+                const Item& it = *item_slot(slot);
+                const int bm0 = it.base_map[0], row0 = it.row0, nrb = (it.rows + 127) >> 7, nct = (it.cols + 127) >> 7;
+                const CUtensorMap* mp = maps + bm0;
+                for (int ct = 0; ct < nct && ok; ++ct)
+                    for (int rb = 0; rb < nrb && ok; ++rb, ++b_count) {
+                        const uint32_t bs = b_count % (uint32_t)n_bslots, bph = (b_count / (uint32_t)n_bslots) & 1u;
+                        ok = TWAIT(1, mbar_wait(bempty_bar(bs), bph ^ 1u, err)) ? 1 : 0;
+                        if (ok && elect_one()) {
+                            mbar_expect_tx(bfull_bar(bs), TILE_BYTES);
+#pragma unroll
+                            for (int h = 0; h < 2; ++h)
+                                tma_load_2d(base_tile(bs) + h * 16384u, mp, 128 * ct + 64 * h, row0 + 128 * rb, bfull_bar(bs));
+                        }
+                        __syncwarp();
+                    }
+            } else if (n_base > 0) {
                 // the item's base tile(s): hi [+ lo], each two 64-column halves of 128 rows (converged warp, one
                 // elected lane issues)
                 const Item& it = *item_slot(slot);
@@ -602,6 +628,42 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 const uint32_t slot = n_done % ITEM_SLOTS, iphase = (n_done / ITEM_SLOTS) & 1u;
                 if (!(ok = TWAIT(3, mbar_wait(ifull_bar(slot), iphase, err)))) break;
                 const Item& it = *item_slot(slot);
+                if (strip) {
+                    // strip item: warp 9 loads the strip's resident A tiles once ([row block][K-atom]); warp 10 streams
+                    // the B K-atoms of every column tile through the 16 KB ring (each serves both row blocks)
+                    const int nrb = (it.rows + 127) >> 7, nct = (it.cols + 127) >> 7;
+                    const int na = it.atoms[0] + it.atoms[1];
+                    if (!is_b) {
+                        if (!(ok = TWAIT(2, mbar_wait(parked_bar(1), (n_done & 1u) ^ 1u, err)))) break;   // L buffer free
+                        if (elect_one()) {
+                            mbar_expect_tx(parked_bar(0), (uint32_t)(nrb * na) * A_BYTES);
+                            for (int rb = 0; rb < nrb; ++rb) {
+                                int a = 0;
+                                for (int seg = 0; seg < 2; ++seg)
+                                    for (int t = 0; t < it.atoms[seg]; ++t, ++a)
+                                        tma_load_2d(smem0 + (uint32_t)(rb * 2 + a) * A_BYTES, maps + it.map_a[seg],
+                                                    it.a_c0[seg] + 64 * t, it.a_r0[seg] + 128 * rb, parked_bar(0));
+                            }
+                        }
+                        __syncwarp();
+                    } else {
+                        for (int ct = 0; ct < nct && ok; ++ct)
+                            for (int seg = 0; seg < 2 && ok; ++seg)
+                                for (int t = 0; t < it.atoms[seg]; ++t) {
+                                    if (!TWAIT(2, mbar_wait(empty_bar(stage), phase ^ 1u, err))) { ok = false; break; }
+                                    if (elect_one()) {
+                                        mbar_expect_tx(full_bar(stage), B_BYTES);
+                                        tma_load_2d(smem0 + STRIP_L_BYTES + stage * B_BYTES, maps + it.map_b[seg],
+                                                    it.b_c0[seg] + 64 * t, it.b_r0[seg] + 128 * ct, full_bar(stage));
+                                    }
+                                    __syncwarp();
+                                    if (++stage == (uint32_t)STRIP_RING) { stage = 0; phase ^= 1u; }
+                                }
+                    }
+                    __syncwarp();
+                    if (elect_one()) mbar_arrive(iempty_bar(slot));
+                    continue;
+                }
                 const int a_mn = it.a_mn, b_mn = it.b_mn, nbx = it.N >> 6;
                 const uint32_t tx = is_b ? (uint32_t)it.N * 128u : (uint32_t)A_BYTES;
 #pragma unroll 1
@@ -640,7 +702,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
     } else if (warp == MMA_WARP) {
         // ===== MMA issuer (converged warp, one elected lane issues) =====
         {
-            uint32_t stage = 0, phase = 0, n_done = 0;
+            uint32_t stage = 0, phase = 0, n_done = 0, t_count = 0;
             bool ok = true;
             for (int i = blockIdx.x; i < n_items && ok; i += gridDim.x, ++n_done) {
                 const uint32_t slot = n_done % ITEM_SLOTS, iphase = (n_done / ITEM_SLOTS) & 1u;
@@ -651,6 +713,49 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 int total = 0;
 #pragma unroll
                 for (int seg = 0; seg < NSEG; ++seg) total += it.atoms[seg];
+                if (strip) {
+                    // strip item: A tiles resident, per column tile the B atoms serve both row blocks
+                    const int nrb = (it.rows + 127) >> 7, nct = (it.cols + 127) >> 7;
+                    __syncwarp();
+                    if (elect_one()) mbar_arrive(iempty_bar(slot));
+                    if (!(ok = TWAIT(0, mbar_wait(parked_bar(0), n_done & 1u, err)))) break;       // A tiles landed
+                    tc_fence_after();
+                    for (int ct = 0; ct < nct && ok; ++ct) {
+                        for (int rb = 0; rb < nrb && ok; ++rb, ++t_count) {
+                            const uint32_t acc = t_count % n_acc, aphase = (t_count / n_acc) & 1u;
+                            if (!(ok = TWAIT(1, mbar_wait(tempty_bar(acc), aphase ^ 1u, err)))) break;
+                            tc_fence_after();
+                            const uint32_t d = tmem_base + acc * 128u;
+                            for (int a = 0; a < total; ++a) {
+                                const uint32_t st_a = (stage + (uint32_t)a) % STRIP_RING;
+                                const uint32_t ph_a = phase ^ ((stage + (uint32_t)a) >= (uint32_t)STRIP_RING ? 1u : 0u);
+                                if (rb == 0) {
+                                    if (!(ok = TWAIT(2, mbar_wait(full_bar(st_a), ph_a, err)))) break;
+                                    tc_fence_after();
+                                }
+                                const uint32_t sa = smem0 + (uint32_t)(rb * 2 + a) * A_BYTES;
+                                const uint32_t sb = smem0 + STRIP_L_BYTES + st_a * B_BYTES;
+                                if (elect_one()) {
+#pragma unroll
+                                    for (int kk = 0; kk < 4; ++kk)
+                                        tc_mma_bf16(d, smem_desc(sa + 32u * kk, 16u, 1024u), smem_desc(sb + 32u * kk, 16u, 1024u),
+                                                    idesc, (a | kk) ? 1u : 0u);
+                                }
+                                __syncwarp();
+                            }
+                            if (ok && elect_one()) tc_commit(tfull_bar(acc));
+                            __syncwarp();
+                        }
+                        if (ok && elect_one())
+                            for (int a = 0; a < total; ++a) tc_commit(empty_bar((stage + (uint32_t)a) % STRIP_RING));
+                        __syncwarp();
+                        stage += (uint32_t)total;
+                        if (stage >= (uint32_t)STRIP_RING) { stage -= STRIP_RING; phase ^= 1u; }
+                    }
+                    if (ok && elect_one()) tc_commit(parked_bar(1));       // A tiles free once these MMAs retire
+                    __syncwarp();
+                    continue;
+                }
                 __syncwarp();
                 if (elect_one()) mbar_arrive(iempty_bar(slot));
                 const uint32_t acc = n_done % n_acc, aphase = (n_done / n_acc) & 1u;
@@ -805,7 +910,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
         if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     } else {
         // ===== epilogue warps 0..7 =====
-        uint32_t n_done = 0;
+        uint32_t n_done = 0, s_tiles = 0;
         int pending_slot = -1;
         bool ok = true;
         for (int i = blockIdx.x; i < n_items && ok; i += gridDim.x, ++n_done) {
@@ -816,6 +921,51 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
             // the tensor's amax (EPI_CAST) is fetched before the data waits, so its latency hides behind them
             uint32_t amax_bits = 0;
             if (ok && item_slot(slot)->mode == EPI_CAST) amax_bits = *reinterpret_cast<volatile uint32_t*>(item_slot(slot)->amax);
+            if (strip) {
+                // strip item: (column tile, row block) tiles in order; one amax atomic per warp per strip
+                ok = __all_sync(0xFFFFFFFFu, ok);
+                if (!ok) break;
+                const Item& it = *item_slot(slot);
+                const int nrb = (it.rows + 127) >> 7, nct = (it.cols + 127) >> 7;
+                uint32_t run_max = 0;
+                for (int ct = 0; ct < nct && ok; ++ct)
+                    for (int rb = 0; rb < nrb && ok; ++rb, ++s_tiles) {
+                        const uint32_t sacc = s_tiles % n_acc, saph = (s_tiles / n_acc) & 1u;
+                        const uint32_t sbs = s_tiles % (uint32_t)n_bslots, sbph = (s_tiles / (uint32_t)n_bslots) & 1u;
+                        ok = TWAIT(1, mbar_wait(bfull_bar(sbs), sbph, err));
+                        ok = ok && TWAIT(2, mbar_wait(tfull_bar(sacc), saph, err));
+                        ok = __all_sync(0xFFFFFFFFu, ok);
+                        if (!ok) break;
+                        tc_fence_after();
+                        const long long t_s0 = prof ? clock64() : 0;
+                        const bool stored = epilogue_tile(it, tmem_base + sacc * 128u, base_tile(sbs), 1, warp, lane, s_red, maps, amax_bits,
+                                                          it.row0 + 128 * rb, 128 * ct, it.write_scale != 0 && ct == 0 && rb == 0,
+                                                          it.mode == EPI_BLOCKCAST ? it.scale_inv_out + (size_t)((it.row0 >> 7) + rb) * nct + ct
+                                                                                   : it.scale_inv_out,
+                                                          &run_max);
+                        tc_fence_before();
+                        __syncwarp();
+                        if (lane == 0) mbar_arrive(tempty_bar(sacc));
+                        if (threadIdx.x == 0 && pending_slot >= 0) {
+                            asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+                            mbar_arrive(bempty_bar(pending_slot));
+                            pending_slot = -1;
+                        }
+                        epi_sync();
+                        if (threadIdx.x == 0) {
+                            if (stored) pending_slot = (int)sbs;
+                            else mbar_arrive(bempty_bar(sbs));
+                        }
+                        if (prof) pw[3] += clock64() - t_s0;
+                    }
+                if (ok && it.mode == EPI_AMAX) {
+                    run_max = warp_max_u32(run_max);
+                    if (lane == 0 && run_max != 0u) atomicMax(it.amax, run_max);
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(iempty_bar(slot));
+                continue;
+            }
             if (ok && n_base > 0) ok = TWAIT(1, mbar_wait(bfull_bar(bs), bphase, err));
             ok = ok && TWAIT(2, mbar_wait(tfull_bar(acc), aphase, err));
             const long long t_e0 = prof ? clock64() : 0;
@@ -825,7 +975,8 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
             const Item& it = *item_slot(slot);
             bool stored = false;
             if (it.base_map[0] >= 0)
-                stored = epilogue_tile(it, tmem_base + acc * 128u, base_tile(bs), it.base_map[1] >= 0 ? 2 : 1, warp, lane, s_red, maps, amax_bits);
+                stored = epilogue_tile(it, tmem_base + acc * 128u, base_tile(bs), it.base_map[1] >= 0 ? 2 : 1, warp, lane, s_red, maps, amax_bits,
+                                       it.row0, it.col0, it.write_scale != 0, it.scale_inv_out, nullptr);
             else
                 epilogue(it, tmem_base + acc * 128u, warp, lane, s_red);
             tc_fence_before();
