@@ -353,9 +353,10 @@ gf8_status fast_encode_many(gf8_ctx* c, int n, const int* layers, const void* co
                 f.mode = L.desc.scaling == GF8_SCALE_TENSOR ? EPI_AMAX : EPI_BLOCKCAST;
                 f.out = codes[i]; f.amax = p->d_amax + 2 * t; f.done = p->d_amax + 2 * t + 1; f.scale_inv = sinv[i];
                 if (dt == GF8_DT_BF16) {
-                    CUtensorMap mc;
-                    if ((s = make_map_u8(c, &mc, codes[i], m, nn)) != GF8_OK) break;
-                    f.out_map = pb.add_single(codes[i], mc);
+                    CUtensorMap mc[2];                              // [0] one CTA-wide tile, [1] one warp's sub-tile
+                    if ((s = make_map_u8(c, &mc[0], codes[i], m, nn)) != GF8_OK) break;
+                    if ((s = make_map_u8(c, &mc[1], codes[i], m, nn, true)) != GF8_OK) break;
+                    f.out_map = pb.add_map(codes[i], mc);
                 }
             }
             add_transform(pb, L, slot, src_map, -1, false, false, f);

@@ -78,14 +78,15 @@ gf8_status make_map(gf8_ctx* c, CUtensorMap* out, const void* ptr, uint64_t rows
 }
 
 // FP8 code matrix [rows][cols] bytes -> TMA store map, 128 x 128 boxes (one update tile), 128 B swizzle.
-gf8_status make_map_u8(gf8_ctx* c, CUtensorMap* out, const void* ptr, uint64_t rows, uint64_t cols) {
+gf8_status make_map_u8(gf8_ctx* c, CUtensorMap* out, const void* ptr, uint64_t rows, uint64_t cols, bool per_warp = false) {
     const cuuint64_t gdim[2] = {cols, rows};
     const cuuint64_t gstride[1] = {cols};
-    const cuuint32_t box[2] = {128, 128};
+    // per_warp: 64 x 32 boxes, no swizzle (one epilogue warp's sub-tile); else 128 x 128 boxes, 128 B swizzle
+    const cuuint32_t box[2] = {per_warp ? 64u : 128u, per_warp ? 32u : 128u};
     const cuuint32_t estr[2] = {1, 1};
     const CUresult r = ((EncodeTiledFn)c->encode_tiled)(out, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(ptr), gdim,
                                                         gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                                                        CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                                                        per_warp ? CU_TENSOR_MAP_SWIZZLE_NONE : CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
                                                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return fail(c, GF8_ERR_CUDA, "cuTensorMapEncodeTiled (u8) failed (%d) for %llu x %llu", (int)r,
                                        (unsigned long long)rows, (unsigned long long)cols);

@@ -432,8 +432,8 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
         if (write_scale && r == 0 && half == 0) *sinv_out = si;
     }
     if (mode == EPI_CAST || mode == EPI_BLOCKCAST) {
-        // 64 codes of this row half; the 128 x 128-byte code tile then overwrites the (consumed) first half of
-        // the base tile in the store map's 128 B swizzle
+        // 64 codes of this row half.  Each warp owns a 32-row x 64-byte sub-tile: it stages it over its own (consumed)
+        // base rows and issues its own TMA store (map out_map + 1: 64 x 32 boxes), so the cast needs no CTA-wide sync.
         uint4 cd[4];
 #pragma unroll
         for (int g = 0; g < 2; ++g) {
@@ -441,14 +441,14 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
             cd[2 * g] = fmt == 0 ? codes16<0>(v, scale) : codes16<1>(v, scale);
             cd[2 * g + 1] = fmt == 0 ? codes16<0>(v + 16, scale) : codes16<1>(v + 16, scale);
         }
-        epi_sync();                               // every thread has read its base data
+        __syncwarp();                             // every lane of this warp has read its base rows
+        const uint32_t sub = tile + (uint32_t)half * 16384u + (uint32_t)((warp & 3) * 32) * 128u;   // this warp's 4 KB
 #pragma unroll
-        for (int q = 0; q < 4; ++q)
-            sts128(tile + (uint32_t)r * 128u + (((uint32_t)(4 * half + q) ^ (uint32_t)(r & 7)) << 4), cd[q]);
+        for (int q = 0; q < 4; ++q) sts128(sub + (uint32_t)lane * 64u + 16u * q, cd[q]);
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        epi_sync();
-        if (threadIdx.x == 0) {
-            tma_store_2d(maps + it.out_map, tile, col0, row0);
+        __syncwarp();
+        if (lane == 0) {
+            tma_store_2d(maps + it.out_map + 1, sub, col0 + cbase, row0 + (warp & 3) * 32);
             asm volatile("cp.async.bulk.commit_group;" ::: "memory");
         }
         return true;
@@ -538,7 +538,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
             mbar_init(parked_bar(a), 1); mbar_init(sready_bar(a), 1);
             mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), EPI_WARPS);
         }
-        for (int b = 0; b < MAX_BASE_SLOTS; ++b) { mbar_init(bfull_bar(b), 1); mbar_init(bempty_bar(b), 1); }
+        for (int b = 0; b < MAX_BASE_SLOTS; ++b) { mbar_init(bfull_bar(b), 1); mbar_init(bempty_bar(b), EPI_WARPS); }
         for (int s = 0; s < ITEM_SLOTS; ++s) { mbar_init(ifull_bar(s), 1); mbar_init(iempty_bar(s), EPI_WARPS + 3); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
@@ -898,7 +898,8 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
             }
             tc_fence_before();
             epi_sync();                       // base tile consumed, amax atomics issued, parked info visible
-            if (threadIdx.x == 0) { mbar_arrive(parked_bar(acc)); mbar_arrive(bempty_bar(bs)); }
+            if (threadIdx.x == 0) mbar_arrive(parked_bar(acc));
+            if (lane == 0) mbar_arrive(bempty_bar(bs));
             __syncwarp();
             if (lane == 0) mbar_arrive(iempty_bar(slot));
             if (prof) pw[3] += clock64() - t_e0;
@@ -945,17 +946,17 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                                                           &run_max);
                         tc_fence_before();
                         __syncwarp();
-                        if (lane == 0) mbar_arrive(tempty_bar(sacc));
-                        if (threadIdx.x == 0 && pending_slot >= 0) {
-                            asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-                            mbar_arrive(bempty_bar(pending_slot));
-                            pending_slot = -1;
+                        // every warp returns the base slot itself; after a TMA store from it, one tile later (when
+                        // the store has read its shared memory), so the wait overlaps the next tile
+                        if (lane == 0) {
+                            mbar_arrive(tempty_bar(sacc));
+                            if (pending_slot >= 0) {
+                                asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+                                mbar_arrive(bempty_bar(pending_slot));
+                            }
+                            if (!stored) mbar_arrive(bempty_bar(sbs));
                         }
-                        epi_sync();
-                        if (threadIdx.x == 0) {
-                            if (stored) pending_slot = (int)sbs;
-                            else mbar_arrive(bempty_bar(sbs));
-                        }
+                        pending_slot = stored ? (int)sbs : -1;
                         if (prof) pw[3] += clock64() - t_s0;
                     }
                 if (ok && it.mode == EPI_AMAX) {
@@ -988,20 +989,18 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 // the base slot goes back to the producer once every epilogue thread is done with it and the TMA
                 // store issued from it (if any) has read it.  That store wait is deferred by one item, so it
                 // overlaps the next tile instead of stalling this warp.
-                if (threadIdx.x == 0 && pending_slot >= 0) {
-                    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-                    mbar_arrive(bempty_bar(pending_slot));
-                    pending_slot = -1;
+                if (lane == 0) {
+                    if (pending_slot >= 0) {
+                        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+                        mbar_arrive(bempty_bar(pending_slot));
+                    }
+                    if (!stored) mbar_arrive(bempty_bar(bs));
                 }
-                epi_sync();
-                if (threadIdx.x == 0) {
-                    if (stored) pending_slot = (int)bs;
-                    else mbar_arrive(bempty_bar(bs));
-                }
+                pending_slot = stored ? (int)bs : -1;
             }
             if (prof) pw[4] += clock64() - t_p0;
         }
-        if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // (pending slot: kernel ends)
+        if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // (pending slot: kernel ends)
     }
 #undef TWAIT
     if (prof && lane == 0 && (warp == 0 || warp == OPERAND_WARP || warp == MMA_WARP)) {
