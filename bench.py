@@ -94,6 +94,22 @@ class ClockSampler:
 
 
 # ----------------------------------------------------------------------------------------------------
+def max_over_ranks(ms, world, device):
+    """Replica timing rule: every rank times its own replica on its device; the job's time is the MAX over ranks."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    tt = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    return float(tt.item())
+
+
+def job_value(world, R, n_el, ms_step):
+    """Whole-job GB/s of BF16 gradient encoded+decoded: `world` independent replicas of R ranks x n_el elements."""
+    return world * R * n_el * 2 / (ms_step * 1e-3) / 1e9
+
+
 def cpu_sample(cfg_index, seed_rank=0):
     """The bounded oracle sample: layer-0 q, k, v, o matrices of the config (side BOTH, the config's k),
     R = 1: oracle encode (O3 + O4) and reduce_decoded (O5 + O6).  Returns (elements, seconds, cores, text)."""
@@ -274,13 +290,10 @@ def run_gf8(args):
     ms = e0.elapsed_time(e1)
     enc_ms = sum(a.elapsed_time(b) for a, b, _ in seg) / args.steps
     red_ms = sum(b.elapsed_time(c) for _, b, c in seg) / args.steps
-    if world > 1:
-        tt = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms = float(tt.item())
+    ms = max_over_ranks(ms, world, dev)
     ms_step = ms / args.steps
     esz = 2 if cfg.dtype == "bf16" else 4
-    value = world * R * n_el * 2 / (ms_step * 1e-3) / 1e9
+    value = job_value(world, R, n_el, ms_step)
 
     # ---- roofline of the dominant call: encode (3 B/element: 2 read BF16 + 1 write FP8)
     hbm_peak, tf_peak, which = _peaks()
@@ -324,11 +337,8 @@ def run_gf8(args):
         b.record()
         barrier()
         ems = a.elapsed_time(b) / k2
-        if world > 1:
-            tt = torch.tensor([ems], device=dev, dtype=torch.float64)
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            ems = float(tt.item())
-        e2e = {"value": world * R * n_el * 2 / (ems * 1e-3) / 1e9, "unit": UNIT,
+        ems = max_over_ranks(ems, world, dev)
+        e2e = {"value": job_value(world, R, n_el, ems), "unit": UNIT,
                "h2d_bytes_per_step": R * n_el * esz, "d2h_bytes_per_step": n_el * esz, "steps": k2, "ms_per_step": ems}
 
     cpu = None
