@@ -284,6 +284,22 @@ enum { PLAN_ENCODE = 1, PLAN_DECODE = 2, PLAN_WHITEN = 3, PLAN_FACTOR = 4 };
 
 inline void key_ptr(std::vector<uint64_t>& k, const void* p) { k.push_back((uint64_t)(uintptr_t)p); }
 
+gf8_status aux_fork(gf8_ctx* c, cudaStream_t st) {
+    if (!c->aux_stream) {
+        CU_TRY(c, cudaStreamCreateWithFlags(&c->aux_stream, cudaStreamNonBlocking));
+        CU_TRY(c, cudaEventCreateWithFlags(&c->aux_fork_ev, cudaEventDisableTiming));
+        CU_TRY(c, cudaEventCreateWithFlags(&c->aux_join_ev, cudaEventDisableTiming));
+    }
+    CU_TRY(c, cudaEventRecord(c->aux_fork_ev, st));
+    CU_TRY(c, cudaStreamWaitEvent(c->aux_stream, c->aux_fork_ev, 0));
+    return GF8_OK;
+}
+gf8_status aux_join(gf8_ctx* c, cudaStream_t st) {
+    CU_TRY(c, cudaEventRecord(c->aux_join_ev, c->aux_stream));
+    CU_TRY(c, cudaStreamWaitEvent(st, c->aux_join_ev, 0));
+    return GF8_OK;
+}
+
 // encode (PLAN_ENCODE) or the transform tap (PLAN_WHITEN: codes == nullptr, taps[i] receives FP32 W~).
 gf8_status fast_encode_many(gf8_ctx* c, int n, const int* layers, const void* const* grads, gf8_dtype dt,
                             uint8_t* const* codes, float* const* sinv, float* const* taps, cudaStream_t st) {
@@ -365,21 +381,30 @@ gf8_status fast_encode_many(gf8_ctx* c, int n, const int* layers, const void* co
         if (s == GF8_OK) s = plan_store(c, key, p);
         if (s != GF8_OK) { plan_free(p); return s; }
     }
+    // The problems outside the tensor-core engine (Euclidean tensors: HBM-bound streaming kernels) run on the
+    // context's auxiliary stream, concurrently with the engine's stages (bound inside the SM), and join at the end.
+    const bool overlap = !p->plain.empty() && p->stage_cnt[0] + p->stage_cnt[1] + p->stage_cnt[5] + p->stage_cnt[3] > 0 && !tap;
+    cudaStream_t sp = st;
+    if (overlap) {
+        GF_TRY(aux_fork(c, st));
+        sp = c->aux_stream;
+    }
+    for (int i : p->plain) {
+        if (tap) {
+            LayerState& L = c->layers[layers[i]];
+            if (dt == GF8_DT_BF16) GF_TRY(transform_simt<bf16>(c, sp, L, (const bf16*)grads[i], taps[i], false));
+            else GF_TRY(transform_simt<float>(c, sp, L, (const float*)grads[i], taps[i], false));
+        } else {
+            GF_TRY(encode_one(c, layers[i], grads[i], dt, codes[i], sinv[i], sp));
+        }
+    }
     for (const Plan::Convert& cv : p->converts) {
         convert_kernel<float, bf16><<<grid_for(c, cv.numel, 256, 8), 256, 0, st>>>(cv.src, cv.numel, cv.dst);
         LAUNCH_CHECK(c);
     }
     if (p->n_amax) CU_TRY(c, cudaMemsetAsync(p->d_amax, 0, p->n_amax * sizeof(uint32_t), st));
     GF_TRY(plan_run_stages(c, st, p));
-    for (int i : p->plain) {
-        if (tap) {
-            LayerState& L = c->layers[layers[i]];
-            if (dt == GF8_DT_BF16) GF_TRY(transform_simt<bf16>(c, st, L, (const bf16*)grads[i], taps[i], false));
-            else GF_TRY(transform_simt<float>(c, st, L, (const float*)grads[i], taps[i], false));
-        } else {
-            GF_TRY(encode_one(c, layers[i], grads[i], dt, codes[i], sinv[i], st));
-        }
-    }
+    if (overlap) GF_TRY(aux_join(c, st));
     return GF8_OK;
 }
 
@@ -445,9 +470,16 @@ gf8_status fast_reduce_decoded_many(gf8_ctx* c, int n, const int* layers, const 
         GF_TRY(reduce_dev<float>(c, st, codes + (size_t)i * R, sinv + (size_t)i * R, R, average, L.desc.d_out, L.desc.d_in,
                                  L.desc.fmt, L.desc.scaling, rd.uhat, rd.u16, rd.u16_lo));
     }
-    GF_TRY(plan_run_stages(c, st, p));
+    const bool overlap = !p->plain.empty() && !p->reduces.empty();
+    cudaStream_t sp = st;
+    if (overlap) {
+        GF_TRY(aux_fork(c, st));
+        sp = c->aux_stream;
+    }
     for (int i : p->plain)
-        GF_TRY(reduce_decoded_one(c, layers[i], codes + (size_t)i * R, sinv + (size_t)i * R, R, average, outs[i], dt, st));
+        GF_TRY(reduce_decoded_one(c, layers[i], codes + (size_t)i * R, sinv + (size_t)i * R, R, average, outs[i], dt, sp));
+    GF_TRY(plan_run_stages(c, st, p));
+    if (overlap) GF_TRY(aux_join(c, st));
     return GF8_OK;
 }
 
@@ -627,6 +659,7 @@ gf8_status gf8_destroy(gf8_ctx* ctx) {
         if (ctx->rs_ev[q]) cudaEventDestroy(ctx->rs_ev[q]);
     }
     if (ctx->rs_fork) cudaEventDestroy(ctx->rs_fork);
+    if (ctx->aux_stream) { cudaStreamDestroy(ctx->aux_stream); cudaEventDestroy(ctx->aux_fork_ev); cudaEventDestroy(ctx->aux_join_ev); }
     for (Plan* p : ctx->plan_order) plan_free(p);
     for (auto& kv : ctx->fac_plans) plan_free(kv.second);
     for (LayerState& L : ctx->layers)

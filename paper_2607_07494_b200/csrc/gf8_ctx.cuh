@@ -80,6 +80,9 @@ struct gf8_ctx {
     cudaStream_t rs_stream[GF8_REFRESH_STREAMS] = {};
     cudaEvent_t rs_ev[GF8_REFRESH_STREAMS] = {};
     cudaEvent_t rs_fork = nullptr;
+    // auxiliary stream: the streaming kernels of Euclidean tensors overlap the tensor-core stages of a batched call
+    cudaStream_t aux_stream = nullptr;
+    cudaEvent_t aux_fork_ev = nullptr, aux_join_ev = nullptr;
     // tap scratch (gf8_quantize_f32 with arbitrary shapes)
     uint32_t* tap_amax = nullptr; float* tap_scale = nullptr; size_t tap_cap = 0;
     // host-step staging
