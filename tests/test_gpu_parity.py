@@ -203,6 +203,52 @@ def test_fast_g5_reduce_decoded(name):
     assert relfro(to_np64(one), want1) <= TOL_FAST
 
 
+def test_fast_full_size_shapes_in_the_bench_launch_configuration():
+    """BASELINE.json configs[2] shapes (gate 4096x1536, down 1536x4096, q 1536x1536; k = 64, BOTH, BF16, E4M3 per
+    tensor) through ONE batched call per direction, as bench.py issues them (strip items, R payloads per layer):
+    transform against the oracle, fused codes bit-identical to the oracle quantizer on the GPU's tapped W~, and the
+    batched reduce_decoded against the oracle."""
+    shapes = [(4096, 1536), (1536, 4096), (1536, 1536)]
+    k, R, lam = 64, 3, 1e-3
+    lays = [gf8.Layer(m, n, gf8.SIDE_BOTH, k, k, gf8.E4M3, gf8.SCALE_TENSOR, lam) for m, n in shapes]
+    ctx = gf8.create(lays, gf8.PREC_FAST)
+    bases = []
+    for i, (m, n) in enumerate(shapes):
+        bs = {}
+        for side, d in ((gf8.SIDE_IN, n), (gf8.SIDE_OUT, m)):
+            U = synth.rand_orthonormal(d, k, "cuda", 91, i, side).contiguous()
+            mu = (np.arange(1, k + 1, dtype=np.float64)) ** -2.0
+            tail = float(((np.arange(k + 1, d + 1, dtype=np.float64)) ** -2.0).mean())
+            rho, e, eb = oracle.multipliers(mu, d, float(mu.sum() + tail * (d - k)), lam)
+            ctx.set_basis(i, side, U, torch.from_numpy(mu).float().cuda(), float(rho))
+            bs[side] = oracle.Basis(U.double().cpu().numpy(), mu, rho, e, eb)
+        bases.append(bs)
+    grads = [[synth.rank_gradient(synth.gradient(m, n, "cuda", 92, i), r, 93, i).to(torch.bfloat16) for r in range(R)]
+             for i, (m, n) in enumerate(shapes)]
+    ids = [i for i in range(len(shapes)) for _ in range(R)]
+    flat = [grads[i][r] for i in range(len(shapes)) for r in range(R)]
+    codes = [torch.empty(g.shape, dtype=torch.uint8, device="cuda") for g in flat]
+    sinvs = [torch.empty(1, dtype=torch.float32, device="cuda") for _ in flat]
+    ctx.encode_many(ids, flat, codes, sinvs)
+    ctx.sync_check()
+    for i in (0, 1):                                                 # the two large shapes, rank 1
+        g = grads[i][1]
+        wt = ctx.whiten_f32(i, g)
+        oc, os_ = oracle.quantize(wt.cpu().numpy(), gf8.E4M3, gf8.SCALE_TENSOR)
+        j = i * R + 1
+        assert np.array_equal(codes[j].cpu().numpy(), oc) and np.array_equal(sinvs[j].cpu().numpy(), os_)
+        _, _, x = oracle.encode(to_np64(g), bases[i][gf8.SIDE_OUT], bases[i][gf8.SIDE_IN])
+        assert relfro(to_np64(wt), x) <= TOL_FAST
+    outs = [torch.empty(m, n, dtype=torch.bfloat16, device="cuda") for m, n in shapes]
+    ctx.reduce_decoded_many(list(range(len(shapes))), codes, sinvs, R, outs, average=True)
+    ctx.sync_check()
+    for i in (0, 1):
+        pc = [codes[i * R + r].cpu().numpy() for r in range(R)]
+        ps = [sinvs[i * R + r].cpu().numpy() for r in range(R)]
+        want = oracle.reduce_decoded(pc, ps, bases[i][gf8.SIDE_OUT], bases[i][gf8.SIDE_IN])
+        assert relfro(to_np64(outs[i]), want) <= 2 * TOL_FAST
+
+
 def test_fast_batched_matches_single_calls():
     """encode_many / reduce_decoded_many with repeated layer ids (R ranks in one launch set) give the
     same bytes as one call per payload."""
