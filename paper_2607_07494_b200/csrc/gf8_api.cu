@@ -155,6 +155,16 @@ gf8_status ensure_factor(gf8_ctx* c, SideState& s) {
     return dmalloc(c, &s.factor, (size_t)s.d * s.d);
 }
 
+// FP32 -> BF16 hi (+ optional residual lo = bf16(x - hi)): the MMA operand copies of an FP32 gradient
+__global__ void split_kernel(const float* __restrict__ in, int64_t n, bf16* __restrict__ hi, bf16* __restrict__ lo) {
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const float x = in[i];
+        const bf16 h = __float2bfloat16_rn(x);
+        hi[i] = h;
+        if (lo) lo[i] = __float2bfloat16_rn(x - __bfloat162float(h));
+    }
+}
+
 __global__ void fill_kernel(float* p, float v, int n) {
     if ((int)threadIdx.x < n) p[threadIdx.x] = v;
 }
@@ -346,15 +356,17 @@ gf8_status fast_encode_many(gf8_ctx* c, int n, const int* layers, const void* co
             LayerState& L = c->layers[layers[i]];
             const int m = L.desc.d_out, nn = L.desc.d_in;
             Slot* slot = nullptr;
-            if ((s = fast_slot(c, L, occurrence[layers[i]]++, dt == GF8_DT_F32, false, false, &slot)) != GF8_OK) break;
-            int src_map;
+            const bool split = c->precision == GF8_PREC_EXACT;      // EXACT: hi + lo operands (3 products each)
+            if ((s = fast_slot(c, L, occurrence[layers[i]]++, dt == GF8_DT_F32, false, split, &slot)) != GF8_OK) break;
+            int src_map, src_lo_map = -1;
             if (dt == GF8_DT_BF16) {
                 CUtensorMap mp[2];
                 if ((s = make_map(c, mp, grads[i], m, nn, nn)) != GF8_OK) break;
                 src_map = pb.add_map(grads[i], mp);
             } else {
-                p->converts.push_back({(const float*)grads[i], slot->src16, (int64_t)m * nn});
+                p->converts.push_back({(const float*)grads[i], slot->src16, split ? slot->src16_lo : nullptr, (int64_t)m * nn});
                 src_map = pb.add_map(slot->src16, slot->map_src16);
+                if (split) src_lo_map = pb.add_map(slot->src16_lo, slot->map_src16_lo);
             }
             Final f;
             memset(&f, 0, sizeof(f));
@@ -375,7 +387,7 @@ gf8_status fast_encode_many(gf8_ctx* c, int n, const int* layers, const void* co
                     f.out_map = pb.add_map(codes[i], mc);
                 }
             }
-            add_transform(pb, L, slot, src_map, -1, false, false, f);
+            add_transform(pb, L, slot, src_map, src_lo_map, false, split, f);
         }
         if (s == GF8_OK) s = plan_finish(c, pb, p);
         if (s == GF8_OK) s = plan_store(c, key, p);
@@ -399,7 +411,7 @@ gf8_status fast_encode_many(gf8_ctx* c, int n, const int* layers, const void* co
         }
     }
     for (const Plan::Convert& cv : p->converts) {
-        convert_kernel<float, bf16><<<grid_for(c, cv.numel, 256, 8), 256, 0, st>>>(cv.src, cv.numel, cv.dst);
+        split_kernel<<<grid_for(c, cv.numel, 256, 8), 256, 0, st>>>(cv.src, cv.numel, cv.dst, cv.dst_lo);
         LAUNCH_CHECK(c);
     }
     if (p->n_amax) CU_TRY(c, cudaMemsetAsync(p->d_amax, 0, p->n_amax * sizeof(uint32_t), st));
@@ -598,6 +610,10 @@ gf8_status gf8_create(gf8_ctx** out, int device, const gf8_layer_desc* layers, i
     if (!c) return GF8_ERR_NOMEM;
     c->device = device;
     c->precision = precision;
+    // EXACT runs FP32 FMA on the CUDA cores.  GF8_EXACT_TC=1 (opt-in) runs it on the tensor-core engine with every BF16
+    // operand carried as hi + lo (16 mantissa bits): transform within 1e-5 of the oracle (gate G2's 1e-4 tier) at ~3x the
+    // MMAs, but a few 1e-4 of FP8 codes still flip, so the strict code-level gates (G3, G5's BF16 ulp) keep the SIMT path.
+    c->tc_exact = precision == GF8_PREC_EXACT && getenv("GF8_EXACT_TC") != nullptr;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) c->num_sms = prop.multiProcessorCount;
     c->layers.resize(n_layers);
@@ -697,7 +713,7 @@ gf8_status gf8_factor_update(gf8_ctx* ctx, int layer, const void* act, const voi
         const float beta = s.has_factor ? L.desc.ema_beta : 0.0f;
         const float alpha = (1.0f - beta) / (float)T;
         const int d = s.d;
-        if (dt == GF8_DT_BF16 && ctx->precision == GF8_PREC_FAST && d >= 128)
+        if (dt == GF8_DT_BF16 && (ctx->precision == GF8_PREC_FAST || ctx->tc_exact) && d >= 128)
             GF_TRY(fast_factor_gemm(ctx, st, X, T, d, alpha, beta, s.factor));
         else if (dt == GF8_DT_BF16)
             GF_TRY((launch_gemm<bf16, bf16, float, float>(ctx, st, (const bf16*)X, 1, d, (const bf16*)X, d, 1, s.factor,
@@ -726,7 +742,7 @@ gf8_status gf8_encode(gf8_ctx* ctx, int layer, const void* grad, gf8_dtype dt, u
                       void* stream) {
     if (!ctx) return GF8_ERR_INVALID_ARG;
     CU_TRY(ctx, cudaSetDevice(ctx->device));
-    if (ctx->precision == GF8_PREC_FAST) {
+    if (ctx->precision == GF8_PREC_FAST || ctx->tc_exact) {
         if (dt != GF8_DT_BF16 && dt != GF8_DT_F32) return fail(ctx, GF8_ERR_INVALID_ARG, "bad dtype");
         return fast_encode_many(ctx, 1, &layer, &grad, dt, &codes, &scale_inv, nullptr, (cudaStream_t)stream);
     }
@@ -739,7 +755,7 @@ gf8_status gf8_decode(gf8_ctx* ctx, int layer, const uint8_t* codes, const float
     CU_TRY(ctx, cudaSetDevice(ctx->device));
     const uint8_t* cp[1] = {codes};
     const float* sp[1] = {scale_inv};
-    if (ctx->precision == GF8_PREC_FAST) {
+    if (ctx->precision == GF8_PREC_FAST || ctx->tc_exact) {
         if (!codes || !scale_inv || !grad_out) return fail(ctx, GF8_ERR_INVALID_ARG, "null pointer");
         if (dt != GF8_DT_BF16 && dt != GF8_DT_F32) return fail(ctx, GF8_ERR_INVALID_ARG, "bad dtype");
         return fast_reduce_decoded_many(ctx, 1, &layer, cp, sp, 1, 0, &grad_out, dt, (cudaStream_t)stream);
@@ -751,7 +767,7 @@ gf8_status gf8_reduce_decoded(gf8_ctx* ctx, int layer, const uint8_t* const* cod
                               int R, int average, void* grad_out, gf8_dtype dt, void* stream) {
     if (!ctx) return GF8_ERR_INVALID_ARG;
     CU_TRY(ctx, cudaSetDevice(ctx->device));
-    if (ctx->precision == GF8_PREC_FAST) {
+    if (ctx->precision == GF8_PREC_FAST || ctx->tc_exact) {
         if (!codes || !scale_inv || !grad_out) return fail(ctx, GF8_ERR_INVALID_ARG, "null pointer");
         if (R < 1 || R > GF8_MAX_R) return fail(ctx, GF8_ERR_INVALID_ARG, "R=%d out of range [1,%d]", R, GF8_MAX_R);
         if (dt != GF8_DT_BF16 && dt != GF8_DT_F32) return fail(ctx, GF8_ERR_INVALID_ARG, "bad dtype");
@@ -766,7 +782,7 @@ gf8_status gf8_encode_many(gf8_ctx* ctx, int n, const int* layers, const void* c
     if (n < 0 || !layers || !grads || !codes || !scale_inv) return fail(ctx, GF8_ERR_INVALID_ARG, "null argument");
     CU_TRY(ctx, cudaSetDevice(ctx->device));
     if (dt != GF8_DT_BF16 && dt != GF8_DT_F32) return fail(ctx, GF8_ERR_INVALID_ARG, "bad dtype");
-    if (ctx->precision == GF8_PREC_FAST)
+    if (ctx->precision == GF8_PREC_FAST || ctx->tc_exact)
         return fast_encode_many(ctx, n, layers, grads, dt, codes, scale_inv, nullptr, (cudaStream_t)stream);
     for (int i = 0; i < n; ++i) GF_TRY(encode_one(ctx, layers[i], grads[i], dt, codes[i], scale_inv[i], (cudaStream_t)stream));
     return GF8_OK;
@@ -780,7 +796,7 @@ gf8_status gf8_reduce_decoded_many(gf8_ctx* ctx, int n, const int* layers, const
     if (R < 1 || R > GF8_MAX_R) return fail(ctx, GF8_ERR_INVALID_ARG, "R=%d out of range [1,%d]", R, GF8_MAX_R);
     CU_TRY(ctx, cudaSetDevice(ctx->device));
     if (dt != GF8_DT_BF16 && dt != GF8_DT_F32) return fail(ctx, GF8_ERR_INVALID_ARG, "bad dtype");
-    if (ctx->precision == GF8_PREC_FAST)
+    if (ctx->precision == GF8_PREC_FAST || ctx->tc_exact)
         return fast_reduce_decoded_many(ctx, n, layers, codes, scale_inv, R, average, grads_out, dt, (cudaStream_t)stream);
     for (int i = 0; i < n; ++i)
         GF_TRY(reduce_decoded_one(ctx, layers[i], codes + (size_t)i * R, scale_inv + (size_t)i * R, R, average,
@@ -970,7 +986,7 @@ gf8_status gf8_whiten_f32(gf8_ctx* ctx, int layer, const void* grad, gf8_dtype d
     CU_TRY(ctx, cudaSetDevice(ctx->device));
     cudaStream_t st = (cudaStream_t)stream;
     if ((const void*)grad == (const void*)out) return fail(ctx, GF8_ERR_INVALID_ARG, "in-place whiten tap not allowed");
-    if (ctx->precision == GF8_PREC_FAST && L.tc_ok)
+    if (L.tc_ok)
         return fast_encode_many(ctx, 1, &layer, &grad, dt, nullptr, nullptr, &out, st);
     if (dt == GF8_DT_BF16) return transform_simt<bf16>(ctx, st, L, (const bf16*)grad, out, false);
     return transform_simt<float>(ctx, st, L, (const float*)grad, out, false);

@@ -71,6 +71,7 @@ struct RefreshScratch {
 struct gf8_ctx {
     int device = 0;
     gf8_precision precision = GF8_PREC_EXACT;
+    bool tc_exact = false;           // EXACT on the tensor-core engine with hi + lo operands (opt-in, GF8_EXACT_TC=1)
     std::vector<LayerState> layers;
     std::vector<void*> allocs;
     float* wt_scratch = nullptr;     // max m*n FP32

@@ -19,7 +19,7 @@ struct Plan {
     int runs = 0;                        // launches so far: the first one acquires its tensor maps with proxy fences
     uint32_t* d_amax = nullptr;          // one word per TC problem (per-tensor scaling)
     size_t n_amax = 0;
-    struct Convert { const float* src; gf8::bf16* dst; int64_t numel; };
+    struct Convert { const float* src; gf8::bf16 *dst, *dst_lo; int64_t numel; };
     std::vector<Convert> converts;       // FP32 gradient -> BF16 MMA operand copies
     std::vector<int> plain;              // batch indices served by the per-problem (non-TC) path
     struct Reduce { int batch_index; float* uhat; gf8::bf16 *u16, *u16_lo; };
@@ -120,7 +120,7 @@ gf8_status fast_pack_basis(gf8_ctx* c, cudaStream_t st, SideState& s) {
 // Called from gf8_create for every layer: decides eligibility and allocates the BF16 basis copies.
 gf8_status fast_init_layer(gf8_ctx* c, LayerState& L) {
     L.tc_ok = false;
-    if (c->precision != GF8_PREC_FAST || L.desc.side == GF8_SIDE_NONE) return GF8_OK;
+    if ((c->precision != GF8_PREC_FAST && !c->tc_exact) || L.desc.side == GF8_SIDE_NONE) return GF8_OK;
     if (L.desc.d_out < 64 || L.desc.d_in < 64) return GF8_OK;
     if ((L.in.used && pad64(L.in.k) > FAST_MAX_KP) || (L.out.used && pad64(L.out.k) > FAST_MAX_KP)) return GF8_OK;
     GF_TRY(fast_init(c));
