@@ -31,7 +31,7 @@ namespace {
 using gf8::bf16;
 using gf8::tc::Item;
 
-constexpr int FAST_MAX_KP = 256;   // two 128-column accumulator chunks per panel
+constexpr int FAST_MAX_KP = 512;   // GF8_MAX_RANK: panels are cut into 128-column accumulator chunks
 constexpr size_t FAST_MAX_PLANS = 64;
 
 inline int pad64(int k) { return (k + 63) / 64 * 64; }

@@ -148,6 +148,7 @@ FAST_CASES.update({
     "llama600m-q": dict(m=1536, n=1536, kG=64, kA=64, side=gf8.SIDE_BOTH, dtype="bf16", seed=5, T=4096, q=2),
     "wide-k96": dict(m=640, n=1168, kG=96, kA=80, side=gf8.SIDE_BOTH, dtype="bf16", seed=6, q=2),
     "in-only-block": dict(m=384, n=528, kG=0, kA=32, side=gf8.SIDE_IN, dtype="bf16", seed=7, scaling=gf8.SCALE_BLOCK128),
+    "rank-512": dict(m=640, n=768, kG=512, kA=384, side=gf8.SIDE_BOTH, dtype="bf16", seed=8, q=2),
 })
 _fcache = {}
 
