@@ -274,6 +274,58 @@ def test_exact_on_tensor_cores_meets_the_transform_tier(name, monkeypatch):
     assert relfro(to_np64(got), want) <= TOL_EXACT
 
 
+def test_config4_style_loop_with_periodic_refresh():
+    """BASELINE.json configs[4] in miniature: R = 16 perturbed replicas of one gradient, encode x 16 -> FP32 sum of the
+    decoded payloads -> unwhiten, with an EMA factor update + warm basis refresh (q = 2) every 10 steps.  After the
+    last refresh the GPU's transform T is compared with the oracle run through the same updates (G7), and the last
+    step's averaged gradient with the oracle codec on the GPU's basis (G5, FAST tier)."""
+    m, n, k, R, lam, beta, T = 384, 512, 32, 16, 1e-3, 0.9, 2048
+    lay = gf8.Layer(m, n, gf8.SIDE_BOTH, k, k, gf8.E4M3, gf8.SCALE_TENSOR, lam, beta)
+    ctx = gf8.create([lay], gf8.PREC_FAST)
+    G = synth.gradient(m, n, "cuda", 404, 0).to(torch.bfloat16)
+    ctx.set_basis(0, gf8.SIDE_IN, synth.start_basis(n, k, "cuda", 404, 1))
+    ctx.set_basis(0, gf8.SIDE_OUT, synth.start_basis(m, k, "cuda", 404, 2))
+    A = Gf = None
+    VA, VG = to_np64(synth.start_basis(n, k, "cuda", 404, 1)), to_np64(synth.start_basis(m, k, "cuda", 404, 2))
+    codes = [torch.empty((m, n), dtype=torch.uint8, device="cuda") for _ in range(R)]
+    sinvs = [torch.empty(1, dtype=torch.float32, device="cuda") for _ in range(R)]
+    out = torch.empty((m, n), dtype=torch.bfloat16, device="cuda")
+    for step in range(21):
+        if step % 10 == 0:
+            X = synth.factor_samples(T, n, "cuda", 404, 3, step).to(torch.bfloat16)
+            D = synth.factor_samples(T, m, "cuda", 404, 4, step).to(torch.bfloat16)
+            ctx.factor_update(0, X, D)
+            ctx.refresh_basis_many([0], 8 if step == 0 else 2)
+            first = A is None
+            A = oracle.factor_accumulate(to_np64(X), A, 0.0 if first else beta)
+            Gf = oracle.factor_accumulate(to_np64(D), Gf, 0.0 if first else beta)
+            bA = oracle.refresh_basis(A, VA, 8 if first else 2, lam)
+            bG = oracle.refresh_basis(Gf, VG, 8 if first else 2, lam)
+            VA, VG = bA.U, bG.U                                    # warm start, as the library does
+        grads = [synth.rank_gradient(G, r, 404, step).to(torch.bfloat16) for r in range(R)]
+        ctx.encode_many([0] * R, grads, codes, sinvs)
+        ctx.reduce_decoded_many([0], codes, sinvs, R, [out], average=True)
+    ctx.sync_check()
+    # G7 on the transform after three refreshes
+    for side, b, d in ((gf8.SIDE_IN, bA, n), (gf8.SIDE_OUT, bG, m)):
+        U, mu, rho = ctx.get_basis(0, side)
+        Dg = np.sqrt(rho / (to_np64(mu) + lam))
+        Tg = np.eye(d) + to_np64(U) @ np.diag(Dg - 1.0) @ to_np64(U).T
+        To = oracle.build_T(b.U, b.e)
+        assert relfro(Tg, To) <= 1e-3, relfro(Tg, To)
+    # G5 (FAST) on the last step with the GPU's own basis handed to the oracle
+    def gb(side):
+        U, mu, rho = ctx.get_basis(0, side)
+        mu64 = to_np64(mu)
+        Dm = np.sqrt(rho / (mu64 + lam))
+        return oracle.Basis(to_np64(U), mu64, rho, Dm - 1.0, 1.0 / Dm - 1.0)
+    want = oracle.reduce_decoded([c_.cpu().numpy() for c_ in codes], [s_.cpu().numpy() for s_ in sinvs], gb(gf8.SIDE_OUT),
+                                 gb(gf8.SIDE_IN))
+    assert relfro(to_np64(out), want) <= 2 * TOL_FAST
+    # the averaged decoded gradient is close to the shared gradient (16 independent perturbations average out)
+    assert relfro(to_np64(out), to_np64(G)) <= 0.1
+
+
 def test_fast_batched_matches_single_calls():
     """encode_many / reduce_decoded_many with repeated layer ids (R ranks in one launch set) give the
     same bytes as one call per payload."""
