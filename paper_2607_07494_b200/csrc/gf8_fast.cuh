@@ -48,7 +48,7 @@ gf8_status fast_init(gf8_ctx* c) {
     if (!fn || q != cudaDriverEntryPointSuccess) return fail(c, GF8_ERR_CUDA, "cuTensorMapEncodeTiled not available");
     c->encode_tiled = fn;
     GF_TRY(dmalloc(c, &c->d_err, 1));
-    GF_TRY(dmalloc(c, &c->d_prof, (size_t)c->num_sms * 18 + 64));
+    GF_TRY(dmalloc(c, &c->d_prof, (size_t)c->num_sms * 36 + 64));
     CU_TRY(c, cudaMemset(c->d_err, 0, sizeof(int)));
     CU_TRY(c, cudaFuncSetAttribute(gf8::tc::tc_items_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                    gf8::tc::SMEM_BYTES));
@@ -457,19 +457,30 @@ gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
         const int n_bslots = fuse ? 3 : (n_base ? std::max(1, (gf8::tc::MAX_STAGES - n_stages) / n_base) : 1);
         if (n_base && !fuse && n_stages + n_bslots * n_base > gf8::tc::MAX_STAGES) n_stages = gf8::tc::MAX_STAGES - n_bslots * n_base;
         if (fuse && grid < c->num_sms && p->stage_cnt[s] > grid) return fail(c, GF8_ERR_BAD_STATE, "fused stage needs a full grid");
+        // GF8_TC_DBG (debug only, results are wrong with the ablation bits): 1 skip the MMAs, 2 skip the tensor-map
+        // fences, 4 print a per-role wait profile, 32 skip the strip epilogue's work, 64 skip the strip base loads,
+        // 128 skip the strip B loads, 256 print each stage's device time (serialises the stream)
         if (const char* e = getenv("GF8_TC_DBG")) dbg = atoi(e);
         if (!first_run) dbg |= 2;        // tensor maps are written once by the host before the plan's first launch
         if (const char* e = getenv("GF8_TC_ONLY")) only = atoi(e);
         if (only >= 0 && only != s) continue;
+        cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+        if (dbg & 256) { cudaEventCreate(&ev0); cudaEventCreate(&ev1); cudaEventRecord(ev0, st); }
         gf8::tc::tc_items_kernel<<<grid, gf8::tc::THREADS, gf8::tc::SMEM_BYTES, st>>>(
             p->d_items + p->stage_off[s], p->stage_cnt[s], p->d_maps, c->d_err, n_stages, n_base, n_bslots, kmode, dbg, (dbg & 4) ? c->d_prof : nullptr);
+        if (dbg & 256) {                 // GF8_TC_DBG bit 8: per-stage device time (serialises the stream)
+            float ms = 0;
+            cudaEventRecord(ev1, st); cudaEventSynchronize(ev1); cudaEventElapsedTime(&ms, ev0, ev1);
+            fprintf(stderr, "stage %d: %d items, %.1f us\n", s, p->stage_cnt[s], ms * 1e3);
+            cudaEventDestroy(ev0); cudaEventDestroy(ev1);
+        }
         if (dbg & 4) {
-            std::vector<long long> h((size_t)c->num_sms * 18);
+            std::vector<long long> h((size_t)c->num_sms * 36);
             cudaMemcpy(h.data(), c->d_prof, h.size() * sizeof(long long), cudaMemcpyDeviceToHost);
-            const char* roles[3] = {"epilogue", "producer", "mma"};
-            for (int r = 0; r < 3; ++r) {
+            const char* roles[6] = {"epilogue", "base", "load A", "load B", "mma", "mma 2"};
+            for (int r = 0; r < 6; ++r) {
                 double a[6] = {0, 0, 0, 0, 0, 0};
-                for (int b = 0; b < grid; ++b) for (int q = 0; q < 6; ++q) a[q] += (double)h[((size_t)b * 3 + r) * 6 + q] / grid;
+                for (int b = 0; b < grid; ++b) for (int q = 0; q < 6; ++q) a[q] += (double)h[((size_t)b * 6 + r) * 6 + q] / grid;
                 fprintf(stderr, "stage %d %-8s waits[0..2] %.0f %.0f %.0f  work %.0f  post %.0f  total %.0f cycles (avg/CTA)\n", s, roles[r], a[0], a[1], a[2], a[3], a[4], a[5]);
             }
         }

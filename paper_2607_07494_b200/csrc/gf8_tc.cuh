@@ -396,26 +396,29 @@ __device__ __forceinline__ void tile_values32(uint32_t taddr, uint32_t row, int 
 }
 
 // Returns true if a TMA store was issued from `tile` (the caller waits for its smem reads before reuse).
-// Each warp covers 32 rows x 64 columns (its half) as four 16-column chunks.
+// All eight warps share the tile: warp w covers rows 32 (w & 3) .. +31 of the 64-column half w >> 2.
 __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc, uint32_t tile, int n_base, int warp,
-                                              int lane, uint32_t* s_red, const CUtensorMap* maps, uint32_t amax_bits,
+                                              int lane, uint32_t* s_red, const CUtensorMap* maps, float cast_scale, float cast_si,
                                               int row0, int col0, bool write_scale, float* sinv_out, uint32_t* run_max) {
     // (row0, col0) = the tile's origin: the item's own for tile items, a tile of the strip for strip items;
     // run_max != null: EPI_AMAX accumulates into the caller's per-thread running maximum (one atomic per strip)
-    const int r = (warp & 3) * 32 + lane, half = warp >> 2, cbase = half * 64;
-    const uint32_t taddr = tmem_acc + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)cbase;
-    const uint32_t row = tile + (uint32_t)half * 16384u + (uint32_t)r * 128u;
+    const int r = (warp & 3) * 32 + lane;
+    const int h0 = warp >> 2, h1 = h0 + 1;
+    const uint32_t taddr0 = tmem_acc + ((uint32_t)((warp & 3) * 32) << 16);
+    const uint32_t row_lo = tile + (uint32_t)r * 128u;
+    const bool lead = r == 0 && h0 == 0;
     const int mode = it.mode, fmt = it.fmt;
     float v[32];
     float scale = 1.0f;
     if (mode == EPI_BLOCKCAST || mode == EPI_AMAX) {
         uint32_t loc = 0;
+        for (int h = h0; h < h1; ++h)
 #pragma unroll
-        for (int g = 0; g < 2; ++g) {
-            tile_values32(taddr, row, n_base, r, g, v);
+            for (int g = 0; g < 2; ++g) {
+                tile_values32(taddr0 + 64u * h, row_lo + 16384u * h, n_base, r, g, v);
 #pragma unroll
-            for (int u = 0; u < 32; ++u) loc = max(loc, __float_as_uint(v[u]) & 0x7FFFFFFFu);
-        }
+                for (int u = 0; u < 32; ++u) loc = max(loc, __float_as_uint(v[u]) & 0x7FFFFFFFu);
+            }
         if (mode == EPI_AMAX) {
             if (run_max) { *run_max = max(*run_max, loc); return false; }
             loc = warp_max_u32(loc);
@@ -425,35 +428,38 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
         const uint32_t bits = epi_block_max(loc, warp, lane, s_red);
         float si;
         scales_from_amax(bits, fmt == 0 ? 448.0f : 57344.0f, scale, si);
-        if (r == 0 && half == 0) *sinv_out = si;
+        if (lead) *sinv_out = si;
     } else if (mode == EPI_CAST) {
-        float si;
-        scales_from_amax(amax_bits, fmt == 0 ? 448.0f : 57344.0f, scale, si);
-        if (write_scale && r == 0 && half == 0) *sinv_out = si;
+        scale = cast_scale;                       // (from the tensor's amax, once per item by the caller)
+        if (write_scale && lead) *sinv_out = cast_si;
     }
     if (mode == EPI_CAST || mode == EPI_BLOCKCAST) {
-        // 64 codes of this row half.  Each warp owns a 32-row x 64-byte sub-tile: it stages it over its own (consumed)
-        // base rows and issues its own TMA store (map out_map + 1: 64 x 32 boxes), so the cast needs no CTA-wide sync.
-        uint4 cd[4];
+        // 64 codes per row half, written straight from registers: every thread owns 64 contiguous bytes of its row
+        // (four 16-byte stores; L2 merges the sectors), so the cast needs neither shared-memory staging nor a
+        // generic -> async proxy fence, and the base slot goes back to the producer at once.
+        const int grow = row0 + r;
+        const bool row_ok = grow < it.row0 + it.rows;
+        for (int h = h0; h < h1; ++h) {
+            uint4 cd[4];
 #pragma unroll
-        for (int g = 0; g < 2; ++g) {
-            tile_values32(taddr, row, n_base, r, g, v);
-            cd[2 * g] = fmt == 0 ? codes16<0>(v, scale) : codes16<1>(v, scale);
-            cd[2 * g + 1] = fmt == 0 ? codes16<0>(v + 16, scale) : codes16<1>(v + 16, scale);
-        }
-        __syncwarp();                             // every lane of this warp has read its base rows
-        const uint32_t sub = tile + (uint32_t)half * 16384u + (uint32_t)((warp & 3) * 32) * 128u;   // this warp's 4 KB
+            for (int g = 0; g < 2; ++g) {
+                tile_values32(taddr0 + 64u * h, row_lo + 16384u * h, n_base, r, g, v);
+                cd[2 * g] = fmt == 0 ? codes16<0>(v, scale) : codes16<1>(v, scale);
+                cd[2 * g + 1] = fmt == 0 ? codes16<0>(v + 16, scale) : codes16<1>(v + 16, scale);
+            }
+            if (row_ok) {
+                uint8_t* p = reinterpret_cast<uint8_t*>(it.out) + (int64_t)grow * it.out_ld + col0 + 64 * h;
 #pragma unroll
-        for (int q = 0; q < 4; ++q) sts128(sub + (uint32_t)lane * 64u + 16u * q, cd[q]);
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-        __syncwarp();
-        if (lane == 0) {
-            tma_store_2d(maps + it.out_map + 1, sub, col0 + cbase, row0 + (warp & 3) * 32);
-            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                for (int q = 0; q < 4; ++q)
+                    if (col0 + 64 * h + 16 * q < it.col0 + it.cols) *reinterpret_cast<uint4*>(p + 16 * q) = cd[q];
+            }
         }
-        return true;
+        return false;
     }
-    // EPI_STORE, BF16 output in place of the hi tile (same layout), or FP32 output straight to global memory
+    // EPI_STORE: BF16 output in place of the hi tile (same layout) and out through a TMA
+    // store, or FP32 output straight to global memory
+    const int half = h0, cbase = half * 64;
+    const uint32_t taddr = taddr0 + (uint32_t)cbase, row = row_lo + 16384u * half;
     if (it.out_type == TY_BF16) {
 #pragma unroll
         for (int g = 0; g < 2; ++g) {
@@ -527,19 +533,21 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
     auto iempty_bar = [&](int s) { return bars + 8u * (2 * MAX_STAGES + 8 + 2 * MAX_BASE_SLOTS + ITEM_SLOTS + s); };
     auto parked_bar = [&](int a) { return bars + 8u * (2 * MAX_STAGES + 8 + 2 * MAX_BASE_SLOTS + 2 * ITEM_SLOTS + a); };
     auto sready_bar = [&](int a) { return bars + 8u * (2 * MAX_STAGES + 8 + 2 * MAX_BASE_SLOTS + 2 * ITEM_SLOTS + 4 + a); };
+    auto drain_bar = [&](int a) { return bars + 8u * (2 * MAX_STAGES + 8 + 2 * MAX_BASE_SLOTS + 2 * ITEM_SLOTS + 8 + a); };
     float* s_scale = reinterpret_cast<float*>(s_red + 8);     // fused update: scale of each parked tile's tensor
     const uint32_t n_acc = 4u;                       // TMEM accumulator slots in rotation (4 x 128 columns)
     auto base_tile = [&](uint32_t b) { return base0 + b * (uint32_t)n_base * TILE_BYTES; };
     auto item_slot = [&](uint32_t s) { return reinterpret_cast<const Item*>(s_items + s * ITEM_BYTES); };
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < MAX_STAGES; ++s) { mbar_init(full_bar(s), strip ? 1 : 2); mbar_init(empty_bar(s), 1); }
+        for (int s = 0; s < MAX_STAGES; ++s) { mbar_init(full_bar(s), strip ? 1 : 2); mbar_init(empty_bar(s), strip ? 2 : 1); }
         for (int a = 0; a < 4; ++a) {
-            mbar_init(parked_bar(a), 1); mbar_init(sready_bar(a), 1);
+            mbar_init(parked_bar(a), strip && a == 1 ? 2 : 1); mbar_init(sready_bar(a), 1);
             mbar_init(tfull_bar(a), 1); mbar_init(tempty_bar(a), EPI_WARPS);
         }
+        mbar_init(drain_bar(0), 1); mbar_init(drain_bar(1), 1);
         for (int b = 0; b < MAX_BASE_SLOTS; ++b) { mbar_init(bfull_bar(b), 1); mbar_init(bempty_bar(b), EPI_WARPS); }
-        for (int s = 0; s < ITEM_SLOTS; ++s) { mbar_init(ifull_bar(s), 1); mbar_init(iempty_bar(s), EPI_WARPS + 3); }
+        for (int s = 0; s < ITEM_SLOTS; ++s) { mbar_init(ifull_bar(s), 1); mbar_init(iempty_bar(s), EPI_WARPS + (strip ? 4 : 3)); }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == MMA_WARP) {
@@ -583,10 +591,13 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                         const uint32_t bs = b_count % (uint32_t)n_bslots, bph = (b_count / (uint32_t)n_bslots) & 1u;
                         ok = TWAIT(1, mbar_wait(bempty_bar(bs), bph ^ 1u, err)) ? 1 : 0;
                         if (ok && elect_one()) {
+                            if (dbg & 64) mbar_arrive(bfull_bar(bs));
+                            else {
                             mbar_expect_tx(bfull_bar(bs), TILE_BYTES);
 #pragma unroll
                             for (int h = 0; h < 2; ++h)
                                 tma_load_2d(base_tile(bs) + h * 16384u, mp, 128 * ct + 64 * h, row0 + 128 * rb, bfull_bar(bs));
+                            }
                         }
                         __syncwarp();
                     }
@@ -652,9 +663,12 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                                 for (int t = 0; t < it.atoms[seg]; ++t) {
                                     if (!TWAIT(2, mbar_wait(empty_bar(stage), phase ^ 1u, err))) { ok = false; break; }
                                     if (elect_one()) {
+                                        if (dbg & 128) mbar_arrive(full_bar(stage));
+                                        else {
                                         mbar_expect_tx(full_bar(stage), B_BYTES);
                                         tma_load_2d(smem0 + STRIP_L_BYTES + stage * B_BYTES, maps + it.map_b[seg],
                                                     it.b_c0[seg] + 64 * t, it.b_r0[seg] + 128 * ct, full_bar(stage));
+                                        }
                                     }
                                     __syncwarp();
                                     if (++stage == (uint32_t)STRIP_RING) { stage = 0; phase ^= 1u; }
@@ -699,8 +713,11 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 if (elect_one()) mbar_arrive(iempty_bar(slot));
             }
         }
-    } else if (warp == MMA_WARP) {
+    } else if (warp == MMA_WARP || (strip && warp == SYNC_WARP)) {
         // ===== MMA issuer (converged warp, one elected lane issues) =====
+        // Strip items have two issuers: warp 11 takes row block 0 of every column tile, warp 12 row block 1.  One
+        // issuer's serial stream (barrier waits, fences, 8 MMAs and the commits of a tile) is otherwise what bounds the
+        // tile rate (measured: ~1400 cycles per tile with everything else switched off).
         {
             uint32_t stage = 0, phase = 0, n_done = 0, t_count = 0;
             bool ok = true;
@@ -716,38 +733,40 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 if (strip) {
                     // strip item: A tiles resident, per column tile the B atoms serve both row blocks
                     const int nrb = (it.rows + 127) >> 7, nct = (it.cols + 127) >> 7;
+                    const int rb = warp == MMA_WARP ? 0 : 1;
+                    const bool mine = rb < nrb;              // (a 128-row strip: the second issuer only keeps the barriers in step)
                     __syncwarp();
                     if (elect_one()) mbar_arrive(iempty_bar(slot));
                     if (!(ok = TWAIT(0, mbar_wait(parked_bar(0), n_done & 1u, err)))) break;       // A tiles landed
                     tc_fence_after();
                     for (int ct = 0; ct < nct && ok; ++ct) {
-                        for (int rb = 0; rb < nrb && ok; ++rb, ++t_count) {
-                            const uint32_t acc = t_count % n_acc, aphase = (t_count / n_acc) & 1u;
+                        const uint32_t tc_ = t_count + (uint32_t)rb;
+                        const uint32_t acc = tc_ % n_acc, aphase = (tc_ / n_acc) & 1u;
+                        t_count += (uint32_t)nrb;
+                        if (mine) {
                             if (!(ok = TWAIT(1, mbar_wait(tempty_bar(acc), aphase ^ 1u, err)))) break;
                             tc_fence_after();
-                            const uint32_t d = tmem_base + acc * 128u;
-                            for (int a = 0; a < total; ++a) {
-                                const uint32_t st_a = (stage + (uint32_t)a) % STRIP_RING;
-                                const uint32_t ph_a = phase ^ ((stage + (uint32_t)a) >= (uint32_t)STRIP_RING ? 1u : 0u);
-                                if (rb == 0) {
-                                    if (!(ok = TWAIT(2, mbar_wait(full_bar(st_a), ph_a, err)))) break;
-                                    tc_fence_after();
-                                }
-                                const uint32_t sa = smem0 + (uint32_t)(rb * 2 + a) * A_BYTES;
-                                const uint32_t sb = smem0 + STRIP_L_BYTES + st_a * B_BYTES;
-                                if (elect_one()) {
+                        }
+                        const uint32_t d = tmem_base + acc * 128u;
+                        for (int a = 0; a < total; ++a) {
+                            const uint32_t st_a = (stage + (uint32_t)a) % STRIP_RING;
+                            const uint32_t ph_a = phase ^ ((stage + (uint32_t)a) >= (uint32_t)STRIP_RING ? 1u : 0u);
+                            if (!(ok = TWAIT(2, mbar_wait(full_bar(st_a), ph_a, err)))) break;
+                            tc_fence_after();
+                            const uint32_t sa = smem0 + (uint32_t)(rb * 2 + a) * A_BYTES;
+                            const uint32_t sb = smem0 + STRIP_L_BYTES + st_a * B_BYTES;
+                            if (elect_one()) {
+                                if (mine && !(dbg & 1)) {
 #pragma unroll
                                     for (int kk = 0; kk < 4; ++kk)
                                         tc_mma_bf16(d, smem_desc(sa + 32u * kk, 16u, 1024u), smem_desc(sb + 32u * kk, 16u, 1024u),
                                                     idesc, (a | kk) ? 1u : 0u);
                                 }
-                                __syncwarp();
+                                tc_commit(empty_bar(st_a));      // (two arrivals free the ring stage: one per issuer)
                             }
-                            if (ok && elect_one()) tc_commit(tfull_bar(acc));
                             __syncwarp();
                         }
-                        if (ok && elect_one())
-                            for (int a = 0; a < total; ++a) tc_commit(empty_bar((stage + (uint32_t)a) % STRIP_RING));
+                        if (ok && mine && elect_one()) tc_commit(tfull_bar(acc));
                         __syncwarp();
                         stage += (uint32_t)total;
                         if (stage >= (uint32_t)STRIP_RING) { stage -= STRIP_RING; phase ^= 1u; }
@@ -780,6 +799,15 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 }
                 if (ok && elect_one()) tc_commit(tfull_bar(acc));   // accumulator complete -> epilogue
                 __syncwarp();
+            }
+            // Drain: commits complete in issue order, so once this last one has arrived no mbarrier arrive of this
+            // issuer is still in flight when the CTA exits (a late arrive would land in the shared memory of the
+            // next kernel's CTA on this SM).
+            if (ok) {
+                const uint32_t db = drain_bar(warp == MMA_WARP ? 0 : 1);
+                if (elect_one()) tc_commit(db);
+                __syncwarp();
+                mbar_wait(db, 0u, err);
             }
         }
     } else if (warp == SYNC_WARP) {
@@ -920,8 +948,10 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
             const uint32_t bs = n_base > 0 ? n_done % (uint32_t)n_bslots : 0u, bphase = n_base > 0 ? (n_done / (uint32_t)n_bslots) & 1u : 0u;
             ok = TWAIT(0, mbar_wait(ifull_bar(slot), iphase, err));
             // the tensor's amax (EPI_CAST) is fetched before the data waits, so its latency hides behind them
-            uint32_t amax_bits = 0;
-            if (ok && item_slot(slot)->mode == EPI_CAST) amax_bits = *reinterpret_cast<volatile uint32_t*>(item_slot(slot)->amax);
+            float cast_scale = 1.0f, cast_si = 1.0f;
+            if (ok && item_slot(slot)->mode == EPI_CAST)
+                scales_from_amax(*reinterpret_cast<volatile uint32_t*>(item_slot(slot)->amax), item_slot(slot)->fmt == 0 ? 448.0f : 57344.0f,
+                                 cast_scale, cast_si);
             if (strip) {
                 // strip item: (column tile, row block) tiles in order; one amax atomic per warp per strip
                 ok = __all_sync(0xFFFFFFFFu, ok);
@@ -939,24 +969,16 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                         if (!ok) break;
                         tc_fence_after();
                         const long long t_s0 = prof ? clock64() : 0;
-                        const bool stored = epilogue_tile(it, tmem_base + sacc * 128u, base_tile(sbs), 1, warp, lane, s_red, maps, amax_bits,
-                                                          it.row0 + 128 * rb, 128 * ct, it.write_scale != 0 && ct == 0 && rb == 0,
-                                                          it.mode == EPI_BLOCKCAST ? it.scale_inv_out + (size_t)((it.row0 >> 7) + rb) * nct + ct
-                                                                                   : it.scale_inv_out,
-                                                          &run_max);
+                        if (!(dbg & 32))
+                            epilogue_tile(it, tmem_base + sacc * 128u, base_tile(sbs), 1, warp, lane, s_red, maps, cast_scale, cast_si,
+                                          it.row0 + 128 * rb, 128 * ct, it.write_scale != 0 && ct == 0 && rb == 0,
+                                          it.mode == EPI_BLOCKCAST ? it.scale_inv_out + (size_t)((it.row0 >> 7) + rb) * nct + ct
+                                                                   : it.scale_inv_out,
+                                          &run_max);
                         tc_fence_before();
                         __syncwarp();
-                        // every warp returns the base slot itself; after a TMA store from it, one tile later (when
-                        // the store has read its shared memory), so the wait overlaps the next tile
-                        if (lane == 0) {
-                            mbar_arrive(tempty_bar(sacc));
-                            if (pending_slot >= 0) {
-                                asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-                                mbar_arrive(bempty_bar(pending_slot));
-                            }
-                            if (!stored) mbar_arrive(bempty_bar(sbs));
-                        }
-                        pending_slot = stored ? (int)sbs : -1;
+                        // (codes leave through plain stores, so the base slot goes straight back to the producer)
+                        if (lane == 0) { mbar_arrive(tempty_bar(sacc)); mbar_arrive(bempty_bar(sbs)); }
                         if (prof) pw[3] += clock64() - t_s0;
                     }
                 if (ok && it.mode == EPI_AMAX) {
@@ -976,7 +998,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
             const Item& it = *item_slot(slot);
             bool stored = false;
             if (it.base_map[0] >= 0)
-                stored = epilogue_tile(it, tmem_base + acc * 128u, base_tile(bs), it.base_map[1] >= 0 ? 2 : 1, warp, lane, s_red, maps, amax_bits,
+                stored = epilogue_tile(it, tmem_base + acc * 128u, base_tile(bs), it.base_map[1] >= 0 ? 2 : 1, warp, lane, s_red, maps, cast_scale, cast_si,
                                        it.row0, it.col0, it.write_scale != 0, it.scale_inv_out, nullptr);
             else
                 epilogue(it, tmem_base + acc * 128u, warp, lane, s_red);
@@ -991,7 +1013,9 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 // overlaps the next tile instead of stalling this warp.
                 if (lane == 0) {
                     if (pending_slot >= 0) {
-                        asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+                        // (the group just committed by this tile's own store may stay in flight)
+                        if (stored) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+                        else asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
                         mbar_arrive(bempty_bar(pending_slot));
                     }
                     if (!stored) mbar_arrive(bempty_bar(bs));
@@ -1003,10 +1027,10 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
         if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // (pending slot: kernel ends)
     }
 #undef TWAIT
-    if (prof && lane == 0 && (warp == 0 || warp == OPERAND_WARP || warp == MMA_WARP)) {
-        const int role = warp == 0 ? 0 : (warp == OPERAND_WARP ? 1 : 2);
+    if (prof && lane == 0 && (warp == 0 || warp >= PRODUCER_WARP)) {
+        const int role = warp == 0 ? 0 : warp - PRODUCER_WARP + 1;       // epilogue, base producer, A, B, MMA, MMA 2 / sync
         pw[5] = clock64() - t_start;
-        for (int q = 0; q < 6; ++q) prof[((size_t)blockIdx.x * 3 + role) * 6 + q] = pw[q];
+        for (int q = 0; q < 6; ++q) prof[((size_t)blockIdx.x * 6 + role) * 6 + q] = pw[q];
     }
     tc_fence_before();
     __syncthreads();
