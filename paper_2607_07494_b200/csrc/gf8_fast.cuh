@@ -12,7 +12,7 @@
 struct Plan {
     CUtensorMap* d_maps = nullptr;
     gf8::tc::Item* d_items = nullptr;
-    // stages: 0 P', 1 Q^T (+S), 2 Q'^T, 3 update tiles (amax / block cast / store), 4 update tiles (cast),
+    // stages: 0 P' and Q^T, 1 S, 2 Q'^T, 3 update tiles (amax / block cast / store), 4 update tiles (cast),
     //         5 update strips (amax / block cast), 6 update strips (cast), 7 fused update (opt-in)
     int stage_off[8] = {0, 0, 0, 0, 0, 0, 0, 0}, stage_cnt[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     int stage_base[8] = {0, 0, 0, 0, 0, 0, 0, 0};  // streamed base tiles per item in that stage's launch (0, 1 or 2)
@@ -194,6 +194,8 @@ struct PlanBuilder {
     std::vector<CUtensorMap> maps;
     std::map<const void*, int> map_index;      // buffer -> index (static maps are shared by all problems)
     std::vector<Item> stage[8];
+    std::vector<int> prob0;                    // stage 0: the problem (add_transform call) each item belongs to
+    int cur_problem = 0;
     // registers both box heights of a buffer; returns the index of the 64-row-box map, +1 is the 128-row-box map
     int add_map(const void* key, const CUtensorMap* m2) {
         auto it = map_index.find(key);
@@ -270,7 +272,12 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
         if (a.lo >= 0) one(a.lo, b.hi);
         if (b.lo >= 0) one(a.hi, b.lo);
     };
-    // panels wider than 128 basis columns are cut into 128-column accumulator chunks (nc)
+    // panels wider than 128 basis columns are cut into 128-column accumulator chunks (nc).
+    // The row panels (P') and the column panels (Q^T) of a problem both stream the whole source: they share stage 0
+    // and stay next to each other in its item list, so the CTAs working on one problem at a time fetch every source
+    // byte from HBM once and find it in L2 the second time.
+    const int problem = pb.cur_problem++;
+    auto push0 = [&](const Item& it) { pb.stage[0].push_back(it); pb.prob0.push_back(problem); };
     if (useA)      // P' = (src U_A) E_A : row panels
         for (int i0 = 0; i0 < m; i0 += 128)
             for (int nc = 0; nc < kpA; nc += 128) {
@@ -281,7 +288,7 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
                 it.mode = EPI_STORE; it.out = s->Pp; it.out_lo = split ? s->Pp_lo : nullptr; it.out_ld = kpA;
                 it.out_type = TY_BF16; it.colscale = eA + nc;
                 it.row0 = i0; it.col0 = nc; it.rows = std::min(128, m - i0); it.cols = it.N;
-                pb.stage[0].push_back(it);
+                push0(it);
             }
     if (useG) {    // Q^T = src^T U_G : column panels (A is MN-major)
         for (int j0 = 0; j0 < n; j0 += 128)
@@ -296,7 +303,7 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
                     it.out = s->Qpt; it.out_lo = split ? s->Qpt_lo : nullptr; it.out_ld = kpG; it.out_type = TY_BF16;
                     it.colscale = eG + nc;
                 }
-                pb.stage[1].push_back(it);
+                push0(it);
             }
         if (useA) {
             // (S E_A)^T = P'^T U_G, stored transposed as SEA[g][a]
@@ -402,8 +409,26 @@ void plan_free(Plan* p) {
 // Upload the builder's maps and items (longest contractions first within a stage: CTAs take items round-robin).
 gf8_status plan_finish(gf8_ctx* c, PlanBuilder& pb, Plan* p) {
     std::vector<Item> all;
+    if (pb.prob0.size() == pb.stage[0].size() && !pb.stage[0].empty()) {
+        // stage 0: heaviest problems first, each problem's panels contiguous (L2 reuse of the source, see add_transform)
+        std::vector<int64_t> work(pb.cur_problem, 0);
+        for (size_t i = 0; i < pb.stage[0].size(); ++i)
+            for (int g = 0; g < gf8::tc::NSEG; ++g) work[pb.prob0[i]] += pb.stage[0][i].atoms[g];
+        std::vector<int> order(pb.stage[0].size());
+        for (size_t i = 0; i < order.size(); ++i) order[i] = (int)i;
+        std::stable_sort(order.begin(), order.end(), [&](int a, int b) {
+            const int pa = pb.prob0[a], pq = pb.prob0[b];
+            if (work[pa] != work[pq]) return work[pa] > work[pq];
+            return pa < pq;
+        });
+        std::vector<Item> sorted;
+        sorted.reserve(order.size());
+        for (int i : order) sorted.push_back(pb.stage[0][i]);
+        pb.stage[0].swap(sorted);
+    }
     for (int s = 0; s < 8; ++s) {
-        std::stable_sort(pb.stage[s].begin(), pb.stage[s].end(), [](const Item& a, const Item& b) {
+        const bool grouped = s == 0 && pb.prob0.size() == pb.stage[0].size();
+        if (!grouped) std::stable_sort(pb.stage[s].begin(), pb.stage[s].end(), [](const Item& a, const Item& b) {
             int64_t ta = 0, tb = 0;
             for (int g = 0; g < gf8::tc::NSEG; ++g) { ta += a.atoms[g]; tb += b.atoms[g]; }
             if (a.strip) ta *= (int64_t)((a.rows + 127) / 128) * ((a.cols + 127) / 128);
