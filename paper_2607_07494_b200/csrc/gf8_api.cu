@@ -476,11 +476,37 @@ gf8_status fast_reduce_decoded_many(gf8_ctx* c, int n, const int* layers, const 
         if (s == GF8_OK) s = plan_store(c, key, p);
         if (s != GF8_OK) { plan_free(p); return s; }
     }
-    for (const Plan::Reduce& rd : p->reduces) {
-        const int i = rd.batch_index;
-        const LayerState& L = c->layers[layers[i]];
-        GF_TRY(reduce_dev<float>(c, st, codes + (size_t)i * R, sinv + (size_t)i * R, R, average, L.desc.d_out, L.desc.d_in,
-                                 L.desc.fmt, L.desc.scaling, rd.uhat, rd.u16, rd.u16_lo));
+    // payload reduction into the slots: grouped launches (same format / scaling, R <= 8), else one launch per tensor
+    for (size_t q = 0; q < p->reduces.size();) {
+        const Plan::Reduce& rd0 = p->reduces[q];
+        const LayerState& L0 = c->layers[layers[rd0.batch_index]];
+        if (R > 8 || rd0.uhat) {
+            const int i = rd0.batch_index;
+            GF_TRY(reduce_dev<float>(c, st, codes + (size_t)i * R, sinv + (size_t)i * R, R, average, L0.desc.d_out, L0.desc.d_in,
+                                     L0.desc.fmt, L0.desc.scaling, rd0.uhat, rd0.u16, rd0.u16_lo));
+            ++q;
+            continue;
+        }
+        ReduceBatch b;
+        memset(&b, 0, sizeof(b));
+        b.R = R; b.average = average; b.scaling = L0.desc.scaling;
+        int64_t blocks = 0;
+        while (q < p->reduces.size() && b.n_jobs < REDUCE_MAX_JOBS) {
+            const Plan::Reduce& rd = p->reduces[q];
+            const int i = rd.batch_index;
+            const LayerState& L = c->layers[layers[i]];
+            if (L.desc.fmt != L0.desc.fmt || L.desc.scaling != L0.desc.scaling || rd.uhat) break;
+            ReduceJob& jb = b.job[b.n_jobs++];
+            for (int r = 0; r < R; ++r) { jb.codes[r] = codes[(size_t)i * R + r]; jb.sinv[r] = sinv[(size_t)i * R + r]; }
+            jb.out16 = rd.u16; jb.out16_lo = rd.u16_lo;
+            jb.n_groups = (int64_t)L.desc.d_out * L.desc.d_in / 16; jb.n = L.desc.d_in;
+            jb.first_block = blocks;
+            blocks += (jb.n_groups + REDUCE_GROUPS_PER_BLOCK - 1) / REDUCE_GROUPS_PER_BLOCK;
+            ++q;
+        }
+        if (L0.desc.fmt == GF8_E4M3) reduce_many_kernel<0><<<(unsigned)blocks, 256, 0, st>>>(b);
+        else reduce_many_kernel<1><<<(unsigned)blocks, 256, 0, st>>>(b);
+        LAUNCH_CHECK(c);
     }
     const bool overlap = !p->plain.empty() && !p->reduces.empty();
     cudaStream_t sp = st;

@@ -210,6 +210,85 @@ __global__ void __launch_bounds__(256) reduce_kernel(const __grid_constant__ Red
     }
 }
 
+// Grouped form of the reduction for the FAST decode path: up to 22 tensors per launch (the jobs travel as kernel
+// parameters), R <= 8 payloads each, result written as hi + lo BF16 (the operands of the unwhitening MMAs).
+// Block b covers 1024 16-element groups of its job; a thread keeps all R 16-byte loads of a group in flight.
+// Same arithmetic as reduce_kernel: acc = fma(value_r, scale_inv_r, acc) in rank order, then * (1/R).
+constexpr int REDUCE_MAX_JOBS = 22, REDUCE_GROUPS_PER_BLOCK = 1024;
+struct ReduceJob {
+    const uint8_t* codes[8];
+    const float* sinv[8];
+    bf16* out16;
+    bf16* out16_lo;
+    int64_t n_groups;             // m * n / 16
+    int64_t n;                    // columns (block scaling only)
+    int64_t first_block;          // first block of this job in the launch
+};
+struct ReduceBatch {
+    int32_t n_jobs, R, average, scaling;
+    ReduceJob job[REDUCE_MAX_JOBS];
+};
+
+template <int FMT>
+__global__ void __launch_bounds__(256) reduce_many_kernel(const __grid_constant__ ReduceBatch b) {
+    int j = 0;
+    while (j + 1 < b.n_jobs && (int64_t)blockIdx.x >= b.job[j + 1].first_block) ++j;
+    const ReduceJob& jb = b.job[j];
+    const int R = b.R;
+    const float invR = __fdiv_rn(1.0f, (float)R);
+    const int64_t g0 = ((int64_t)blockIdx.x - jb.first_block) * REDUCE_GROUPS_PER_BLOCK;
+    const int64_t bn = (jb.n + 127) / 128;
+#pragma unroll 1
+    for (int it = 0; it < REDUCE_GROUPS_PER_BLOCK / 256; ++it) {
+        const int64_t g = g0 + it * 256 + threadIdx.x;
+        if (g >= jb.n_groups) break;
+        const int64_t e0 = g * 16;
+        int64_t sidx = 0;
+        if (b.scaling != 0) { const int64_t r = e0 / jb.n, c = e0 % jb.n; sidx = (r / 128) * bn + c / 128; }
+        uint4 c[8];
+        float s[8];
+#pragma unroll
+        for (int r = 0; r < 8; ++r)
+            if (r < R) { c[r] = ld_stream(reinterpret_cast<const uint4*>(jb.codes[r] + e0)); s[r] = __ldg(jb.sinv[r] + sidx); }
+        float acc[16];
+#pragma unroll
+        for (int u = 0; u < 16; ++u) acc[u] = 0.0f;
+#pragma unroll
+        for (int r = 0; r < 8; ++r)
+            if (r < R) {
+                float v[16];
+                fp8x4_to_f32x4<FMT>(c[r].x, v); fp8x4_to_f32x4<FMT>(c[r].y, v + 4);
+                fp8x4_to_f32x4<FMT>(c[r].z, v + 8); fp8x4_to_f32x4<FMT>(c[r].w, v + 12);
+#pragma unroll
+                for (int u = 0; u < 16; ++u) acc[u] = __fmaf_rn(v[u], s[r], acc[u]);
+            }
+        if (b.average) {
+#pragma unroll
+            for (int u = 0; u < 16; ++u) acc[u] = __fmul_rn(acc[u], invR);
+        }
+        uint32_t w[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const __nv_bfloat162 h = __floats2bfloat162_rn(acc[2 * u], acc[2 * u + 1]);
+            w[u] = *reinterpret_cast<const uint32_t*>(&h);
+        }
+        uint4* o2 = reinterpret_cast<uint4*>(jb.out16 + e0);
+        o2[0] = make_uint4(w[0], w[1], w[2], w[3]);
+        o2[1] = make_uint4(w[4], w[5], w[6], w[7]);
+        if (jb.out16_lo) {
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const float2 hi = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(&w[u]));
+                const __nv_bfloat162 h = __floats2bfloat162_rn(acc[2 * u] - hi.x, acc[2 * u + 1] - hi.y);
+                w[u] = *reinterpret_cast<const uint32_t*>(&h);
+            }
+            uint4* o3 = reinterpret_cast<uint4*>(jb.out16_lo + e0);
+            o3[0] = make_uint4(w[0], w[1], w[2], w[3]);
+            o3[1] = make_uint4(w[4], w[5], w[6], w[7]);
+        }
+    }
+}
+
 // FP32 -> BF16 (RNE) / FP32 copy of a contiguous tensor, and BF16 -> FP32 widening.
 template <typename TI, typename TO>
 __global__ void __launch_bounds__(256) convert_kernel(const TI* __restrict__ in, int64_t numel, TO* __restrict__ out) {

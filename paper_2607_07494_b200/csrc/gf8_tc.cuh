@@ -567,7 +567,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
     if (warp == PRODUCER_WARP) {
         // ===== item fetch (whole warp) + TMA producer (lane 0) =====
         constexpr int NCHUNK = ITEM_BYTES / 16;
-        uint32_t stage = 0, phase = 0, n_done = 0, b_count = 0;
+        uint32_t stage = 0, phase = 0, n_done = 0, b_bs = 0, b_bph = 0;
         int ok = 1;
         uint4 nxt = make_uint4(0, 0, 0, 0);
         if ((int)blockIdx.x < n_items && lane < NCHUNK) nxt = __ldg(reinterpret_cast<const uint4*>(items + blockIdx.x) + lane);
@@ -587,8 +587,9 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 const int bm0 = it.base_map[0], row0 = it.row0, nrb = (it.rows + 127) >> 7, nct = (it.cols + 127) >> 7;
                 const CUtensorMap* mp = maps + bm0;
                 for (int ct = 0; ct < nct && ok; ++ct)
-                    for (int rb = 0; rb < nrb && ok; ++rb, ++b_count) {
-                        const uint32_t bs = b_count % (uint32_t)n_bslots, bph = (b_count / (uint32_t)n_bslots) & 1u;
+                    for (int rb = 0; rb < nrb && ok; ++rb) {
+                        const uint32_t bs = b_bs, bph = b_bph;
+                        if (++b_bs == (uint32_t)n_bslots) { b_bs = 0; b_bph ^= 1u; }
                         ok = TWAIT(1, mbar_wait(bempty_bar(bs), bph ^ 1u, err)) ? 1 : 0;
                         if (ok && elect_one()) {
                             if (dbg & 64) mbar_arrive(bfull_bar(bs));
@@ -939,7 +940,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
         if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     } else {
         // ===== epilogue warps 0..7 =====
-        uint32_t n_done = 0, s_tiles = 0;
+        uint32_t n_done = 0, s_tiles = 0, s_bs = 0, s_bph = 0;
         int pending_slot = -1;
         bool ok = true;
         for (int i = blockIdx.x; i < n_items && ok; i += gridDim.x, ++n_done) {
@@ -962,7 +963,8 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 for (int ct = 0; ct < nct && ok; ++ct)
                     for (int rb = 0; rb < nrb && ok; ++rb, ++s_tiles) {
                         const uint32_t sacc = s_tiles % n_acc, saph = (s_tiles / n_acc) & 1u;
-                        const uint32_t sbs = s_tiles % (uint32_t)n_bslots, sbph = (s_tiles / (uint32_t)n_bslots) & 1u;
+                        const uint32_t sbs = s_bs, sbph = s_bph;       // = s_tiles % n_bslots, (s_tiles / n_bslots) & 1
+                        if (++s_bs == (uint32_t)n_bslots) { s_bs = 0; s_bph ^= 1u; }
                         ok = TWAIT(1, mbar_wait(bfull_bar(sbs), sbph, err));
                         ok = ok && TWAIT(2, mbar_wait(tfull_bar(sacc), saph, err));
                         ok = __all_sync(0xFFFFFFFFu, ok);
