@@ -15,6 +15,7 @@ struct Plan {
     // stages: 0 P' and Q^T, 1 S, 2 Q'^T, 3 update tiles (amax / block cast / store), 4 update tiles (cast),
     //         5 update strips (amax / block cast), 6 update strips (cast), 7 fused update (opt-in)
     int stage_off[8] = {0, 0, 0, 0, 0, 0, 0, 0}, stage_cnt[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    int stage_wide[8] = {0, 0, 0, 0, 0, 0, 0, 0};  // the stage holds 256-row panel items: wide operand stages (kmode 3)
     int stage_base[8] = {0, 0, 0, 0, 0, 0, 0, 0};  // streamed base tiles per item in that stage's launch (0, 1 or 2)
     int runs = 0;                        // launches so far: the first one acquires its tensor maps with proxy fences
     uint32_t* d_amax = nullptr;          // one word per TC problem (per-tensor scaling)
@@ -278,8 +279,10 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
     // byte from HBM once and find it in L2 the second time.
     const int problem = pb.cur_problem++;
     auto push0 = [&](const Item& it) { pb.stage[0].push_back(it); pb.prob0.push_back(problem); };
+    // (kp <= 64: one item covers 256 rows, its two 128-row accumulators share every basis atom the loader brings in)
+    const int stepA = kpA <= 64 ? 256 : 128, stepG = kpG <= 64 ? 256 : 128;
     if (useA)      // P' = (src U_A) E_A : row panels
-        for (int i0 = 0; i0 < m; i0 += 128)
+        for (int i0 = 0; i0 < m; i0 += stepA)
             for (int nc = 0; nc < kpA; nc += 128) {
                 Item it = blank_item();
                 int seg = 0;
@@ -287,17 +290,17 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
                 add_product(it, seg, mSrc, mUAt, (n + 63) / 64, 0, i0, 0, nc);
                 it.mode = EPI_STORE; it.out = s->Pp; it.out_lo = split ? s->Pp_lo : nullptr; it.out_ld = kpA;
                 it.out_type = TY_BF16; it.colscale = eA + nc;
-                it.row0 = i0; it.col0 = nc; it.rows = std::min(128, m - i0); it.cols = it.N;
+                it.row0 = i0; it.col0 = nc; it.rows = std::min(stepA, m - i0); it.cols = it.N;
                 push0(it);
             }
     if (useG) {    // Q^T = src^T U_G : column panels (A is MN-major)
-        for (int j0 = 0; j0 < n; j0 += 128)
+        for (int j0 = 0; j0 < n; j0 += stepG)
             for (int nc = 0; nc < kpG; nc += 128) {
                 Item it = blank_item();
                 int seg = 0;
                 it.a_mn = 1; it.N = std::min(128, kpG - nc);
                 add_product(it, seg, mSrc, mUGt, (m + 63) / 64, j0, 0, 0, nc);
-                it.mode = EPI_STORE; it.row0 = j0; it.col0 = nc; it.rows = std::min(128, n - j0); it.cols = it.N;
+                it.mode = EPI_STORE; it.row0 = j0; it.col0 = nc; it.rows = std::min(stepG, n - j0); it.cols = it.N;
                 if (useA) { it.out = s->Qt; it.out_ld = kpG; it.out_type = TY_F32; }
                 else {
                     it.out = s->Qpt; it.out_lo = split ? s->Qpt_lo : nullptr; it.out_ld = kpG; it.out_type = TY_BF16;
@@ -319,7 +322,7 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
                     pb.stage[1].push_back(it);
                 }
             // Q'^T = (Q^T + U_A (S E_A)^T) E_G
-            for (int j0 = 0; j0 < n; j0 += 128)
+            for (int j0 = 0; j0 < n; j0 += stepG)
                 for (int nc = 0; nc < kpG; nc += 128) {
                     Item it = blank_item();
                     int seg = 0;
@@ -328,7 +331,7 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
                     it.mode = EPI_STORE; it.base = s->Qt; it.base_ld = kpG; it.base_type = TY_F32;
                     it.out = s->Qpt; it.out_lo = split ? s->Qpt_lo : nullptr; it.out_ld = kpG; it.out_type = TY_BF16;
                     it.colscale = eG + nc;
-                    it.row0 = j0; it.col0 = nc; it.rows = std::min(128, n - j0); it.cols = it.N;
+                    it.row0 = j0; it.col0 = nc; it.rows = std::min(stepG, n - j0); it.cols = it.N;
                     pb.stage[2].push_back(it);
                 }
         }
@@ -437,8 +440,12 @@ gf8_status plan_finish(gf8_ctx* c, PlanBuilder& pb, Plan* p) {
         });
         p->stage_off[s] = (int)all.size();
         p->stage_cnt[s] = (int)pb.stage[s].size();
-        for (const Item& it : pb.stage[s])
+        for (const Item& it : pb.stage[s]) {
             p->stage_base[s] = std::max(p->stage_base[s], (it.base_map[0] >= 0 ? 1 : 0) + (it.base_map[1] >= 0 ? 1 : 0));
+            if (!it.strip && it.rows > 128) p->stage_wide[s] |= 1;
+            if (it.N > 64) p->stage_wide[s] |= 2;
+        }
+        if (!(p->stage_wide[s] & 1)) p->stage_wide[s] = 0;            // 0 none, 1 wide (B <= 8 KB), 3 wide with N = 128 items
         all.insert(all.end(), pb.stage[s].begin(), pb.stage[s].end());
     }
     if (all.empty()) return GF8_OK;
@@ -474,9 +481,10 @@ gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
         const int n_base = p->stage_base[s];
         // shared-memory split: update stages keep a short operand ring (their operands are L2-resident) and give
         // the rest to base tiles in flight (the HBM stream); panel stages give everything to the operand ring
-        const int fuse = s == 7 ? 1 : 0, strip = (s == 5 || s == 6) ? 1 : 0, kmode = fuse ? 1 : (strip ? 2 : 0);
+        const int fuse = s == 7 ? 1 : 0, strip = (s == 5 || s == 6) ? 1 : 0, wide = p->stage_wide[s] && !n_base ? 1 : 0;
+        const int kmode = fuse ? 1 : (strip ? 2 : (wide ? (p->stage_wide[s] == 3 ? 4 : 3) : 0));
         // shared-memory split of the tile-mode update stages: 3 operand stages + the rest as base tiles in flight
-        int n_stages = n_base ? (strip ? 4 : 3) : gf8::tc::MAX_STAGES, dbg = 0, only = -1;
+        int n_stages = n_base ? (strip ? 4 : 3) : (wide ? (p->stage_wide[s] == 3 ? 4 : 5) : gf8::tc::MAX_STAGES), dbg = 0, only = -1;
         // (strip stages: 64 KB of resident A tiles + 4 x 16 KB of B atoms = the first four 32 KB units, then 3 base slots)
         // (the fused stage gives one base slot's worth of shared memory to its two code-tile staging buffers)
         const int n_bslots = fuse ? 3 : (n_base ? std::max(1, (gf8::tc::MAX_STAGES - n_stages) / n_base) : 1);

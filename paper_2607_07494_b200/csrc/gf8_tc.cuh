@@ -237,11 +237,12 @@ __device__ __forceinline__ uint32_t epi_block_max(uint32_t loc, int warp, int la
 
 // One accumulator tile -> global memory with the base (if any) read straight from global memory: the small
 // panels (P', Q^T, S, Q'^T) and FP32 gradients.  Thread = one row, 16 columns per tcgen05.ld.
-__device__ __forceinline__ void epilogue(const Item& it, uint32_t tmem_acc, int warp, int lane, uint32_t* s_red) {
-    const int r = (warp & 3) * 32 + lane, half = warp >> 2;
+__device__ __forceinline__ void epilogue(const Item& it, uint32_t tmem_acc, int warp, int lane, uint32_t* s_red, int rblk = 0) {
+    // rblk = 1: the second row block of a 256-row panel item (rows 128.., accumulator 64 columns further on)
+    const int r = rblk * 128 + (warp & 3) * 32 + lane, half = warp >> 2;
     const bool row_ok = r < it.rows;
     const int64_t grow = it.row0 + r;
-    const uint32_t taddr = tmem_acc + ((uint32_t)((warp & 3) * 32) << 16);
+    const uint32_t taddr = tmem_acc + ((uint32_t)((warp & 3) * 32) << 16) + 64u * (uint32_t)rblk;
     const int nch = it.cols >> 4;
     const int cb = half ? ((nch + 1) >> 1) << 4 : 0, ce = half ? nch << 4 : ((nch + 1) >> 1) << 4;
     uint32_t a[16];
@@ -515,7 +516,13 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
     const int fuse = kmode == 1 ? 1 : 0;           // kmode: 0 = tile items, 1 = fused update (TMEM-parked), 2 = strip items
     const bool strip = kmode == 2;
     const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;          // 1024-byte aligned (swizzle atoms)
-    const uint32_t base0 = smem0 + (uint32_t)n_stages * STAGE_BYTES;        // base tiles: [acc][n_base] x 32 KB
+    // kmode 3 = tile items with wide operand stages: [A rows 0-127 | A rows 128-255 | B (N <= 64)] = 40 KB, for panel
+    // items of up to 256 rows (two accumulators of 64 columns in one TMEM slot share every B atom)
+    // (kmode 4: the same with a 16 KB B area, 48 KB stages, when the launch also holds N = 128 items)
+    const bool wide = kmode == 3 || kmode == 4;
+    const uint32_t stage_bytes = kmode == 3 ? 40960u : (kmode == 4 ? 49152u : (uint32_t)STAGE_BYTES);
+    const uint32_t b_off = wide ? 32768u : (uint32_t)A_BYTES;
+    const uint32_t base0 = smem0 + (uint32_t)n_stages * stage_bytes;        // base tiles: [acc][n_base] x 32 KB
     const uint32_t bars = smem0 + DATA_BYTES;
     uint8_t* gen0 = smem_raw + (smem0 - smem_u32(smem_raw));
     uint32_t* s_tmem = reinterpret_cast<uint32_t*>(gen0 + DATA_BYTES + 384);
@@ -680,7 +687,8 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                     continue;
                 }
                 const int a_mn = it.a_mn, b_mn = it.b_mn, nbx = it.N >> 6;
-                const uint32_t tx = is_b ? (uint32_t)it.N * 128u : (uint32_t)A_BYTES;
+                const int nrb = (wide && it.rows > 128) ? 2 : 1;
+                const uint32_t tx = is_b ? (uint32_t)it.N * 128u : (uint32_t)(nrb * A_BYTES);
 #pragma unroll 1
                 for (int seg = 0; seg < NSEG && ok; ++seg) {
                     const int na = it.atoms[seg];
@@ -691,19 +699,22 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                     __syncwarp();
                     for (int t = 0; t < na; ++t) {
                         if (!TWAIT(2, mbar_wait(empty_bar(stage), phase ^ 1u, err))) { ok = false; break; }
-                        const uint32_t sa = smem0 + stage * STAGE_BYTES;
+                        const uint32_t sa = smem0 + stage * stage_bytes;
                         if (elect_one()) {
                             mbar_expect_tx(full_bar(stage), tx);
                             if (is_b && b_mn) {       // N / 64 boxes of 64 K-rows x 64 contiguous N elements
                                 for (int h = 0; h < nbx; ++h)
-                                    tma_load_2d(sa + A_BYTES + 8192u * h, mp, c0 + 64 * h, r0 + 64 * t, full_bar(stage));
+                                    tma_load_2d(sa + b_off + 8192u * h, mp, c0 + 64 * h, r0 + 64 * t, full_bar(stage));
                             } else if (is_b) {        // N rows x 64 columns, one box
-                                tma_load_2d(sa + A_BYTES, mp, c0 + 64 * t, r0, full_bar(stage));
-                            } else if (a_mn) {        // two 64 x 64 boxes: 64 K-rows of 128 contiguous M elements
-                                tma_load_2d(sa, mp, c0, r0 + 64 * t, full_bar(stage));
-                                tma_load_2d(sa + 8192, mp, c0 + 64, r0 + 64 * t, full_bar(stage));
-                            } else {                  // one 128-row x 64-column box
-                                tma_load_2d(sa, mp, c0 + 64 * t, r0, full_bar(stage));
+                                tma_load_2d(sa + b_off, mp, c0 + 64 * t, r0, full_bar(stage));
+                            } else if (a_mn) {        // per row block two 64 x 64 boxes: 64 K-rows of 128 contiguous M elements
+                                for (int rb = 0; rb < nrb; ++rb) {
+                                    tma_load_2d(sa + 16384u * rb, mp, c0 + 128 * rb, r0 + 64 * t, full_bar(stage));
+                                    tma_load_2d(sa + 16384u * rb + 8192, mp, c0 + 128 * rb + 64, r0 + 64 * t, full_bar(stage));
+                                }
+                            } else {                  // per row block one 128-row x 64-column box
+                                for (int rb = 0; rb < nrb; ++rb)
+                                    tma_load_2d(sa + 16384u * rb, mp, c0 + 64 * t, r0 + 128 * rb, full_bar(stage));
                             }
                         }
                         __syncwarp();
@@ -782,16 +793,22 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 if (!(ok = TWAIT(1, mbar_wait(tempty_bar(acc), aphase ^ 1u, err)))) break;
                 tc_fence_after();
                 const uint32_t d = tmem_base + acc * 128u;
+                const bool nrb2 = wide && it.rows > 128;
                 for (int t = 0; t < total; ++t) {
                     if (!(ok = TWAIT(2, mbar_wait(full_bar(stage), phase, err)))) break;
                     tc_fence_after();
-                    const uint32_t sa = smem0 + stage * STAGE_BYTES, sb = sa + A_BYTES;
+                    const uint32_t sa = smem0 + stage * stage_bytes, sb = sa + b_off;
                     if (elect_one()) {
 #pragma unroll
                         for (int kk = 0; kk < 4; ++kk) {
                             const uint64_t da = a_mn ? smem_desc(sa + 2048u * kk, 8192u, 1024u) : smem_desc(sa + 32u * kk, 16u, 1024u);
                             const uint64_t db = b_mn ? smem_desc(sb + 2048u * kk, 8192u, 1024u) : smem_desc(sb + 32u * kk, 16u, 1024u);
                             if (!(dbg & 1)) tc_mma_bf16(d, da, db, idesc, (t | kk) ? 1u : 0u);
+                            if (nrb2 && !(dbg & 1)) {     // second row block: A 16 KB further on, accumulator 64 columns further on
+                                const uint64_t da2 = a_mn ? smem_desc(sa + 16384u + 2048u * kk, 8192u, 1024u)
+                                                          : smem_desc(sa + 16384u + 32u * kk, 16u, 1024u);
+                                tc_mma_bf16(d + 64u, da2, db, idesc, (t | kk) ? 1u : 0u);
+                            }
                         }
                         tc_commit(empty_bar(stage));      // frees the smem stage when these MMAs retire
                     }
@@ -1002,8 +1019,10 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
             if (it.base_map[0] >= 0)
                 stored = epilogue_tile(it, tmem_base + acc * 128u, base_tile(bs), it.base_map[1] >= 0 ? 2 : 1, warp, lane, s_red, maps, cast_scale, cast_si,
                                        it.row0, it.col0, it.write_scale != 0, it.scale_inv_out, nullptr);
-            else
+            else {
                 epilogue(it, tmem_base + acc * 128u, warp, lane, s_red);
+                if (wide && it.rows > 128) epilogue(it, tmem_base + acc * 128u, warp, lane, s_red, 1);
+            }
             tc_fence_before();
             __syncwarp();
             if (prof) pw[3] += clock64() - t_e0;
