@@ -18,6 +18,7 @@ struct Plan {
     int stage_wide[8] = {0, 0, 0, 0, 0, 0, 0, 0};  // the stage holds 256-row panel items: wide operand stages (kmode 3)
     int stage_base[8] = {0, 0, 0, 0, 0, 0, 0, 0};  // streamed base tiles per item in that stage's launch (0, 1 or 2)
     int runs = 0;                        // launches so far: the first one acquires its tensor maps with proxy fences
+    int* d_ctr = nullptr;                // one item counter per stage (dynamic item hand-out), zeroed before every run
     uint32_t* d_amax = nullptr;          // one word per TC problem (per-tensor scaling)
     size_t n_amax = 0;
     struct Convert { const float* src; gf8::bf16 *dst, *dst_lo; int64_t numel; };
@@ -406,6 +407,7 @@ void plan_free(Plan* p) {
     cudaFree(p->d_maps);
     cudaFree(p->d_items);
     cudaFree(p->d_amax);
+    cudaFree(p->d_ctr);
     delete p;
 }
 
@@ -454,6 +456,8 @@ gf8_status plan_finish(gf8_ctx* c, PlanBuilder& pb, Plan* p) {
     p->d_maps = (CUtensorMap*)q;
     if (cudaMalloc(&q, all.size() * sizeof(Item)) != cudaSuccess) { cudaGetLastError(); return fail(c, GF8_ERR_NOMEM, "plan items"); }
     p->d_items = (Item*)q;
+    if (cudaMalloc(&q, 8 * sizeof(int)) != cudaSuccess) { cudaGetLastError(); return fail(c, GF8_ERR_NOMEM, "plan counters"); }
+    p->d_ctr = (int*)q;
     CU_TRY(c, cudaMemcpy(p->d_maps, pb.maps.data(), pb.maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice));
     CU_TRY(c, cudaMemcpy(p->d_items, all.data(), all.size() * sizeof(Item), cudaMemcpyHostToDevice));
     return GF8_OK;
@@ -475,6 +479,7 @@ gf8_status plan_store(gf8_ctx* c, const std::vector<uint64_t>& key, Plan* p) {
 
 gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
     const bool first_run = p->runs++ == 0;
+    if (p->d_ctr) CU_TRY(c, cudaMemsetAsync(p->d_ctr, 0, 8 * sizeof(int), st));
     for (int s = 0; s < 8; ++s) {
         if (!p->stage_cnt[s]) continue;
         const int grid = std::min(p->stage_cnt[s], c->num_sms);
@@ -500,7 +505,8 @@ gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
         cudaEvent_t ev0 = nullptr, ev1 = nullptr;
         if (dbg & 256) { cudaEventCreate(&ev0); cudaEventCreate(&ev1); cudaEventRecord(ev0, st); }
         gf8::tc::tc_items_kernel<<<grid, gf8::tc::THREADS, gf8::tc::SMEM_BYTES, st>>>(
-            p->d_items + p->stage_off[s], p->stage_cnt[s], p->d_maps, c->d_err, n_stages, n_base, n_bslots, kmode, dbg, (dbg & 4) ? c->d_prof : nullptr);
+            p->d_items + p->stage_off[s], p->stage_cnt[s], p->d_maps, c->d_err, n_stages, n_base, n_bslots, kmode, dbg, (dbg & 4) ? c->d_prof : nullptr,
+            (fuse || getenv("GF8_TC_STATIC")) ? nullptr : p->d_ctr + s);
         if (dbg & 256) {                 // GF8_TC_DBG bit 8: per-stage device time (serialises the stream)
             float ms = 0;
             cudaEventRecord(ev1, st); cudaEventSynchronize(ev1); cudaEventElapsedTime(&ms, ev0, ev1);

@@ -52,7 +52,8 @@ enum Epi : int32_t {
     EPI_STORE_T = 1,     // out[c][r] = acc * colscale  (BF16, transposed store; the small S matrix)
     EPI_AMAX = 2,        // atomicMax(amax, max |base + acc|)        (a5, per-tensor scale)
     EPI_CAST = 3,        // codes = fp8((base + acc) * scale(amax))  (a6)
-    EPI_BLOCKCAST = 4    // per-128x128-block amax + scale + cast in one pass (a5 + a6)
+    EPI_BLOCKCAST = 4,   // per-128x128-block amax + scale + cast in one pass (a5 + a6)
+    EPI_END = -1         // written into the item ring by the fetch warp: no more items for this CTA
 };
 enum Ty : int32_t { TY_NONE = 0, TY_BF16 = 1, TY_F32 = 2 };
 
@@ -511,10 +512,14 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
 __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __restrict__ items, int n_items,
                                                               const CUtensorMap* __restrict__ maps, int* err,
                                                               int n_stages, int n_base, int n_bslots, int kmode, int dbg,
-                                                              long long* __restrict__ prof) {
+                                                              long long* __restrict__ prof, int* ctr) {
     extern __shared__ uint8_t smem_raw[];
     const int fuse = kmode == 1 ? 1 : 0;           // kmode: 0 = tile items, 1 = fused update (TMEM-parked), 2 = strip items
     const bool strip = kmode == 2;
+    // ctr != null: items are handed out dynamically (atomic counter, list order = start order), so item durations may
+    // differ without idling CTAs and the planner's ordering decides which items run at the same time (L2 reuse).
+    // The fused update keeps the static round-robin (its cast of parked tiles counts on it).
+    const bool dyn = ctr != nullptr && !fuse;
     const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;          // 1024-byte aligned (swizzle atoms)
     // kmode 3 = tile items with wide operand stages: [A rows 0-127 | A rows 128-255 | B (N <= 64)] = 40 KB, for panel
     // items of up to 256 rows (two accumulators of 64 columns in one TMEM slot share every B atom)
@@ -577,17 +582,30 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
         uint32_t stage = 0, phase = 0, n_done = 0, b_bs = 0, b_bph = 0;
         int ok = 1;
         uint4 nxt = make_uint4(0, 0, 0, 0);
-        if ((int)blockIdx.x < n_items && lane < NCHUNK) nxt = __ldg(reinterpret_cast<const uint4*>(items + blockIdx.x) + lane);
-        for (int i = blockIdx.x; i < n_items && ok; i += gridDim.x, ++n_done) {
+        auto claim = [&](int after) {          // index of this CTA's next item (claimed one item ahead of its use)
+            if (!dyn) return after + (int)gridDim.x;
+            int v = 0;
+            if (lane == 0) v = atomicAdd(ctr, 1);
+            return __shfl_sync(0xFFFFFFFFu, v, 0);
+        };
+        int i = dyn ? claim(0) : (int)blockIdx.x;
+        if (i < n_items && lane < NCHUNK) nxt = __ldg(reinterpret_cast<const uint4*>(items + i) + lane);
+        for (; (dyn || i < n_items) && ok; ++n_done) {
             const uint32_t slot = n_done % ITEM_SLOTS, iphase = (n_done / ITEM_SLOTS) & 1u;
             if (lane == 0) ok = TWAIT(0, mbar_wait(iempty_bar(slot), iphase ^ 1u, err)) ? 1 : 0;
             ok = __shfl_sync(0xFFFFFFFFu, ok, 0);
             if (!ok) break;
+            if (i >= n_items) {                 // (dynamic only) tell the other roles this CTA is done
+                if (lane == 0) reinterpret_cast<Item*>(s_items + slot * ITEM_BYTES)->mode = EPI_END;
+                __syncwarp();
+                if (lane == 0) mbar_arrive(ifull_bar(slot));
+                break;
+            }
             if (lane < NCHUNK) reinterpret_cast<uint4*>(s_items + slot * ITEM_BYTES)[lane] = nxt;
             __syncwarp();
             if (lane == 0) mbar_arrive(ifull_bar(slot));
-            if (i + (int)gridDim.x < n_items && lane < NCHUNK)
-                nxt = __ldg(reinterpret_cast<const uint4*>(items + i + gridDim.x) + lane);
+            i = claim(i);
+            if (i < n_items && lane < NCHUNK) nxt = __ldg(reinterpret_cast<const uint4*>(items + i) + lane);
             if (strip) {
                 // strip item: one base tile per (column tile, row block), in the order the epilogue consumes them
                 const Item& it = *item_slot(slot);
@@ -643,9 +661,10 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
             const bool is_b = warp != OPERAND_WARP;
             uint32_t stage = 0, phase = 0, n_done = 0;
             bool ok = true;
-            for (int i = blockIdx.x; i < n_items && ok; i += gridDim.x, ++n_done) {
+            for (int i = blockIdx.x; (dyn || i < n_items) && ok; i += gridDim.x, ++n_done) {
                 const uint32_t slot = n_done % ITEM_SLOTS, iphase = (n_done / ITEM_SLOTS) & 1u;
                 if (!(ok = TWAIT(3, mbar_wait(ifull_bar(slot), iphase, err)))) break;
+                if (dyn && item_slot(slot)->mode == EPI_END) break;
                 const Item& it = *item_slot(slot);
                 if (strip) {
                     // strip item: warp 9 loads the strip's resident A tiles once ([row block][K-atom]); warp 10 streams
@@ -733,9 +752,10 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
         {
             uint32_t stage = 0, phase = 0, n_done = 0, t_count = 0;
             bool ok = true;
-            for (int i = blockIdx.x; i < n_items && ok; i += gridDim.x, ++n_done) {
+            for (int i = blockIdx.x; (dyn || i < n_items) && ok; i += gridDim.x, ++n_done) {
                 const uint32_t slot = n_done % ITEM_SLOTS, iphase = (n_done / ITEM_SLOTS) & 1u;
                 if (!(ok = TWAIT(0, mbar_wait(ifull_bar(slot), iphase, err)))) break;
+                if (dyn && item_slot(slot)->mode == EPI_END) break;
                 const Item& it = *item_slot(slot);
                 const int a_mn = it.a_mn, b_mn = it.b_mn;
                 const uint32_t idesc = instr_desc(it.N, a_mn, b_mn);
@@ -960,11 +980,12 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
         uint32_t n_done = 0, s_tiles = 0, s_bs = 0, s_bph = 0;
         int pending_slot = -1;
         bool ok = true;
-        for (int i = blockIdx.x; i < n_items && ok; i += gridDim.x, ++n_done) {
+        for (int i = blockIdx.x; (dyn || i < n_items) && ok; i += gridDim.x, ++n_done) {
             const uint32_t slot = n_done % ITEM_SLOTS, iphase = (n_done / ITEM_SLOTS) & 1u;
             const uint32_t acc = n_done % n_acc, aphase = (n_done / n_acc) & 1u;
             const uint32_t bs = n_base > 0 ? n_done % (uint32_t)n_bslots : 0u, bphase = n_base > 0 ? (n_done / (uint32_t)n_bslots) & 1u : 0u;
             ok = TWAIT(0, mbar_wait(ifull_bar(slot), iphase, err));
+            if (ok && dyn && item_slot(slot)->mode == EPI_END) break;
             // the tensor's amax (EPI_CAST) is fetched before the data waits, so its latency hides behind them
             float cast_scale = 1.0f, cast_si = 1.0f;
             if (ok && item_slot(slot)->mode == EPI_CAST)
