@@ -426,9 +426,54 @@ gf8_status plan_finish(gf8_ctx* c, PlanBuilder& pb, Plan* p) {
             if (work[pa] != work[pq]) return work[pa] > work[pq];
             return pa < pq;
         });
+        // Waves (items are handed out in list order, so list order is start order).  Within a problem the row panels
+        // sweep the source along its columns and the column panels along its rows; when one kind is rho times longer
+        // (m != n), the short panels are cut into rho bands along the long panels' sweep and band b is listed one
+        // wave later than band b - 1, for a group of as many problems as the SMs hold at once.  Each band then runs
+        // while the long panels cross it, and the second reader of a source byte finds it in L2.
+        struct Prob { std::vector<int> lng, sht; int rho = 1; };
+        std::vector<Prob> probs;
+        for (size_t q = 0; q < order.size();) {
+            const int pid = pb.prob0[order[q]];
+            std::vector<int> rowp, colp;
+            int64_t ar = 0, ac = 0;
+            for (; q < order.size() && pb.prob0[order[q]] == pid; ++q) {
+                const Item& it = pb.stage[0][order[q]];
+                int64_t a = 0;
+                for (int g = 0; g < gf8::tc::NSEG; ++g) a += it.atoms[g];
+                if (it.a_mn) { colp.push_back(order[q]); ac = a; } else { rowp.push_back(order[q]); ar = a; }
+            }
+            Prob pr;
+            const bool col_long = ac > ar;
+            pr.lng = col_long ? colp : rowp;
+            pr.sht = col_long ? rowp : colp;
+            if (pr.lng.empty()) { pr.lng.swap(pr.sht); }
+            const int64_t al = std::max(ar, ac), as = std::min(ar, ac);
+            pr.rho = (!pr.sht.empty() && as > 0) ? (int)std::max<int64_t>(1, (al + as / 2) / as) : 1;
+            pr.rho = std::min<int>(pr.rho, (int)std::max<size_t>(1, pr.sht.size()));
+            probs.push_back(std::move(pr));
+        }
         std::vector<Item> sorted;
         sorted.reserve(order.size());
-        for (int i : order) sorted.push_back(pb.stage[0][i]);
+        for (size_t g0 = 0; g0 < probs.size();) {
+            const Prob& first = probs[g0];
+            const int per = (int)first.lng.size() + (int)((first.sht.size() + first.rho - 1) / first.rho);
+            const size_t G = (size_t)std::max(1, c->num_sms / std::max(1, per));
+            const size_t g1 = std::min(probs.size(), g0 + G);
+            int waves = 1;
+            for (size_t q = g0; q < g1; ++q) waves = std::max(waves, probs[q].rho);
+            for (int w = 0; w < waves; ++w)
+                for (size_t q = g0; q < g1; ++q) {
+                    const Prob& pr = probs[q];
+                    if (w == 0) for (int i : pr.lng) sorted.push_back(pb.stage[0][i]);
+                    if (w < pr.rho) {
+                        const size_t nb = (pr.sht.size() + pr.rho - 1) / pr.rho;
+                        for (size_t k = (size_t)w * nb; k < std::min(pr.sht.size(), (size_t)(w + 1) * nb); ++k)
+                            sorted.push_back(pb.stage[0][pr.sht[k]]);
+                    }
+                }
+            g0 = g1;
+        }
         pb.stage[0].swap(sorted);
     }
     for (int s = 0; s < 8; ++s) {
