@@ -549,9 +549,25 @@ gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
         if (only >= 0 && only != s) continue;
         cudaEvent_t ev0 = nullptr, ev1 = nullptr;
         if (dbg & 256) { cudaEventCreate(&ev0); cudaEventCreate(&ev1); cudaEventRecord(ev0, st); }
+        static std::vector<std::pair<int, std::pair<cudaEvent_t, cudaEvent_t>>> pend;     // bit 9: the same without serialising
+        if (dbg & 512) {
+            if (s == 0 || pend.size() > 64) {
+                for (auto& e : pend) {
+                    float ms = 0;
+                    cudaEventSynchronize(e.second.second); cudaEventElapsedTime(&ms, e.second.first, e.second.second);
+                    fprintf(stderr, "stage %d (async): %.1f us\n", e.first, ms * 1e3);
+                    cudaEventDestroy(e.second.first); cudaEventDestroy(e.second.second);
+                }
+                pend.clear();
+            }
+            cudaEvent_t a, b;
+            cudaEventCreate(&a); cudaEventCreate(&b); cudaEventRecord(a, st);
+            pend.push_back({s, {a, b}});
+        }
         gf8::tc::tc_items_kernel<<<grid, gf8::tc::THREADS, gf8::tc::SMEM_BYTES, st>>>(
             p->d_items + p->stage_off[s], p->stage_cnt[s], p->d_maps, c->d_err, n_stages, n_base, n_bslots, kmode, dbg, (dbg & 4) ? c->d_prof : nullptr,
             (fuse || getenv("GF8_TC_STATIC")) ? nullptr : p->d_ctr + s);
+        if (dbg & 512) cudaEventRecord(pend.back().second.second, st);
         if (dbg & 256) {                 // GF8_TC_DBG bit 8: per-stage device time (serialises the stream)
             float ms = 0;
             cudaEventRecord(ev1, st); cudaEventSynchronize(ev1); cudaEventElapsedTime(&ms, ev0, ev1);
