@@ -44,7 +44,7 @@ constexpr int FUSE_LAG = 2;                      // fused update: tiles parked i
                                                  // (2 parked + 1 in the epilogue + 1 under the MMAs = 4 slots)
 constexpr int CODE_TILE_BYTES = 128 * 128;       // staging of one 128 x 128 FP8 code tile
 constexpr int STRIP_L_BYTES = 4 * A_BYTES;       // strip mode: resident A tiles, [row block 0/1][K-atom 0/1]
-constexpr int STRIP_RING = 4;                    // strip mode: ring of 16 KB B K-atoms
+constexpr int STRIP_RING = 2;                    // strip mode: ring of column-tile stages, each the (up to two) 16 KB B K-atoms of a column tile
 constexpr int NSEG = 6;                          // operand segments per item (hi/lo split products)
 
 enum Epi : int32_t {
@@ -685,21 +685,23 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                         }
                         __syncwarp();
                     } else {
-                        for (int ct = 0; ct < nct && ok; ++ct)
-                            for (int seg = 0; seg < 2 && ok; ++seg)
-                                for (int t = 0; t < it.atoms[seg]; ++t) {
-                                    if (!TWAIT(2, mbar_wait(empty_bar(stage), phase ^ 1u, err))) { ok = false; break; }
-                                    if (elect_one()) {
-                                        if (dbg & 128) mbar_arrive(full_bar(stage));
-                                        else {
-                                        mbar_expect_tx(full_bar(stage), B_BYTES);
-                                        tma_load_2d(smem0 + STRIP_L_BYTES + stage * B_BYTES, maps + it.map_b[seg],
-                                                    it.b_c0[seg] + 64 * t, it.b_r0[seg] + 128 * ct, full_bar(stage));
-                                        }
-                                    }
-                                    __syncwarp();
-                                    if (++stage == (uint32_t)STRIP_RING) { stage = 0; phase ^= 1u; }
+                        // one ring stage = the (up to two) B K-atoms of a column tile, under one barrier pair
+                        for (int ct = 0; ct < nct && ok; ++ct) {
+                            if (!TWAIT(2, mbar_wait(empty_bar(stage), phase ^ 1u, err))) { ok = false; break; }
+                            if (elect_one()) {
+                                if (dbg & 128) mbar_arrive(full_bar(stage));
+                                else {
+                                    mbar_expect_tx(full_bar(stage), (uint32_t)na * B_BYTES);
+                                    int a = 0;
+                                    for (int seg = 0; seg < 2; ++seg)
+                                        for (int t = 0; t < it.atoms[seg]; ++t, ++a)
+                                            tma_load_2d(smem0 + STRIP_L_BYTES + (stage * 2u + (uint32_t)a) * B_BYTES, maps + it.map_b[seg],
+                                                        it.b_c0[seg] + 64 * t, it.b_r0[seg] + 128 * ct, full_bar(stage));
                                 }
+                            }
+                            __syncwarp();
+                            if (++stage == (uint32_t)STRIP_RING) { stage = 0; phase ^= 1u; }
+                        }
                     }
                     __syncwarp();
                     if (elect_one()) mbar_arrive(iempty_bar(slot));
@@ -780,28 +782,23 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                             tc_fence_after();
                         }
                         const uint32_t d = tmem_base + acc * 128u;
-                        for (int a = 0; a < total; ++a) {
-                            const uint32_t st_a = (stage + (uint32_t)a) % STRIP_RING;
-                            const uint32_t ph_a = phase ^ ((stage + (uint32_t)a) >= (uint32_t)STRIP_RING ? 1u : 0u);
-                            if (!(ok = TWAIT(2, mbar_wait(full_bar(st_a), ph_a, err)))) break;
-                            tc_fence_after();
-                            const uint32_t sa = smem0 + (uint32_t)(rb * 2 + a) * A_BYTES;
-                            const uint32_t sb = smem0 + STRIP_L_BYTES + st_a * B_BYTES;
-                            if (elect_one()) {
-                                if (mine && !(dbg & 1)) {
+                        if (!(ok = TWAIT(2, mbar_wait(full_bar(stage), phase, err)))) break;     // both B atoms of the column tile
+                        tc_fence_after();
+                        if (elect_one()) {
+                            if (mine && !(dbg & 1))
+                                for (int a = 0; a < total; ++a) {
+                                    const uint32_t sa = smem0 + (uint32_t)(rb * 2 + a) * A_BYTES;
+                                    const uint32_t sb = smem0 + STRIP_L_BYTES + (stage * 2u + (uint32_t)a) * B_BYTES;
 #pragma unroll
                                     for (int kk = 0; kk < 4; ++kk)
                                         tc_mma_bf16(d, smem_desc(sa + 32u * kk, 16u, 1024u), smem_desc(sb + 32u * kk, 16u, 1024u),
                                                     idesc, (a | kk) ? 1u : 0u);
                                 }
-                                tc_commit(empty_bar(st_a));      // (two arrivals free the ring stage: one per issuer)
-                            }
-                            __syncwarp();
+                            tc_commit(empty_bar(stage));         // (two arrivals free the ring stage: one per issuer)
+                            if (mine) tc_commit(tfull_bar(acc));
                         }
-                        if (ok && mine && elect_one()) tc_commit(tfull_bar(acc));
                         __syncwarp();
-                        stage += (uint32_t)total;
-                        if (stage >= (uint32_t)STRIP_RING) { stage -= STRIP_RING; phase ^= 1u; }
+                        if (++stage == (uint32_t)STRIP_RING) { stage = 0; phase ^= 1u; }
                     }
                     if (ok && elect_one()) tc_commit(parked_bar(1));       // A tiles free once these MMAs retire
                     __syncwarp();
