@@ -149,6 +149,11 @@ FAST_CASES.update({
     "wide-k96": dict(m=640, n=1168, kG=96, kA=80, side=gf8.SIDE_BOTH, dtype="bf16", seed=6, q=2),
     "in-only-block": dict(m=384, n=528, kG=0, kA=32, side=gf8.SIDE_IN, dtype="bf16", seed=7, scaling=gf8.SCALE_BLOCK128),
     "rank-512": dict(m=640, n=768, kG=512, kA=384, side=gf8.SIDE_BOTH, dtype="bf16", seed=8, q=2),
+    # 256-row panel items whose second row block is ragged (400 = 256 + 144, 464 = 256 + 208)
+    "ragged-wide-panels": dict(m=400, n=464, kG=32, kA=48, side=gf8.SIDE_BOTH, dtype="bf16", seed=9, q=2),
+    # 4:1 and 1:4 problems: the planner lists the short panels in bands behind the long panels' sweep
+    "tall-4to1": dict(m=1024, n=256, kG=32, kA=32, side=gf8.SIDE_BOTH, dtype="bf16", seed=10, q=2),
+    "wide-1to4": dict(m=256, n=1024, kG=32, kA=32, side=gf8.SIDE_BOTH, dtype="bf16", seed=11, q=2),
 })
 _fcache = {}
 
