@@ -579,7 +579,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
     if (warp == PRODUCER_WARP) {
         // ===== item fetch (whole warp) + TMA producer (lane 0) =====
         constexpr int NCHUNK = ITEM_BYTES / 16;
-        uint32_t stage = 0, phase = 0, n_done = 0, b_bs = 0, b_bph = 0;
+        uint32_t n_done = 0, b_bs = 0, b_bph = 0;
         int ok = 1;
         uint4 nxt = make_uint4(0, 0, 0, 0);
         auto claim = [&](int after) {          // index of this CTA's next item (claimed one item ahead of its use)
