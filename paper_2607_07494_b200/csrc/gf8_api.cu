@@ -401,6 +401,8 @@ gf8_status fast_encode_many(gf8_ctx* c, int n, const int* layers, const void* co
         GF_TRY(aux_fork(c, st));
         sp = c->aux_stream;
     }
+    // (with full-size grids they take turns with the stages rather than share SMs; capping them at the one CTA per SM
+    //  that fits beside a tensor-core CTA made the 48 dependent launches of config 2 the longer path: measured slower)
     for (int i : p->plain) {
         if (tap) {
             LayerState& L = c->layers[layers[i]];
@@ -514,8 +516,14 @@ gf8_status fast_reduce_decoded_many(gf8_ctx* c, int n, const int* layers, const 
         GF_TRY(aux_fork(c, st));
         sp = c->aux_stream;
     }
-    for (int i : p->plain)
-        GF_TRY(reduce_decoded_one(c, layers[i], codes + (size_t)i * R, sinv + (size_t)i * R, R, average, outs[i], dt, sp));
+    // one CTA per SM for the Euclidean tensors' reduction: that is what fits beside a tensor-core CTA (registers, 2 KB
+    // of shared memory), so it runs concurrently with the stages instead of taking turns with them
+    if (overlap) c->aux_per_sm = 1;
+    for (int i : p->plain) {
+        const gf8_status rs = reduce_decoded_one(c, layers[i], codes + (size_t)i * R, sinv + (size_t)i * R, R, average, outs[i], dt, sp);
+        if (rs != GF8_OK) { c->aux_per_sm = 0; return rs; }
+    }
+    c->aux_per_sm = 0;
     GF_TRY(plan_run_stages(c, st, p));
     if (overlap) GF_TRY(aux_join(c, st));
     return GF8_OK;

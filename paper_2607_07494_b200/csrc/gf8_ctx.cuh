@@ -103,6 +103,7 @@ struct gf8_ctx {
     bool tc_attr_set = false;
     int64_t launches = 0;
     int num_sms = 148;
+    int aux_per_sm = 0;              // > 0: cap streaming grids at this many CTAs per SM (kernels that share SMs with the TC engine)
     char err[512] = {0};
 };
 
@@ -160,7 +161,7 @@ inline float fmax_of(int fmt) { return fmt == GF8_E4M3 ? 448.0f : 57344.0f; }
 
 inline int grid_for(gf8_ctx* c, int64_t work_items, int threads, int per_sm) {
     int64_t blocks = (work_items + threads - 1) / threads;
-    const int64_t cap = (int64_t)c->num_sms * per_sm;
+    const int64_t cap = (int64_t)c->num_sms * (c->aux_per_sm > 0 ? std::min(per_sm, c->aux_per_sm) : per_sm);
     if (blocks > cap) blocks = cap;
     if (blocks < 1) blocks = 1;
     return (int)blocks;

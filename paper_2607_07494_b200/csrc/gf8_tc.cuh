@@ -34,7 +34,10 @@ constexpr int STAGE_BYTES = A_BYTES + B_BYTES;   // 32 KB
 constexpr int TILE_BYTES = 128 * 128 * 2;        // one streamed 128 x 128 BF16 base tile (two 64-column halves)
 constexpr int DATA_BYTES = MAX_STAGES * STAGE_BYTES;   // 224 KB, split at launch into ring stages + base tiles
 constexpr int MISC_BYTES = 2048;                 // barriers, TMEM address, reductions, parked-tile info, item ring
-constexpr int SMEM_BYTES = DATA_BYTES + 1024 /*alignment slack*/ + MISC_BYTES;
+// 226 KB: the dynamic shared memory is declared 1024-byte aligned (checked at kernel entry), so no alignment slack is
+// needed, and 2 KB of the SM's 228 KB stay free: one block of a streaming kernel (1 KB system slice + <= 1 KB of its own)
+// fits beside a tensor-core CTA, which is what lets the auxiliary stream's kernels overlap the stages.
+constexpr int SMEM_BYTES = DATA_BYTES + MISC_BYTES;
 constexpr int EPI_WARPS = 8, PRODUCER_WARP = 8, OPERAND_WARP = 9, MMA_WARP = 11, SYNC_WARP = 12;
 constexpr int THREADS = 32 * (EPI_WARPS + 5);
 constexpr int ITEM_SLOTS = 4;                    // shared-memory ring of item descriptors
@@ -513,14 +516,18 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                                                               const CUtensorMap* __restrict__ maps, int* err,
                                                               int n_stages, int n_base, int n_bslots, int kmode, int dbg,
                                                               long long* __restrict__ prof, int* ctr) {
-    extern __shared__ uint8_t smem_raw[];
+    extern __shared__ __align__(1024) uint8_t smem_raw[];
     const int fuse = kmode == 1 ? 1 : 0;           // kmode: 0 = tile items, 1 = fused update (TMEM-parked), 2 = strip items
     const bool strip = kmode == 2;
     // ctr != null: items are handed out dynamically (atomic counter, list order = start order), so item durations may
     // differ without idling CTAs and the planner's ordering decides which items run at the same time (L2 reuse).
     // The fused update keeps the static round-robin (its cast of parked tiles counts on it).
     const bool dyn = ctr != nullptr && !fuse;
-    const uint32_t smem0 = (smem_u32(smem_raw) + 1023u) & ~1023u;          // 1024-byte aligned (swizzle atoms)
+    const uint32_t smem0 = smem_u32(smem_raw);                              // 1024-byte aligned (swizzle atoms)
+    if (smem0 & 1023u) {                                                    // (never seen; fail loudly rather than corrupt tiles)
+        if (threadIdx.x == 0) atomicExch(err, 3);
+        return;
+    }
     // kmode 3 = tile items with wide operand stages: [A rows 0-127 | A rows 128-255 | B (N <= 64)] = 40 KB, for panel
     // items of up to 256 rows (two accumulators of 64 columns in one TMEM slot share every B atom)
     // (kmode 4: the same with a 16 KB B area, 48 KB stages, when the launch also holds N = 128 items)
