@@ -296,7 +296,11 @@ inline void key_ptr(std::vector<uint64_t>& k, const void* p) { k.push_back((uint
 
 gf8_status aux_fork(gf8_ctx* c, cudaStream_t st) {
     if (!c->aux_stream) {
-        CU_TRY(c, cudaStreamCreateWithFlags(&c->aux_stream, cudaStreamNonBlocking));
+        // lowest priority: its blocks take the room the tensor-core CTAs leave on an SM (one 256-thread block fits
+        // beside one), instead of holding the SMs the next stage's CTAs are waiting for
+        int lo = 0, hi = 0;
+        CU_TRY(c, cudaDeviceGetStreamPriorityRange(&lo, &hi));
+        CU_TRY(c, cudaStreamCreateWithPriority(&c->aux_stream, cudaStreamNonBlocking, lo));
         CU_TRY(c, cudaEventCreateWithFlags(&c->aux_fork_ev, cudaEventDisableTiming));
         CU_TRY(c, cudaEventCreateWithFlags(&c->aux_join_ev, cudaEventDisableTiming));
     }
