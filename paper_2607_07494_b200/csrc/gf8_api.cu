@@ -346,13 +346,19 @@ gf8_status fast_encode_many(gf8_ctx* c, int n, const int* layers, const void* co
         std::map<int, size_t> occurrence;
         std::vector<int> tc_idx;
         for (int i = 0; i < n; ++i) {
-            if (c->layers[layers[i]].tc_ok) tc_idx.push_back(i); else p->plain.push_back(i);
+            const LayerState& Li = c->layers[layers[i]];
+            if (Li.tc_ok) tc_idx.push_back(i);
+            else if (!tap && dt == GF8_DT_BF16 && Li.desc.side == GF8_SIDE_NONE && Li.desc.scaling == GF8_SCALE_TENSOR &&
+                     ((int64_t)Li.desc.d_out * Li.desc.d_in) % 16 == 0)
+                p->grouped.push_back(i);         // Euclidean tensors: grouped amax + cast launches
+            else p->plain.push_back(i);
         }
         p->n_amax = 2 * tc_idx.size();           // per TC problem: amax word + parked-tile counter
+        p->n_plain_amax = p->grouped.size();
         gf8_status s = GF8_OK;
-        if (p->n_amax) {
+        if (p->n_amax + p->n_plain_amax) {
             void* q = nullptr;
-            if (cudaMalloc(&q, p->n_amax * sizeof(uint32_t)) != cudaSuccess) { cudaGetLastError(); plan_free(p); return fail(c, GF8_ERR_NOMEM, "plan amax"); }
+            if (cudaMalloc(&q, (p->n_amax + p->n_plain_amax) * sizeof(uint32_t)) != cudaSuccess) { cudaGetLastError(); plan_free(p); return fail(c, GF8_ERR_NOMEM, "plan amax"); }
             p->d_amax = (uint32_t*)q;
         }
         for (size_t t = 0; t < tc_idx.size() && s == GF8_OK; ++t) {
@@ -399,7 +405,7 @@ gf8_status fast_encode_many(gf8_ctx* c, int n, const int* layers, const void* co
     }
     // The problems outside the tensor-core engine (Euclidean tensors: HBM-bound streaming kernels) run on the
     // context's auxiliary stream, concurrently with the engine's stages (bound inside the SM), and join at the end.
-    const bool overlap = !p->plain.empty() && p->stage_cnt[0] + p->stage_cnt[1] + p->stage_cnt[5] + p->stage_cnt[3] > 0 && !tap;
+    const bool overlap = !(p->plain.empty() && p->grouped.empty()) && p->stage_cnt[0] + p->stage_cnt[1] + p->stage_cnt[5] + p->stage_cnt[3] > 0 && !tap;
     cudaStream_t sp = st;
     if (overlap) {
         GF_TRY(aux_fork(c, st));
@@ -414,6 +420,34 @@ gf8_status fast_encode_many(gf8_ctx* c, int n, const int* layers, const void* co
             else GF_TRY(transform_simt<float>(c, sp, L, (const float*)grads[i], taps[i], false));
         } else {
             GF_TRY(encode_one(c, layers[i], grads[i], dt, codes[i], sinv[i], sp));
+        }
+    }
+    if (!p->grouped.empty()) {
+        CU_TRY(c, cudaMemsetAsync(p->d_amax + p->n_amax, 0, p->n_plain_amax * sizeof(uint32_t), sp));
+        for (size_t q = 0; q < p->grouped.size();) {
+            const int fmt0 = c->layers[layers[p->grouped[q]]].desc.fmt;
+            QuantBatch b;
+            memset(&b, 0, sizeof(b));
+            int64_t blocks = 0;
+            while (q < p->grouped.size() && b.n_jobs < QUANT_MAX_JOBS) {
+                const int i = p->grouped[q];
+                const LayerState& L = c->layers[layers[i]];
+                if (L.desc.fmt != fmt0) break;
+                if (!grads[i] || !codes[i] || !sinv[i]) return fail(c, GF8_ERR_INVALID_ARG, "null pointer");
+                if (!aligned16(grads[i]) || !aligned16(codes[i])) return fail(c, GF8_ERR_UNSUPPORTED, "pointers must be 16-byte aligned");
+                QuantJob& jb = b.job[b.n_jobs++];
+                jb.x = (const bf16*)grads[i]; jb.codes = codes[i]; jb.scale_inv = sinv[i];
+                jb.amax_bits = p->d_amax + p->n_amax + q;
+                jb.nvec = (int64_t)L.desc.d_out * L.desc.d_in / 8;
+                jb.first_block = blocks;
+                blocks += (jb.nvec + QUANT_VEC_PER_BLOCK - 1) / QUANT_VEC_PER_BLOCK;
+                ++q;
+            }
+            amax_many_kernel<<<(unsigned)blocks, 256, 0, sp>>>(b);
+            LAUNCH_CHECK(c);
+            if (fmt0 == GF8_E4M3) cast_many_kernel<0><<<(unsigned)blocks, 256, 0, sp>>>(b);
+            else cast_many_kernel<1><<<(unsigned)blocks, 256, 0, sp>>>(b);
+            LAUNCH_CHECK(c);
         }
     }
     for (const Plan::Convert& cv : p->converts) {

@@ -21,6 +21,8 @@ struct Plan {
     int* d_ctr = nullptr;                // one item counter per stage (dynamic item hand-out), zeroed before every run
     uint32_t* d_amax = nullptr;          // one word per TC problem (per-tensor scaling)
     size_t n_amax = 0;
+    size_t n_plain_amax = 0;             // amax words of the grouped Euclidean encode, after the n_amax words
+    std::vector<int> grouped;            // plain problems taken by the grouped Euclidean encode (BF16, per-tensor scale)
     struct Convert { const float* src; gf8::bf16 *dst, *dst_lo; int64_t numel; };
     std::vector<Convert> converts;       // FP32 gradient -> BF16 MMA operand copies
     std::vector<int> plain;              // batch indices served by the per-problem (non-TC) path

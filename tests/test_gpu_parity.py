@@ -352,6 +352,46 @@ def test_fast_batched_matches_single_calls():
     assert torch.equal(outs[0], out1)
 
 
+def test_fast_batched_call_with_euclidean_tensors_is_bit_exact_for_them():
+    """A FAST batched call that mixes whitened and Euclidean (side = NONE) tensors: the Euclidean ones go through the
+    grouped amax + cast launches (E4M3 and E5M2 groups, a ragged size) and the grouped / per-tensor reductions, and
+    stay bit-exact against the oracle's plain FP8 codec."""
+    lays = [gf8.Layer(256, 384, gf8.SIDE_BOTH, 16, 16), gf8.Layer(400, 272, gf8.SIDE_NONE),
+            gf8.Layer(176, 656, gf8.SIDE_NONE, 0, 0, gf8.E5M2), gf8.Layer(1008, 96, gf8.SIDE_NONE)]
+    ctx = gf8.create(lays, gf8.PREC_FAST)
+    ctx.set_basis(0, gf8.SIDE_IN, synth.rand_orthonormal(384, 16, "cuda", 61, 1).contiguous(),
+                  torch.arange(1, 17, device="cuda", dtype=torch.float32) ** -2.0, 0.02)
+    ctx.set_basis(0, gf8.SIDE_OUT, synth.rand_orthonormal(256, 16, "cuda", 61, 2).contiguous(),
+                  torch.arange(1, 17, device="cuda", dtype=torch.float32) ** -2.0, 0.02)
+    R = 2
+    ids, grads = [], []
+    for r in range(R):
+        for i, l in enumerate(lays):
+            ids.append(i)
+            grads.append((synth.gradient(l.d_out, l.d_in, "cuda", 62, i) * (1.0 + r)).to(torch.bfloat16).contiguous())
+    codes = [torch.empty((lays[i].d_out, lays[i].d_in), dtype=torch.uint8, device="cuda") for i in ids]
+    sinvs = [torch.empty(1, dtype=torch.float32, device="cuda") for _ in ids]
+    ctx.encode_many(ids, grads, codes, sinvs)
+    ctx.sync_check()
+    for q, i in enumerate(ids):
+        if lays[i].side != gf8.SIDE_NONE:
+            continue
+        oc, os_ = oracle.quantize(grads[q].float().cpu().numpy(), lays[i].fmt, lays[i].scaling)
+        assert np.array_equal(codes[q].cpu().numpy(), oc) and np.array_equal(sinvs[q].cpu().numpy(), os_), (q, i)
+    # decode: payload (layer i, rank r) sits at index r * len(lays) + i
+    outs = [torch.empty((l.d_out, l.d_in), dtype=torch.bfloat16, device="cuda") for l in lays]
+    pc = [codes[r * len(lays) + i] for i in range(len(lays)) for r in range(R)]
+    ps = [sinvs[r * len(lays) + i] for i in range(len(lays)) for r in range(R)]
+    ctx.reduce_decoded_many(list(range(len(lays))), pc, ps, R, outs, average=True)
+    ctx.sync_check()
+    for i, l in enumerate(lays):
+        if l.side != gf8.SIDE_NONE:
+            continue
+        want = oracle.reduce([pc[i * R + r].cpu().numpy() for r in range(R)], [ps[i * R + r].cpu().numpy() for r in range(R)],
+                             l.fmt, l.scaling)
+        assert np.array_equal(bf16_bits(outs[i]), oracle.to_bf16_bits(want.astype(np.float64))), i
+
+
 def test_fast_fused_update_matches_two_pass(monkeypatch):
     """The opt-in fused update (W~ tiles parked in TMEM across the tensor-wide amax, GF8_TC_FUSE=1) produces the
     same codes and scales as the default amax pass + cast pass."""
