@@ -291,6 +291,7 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
                 int seg = 0;
                 it.N = std::min(128, kpA - nc);
                 add_product(it, seg, mSrc, mUAt, (n + 63) / 64, 0, i0, 0, nc);
+                it.tri = (seg == 3 && it.N <= 64) ? 1 : 0;      // split products of one operand pair: interleaved per K-atom
                 it.mode = EPI_STORE; it.out = s->Pp; it.out_lo = split ? s->Pp_lo : nullptr; it.out_ld = kpA;
                 it.out_type = TY_BF16; it.colscale = eA + nc;
                 it.row0 = i0; it.col0 = nc; it.rows = std::min(stepA, m - i0); it.cols = it.N;
@@ -303,6 +304,7 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
                 int seg = 0;
                 it.a_mn = 1; it.N = std::min(128, kpG - nc);
                 add_product(it, seg, mSrc, mUGt, (m + 63) / 64, j0, 0, 0, nc);
+                it.tri = (seg == 3 && it.N <= 64) ? 1 : 0;
                 it.mode = EPI_STORE; it.row0 = j0; it.col0 = nc; it.rows = std::min(stepG, n - j0); it.cols = it.N;
                 if (useA) { it.out = s->Qt; it.out_ld = kpG; it.out_type = TY_F32; }
                 else {
@@ -495,6 +497,10 @@ gf8_status plan_finish(gf8_ctx* c, PlanBuilder& pb, Plan* p) {
             if (it.N > 64) p->stage_wide[s] |= 2;
         }
         if (!(p->stage_wide[s] & 1)) p->stage_wide[s] = 0;            // 0 none, 1 wide (B <= 8 KB), 3 wide with N = 128 items
+        bool all_tri = !pb.stage[s].empty() && !getenv("GF8_TC_NOTRI");
+        for (const Item& it : pb.stage[s]) all_tri = all_tri && it.tri != 0;
+        if (all_tri) p->stage_wide[s] = 5;                            // 5: every item interleaves its split products (kmode 5)
+        else for (Item& it : pb.stage[s]) it.tri = 0;
         all.insert(all.end(), pb.stage[s].begin(), pb.stage[s].end());
     }
     if (all.empty()) return GF8_OK;
@@ -534,9 +540,9 @@ gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
         // shared-memory split: update stages keep a short operand ring (their operands are L2-resident) and give
         // the rest to base tiles in flight (the HBM stream); panel stages give everything to the operand ring
         const int fuse = s == 7 ? 1 : 0, strip = (s == 5 || s == 6) ? 1 : 0, wide = p->stage_wide[s] && !n_base ? 1 : 0;
-        const int kmode = fuse ? 1 : (strip ? 2 : (wide ? (p->stage_wide[s] == 3 ? 4 : 3) : 0));
+        const int kmode = fuse ? 1 : (strip ? 2 : (wide ? (p->stage_wide[s] == 5 ? 5 : (p->stage_wide[s] == 3 ? 4 : 3)) : 0));
         // shared-memory split of the tile-mode update stages: 3 operand stages + the rest as base tiles in flight
-        int n_stages = n_base ? (strip ? 4 : 3) : (wide ? (p->stage_wide[s] == 3 ? 4 : 5) : gf8::tc::MAX_STAGES), dbg = 0, only = -1;
+        int n_stages = n_base ? (strip ? 4 : 3) : (wide ? (p->stage_wide[s] == 5 ? 2 : (p->stage_wide[s] == 3 ? 4 : 5)) : gf8::tc::MAX_STAGES), dbg = 0, only = -1;
         // (strip stages: 64 KB of resident A tiles + 4 x 16 KB of B atoms = the first four 32 KB units, then 3 base slots)
         // (the fused stage gives one base slot's worth of shared memory to its two code-tile staging buffers)
         const int n_bslots = fuse ? 3 : (n_base ? std::max(1, (gf8::tc::MAX_STAGES - n_stages) / n_base) : 1);

@@ -74,6 +74,8 @@ struct __align__(16) Item {
     int32_t base_map[2];          // >= 0: the base tile (hi [+ lo]) is streamed by TMA into shared memory
     int32_t b_mn;                 // 1: B is MN-major too (the factor GEMM X^T X reads both operands from X)
     int32_t strip;                // 1: strip item of the update (up to 256 rows x all columns; see tc_items_kernel)
+    int32_t tri;                  // 1: segments 0..2 are the split products hi*hi, lo*hi, hi*lo of one operand pair: in a kmode 5
+    int32_t pad_;                 //    launch every K-atom brings A_hi, A_lo, B_hi, B_lo in once and feeds all three
     int64_t base_ld, out_ld;
     const void* base;
     void* out;
@@ -531,9 +533,11 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
     // kmode 3 = tile items with wide operand stages: [A rows 0-127 | A rows 128-255 | B (N <= 64)] = 40 KB, for panel
     // items of up to 256 rows (two accumulators of 64 columns in one TMEM slot share every B atom)
     // (kmode 4: the same with a 16 KB B area, 48 KB stages, when the launch also holds N = 128 items)
-    const bool wide = kmode == 3 || kmode == 4;
-    const uint32_t stage_bytes = kmode == 3 ? 40960u : (kmode == 4 ? 49152u : (uint32_t)STAGE_BYTES);
-    const uint32_t b_off = wide ? 32768u : (uint32_t)A_BYTES;
+    // (kmode 5: wide stages for interleaved split products: [A_hi 32 KB | A_lo 32 KB | B_hi 8 KB | B_lo 8 KB] = 80 KB)
+    const bool tri = kmode == 5;
+    const bool wide = kmode == 3 || kmode == 4 || tri;
+    const uint32_t stage_bytes = kmode == 3 ? 40960u : (kmode == 4 ? 49152u : (tri ? 81920u : (uint32_t)STAGE_BYTES));
+    const uint32_t b_off = tri ? 65536u : (wide ? 32768u : (uint32_t)A_BYTES);
     const uint32_t base0 = smem0 + (uint32_t)n_stages * stage_bytes;        // base tiles: [acc][n_base] x 32 KB
     const uint32_t bars = smem0 + DATA_BYTES;
     uint8_t* gen0 = smem_raw + (smem0 - smem_u32(smem_raw));
@@ -717,6 +721,41 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 const int a_mn = it.a_mn, b_mn = it.b_mn, nbx = it.N >> 6;
                 const int nrb = (wide && it.rows > 128) ? 2 : 1;
                 const uint32_t tx = is_b ? (uint32_t)it.N * 128u : (uint32_t)(nrb * A_BYTES);
+                if (tri) {
+                    // interleaved split products: per K-atom the hi and the lo tile of this warp's operand, once each
+                    const CUtensorMap* m_hi = maps + (is_b ? it.map_b[0] : it.map_a[0]);
+                    const CUtensorMap* m_lo = maps + (is_b ? it.map_b[2] : it.map_a[1]);
+                    const int c0 = is_b ? it.b_c0[0] : it.a_c0[0], r0 = is_b ? it.b_r0[0] : it.a_r0[0];
+                    if (!(dbg & 2) && elect_one()) { tmap_acquire(m_hi); tmap_acquire(m_lo); }
+                    __syncwarp();
+                    for (int t = 0; t < it.atoms[0]; ++t) {
+                        if (!TWAIT(2, mbar_wait(empty_bar(stage), phase ^ 1u, err))) { ok = false; break; }
+                        const uint32_t sa = smem0 + stage * stage_bytes;
+                        if (elect_one()) {
+                            mbar_expect_tx(full_bar(stage), 2u * tx);
+                            for (int v = 0; v < 2; ++v) {
+                                const CUtensorMap* mp = v ? m_lo : m_hi;
+                                if (is_b) {               // N rows x 64 columns, one box (B is K-major in panel items)
+                                    tma_load_2d(sa + b_off + (uint32_t)v * 8192u, mp, c0 + 64 * t, r0, full_bar(stage));
+                                } else if (a_mn) {
+                                    for (int rb = 0; rb < nrb; ++rb) {
+                                        const uint32_t d = sa + 32768u * v + 16384u * rb;
+                                        tma_load_2d(d, mp, c0 + 128 * rb, r0 + 64 * t, full_bar(stage));
+                                        tma_load_2d(d + 8192, mp, c0 + 128 * rb + 64, r0 + 64 * t, full_bar(stage));
+                                    }
+                                } else {
+                                    for (int rb = 0; rb < nrb; ++rb)
+                                        tma_load_2d(sa + 32768u * v + 16384u * rb, mp, c0 + 64 * t, r0 + 128 * rb, full_bar(stage));
+                                }
+                            }
+                        }
+                        __syncwarp();
+                        if (++stage == (uint32_t)n_stages) { stage = 0; phase ^= 1u; }
+                    }
+                    __syncwarp();
+                    if (elect_one()) mbar_arrive(iempty_bar(slot));
+                    continue;
+                }
 #pragma unroll 1
                 for (int seg = 0; seg < NSEG && ok; ++seg) {
                     const int na = it.atoms[seg];
@@ -818,6 +857,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 tc_fence_after();
                 const uint32_t d = tmem_base + acc * 128u;
                 const bool nrb2 = wide && it.rows > 128;
+                if (tri) total = it.atoms[0];              // one ring stage per K-atom carries all three products
                 for (int t = 0; t < total; ++t) {
                     if (!(ok = TWAIT(2, mbar_wait(full_bar(stage), phase, err)))) break;
                     tc_fence_after();
@@ -832,6 +872,16 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                                 const uint64_t da2 = a_mn ? smem_desc(sa + 16384u + 2048u * kk, 8192u, 1024u)
                                                           : smem_desc(sa + 16384u + 32u * kk, 16u, 1024u);
                                 tc_mma_bf16(d + 64u, da2, db, idesc, (t | kk) ? 1u : 0u);
+                            }
+                            if (tri && !(dbg & 1)) {      // + A_lo * B_hi + A_hi * B_lo (A_lo 32 KB, B_lo 8 KB further on)
+                                const uint64_t db_lo = smem_desc(sb + 8192u + 32u * kk, 16u, 1024u);
+                                for (int rb = 0; rb < (nrb2 ? 2 : 1); ++rb) {
+                                    const uint32_t a_hi = sa + 16384u * rb, a_lo = a_hi + 32768u;
+                                    const uint64_t dl = a_mn ? smem_desc(a_lo + 2048u * kk, 8192u, 1024u) : smem_desc(a_lo + 32u * kk, 16u, 1024u);
+                                    const uint64_t dh = a_mn ? smem_desc(a_hi + 2048u * kk, 8192u, 1024u) : smem_desc(a_hi + 32u * kk, 16u, 1024u);
+                                    tc_mma_bf16(d + 64u * rb, dl, db, idesc, 1u);
+                                    tc_mma_bf16(d + 64u * rb, dh, db_lo, idesc, 1u);
+                                }
                             }
                         }
                         tc_commit(empty_bar(stage));      // frees the smem stage when these MMAs retire
