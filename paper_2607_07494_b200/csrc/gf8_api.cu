@@ -15,6 +15,7 @@ using namespace gf8;
 
 #include "gf8_ctx.cuh"
 #include "gf8_fast.cuh"
+#include "gf8_stream_host.cuh"
 
 namespace {
 
@@ -460,6 +461,47 @@ gf8_status fast_encode_many(gf8_ctx* c, int n, const int* layers, const void* co
     return GF8_OK;
 }
 
+// Batched encode / transform tap on the FAST path: the problems the streaming engine takes (BF16 gradients, k <= 64 per
+// side, d_in a multiple of 64) run in its single persistent launch; the rest (Euclidean tensors, other shapes) go through
+// the item engine / streaming kernels on the auxiliary stream, concurrently.
+gf8_status encode_dispatch(gf8_ctx* c, int n, const int* layers, const void* const* grads, gf8_dtype dt, uint8_t* const* codes,
+                           float* const* sinv, float* const* taps, cudaStream_t st) {
+    const bool tap = taps != nullptr;
+    std::vector<int> sidx, rest;
+    for (int i = 0; i < n; ++i) {
+        GF_TRY(check_layer(c, layers[i]));
+        LayerState& L = c->layers[layers[i]];
+        if (!grads[i] || (!tap && (!codes[i] || !sinv[i])) || (tap && !taps[i])) return fail(c, GF8_ERR_INVALID_ARG, "null pointer");
+        if (!aligned16(grads[i]) || (!tap && !aligned16(codes[i])) || (tap && !aligned16(taps[i])))
+            return fail(c, GF8_ERR_UNSUPPORTED, "pointers must be 16-byte aligned");
+        GF_TRY(check_basis(c, L, layers[i]));
+        if (stream_eligible(c, L, dt, tap)) sidx.push_back(i); else rest.push_back(i);
+    }
+    if (sidx.empty()) return fast_encode_many(c, n, layers, grads, dt, codes, sinv, taps, st);
+    gf8_status rs = GF8_OK;
+    if (!rest.empty()) {
+        const size_t nr = rest.size();
+        std::vector<int> l2(nr);
+        std::vector<const void*> g2(nr);
+        std::vector<uint8_t*> c2(nr);
+        std::vector<float*> s2(nr), t2(nr);
+        for (size_t q = 0; q < nr; ++q) {
+            const int i = rest[q];
+            l2[q] = layers[i]; g2[q] = grads[i];
+            c2[q] = tap ? nullptr : codes[i]; s2[q] = tap ? nullptr : sinv[i]; t2[q] = tap ? taps[i] : nullptr;
+        }
+        GF_TRY(aux_fork(c, st));
+        rs = fast_encode_many(c, (int)nr, l2.data(), g2.data(), dt, tap ? nullptr : c2.data(), tap ? nullptr : s2.data(),
+                              tap ? t2.data() : nullptr, c->aux_stream);
+    }
+    if (rs == GF8_OK) rs = stream_run(c, sidx, layers, grads, codes, sinv, taps, st);
+    if (!rest.empty()) {
+        const gf8_status js = aux_join(c, st);
+        if (rs == GF8_OK) rs = js;
+    }
+    return rs;
+}
+
 gf8_status fast_reduce_decoded_many(gf8_ctx* c, int n, const int* layers, const uint8_t* const* codes,
                                     const float* const* sinv, int R, int average, void* const* outs, gf8_dtype dt,
                                     cudaStream_t st) {
@@ -749,6 +791,7 @@ gf8_status gf8_destroy(gf8_ctx* ctx) {
     if (ctx->rs_fork) cudaEventDestroy(ctx->rs_fork);
     if (ctx->aux_stream) { cudaStreamDestroy(ctx->aux_stream); cudaEventDestroy(ctx->aux_fork_ev); cudaEventDestroy(ctx->aux_join_ev); }
     for (Plan* p : ctx->plan_order) plan_free(p);
+    for (SPlan* p : ctx->splans) splan_free(p);
     for (auto& kv : ctx->fac_plans) plan_free(kv.second);
     for (LayerState& L : ctx->layers)
         for (Slot* sl : L.slots) delete sl;
@@ -816,7 +859,7 @@ gf8_status gf8_encode(gf8_ctx* ctx, int layer, const void* grad, gf8_dtype dt, u
     CU_TRY(ctx, cudaSetDevice(ctx->device));
     if (ctx->precision == GF8_PREC_FAST || ctx->tc_exact) {
         if (dt != GF8_DT_BF16 && dt != GF8_DT_F32) return fail(ctx, GF8_ERR_INVALID_ARG, "bad dtype");
-        return fast_encode_many(ctx, 1, &layer, &grad, dt, &codes, &scale_inv, nullptr, (cudaStream_t)stream);
+        return encode_dispatch(ctx, 1, &layer, &grad, dt, &codes, &scale_inv, nullptr, (cudaStream_t)stream);
     }
     return encode_one(ctx, layer, grad, dt, codes, scale_inv, (cudaStream_t)stream);
 }
@@ -855,7 +898,7 @@ gf8_status gf8_encode_many(gf8_ctx* ctx, int n, const int* layers, const void* c
     CU_TRY(ctx, cudaSetDevice(ctx->device));
     if (dt != GF8_DT_BF16 && dt != GF8_DT_F32) return fail(ctx, GF8_ERR_INVALID_ARG, "bad dtype");
     if (ctx->precision == GF8_PREC_FAST || ctx->tc_exact)
-        return fast_encode_many(ctx, n, layers, grads, dt, codes, scale_inv, nullptr, (cudaStream_t)stream);
+        return encode_dispatch(ctx, n, layers, grads, dt, codes, scale_inv, nullptr, (cudaStream_t)stream);
     for (int i = 0; i < n; ++i) GF_TRY(encode_one(ctx, layers[i], grads[i], dt, codes[i], scale_inv[i], (cudaStream_t)stream));
     return GF8_OK;
 }
@@ -1059,7 +1102,7 @@ gf8_status gf8_whiten_f32(gf8_ctx* ctx, int layer, const void* grad, gf8_dtype d
     cudaStream_t st = (cudaStream_t)stream;
     if ((const void*)grad == (const void*)out) return fail(ctx, GF8_ERR_INVALID_ARG, "in-place whiten tap not allowed");
     if (L.tc_ok)
-        return fast_encode_many(ctx, 1, &layer, &grad, dt, nullptr, nullptr, &out, st);
+        return encode_dispatch(ctx, 1, &layer, &grad, dt, nullptr, nullptr, &out, st);
     if (dt == GF8_DT_BF16) return transform_simt<bf16>(ctx, st, L, (const bf16*)grad, out, false);
     return transform_simt<float>(ctx, st, L, (const float*)grad, out, false);
 }
