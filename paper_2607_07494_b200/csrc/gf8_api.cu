@@ -694,11 +694,11 @@ gf8_status gf8_sync_check(gf8_ctx* ctx, void* stream) {
     CU_TRY(ctx, cudaSetDevice(ctx->device));
     CU_TRY(ctx, cudaStreamSynchronize((cudaStream_t)stream));
     if (ctx->d_err) {
-        int e = 0;
-        CU_TRY(ctx, cudaMemcpy(&e, ctx->d_err, sizeof(int), cudaMemcpyDeviceToHost));
-        if (e) {
-            cudaMemset(ctx->d_err, 0, sizeof(int));
-            return fail(ctx, GF8_ERR_CUDA, "tensor-core pipeline time-out (error flag %d)", e);
+        int e[2] = {0, 0};
+        CU_TRY(ctx, cudaMemcpy(e, ctx->d_err, 2 * sizeof(int), cudaMemcpyDeviceToHost));
+        if (e[0]) {
+            cudaMemset(ctx->d_err, 0, 2 * sizeof(int));
+            return fail(ctx, GF8_ERR_CUDA, "tensor-core pipeline time-out (error flag %d, first timed-out wait at gf8_stream.cuh:%d)", e[0], e[1]);
         }
     }
     return GF8_OK;

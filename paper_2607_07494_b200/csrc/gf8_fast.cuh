@@ -51,9 +51,9 @@ gf8_status fast_init(gf8_ctx* c) {
     CU_TRY(c, cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q));
     if (!fn || q != cudaDriverEntryPointSuccess) return fail(c, GF8_ERR_CUDA, "cuTensorMapEncodeTiled not available");
     c->encode_tiled = fn;
-    GF_TRY(dmalloc(c, &c->d_err, 1));
-    GF_TRY(dmalloc(c, &c->d_prof, (size_t)c->num_sms * 36 + 64));
-    CU_TRY(c, cudaMemset(c->d_err, 0, sizeof(int)));
+    GF_TRY(dmalloc(c, &c->d_err, 4));
+    GF_TRY(dmalloc(c, &c->d_prof, (size_t)32768));
+    CU_TRY(c, cudaMemset(c->d_err, 0, 4 * sizeof(int)));
     CU_TRY(c, cudaFuncSetAttribute(gf8::tc::tc_items_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                    gf8::tc::SMEM_BYTES));
     return GF8_OK;

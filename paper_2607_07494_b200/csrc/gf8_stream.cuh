@@ -5,8 +5,8 @@
 //
 // Low-rank form:   P'  = (Wg U_A) E_A            row panels of 256 rows        (K_PANEL_P)
 //                                Q^T = Wg^T U_G                column panels of 256 columns  (K_PANEL_Q)
-//                                (S E_A)^T = P'^T U_G          one item per tensor           (K_S)
-//                                Q'^T = (Q^T + U_A (S E_A)^T) E_G                            (K_QP)
+//                                (S E_A)^T = sum_i P.(i)^T U_G(i)   partial per row panel, summed in panel order (K_SP)
+//                                Q.^T = (Q^T + U_A (S E_A)^T) E_G   last K-step of the column panel item
 //                                W~  = Wg + [P' | U_G] [U_A | Q'^T]^T   128 x 128 tiles      (K_UPD)
 // Work hand-out: the "pass-1" items (P, Q, S, Q') sit in one list in tensor-group order and are claimed
 // dynamically (atomic counter); the update tiles are assigned statically (tile u -> CTA u mod grid) so that the
@@ -18,7 +18,10 @@
 // CTA (grid <= #SMs, 1 CTA / SM); a CTA never holds more than three parked tiles of incomplete tensors, and
 // host code only sends tensors with <= 3 * grid tiles here.
 //
-// Roles (12 warps): 0-7 epilogue, 8 scheduler (+ base-tile TMA), 9 operand TMA, 10 MMA issue, 11 grid-level sync.
+// Two pipelines share every SM, so a long panel item never delays the CTA's update tiles (whose tensors complete in
+// lock step across CTAs) and the HBM-bound streaming of new gradients overlaps the issue-bound update epilogues:
+//   update pipeline: warp 0 scheduler (+ base-tile TMA), 1 operand TMA, 2 MMA issue, 3 grid-level sync, 10-25 epilogue (cast the slot's previous tile, then park)
+//   pass-1 pipeline: warp 4 item claim + operand TMA, 5 MMA issue, 6-9 epilogue
 #pragma once
 #include "gf8_tc.cuh"
 
@@ -27,19 +30,24 @@ namespace st {
 
 using namespace gf8::tc;     // PTX wrappers (mbarrier, TMA, tcgen05)
 
-constexpr int NS = 3;                       // operand ring stages
-constexpr int STG_BYTES = 40960;            // [A 32 KB | B 8 KB]  or  [A 16 KB | B 16 KB] (update)
-constexpr int NB = 3;                       // streamed base tiles in flight
+constexpr int NS = 2;                       // pass-1 operand ring stages
+constexpr int STG_BYTES = 40960;            // [A 32 KB | B 8 KB]
+constexpr int US = 2;                       // update operand ring stages
+constexpr int USTG_BYTES = 32768;           // [A 16 KB | B 16 KB]: one K-atom of an update tile
+constexpr int NB = 2;                       // streamed base tiles in flight
 constexpr int BASE_BYTES = 32768;           // 128 x 128 BF16 (two 64-column halves)
-constexpr int RS = 8;                       // item ring entries
+constexpr int RS = 8;                       // update item ring entries
+constexpr int PRS = 4;                      // pass-1 item ring entries
 constexpr int NPARK = 3;                    // TMEM slots 0..2: update tiles (parked); slot 3: pass-1 items
-constexpr int S_DATA = NS * STG_BYTES + NB * BASE_BYTES;     // 218 KB... see static_assert below
-constexpr int S_MISC = 2048;
+constexpr int S_DATA = NS * STG_BYTES + US * USTG_BYTES + NB * BASE_BYTES;     // 208 KB
+constexpr int S_MISC = 3072;
 constexpr int S_BYTES = S_DATA + S_MISC;
-constexpr int S_THREADS = 384;
+constexpr int S_THREADS = 832;
+// warp roles: the spinning / issuing roles take the low warp ids, the arithmetic-heavy epilogues the high ones
+constexpr int W_USCHED = 0, W_ULOAD = 1, W_UMMA = 2, W_SYNC = 3, W_PPROD = 4, W_PMMA = 5, W_PEPI = 6, W_UEPI = 10;
 static_assert(S_BYTES <= 227 * 1024, "shared memory budget");
 
-enum Kind : int32_t { K_END = 0, K_PANEL_P = 1, K_PANEL_Q = 2, K_S = 3, K_QP = 4, K_UPD = 5 };
+enum Kind : int32_t { K_END = 0, K_PANEL_P = 1, K_PANEL_Q = 2, K_SP = 3, K_UPD = 5 };
 enum Mode : int32_t { M_PARK = 0, M_BLOCK = 1, M_TAP = 2 };
 // words of a tensor's sync block (zeroed before every launch)
 enum Sync : int32_t { SY_AMAX = 0, SY_P = 1, SY_Q = 2, SY_S = 3, SY_QP = 4, SY_TILES = 5, SY_WORDS = 8 };
@@ -54,15 +62,21 @@ struct __align__(16) STensor {
     int32_t map_src_b, map_UAt, map_UGt, map_UA128;
     int32_t map_UA256, map_UG128, map_Pp128, map_Pp64;
     int32_t map_Qpt128, map_SEA, pad0, pad1;
-    bf16* Pp; float* Qt; bf16* Qpt; bf16* SEA;
+    bf16* Pp; float* Spart; bf16* Qpt; bf16* SEA;
     const float* eA; const float* eG;
     uint8_t* codes; float* scale_inv; float* tap;
     uint32_t* sync;
     int64_t byte_pos;                      // gradient bytes of the tensors before this one (lead control)
-    int64_t pad2;
+    int64_t pad2[7];
 };
+static_assert(sizeof(STensor) == 256, "tensor record size");
 
-struct P1Item { int32_t kind, tensor, r0, rows; };
+// Pass-1 item.  gate_tensor >= 0: a panel may start only when that (earlier) tensor's update is complete (gate_total tiles
+// parked), which keeps the gradient bytes between the two pipelines' frontiers within L2 (lead control).
+struct __align__(16) P1Item { int32_t kind, tensor, r0, rows, gate_tensor, gate_total, pad0, pad1; };
+// Update tile u (CTA u mod grid runs it): its tensor, tile coordinates (ti | tj << 16), the count its tensor's SY_QP word must
+// reach (low 16 bits) and the tile count of the tensor whose parked tile held this TMEM slot before (high 16 bits; tile u - 3 grid)
+struct __align__(16) TileEnt { int32_t tensor, tij, dep_old, old_tensor; };
 
 // What a role needs to know about an item (shared-memory ring entry, written by the scheduler warp).
 struct __align__(16) RItem {
@@ -83,6 +97,12 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map
         "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
         ::"r"(dst), "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2) : "memory");
 }
+__device__ __forceinline__ void tma_prefetch_2d(const CUtensorMap* map, int c0, int c1) {
+    asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global [%0, {%1, %2}];" ::"l"(map), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_3d(const CUtensorMap* map, int c0, int c1, int c2) {
+    asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global [%0, {%1, %2, %3}];" ::"l"(map), "r"(c0), "r"(c1), "r"(c2) : "memory");
+}
 __device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {
     uint32_t done;
     asm volatile(
@@ -90,9 +110,26 @@ __device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {
         : "=r"(done) : "r"(bar), "r"(parity) : "memory");
     return done != 0;
 }
+__device__ __forceinline__ bool mbar_try(uint32_t bar, uint32_t parity) {     // one try_wait: sleeps up to ~1 us unless the phase completes
+    uint32_t done;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done) : "r"(bar), "r"(parity), "r"(1000u) : "memory");
+    return done != 0;
+}
+__device__ __forceinline__ void mbar_nap(uint32_t bar, uint32_t parity) {     // sleep until the phase completes, ~0.3 us at most
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t}"
+        ::"r"(bar), "r"(parity), "r"(300u) : "memory");
+}
 __device__ __forceinline__ uint32_t ld_acquire(const uint32_t* p) {
     uint32_t v;
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ uint32_t ld_relaxed(const uint32_t* p) {
+    uint32_t v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
 __device__ __forceinline__ void red_release_add(uint32_t* p, uint32_t v) {
@@ -108,6 +145,20 @@ __device__ __forceinline__ float max3abs(float m, float a, float b) {
     float r;
     asm("max.NaN.f32 %0, %1, %2, %3;" : "=f"(r) : "f"(fabsf(a)), "f"(fabsf(b)), "f"(m));
     return r;
+}
+__device__ __forceinline__ void tmem_ld16_nowait(uint32_t taddr, uint32_t* v) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+        : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* v) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+        ::"r"(taddr), "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]),
+          "r"(v[8]), "r"(v[9]), "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15])
+        : "memory");
 }
 __device__ __forceinline__ void fence_async_global() { asm volatile("fence.proxy.async.global;" ::: "memory"); }
 // four FP8 codes of (v0..v3) * s : packed multiplies + packed converts
@@ -147,45 +198,70 @@ __global__ void patch_kernel(STensor* T, int nT, const void* const* ptrs, const 
 }
 
 // ---- the kernel ------------------------------------------------------------------------------------------------------
+// GF8_STREAM_PROF (debug builds only): per-role cycle accounting, 8 counters per role per CTA, written to `prof`.
+#ifdef GF8_STREAM_PROF
+#define PROF_DECL long long pf[8] = {0, 0, 0, 0, 0, 0, 0, 0}; const long long pf_t0 = clock64();
+#define PROF(slot, ...) { const long long _t = clock64(); __VA_ARGS__; pf[slot] += clock64() - _t; }
+#define PROF_OUT(role) { pf[7] = clock64() - pf_t0; if (prof) for (int _q = 0; _q < 8; ++_q) prof[((size_t)blockIdx.x * 8 + (role)) * 8 + _q] = pf[_q]; }
+#else
+#define PROF_DECL
+#define PROF(slot, ...) { __VA_ARGS__; }
+#define PROF_OUT(role) {}
+#endif
 __global__ void __launch_bounds__(S_THREADS, 1)
 stream_kernel(const STensor* __restrict__ T, int nT, const P1Item* __restrict__ p1, int n_p1, int n_upd,
-              const CUtensorMap* __restrict__ maps, int* ctr, int* err, long long lead_bytes, int tap) {
+              const TileEnt* __restrict__ tiles, const uint32_t* sync_base, const CUtensorMap* __restrict__ maps, int* ctr, int* err,
+              int tap, long long* prof) {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
     const uint32_t smem0 = smem_u32(smem_raw);
     if (smem0 & 1023u) { if (threadIdx.x == 0) atomicExch(err, 3); return; }
-    const uint32_t base0 = smem0 + NS * STG_BYTES;
+    const uint32_t ustg0 = smem0 + NS * STG_BYTES;               // update operand stages
+    const uint32_t base0 = ustg0 + US * USTG_BYTES;              // update base tiles
     const uint32_t bars = smem0 + S_DATA;
     uint8_t* misc = smem_raw + S_DATA;
-    auto full_bar = [&](uint32_t s) { return bars + 8u * s; };
-    auto empty_bar = [&](uint32_t s) { return bars + 8u * (3 + s); };
-    auto bfull_bar = [&](uint32_t s) { return bars + 8u * (6 + s); };
-    auto bempty_bar = [&](uint32_t s) { return bars + 8u * (9 + s); };
-    auto tfull_bar = [&](uint32_t s) { return bars + 8u * (12 + s); };
-    auto tempty_bar = [&](uint32_t s) { return bars + 8u * (16 + s); };
-    auto ifull_bar = [&](uint32_t s) { return bars + 8u * (20 + s); };
-    auto iempty_bar = [&](uint32_t s) { return bars + 8u * (28 + s); };
-    auto parked_bar = [&](uint32_t s) { return bars + 8u * (36 + s); };
-    auto sready_bar = [&](uint32_t s) { return bars + 8u * (39 + s); };
-    const uint32_t pdone_bar = bars + 8u * 42, drain_bar = bars + 8u * 43;
-    uint32_t* s_tmem = reinterpret_cast<uint32_t*>(misc + 352);
-    float* s_scale = reinterpret_cast<float*>(misc + 368);
-    uint32_t* s_wmax = reinterpret_cast<uint32_t*>(misc + 384);          // [3][8]
-    volatile int* s_nupd = reinterpret_cast<volatile int*>(misc + 480);  // parked tiles of this CTA (-1: not known yet)
-    Parked* s_park = reinterpret_cast<Parked*>(misc + 512);              // [3]
-    RItem* s_items = reinterpret_cast<RItem*>(misc + 768);               // [RS]
+    // update pipeline barriers
+    auto full_bar = [&](uint32_t s) { return bars + 8u * s; };                  // [US]
+    auto empty_bar = [&](uint32_t s) { return bars + 8u * (2 + s); };           // [US]
+    auto bfull_bar = [&](uint32_t s) { return bars + 8u * (4 + s); };           // [NB]
+    auto bempty_bar = [&](uint32_t s) { return bars + 8u * (6 + s); };          // [NB]
+    auto tfull_bar = [&](uint32_t s) { return bars + 8u * (8 + s); };           // [4] (slot 3: pass-1)
+    auto tempty_bar = [&](uint32_t s) { return bars + 8u * (12 + s); };         // [4]
+    auto ifull_bar = [&](uint32_t s) { return bars + 8u * (16 + s); };          // [RS]
+    auto iempty_bar = [&](uint32_t s) { return bars + 8u * (24 + s); };         // [RS]
+    auto parked_bar = [&](uint32_t s) { return bars + 8u * (32 + s); };         // [NPARK]
+    auto sready_bar = [&](uint32_t s) { return bars + 8u * (35 + s); };         // [NPARK]
+    // pass-1 pipeline barriers
+    auto pfull_bar = [&](uint32_t s) { return bars + 8u * (38 + s); };          // [NS]
+    auto pempty_bar = [&](uint32_t s) { return bars + 8u * (40 + s); };         // [NS]
+    auto pifull_bar = [&](uint32_t s) { return bars + 8u * (42 + s); };         // [PRS]
+    auto piempty_bar = [&](uint32_t s) { return bars + 8u * (46 + s); };        // [PRS]
+    const uint32_t plocal_bar = bars + 8u * 50, drain_bar0 = bars + 8u * 51, drain_bar1 = bars + 8u * 52;
+    uint32_t* s_tmem = reinterpret_cast<uint32_t*>(misc + 432);
+    float* s_scale = reinterpret_cast<float*>(misc + 448);               // [3]
+    volatile int* s_slack = reinterpret_cast<volatile int*>(misc + 472);  // [0] cast warps wait for a tensor, [1] scheduler waits for readiness / is done
+    volatile int* s_nupd = reinterpret_cast<volatile int*>(misc + 464);  // parked tiles of this CTA (-1: not known yet)
+    uint32_t* s_wmax = reinterpret_cast<uint32_t*>(misc + 2832);         // [3][16]
+    Parked* s_park = reinterpret_cast<Parked*>(misc + 576);              // [3] x 64 B
+    RItem* s_items = reinterpret_cast<RItem*>(misc + 768);               // [RS] x 128 B   -> 1792
+    RItem* s_pitems = reinterpret_cast<RItem*>(misc + 1792);             // [PRS] x 128 B  -> 2304
+    STensor* s_cur = reinterpret_cast<STensor*>(misc + 2304);            // tensor of the next update tile   -> 2560
+    STensor* s_p1t = reinterpret_cast<STensor*>(misc + 2560);            // tensor of the pass-1 item        -> 2816
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
     if (threadIdx.x == 0) {
-        for (int s = 0; s < NS; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-        for (int s = 0; s < NB; ++s) { mbar_init(bfull_bar(s), 1); mbar_init(bempty_bar(s), 8); }
-        for (int s = 0; s < 4; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), 8); }
-        for (int s = 0; s < RS; ++s) { mbar_init(ifull_bar(s), 1); mbar_init(iempty_bar(s), 10); }
-        for (int s = 0; s < NPARK; ++s) { mbar_init(parked_bar(s), 8); mbar_init(sready_bar(s), 1); }
-        mbar_init(pdone_bar, 8); mbar_init(drain_bar, 1);
-        *s_nupd = -1;
+        for (int s = 0; s < US; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+        for (int s = 0; s < NB; ++s) { mbar_init(bfull_bar(s), 1); mbar_init(bempty_bar(s), 16); }
+        for (int s = 0; s < 3; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), 16); }
+        mbar_init(tfull_bar(3), 1); mbar_init(tempty_bar(3), 4);
+        for (int s = 0; s < RS; ++s) { mbar_init(ifull_bar(s), 1); mbar_init(iempty_bar(s), 18); }
+        for (int s = 0; s < NPARK; ++s) { mbar_init(parked_bar(s), 16); mbar_init(sready_bar(s), 1); }
+        for (int s = 0; s < NS; ++s) { mbar_init(pfull_bar(s), 1); mbar_init(pempty_bar(s), 1); }
+        for (int s = 0; s < PRS; ++s) { mbar_init(pifull_bar(s), 1); mbar_init(piempty_bar(s), 5); }
+        mbar_init(plocal_bar, 1); mbar_init(drain_bar0, 1); mbar_init(drain_bar1, 1);
+        *s_nupd = -1; s_slack[0] = 0; s_slack[1] = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    if (warp == 10) {
+    if (warp == W_UMMA) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(s_tmem)), "r"(512) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
     }
@@ -194,191 +270,528 @@ stream_kernel(const STensor* __restrict__ T, int nT, const P1Item* __restrict__ 
     tc_fence_after();
     const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(s_tmem);
     auto errset = [&]() { return *reinterpret_cast<volatile int*>(err) != 0; };
+#ifdef GF8_STREAM_PROF
+    // event trace of CTA 0 and CTA 77 (tiles < 48): prof[20480 + (cta ? 2048 : 0) + (code * 48 + tile)] = globaltimer
+    auto EV = [&](int code, uint32_t tile) {
+        if ((blockIdx.x == 0 || blockIdx.x == 77) && tile < 48u && prof) {
+            unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+            prof[20480 + (blockIdx.x ? 2048 : 0) + code * 48 + tile] = (long long)t;
+        }
+    };
+#else
+    auto EV = [&](int, uint32_t) {};
+#endif
+    // bounded barrier wait; the first one that times out leaves its source line in err[1] (read by gf8_sync_check)
+    auto mw = [&](int line, uint32_t bar, uint32_t par, int* e) -> bool {
+#ifdef GF8_STREAM_PROF
+        if (lane == 0 && prof) prof[16384 + blockIdx.x * 32 + warp] = line;       // heartbeat: the wait this warp is in
+#endif
+        if (mbar_wait(bar, par, e)) return true;
+        atomicCAS(e + 1, 0, line);
+        return false;
+    };
+    auto load_tensor = [&](STensor* dst, int t) {          // 256 B record, lanes 0..15 (the record is patched per call: read from L2)
+        if (lane < 16) reinterpret_cast<uint4*>(dst)[lane] = __ldcg(reinterpret_cast<const uint4*>(T + t) + lane);
+        __syncwarp();
+    };
+    // blocking poll of a counter (converged warp); the data it guards is only read through TMA / ld.global.cg, i.e. from L2,
+    // where the producer's release made it visible before the counter moved
+    auto poll_ge = [&](const uint32_t* p, uint32_t target) -> bool {
+        uint32_t v = 0;
+        for (uint32_t spin = 0;; ++spin) {
+            if (lane == 0) v = ld_relaxed(p);
+            v = __shfl_sync(0xFFFFFFFFu, v, 0);
+            if (v >= target) return true;
+            if (spin > (1u << 24) || ((spin & 255u) == 255u && errset())) { if (lane == 0) atomicExch(err, 4); return false; }
+        }
+    };
 
-    if (warp == 8) {
-        // ===== scheduler (lane 0): chooses this CTA's next item, writes it into the ring, streams update base tiles =====
-        if (lane == 0) {
-            uint32_t nring = 0, q = 0;
-            int u = blockIdx.x, tu = 0;
-            int old0 = -1, old1 = -1, old2 = -1;          // tensors of the update tiles q-3, q-2, q-1 (-1: nothing to wait for)
-            int n_parked = 0;
-            bool ok = true;
-            auto push = [&](const RItem& it) -> bool {
-                const uint32_t slot = nring % RS, ph = (nring / RS) & 1u;
-                if (!mbar_wait(iempty_bar(slot), ph ^ 1u, err)) return false;
+    if (warp == W_USCHED) {
+        // ===== update scheduler (converged warp): my next tile (static: tile u -> CTA u mod grid) once its tensor is ready =====
+        PROF_DECL
+        uint32_t nring = 0, q = 0;
+        int u = blockIdx.x, cur_t = -1, n_parked = 0;
+        bool ok = true;
+        TileEnt ent = {0, 0, 0, 0};
+        if (u < n_upd && lane == 0) ent = tiles[u];
+        auto bcast_ent = [&]() {
+            ent.tensor = __shfl_sync(0xFFFFFFFFu, ent.tensor, 0); ent.tij = __shfl_sync(0xFFFFFFFFu, ent.tij, 0);
+            ent.dep_old = __shfl_sync(0xFFFFFFFFu, ent.dep_old, 0); ent.old_tensor = __shfl_sync(0xFFFFFFFFu, ent.old_tensor, 0);
+        };
+        bcast_ent();
+        auto push = [&](const RItem& it) -> bool {               // lane 0 writes the entry
+            const uint32_t slot = nring % RS, ph = (nring / RS) & 1u;
+            bool w_ok;
+            PROF(0, w_ok = mw(__LINE__, iempty_bar(slot), ph ^ 1u, err));
+            if (!w_ok) return false;
+            if (lane == 0) {
                 const uint4* src = reinterpret_cast<const uint4*>(&it);
                 uint4* dst = reinterpret_cast<uint4*>(s_items + slot);
 #pragma unroll
                 for (int w = 0; w < 8; ++w) dst[w] = src[w];
-                mbar_arrive(ifull_bar(slot));             // (release: the entry is visible to whoever acquires the barrier)
-                ++nring;
-                return true;
-            };
-            auto wait_ge = [&](const uint32_t* p, uint32_t target) -> bool {
-                for (uint32_t spin = 0; ld_acquire(p) < target; ++spin) {
-                    if (spin > (1u << 22) || ((spin & 255u) == 255u && errset())) { atomicExch(err, 4); return false; }
-                    __nanosleep(64);
-                }
-                return true;
-            };
-            while (ok) {
-                while (tu < nT && u >= T[tu].upd_start + T[tu].n_tiles) ++tu;
-                const bool have_upd = u < n_upd && tu < nT;
-                bool can = false;
-                if (have_upd) {
-                    const STensor& t = T[tu];
-                    can = t.dep_target == 0 || ld_acquire(t.sync + t.dep_idx) >= (uint32_t)t.dep_target;
-                    if (can && old0 >= 0) { const STensor& o = T[old0]; can = ld_acquire(o.sync + SY_TILES) >= (uint32_t)o.n_tiles; }
-                }
-                if (can) {
-                    const STensor& t = T[tu];
-                    const int tile = u - t.upd_start, ti = tile / t.tiles_n, tj = tile % t.tiles_n;
-                    RItem it;
-                    it.kind = K_UPD; it.slot = (int)(q % NPARK); it.r0 = ti * 128; it.c0 = tj * 128;
-                    it.rows = min(128, t.m - it.r0); it.cols = min(128, t.n - it.c0);
-                    it.ksteps = (t.useA ? 1 : 0) + (t.useG ? 1 : 0); it.mode = t.mode;
-                    it.mapA0 = t.useA ? t.map_Pp128 : t.map_UG128; it.mapB0 = t.useA ? t.map_UA128 : t.map_Qpt128;
-                    it.mapA1 = t.map_UG128; it.mapB1 = t.map_Qpt128;
-                    it.fmt = t.fmt; it.ld = t.n; it.nrb = 1; it.bslot = (int)(q % NB);
-                    it.total = t.n_tiles; it.first = tile == 0 ? 1 : 0; it.n_cols_tile = 128; it.out_f32 = 0;
-                    it.out = t.mode == M_TAP ? (void*)t.tap : (void*)t.codes; it.base32 = nullptr; it.colscale = nullptr; it.sync = t.sync;
-                    it.scale_inv = t.mode == M_BLOCK ? t.scale_inv + (size_t)ti * t.tiles_n + tj : t.scale_inv;
-                    it.done_ctr = nullptr;
-                    if (!(ok = push(it))) break;
-                    // base tile: 128 rows x 128 columns of the gradient (two 64-column halves) in one 3-D box
-                    const uint32_t bs = q % NB, bph = (q / NB) & 1u;
-                    if (!(ok = mbar_wait(bempty_bar(bs), bph ^ 1u, err))) break;
-                    const CUtensorMap* mp = maps + t.map_src_b;
-                    tmap_acquire(mp);
-                    mbar_expect_tx(bfull_bar(bs), BASE_BYTES);
-                    tma_load_3d(base0 + bs * BASE_BYTES, mp, 0, it.r0, tj * 2, bfull_bar(bs));
-                    old0 = old1; old1 = old2; old2 = t.mode == M_PARK ? tu : -1;
-                    if (t.mode != M_TAP) ++n_parked;
-                    u += (int)gridDim.x; ++q;
-                    continue;
-                }
-                int c = *reinterpret_cast<volatile int*>(ctr);
-                if (c < n_p1) {
-                    const P1Item pk = p1[c];
-                    const bool panel = pk.kind == K_PANEL_P || pk.kind == K_PANEL_Q;
-                    if (!panel || !have_upd || T[pk.tensor].byte_pos - T[tu].byte_pos <= lead_bytes) {
-                        c = atomicAdd(ctr, 1);
-                        if (c < n_p1) {
-                            const P1Item pi = p1[c];
-                            const STensor& t = T[pi.tensor];
-                            RItem it;
-                            it.kind = pi.kind; it.slot = 3; it.r0 = pi.r0; it.c0 = 0; it.rows = pi.rows; it.cols = 64; it.mode = 0;
-                            it.mapA1 = it.mapB1 = -1; it.fmt = 0; it.ld = 64; it.nrb = pi.rows > 128 ? 2 : 1; it.bslot = 0;
-                            it.total = it.first = 0; it.n_cols_tile = 64; it.out_f32 = 0; it.base32 = nullptr; it.colscale = nullptr;
-                            it.sync = t.sync; it.scale_inv = nullptr;
-                            if (pi.kind == K_PANEL_P) {
-                                it.ksteps = (t.n + 63) / 64; it.mapA0 = t.map_src_p; it.mapB0 = t.map_UAt;
-                                it.out = t.Pp; it.colscale = t.eA; it.done_ctr = t.sync + SY_P;
-                            } else if (pi.kind == K_PANEL_Q) {
-                                it.ksteps = (t.m + 63) / 64; it.mapA0 = t.map_src_q; it.mapB0 = t.map_UGt;
-                                if (t.useA) { it.out = t.Qt; it.out_f32 = 1; } else { it.out = t.Qpt; it.colscale = t.eG; }
-                                it.done_ctr = t.sync + SY_Q;
-                            } else if (pi.kind == K_S) {
-                                it.ksteps = (t.m + 63) / 64; it.mapA0 = t.map_Pp64; it.mapB0 = t.map_UGt;
-                                it.out = t.SEA; it.done_ctr = t.sync + SY_S; it.nrb = 1;
-                                if (!(ok = wait_ge(t.sync + SY_P, (uint32_t)t.nP))) break;
-                            } else {   // K_QP
-                                it.ksteps = 1; it.mapA0 = t.map_UA256; it.mapB0 = t.map_SEA;
-                                it.out = t.Qpt; it.base32 = t.Qt; it.colscale = t.eG; it.done_ctr = t.sync + SY_QP;
-                                if (!(ok = wait_ge(t.sync + SY_S, 1u) && wait_ge(t.sync + SY_Q, (uint32_t)t.nQ))) break;
-                            }
-                            if (!(ok = push(it))) break;
-                            continue;
-                        }
-                    }
-                }
-                if (!have_upd && c >= n_p1) break;
-                if (errset()) { ok = false; break; }
-                __nanosleep(200);
+                mbar_arrive(ifull_bar(slot));                     // (release: the entry is visible to whoever acquires the barrier)
             }
-            *s_nupd = n_parked;
-            RItem e;
-            e.kind = K_END;
-            push(e);
+            __syncwarp();
+            ++nring;
+            return true;
+        };
+        while (ok && u < n_upd) {
+            if (cur_t != ent.tensor) { cur_t = ent.tensor; PROF(4, load_tensor(s_cur, cur_t)); }
+            // lane 0: my tile's tensor is ready (Q' / P' complete); lane 1: the tile that held this TMEM slot (3 back) belongs to
+            // a complete tensor, so its cast is under way and the slot frees without waiting on other CTAs
+            for (uint32_t spin = 0;; ++spin) {
+                uint32_t v = 0xFFFFFFFFu;
+                const long long _t0 = clock64();
+                if (lane == 0 && (ent.dep_old & 0xFFFF)) v = ld_relaxed(sync_base + (size_t)ent.tensor * SY_WORDS + SY_QP);
+                if (lane == 1 && ent.old_tensor >= 0) v = ld_relaxed(sync_base + (size_t)ent.old_tensor * SY_WORDS + SY_TILES);
+                const uint32_t v0 = __shfl_sync(0xFFFFFFFFu, v, 0), v1 = __shfl_sync(0xFFFFFFFFu, v, 1);
+                const bool rdy = v0 >= (uint32_t)(ent.dep_old & 0xFFFF), oldok = true || v1 >= (uint32_t)(ent.dep_old >> 16);
+                if (rdy && oldok) { if (lane == 0) s_slack[1] = 0; break; }
+                if (lane == 0) s_slack[1] = 1;
+                if (spin > (1u << 24) || ((spin & 255u) == 255u && errset())) { if (lane == 0) atomicExch(err, 6); ok = false; break; }
+#ifdef GF8_STREAM_PROF
+                pf[rdy ? 2 : 1] += clock64() - _t0;
+#endif
+            }
+            if (!ok) break;
+            if (lane == 0) EV(0, q);
+            const STensor& t = *s_cur;
+            const int ti = ent.tij & 0xFFFF, tj = ent.tij >> 16;
+            RItem it;
+            it.kind = K_UPD; it.slot = (int)(q % NPARK); it.r0 = ti * 128; it.c0 = tj * 128;
+            it.rows = min(128, t.m - it.r0); it.cols = min(128, t.n - it.c0);
+            it.ksteps = (t.useA ? 1 : 0) + (t.useG ? 1 : 0); it.mode = t.mode;
+            it.mapA0 = t.useA ? t.map_Pp128 : t.map_UG128; it.mapB0 = t.useA ? t.map_UA128 : t.map_Qpt128;
+            it.mapA1 = t.map_UG128; it.mapB1 = t.map_Qpt128;
+            it.fmt = t.fmt; it.ld = t.n; it.nrb = 1; it.bslot = (int)(q % NB);
+            it.total = t.n_tiles; it.first = (ti | tj) == 0 ? 1 : 0; it.n_cols_tile = 128; it.out_f32 = 0;
+            it.out = t.mode == M_TAP ? (void*)t.tap : (void*)t.codes; it.base32 = nullptr; it.colscale = nullptr; it.sync = t.sync;
+            it.scale_inv = t.mode == M_BLOCK ? t.scale_inv + (size_t)ti * t.tiles_n + tj : t.scale_inv;
+            it.done_ctr = nullptr;
+            if (!(ok = push(it))) break;
+            // base tile: 128 rows x 128 columns of the gradient (two 64-column halves) in one 3-D box
+            const uint32_t bs = q % NB, bph = (q / NB) & 1u;
+            PROF(3, ok = mw(__LINE__, bempty_bar(bs), bph ^ 1u, err));
+            if (!ok) break;
+            if (lane == 0) {
+                const CUtensorMap* mp = maps + t.map_src_b;
+                tmap_acquire(mp);
+                mbar_expect_tx(bfull_bar(bs), BASE_BYTES);
+                tma_load_3d(base0 + bs * BASE_BYTES, mp, 0, it.r0, tj * 2, bfull_bar(bs));
+            }
+            if (t.mode != M_TAP) ++n_parked;
+            u += (int)gridDim.x; ++q;
+            if (u < n_upd && lane == 0) ent = tiles[u];
+            bcast_ent();
         }
-    } else if (warp == 9) {
-        // ===== operand loader (converged warp, one elected lane issues the TMA loads) =====
+        if (lane == 0) { PROF_OUT(0) *s_nupd = n_parked; s_slack[1] = 1; }      // (no update tiles left: pass-1 work is welcome)
+        __syncwarp();
+        RItem e;
+        e.kind = K_END;
+        push(e);
+    } else if (warp == W_ULOAD) {
+        // ===== update operand loader (converged warp, one elected lane issues the TMA loads) =====
         uint32_t stage = 0, phase = 0;
         bool ok = true;
+        PROF_DECL
         for (uint32_t nr = 0; ok; ++nr) {
             const uint32_t slot = nr % RS;
-            if (!(ok = mbar_wait(ifull_bar(slot), (nr / RS) & 1u, err))) break;
+            PROF(0, ok = mw(__LINE__, ifull_bar(slot), (nr / RS) & 1u, err));
+            if (!ok) break;
             const RItem& it = s_items[slot];
-            const int kind = it.kind;
-            if (kind == K_END) break;
+            if (it.kind == K_END) break;
             const int ksteps = it.ksteps, r0 = it.r0, c0 = it.c0;
             const CUtensorMap* mA0 = maps + it.mapA0; const CUtensorMap* mB0 = maps + it.mapB0;
-            const CUtensorMap* mA1 = maps + (it.mapA1 >= 0 ? it.mapA1 : it.mapA0);
-            const CUtensorMap* mB1 = maps + (it.mapB1 >= 0 ? it.mapB1 : it.mapB0);
+            const CUtensorMap* mA1 = maps + it.mapA1; const CUtensorMap* mB1 = maps + it.mapB1;
             __syncwarp();
             if (elect_one()) {
                 mbar_arrive(iempty_bar(slot));
                 tmap_acquire(mA0); tmap_acquire(mB0);
-                if (kind == K_UPD && ksteps > 1) { tmap_acquire(mA1); tmap_acquire(mB1); }
-                fence_async_global();      // P', Q'^T, (S E_A)^T were written by other CTAs through the generic proxy
+                if (ksteps > 1) { tmap_acquire(mA1); tmap_acquire(mB1); }
+                fence_async_global();      // P', Q'^T were written by other CTAs through the generic proxy
             }
             __syncwarp();
             for (int t = 0; t < ksteps && ok; ++t) {
-                if (!(ok = mbar_wait(empty_bar(stage), phase ^ 1u, err))) break;
-                const uint32_t sa = smem0 + stage * STG_BYTES, fb = full_bar(stage);
+                PROF(2, ok = mw(__LINE__, empty_bar(stage), phase ^ 1u, err));
+                if (!ok) break;
+                const uint32_t sa = ustg0 + stage * USTG_BYTES, fb = full_bar(stage);
                 if (elect_one()) {
-                    if (kind == K_PANEL_P) {
-                        mbar_expect_tx(fb, 40960u);
-                        tma_load_2d(sa, mA0, 64 * t, r0, fb);
-                        tma_load_2d(sa + 32768u, mB0, 64 * t, 0, fb);
-                    } else if (kind == K_PANEL_Q) {
-                        mbar_expect_tx(fb, 40960u);
-                        tma_load_3d(sa, mA0, 0, 64 * t, r0 >> 6, fb);
-                        tma_load_2d(sa + 32768u, mB0, 64 * t, 0, fb);
-                    } else if (kind == K_S) {
-                        mbar_expect_tx(fb, 16384u);
-                        tma_load_2d(sa, mA0, 0, 64 * t, fb);
-                        tma_load_2d(sa + 32768u, mB0, 64 * t, 0, fb);
-                    } else if (kind == K_QP) {
-                        mbar_expect_tx(fb, 40960u);
-                        tma_load_2d(sa, mA0, 0, r0, fb);
-                        tma_load_2d(sa + 32768u, mB0, 0, 0, fb);
-                    } else {   // K_UPD
-                        mbar_expect_tx(fb, 32768u);
-                        tma_load_2d(sa, t ? mA1 : mA0, 0, r0, fb);
-                        tma_load_2d(sa + 16384u, t ? mB1 : mB0, 0, c0, fb);
-                    }
+                    mbar_expect_tx(fb, 32768u);
+                    tma_load_2d(sa, t ? mA1 : mA0, 0, r0, fb);
+                    tma_load_2d(sa + 16384u, t ? mB1 : mB0, 0, c0, fb);
                 }
                 __syncwarp();
-                if (++stage == NS) { stage = 0; phase ^= 1u; }
+                if (++stage == US) { stage = 0; phase ^= 1u; }
             }
         }
-    } else if (warp == 10) {
-        // ===== MMA issuer (converged warp, one elected lane issues) =====
-        uint32_t stage = 0, phase = 0, use0 = 0, use1 = 0, use2 = 0, use3 = 0;
+        if (lane == 0) PROF_OUT(1)
+    } else if (warp == W_UMMA) {
+        // ===== update MMA issuer (converged warp, one elected lane issues) =====
+        uint32_t stage = 0, phase = 0;
         bool ok = true;
+        PROF_DECL
+        const uint32_t idesc = instr_desc(128, 0, 0);
         for (uint32_t nr = 0; ok; ++nr) {
             const uint32_t rslot = nr % RS;
-            if (!(ok = mbar_wait(ifull_bar(rslot), (nr / RS) & 1u, err))) break;
+            PROF(0, ok = mw(__LINE__, ifull_bar(rslot), (nr / RS) & 1u, err));
+            if (!ok) break;
             const RItem& it = s_items[rslot];
-            const int kind = it.kind;
-            if (kind == K_END) break;
-            const int ksteps = it.ksteps, nrb = it.nrb;
-            const uint32_t slot = (uint32_t)it.slot;
+            if (it.kind == K_END) break;
+            const int ksteps = it.ksteps;
             __syncwarp();
             if (elect_one()) mbar_arrive(iempty_bar(rslot));
-            const bool upd = kind == K_UPD, a_mn = kind == K_PANEL_Q || kind == K_S;
-            const uint32_t idesc = instr_desc(upd ? 128 : 64, a_mn ? 1 : 0, 0);
-            const uint32_t b_off = upd ? 16384u : 32768u;
-            const uint32_t uses = slot == 0 ? use0 : (slot == 1 ? use1 : (slot == 2 ? use2 : use3));
-            if (slot == 0) ++use0; else if (slot == 1) ++use1; else if (slot == 2) ++use2; else ++use3;
-            if (!(ok = mbar_wait(tempty_bar(slot), (uses & 1u) ^ 1u, err))) break;
+            const uint32_t slot = nr % NPARK;                        // (every ring entry before K_END is an update tile)
+            PROF(1, ok = mw(__LINE__, tempty_bar(slot), ((nr / NPARK) & 1u) ^ 1u, err));
+            if (!ok) break;
             tc_fence_after();
+            if (lane == 0) EV(2, nr);
             const uint32_t d = tmem_base + slot * 128u;
             for (int t = 0; t < ksteps && ok; ++t) {
-                if (!(ok = mbar_wait(full_bar(stage), phase, err))) break;
+                PROF(3, ok = mw(__LINE__, full_bar(stage), phase, err));
+                if (!ok) break;
                 tc_fence_after();
-                const uint32_t sa = smem0 + stage * STG_BYTES, sb = sa + b_off;
+                const uint32_t sa = ustg0 + stage * USTG_BYTES, sb = sa + 16384u;
+                if (elect_one()) {
+#pragma unroll
+                    for (int kk = 0; kk < 4; ++kk)
+                        tc_mma_bf16(d, smem_desc(sa + 32u * kk, 16u, 1024u), smem_desc(sb + 32u * kk, 16u, 1024u), idesc, (t | kk) ? 1u : 0u);
+                    tc_commit(empty_bar(stage));
+                }
+                __syncwarp();
+                if (++stage == US) { stage = 0; phase ^= 1u; }
+            }
+            if (ok && elect_one()) tc_commit(tfull_bar(slot));
+            __syncwarp();
+            if (lane == 0) EV(3, nr);
+        }
+        if (lane == 0) PROF_OUT(2)
+        if (ok) {      // drain: no commit of this issuer may still be in flight when the CTA exits
+            if (elect_one()) tc_commit(drain_bar0);
+            __syncwarp();
+            mw(__LINE__, drain_bar0, 0u, err);
+        }
+    }
+    else if (warp == W_SYNC) {
+        // ===== grid-level sync (lanes 0..2, one per parking slot): tile parked -> tensor counter; tensor complete -> scale =====
+        if (lane < NPARK) {
+            for (uint32_t k = 0;; ++k) {
+                bool stop = false;
+                for (uint32_t spin = 0; !mbar_test(parked_bar(lane), k & 1u); ++spin) {      // (no nanosleep: its granularity is > 1 us here)
+                    const int tot = *s_nupd;
+                    if ((tot >= 0 && (int)(k * NPARK + lane) >= tot) || ((spin & 1023u) == 1023u && errset())) { stop = true; break; }
+                }
+                if (stop) break;
+                EV(6, k * NPARK + lane);
+                const Parked pk = s_park[lane];
+                uint32_t mx = 0;
+#pragma unroll
+                for (int w = 0; w < 16; ++w) mx = max(mx, s_wmax[lane * 16 + w]);
+                float scale, si;
+                const float fmax = pk.fmt == 0 ? 448.0f : 57344.0f;
+                if (pk.local) {
+                    scales_from_amax(mx, fmax, scale, si);
+                    *pk.scale_inv = si;
+                    red_release_add(pk.sync + SY_TILES, 1u);          // (lead control of the pass-1 pipeline counts tiles)
+                } else {
+                    // the tile's amax reaches L2 (an atomic WITH return has been performed when its value arrives) before the tile is
+                    // counted: the count carries a data dependency on the returned value instead of a (slow) gpu-scope release fence
+                    const uint32_t old = atomicMax(pk.sync + SY_AMAX, mx);
+                    asm volatile("red.relaxed.gpu.global.add.u32 [%0], %1;" ::"l"(pk.sync + SY_TILES), "r"(1u + (old & 0u)) : "memory");
+                    EV(7, k * NPARK + lane);
+                    bool bad = false;
+                    for (uint32_t spin = 0; ld_relaxed(pk.sync + SY_TILES) < (uint32_t)pk.total; ++spin) {
+                        if (spin > (1u << 24) || ((spin & 255u) == 255u && errset())) { bad = true; break; }
+                    }
+                    if (bad) { atomicExch(err, 2); break; }
+                    scales_from_amax(*reinterpret_cast<volatile uint32_t*>(pk.sync + SY_AMAX), fmax, scale, si);
+                    if (pk.first) *pk.scale_inv = si;
+                }
+                s_scale[lane] = scale;
+                mbar_arrive(sready_bar(lane));
+                EV(8, k * NPARK + lane);
+            }
+        }
+    } else if (warp >= W_UEPI) {
+        // ===== update epilogue warps (16): warp w reaches TMEM lanes 32 (w & 3) .. +31 and takes the 32-column quarter (w - W_UEPI) >> 2 of
+        // the tile, so each phase is ONE TMEM round trip.  Per tile, in ring order: cast the tile that held this TMEM slot before
+        // (tile q - 3: its scale arrives when its tensor is complete), then park this one (W~ = base + accumulator, running amax, FP32
+        // tile back into its TMEM slot).  The order is forced -- the MMAs of tile q cannot run before tile q - 3 has left the slot -- so
+        // every wait is a plain blocking wait.
+        const int q4 = warp & 3, cq = (warp - W_UEPI) >> 2, ew = warp - W_UEPI;
+        const int r = q4 * 32 + lane;                           // accumulator row of this thread
+        const uint32_t lane_off = ((uint32_t)(q4 * 32) << 16) + 32u * (uint32_t)cq;
+        bool ok = true;
+        PROF_DECL
+        auto cast_tile = [&](uint32_t k) -> bool {              // tile k of this CTA (ordinal): scale, FP8 cast, store, free the slot
+            const uint32_t slot = k % NPARK;
+            bool w_ok;
+            if (ew == 0 && lane == 0 && !mbar_test(sready_bar(slot), (k / NPARK) & 1u)) s_slack[0] = 1;   // this CTA is ahead of the grid
+            PROF(0, w_ok = mw(__LINE__, sready_bar(slot), (k / NPARK) & 1u, err));
+            if (!w_ok) return false;
+            if (ew == 0 && lane == 0) { s_slack[0] = 0; EV(9, k); }
+            const Parked pk = s_park[slot];
+            const float scale = s_scale[slot];
+            uint32_t a[32];
+            tmem_ld32_nowait(tmem_base + slot * 128u + lane_off, a);
+            tmem_wait();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(tempty_bar(slot));        // (the tile is in registers: its slot may take the next accumulator)
+            uint4 cd[2];
+            uint32_t* cw = reinterpret_cast<uint32_t*>(cd);
+            if (pk.fmt == 0) {
+#pragma unroll
+                for (int j = 0; j < 8; ++j)
+                    cw[j] = cast4<0>(__uint_as_float(a[4 * j]), __uint_as_float(a[4 * j + 1]), __uint_as_float(a[4 * j + 2]), __uint_as_float(a[4 * j + 3]), scale);
+            } else {
+#pragma unroll
+                for (int j = 0; j < 8; ++j)
+                    cw[j] = cast4<1>(__uint_as_float(a[4 * j]), __uint_as_float(a[4 * j + 1]), __uint_as_float(a[4 * j + 2]), __uint_as_float(a[4 * j + 3]), scale);
+            }
+            if (r < pk.rows) {
+                uint8_t* orow = pk.out + (int64_t)(pk.row0 + r) * pk.ld + pk.col0 + 32 * cq;
+#pragma unroll
+                for (int h = 0; h < 2; ++h)
+                    if (32 * cq + 16 * h < pk.cols) *reinterpret_cast<uint4*>(orow + 16 * h) = cd[h];
+            }
+            if (ew == 0 && lane == 0) EV(10, k);
+            return true;
+        };
+        uint32_t nq = 0, ncast = 0, npark = 0, idle = 0;
+        bool have = false, done = false;
+        for (;;) {
+            // one shared-memory round trip per look: lane 0 the oldest parked tile's scale, lane 1 the next ring entry, lanes 2 / 3
+            // the next tile's accumulator / base tile.  Casting comes first: it frees a TMEM slot for the MMAs of a later tile.
+            uint32_t hit = 0;
+            if (lane < 4) {
+                uint32_t bar, par;
+                bool want;
+                if (lane == 0) { want = ncast < npark; bar = sready_bar(ncast % NPARK); par = (ncast / NPARK) & 1u; }
+                else if (lane == 1) { want = !done && !have; bar = ifull_bar(nq % RS); par = (nq / RS) & 1u; }
+                else if (lane == 2) { want = !done; bar = tfull_bar(nq % NPARK); par = (nq / NPARK) & 1u; }
+                else { want = !done; bar = bfull_bar(nq % NB); par = (nq / NB) & 1u; }
+                hit = want && mbar_test(bar, par) ? 1u : 0u;
+            }
+            const uint32_t mask = __ballot_sync(0xFFFFFFFFu, hit != 0);
+            if (mask & 1u) { if (!(ok = cast_tile(ncast))) break; ++ncast; idle = 0; continue; }
+            if ((mask & 2u) && !have) {
+                have = true;
+                if (s_items[nq % RS].kind == K_END) { done = true; have = false; }
+            }
+            if (!(have && (mask & 12u) == 12u)) {
+                if (done && ncast == npark) break;
+                if (++idle > (1u << 22) || ((idle & 1023u) == 1023u && errset())) { if (lane == 0) atomicExch(err, 5); ok = false; break; }
+                // nothing to do yet: a short sleep on the event that usually comes first
+                if (lane == 0) {
+                    if (ncast < npark) mbar_nap(sready_bar(ncast % NPARK), (ncast / NPARK) & 1u);
+                    else if (!done) mbar_nap(have ? tfull_bar(nq % NPARK) : ifull_bar(nq % RS), have ? (nq / NPARK) & 1u : (nq / RS) & 1u);
+                }
+                __syncwarp();
+                continue;
+            }
+            idle = 0;
+            const uint32_t rslot = nq % RS, slot = nq % NPARK, bs = nq % NB;
+            const RItem& it = s_items[rslot];
+            const int mode = it.mode;
+            tc_fence_after();
+            if (ew == 0 && lane == 0) EV(4, nq);
+            const uint32_t taddr = tmem_base + slot * 128u + lane_off;
+            const uint32_t brow = base0 + bs * BASE_BYTES + (uint32_t)(cq >> 1) * 16384u + (uint32_t)r * 128u;
+            uint32_t a[32];
+            tmem_ld32_nowait(taddr, a);
+            uint4 b[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) b[j] = lds128(brow + (((uint32_t)(4 * (cq & 1) + j) ^ (uint32_t)(r & 7)) << 4));
+            tmem_wait();
+            float* v = reinterpret_cast<float*>(a);
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const uint32_t w[4] = {b[j].x, b[j].y, b[j].z, b[j].w};
+#pragma unroll
+                for (int e = 0; e < 4; ++e)
+                    add_bf16x2(w[e], v[8 * j + 2 * e], v[8 * j + 2 * e + 1], v[8 * j + 2 * e], v[8 * j + 2 * e + 1]);
+            }
+            if (mode == M_TAP) {
+                if (r < it.rows) {
+                    float* trow = reinterpret_cast<float*>(it.out) + (int64_t)(it.r0 + r) * it.ld + it.c0 + 32 * cq;
+#pragma unroll
+                    for (int h = 0; h < 8; ++h)
+                        if (32 * cq + 4 * h < it.cols) *reinterpret_cast<float4*>(trow + 4 * h) = make_float4(v[4 * h], v[4 * h + 1], v[4 * h + 2], v[4 * h + 3]);
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) { mbar_arrive(tempty_bar(slot)); mbar_arrive(bempty_bar(bs)); }
+            } else {
+                float mx = 0.0f;
+#pragma unroll
+                for (int e = 0; e < 16; ++e) mx = max3abs(mx, v[2 * e], v[2 * e + 1]);
+                tmem_st32(taddr, a);
+                uint32_t wm;                                    // (non-negative floats and NaN order as integers)
+                asm volatile("redux.sync.max.u32 %0, %1, 0xffffffff;" : "=r"(wm) : "r"(__float_as_uint(mx)));
+                if (lane == 0) s_wmax[slot * 16 + ew] = wm;
+                if (ew == 0 && lane == 0) {
+                    Parked pk;
+                    pk.sync = it.sync; pk.scale_inv = it.scale_inv; pk.out = reinterpret_cast<uint8_t*>(it.out);
+                    pk.ld = it.ld; pk.row0 = it.r0; pk.col0 = it.c0; pk.rows = it.rows; pk.cols = it.cols; pk.fmt = it.fmt;
+                    pk.total = it.total; pk.first = it.first; pk.local = mode == M_BLOCK ? 1 : 0; pk.pad = 0;
+                    s_park[slot] = pk;
+                }
+                tmem_wait_st();
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) { mbar_arrive(parked_bar(slot)); mbar_arrive(bempty_bar(bs)); }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(iempty_bar(rslot));
+            if (ew == 0 && lane == 0) EV(5, nq);
+            if (mode != M_TAP) ++npark;
+            ++nq; have = false;
+        }
+        if (ew == 0 && lane == 0) PROF_OUT(3)
+    }
+    else if (warp == W_PPROD) {
+        // ===== pass-1 producer (converged warp): claims the next item of the list, writes it into the pass-1 ring and streams its
+        // operand K-steps; gradient K-steps are prefetched into L2 a few steps ahead of the two-stage shared-memory ring =====
+        PROF_DECL
+        uint32_t nring = 0, stage = 0, phase = 0, n_sp = 0;
+        bool ok = true;
+        auto push = [&](const RItem& it) -> bool {
+            const uint32_t slot = nring % PRS, ph = (nring / PRS) & 1u;
+            bool w_ok;
+            PROF(0, w_ok = mw(__LINE__, piempty_bar(slot), ph ^ 1u, err));
+            if (!w_ok) return false;
+            if (lane == 0) {
+                const uint4* src = reinterpret_cast<const uint4*>(&it);
+                uint4* dst = reinterpret_cast<uint4*>(s_pitems + slot);
+#pragma unroll
+                for (int w = 0; w < 8; ++w) dst[w] = src[w];
+                mbar_arrive(pifull_bar(slot));
+            }
+            __syncwarp();
+            ++nring;
+            return true;
+        };
+        // one K-step: wait for a free stage, then A (bytes_a) and B (8 KB) by TMA.  akind: 0 = 2-D box at (ca, ra), 1 = 3-D box at (0, ra, ca)
+        auto kstep = [&](const CUtensorMap* mA, int akind, int ca, int ra, uint32_t bytes_a, const CUtensorMap* mB, int cb, int rb_) -> bool {
+            bool w_ok;
+            PROF(3, w_ok = mw(__LINE__, pempty_bar(stage), phase ^ 1u, err));
+            if (!w_ok) return false;
+            const uint32_t sa = smem0 + stage * STG_BYTES, fb = pfull_bar(stage);
+            if (elect_one()) {
+                mbar_expect_tx(fb, bytes_a + 8192u);
+                if (akind) tma_load_3d(sa, mA, 0, ra, ca, fb); else tma_load_2d(sa, mA, ca, ra, fb);
+                tma_load_2d(sa + 32768u, mB, cb, rb_, fb);
+            }
+            __syncwarp();
+            if (++stage == NS) { stage = 0; phase ^= 1u; }
+            return true;
+        };
+        constexpr int PF = 6;                         // L2 prefetch distance in K-steps (32 KB of gradient each)
+        while (ok) {
+            // pass-1 work goes to the CTAs whose update pipeline has slack (it waits for the grid or for readiness): tensors complete
+            // in lock step across CTAs, so a CTA that streams panels while its update tiles are the late ones would hold everyone up
+            PROF(5, for (uint32_t spin = 0; !(s_slack[0] | s_slack[1]) && spin < 64u; ++spin) __nanosleep(100));
+            int c = 0;
+            if (lane == 0) c = atomicAdd(ctr, 1);
+            c = __shfl_sync(0xFFFFFFFFu, c, 0);
+            if (c >= n_p1) break;
+            P1Item pi;
+            if (lane == 0) pi = p1[c];
+            pi.kind = __shfl_sync(0xFFFFFFFFu, pi.kind, 0); pi.tensor = __shfl_sync(0xFFFFFFFFu, pi.tensor, 0);
+            pi.r0 = __shfl_sync(0xFFFFFFFFu, pi.r0, 0); pi.rows = __shfl_sync(0xFFFFFFFFu, pi.rows, 0);
+            pi.gate_tensor = __shfl_sync(0xFFFFFFFFu, pi.gate_tensor, 0); pi.gate_total = __shfl_sync(0xFFFFFFFFu, pi.gate_total, 0);
+            PROF(4, load_tensor(s_p1t, pi.tensor));
+            const STensor& t = *s_p1t;
+            // lead control: this panel's tensor may not run further ahead of the update frontier than the plan's lead
+            if (pi.gate_tensor >= 0) { PROF(1, ok = poll_ge(sync_base + (size_t)pi.gate_tensor * SY_WORDS + SY_TILES, (uint32_t)pi.gate_total)); if (!ok) break; }
+            const bool both = t.useA && t.useG, isP = pi.kind == K_PANEL_P;
+            RItem it;
+            it.kind = pi.kind; it.slot = 3; it.r0 = pi.r0; it.c0 = 0; it.rows = pi.rows; it.cols = 64; it.mode = 0;
+            it.mapA0 = isP ? t.map_src_p : t.map_src_q; it.mapB0 = isP ? t.map_UAt : t.map_UGt; it.mapA1 = it.mapB1 = -1;
+            it.fmt = 0; it.ld = 64; it.nrb = pi.rows > 128 ? 2 : 1; it.bslot = 0;
+            it.total = 0; it.first = (!isP && both) ? 1 : 0;              // first: a Q panel whose last K-step adds U_A (S E_A)^T
+            it.n_cols_tile = 64; it.out_f32 = 0; it.base32 = nullptr; it.sync = t.sync; it.scale_inv = nullptr;
+            const int base_steps = isP ? (t.n + 63) / 64 : (t.m + 63) / 64;
+            it.ksteps = base_steps + it.first;
+            it.out = isP ? (void*)t.Pp : (void*)t.Qpt; it.colscale = isP ? t.eA : t.eG;
+            it.done_ctr = (isP && both) ? nullptr : t.sync + SY_QP;      // (a P panel of a two-sided layer is followed by its S partial)
+            if (!(ok = push(it))) break;
+            const CUtensorMap* mA = maps + it.mapA0; const CUtensorMap* mB = maps + it.mapB0;
+            const int r0 = pi.r0;
+            if (elect_one()) {
+                tmap_acquire(mA); tmap_acquire(mB);
+                for (int ks = 0; ks < min(PF, base_steps); ++ks) {
+                    if (isP) tma_prefetch_2d(mA, 64 * ks, r0); else tma_prefetch_3d(mA, 0, 64 * ks, r0 >> 6);
+                }
+            }
+            __syncwarp();
+            for (int ks = 0; ks < base_steps && ok; ++ks) {
+                if (ks + PF < base_steps && elect_one()) {
+                    if (isP) tma_prefetch_2d(mA, 64 * (ks + PF), r0); else tma_prefetch_3d(mA, 0, 64 * (ks + PF), r0 >> 6);
+                }
+                __syncwarp();
+                ok = isP ? kstep(mA, 0, 64 * ks, r0, 32768u, mB, 64 * ks, 0) : kstep(mA, 1, r0 >> 6, 64 * ks, 32768u, mB, 64 * ks, 0);
+            }
+            if (!ok) break;
+            if (it.first) {
+                // Q'^T = (Q^T + U_A (S E_A)^T) E_G: once the tensor's (S E_A)^T is complete, one more K-step adds U_A (S E_A)^T to
+                // the Q^T accumulators (A = U_A rows of this column panel, K-major; B = (S E_A)^T as [g][a])
+                PROF(2, ok = poll_ge(t.sync + SY_S, 1u));
+                if (!ok) break;
+                const CUtensorMap* mU = maps + t.map_UA256; const CUtensorMap* mS = maps + t.map_SEA;
+                if (elect_one()) { tmap_acquire(mU); tmap_acquire(mS); fence_async_global(); }
+                __syncwarp();
+                if (!(ok = kstep(mU, 0, 0, r0, 32768u, mS, 0, 0))) break;
+            } else if (isP && both) {
+                // S partial of this row panel: (S E_A)^T_i = P'(i)^T U_G(i), K = the panel's rows; P'(i) was just written by this
+                // CTA's pass-1 epilogue (local barrier), read back MN-major through TMA
+                RItem sp = it;
+                sp.kind = K_SP; sp.nrb = 1; sp.ksteps = (pi.rows + 63) / 64; sp.first = 0;
+                sp.mapA0 = t.map_Pp64; sp.mapB0 = t.map_UGt;
+                sp.out = t.Spart + (size_t)(r0 >> 8) * 4096; sp.base32 = t.Spart; sp.colscale = nullptr; sp.total = t.nP;
+                sp.scale_inv = reinterpret_cast<float*>(t.SEA); sp.done_ctr = t.sync + SY_P;
+                if (!(ok = push(sp))) break;
+                PROF(2, ok = mw(__LINE__, plocal_bar, n_sp & 1u, err));
+                ++n_sp;
+                if (!ok) break;
+                const CUtensorMap* mP = maps + t.map_Pp64; const CUtensorMap* mG = maps + t.map_UGt;
+                if (elect_one()) { tmap_acquire(mP); tmap_acquire(mG); fence_async_global(); }
+                __syncwarp();
+                for (int ks = 0; ks < sp.ksteps && ok; ++ks) ok = kstep(mP, 0, 0, r0 + 64 * ks, 8192u, mG, r0 + 64 * ks, 0);
+                if (!ok) break;
+            }
+        }
+        if (lane == 0) PROF_OUT(4)
+        RItem e;
+        e.kind = K_END;
+        push(e);
+    } else if (warp == W_PMMA) {
+        // ===== pass-1 MMA issuer: accumulators in TMEM slot 3 (two 64-column halves, one per 128-row block of the panel) =====
+        uint32_t stage = 0, phase = 0;
+        bool ok = true;
+        PROF_DECL
+        const uint32_t d = tmem_base + 3u * 128u;
+        for (uint32_t nr = 0; ok; ++nr) {
+            const uint32_t rslot = nr % PRS;
+            PROF(0, ok = mw(__LINE__, pifull_bar(rslot), (nr / PRS) & 1u, err));
+            if (!ok) break;
+            const RItem& it = s_pitems[rslot];
+            const int kind = it.kind;
+            if (kind == K_END) break;
+            const int ksteps = it.ksteps, nrb = it.nrb, fused = it.first;
+            __syncwarp();
+            if (elect_one()) mbar_arrive(piempty_bar(rslot));
+            const bool mn = kind == K_PANEL_Q || kind == K_SP;
+            PROF(1, ok = mw(__LINE__, tempty_bar(3), (nr & 1u) ^ 1u, err));
+            if (!ok) break;
+            tc_fence_after();
+            for (int t = 0; t < ksteps && ok; ++t) {
+                PROF(3, ok = mw(__LINE__, pfull_bar(stage), phase, err));
+                if (!ok) break;
+                tc_fence_after();
+                const uint32_t sa = smem0 + stage * STG_BYTES, sb = sa + 32768u;
+                const bool a_mn = mn && !(fused && t == ksteps - 1);          // (the fused Q' step reads U_A K-major)
+                const uint32_t idesc = instr_desc(64, a_mn ? 1 : 0, 0);
                 if (elect_one()) {
 #pragma unroll
                     for (int kk = 0; kk < 4; ++kk) {
@@ -389,254 +802,131 @@ stream_kernel(const STensor* __restrict__ T, int nT, const P1Item* __restrict__ 
                             tc_mma_bf16(d + 64u * rb, da, db, idesc, (t | kk) ? 1u : 0u);
                         }
                     }
-                    tc_commit(empty_bar(stage));
+                    tc_commit(pempty_bar(stage));
                 }
                 __syncwarp();
                 if (++stage == NS) { stage = 0; phase ^= 1u; }
             }
-            if (ok && elect_one()) tc_commit(tfull_bar(slot));
+            if (ok && elect_one()) tc_commit(tfull_bar(3));
             __syncwarp();
         }
-        if (ok) {      // drain: no commit of this issuer may still be in flight when the CTA exits
-            if (elect_one()) tc_commit(drain_bar);
+        if (lane == 0) PROF_OUT(5)
+        if (ok) {
+            if (elect_one()) tc_commit(drain_bar1);
             __syncwarp();
-            mbar_wait(drain_bar, 0u, err);
-        }
-    }
-    else if (warp == 11) {
-        // ===== grid-level sync (lanes 0..2, one per parking slot): tile parked -> tensor counter; tensor complete -> scale =====
-        if (lane < NPARK) {
-            for (uint32_t k = 0;; ++k) {
-                bool stop = false;
-                for (uint32_t spin = 0; !mbar_test(parked_bar(lane), k & 1u); ++spin) {
-                    const int tot = *s_nupd;
-                    if ((tot >= 0 && (int)(k * NPARK + lane) >= tot) || ((spin & 1023u) == 1023u && errset())) { stop = true; break; }
-                    __nanosleep(64);
-                }
-                if (stop) break;
-                const Parked pk = s_park[lane];
-                uint32_t mx = 0;
-#pragma unroll
-                for (int w = 0; w < 8; ++w) mx = max(mx, s_wmax[lane * 8 + w]);
-                float scale, si;
-                const float fmax = pk.fmt == 0 ? 448.0f : 57344.0f;
-                if (pk.local) {
-                    scales_from_amax(mx, fmax, scale, si);
-                    *pk.scale_inv = si;
-                } else {
-                    if (mx) atomicMax(pk.sync + SY_AMAX, mx);
-                    red_release_add(pk.sync + SY_TILES, 1u);
-                    bool bad = false;
-                    for (uint32_t spin = 0; ld_acquire(pk.sync + SY_TILES) < (uint32_t)pk.total; ++spin) {
-                        if (spin > (1u << 22) || ((spin & 255u) == 255u && errset())) { bad = true; break; }
-                        __nanosleep(64);
-                    }
-                    if (bad) { atomicExch(err, 2); break; }
-                    scales_from_amax(*reinterpret_cast<volatile uint32_t*>(pk.sync + SY_AMAX), fmax, scale, si);
-                    if (pk.first) *pk.scale_inv = si;
-                }
-                s_scale[lane] = scale;
-                mbar_arrive(sready_bar(lane));
-            }
+            mw(__LINE__, drain_bar1, 0u, err);
         }
     } else {
-        // ===== epilogue warps 0..7: each warp follows the item ring on its own (no block-level barrier) =====
-        const int q4 = warp & 3, half = warp >> 2;
-        const int r = q4 * 32 + lane;                           // accumulator row (TMEM lane) of this thread
+        // ===== pass-1 epilogue warps W_PEPI..+3 (a warp reaches the TMEM lane quarter warp & 3): panel rows straight to global memory =====
+        const int q4 = warp & 3;
+        const int r = q4 * 32 + lane, tid = threadIdx.x - W_PEPI * 32;
         const uint32_t lane_off = (uint32_t)(q4 * 32) << 16;
-        uint32_t nr = 0, nq = 0, ncast = 0, use3 = 0, idle = 0;
-        bool have = false, done = false, ok = true;
-        auto test = [&](uint32_t bar, uint32_t par) -> bool {
-            uint32_t v = 0;
-            if (lane == 0) v = mbar_test(bar, par) ? 1u : 0u;
-            return __shfl_sync(0xFFFFFFFFu, v, 0) != 0;
-        };
-        while (ok) {
-            // (1) the oldest parked tile whose scale has arrived: scale, cast, store, free its TMEM slot
-            if (ncast < nq && test(sready_bar(ncast % NPARK), (ncast / NPARK) & 1u)) {
-                const uint32_t slot = ncast % NPARK;
-                const Parked pk = s_park[slot];
-                const float scale = s_scale[slot];
-                const uint32_t taddr = tmem_base + slot * 128u + lane_off + (uint32_t)half * 64u;
-                const bool row_ok = r < pk.rows;
-                uint8_t* orow = pk.out + (int64_t)(pk.row0 + r) * pk.ld + pk.col0 + 64 * half;
-#pragma unroll
-                for (int g = 0; g < 2; ++g) {
-                    uint32_t a[32];
-                    tmem_ld32_nowait(taddr + 32u * g, a);
-                    tmem_wait();
-                    uint4 cd[2];
-                    uint32_t* cw = reinterpret_cast<uint32_t*>(cd);
-                    if (pk.fmt == 0) {
-#pragma unroll
-                        for (int j = 0; j < 8; ++j)
-                            cw[j] = cast4<0>(__uint_as_float(a[4 * j]), __uint_as_float(a[4 * j + 1]), __uint_as_float(a[4 * j + 2]), __uint_as_float(a[4 * j + 3]), scale);
-                    } else {
-#pragma unroll
-                        for (int j = 0; j < 8; ++j)
-                            cw[j] = cast4<1>(__uint_as_float(a[4 * j]), __uint_as_float(a[4 * j + 1]), __uint_as_float(a[4 * j + 2]), __uint_as_float(a[4 * j + 3]), scale);
-                    }
-                    if (row_ok) {
-#pragma unroll
-                        for (int h = 0; h < 2; ++h)
-                            if (64 * half + 32 * g + 16 * h < pk.cols) *reinterpret_cast<uint4*>(orow + 32 * g + 16 * h) = cd[h];
-                    }
-                }
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(tempty_bar(slot));
-                ++ncast; idle = 0;
-                continue;
-            }
-            if (!done) {
-                const uint32_t rslot = nr % RS;
-                if (!have && test(ifull_bar(rslot), (nr / RS) & 1u)) {
-                    have = true;
-                    if (s_items[rslot].kind == K_END) { done = true; have = false; }
-                }
-                if (have) {
-                    const RItem& it = s_items[rslot];
-                    const int kind = it.kind;
-                    const uint32_t slot = (uint32_t)it.slot;
-                    const bool upd = kind == K_UPD;
-                    const uint32_t tpar = upd ? (nq / NPARK) & 1u : use3 & 1u;
-                    if (test(tfull_bar(slot), tpar) && (!upd || test(bfull_bar(nq % NB), (nq / NB) & 1u))) {
-                        tc_fence_after();
-                        if (upd) {
-                            const uint32_t bs = nq % NB;
-                            const uint32_t taddr = tmem_base + slot * 128u + lane_off + (uint32_t)half * 64u;
-                            const uint32_t brow = base0 + bs * BASE_BYTES + (uint32_t)half * 16384u + (uint32_t)r * 128u;
-                            const int mode = it.mode;
-                            float mx = 0.0f;
-                            float* trow = mode == M_TAP ? reinterpret_cast<float*>(it.out) + (int64_t)(it.r0 + r) * it.ld + it.c0 + 64 * half : nullptr;
-#pragma unroll
-                            for (int g = 0; g < 2; ++g) {
-                                uint32_t a[32];
-                                tmem_ld32_nowait(taddr + 32u * g, a);
-                                uint4 b[4];
-#pragma unroll
-                                for (int j = 0; j < 4; ++j) b[j] = lds128(brow + (((uint32_t)(4 * g + j) ^ (uint32_t)(r & 7)) << 4));
-                                tmem_wait();
-                                float v[32];
-#pragma unroll
-                                for (int j = 0; j < 4; ++j) {
-                                    const uint32_t w[4] = {b[j].x, b[j].y, b[j].z, b[j].w};
-#pragma unroll
-                                    for (int e = 0; e < 4; ++e)
-                                        add_bf16x2(w[e], __uint_as_float(a[8 * j + 2 * e]), __uint_as_float(a[8 * j + 2 * e + 1]), v[8 * j + 2 * e], v[8 * j + 2 * e + 1]);
-                                }
-                                if (mode == M_TAP) {
-                                    if (r < it.rows) {
-#pragma unroll
-                                        for (int h = 0; h < 8; ++h)
-                                            if (64 * half + 32 * g + 4 * h < it.cols)
-                                                *reinterpret_cast<float4*>(trow + 32 * g + 4 * h) = make_float4(v[4 * h], v[4 * h + 1], v[4 * h + 2], v[4 * h + 3]);
-                                    }
-                                } else {
-#pragma unroll
-                                    for (int e = 0; e < 16; ++e) mx = max3abs(mx, v[2 * e], v[2 * e + 1]);
-                                    uint32_t wv[32];
-#pragma unroll
-                                    for (int e = 0; e < 32; ++e) wv[e] = __float_as_uint(v[e]);
-                                    tmem_st32(taddr + 32u * g, wv);
-                                }
-                            }
-                            if (mode == M_TAP) {
-                                tc_fence_before();
-                                __syncwarp();
-                                if (lane == 0) { mbar_arrive(tempty_bar(slot)); mbar_arrive(bempty_bar(bs)); }
-                                ++ncast;                     // nothing parked: the tile is finished
-                            } else {
-                                tmem_wait_st();
-                                const uint32_t wm = warp_max_u32(__float_as_uint(mx));     // (non-negative floats and NaN order as integers)
-                                if (lane == 0) s_wmax[slot * 8 + warp] = wm;
-                                if (threadIdx.x == 0) {
-                                    Parked pk;
-                                    pk.sync = it.sync; pk.scale_inv = it.scale_inv; pk.out = reinterpret_cast<uint8_t*>(it.out);
-                                    pk.ld = it.ld; pk.row0 = it.r0; pk.col0 = it.c0; pk.rows = it.rows; pk.cols = it.cols; pk.fmt = it.fmt;
-                                    pk.total = it.total; pk.first = it.first; pk.local = mode == M_BLOCK ? 1 : 0; pk.pad = 0;
-                                    s_park[slot] = pk;
-                                }
-                                tc_fence_before();
-                                __syncwarp();
-                                if (lane == 0) { mbar_arrive(parked_bar(slot)); mbar_arrive(bempty_bar(bs)); }
-                            }
-                            ++nq;
-                        } else {
-                            // pass-1 item: a panel of up to 256 rows x 64 columns (row block = warp >> 2), straight to global memory
-                            const int rb = half, rr = 128 * rb + r;
-                            const bool row_ok = rb < it.nrb && rr < it.rows && (kind != K_S || r < 64);
-                            const int64_t grow = it.r0 + rr;
-                            const uint32_t taddr = tmem_base + 3u * 128u + lane_off + 64u * (uint32_t)rb;
-                            if (rb < it.nrb) {
+        volatile int* s_last = reinterpret_cast<volatile int*>(misc + 468);
+        volatile int* s_pok = reinterpret_cast<volatile int*>(misc + 2816);      // [4]
+        bool ok = true;
+        PROF_DECL
+        auto group_sync = [&]() { asm volatile("bar.sync 2, 128;" ::: "memory"); };
+        for (uint32_t nr = 0; ok; ++nr) {
+            const uint32_t rslot = nr % PRS;
+            PROF(0, ok = mw(__LINE__, pifull_bar(rslot), (nr / PRS) & 1u, err));
+            const RItem& it = s_pitems[rslot];
+            const int kind = it.kind;
+            if (ok && kind == K_END) break;
+            if (ok) { PROF(1, ok = mw(__LINE__, tfull_bar(3), nr & 1u, err)); }
+            // the four warps leave together (they meet at CTA-level barriers below): agree on `ok` first
+            if (lane == 0) s_pok[warp - W_PEPI] = ok ? 1 : 0;
+            group_sync();
+            ok = (s_pok[0] & s_pok[1] & s_pok[2] & s_pok[3]) != 0;
+            group_sync();
+            if (!ok) break;
+            tc_fence_after();
+            const int nrb = it.nrb;
+            for (int rb = 0; rb < nrb; ++rb) {
+                const int rr = 128 * rb + r;
+                const bool row_ok = kind == K_SP ? r < 64 : rr < it.rows;
+                const int64_t grow = it.r0 + rr;
+                const uint32_t taddr = tmem_base + 3u * 128u + lane_off + 64u * (uint32_t)rb;
 #pragma unroll 1
-                                for (int c0 = 0; c0 < 64; c0 += 16) {
-                                    uint32_t a[16];
-                                    tmem_ld16(taddr + c0, a);
-                                    if (!row_ok) continue;
-                                    float v[16];
-#pragma unroll
-                                    for (int e = 0; e < 16; ++e) v[e] = __uint_as_float(a[e]);
-                                    if (kind == K_S) {
-                                        bf16* o = reinterpret_cast<bf16*>(it.out);
-#pragma unroll
-                                        for (int e = 0; e < 16; ++e) o[(int64_t)(c0 + e) * 64 + r] = __float2bfloat16_rn(v[e]);
-                                        continue;
-                                    }
-                                    if (it.base32) {
-                                        const float4* bp = reinterpret_cast<const float4*>(it.base32 + grow * 64 + c0);
-#pragma unroll
-                                        for (int e = 0; e < 4; ++e) {
-                                            const float4 x = __ldcg(bp + e);
-                                            v[4 * e] += x.x; v[4 * e + 1] += x.y; v[4 * e + 2] += x.z; v[4 * e + 3] += x.w;
-                                        }
-                                    }
-                                    if (it.colscale) {
-#pragma unroll
-                                        for (int e = 0; e < 16; ++e) v[e] *= __ldg(it.colscale + c0 + e);
-                                    }
-                                    if (it.out_f32) {
-                                        float4* o = reinterpret_cast<float4*>(reinterpret_cast<float*>(it.out) + grow * 64 + c0);
-#pragma unroll
-                                        for (int e = 0; e < 4; ++e) o[e] = make_float4(v[4 * e], v[4 * e + 1], v[4 * e + 2], v[4 * e + 3]);
-                                    } else {
-                                        uint32_t w[8];
-#pragma unroll
-                                        for (int e = 0; e < 8; ++e) {
-                                            const __nv_bfloat162 h2 = __floats2bfloat162_rn(v[2 * e], v[2 * e + 1]);
-                                            w[e] = *reinterpret_cast<const uint32_t*>(&h2);
-                                        }
-                                        uint4* o = reinterpret_cast<uint4*>(reinterpret_cast<bf16*>(it.out) + grow * 64 + c0);
-                                        o[0] = make_uint4(w[0], w[1], w[2], w[3]);
-                                        o[1] = make_uint4(w[4], w[5], w[6], w[7]);
-                                    }
-                                }
-                            }
-                            fence_async_global();            // these panels are read back through TMA (async proxy) by other CTAs
-                            tc_fence_before();
-                            __syncwarp();
-                            if (lane == 0) { mbar_arrive(tempty_bar(3)); mbar_arrive(pdone_bar); }
-                            if (warp == 0) {                 // all eight warps' stores happen-before this release
-                                ok = mbar_wait(pdone_bar, use3 & 1u, err);
-                                if (lane == 0) red_release_add(it.done_ctr, 1u);
-                            }
-                            ++use3;
-                        }
+                for (int ch = 0; ch < 4; ++ch) {         // (rolled: see the update park warps)
+                    uint32_t a[16];
+                    tmem_ld16_nowait(taddr + 16u * ch, a);
+                    tmem_wait();
+                    if (rb == nrb - 1 && ch == 3) {      // accumulators are in registers: the MMAs of the next item may overwrite them
+                        tc_fence_before();
                         __syncwarp();
-                        if (lane == 0) mbar_arrive(iempty_bar(rslot));
-                        ++nr; have = false; idle = 0;
+                        if (lane == 0) mbar_arrive(tempty_bar(3));
+                    }
+                    if (!row_ok) continue;
+                    if (kind == K_SP) {              // FP32 partial [a][g] of this row panel
+                        float4* o = reinterpret_cast<float4*>(reinterpret_cast<float*>(it.out) + r * 64 + 16 * ch);
+#pragma unroll
+                        for (int e = 0; e < 4; ++e)
+                            __stcg(o + e, make_float4(__uint_as_float(a[4 * e]), __uint_as_float(a[4 * e + 1]), __uint_as_float(a[4 * e + 2]), __uint_as_float(a[4 * e + 3])));
                         continue;
                     }
+                    uint32_t w[8];
+#pragma unroll
+                    for (int e = 0; e < 8; ++e) {
+                        const float2 cs = __ldg(reinterpret_cast<const float2*>(it.colscale + 16 * ch) + e);
+                        const __nv_bfloat162 h2 = __floats2bfloat162_rn(__uint_as_float(a[2 * e]) * cs.x, __uint_as_float(a[2 * e + 1]) * cs.y);
+                        w[e] = *reinterpret_cast<const uint32_t*>(&h2);
+                    }
+                    uint4* o = reinterpret_cast<uint4*>(reinterpret_cast<bf16*>(it.out) + grow * 64 + 16 * ch);
+                    o[0] = make_uint4(w[0], w[1], w[2], w[3]);
+                    o[1] = make_uint4(w[4], w[5], w[6], w[7]);
                 }
-            } else if (ncast == nq) break;
-            if (++idle > (1u << 24)) { if (lane == 0) atomicExch(err, 5); break; }
-            if ((idle & 4095u) == 4095u && errset()) break;
-            __nanosleep(20);
+            }
+            // completion: the four warps' stores happen-before the release below (CTA barrier, then a gpu-scope release by one thread)
+            fence_async_global();            // these panels are read back through TMA (async proxy)
+            uint32_t* done_ctr = it.done_ctr;
+            const int total = it.total;
+            const float* parts = it.base32;
+            bf16* sea = reinterpret_cast<bf16*>(it.scale_inv);
+            uint32_t* sync = it.sync;
+            __syncwarp();
+            if (lane == 0) mbar_arrive(piempty_bar(rslot));
+            group_sync();
+            if (kind == K_SP) {
+                // the panel that completes the tensor's set of partials sums them in panel order (deterministic) into (S E_A)^T
+                if (tid == 0) {
+                    uint32_t old;
+                    asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(old) : "l"(done_ctr) : "memory");
+                    *s_last = old == (uint32_t)(total - 1) ? 1 : 0;
+                }
+                group_sync();
+                if (*s_last) {
+                    float acc[32];
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) acc[e] = 0.0f;
+                    for (int p = 0; p < total; ++p) {
+                        const float4* src = reinterpret_cast<const float4*>(parts + (size_t)p * 4096 + tid * 32);
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) {
+                            const float4 x = __ldcg(src + e);
+                            acc[4 * e] += x.x; acc[4 * e + 1] += x.y; acc[4 * e + 2] += x.z; acc[4 * e + 3] += x.w;
+                        }
+                    }
+                    const int a_ = (tid * 32) >> 6, g0 = (tid * 32) & 63;       // element (a, g0 + e) -> SEA[g0 + e][a]
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) sea[(g0 + e) * 64 + a_] = __float2bfloat16_rn(acc[e]);
+                    fence_async_global();
+                    group_sync();
+                    if (tid == 0) red_release_add(sync + SY_S, 1u);
+                }
+            } else if (done_ctr) {
+                if (tid == 0) red_release_add(done_ctr, 1u);
+            } else {
+                if (tid == 0) mbar_arrive(plocal_bar);          // P' of this panel is in global memory: its S partial may start
+            }
         }
+        if (tid == 0) PROF_OUT(6)
     }
+#ifdef GF8_STREAM_PROF
+    if (lane == 0 && prof) prof[16384 + blockIdx.x * 32 + warp] = 9999;
+#endif
     tc_fence_before();
     __syncthreads();
-    if (warp == 10) {
+    if (warp == W_UMMA) {
         tc_fence_after();
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(512) : "memory");
     }

@@ -4,12 +4,14 @@
 #pragma once
 #include "gf8_fast.cuh"
 #include "gf8_stream.cuh"
+#include <time.h>
 
 struct SPlan {
     std::vector<uint64_t> key;
     int nT = 0, n_p1 = 0, n_upd = 0, n_maps = 0, n_shapes = 0, grid = 0, tap = 0;
     gf8::st::STensor* d_T = nullptr;
     gf8::st::P1Item* d_p1 = nullptr;
+    gf8::st::TileEnt* d_tiles = nullptr;     // one entry per update tile, in global tile order (tile u -> CTA u mod grid)
     CUtensorMap *d_maps = nullptr, *d_tmpl = nullptr;
     int* d_shape_of = nullptr;
     const void** d_ptrs = nullptr;
@@ -27,12 +29,11 @@ struct SPlan {
 namespace {
 
 constexpr size_t S_MAX_PLANS = 16;
-constexpr long long S_GROUP_BYTES = 24ll << 20;      // gradient bytes per pass-1 group
-constexpr long long S_LEAD_BYTES = 72ll << 20;       // pass-1 may lead the update by this much gradient (L2 residency)
+constexpr long long S_LEAD_BYTES = 80ll << 20;       // pass-1 may lead the update by this much gradient (L2 residency)
 
 void splan_free(SPlan* p) {
     if (!p) return;
-    cudaFree(p->d_T); cudaFree(p->d_p1); cudaFree(p->d_maps); cudaFree(p->d_tmpl); cudaFree(p->d_shape_of);
+    cudaFree(p->d_T); cudaFree(p->d_p1); cudaFree(p->d_tiles); cudaFree(p->d_maps); cudaFree(p->d_tmpl); cudaFree(p->d_shape_of);
     cudaFree((void*)p->d_ptrs); cudaFree(p->d_sync); cudaFree(p->d_arena);
     for (int q = 0; q < 2; ++q) {
         if (p->h_ptrs[q]) cudaFreeHost((void*)p->h_ptrs[q]);
@@ -101,7 +102,7 @@ gf8_status splan_build(gf8_ctx* c, SPlan* p, const std::vector<int>& lay, bool t
     for (int i = 0; i < nT; ++i) {
         const LayerState& L = c->layers[lay[i]];
         const size_t m = L.desc.d_out, n = L.desc.d_in;
-        oPp[i] = take(m * 64 * 2); oQt[i] = take(n * 64 * 4); oQpt[i] = take(n * 64 * 2); oSEA[i] = take(64 * 64 * 2);
+        oPp[i] = take(m * 64 * 2); oQt[i] = take(((m + 255) / 256) * 16384); oQpt[i] = take(n * 64 * 2); oSEA[i] = take(64 * 64 * 2);
     }
     void* q = nullptr;
     if (cudaMalloc(&q, arena) != cudaSuccess) { cudaGetLastError(); return fail(c, GF8_ERR_NOMEM, "stream plan arena (%zu bytes)", arena); }
@@ -110,16 +111,8 @@ gf8_status splan_build(gf8_ctx* c, SPlan* p, const std::vector<int>& lay, bool t
     std::vector<CUtensorMap> tmpl;
     std::vector<int> shape_of(nT);
     std::vector<P1Item> p1;
-    std::vector<int> pend;                // tensors of the previous group: their S and Q' items follow this group's panels
-    auto flush_pending = [&]() {
-        for (int t : pend) if (T[t].useA && T[t].useG) p1.push_back({K_S, t, 0, 64});
-        for (int t : pend) if (T[t].useA && T[t].useG)
-            for (int j0 = 0; j0 < T[t].n; j0 += 256) p1.push_back({K_QP, t, j0, std::min(256, T[t].n - j0)});
-        pend.clear();
-    };
-    long long byte_pos = 0, group_bytes = 0;
-    int upd = 0;
-    std::vector<int> cur;
+    long long byte_pos = 0;
+    int upd = 0, gate_next = 0;
     for (int i = 0; i < nT && s == GF8_OK; ++i) {
         LayerState& L = c->layers[lay[i]];
         STensor& t = T[i];
@@ -128,11 +121,10 @@ gf8_status splan_build(gf8_ctx* c, SPlan* p, const std::vector<int>& lay, bool t
         t.fmt = L.desc.fmt; t.mode = tap ? M_TAP : (L.desc.scaling == GF8_SCALE_TENSOR ? M_PARK : M_BLOCK);
         t.tiles_n = (t.n + 127) / 128; t.n_tiles = ((t.m + 127) / 128) * t.tiles_n;
         t.nP = t.useA ? (t.m + 255) / 256 : 0; t.nQ = t.useG ? (t.n + 255) / 256 : 0; t.nQP = (t.useA && t.useG) ? t.nQ : 0;
-        if (t.useA && t.useG) { t.dep_idx = SY_QP; t.dep_target = t.nQP; }
-        else if (t.useA) { t.dep_idx = SY_P; t.dep_target = t.nP; }
-        else { t.dep_idx = SY_Q; t.dep_target = t.nQ; }
+        t.dep_idx = SY_QP;               // the last pass-1 stage of a tensor counts on SY_QP (Q' items; P / Q panels if one-sided)
+        t.dep_target = (t.useA && t.useG) ? t.nQP : (t.useA ? t.nP : t.nQ);
         t.upd_start = upd; upd += t.n_tiles;
-        t.Pp = (bf16*)(p->d_arena + oPp[i]); t.Qt = (float*)(p->d_arena + oQt[i]); t.Qpt = (bf16*)(p->d_arena + oQpt[i]);
+        t.Pp = (bf16*)(p->d_arena + oPp[i]); t.Spart = (float*)(p->d_arena + oQt[i]); t.Qpt = (bf16*)(p->d_arena + oQpt[i]);
         t.SEA = (bf16*)(p->d_arena + oSEA[i]);
         t.eA = L.in.e; t.eG = L.out.e;
         t.byte_pos = byte_pos;
@@ -158,22 +150,15 @@ gf8_status splan_build(gf8_ctx* c, SPlan* p, const std::vector<int>& lay, bool t
             tmpl.insert(tmpl.end(), mp, mp + 3);
         }
         shape_of[i] = f->second;
-        // pass-1 items of this tensor; a group is closed once it holds S_GROUP_BYTES of gradient
         const long long bytes = (long long)t.m * t.n * 2;
-        if (group_bytes > 0 && group_bytes + bytes > S_GROUP_BYTES) {
-            flush_pending();
-            pend.swap(cur);
-            group_bytes = 0;
-        }
-        for (int i0 = 0; t.useA && i0 < t.m; i0 += 256) p1.push_back({K_PANEL_P, i, i0, std::min(256, t.m - i0)});
-        for (int j0 = 0; t.useG && j0 < t.n; j0 += 256) p1.push_back({K_PANEL_Q, i, j0, std::min(256, t.n - j0)});
-        cur.push_back(i);
-        group_bytes += bytes; byte_pos += bytes;
+        // lead control: the last tensor that lies wholly more than S_LEAD_BYTES of gradient behind this one must be complete
+        while (gate_next < i && T[gate_next].byte_pos + (long long)T[gate_next].m * T[gate_next].n * 2 + S_LEAD_BYTES <= t.byte_pos) ++gate_next;
+        const int gate = (tap || gate_next == 0) ? -1 : gate_next - 1, gate_total = gate >= 0 ? T[gate].n_tiles : 0;
+        for (int i0 = 0; t.useA && i0 < t.m; i0 += 256) p1.push_back({K_PANEL_P, i, i0, std::min(256, t.m - i0), gate, gate_total, 0, 0});
+        for (int j0 = 0; t.useG && j0 < t.n; j0 += 256) p1.push_back({K_PANEL_Q, i, j0, std::min(256, t.n - j0), gate, gate_total, 0, 0});
+        byte_pos += bytes;
     }
     if (s != GF8_OK) return s;
-    flush_pending();
-    pend.swap(cur);
-    flush_pending();
     // dynamic maps follow the static ones
     const int n_static = (int)maps.size();
     for (int i = 0; i < nT; ++i) { T[i].map_src_p = n_static + 3 * i; T[i].map_src_q = n_static + 3 * i + 1; T[i].map_src_b = n_static + 3 * i + 2; }
@@ -181,9 +166,24 @@ gf8_status splan_build(gf8_ctx* c, SPlan* p, const std::vector<int>& lay, bool t
     p->grid = std::max(1, std::min(c->num_sms, std::max(p->n_upd, p->n_p1)));
     for (int i = 0; i < nT; ++i)
         if (T[i].mode == M_PARK && T[i].n_tiles > NPARK * p->grid) return fail(c, GF8_ERR_BAD_STATE, "stream plan: tensor too large to park");
+    std::vector<TileEnt> tiles((size_t)upd);
+    {
+        std::vector<int> tile_tensor((size_t)upd);
+        for (int i = 0; i < nT; ++i)
+            for (int k = 0; k < T[i].n_tiles; ++k) tile_tensor[(size_t)T[i].upd_start + k] = i;
+        for (int u = 0; u < upd; ++u) {
+            const STensor& t = T[tile_tensor[u]];
+            const int k = u - t.upd_start, prev = u - NPARK * p->grid;
+            TileEnt e;
+            e.tensor = tile_tensor[u]; e.tij = (k / t.tiles_n) | ((k % t.tiles_n) << 16);
+            e.old_tensor = (prev >= 0 && T[tile_tensor[prev]].mode == M_PARK) ? tile_tensor[prev] : -1;
+            e.dep_old = t.dep_target | ((e.old_tensor >= 0 ? T[e.old_tensor].n_tiles : 0) << 16);
+            tiles[u] = e;
+        }
+    }
     p->sync_bytes = ((size_t)nT * SY_WORDS + 4) * sizeof(uint32_t);
     auto dm = [&](void** out, size_t bytes) -> bool { return cudaMalloc(out, std::max<size_t>(bytes, 16)) == cudaSuccess; };
-    if (!dm((void**)&p->d_T, sizeof(STensor) * nT) || !dm((void**)&p->d_p1, sizeof(P1Item) * p1.size()) ||
+    if (!dm((void**)&p->d_T, sizeof(STensor) * nT) || !dm((void**)&p->d_tiles, sizeof(TileEnt) * tiles.size()) || !dm((void**)&p->d_p1, sizeof(P1Item) * p1.size()) ||
         !dm((void**)&p->d_maps, sizeof(CUtensorMap) * p->n_maps) || !dm((void**)&p->d_tmpl, sizeof(CUtensorMap) * tmpl.size()) ||
         !dm((void**)&p->d_shape_of, sizeof(int) * nT) || !dm((void**)&p->d_ptrs, sizeof(void*) * 3 * nT) || !dm((void**)&p->d_sync, p->sync_bytes)) {
         cudaGetLastError();
@@ -191,6 +191,7 @@ gf8_status splan_build(gf8_ctx* c, SPlan* p, const std::vector<int>& lay, bool t
     }
     for (int i = 0; i < nT; ++i) T[i].sync = p->d_sync + (size_t)i * SY_WORDS;
     CU_TRY(c, cudaMemcpy(p->d_T, T.data(), sizeof(STensor) * nT, cudaMemcpyHostToDevice));
+    if (!tiles.empty()) CU_TRY(c, cudaMemcpy(p->d_tiles, tiles.data(), sizeof(TileEnt) * tiles.size(), cudaMemcpyHostToDevice));
     if (!p1.empty()) CU_TRY(c, cudaMemcpy(p->d_p1, p1.data(), sizeof(P1Item) * p1.size(), cudaMemcpyHostToDevice));
     if (n_static) CU_TRY(c, cudaMemcpy(p->d_maps, maps.data(), sizeof(CUtensorMap) * n_static, cudaMemcpyHostToDevice));
     CU_TRY(c, cudaMemcpy(p->d_tmpl, tmpl.data(), sizeof(CUtensorMap) * tmpl.size(), cudaMemcpyHostToDevice));
@@ -253,8 +254,57 @@ gf8_status stream_run(gf8_ctx* c, const std::vector<int>& idx, const int* layers
     }
     CU_TRY(c, cudaMemsetAsync(p->d_sync, 0, p->sync_bytes, st));
     int* ctr = reinterpret_cast<int*>(p->d_sync + (size_t)p->nT * SY_WORDS);
-    stream_kernel<<<p->grid, S_THREADS, S_BYTES, st>>>(p->d_T, p->nT, p->d_p1, p->n_p1, p->n_upd, p->d_maps, ctr, c->d_err, S_LEAD_BYTES, p->tap);
+    stream_kernel<<<p->grid, S_THREADS, S_BYTES, st>>>(p->d_T, p->nT, p->d_p1, p->n_p1, p->n_upd, p->d_tiles, p->d_sync, p->d_maps, ctr, c->d_err, p->tap, c->d_prof);
     LAUNCH_CHECK(c);
+#ifdef GF8_STREAM_PROF
+    if (getenv("GF8_HEARTBEAT")) {   // debug builds only: where every warp is waiting 3 s after the launch (hang hunting)
+        cudaStream_t s2; cudaStreamCreateWithFlags(&s2, cudaStreamNonBlocking);
+        std::vector<long long> hb(32 * 160);
+        struct timespec ts = {3, 0}; nanosleep(&ts, nullptr);
+        cudaMemcpyAsync(hb.data(), c->d_prof + 16384, hb.size() * sizeof(long long), cudaMemcpyDeviceToHost, s2);
+        cudaStreamSynchronize(s2);
+        for (int b = 0; b < p->grid; ++b) {
+            fprintf(stderr, "cta %3d:", b);
+            for (int w = 0; w < 26; ++w) fprintf(stderr, " %lld", hb[(size_t)b * 32 + w]);
+            fprintf(stderr, "\n");
+        }
+    }
+    {   // debug builds only: average per-role wait profile of this launch (serialises the stream)
+        std::vector<long long> h((size_t)p->grid * 64);
+        cudaStreamSynchronize(st);
+        cudaMemcpy(h.data(), c->d_prof, h.size() * sizeof(long long), cudaMemcpyDeviceToHost);
+        if (getenv("GF8_TRACE")) {
+            std::vector<long long> ev(4096);
+            cudaMemcpy(ev.data(), c->d_prof + 20480, ev.size() * sizeof(long long), cudaMemcpyDeviceToHost);
+            for (int cta = 0; cta < 2; ++cta) {
+                const long long t0 = ev[cta * 2048 + 0];
+                fprintf(stderr, "trace cta %d: tile | ready mma0 mma1 park0 park1 seen rel done cast0 cast1 (ns from first ready)\n", cta ? 77 : 0);
+                for (int t = 0; t < 40; ++t) {
+                    fprintf(stderr, "  %2d |", t);
+                    for (int code : {0, 2, 3, 4, 5, 6, 7, 8, 9, 10}) fprintf(stderr, " %7lld", ev[cta * 2048 + code * 48 + t] - t0);
+                    fprintf(stderr, "\n");
+                }
+            }
+        }
+        if (getenv("GF8_PERCTA")) {      // per-CTA: sready wait of the epilogue (role 3, slot 0) against pass-1 activity (role 4 total - waits; role 5 full wait)
+            for (int b = 0; b < p->grid; ++b) {
+                const long long* e = &h[((size_t)b * 8 + 3) * 8];
+                const long long* pp = &h[((size_t)b * 8 + 4) * 8];
+                const long long* pm = &h[((size_t)b * 8 + 5) * 8];
+                const long long* um = &h[((size_t)b * 8 + 2) * 8];
+                fprintf(stderr, "cta %3d: epi sready-wait %8lld ifull %8lld tfull %8lld | u-mma tempty %8lld full %8lld | p-prod gate %8lld dep %8lld pempty %8lld slack %8lld | p-mma idle %8lld\n", b, e[0], e[1], e[2],
+                        um[1], um[3], pp[1], pp[2], pp[3], pp[5], pm[0]);
+            }
+        }
+        const char* roles[7] = {"u-sched", "u-load", "u-mma", "u-epi0", "p-prod", "p-mma", "p-epi"};
+        for (int r = 0; r < 7; ++r) {
+            double a[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+            for (int b = 0; b < p->grid; ++b) for (int q = 0; q < 8; ++q) a[q] += (double)h[((size_t)b * 8 + r) * 8 + q] / p->grid;
+            fprintf(stderr, "stream prof %-7s %9.0f %9.0f %9.0f %9.0f %9.0f %9.0f %9.0f | total %9.0f cycles (avg / CTA)\n", roles[r], a[0], a[1], a[2], a[3],
+                    a[4], a[5], a[6], a[7]);
+        }
+    }
+#endif
     return GF8_OK;
 }
 
