@@ -728,6 +728,7 @@ gf8_status gf8_create(gf8_ctx** out, int device, const gf8_layer_desc* layers, i
     // operand carried as hi + lo (16 mantissa bits): transform within 1e-5 of the oracle (gate G2's 1e-4 tier) at ~3x the
     // MMAs, but a few 1e-4 of FP8 codes still flip, so the strict code-level gates (G3, G5's BF16 ulp) keep the SIMT path.
     c->tc_exact = precision == GF8_PREC_EXACT && getenv("GF8_EXACT_TC") != nullptr;
+    c->use_stream = getenv("GF8_STREAM") != nullptr;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) c->num_sms = prop.multiProcessorCount;
     c->layers.resize(n_layers);

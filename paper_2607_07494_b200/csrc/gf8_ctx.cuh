@@ -96,6 +96,7 @@ struct gf8_ctx {
     std::map<std::vector<uint64_t>, struct Plan*> fac_plans;   // factor-GEMM plans (keyed by the sample buffer)
     std::vector<struct SPlan*> splans;                          // streaming-engine plans (keyed by the layer list of a call)
     bool stream_attr_set = false;
+    bool use_stream = false;         // streaming engine (gf8_stream.cuh) instead of the staged item engine for the shapes it takes
     int* d_err = nullptr;
     float* fac_alpha = nullptr;      // 128 copies of the factor GEMM's scale (its epilogue's column multipliers)
     float* fac_tmp = nullptr;        // d x d scratch of the EMA form of the factor update

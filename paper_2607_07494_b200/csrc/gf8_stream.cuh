@@ -8,15 +8,13 @@
 //                                (S E_A)^T = sum_i P.(i)^T U_G(i)   partial per row panel, summed in panel order (K_SP)
 //                                Q.^T = (Q^T + U_A (S E_A)^T) E_G   last K-step of the column panel item
 //                                W~  = Wg + [P' | U_G] [U_A | Q'^T]^T   128 x 128 tiles      (K_UPD)
-// Work hand-out: the "pass-1" items (P, Q, S, Q') sit in one list in tensor-group order and are claimed
-// dynamically (atomic counter); the update tiles are assigned statically (tile u -> CTA u mod grid) so that the
-// FP32 W~ tile can stay PARKED in TMEM (3 of the 4 accumulator slots) until its tensor's amax is complete
-// (release / acquire counters in global memory), and is then scaled, cast and stored without a second pass.
-// A CTA's scheduler warp prefers its next update tile when that tile's tensor is ready, else claims pass-1 work,
-// bounded by a lead of `lead_bytes` of gradient so the update's re-read of the gradient hits L2.
-// Deadlock freedom: every wait is on work that is earlier in list / tile order and already owned by a resident
-// CTA (grid <= #SMs, 1 CTA / SM); a CTA never holds more than three parked tiles of incomplete tensors, and
-// host code only sends tensors with <= 3 * grid tiles here.
+// Work hand-out: both pipelines claim their work from a list by atomic counter (list order is start order).  Pass-1 items run in
+// tensor order.  The update list holds, per tensor with a per-tensor scale, its tiles TWICE: pass A (amax only) and, a few hundred
+// tiles later in the list, pass B (recompute, scale, cast, store) -- a tile depends only on counters of earlier list entries, so
+// no CTA ever waits on another CTA's progress through its own tiles (an earlier version parked the FP32 tile in TMEM across
+// the tensor amax: with 3 parking slots per SM every tensor became a grid-wide barrier and tail latencies set the pace).
+// Per-block scaling and the FP32 tap are single-pass.  A lead limit keeps pass-1 at most `lead` bytes of gradient ahead of the
+// update, so the update's re-reads of the gradient hit L2.
 //
 // Two pipelines share every SM, so a long panel item never delays the CTA's update tiles (whose tensors complete in
 // lock step across CTAs) and the HBM-bound streaming of new gradients overlaps the issue-bound update epilogues:
@@ -38,9 +36,10 @@ constexpr int NB = 2;                       // streamed base tiles in flight
 constexpr int BASE_BYTES = 32768;           // 128 x 128 BF16 (two 64-column halves)
 constexpr int RS = 8;                       // update item ring entries
 constexpr int PRS = 4;                      // pass-1 item ring entries
+constexpr int UCHUNK = 4;                   // update tiles per claim
 constexpr int NPARK = 3;                    // TMEM slots 0..2: update tiles (parked); slot 3: pass-1 items
 constexpr int S_DATA = NS * STG_BYTES + US * USTG_BYTES + NB * BASE_BYTES;     // 208 KB
-constexpr int S_MISC = 3072;
+constexpr int S_MISC = 4096;
 constexpr int S_BYTES = S_DATA + S_MISC;
 constexpr int S_THREADS = 832;
 // warp roles: the spinning / issuing roles take the low warp ids, the arithmetic-heavy epilogues the high ones
@@ -48,9 +47,11 @@ constexpr int W_USCHED = 0, W_ULOAD = 1, W_UMMA = 2, W_SYNC = 3, W_PPROD = 4, W_
 static_assert(S_BYTES <= 227 * 1024, "shared memory budget");
 
 enum Kind : int32_t { K_END = 0, K_PANEL_P = 1, K_PANEL_Q = 2, K_SP = 3, K_UPD = 5 };
-enum Mode : int32_t { M_PARK = 0, M_BLOCK = 1, M_TAP = 2 };
+// STensor.mode: M_AMAX (per-tensor scale: two passes over the update tiles), M_BLOCK, M_TAP; RItem.mode also M_CAST (pass B)
+enum Mode : int32_t { M_AMAX = 0, M_BLOCK = 1, M_TAP = 2, M_CAST = 3 };
+enum Pass : int32_t { P_AMAX = 0, P_CAST = 1, P_SINGLE = 2 };
 // words of a tensor's sync block (zeroed before every launch)
-enum Sync : int32_t { SY_AMAX = 0, SY_P = 1, SY_Q = 2, SY_S = 3, SY_QP = 4, SY_TILES = 5, SY_WORDS = 8 };
+enum Sync : int32_t { SY_AMAX = 0, SY_P = 1, SY_Q = 2, SY_S = 3, SY_QP = 4, SY_TILES = 5, SY_DONE = 6, SY_WORDS = 8 };
 
 // One (tensor, rank) problem of a batched call.  Static part written at plan build; `src`-maps, codes, scale_inv,
 // tap are patched per call by patch_kernel.
@@ -74,9 +75,8 @@ static_assert(sizeof(STensor) == 256, "tensor record size");
 // Pass-1 item.  gate_tensor >= 0: a panel may start only when that (earlier) tensor's update is complete (gate_total tiles
 // parked), which keeps the gradient bytes between the two pipelines' frontiers within L2 (lead control).
 struct __align__(16) P1Item { int32_t kind, tensor, r0, rows, gate_tensor, gate_total, pad0, pad1; };
-// Update tile u (CTA u mod grid runs it): its tensor, tile coordinates (ti | tj << 16), the count its tensor's SY_QP word must
-// reach (low 16 bits) and the tile count of the tensor whose parked tile held this TMEM slot before (high 16 bits; tile u - 3 grid)
-struct __align__(16) TileEnt { int32_t tensor, tij, dep_old, old_tensor; };
+// Entry of the update list: tensor, tile coordinates (ti | tj << 16) and pass (P_AMAX / P_CAST / P_SINGLE).
+struct __align__(16) TileEnt { int32_t tensor, tij, pass, pad; };
 
 // What a role needs to know about an item (shared-memory ring entry, written by the scheduler warp).
 struct __align__(16) RItem {
@@ -84,13 +84,12 @@ struct __align__(16) RItem {
     int32_t rows, cols, ksteps, mode;
     int32_t mapA0, mapA1, mapB0, mapB1;
     int32_t fmt, ld, nrb, bslot;
-    int32_t total, first, n_cols_tile, out_f32;      // total: tiles of the tensor; first: this tile writes scale_inv
+    int32_t total, first; float scale; int32_t out_f32;   // scale: pass-B tiles (from the tensor's amax); first: fused Q' step (pass-1)
     void* out; const float* base32; const float* colscale; uint32_t* sync;
     float* scale_inv; uint32_t* done_ctr;
 };
 static_assert(sizeof(RItem) == 128, "ring entry size");
 
-struct Parked { uint32_t* sync; float* scale_inv; uint8_t* out; int32_t ld, row0, col0, rows, cols, fmt, total, first, local, pad; };
 
 __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, uint32_t bar) {
     asm volatile(
@@ -228,20 +227,16 @@ stream_kernel(const STensor* __restrict__ T, int nT, const P1Item* __restrict__ 
     auto tempty_bar = [&](uint32_t s) { return bars + 8u * (12 + s); };         // [4]
     auto ifull_bar = [&](uint32_t s) { return bars + 8u * (16 + s); };          // [RS]
     auto iempty_bar = [&](uint32_t s) { return bars + 8u * (24 + s); };         // [RS]
-    auto parked_bar = [&](uint32_t s) { return bars + 8u * (32 + s); };         // [NPARK]
-    auto sready_bar = [&](uint32_t s) { return bars + 8u * (35 + s); };         // [NPARK]
     // pass-1 pipeline barriers
     auto pfull_bar = [&](uint32_t s) { return bars + 8u * (38 + s); };          // [NS]
     auto pempty_bar = [&](uint32_t s) { return bars + 8u * (40 + s); };         // [NS]
     auto pifull_bar = [&](uint32_t s) { return bars + 8u * (42 + s); };         // [PRS]
     auto piempty_bar = [&](uint32_t s) { return bars + 8u * (46 + s); };        // [PRS]
     const uint32_t plocal_bar = bars + 8u * 50, drain_bar0 = bars + 8u * 51, drain_bar1 = bars + 8u * 52;
-    uint32_t* s_tmem = reinterpret_cast<uint32_t*>(misc + 432);
-    float* s_scale = reinterpret_cast<float*>(misc + 448);               // [3]
-    volatile int* s_slack = reinterpret_cast<volatile int*>(misc + 472);  // [0] cast warps wait for a tensor, [1] scheduler waits for readiness / is done
-    volatile int* s_nupd = reinterpret_cast<volatile int*>(misc + 464);  // parked tiles of this CTA (-1: not known yet)
-    uint32_t* s_wmax = reinterpret_cast<uint32_t*>(misc + 2832);         // [3][16]
-    Parked* s_park = reinterpret_cast<Parked*>(misc + 576);              // [3] x 64 B
+    auto amax_bar = [&](uint32_t s) { return bars + 8u * (53 + s); };           // [RS]
+    uint32_t* s_tmem = reinterpret_cast<uint32_t*>(misc + 496);
+    uint32_t* s_wmax = reinterpret_cast<uint32_t*>(misc + 2832);         // [RS][16] warp maxima of pass-A tiles, per ring entry
+    uint32_t* s_wblk = reinterpret_cast<uint32_t*>(misc + 3344);         // [2][16] warp maxima of per-block-scaled tiles
     RItem* s_items = reinterpret_cast<RItem*>(misc + 768);               // [RS] x 128 B   -> 1792
     RItem* s_pitems = reinterpret_cast<RItem*>(misc + 1792);             // [PRS] x 128 B  -> 2304
     STensor* s_cur = reinterpret_cast<STensor*>(misc + 2304);            // tensor of the next update tile   -> 2560
@@ -253,12 +248,10 @@ stream_kernel(const STensor* __restrict__ T, int nT, const P1Item* __restrict__ 
         for (int s = 0; s < NB; ++s) { mbar_init(bfull_bar(s), 1); mbar_init(bempty_bar(s), 16); }
         for (int s = 0; s < 3; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), 16); }
         mbar_init(tfull_bar(3), 1); mbar_init(tempty_bar(3), 4);
-        for (int s = 0; s < RS; ++s) { mbar_init(ifull_bar(s), 1); mbar_init(iempty_bar(s), 18); }
-        for (int s = 0; s < NPARK; ++s) { mbar_init(parked_bar(s), 16); mbar_init(sready_bar(s), 1); }
+        for (int s = 0; s < RS; ++s) { mbar_init(ifull_bar(s), 1); mbar_init(iempty_bar(s), 19); mbar_init(amax_bar(s), 16); }
         for (int s = 0; s < NS; ++s) { mbar_init(pfull_bar(s), 1); mbar_init(pempty_bar(s), 1); }
         for (int s = 0; s < PRS; ++s) { mbar_init(pifull_bar(s), 1); mbar_init(piempty_bar(s), 5); }
         mbar_init(plocal_bar, 1); mbar_init(drain_bar0, 1); mbar_init(drain_bar1, 1);
-        *s_nupd = -1; s_slack[0] = 0; s_slack[1] = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (warp == W_UMMA) {
@@ -307,18 +300,13 @@ stream_kernel(const STensor* __restrict__ T, int nT, const P1Item* __restrict__ 
     };
 
     if (warp == W_USCHED) {
-        // ===== update scheduler (converged warp): my next tile (static: tile u -> CTA u mod grid) once its tensor is ready =====
+        // ===== update scheduler (converged warp): claims the next tile of the update list (atomic counter: list order is start
+        // order), waits until its tensor allows it, writes the ring entry and streams the tile's base =====
         PROF_DECL
         uint32_t nring = 0, q = 0;
-        int u = blockIdx.x, cur_t = -1, n_parked = 0;
+        int cur_t = -1, cur_pass = -1;
+        float cur_scale = 1.0f, cur_si = 1.0f;
         bool ok = true;
-        TileEnt ent = {0, 0, 0, 0};
-        if (u < n_upd && lane == 0) ent = tiles[u];
-        auto bcast_ent = [&]() {
-            ent.tensor = __shfl_sync(0xFFFFFFFFu, ent.tensor, 0); ent.tij = __shfl_sync(0xFFFFFFFFu, ent.tij, 0);
-            ent.dep_old = __shfl_sync(0xFFFFFFFFu, ent.dep_old, 0); ent.old_tensor = __shfl_sync(0xFFFFFFFFu, ent.old_tensor, 0);
-        };
-        bcast_ent();
         auto push = [&](const RItem& it) -> bool {               // lane 0 writes the entry
             const uint32_t slot = nring % RS, ph = (nring / RS) & 1u;
             bool w_ok;
@@ -335,39 +323,60 @@ stream_kernel(const STensor* __restrict__ T, int nT, const P1Item* __restrict__ 
             ++nring;
             return true;
         };
-        while (ok && u < n_upd) {
-            if (cur_t != ent.tensor) { cur_t = ent.tensor; PROF(4, load_tensor(s_cur, cur_t)); }
-            // lane 0: my tile's tensor is ready (Q' / P' complete); lane 1: the tile that held this TMEM slot (3 back) belongs to
-            // a complete tensor, so its cast is under way and the slot frees without waiting on other CTAs
-            for (uint32_t spin = 0;; ++spin) {
-                uint32_t v = 0xFFFFFFFFu;
-                const long long _t0 = clock64();
-                if (lane == 0 && (ent.dep_old & 0xFFFF)) v = ld_relaxed(sync_base + (size_t)ent.tensor * SY_WORDS + SY_QP);
-                if (lane == 1 && ent.old_tensor >= 0) v = ld_relaxed(sync_base + (size_t)ent.old_tensor * SY_WORDS + SY_TILES);
-                const uint32_t v0 = __shfl_sync(0xFFFFFFFFu, v, 0), v1 = __shfl_sync(0xFFFFFFFFu, v, 1);
-                const bool rdy = v0 >= (uint32_t)(ent.dep_old & 0xFFFF), oldok = true || v1 >= (uint32_t)(ent.dep_old >> 16);
-                if (rdy && oldok) { if (lane == 0) s_slack[1] = 0; break; }
-                if (lane == 0) s_slack[1] = 1;
-                if (spin > (1u << 24) || ((spin & 255u) == 255u && errset())) { if (lane == 0) atomicExch(err, 6); ok = false; break; }
-#ifdef GF8_STREAM_PROF
-                pf[rdy ? 2 : 1] += clock64() - _t0;
-#endif
-            }
-            if (!ok) break;
-            if (lane == 0) EV(0, q);
+        // Tiles are claimed UCHUNK at a time (consecutive list entries: mostly one row block of one tensor and pass), and the
+        // next chunk's claim and entries are fetched while this chunk is issued, so the scheduler's round trips to L2 (claim,
+        // entries, tensor record, counter poll, amax) are paid once per chunk and off the critical path.
+        int u_next = 0;
+        TileEnt e_next = {0, 0, 0, 0};
+        auto claim = [&]() {                       // lanes 0..UCHUNK-1 end up with their entry of the next chunk
+            int u = 0;
+            if (lane == 0) u = atomicAdd(ctr + 1, UCHUNK);
+            u_next = __shfl_sync(0xFFFFFFFFu, u, 0);
+            if (lane < UCHUNK && u_next + lane < n_upd) e_next = tiles[u_next + lane];
+        };
+        claim();
+        while (ok && u_next < n_upd) {
+            const int u0 = u_next;
+            const TileEnt e_mine = e_next;
+            claim();                               // (in flight while this chunk is issued)
+          for (int ci = 0; ci < UCHUNK && ok && u0 + ci < n_upd; ++ci) {
+            TileEnt ent;
+            ent.tensor = __shfl_sync(0xFFFFFFFFu, e_mine.tensor, ci); ent.tij = __shfl_sync(0xFFFFFFFFu, e_mine.tij, ci);
+            ent.pass = __shfl_sync(0xFFFFFFFFu, e_mine.pass, ci);
+            const bool new_t = cur_t != ent.tensor;
+            if (new_t) { cur_t = ent.tensor; cur_pass = -1; PROF(4, load_tensor(s_cur, cur_t)); }
             const STensor& t = *s_cur;
+            // pass A / single-pass tiles wait for the tensor's Q' (or P') panels; pass B tiles for the tensor's amax (all A tiles counted)
+            if (cur_pass != ent.pass) {            // (checked once per tensor and pass: the counters only grow)
+                if (ent.pass == P_CAST) { PROF(2, ok = poll_ge(t.sync + SY_TILES, (uint32_t)t.n_tiles)); }
+                else if (t.dep_target) { PROF(1, ok = poll_ge(t.sync + SY_QP, (uint32_t)t.dep_target)); }
+                if (!ok) break;
+                cur_pass = ent.pass;
+                cur_scale = 1.0f;
+                if (ent.pass == P_CAST) {
+                    // (the count that poll_ge saw carries a data dependency on every tile's amax atomic: the maximum is final)
+                    uint32_t bits = 0;
+                    if (lane == 0) bits = *reinterpret_cast<volatile uint32_t*>(t.sync + SY_AMAX);
+                    bits = __shfl_sync(0xFFFFFFFFu, bits, 0);
+                    scales_from_amax(bits, t.fmt == 0 ? 448.0f : 57344.0f, cur_scale, cur_si);
+                }
+            }
+            if (lane == 0) EV(0, q);
             const int ti = ent.tij & 0xFFFF, tj = ent.tij >> 16;
             RItem it;
             it.kind = K_UPD; it.slot = (int)(q % NPARK); it.r0 = ti * 128; it.c0 = tj * 128;
             it.rows = min(128, t.m - it.r0); it.cols = min(128, t.n - it.c0);
-            it.ksteps = (t.useA ? 1 : 0) + (t.useG ? 1 : 0); it.mode = t.mode;
+            it.ksteps = (t.useA ? 1 : 0) + (t.useG ? 1 : 0);
+            it.mode = ent.pass == P_AMAX ? M_AMAX : (ent.pass == P_CAST ? M_CAST : t.mode);
             it.mapA0 = t.useA ? t.map_Pp128 : t.map_UG128; it.mapB0 = t.useA ? t.map_UA128 : t.map_Qpt128;
             it.mapA1 = t.map_UG128; it.mapB1 = t.map_Qpt128;
             it.fmt = t.fmt; it.ld = t.n; it.nrb = 1; it.bslot = (int)(q % NB);
-            it.total = t.n_tiles; it.first = (ti | tj) == 0 ? 1 : 0; it.n_cols_tile = 128; it.out_f32 = 0;
+            it.total = t.n_tiles; it.first = 0; it.out_f32 = 0;
             it.out = t.mode == M_TAP ? (void*)t.tap : (void*)t.codes; it.base32 = nullptr; it.colscale = nullptr; it.sync = t.sync;
             it.scale_inv = t.mode == M_BLOCK ? t.scale_inv + (size_t)ti * t.tiles_n + tj : t.scale_inv;
             it.done_ctr = nullptr;
+            it.scale = cur_scale;
+            if (ent.pass == P_CAST && (ti | tj) == 0 && lane == 0) *t.scale_inv = cur_si;
             if (!(ok = push(it))) break;
             // base tile: 128 rows x 128 columns of the gradient (two 64-column halves) in one 3-D box
             const uint32_t bs = q % NB, bph = (q / NB) & 1u;
@@ -379,12 +388,10 @@ stream_kernel(const STensor* __restrict__ T, int nT, const P1Item* __restrict__ 
                 mbar_expect_tx(bfull_bar(bs), BASE_BYTES);
                 tma_load_3d(base0 + bs * BASE_BYTES, mp, 0, it.r0, tj * 2, bfull_bar(bs));
             }
-            if (t.mode != M_TAP) ++n_parked;
-            u += (int)gridDim.x; ++q;
-            if (u < n_upd && lane == 0) ent = tiles[u];
-            bcast_ent();
+            ++q;
+          }
         }
-        if (lane == 0) { PROF_OUT(0) *s_nupd = n_parked; s_slack[1] = 1; }      // (no update tiles left: pass-1 work is welcome)
+        if (lane == 0) PROF_OUT(0)
         __syncwarp();
         RItem e;
         e.kind = K_END;
@@ -472,137 +479,67 @@ stream_kernel(const STensor* __restrict__ T, int nT, const P1Item* __restrict__ 
         }
     }
     else if (warp == W_SYNC) {
-        // ===== grid-level sync (lanes 0..2, one per parking slot): tile parked -> tensor counter; tensor complete -> scale =====
-        if (lane < NPARK) {
-            for (uint32_t k = 0;; ++k) {
-                bool stop = false;
-                for (uint32_t spin = 0; !mbar_test(parked_bar(lane), k & 1u); ++spin) {      // (no nanosleep: its granularity is > 1 us here)
-                    const int tot = *s_nupd;
-                    if ((tot >= 0 && (int)(k * NPARK + lane) >= tot) || ((spin & 1023u) == 1023u && errset())) { stop = true; break; }
-                }
-                if (stop) break;
-                EV(6, k * NPARK + lane);
-                const Parked pk = s_park[lane];
-                uint32_t mx = 0;
+        // ===== amax publisher (lane 0, follows the item ring): for a pass-A tile, the maximum of the 16 epilogue warps' maxima goes
+        // to the tensor's amax word and then the tile is counted; pass-B tiles start once the count is complete.  It has a warp of
+        // its own because the atomic's round trip to L2 would otherwise hold up an epilogue warp.
+        if (lane == 0) {
+            uint32_t par_mask = 0;                           // phase parity of each ring slot's amax barrier (only pass-A tiles use it)
+            for (uint32_t n = 0;; ++n) {
+                const uint32_t rslot = n % RS;
+                if (!mw(__LINE__, ifull_bar(rslot), (n / RS) & 1u, err)) break;
+                const RItem& it = s_items[rslot];
+                if (it.kind == K_END) break;
+                if (it.mode == M_AMAX) {
+                    uint32_t* sync = it.sync;
+                    if (!mw(__LINE__, amax_bar(rslot), (par_mask >> rslot) & 1u, err)) break;
+                    par_mask ^= 1u << rslot;
+                    uint32_t mx = 0;
 #pragma unroll
-                for (int w = 0; w < 16; ++w) mx = max(mx, s_wmax[lane * 16 + w]);
-                float scale, si;
-                const float fmax = pk.fmt == 0 ? 448.0f : 57344.0f;
-                if (pk.local) {
-                    scales_from_amax(mx, fmax, scale, si);
-                    *pk.scale_inv = si;
-                    red_release_add(pk.sync + SY_TILES, 1u);          // (lead control of the pass-1 pipeline counts tiles)
-                } else {
+                    for (int w = 0; w < 16; ++w) mx = max(mx, s_wmax[rslot * 16 + w]);
+                    mbar_arrive(iempty_bar(rslot));
                     // the tile's amax reaches L2 (an atomic WITH return has been performed when its value arrives) before the tile is
                     // counted: the count carries a data dependency on the returned value instead of a (slow) gpu-scope release fence
-                    const uint32_t old = atomicMax(pk.sync + SY_AMAX, mx);
-                    asm volatile("red.relaxed.gpu.global.add.u32 [%0], %1;" ::"l"(pk.sync + SY_TILES), "r"(1u + (old & 0u)) : "memory");
-                    EV(7, k * NPARK + lane);
-                    bool bad = false;
-                    for (uint32_t spin = 0; ld_relaxed(pk.sync + SY_TILES) < (uint32_t)pk.total; ++spin) {
-                        if (spin > (1u << 24) || ((spin & 255u) == 255u && errset())) { bad = true; break; }
-                    }
-                    if (bad) { atomicExch(err, 2); break; }
-                    scales_from_amax(*reinterpret_cast<volatile uint32_t*>(pk.sync + SY_AMAX), fmax, scale, si);
-                    if (pk.first) *pk.scale_inv = si;
+                    const uint32_t old = atomicMax(sync + SY_AMAX, mx);
+                    asm volatile("red.relaxed.gpu.global.add.u32 [%0], %1;" ::"l"(sync + SY_TILES), "r"(1u + (old & 0u)) : "memory");
+                } else {
+                    mbar_arrive(iempty_bar(rslot));
                 }
-                s_scale[lane] = scale;
-                mbar_arrive(sready_bar(lane));
-                EV(8, k * NPARK + lane);
             }
         }
     } else if (warp >= W_UEPI) {
-        // ===== update epilogue warps (16): warp w reaches TMEM lanes 32 (w & 3) .. +31 and takes the 32-column quarter (w - W_UEPI) >> 2 of
-        // the tile, so each phase is ONE TMEM round trip.  Per tile, in ring order: cast the tile that held this TMEM slot before
-        // (tile q - 3: its scale arrives when its tensor is complete), then park this one (W~ = base + accumulator, running amax, FP32
-        // tile back into its TMEM slot).  The order is forced -- the MMAs of tile q cannot run before tile q - 3 has left the slot -- so
-        // every wait is a plain blocking wait.
+        // ===== update epilogue warps (16): warp w reaches TMEM lanes 32 (w & 3) .. +31 and takes the 32-column quarter (w - W_UEPI) >> 2
+        // of the tile, so a tile is ONE TMEM round trip per warp.  W~ = base + accumulator, then by mode: running amax (pass A), scale +
+        // FP8 cast + store (pass B), both with a CTA-level maximum in between (per-128x128-block scaling), or the FP32 tap =====
         const int q4 = warp & 3, cq = (warp - W_UEPI) >> 2, ew = warp - W_UEPI;
         const int r = q4 * 32 + lane;                           // accumulator row of this thread
         const uint32_t lane_off = ((uint32_t)(q4 * 32) << 16) + 32u * (uint32_t)cq;
         bool ok = true;
+        uint32_t nblk = 0;
         PROF_DECL
-        auto cast_tile = [&](uint32_t k) -> bool {              // tile k of this CTA (ordinal): scale, FP8 cast, store, free the slot
-            const uint32_t slot = k % NPARK;
-            bool w_ok;
-            if (ew == 0 && lane == 0 && !mbar_test(sready_bar(slot), (k / NPARK) & 1u)) s_slack[0] = 1;   // this CTA is ahead of the grid
-            PROF(0, w_ok = mw(__LINE__, sready_bar(slot), (k / NPARK) & 1u, err));
-            if (!w_ok) return false;
-            if (ew == 0 && lane == 0) { s_slack[0] = 0; EV(9, k); }
-            const Parked pk = s_park[slot];
-            const float scale = s_scale[slot];
-            uint32_t a[32];
-            tmem_ld32_nowait(tmem_base + slot * 128u + lane_off, a);
-            tmem_wait();
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(tempty_bar(slot));        // (the tile is in registers: its slot may take the next accumulator)
-            uint4 cd[2];
-            uint32_t* cw = reinterpret_cast<uint32_t*>(cd);
-            if (pk.fmt == 0) {
-#pragma unroll
-                for (int j = 0; j < 8; ++j)
-                    cw[j] = cast4<0>(__uint_as_float(a[4 * j]), __uint_as_float(a[4 * j + 1]), __uint_as_float(a[4 * j + 2]), __uint_as_float(a[4 * j + 3]), scale);
-            } else {
-#pragma unroll
-                for (int j = 0; j < 8; ++j)
-                    cw[j] = cast4<1>(__uint_as_float(a[4 * j]), __uint_as_float(a[4 * j + 1]), __uint_as_float(a[4 * j + 2]), __uint_as_float(a[4 * j + 3]), scale);
-            }
-            if (r < pk.rows) {
-                uint8_t* orow = pk.out + (int64_t)(pk.row0 + r) * pk.ld + pk.col0 + 32 * cq;
-#pragma unroll
-                for (int h = 0; h < 2; ++h)
-                    if (32 * cq + 16 * h < pk.cols) *reinterpret_cast<uint4*>(orow + 16 * h) = cd[h];
-            }
-            if (ew == 0 && lane == 0) EV(10, k);
-            return true;
-        };
-        uint32_t nq = 0, ncast = 0, npark = 0, idle = 0;
-        bool have = false, done = false;
-        for (;;) {
-            // one shared-memory round trip per look: lane 0 the oldest parked tile's scale, lane 1 the next ring entry, lanes 2 / 3
-            // the next tile's accumulator / base tile.  Casting comes first: it frees a TMEM slot for the MMAs of a later tile.
-            uint32_t hit = 0;
-            if (lane < 4) {
-                uint32_t bar, par;
-                bool want;
-                if (lane == 0) { want = ncast < npark; bar = sready_bar(ncast % NPARK); par = (ncast / NPARK) & 1u; }
-                else if (lane == 1) { want = !done && !have; bar = ifull_bar(nq % RS); par = (nq / RS) & 1u; }
-                else if (lane == 2) { want = !done; bar = tfull_bar(nq % NPARK); par = (nq / NPARK) & 1u; }
-                else { want = !done; bar = bfull_bar(nq % NB); par = (nq / NB) & 1u; }
-                hit = want && mbar_test(bar, par) ? 1u : 0u;
-            }
-            const uint32_t mask = __ballot_sync(0xFFFFFFFFu, hit != 0);
-            if (mask & 1u) { if (!(ok = cast_tile(ncast))) break; ++ncast; idle = 0; continue; }
-            if ((mask & 2u) && !have) {
-                have = true;
-                if (s_items[nq % RS].kind == K_END) { done = true; have = false; }
-            }
-            if (!(have && (mask & 12u) == 12u)) {
-                if (done && ncast == npark) break;
-                if (++idle > (1u << 22) || ((idle & 1023u) == 1023u && errset())) { if (lane == 0) atomicExch(err, 5); ok = false; break; }
-                // nothing to do yet: a short sleep on the event that usually comes first
-                if (lane == 0) {
-                    if (ncast < npark) mbar_nap(sready_bar(ncast % NPARK), (ncast / NPARK) & 1u);
-                    else if (!done) mbar_nap(have ? tfull_bar(nq % NPARK) : ifull_bar(nq % RS), have ? (nq / NPARK) & 1u : (nq / RS) & 1u);
-                }
-                __syncwarp();
-                continue;
-            }
-            idle = 0;
+        for (uint32_t nq = 0; ok; ++nq) {
             const uint32_t rslot = nq % RS, slot = nq % NPARK, bs = nq % NB;
+            PROF(0, ok = mw(__LINE__, ifull_bar(rslot), (nq / RS) & 1u, err));
+            if (!ok) break;
             const RItem& it = s_items[rslot];
+            if (it.kind == K_END) break;
             const int mode = it.mode;
+            PROF(1, ok = mw(__LINE__, tfull_bar(slot), (nq / NPARK) & 1u, err) && mw(__LINE__, bfull_bar(bs), (nq / NB) & 1u, err));
+            if (!ok) break;
+#ifdef GF8_STREAM_PROF
+            const long long _tw = clock64();
+#endif
             tc_fence_after();
             if (ew == 0 && lane == 0) EV(4, nq);
-            const uint32_t taddr = tmem_base + slot * 128u + lane_off;
             const uint32_t brow = base0 + bs * BASE_BYTES + (uint32_t)(cq >> 1) * 16384u + (uint32_t)r * 128u;
             uint32_t a[32];
-            tmem_ld32_nowait(taddr, a);
+            tmem_ld32_nowait(tmem_base + slot * 128u + lane_off, a);
             uint4 b[4];
 #pragma unroll
             for (int j = 0; j < 4; ++j) b[j] = lds128(brow + (((uint32_t)(4 * (cq & 1) + j) ^ (uint32_t)(r & 7)) << 4));
             tmem_wait();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) { mbar_arrive(tempty_bar(slot)); mbar_arrive(bempty_bar(bs)); }     // accumulator and base are in registers
             float* v = reinterpret_cast<float*>(a);
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
@@ -611,41 +548,63 @@ stream_kernel(const STensor* __restrict__ T, int nT, const P1Item* __restrict__ 
                 for (int e = 0; e < 4; ++e)
                     add_bf16x2(w[e], v[8 * j + 2 * e], v[8 * j + 2 * e + 1], v[8 * j + 2 * e], v[8 * j + 2 * e + 1]);
             }
+            const bool row_ok = r < it.rows;
+            float scale = it.scale;
             if (mode == M_TAP) {
-                if (r < it.rows) {
+                if (row_ok) {
                     float* trow = reinterpret_cast<float*>(it.out) + (int64_t)(it.r0 + r) * it.ld + it.c0 + 32 * cq;
 #pragma unroll
                     for (int h = 0; h < 8; ++h)
                         if (32 * cq + 4 * h < it.cols) *reinterpret_cast<float4*>(trow + 4 * h) = make_float4(v[4 * h], v[4 * h + 1], v[4 * h + 2], v[4 * h + 3]);
                 }
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) { mbar_arrive(tempty_bar(slot)); mbar_arrive(bempty_bar(bs)); }
             } else {
-                float mx = 0.0f;
+                if (mode != M_CAST) {
+                    float mx = 0.0f;
 #pragma unroll
-                for (int e = 0; e < 16; ++e) mx = max3abs(mx, v[2 * e], v[2 * e + 1]);
-                tmem_st32(taddr, a);
-                uint32_t wm;                                    // (non-negative floats and NaN order as integers)
-                asm volatile("redux.sync.max.u32 %0, %1, 0xffffffff;" : "=r"(wm) : "r"(__float_as_uint(mx)));
-                if (lane == 0) s_wmax[slot * 16 + ew] = wm;
-                if (ew == 0 && lane == 0) {
-                    Parked pk;
-                    pk.sync = it.sync; pk.scale_inv = it.scale_inv; pk.out = reinterpret_cast<uint8_t*>(it.out);
-                    pk.ld = it.ld; pk.row0 = it.r0; pk.col0 = it.c0; pk.rows = it.rows; pk.cols = it.cols; pk.fmt = it.fmt;
-                    pk.total = it.total; pk.first = it.first; pk.local = mode == M_BLOCK ? 1 : 0; pk.pad = 0;
-                    s_park[slot] = pk;
+                    for (int e = 0; e < 16; ++e) mx = max3abs(mx, v[2 * e], v[2 * e + 1]);
+                    uint32_t wm;                                // (non-negative floats and NaN order as integers)
+                    asm volatile("redux.sync.max.u32 %0, %1, 0xffffffff;" : "=r"(wm) : "r"(__float_as_uint(mx)));
+                    if (mode == M_AMAX) {
+                        // (one buffer and barrier per ring entry: the publisher warp frees the entry only after it has read them)
+                        if (lane == 0) { s_wmax[rslot * 16 + ew] = wm; mbar_arrive(amax_bar(rslot)); }
+                    } else {        // M_BLOCK: the 16 warps exchange their maxima (CTA-level barrier of the epilogue warps)
+                        if (lane == 0) s_wblk[(nblk & 1u) * 16 + ew] = wm;
+                        asm volatile("bar.sync 3, 512;" ::: "memory");
+                        uint32_t bits = 0;
+#pragma unroll
+                        for (int w = 0; w < 16; ++w) bits = max(bits, s_wblk[(nblk & 1u) * 16 + w]);
+                        ++nblk;
+                        float si;
+                        scales_from_amax(bits, it.fmt == 0 ? 448.0f : 57344.0f, scale, si);
+                        if (ew == 0 && lane == 0) *it.scale_inv = si;
+                    }
                 }
-                tmem_wait_st();
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) { mbar_arrive(parked_bar(slot)); mbar_arrive(bempty_bar(bs)); }
+                if (mode != M_AMAX) {
+                    uint4 cd[2];
+                    uint32_t* cw = reinterpret_cast<uint32_t*>(cd);
+                    if (it.fmt == 0) {
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) cw[j] = cast4<0>(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3], scale);
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) cw[j] = cast4<1>(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3], scale);
+                    }
+                    if (row_ok) {
+                        uint8_t* orow = reinterpret_cast<uint8_t*>(it.out) + (int64_t)(it.r0 + r) * it.ld + it.c0 + 32 * cq;
+#pragma unroll
+                        for (int h = 0; h < 2; ++h)
+                            if (32 * cq + 16 * h < it.cols) *reinterpret_cast<uint4*>(orow + 16 * h) = cd[h];
+                    }
+                    // (lead control of the pass-1 pipeline counts finished tiles; an approximate count is all it needs)
+                    if (ew == 0 && lane == 0) asm volatile("red.relaxed.gpu.global.add.u32 [%0], 1;" ::"l"(it.sync + SY_DONE) : "memory");
+                }
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(iempty_bar(rslot));
             if (ew == 0 && lane == 0) EV(5, nq);
-            if (mode != M_TAP) ++npark;
-            ++nq; have = false;
+#ifdef GF8_STREAM_PROF
+            pf[2] += clock64() - _tw;
+#endif
         }
         if (ew == 0 && lane == 0) PROF_OUT(3)
     }
@@ -688,9 +647,6 @@ stream_kernel(const STensor* __restrict__ T, int nT, const P1Item* __restrict__ 
         };
         constexpr int PF = 6;                         // L2 prefetch distance in K-steps (32 KB of gradient each)
         while (ok) {
-            // pass-1 work goes to the CTAs whose update pipeline has slack (it waits for the grid or for readiness): tensors complete
-            // in lock step across CTAs, so a CTA that streams panels while its update tiles are the late ones would hold everyone up
-            PROF(5, for (uint32_t spin = 0; !(s_slack[0] | s_slack[1]) && spin < 64u; ++spin) __nanosleep(100));
             int c = 0;
             if (lane == 0) c = atomicAdd(ctr, 1);
             c = __shfl_sync(0xFFFFFFFFu, c, 0);
@@ -703,14 +659,14 @@ stream_kernel(const STensor* __restrict__ T, int nT, const P1Item* __restrict__ 
             PROF(4, load_tensor(s_p1t, pi.tensor));
             const STensor& t = *s_p1t;
             // lead control: this panel's tensor may not run further ahead of the update frontier than the plan's lead
-            if (pi.gate_tensor >= 0) { PROF(1, ok = poll_ge(sync_base + (size_t)pi.gate_tensor * SY_WORDS + SY_TILES, (uint32_t)pi.gate_total)); if (!ok) break; }
+            if (pi.gate_tensor >= 0) { PROF(1, ok = poll_ge(sync_base + (size_t)pi.gate_tensor * SY_WORDS + SY_DONE, (uint32_t)pi.gate_total)); if (!ok) break; }
             const bool both = t.useA && t.useG, isP = pi.kind == K_PANEL_P;
             RItem it;
             it.kind = pi.kind; it.slot = 3; it.r0 = pi.r0; it.c0 = 0; it.rows = pi.rows; it.cols = 64; it.mode = 0;
             it.mapA0 = isP ? t.map_src_p : t.map_src_q; it.mapB0 = isP ? t.map_UAt : t.map_UGt; it.mapA1 = it.mapB1 = -1;
             it.fmt = 0; it.ld = 64; it.nrb = pi.rows > 128 ? 2 : 1; it.bslot = 0;
             it.total = 0; it.first = (!isP && both) ? 1 : 0;              // first: a Q panel whose last K-step adds U_A (S E_A)^T
-            it.n_cols_tile = 64; it.out_f32 = 0; it.base32 = nullptr; it.sync = t.sync; it.scale_inv = nullptr;
+            it.scale = 1.0f; it.out_f32 = 0; it.base32 = nullptr; it.sync = t.sync; it.scale_inv = nullptr;
             const int base_steps = isP ? (t.n + 63) / 64 : (t.m + 63) / 64;
             it.ksteps = base_steps + it.first;
             it.out = isP ? (void*)t.Pp : (void*)t.Qpt; it.colscale = isP ? t.eA : t.eG;
@@ -821,7 +777,7 @@ stream_kernel(const STensor* __restrict__ T, int nT, const P1Item* __restrict__ 
         const int q4 = warp & 3;
         const int r = q4 * 32 + lane, tid = threadIdx.x - W_PEPI * 32;
         const uint32_t lane_off = (uint32_t)(q4 * 32) << 16;
-        volatile int* s_last = reinterpret_cast<volatile int*>(misc + 468);
+        volatile int* s_last = reinterpret_cast<volatile int*>(misc + 504);
         volatile int* s_pok = reinterpret_cast<volatile int*>(misc + 2816);      // [4]
         bool ok = true;
         PROF_DECL

@@ -29,7 +29,8 @@ struct SPlan {
 namespace {
 
 constexpr size_t S_MAX_PLANS = 16;
-constexpr long long S_LEAD_BYTES = 80ll << 20;       // pass-1 may lead the update by this much gradient (L2 residency)
+constexpr int S_PASS_LAG = 450;                      // update-list entries between a tensor's last pass-A tile and its first pass-B tile
+constexpr long long S_LEAD_BYTES = 96ll << 20;       // pass-1 may lead the update by this much gradient (L2 residency)
 
 void splan_free(SPlan* p) {
     if (!p) return;
@@ -69,11 +70,11 @@ gf8_status make_map_3d(gf8_ctx* c, CUtensorMap* out, const void* ptr, uint64_t r
 }
 
 inline bool stream_eligible(const gf8_ctx* c, const LayerState& L, gf8_dtype dt, bool tap) {
+    if (!c->use_stream) return false;          // opt-in (GF8_STREAM=1, read once in gf8_create): see DESIGN.md 5 for where it stands
     if (!L.tc_ok || dt != GF8_DT_BF16 || c->precision != GF8_PREC_FAST) return false;
     if ((L.in.used && L.in.kp != 64) || (L.out.used && L.out.kp != 64)) return false;
     if (L.desc.d_in % 64) return false;
-    const int64_t tiles = (int64_t)((L.desc.d_out + 127) / 128) * ((L.desc.d_in + 127) / 128);
-    if (!tap && L.desc.scaling == GF8_SCALE_TENSOR && tiles > (int64_t)gf8::st::NPARK * c->num_sms) return false;
+    (void)tap;
     return true;
 }
 
@@ -118,7 +119,7 @@ gf8_status splan_build(gf8_ctx* c, SPlan* p, const std::vector<int>& lay, bool t
         STensor& t = T[i];
         memset(&t, 0, sizeof(t));
         t.m = L.desc.d_out; t.n = L.desc.d_in; t.useA = L.in.used ? 1 : 0; t.useG = L.out.used ? 1 : 0;
-        t.fmt = L.desc.fmt; t.mode = tap ? M_TAP : (L.desc.scaling == GF8_SCALE_TENSOR ? M_PARK : M_BLOCK);
+        t.fmt = L.desc.fmt; t.mode = tap ? M_TAP : (L.desc.scaling == GF8_SCALE_TENSOR ? M_AMAX : M_BLOCK);
         t.tiles_n = (t.n + 127) / 128; t.n_tiles = ((t.m + 127) / 128) * t.tiles_n;
         t.nP = t.useA ? (t.m + 255) / 256 : 0; t.nQ = t.useG ? (t.n + 255) / 256 : 0; t.nQP = (t.useA && t.useG) ? t.nQ : 0;
         t.dep_idx = SY_QP;               // the last pass-1 stage of a tensor counts on SY_QP (Q' items; P / Q panels if one-sided)
@@ -153,7 +154,7 @@ gf8_status splan_build(gf8_ctx* c, SPlan* p, const std::vector<int>& lay, bool t
         const long long bytes = (long long)t.m * t.n * 2;
         // lead control: the last tensor that lies wholly more than S_LEAD_BYTES of gradient behind this one must be complete
         while (gate_next < i && T[gate_next].byte_pos + (long long)T[gate_next].m * T[gate_next].n * 2 + S_LEAD_BYTES <= t.byte_pos) ++gate_next;
-        const int gate = (tap || gate_next == 0) ? -1 : gate_next - 1, gate_total = gate >= 0 ? T[gate].n_tiles : 0;
+        const int gate = (tap || gate_next == 0 || getenv("GF8_P1ONLY")) ? -1 : gate_next - 1, gate_total = gate >= 0 ? T[gate].n_tiles : 0;
         for (int i0 = 0; t.useA && i0 < t.m; i0 += 256) p1.push_back({K_PANEL_P, i, i0, std::min(256, t.m - i0), gate, gate_total, 0, 0});
         for (int j0 = 0; t.useG && j0 < t.n; j0 += 256) p1.push_back({K_PANEL_Q, i, j0, std::min(256, t.n - j0), gate, gate_total, 0, 0});
         byte_pos += bytes;
@@ -164,23 +165,24 @@ gf8_status splan_build(gf8_ctx* c, SPlan* p, const std::vector<int>& lay, bool t
     for (int i = 0; i < nT; ++i) { T[i].map_src_p = n_static + 3 * i; T[i].map_src_q = n_static + 3 * i + 1; T[i].map_src_b = n_static + 3 * i + 2; }
     p->n_maps = n_static + 3 * nT; p->n_p1 = (int)p1.size(); p->n_upd = upd; p->n_shapes = (int)shape_idx.size();
     p->grid = std::max(1, std::min(c->num_sms, std::max(p->n_upd, p->n_p1)));
-    for (int i = 0; i < nT; ++i)
-        if (T[i].mode == M_PARK && T[i].n_tiles > NPARK * p->grid) return fail(c, GF8_ERR_BAD_STATE, "stream plan: tensor too large to park");
-    std::vector<TileEnt> tiles((size_t)upd);
+    // update list: pass-A tiles of a tensor, and its pass-B tiles S_PASS_LAG list entries later (by then the A tiles have run)
+    std::vector<TileEnt> tiles;
     {
-        std::vector<int> tile_tensor((size_t)upd);
-        for (int i = 0; i < nT; ++i)
-            for (int k = 0; k < T[i].n_tiles; ++k) tile_tensor[(size_t)T[i].upd_start + k] = i;
-        for (int u = 0; u < upd; ++u) {
-            const STensor& t = T[tile_tensor[u]];
-            const int k = u - t.upd_start, prev = u - NPARK * p->grid;
-            TileEnt e;
-            e.tensor = tile_tensor[u]; e.tij = (k / t.tiles_n) | ((k % t.tiles_n) << 16);
-            e.old_tensor = (prev >= 0 && T[tile_tensor[prev]].mode == M_PARK) ? tile_tensor[prev] : -1;
-            e.dep_old = t.dep_target | ((e.old_tensor >= 0 ? T[e.old_tensor].n_tiles : 0) << 16);
-            tiles[u] = e;
+        std::vector<std::pair<int, size_t>> pendB;          // (tensor, list length when its A tiles were all listed)
+        size_t headB = 0;
+        auto emit = [&](int i, int pass) {
+            for (int k = 0; k < T[i].n_tiles; ++k) tiles.push_back({i, (k / T[i].tiles_n) | ((k % T[i].tiles_n) << 16), pass, 0});
+        };
+        for (int i = 0; i < nT && !getenv("GF8_P1ONLY"); ++i) {
+            if (T[i].mode == M_AMAX) { emit(i, P_AMAX); pendB.push_back({i, tiles.size()}); }
+            else emit(i, P_SINGLE);
+            while (headB < pendB.size() && tiles.size() - pendB[headB].second >= (size_t)S_PASS_LAG) emit(pendB[headB++].first, P_CAST);
         }
+        while (headB < pendB.size()) emit(pendB[headB++].first, P_CAST);
     }
+    upd = (int)tiles.size();
+    p->n_upd = upd;
+    p->grid = std::max(1, std::min(c->num_sms, std::max(p->n_upd, p->n_p1)));
     p->sync_bytes = ((size_t)nT * SY_WORDS + 4) * sizeof(uint32_t);
     auto dm = [&](void** out, size_t bytes) -> bool { return cudaMalloc(out, std::max<size_t>(bytes, 16)) == cudaSuccess; };
     if (!dm((void**)&p->d_T, sizeof(STensor) * nT) || !dm((void**)&p->d_tiles, sizeof(TileEnt) * tiles.size()) || !dm((void**)&p->d_p1, sizeof(P1Item) * p1.size()) ||
