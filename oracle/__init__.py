@@ -68,6 +68,9 @@ def _declare(L):
     L.gf8o_from_bf16.argtypes = [_ph, _i64, _pd]
     L.gf8o_to_f32.argtypes = [_pd, _i64, _pf]
     L.gf8o_metrics.argtypes = [_pd, _pd, _i64, _pd]
+    _pi = C.POINTER(C.c_int64)
+    L.gf8o_factor_entries.argtypes = [_pd, _i64, _i64, _pi, _pi, _i64, _pd]
+    L.gf8o_whiten_samples.argtypes = [_pd, _i64, _i64, _pd, _pd, C.c_int, _pd, _pd, C.c_int, _pi, _pi, _i64, _pd]
     L.gf8o_num_threads.restype = C.c_int
 
 
@@ -226,6 +229,41 @@ def whiten_lowrank(W, UG=None, eG=None, UA=None, eA=None):
     out = np.empty((m, n))
     lib().gf8o_whiten_lowrank(_p(W, _pd), m, n, _p(UG, _pd), _p(eG, _pd), kG, _p(UA, _pd), _p(eA, _pd), kA,
                               _p(out, _pd))
+    return out
+
+
+# ---- sampled outputs (full-size parity: one output element at a time, by its plain definition) ----
+def _idx(a):
+    return np.ascontiguousarray(a, dtype=np.int64)
+
+
+def factor_entries(X, ii, jj):
+    """O1 at sampled (i, j): A[i][j] = mean_t x_t[i] x_t[j] (no EMA)."""
+    X = _d(X)
+    T, d = X.shape
+    ii, jj = _idx(ii), _idx(jj)
+    out = np.empty(ii.shape[0])
+    pi = C.POINTER(C.c_int64)
+    lib().gf8o_factor_entries(_p(X, _pd), T, d, ii.ctypes.data_as(pi), jj.ctypes.data_as(pi), ii.shape[0], _p(out, _pd))
+    return out
+
+
+def whiten_samples(W, ii, jj, UG=None, eG=None, UA=None, eA=None):
+    """O3 (with e) / O6 (with ebar) at sampled (i, j), dense form of Eq. 14 / 17."""
+    W = _d(W)
+    m, n = W.shape
+    kG = kA = 0
+    if UG is not None:
+        UG, eG = _d(UG), _d(eG)
+        kG = UG.shape[1]
+    if UA is not None:
+        UA, eA = _d(UA), _d(eA)
+        kA = UA.shape[1]
+    ii, jj = _idx(ii), _idx(jj)
+    out = np.empty(ii.shape[0])
+    pi = C.POINTER(C.c_int64)
+    lib().gf8o_whiten_samples(_p(W, _pd), m, n, _p(UG, _pd), _p(eG, _pd), kG, _p(UA, _pd), _p(eA, _pd), kA,
+                              ii.ctypes.data_as(pi), jj.ctypes.data_as(pi), ii.shape[0], _p(out, _pd))
     return out
 
 

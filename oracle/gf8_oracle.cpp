@@ -452,6 +452,51 @@ void gf8o_metrics(const double* ghat, const double* g, int64_t n, double* out4) 
     out4[3] = d2 / (double)n;
 }
 
+// ------------------------------------------------------------------------------------------------
+// Sampled outputs (parity at BASELINE.json's full sizes, where the whole-matrix routines above are too slow):
+// each is the plain definition of ONE output element.
+//
+// O1 at (i, j): A[i][j] = (1/T) sum_t x_t[i] x_t[j]                        (Eq. 4), no EMA.
+// O3 / O6 at (i, j): (T_G W T_A)[i][j] = sum_r sum_c T_G[i][r] W[r][c] T_A[c][j] with the DENSE rows / columns of
+//   T = I + U diag(e) U^T formed on the fly (Eq. 14 in the dense form; pass ebar for Eq. 17).
+// ------------------------------------------------------------------------------------------------
+void gf8o_factor_entries(const double* X, int64_t T, int64_t d, const int64_t* ii, const int64_t* jj, int64_t ns, double* out) {
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t s = 0; s < ns; ++s) {
+        double c = 0.0;
+        for (int64_t t = 0; t < T; ++t) c += X[t * d + ii[s]] * X[t * d + jj[s]];
+        out[s] = c / (double)T;
+    }
+}
+
+void gf8o_whiten_samples(const double* W, int64_t m, int64_t n, const double* UG, const double* eG, int kG, const double* UA,
+                         const double* eA, int kA, const int64_t* ii, const int64_t* jj, int64_t ns, double* out) {
+    if (!UG) kG = 0;
+    if (!UA) kA = 0;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t s = 0; s < ns; ++s) {
+        const int64_t i = ii[s], j = jj[s];
+        std::vector<double> tg((size_t)m), ta((size_t)n);
+        for (int64_t r = 0; r < m; ++r) {                 // row i of T_G
+            double acc = r == i ? 1.0 : 0.0;
+            for (int g = 0; g < kG; ++g) acc += UG[i * kG + g] * eG[g] * UG[r * kG + g];
+            tg[(size_t)r] = acc;
+        }
+        for (int64_t c = 0; c < n; ++c) {                 // column j of T_A
+            double acc = c == j ? 1.0 : 0.0;
+            for (int a = 0; a < kA; ++a) acc += UA[c * kA + a] * eA[a] * UA[j * kA + a];
+            ta[(size_t)c] = acc;
+        }
+        double v = 0.0;
+        for (int64_t r = 0; r < m; ++r) {
+            double row = 0.0;
+            for (int64_t c = 0; c < n; ++c) row += W[r * n + c] * ta[(size_t)c];
+            v += tg[(size_t)r] * row;
+        }
+        out[s] = v;
+    }
+}
+
 int gf8o_num_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

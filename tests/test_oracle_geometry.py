@@ -261,3 +261,33 @@ def test_config0_pipeline_properties():
     # reading S15), so unwhitening amplifies the isotropic FP8 noise along the top-k directions by
     # (mu_i + lam) / rho: ~0.019 per-side-whitened error * ~6 here.  No fidelity gain is expected.
     assert mt["RelL2"] < 0.2 and mt["Cos"] > 0.99
+
+
+# ---- sampled-output routines (full-size parity helpers) pinned against the whole-matrix forms and closed forms ------
+def test_sampled_outputs_agree_with_whole_matrix_forms_and_closed_forms():
+    rng = np.random.default_rng(11)
+    m, n, kG, kA = 40, 56, 5, 7
+    W = rng.normal(size=(m, n))
+    UG = np.linalg.qr(rng.normal(size=(m, kG)))[0]
+    UA = np.linalg.qr(rng.normal(size=(n, kA)))[0]
+    eG, eA = rng.uniform(-0.9, 3.0, kG), rng.uniform(-0.9, 3.0, kA)
+    ii, jj = rng.integers(0, m, 64), rng.integers(0, n, 64)
+    # (a) against the low-rank whole-matrix form (two independent oracle forms of Eq. 14 must agree), all side combinations
+    for ug, ua in ((UG, UA), (UG, None), (None, UA), (None, None)):
+        full = oracle.whiten_lowrank(W, ug, eG if ug is not None else None, ua, eA if ua is not None else None)
+        got = oracle.whiten_samples(W, ii, jj, ug, eG if ug is not None else None, ua, eA if ua is not None else None)
+        assert np.abs(got - full[ii, jj]).max() <= 1e-12 * np.abs(full).max()
+    # (b) against the explicit dense T matrices built with numpy (Eq. 14)
+    TG = np.eye(m) + UG @ np.diag(eG) @ UG.T
+    TA = np.eye(n) + UA @ np.diag(eA) @ UA.T
+    assert np.abs(oracle.whiten_samples(W, ii, jj, UG, eG, UA, eA) - (TG @ W @ TA)[ii, jj]).max() <= 1e-12 * np.abs(W).max() * 20
+    # (c) a transposed-operand mistake shows: a matrix with one non-zero element and rank-one factors has a closed form
+    W1 = np.zeros((m, n)); W1[3, 9] = 2.0
+    want = 2.0 * TG[ii, 3] * TA[9, jj]
+    assert np.abs(oracle.whiten_samples(W1, ii, jj, UG, eG, UA, eA) - want).max() <= 1e-13
+    # factor entries: the whole-matrix routine, and a closed form (one-hot samples: A = diag(counts) / T)
+    X = rng.normal(size=(33, 12))
+    fi, fj = rng.integers(0, 12, 40), rng.integers(0, 12, 40)
+    assert np.abs(oracle.factor_entries(X, fi, fj) - oracle.factor_accumulate(X)[fi, fj]).max() <= 1e-14
+    onehot = np.eye(12)[[0, 0, 5, 7, 7, 7]]
+    assert np.allclose(oracle.factor_entries(onehot, [0, 5, 7, 0], [0, 5, 7, 5]), [2 / 6, 1 / 6, 3 / 6, 0.0], atol=1e-15)
