@@ -143,6 +143,7 @@ def test_g5_reduce_decoded(name):
 
 # ---- the same gates on the FAST (BF16 tensor-core, tcgen05) path: north_star's 2e-3 tier ------------------
 TOL_FAST = 2e-3
+TOL_FAST_BF16 = 2e-3 + 2.0 ** -9     # FAST tier + one BF16 rounding of the result (Tolerances)
 FAST_CASES = dict(CASES)
 FAST_CASES.update({
     "llama600m-q": dict(m=1536, n=1536, kG=64, kA=64, side=gf8.SIDE_BOTH, dtype="bf16", seed=5, T=4096, q=2),
@@ -203,7 +204,7 @@ def test_fast_g5_reduce_decoded(name):
     c.ctx.sync_check()
     assert relfro(to_np64(got32), want) <= TOL_FAST
     got16 = c.ctx.reduce_decoded(0, dc, ds, True, dt=gf8.DT_BF16)
-    assert relfro(to_np64(got16), want) <= 2 * TOL_FAST
+    assert relfro(to_np64(got16), want) <= TOL_FAST_BF16
     one = c.ctx.decode(0, dc[0], ds[0], dt=gf8.DT_F32)
     want1 = c.oracle_reduce_decoded(pays[0][:1], [pays[0][1]], average=False)
     assert relfro(to_np64(one), want1) <= TOL_FAST
@@ -252,7 +253,7 @@ def test_fast_full_size_shapes_in_the_bench_launch_configuration():
         pc = [codes[i * R + r].cpu().numpy() for r in range(R)]
         ps = [sinvs[i * R + r].cpu().numpy() for r in range(R)]
         want = oracle.reduce_decoded(pc, ps, bases[i][gf8.SIDE_OUT], bases[i][gf8.SIDE_IN])
-        assert relfro(to_np64(outs[i]), want) <= 2 * TOL_FAST
+        assert relfro(to_np64(outs[i]), want) <= TOL_FAST_BF16
 
 
 @pytest.mark.parametrize("name", ["config0", "ragged-bf16", "block-e5m2"])
@@ -282,7 +283,8 @@ def test_exact_on_tensor_cores_meets_the_transform_tier(name, monkeypatch):
 def test_config4_style_loop_with_periodic_refresh():
     """BASELINE.json configs[4] in miniature: R = 16 perturbed replicas of one gradient, encode x 16 -> FP32 sum of the
     decoded payloads -> unwhiten, with an EMA factor update + warm basis refresh (q = 2) every 10 steps.  After the
-    last refresh the GPU's transform T is compared with the oracle run through the same updates (G7), and the last
+    last refresh the factors are compared with the oracle's EMA chain (G6) and the GPU's transform T with the oracle's refresh of
+    the same factor bits from the same warm start (G7, 1e-4), and the last
     step's averaged gradient with the oracle codec on the GPU's basis (G5, FAST tier)."""
     m, n, k, R, lam, beta, T = 384, 512, 32, 16, 1e-3, 0.9, 2048
     lay = gf8.Layer(m, n, gf8.SIDE_BOTH, k, k, gf8.E4M3, gf8.SCALE_TENSOR, lam, beta)
@@ -291,7 +293,6 @@ def test_config4_style_loop_with_periodic_refresh():
     ctx.set_basis(0, gf8.SIDE_IN, synth.start_basis(n, k, "cuda", 404, 1))
     ctx.set_basis(0, gf8.SIDE_OUT, synth.start_basis(m, k, "cuda", 404, 2))
     A = Gf = None
-    VA, VG = to_np64(synth.start_basis(n, k, "cuda", 404, 1)), to_np64(synth.start_basis(m, k, "cuda", 404, 2))
     codes = [torch.empty((m, n), dtype=torch.uint8, device="cuda") for _ in range(R)]
     sinvs = [torch.empty(1, dtype=torch.float32, device="cuda") for _ in range(R)]
     out = torch.empty((m, n), dtype=torch.bfloat16, device="cuda")
@@ -300,24 +301,24 @@ def test_config4_style_loop_with_periodic_refresh():
             X = synth.factor_samples(T, n, "cuda", 404, 3, step).to(torch.bfloat16)
             D = synth.factor_samples(T, m, "cuda", 404, 4, step).to(torch.bfloat16)
             ctx.factor_update(0, X, D)
+            warm = {sd: ctx.get_basis(0, sd)[0].clone() for sd in (gf8.SIDE_IN, gf8.SIDE_OUT)} if step else None
             ctx.refresh_basis_many([0], 8 if step == 0 else 2)
-            first = A is None
+            first = A is None                                      # the oracle's own EMA chain of the factors (G6 below)
             A = oracle.factor_accumulate(to_np64(X), A, 0.0 if first else beta)
             Gf = oracle.factor_accumulate(to_np64(D), Gf, 0.0 if first else beta)
-            bA = oracle.refresh_basis(A, VA, 8 if first else 2, lam)
-            bG = oracle.refresh_basis(Gf, VG, 8 if first else 2, lam)
-            VA, VG = bA.U, bG.U                                    # warm start, as the library does
         grads = [synth.rank_gradient(G, r, 404, step).to(torch.bfloat16) for r in range(R)]
         ctx.encode_many([0] * R, grads, codes, sinvs)
         ctx.reduce_decoded_many([0], codes, sinvs, R, [out], average=True)
     ctx.sync_check()
-    # G7 on the transform after three refreshes
-    for side, b, d in ((gf8.SIDE_IN, bA, n), (gf8.SIDE_OUT, bG, m)):
+    # G6 on the EMA chain (three updates), then G7 on the last refresh: the oracle runs O2 on the factor bits the GPU holds,
+    # from the basis the GPU started from
+    assert relfro(to_np64(ctx.get_factor(0, gf8.SIDE_IN)), A) <= TOL_EXACT and relfro(to_np64(ctx.get_factor(0, gf8.SIDE_OUT)), Gf) <= TOL_EXACT
+    for side, d in ((gf8.SIDE_IN, n), (gf8.SIDE_OUT, m)):
         U, mu, rho = ctx.get_basis(0, side)
+        b = oracle.refresh_basis(to_np64(ctx.get_factor(0, side)), to_np64(warm[side]), 2, lam)
         Dg = np.sqrt(rho / (to_np64(mu) + lam))
         Tg = np.eye(d) + to_np64(U) @ np.diag(Dg - 1.0) @ to_np64(U).T
-        To = oracle.build_T(b.U, b.e)
-        assert relfro(Tg, To) <= 1e-3, relfro(Tg, To)
+        assert relfro(Tg, oracle.build_T(b.U, b.e)) <= TOL_EXACT
     # G5 (FAST) on the last step with the GPU's own basis handed to the oracle
     def gb(side):
         U, mu, rho = ctx.get_basis(0, side)
@@ -326,7 +327,7 @@ def test_config4_style_loop_with_periodic_refresh():
         return oracle.Basis(to_np64(U), mu64, rho, Dm - 1.0, 1.0 / Dm - 1.0)
     want = oracle.reduce_decoded([c_.cpu().numpy() for c_ in codes], [s_.cpu().numpy() for s_ in sinvs], gb(gf8.SIDE_OUT),
                                  gb(gf8.SIDE_IN))
-    assert relfro(to_np64(out), want) <= 2 * TOL_FAST
+    assert relfro(to_np64(out), want) <= TOL_FAST_BF16
     # the averaged decoded gradient is close to the shared gradient (16 independent perturbations average out)
     assert relfro(to_np64(out), to_np64(G)) <= 0.1
 
