@@ -218,8 +218,28 @@ __device__ __forceinline__ void load_base16(const Item& it, int64_t off, float* 
     }
 }
 
+// (v0, v1) * s with one packed multiply (FMUL2); the same IEEE products as two FMULs
+__device__ __forceinline__ void mul2(float v0, float v1, float s, float& x0, float& x1) {
+    uint64_t a, ss;
+    asm("mov.b64 %0, {%1, %1};" : "=l"(ss) : "f"(s));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(a) : "f"(v0), "f"(v1));
+    asm("mul.rn.f32x2 %0, %0, %1;" : "+l"(a) : "l"(ss));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(x0), "=f"(x1) : "l"(a));
+}
 template <int FMT>
 __device__ __forceinline__ uint4 codes16(const float* v, float s) {
+    float x[16];
+#pragma unroll
+    for (int u = 0; u < 16; u += 2) mul2(v[u], v[u + 1], s, x[u], x[u + 1]);
+    uint4 q;
+    q.x = f32x4_to_fp8x4<FMT>(x[0], x[1], x[2], x[3]);
+    q.y = f32x4_to_fp8x4<FMT>(x[4], x[5], x[6], x[7]);
+    q.z = f32x4_to_fp8x4<FMT>(x[8], x[9], x[10], x[11]);
+    q.w = f32x4_to_fp8x4<FMT>(x[12], x[13], x[14], x[15]);
+    return q;
+}
+template <int FMT>
+__device__ __forceinline__ uint4 codes16_scalar(const float* v, float s) {
     uint4 o;
     o.x = f32x4_to_fp8x4<FMT>(__fmul_rn(v[0], s), __fmul_rn(v[1], s), __fmul_rn(v[2], s), __fmul_rn(v[3], s));
     o.y = f32x4_to_fp8x4<FMT>(__fmul_rn(v[4], s), __fmul_rn(v[5], s), __fmul_rn(v[6], s), __fmul_rn(v[7], s));
@@ -384,6 +404,21 @@ __device__ __forceinline__ void tile_values32(uint32_t taddr, uint32_t row, int 
     uint4 b[4];
 #pragma unroll
     for (int j = 0; j < 4; ++j) b[j] = lds128(row + (((uint32_t)(4 * g + j) ^ (uint32_t)(r & 7)) << 4));
+    if (n_base == 1) {
+        // one BF16 base: v = float(base) + acc in ONE instruction per element (FHADD.BF16: exact widening, one FP32 rounding --
+        // bit-identical to unpack-then-add, at a third of the instructions)
+        tmem_wait();
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint32_t w[4] = {b[j].x, b[j].y, b[j].z, b[j].w};
+#pragma unroll
+            for (int e = 0; e < 4; ++e)
+                asm("{\n\t.reg .b16 lo, hi;\n\tmov.b32 {lo, hi}, %2;\n\tadd.rn.f32.bf16 %0, lo, %3;\n\tadd.rn.f32.bf16 %1, hi, %4;\n\t}"
+                    : "=f"(v[8 * j + 2 * e]), "=f"(v[8 * j + 2 * e + 1])
+                    : "r"(w[e]), "f"(__uint_as_float(a[8 * j + 2 * e])), "f"(__uint_as_float(a[8 * j + 2 * e + 1])));
+        }
+        return;
+    }
 #pragma unroll
     for (int j = 0; j < 4; ++j) unpack_bf16x8(b[j], v + 8 * j);
     if (n_base > 1) {
@@ -423,8 +458,13 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
 #pragma unroll
             for (int g = 0; g < 2; ++g) {
                 tile_values32(taddr0 + 64u * h, row_lo + 16384u * h, n_base, r, g, v);
+                // max |v| two elements per instruction (FMNMX3, NaN-propagating: a NaN amax orders above every finite value
+                // as an integer, like the bit-pattern maximum it replaces)
+                float mx = __uint_as_float(loc);
 #pragma unroll
-                for (int u = 0; u < 32; ++u) loc = max(loc, __float_as_uint(v[u]) & 0x7FFFFFFFu);
+                for (int u = 0; u < 32; u += 2)
+                    asm("max.NaN.f32 %0, %1, %2, %0;" : "+f"(mx) : "f"(fabsf(v[u])), "f"(fabsf(v[u + 1])));
+                loc = __float_as_uint(mx);
             }
         if (mode == EPI_AMAX) {
             if (run_max) { *run_max = max(*run_max, loc); return false; }
