@@ -9,14 +9,20 @@ namespace gf8 {
 // ---- Cholesky of a k x k SPD Gram matrix, in place, upper factor R (G = R^T R), one CTA -----------
 // G row-major in global memory (k <= 512); only the upper triangle is read and written.
 __global__ void __launch_bounds__(1024) cholesky_upper_kernel(double* __restrict__ G, int k) {
-    __shared__ double s_diag;
+    __shared__ double s_diag, s_dmax;
+    if (threadIdx.x == 0) {
+        double mx = 0.0;
+        for (int j = 0; j < k; ++j) mx = fmax(mx, G[(int64_t)j * k + j]);
+        s_dmax = mx;
+    }
+    __syncthreads();
     for (int j = 0; j < k; ++j) {
         if (threadIdx.x == 0) {
-            double d = G[(int64_t)j * k + j];
-            // Breakdown guard: a non-positive pivot (rank-deficient start basis) becomes a tiny one,
-            // so the column is kept finite and the second CholeskyQR pass re-orthonormalises it.
-            if (!(d > 0.0)) d = 1e-300;
-            s_diag = sqrt(d);
+            const double d = G[(int64_t)j * k + j];
+            // Breakdown guard: a pivot that has cancelled to (FP64) rounding level against the largest diagonal entry means the
+            // column lies in the span of the earlier ones (rank-deficient A V).  It is DEFLATED: a huge R_jj sends the column
+            // of V to ~0 (it then carries Ritz value 0 and contributes nothing to T) instead of blowing it up by 1 / sqrt(tiny).
+            s_diag = (d > 1e-26 * s_dmax && d > 0.0) ? sqrt(d) : 1e150;
             G[(int64_t)j * k + j] = s_diag;
         }
         __syncthreads();
@@ -173,8 +179,8 @@ __global__ void __launch_bounds__(256) multipliers_kernel(const float* __restric
                                                           double lam, double rho_in, float* __restrict__ mu_out,
                                                           float* __restrict__ e, float* __restrict__ ebar,
                                                           float* __restrict__ rho_out) {
-    __shared__ double s_part[256];
-    __shared__ double s_rho;
+    __shared__ double s_part[256], s_tr[256];
+    __shared__ double s_rho, s_floor;
     double tr = 0.0, sm = 0.0;
     if (factor) for (int i = threadIdx.x; i < d; i += blockDim.x) tr += (double)factor[(int64_t)i * d + i];
     for (int i = threadIdx.x; i < k; i += blockDim.x) {
@@ -182,14 +188,20 @@ __global__ void __launch_bounds__(256) multipliers_kernel(const float* __restric
         sm += m;
     }
     s_part[threadIdx.x] = tr - sm;
+    s_tr[threadIdx.x] = factor ? tr : sm;
     __syncthreads();
     if (threadIdx.x == 0) {
-        double t = 0.0;
-        for (int i = 0; i < blockDim.x; ++i) t += s_part[i];
+        double t = 0.0, scale = 0.0;
+        for (int i = 0; i < blockDim.x; ++i) { t += s_part[i]; scale += s_tr[i]; }
         double rho;
         if (!factor) rho = rho_in;
         else if (k < d) rho = fmax(0.0, t / (double)(d - k)) + lam;
         else rho = (mu64 ? fmax(mu64[k - 1], 0.0) : (double)mu32[k - 1]) + lam;
+        // Guard outside the paper's domain (damping 0 with a rank-deficient factor, S13): rho and mu_i + lambda are
+        // floored at 2^-23 of the mean eigenvalue, so D = sqrt(rho / (mu + lambda)) and 1 / D stay finite and positive.
+        const double fl = fmax(scale / (double)(factor ? d : k), 1e-300) * 1.1920928955078125e-7;
+        s_floor = fl;
+        rho = fmax(rho, fl);
         s_rho = rho;
         *rho_out = (float)rho;
     }
@@ -197,7 +209,7 @@ __global__ void __launch_bounds__(256) multipliers_kernel(const float* __restric
     const double rho = s_rho;
     for (int i = threadIdx.x; i < k; i += blockDim.x) {
         const double m = mu64 ? fmax(mu64[i], 0.0) : (double)mu32[i];
-        const double D = sqrt(rho / (m + lam));
+        const double D = sqrt(rho / fmax(m + lam, s_floor));
         mu_out[i] = (float)m;
         e[i] = (float)(D - 1.0);
         ebar[i] = (float)(1.0 / D - 1.0);

@@ -531,7 +531,7 @@ gf8_status plan_store(gf8_ctx* c, const std::vector<uint64_t>& key, Plan* p) {
 }
 
 gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
-    const bool first_run = p->runs++ == 0;
+    p->runs++;
     if (p->d_ctr) CU_TRY(c, cudaMemsetAsync(p->d_ctr, 0, 8 * sizeof(int), st));
     for (int s = 0; s < 8; ++s) {
         if (!p->stage_cnt[s]) continue;
@@ -552,7 +552,6 @@ gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
         // fences, 4 print a per-role wait profile, 32 skip the strip epilogue's work, 64 skip the strip base loads,
         // 128 skip the strip B loads, 256 print each stage's device time (serialises the stream)
         if (const char* e = getenv("GF8_TC_DBG")) dbg = atoi(e);
-        if (!first_run) dbg |= 2;        // tensor maps are written once by the host before the plan's first launch
         if (const char* e = getenv("GF8_TC_ONLY")) only = atoi(e);
         if (only >= 0 && only != s) continue;
         cudaEvent_t ev0 = nullptr, ev1 = nullptr;

@@ -623,6 +623,18 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
     tc_fence_after();
     const uint32_t tmem_base = *reinterpret_cast<volatile uint32_t*>(s_tmem);
 
+    // Tensor maps live in global memory (the plan's array): every CTA acquires a map through the tensormap proxy before its
+    // first use IN THIS LAUNCH (a freed plan's storage may be handed to a new plan, and an SM could otherwise still hold the
+    // old descriptor).  Each issuing warp remembers the last four maps it fenced, so a map costs one fence per CTA per run of
+    // items that use it, not one per item.  Call from converged code.
+    const CUtensorMap *fc0 = nullptr, *fc1 = nullptr, *fc2 = nullptr, *fc3 = nullptr;
+    auto acq = [&](const CUtensorMap* mp) {
+        if (mp != fc0 && mp != fc1 && mp != fc2 && mp != fc3) {
+            if (elect_one()) tmap_acquire(mp);
+            __syncwarp();
+            fc3 = fc2; fc2 = fc1; fc1 = fc0; fc0 = mp;
+        }
+    };
     // optional profile (prof != nullptr): cycles each role spends in each kind of wait, per CTA
     long long pw[6] = {0, 0, 0, 0, 0, 0};
     const long long t_start = clock64();
@@ -662,6 +674,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 const Item& it = *item_slot(slot);
                 const int bm0 = it.base_map[0], row0 = it.row0, nrb = (it.rows + 127) >> 7, nct = (it.cols + 127) >> 7;
                 const CUtensorMap* mp = maps + bm0;
+                acq(mp);
                 for (int ct = 0; ct < nct && ok; ++ct)
                     for (int rb = 0; rb < nrb && ok; ++rb) {
                         const uint32_t bs = b_bs, bph = b_bph;
@@ -687,13 +700,14 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 if (ok) {
                     const int bm0 = it.base_map[0], bm1 = it.base_map[1], col0 = it.col0, row0 = it.row0;
                     const int nb = (bm0 >= 0 ? 1 : 0) + (bm1 >= 0 ? 1 : 0);
+                    if (bm0 >= 0) acq(maps + bm0);
+                    if (bm1 >= 0) acq(maps + bm1);
                     if (elect_one()) {
                         if (nb == 0) mbar_arrive(bfull_bar(acc));
                         else {
                             mbar_expect_tx(bfull_bar(acc), (uint32_t)nb * TILE_BYTES);
                             for (int b = 0; b < nb; ++b) {
                                 const CUtensorMap* mp = maps + (b ? bm1 : bm0);
-                                if (!(dbg & 2)) tmap_acquire(mp);
                                 const uint32_t dst = base_tile(acc) + (uint32_t)b * TILE_BYTES;
 #pragma unroll
                                 for (int h = 0; h < 2; ++h) tma_load_2d(dst + h * 16384u, mp, col0 + 64 * h, row0, bfull_bar(acc));
@@ -722,6 +736,8 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                     // the B K-atoms of every column tile through the 16 KB ring (each serves both row blocks)
                     const int nrb = (it.rows + 127) >> 7, nct = (it.cols + 127) >> 7;
                     const int na = it.atoms[0] + it.atoms[1];
+                    for (int seg = 0; seg < 2; ++seg)
+                        if (it.atoms[seg] > 0) acq(maps + (is_b ? it.map_b[seg] : it.map_a[seg]));
                     if (!is_b) {
                         if (!(ok = TWAIT(2, mbar_wait(parked_bar(1), (n_done & 1u) ^ 1u, err)))) break;   // L buffer free
                         if (elect_one()) {
@@ -766,8 +782,8 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                     const CUtensorMap* m_hi = maps + (is_b ? it.map_b[0] : it.map_a[0]);
                     const CUtensorMap* m_lo = maps + (is_b ? it.map_b[2] : it.map_a[1]);
                     const int c0 = is_b ? it.b_c0[0] : it.a_c0[0], r0 = is_b ? it.b_r0[0] : it.a_r0[0];
-                    if (!(dbg & 2) && elect_one()) { tmap_acquire(m_hi); tmap_acquire(m_lo); }
-                    __syncwarp();
+                    acq(m_hi);
+                    acq(m_lo);
                     for (int t = 0; t < it.atoms[0]; ++t) {
                         if (!TWAIT(2, mbar_wait(empty_bar(stage), phase ^ 1u, err))) { ok = false; break; }
                         const uint32_t sa = smem0 + stage * stage_bytes;
@@ -802,8 +818,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                     if (na <= 0) continue;
                     const CUtensorMap* mp = maps + (is_b ? it.map_b[seg] : it.map_a[seg]);
                     const int c0 = is_b ? it.b_c0[seg] : it.a_c0[seg], r0 = is_b ? it.b_r0[seg] : it.a_r0[seg];
-                    if (!(dbg & 2) && elect_one()) tmap_acquire(mp);
-                    __syncwarp();
+                    acq(mp);
                     for (int t = 0; t < na; ++t) {
                         if (!TWAIT(2, mbar_wait(empty_bar(stage), phase ^ 1u, err))) { ok = false; break; }
                         const uint32_t sa = smem0 + stage * stage_bytes;
@@ -961,8 +976,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 for (;;) {
                     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(pk.done) : "memory");
                     if (seen >= (uint32_t)pk.total) break;
-                    if (++spin > (1u << 22) || ((spin & 0x3FF) == 0 && *reinterpret_cast<volatile int*>(err))) { bad = true; break; }
-                    __nanosleep(32);
+                    if (++spin > (1u << 24) || ((spin & 0x3FF) == 0 && *reinterpret_cast<volatile int*>(err))) { bad = true; break; }
                 }
                 if (bad) { atomicExch(err, 2); break; }
                 float scale, si;

@@ -587,3 +587,26 @@ def test_chain_config0_reports_metrics():
     mg, mo = oracle.metrics(to_np64(out), mean), oracle.metrics(want, mean)
     print("chain config0  gpu:", mg, " oracle:", mo)
     assert abs(mg["RelL2"] - mo["RelL2"]) < 0.02 * mo["RelL2"] and relfro(to_np64(out), want) < 0.02
+
+
+def test_rank_deficient_factor_with_zero_damping_stays_finite():
+    """Outside the paper's domain (S13): T < d samples, k above the factor's rank and damping = 0.  The refresh deflates
+    the dependent columns, rho and mu + lambda are floored, and the codec stays finite and invertible (no Inf / NaN multipliers)."""
+    m, n, k, T = 256, 256, 96, 64
+    ctx = gf8.create([gf8.Layer(m, n, gf8.SIDE_BOTH, k, k, gf8.E4M3, gf8.SCALE_TENSOR, 0.0)])
+    ctx.factor_update(0, synth.factor_samples(T, n, "cuda", 55, 1), synth.factor_samples(T, m, "cuda", 55, 2))
+    ctx.set_basis(0, gf8.SIDE_IN, synth.start_basis(n, k, "cuda", 55, 3))
+    ctx.set_basis(0, gf8.SIDE_OUT, synth.start_basis(m, k, "cuda", 55, 4))
+    ctx.refresh_basis(0, 3)
+    for side in (gf8.SIDE_IN, gf8.SIDE_OUT):
+        U, mu, rho = ctx.get_basis(0, side)
+        assert torch.isfinite(U).all() and torch.isfinite(mu).all() and np.isfinite(rho) and rho > 0
+        assert (mu[T:] <= 1e-6 * mu[0]).all()                 # the factor has rank T: the rest of the Ritz values are ~0
+    G = synth.gradient(m, n, "cuda", 56)
+    wt = ctx.whiten_f32(0, G)
+    assert torch.isfinite(wt).all()
+    c_, s_ = ctx.encode(0, G)
+    out = ctx.decode(0, c_, s_, dt=gf8.DT_F32)
+    # (rho -> 0 makes the model say the tail carries no curvature: the round trip is finite, not accurate -- the floor only
+    #  keeps the multipliers representable)
+    assert torch.isfinite(out).all()
