@@ -398,7 +398,7 @@ gf8_status fast_encode_many(gf8_ctx* c, int n, const int* layers, const void* co
                     f.out_map = pb.add_map(codes[i], mc);
                 }
             }
-            add_transform(pb, L, slot, src_map, src_lo_map, false, split, f);
+            add_transform(pb, L, slot, src_map, src_lo_map, false, split, f, c->opt);
         }
         if (s == GF8_OK) s = plan_finish(c, pb, p);
         if (s == GF8_OK) s = plan_store(c, key, p);
@@ -552,7 +552,7 @@ gf8_status fast_reduce_decoded_many(gf8_ctx* c, int n, const int* layers, const 
                 f.out_map = pb.add_map(outs[i], mo) + 1;           // 128-row boxes
             }
             // the unwhitening multipliers ebar = 1/D - 1 amplify operand rounding, so decode runs split products
-            add_transform(pb, L, slot, src_map, src_lo_map, true, true, f);
+            add_transform(pb, L, slot, src_map, src_lo_map, true, true, f, c->opt);
         }
         if (s == GF8_OK) s = plan_finish(c, pb, p);
         if (s == GF8_OK) s = plan_store(c, key, p);
@@ -729,6 +729,8 @@ gf8_status gf8_create(gf8_ctx** out, int device, const gf8_layer_desc* layers, i
     // MMAs, but a few 1e-4 of FP8 codes still flip, so the strict code-level gates (G3, G5's BF16 ulp) keep the SIMT path.
     c->tc_exact = precision == GF8_PREC_EXACT && getenv("GF8_EXACT_TC") != nullptr;
     c->use_stream = getenv("GF8_STREAM") != nullptr;
+    c->opt.nostrip = getenv("GF8_TC_NOSTRIP") != nullptr; c->opt.fuse = getenv("GF8_TC_FUSE") != nullptr;
+    c->opt.notri = getenv("GF8_TC_NOTRI") != nullptr; c->opt.static_items = getenv("GF8_TC_STATIC") != nullptr;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) c->num_sms = prop.multiProcessorCount;
     c->layers.resize(n_layers);

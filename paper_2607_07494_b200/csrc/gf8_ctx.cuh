@@ -68,7 +68,16 @@ struct RefreshScratch {
     double *V = nullptr, *Y = nullptr, *Gm = nullptr, *Bm = nullptr, *Zm = nullptr, *Zs = nullptr, *mu64 = nullptr;
 };
 
+// Engine switches, read ONCE from the environment in gf8_create (experiments / fall-backs; defaults are what bench.py times).
+struct EngineOptions {
+    bool nostrip = false;        // GF8_TC_NOSTRIP: update as 128 x 128 tile items instead of 256-row strips
+    bool fuse = false;           // GF8_TC_FUSE: single-pass update with W~ parked in TMEM (static round-robin; slower: DESIGN.md 5)
+    bool notri = false;          // GF8_TC_NOTRI: split products as three K-loops instead of interleaved per K-atom
+    bool static_items = false;   // GF8_TC_STATIC: static item assignment instead of the atomic hand-out
+};
+
 struct gf8_ctx {
+    EngineOptions opt;
     int device = 0;
     gf8_precision precision = GF8_PREC_EXACT;
     bool tc_exact = false;           // EXACT on the tensor-core engine with hi + lo operands (opt-in, GF8_EXACT_TC=1)

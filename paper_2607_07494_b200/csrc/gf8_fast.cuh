@@ -241,7 +241,7 @@ inline Item blank_item() {
 // expands to hi*hi + lo*hi + hi*lo, which brings the tensor-core result to ~FP32 accuracy at 3x the MMAs.
 // src_lo_map < 0 means the source is exactly BF16 (a BF16 gradient) and needs no residual.
 void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src_lo_map, bool inverse, bool split,
-                   const Final& f, int c_num_sms = 148) {
+                   const Final& f, const EngineOptions& opt, int c_num_sms = 148) {
     using namespace gf8::tc;
     const int m = L.desc.d_out, n = L.desc.d_in;
     const bool useA = L.in.used, useG = L.out.used;
@@ -347,7 +347,7 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
     // resident in shared memory and every B K-atom [U_A | Q'^T] serves both row blocks, which halves the bytes TMA has
     // to bring in per output tile (96 KB -> 48 KB) and amortises the per-item hand-shakes over 2 x n / 128 tiles.
     if (!split && kpA + kpG <= 128 && f.base_map[0] >= 0 && f.base_map[1] < 0 && f.out_map >= 0 &&
-        (f.mode == EPI_AMAX || f.mode == EPI_BLOCKCAST) && !getenv("GF8_TC_NOSTRIP") && !getenv("GF8_TC_FUSE")) {
+        (f.mode == EPI_AMAX || f.mode == EPI_BLOCKCAST) && !opt.nostrip && !opt.fuse) {
         for (int i0 = 0; i0 < m; i0 += 256) {
             Item it = blank_item();
             int seg = 0;
@@ -382,7 +382,7 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
             it.base_map[1] = f.base_map[1] >= 0 ? f.base_map[1] + 1 : -1;
             const int n_tiles = ((m + 127) / 128) * tiles_n;
             if (f.mode == EPI_AMAX && f.done && f.out_map >= 0 && it.base_map[0] >= 0 && n_tiles <= gf8::tc::FUSE_LAG * c_num_sms &&
-                getenv("GF8_TC_FUSE")) {
+                opt.fuse) {
                 // fused update (opt-in, GF8_TC_FUSE=1): one pass parks the FP32 tile in TMEM, the cast
                 // follows when the tensor amax is complete.  It needs every CTA of the launch co-resident.
                 it.amax = f.amax; it.out = f.out; it.out_ld = n; it.scale_inv_out = f.scale_inv; it.out_map = f.out_map;
@@ -497,7 +497,7 @@ gf8_status plan_finish(gf8_ctx* c, PlanBuilder& pb, Plan* p) {
             if (it.N > 64) p->stage_wide[s] |= 2;
         }
         if (!(p->stage_wide[s] & 1)) p->stage_wide[s] = 0;            // 0 none, 1 wide (B <= 8 KB), 3 wide with N = 128 items
-        bool all_tri = !pb.stage[s].empty() && !getenv("GF8_TC_NOTRI");
+        bool all_tri = !pb.stage[s].empty() && !c->opt.notri;
         for (const Item& it : pb.stage[s]) all_tri = all_tri && it.tri != 0;
         if (all_tri) p->stage_wide[s] = 5;                            // 5: every item interleaves its split products (kmode 5)
         else for (Item& it : pb.stage[s]) it.tri = 0;
@@ -542,12 +542,16 @@ gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
         const int fuse = s == 7 ? 1 : 0, strip = (s == 5 || s == 6) ? 1 : 0, wide = p->stage_wide[s] && !n_base ? 1 : 0;
         const int kmode = fuse ? 1 : (strip ? 2 : (wide ? (p->stage_wide[s] == 5 ? 5 : (p->stage_wide[s] == 3 ? 4 : 3)) : 0));
         // shared-memory split of the tile-mode update stages: 3 operand stages + the rest as base tiles in flight
-        int n_stages = n_base ? (strip ? 4 : 3) : (wide ? (p->stage_wide[s] == 5 ? 2 : (p->stage_wide[s] == 3 ? 4 : 5)) : gf8::tc::MAX_STAGES), dbg = 0, only = -1;
+        int n_stages = n_base ? (strip ? 4 : 3) : (wide ? (p->stage_wide[s] == 5 ? 2 : (p->stage_wide[s] == 3 ? 4 : 5)) : gf8::tc::MAX_STAGES), dbg = 0;
+#ifdef GF8_DEBUG
+        int only = -1;
+#endif
         // (strip stages: 64 KB of resident A tiles + 4 x 16 KB of B atoms = the first four 32 KB units, then 3 base slots)
         // (the fused stage gives one base slot's worth of shared memory to its two code-tile staging buffers)
         const int n_bslots = fuse ? 3 : (n_base ? std::max(1, (gf8::tc::MAX_STAGES - n_stages) / n_base) : 1);
         if (n_base && !fuse && n_stages + n_bslots * n_base > gf8::tc::MAX_STAGES) n_stages = gf8::tc::MAX_STAGES - n_bslots * n_base;
         if (fuse && grid < c->num_sms && p->stage_cnt[s] > grid) return fail(c, GF8_ERR_BAD_STATE, "fused stage needs a full grid");
+#ifdef GF8_DEBUG
         // GF8_TC_DBG (debug only, results are wrong with the ablation bits): 1 skip the MMAs, 2 skip the tensor-map
         // fences, 4 print a per-role wait profile, 32 skip the strip epilogue's work, 64 skip the strip base loads,
         // 128 skip the strip B loads, 256 print each stage's device time (serialises the stream)
@@ -571,9 +575,11 @@ gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
             cudaEventCreate(&a); cudaEventCreate(&b); cudaEventRecord(a, st);
             pend.push_back({s, {a, b}});
         }
+#endif
         gf8::tc::tc_items_kernel<<<grid, gf8::tc::THREADS, gf8::tc::SMEM_BYTES, st>>>(
             p->d_items + p->stage_off[s], p->stage_cnt[s], p->d_maps, c->d_err, n_stages, n_base, n_bslots, kmode, dbg, (dbg & 4) ? c->d_prof : nullptr,
-            (fuse || getenv("GF8_TC_STATIC")) ? nullptr : p->d_ctr + s);
+            (fuse || c->opt.static_items) ? nullptr : p->d_ctr + s);
+#ifdef GF8_DEBUG
         if (dbg & 512) cudaEventRecord(pend.back().second.second, st);
         if (dbg & 256) {                 // GF8_TC_DBG bit 8: per-stage device time (serialises the stream)
             float ms = 0;
@@ -591,6 +597,7 @@ gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
                 fprintf(stderr, "stage %d %-8s waits[0..2] %.0f %.0f %.0f  work %.0f  post %.0f  total %.0f cycles (avg/CTA)\n", s, roles[r], a[0], a[1], a[2], a[3], a[4], a[5]);
             }
         }
+#endif
         LAUNCH_CHECK(c);
     }
     return GF8_OK;

@@ -556,9 +556,18 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
 // so a pipeline bug cannot hang the GPU.
 __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __restrict__ items, int n_items,
                                                               const CUtensorMap* __restrict__ maps, int* err,
-                                                              int n_stages, int n_base, int n_bslots, int kmode, int dbg,
-                                                              long long* __restrict__ prof, int* ctr) {
+                                                              int n_stages, int n_base, int n_bslots, int kmode, int dbg_in,
+                                                              long long* __restrict__ prof_in, int* ctr) {
     extern __shared__ __align__(1024) uint8_t smem_raw[];
+#ifndef GF8_DEBUG
+    // (release builds: the ablation bits of `dbg_in` and the per-role wait profile are compiled out)
+    constexpr int dbg = 0;
+    constexpr long long* prof = nullptr;
+    (void)dbg_in; (void)prof_in;
+#else
+    const int dbg = dbg_in;
+    long long* const prof = prof_in;
+#endif
     const int fuse = kmode == 1 ? 1 : 0;           // kmode: 0 = tile items, 1 = fused update (TMEM-parked), 2 = strip items
     const bool strip = kmode == 2;
     // ctr != null: items are handed out dynamically (atomic counter, list order = start order), so item durations may

@@ -394,19 +394,30 @@ def test_fast_batched_call_with_euclidean_tensors_is_bit_exact_for_them():
 
 
 def test_fast_fused_update_matches_two_pass(monkeypatch):
-    """The opt-in fused update (W~ tiles parked in TMEM across the tensor-wide amax, GF8_TC_FUSE=1) produces the
-    same codes and scales as the default amax pass + cast pass."""
+    """The opt-in fused update (W~ tiles parked in TMEM across the tensor-wide amax, GF8_TC_FUSE=1 when the context is
+    created) produces the same codes and scales as the default amax pass + cast pass."""
     c = fcase("llama600m-q")
     gs = [c.rank_grad(r) for r in range(4)]
-    ref = [tuple(t.clone() for t in c.ctx.encode(0, g)) for g in gs]
-    monkeypatch.setenv("GF8_TC_FUSE", "1")
-    gs2 = [g.clone() for g in gs]                       # new pointers -> a new (fused) plan
-    codes = [torch.empty_like(ref[0][0]) for _ in gs2]
-    sinvs = [torch.empty_like(ref[0][1]) for _ in gs2]
-    c.ctx.encode_many([0] * len(gs2), gs2, codes, sinvs)
-    c.ctx.sync_check()
-    for r in range(len(gs2)):
-        assert torch.equal(codes[r], ref[r][0]) and torch.equal(sinvs[r], ref[r][1])
+
+    def fresh():
+        ctx = gf8.create([c.layer], gf8.PREC_FAST)
+        for side in (gf8.SIDE_IN, gf8.SIDE_OUT):
+            U, mu, rho = c.ctx.get_basis(0, side)
+            ctx.set_basis(0, side, U, mu, rho)
+        return ctx
+
+    outs = []
+    for fuse in (False, True):
+        if fuse:
+            monkeypatch.setenv("GF8_TC_FUSE", "1")
+        ctx = fresh()
+        codes = [torch.empty((c.m, c.n), dtype=torch.uint8, device="cuda") for _ in gs]
+        sinvs = [torch.empty(1, dtype=torch.float32, device="cuda") for _ in gs]
+        ctx.encode_many([0] * len(gs), gs, codes, sinvs)
+        ctx.sync_check()
+        outs.append((codes, sinvs))
+    for r in range(len(gs)):
+        assert torch.equal(outs[0][0][r], outs[1][0][r]) and torch.equal(outs[0][1][r], outs[1][1][r])
 
 
 @pytest.mark.parametrize("name", ["ragged-bf16", "wide-k96"])
