@@ -86,6 +86,13 @@ const char* gf8_last_error(const gf8_ctx* ctx);
 gf8_status gf8_sync_check(gf8_ctx* ctx, void* stream);
 /* Number of kernels this context has launched so far (bench.py's gpu_launches). */
 int64_t gf8_launch_count(const gf8_ctx* ctx);
+/* Per-launch timing of the tensor-core engine's stages, for roofline reporting (bench.py).  While enabled, every stage launch
+ * of a batched FAST call is bracketed by CUDA events on the call's stream (no host synchronisation is added).
+ * gf8_stage_times synchronises `stream`, then writes, for stage s in 0..7 (0 panels P' and Q^T, 1 S, 2 Q'^T, 3 / 4 update tiles
+ * (amax or store / cast), 5 / 6 update strips (amax / cast), 7 fused update), the summed device milliseconds and the number of
+ * launches since the last call, and resets the sums.  ms_out / n_out: HOST arrays of 8. */
+gf8_status gf8_set_stage_timing(gf8_ctx* ctx, int enable);
+gf8_status gf8_stage_times(gf8_ctx* ctx, float* ms_out_host, int* n_out_host, void* stream);
 
 /* ---- geometry state (every K steps) ------------------------------------------------ */
 /* a1.  A <- beta A + (1-beta) X^T X / T,  Gf likewise from Delta (Eq. 4).  The first

@@ -71,6 +71,7 @@ def _declare(L):
     _pi = C.POINTER(C.c_int64)
     L.gf8o_factor_entries.argtypes = [_pd, _i64, _i64, _pi, _pi, _i64, _pd]
     L.gf8o_whiten_samples.argtypes = [_pd, _i64, _i64, _pd, _pd, C.c_int, _pd, _pd, C.c_int, _pi, _pi, _i64, _pd]
+    L.gf8o_set_num_threads.argtypes = [C.c_int]
     L.gf8o_num_threads.restype = C.c_int
 
 
@@ -299,6 +300,10 @@ def metrics(ghat, g):
 
 def num_threads():
     return lib().gf8o_num_threads()
+
+
+def set_num_threads(n):
+    lib().gf8o_set_num_threads(int(n))
 
 
 # ---- whole-codec helpers (composition only; every step above is a C++ call) -----------------------

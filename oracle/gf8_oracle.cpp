@@ -497,6 +497,15 @@ void gf8o_whiten_samples(const double* W, int64_t m, int64_t n, const double* UG
     }
 }
 
+// Threads the OpenMP loops use from now on (bench.py's single-thread baseline figure); no effect without OpenMP.
+void gf8o_set_num_threads(int n) {
+#ifdef _OPENMP
+    if (n >= 1) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
 int gf8o_num_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

@@ -689,6 +689,29 @@ const char* gf8_status_string(gf8_status s) {
 const char* gf8_last_error(const gf8_ctx* ctx) { return ctx ? ctx->err : "null context"; }
 int64_t gf8_launch_count(const gf8_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
+gf8_status gf8_set_stage_timing(gf8_ctx* ctx, int enable) {
+    if (!ctx) return GF8_ERR_INVALID_ARG;
+    ctx->stage_timing = enable != 0;
+    return GF8_OK;
+}
+
+gf8_status gf8_stage_times(gf8_ctx* ctx, float* ms_out, int* n_out, void* stream) {
+    if (!ctx || !ms_out || !n_out) return GF8_ERR_INVALID_ARG;
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    CU_TRY(ctx, cudaStreamSynchronize((cudaStream_t)stream));
+    for (int s = 0; s < 8; ++s) { ms_out[s] = 0.0f; n_out[s] = 0; }
+    for (const gf8_ctx::StageEvent& e : ctx->stage_events) {
+        float ms = 0.0f;
+        CU_TRY(ctx, cudaEventSynchronize(e.b));
+        CU_TRY(ctx, cudaEventElapsedTime(&ms, e.a, e.b));
+        ms_out[e.stage] += ms;
+        n_out[e.stage] += 1;
+        ctx->stage_event_pool.push_back(e);
+    }
+    ctx->stage_events.clear();
+    return GF8_OK;
+}
+
 gf8_status gf8_sync_check(gf8_ctx* ctx, void* stream) {
     if (!ctx) return GF8_ERR_INVALID_ARG;
     CU_TRY(ctx, cudaSetDevice(ctx->device));
@@ -793,6 +816,8 @@ gf8_status gf8_destroy(gf8_ctx* ctx) {
     }
     if (ctx->rs_fork) cudaEventDestroy(ctx->rs_fork);
     if (ctx->aux_stream) { cudaStreamDestroy(ctx->aux_stream); cudaEventDestroy(ctx->aux_fork_ev); cudaEventDestroy(ctx->aux_join_ev); }
+    for (auto* v : {&ctx->stage_events, &ctx->stage_event_pool})
+        for (const gf8_ctx::StageEvent& e : *v) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
     for (Plan* p : ctx->plan_order) plan_free(p);
     for (SPlan* p : ctx->splans) splan_free(p);
     for (auto& kv : ctx->fac_plans) plan_free(kv.second);

@@ -114,6 +114,10 @@ struct gf8_ctx {
     void* encode_tiled = nullptr;    // cuTensorMapEncodeTiled, resolved at run time (no link-time libcuda)
     bool tc_attr_set = false;
     int64_t launches = 0;
+    // stage timing (gf8_set_stage_timing): event pairs recorded around stage launches, drained by gf8_stage_times
+    bool stage_timing = false;
+    struct StageEvent { int stage; cudaEvent_t a, b; };
+    std::vector<StageEvent> stage_events, stage_event_pool;
     int num_sms = 148;
     int aux_per_sm = 0;              // > 0: cap streaming grids at this many CTAs per SM (kernels that share SMs with the TC engine)
     char err[512] = {0};

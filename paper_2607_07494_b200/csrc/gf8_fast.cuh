@@ -576,9 +576,16 @@ gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
             pend.push_back({s, {a, b}});
         }
 #endif
+        gf8_ctx::StageEvent sev{s, nullptr, nullptr};
+        if (c->stage_timing) {
+            if (!c->stage_event_pool.empty()) { sev = c->stage_event_pool.back(); c->stage_event_pool.pop_back(); sev.stage = s; }
+            else { CU_TRY(c, cudaEventCreate(&sev.a)); CU_TRY(c, cudaEventCreate(&sev.b)); }
+            CU_TRY(c, cudaEventRecord(sev.a, st));
+        }
         gf8::tc::tc_items_kernel<<<grid, gf8::tc::THREADS, gf8::tc::SMEM_BYTES, st>>>(
             p->d_items + p->stage_off[s], p->stage_cnt[s], p->d_maps, c->d_err, n_stages, n_base, n_bslots, kmode, dbg, (dbg & 4) ? c->d_prof : nullptr,
             (fuse || c->opt.static_items) ? nullptr : p->d_ctr + s);
+        if (c->stage_timing) { CU_TRY(c, cudaEventRecord(sev.b, st)); c->stage_events.push_back(sev); }
 #ifdef GF8_DEBUG
         if (dbg & 512) cudaEventRecord(pend.back().second.second, st);
         if (dbg & 256) {                 // GF8_TC_DBG bit 8: per-stage device time (serialises the stream)

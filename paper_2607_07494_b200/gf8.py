@@ -23,7 +23,7 @@ MAX_RANK, MAX_R = 512, 64
 
 EXPORTS = [
     "gf8_create", "gf8_destroy", "gf8_payload_size", "gf8_status_string", "gf8_last_error", "gf8_launch_count",
-    "gf8_sync_check",
+    "gf8_sync_check", "gf8_set_stage_timing", "gf8_stage_times",
     "gf8_factor_update", "gf8_refresh_basis", "gf8_encode", "gf8_decode", "gf8_reduce_decoded",
     "gf8_encode_many", "gf8_reduce_decoded_many", "gf8_factor_update_many", "gf8_refresh_basis_many",
     "gf8_step_host", "gf8_get_factor", "gf8_set_factor", "gf8_get_basis", "gf8_set_basis",
@@ -81,6 +81,8 @@ def lib():
         L.gf8_launch_count.restype = i64
         L.gf8_launch_count.argtypes = [vp]
         L.gf8_sync_check.argtypes = [vp, vp]
+        L.gf8_set_stage_timing.argtypes = [vp, i32]
+        L.gf8_stage_times.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(i32), vp]
         L.gf8_factor_update.argtypes = [vp, i32, vp, vp, i64, i32, vp]
         L.gf8_refresh_basis.argtypes = [vp, i32, i32, vp]
         L.gf8_encode.argtypes = [vp, i32, vp, i32, vp, vp, vp]
@@ -185,6 +187,15 @@ class Ctx:
             self.destroy()
         except Exception:
             pass
+
+    def set_stage_timing(self, enable=True):
+        self._ck(lib().gf8_set_stage_timing(self._h, 1 if enable else 0))
+
+    def stage_times(self):
+        """(ms[8], launches[8]) of the tensor-core stages since the last call (synchronises the stream)."""
+        ms, n = (C.c_float * 8)(), (C.c_int * 8)()
+        self._ck(lib().gf8_stage_times(self._h, ms, n, _stream()))
+        return list(ms), list(n)
 
     def launch_count(self) -> int:
         return int(lib().gf8_launch_count(self._h))
