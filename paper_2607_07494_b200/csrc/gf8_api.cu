@@ -16,6 +16,7 @@ using namespace gf8;
 #include "gf8_ctx.cuh"
 #include "gf8_fast.cuh"
 #include "gf8_stream_host.cuh"
+#include "gf8_factor.cuh"
 
 namespace {
 
@@ -166,15 +167,6 @@ __global__ void split_kernel(const float* __restrict__ in, int64_t n, bf16* __re
     }
 }
 
-__global__ void fill_kernel(float* p, float v, int n) {
-    if ((int)threadIdx.x < n) p[threadIdx.x] = v;
-}
-// F <- beta F + C
-__global__ void axpby_kernel(float* __restrict__ F, const float* __restrict__ C, float beta, int64_t n) {
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
-        F[i] = fmaf(beta, F[i], C[i]);
-}
-
 __global__ void widen_kernel(const float* __restrict__ in, int64_t n, double* __restrict__ out) {
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
         out[i] = (double)in[i];
@@ -291,7 +283,7 @@ gf8_status reduce_decoded_one(gf8_ctx* c, int layer, const uint8_t* const* codes
 
 
 // ---- FAST path: batched calls through cached plans of tensor-core items ---------------------------------------
-enum { PLAN_ENCODE = 1, PLAN_DECODE = 2, PLAN_WHITEN = 3, PLAN_FACTOR = 4 };
+enum { PLAN_ENCODE = 1, PLAN_DECODE = 2, PLAN_WHITEN = 3 };
 
 inline void key_ptr(std::vector<uint64_t>& k, const void* p) { k.push_back((uint64_t)(uintptr_t)p); }
 
@@ -610,62 +602,55 @@ gf8_status fast_reduce_decoded_many(gf8_ctx* c, int n, const int* layers, const 
 }
 
 
-// ---- a1 on the tensor cores: C = alpha X^T X (d x d FP32) for BF16 samples X [T][d] (Eq. 4) -----------
-// Both MMA operands are MN-major views of X (64-row boxes): 128 x 128 output tiles, K = T streamed in 64-row atoms.
-// BF16 products are exact in FP32, so only the accumulation order differs from the FP32 reference (gate G6).
-gf8_status fast_factor_gemm(gf8_ctx* c, cudaStream_t st, const void* X, int64_t T, int d, float alpha, float beta,
-                            float* factor) {
-    using namespace gf8::tc;
+// ---- a1 on the tensor cores: F <- beta F + alpha X^T X (d x d FP32) for BF16 samples X [T][d] (Eq. 4) ----
+// One launch of gf8::fac::factor_gemm_kernel runs every job of a call (gf8_factor.cuh).  The job records (one tensor map
+// each) are built on the host and reach the device through two pinned / device buffer pairs used in turn, so the call
+// returns without waiting for the GPU; the buffers grow on demand and nothing else is allocated.
+struct FacReq { const void* X; int64_t T; int d; float alpha, beta; float* F; };
+
+gf8_status fast_factor_many(gf8_ctx* c, cudaStream_t st, const std::vector<FacReq>& reqs) {
+    using namespace gf8::fac;
+    if (reqs.empty()) return GF8_OK;
     GF_TRY(fast_init(c));
-    if (!c->fac_alpha) {
-        GF_TRY(dmalloc(c, &c->fac_alpha, 128));
+    if (!c->fac_attr_set) {
+        CU_TRY(c, cudaFuncSetAttribute(factor_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, F_SMEM));
+        for (int b = 0; b < 2; ++b) CU_TRY(c, cudaEventCreateWithFlags(&c->fac_ev[b], cudaEventDisableTiming));
+        c->fac_attr_set = true;
     }
-    if (beta != 0.0f && c->fac_tmp_cap < (size_t)d * d) {
-        GF_TRY(dmalloc(c, &c->fac_tmp, (size_t)d * d));
-        c->fac_tmp_cap = (size_t)d * d;
-    }
-    std::vector<uint64_t> key = {PLAN_FACTOR, (uint64_t)(uintptr_t)X, (uint64_t)T, (uint64_t)d,
-                                 (uint64_t)(uintptr_t)(beta != 0.0f ? c->fac_tmp : factor)};
-    // factor plans live in their own small cache: sample buffers change from refresh to refresh and must not
-    // evict the per-step encode / decode plans
-    Plan* p = nullptr;
-    auto found = c->fac_plans.find(key);
-    if (found != c->fac_plans.end()) p = found->second;
-    else {
-        p = new (std::nothrow) Plan();
-        if (!p) return fail(c, GF8_ERR_NOMEM, "host allocation failed");
-        PlanBuilder pb;
-        CUtensorMap mx[2];
-        gf8_status s = make_map(c, mx, X, (uint64_t)T, (uint64_t)d, (uint64_t)d);
-        if (s == GF8_OK) {
-            const int mi = pb.add_map(X, mx);
-            float* out = beta != 0.0f ? c->fac_tmp : factor;
-            for (int i0 = 0; i0 < d; i0 += 128)
-                for (int j0 = 0; j0 < d; j0 += 128) {
-                    Item it = blank_item();
-                    it.map_a[0] = mi; it.map_b[0] = mi; it.atoms[0] = (int)((T + 63) / 64);
-                    it.a_c0[0] = i0; it.b_c0[0] = j0; it.a_mn = 1; it.b_mn = 1; it.N = 128;
-                    it.mode = EPI_STORE; it.out = out; it.out_ld = d; it.out_type = TY_F32; it.colscale = c->fac_alpha;
-                    it.row0 = i0; it.col0 = j0; it.rows = std::min(128, d - i0); it.cols = std::min(128, d - j0);
-                    pb.stage[0].push_back(it);
-                }
-            s = plan_finish(c, pb, p);
+    const size_t n = reqs.size();
+    if (c->fac_cap < n) {
+        const size_t cap = std::max<size_t>(2 * c->fac_cap, std::max<size_t>(n, 32));
+        for (int b = 0; b < 2; ++b) {
+            if (c->fac_busy[b]) { CU_TRY(c, cudaEventSynchronize(c->fac_ev[b])); c->fac_busy[b] = false; }
+            if (c->fac_h[b]) { cudaFreeHost(c->fac_h[b]); c->fac_h[b] = nullptr; }
+            if (c->fac_d[b]) { cudaFree(c->fac_d[b]); c->fac_d[b] = nullptr; }
+            CU_TRY(c, cudaMallocHost(&c->fac_h[b], cap * sizeof(FactorJob)));
+            CU_TRY(c, cudaMalloc(&c->fac_d[b], cap * sizeof(FactorJob)));
         }
-        if (s != GF8_OK) { plan_free(p); return s; }
-        if (c->fac_plans.size() >= 32) {
-            CU_TRY(c, cudaDeviceSynchronize());
-            for (auto& kv : c->fac_plans) plan_free(kv.second);
-            c->fac_plans.clear();
-        }
-        c->fac_plans[key] = p;
+        c->fac_cap = cap;
     }
-    fill_kernel<<<1, 128, 0, st>>>(c->fac_alpha, alpha, 128);
+    const int b = c->fac_cur;
+    c->fac_cur ^= 1;
+    if (c->fac_busy[b]) { CU_TRY(c, cudaEventSynchronize(c->fac_ev[b])); c->fac_busy[b] = false; }
+    FactorJob* jobs = static_cast<FactorJob*>(c->fac_h[b]);
+    int tiles = 0;
+    for (size_t i = 0; i < n; ++i) {
+        const FacReq& r = reqs[i];
+        FactorJob& j = jobs[i];
+        memset(&j, 0, sizeof(j));
+        GF_TRY(make_map1(c, &j.map, r.X, (uint64_t)r.T, (uint64_t)r.d, (uint64_t)r.d, 64));
+        j.F = r.F; j.d = r.d; j.T = (int)r.T; j.alpha = r.alpha; j.beta = r.beta;
+        j.nI = (r.d + 127) / 128; j.nJ = (r.d + 255) / 256;
+        j.tile0 = tiles; j.n_tiles = factor_tiles(j.nI, j.nJ);
+        tiles += j.n_tiles;
+    }
+    CU_TRY(c, cudaMemcpyAsync(c->fac_d[b], jobs, n * sizeof(FactorJob), cudaMemcpyHostToDevice, st));
+    const int grid = std::min(tiles, c->num_sms);
+    factor_gemm_kernel<<<grid, F_THREADS, F_SMEM, st>>>(static_cast<const FactorJob*>(c->fac_d[b]), (int)n, tiles, c->d_err);
     LAUNCH_CHECK(c);
-    GF_TRY(plan_run_stages(c, st, p));
-    if (beta != 0.0f) {
-        axpby_kernel<<<grid_for(c, (int64_t)d * d, 256, 8), 256, 0, st>>>(factor, c->fac_tmp, beta, (int64_t)d * d);
-        LAUNCH_CHECK(c);
-    }
+    ++c->launches;
+    CU_TRY(c, cudaEventRecord(c->fac_ev[b], st));
+    c->fac_busy[b] = true;
     return GF8_OK;
 }
 
@@ -820,7 +805,11 @@ gf8_status gf8_destroy(gf8_ctx* ctx) {
         for (const gf8_ctx::StageEvent& e : *v) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
     for (Plan* p : ctx->plan_order) plan_free(p);
     for (SPlan* p : ctx->splans) splan_free(p);
-    for (auto& kv : ctx->fac_plans) plan_free(kv.second);
+    for (int b = 0; b < 2; ++b) {
+        if (ctx->fac_h[b]) cudaFreeHost(ctx->fac_h[b]);
+        if (ctx->fac_d[b]) cudaFree(ctx->fac_d[b]);
+        if (ctx->fac_ev[b]) cudaEventDestroy(ctx->fac_ev[b]);
+    }
     for (LayerState& L : ctx->layers)
         for (Slot* sl : L.slots) delete sl;
     delete ctx;
@@ -836,37 +825,59 @@ gf8_status gf8_payload_size(const gf8_ctx* ctx, int layer, size_t* code_bytes, s
 }
 
 // ---- a1 ---------------------------------------------------------------------------------------------------
+namespace {
+// All factor updates of a call: the arguments of every problem are checked first; BF16 samples of sides with d >= 128 then
+// go to the tensor-core kernel as ONE launch (a batch ends early where a layer repeats, so no factor is written twice by one
+// launch), everything else to the FP32 SIMT GEMM.
+gf8_status factor_update_impl(gf8_ctx* ctx, int n, const int* layers, const void* const* acts, const void* const* gouts,
+                              const int64_t* T, gf8_dtype dt, cudaStream_t st) {
+    if (dt != GF8_DT_BF16 && dt != GF8_DT_F32) return fail(ctx, GF8_ERR_INVALID_ARG, "bad dtype");
+    for (int i = 0; i < n; ++i) {
+        GF_TRY(check_layer(ctx, layers[i]));
+        const LayerState& L = ctx->layers[layers[i]];
+        if (T[i] < 1 || T[i] > 0x7FFFFFFF) return fail(ctx, GF8_ERR_INVALID_ARG, "T out of range");
+        if ((acts[i] && !aligned16(acts[i])) || (gouts[i] && !aligned16(gouts[i])))
+            return fail(ctx, GF8_ERR_UNSUPPORTED, "pointers must be 16-byte aligned");
+        if (L.in.used && !acts[i]) return fail(ctx, GF8_ERR_INVALID_ARG, "layer %d whitens the input side: act required", layers[i]);
+        if (L.out.used && !gouts[i]) return fail(ctx, GF8_ERR_INVALID_ARG, "layer %d whitens the output side: gout required", layers[i]);
+    }
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    std::vector<FacReq> batch;
+    std::vector<int> in_batch;
+    for (int i = 0; i < n; ++i) {
+        LayerState& L = ctx->layers[layers[i]];
+        if (std::find(in_batch.begin(), in_batch.end(), layers[i]) != in_batch.end()) {
+            GF_TRY(fast_factor_many(ctx, st, batch));
+            batch.clear(); in_batch.clear();
+        }
+        in_batch.push_back(layers[i]);
+        for (int sidx = 0; sidx < 2; ++sidx) {
+            SideState& s = sidx == 0 ? L.in : L.out;
+            const void* X = sidx == 0 ? acts[i] : gouts[i];
+            if (!s.used) continue;
+            GF_TRY(ensure_factor(ctx, s));
+            const float beta = s.has_factor ? L.desc.ema_beta : 0.0f;
+            const float alpha = (1.0f - beta) / (float)T[i];
+            const int d = s.d;
+            if (dt == GF8_DT_BF16 && (ctx->precision == GF8_PREC_FAST || ctx->tc_exact) && d >= 128 && d % 8 == 0)
+                batch.push_back(FacReq{X, T[i], d, alpha, beta, s.factor});
+            else if (dt == GF8_DT_BF16)
+                GF_TRY((launch_gemm<bf16, bf16, float, float>(ctx, st, (const bf16*)X, 1, d, (const bf16*)X, d, 1, s.factor,
+                                                              d, d, d, (int)T[i], nullptr, nullptr, alpha, beta)));
+            else
+                GF_TRY((launch_gemm<float, float, float, float>(ctx, st, (const float*)X, 1, d, (const float*)X, d, 1,
+                                                                s.factor, d, d, d, (int)T[i], nullptr, nullptr, alpha, beta)));
+            s.has_factor = true;
+        }
+    }
+    return fast_factor_many(ctx, st, batch);
+}
+}  // namespace
+
 gf8_status gf8_factor_update(gf8_ctx* ctx, int layer, const void* act, const void* gout, int64_t T, gf8_dtype dt,
                              void* stream) {
-    GF_TRY(check_layer(ctx, layer));
-    LayerState& L = ctx->layers[layer];
-    cudaStream_t st = (cudaStream_t)stream;
-    if (T < 1 || T > 0x7FFFFFFF) return fail(ctx, GF8_ERR_INVALID_ARG, "T out of range");
-    if (dt != GF8_DT_BF16 && dt != GF8_DT_F32) return fail(ctx, GF8_ERR_INVALID_ARG, "bad dtype");
-    if ((act && !aligned16(act)) || (gout && !aligned16(gout)))
-        return fail(ctx, GF8_ERR_UNSUPPORTED, "pointers must be 16-byte aligned");
-    if (L.in.used && !act) return fail(ctx, GF8_ERR_INVALID_ARG, "layer %d whitens the input side: act required", layer);
-    if (L.out.used && !gout) return fail(ctx, GF8_ERR_INVALID_ARG, "layer %d whitens the output side: gout required", layer);
-    CU_TRY(ctx, cudaSetDevice(ctx->device));
-    for (int sidx = 0; sidx < 2; ++sidx) {
-        SideState& s = sidx == 0 ? L.in : L.out;
-        const void* X = sidx == 0 ? act : gout;
-        if (!s.used) continue;
-        GF_TRY(ensure_factor(ctx, s));
-        const float beta = s.has_factor ? L.desc.ema_beta : 0.0f;
-        const float alpha = (1.0f - beta) / (float)T;
-        const int d = s.d;
-        if (dt == GF8_DT_BF16 && (ctx->precision == GF8_PREC_FAST || ctx->tc_exact) && d >= 128)
-            GF_TRY(fast_factor_gemm(ctx, st, X, T, d, alpha, beta, s.factor));
-        else if (dt == GF8_DT_BF16)
-            GF_TRY((launch_gemm<bf16, bf16, float, float>(ctx, st, (const bf16*)X, 1, d, (const bf16*)X, d, 1, s.factor,
-                                                          d, d, d, (int)T, nullptr, nullptr, alpha, beta)));
-        else
-            GF_TRY((launch_gemm<float, float, float, float>(ctx, st, (const float*)X, 1, d, (const float*)X, d, 1,
-                                                            s.factor, d, d, d, (int)T, nullptr, nullptr, alpha, beta)));
-        s.has_factor = true;
-    }
-    return GF8_OK;
+    if (!ctx) return GF8_ERR_INVALID_ARG;
+    return factor_update_impl(ctx, 1, &layer, &act, &gout, &T, dt, (cudaStream_t)stream);
 }
 
 // ---- a2 ---------------------------------------------------------------------------------------------------
@@ -951,8 +962,7 @@ gf8_status gf8_factor_update_many(gf8_ctx* ctx, int n, const int* layers, const 
                                   const void* const* gouts, const int64_t* T, gf8_dtype dt, void* stream) {
     if (!ctx) return GF8_ERR_INVALID_ARG;
     if (n < 0 || !layers || !acts || !gouts || !T) return fail(ctx, GF8_ERR_INVALID_ARG, "null argument");
-    for (int i = 0; i < n; ++i) GF_TRY(gf8_factor_update(ctx, layers[i], acts[i], gouts[i], T[i], dt, stream));
-    return GF8_OK;
+    return factor_update_impl(ctx, n, layers, acts, gouts, T, dt, (cudaStream_t)stream);
 }
 
 gf8_status gf8_refresh_basis_many(gf8_ctx* ctx, int n, const int* layers, int n_iter, void* stream) {

@@ -102,14 +102,18 @@ struct gf8_ctx {
     // FAST path: cached launch plans (device item lists + tensor maps), error flag, driver entry point
     std::map<std::vector<uint64_t>, struct Plan*> plans;
     std::vector<struct Plan*> plan_order;
-    std::map<std::vector<uint64_t>, struct Plan*> fac_plans;   // factor-GEMM plans (keyed by the sample buffer)
     std::vector<struct SPlan*> splans;                          // streaming-engine plans (keyed by the layer list of a call)
     bool stream_attr_set = false;
     bool use_stream = false;         // streaming engine (gf8_stream.cuh) instead of the staged item engine for the shapes it takes
     int* d_err = nullptr;
-    float* fac_alpha = nullptr;      // 128 copies of the factor GEMM's scale (its epilogue's column multipliers)
-    float* fac_tmp = nullptr;        // d x d scratch of the EMA form of the factor update
-    size_t fac_tmp_cap = 0;
+    // factor GEMM (gf8_factor.cuh): job records of a call, staged through two pinned / device buffer pairs
+    void* fac_h[2] = {nullptr, nullptr};
+    void* fac_d[2] = {nullptr, nullptr};
+    cudaEvent_t fac_ev[2] = {nullptr, nullptr};
+    bool fac_busy[2] = {false, false};
+    size_t fac_cap = 0;              // job records per buffer
+    int fac_cur = 0;
+    bool fac_attr_set = false;
     long long* d_prof = nullptr;     // debug profile of the TC kernel (GF8_TC_DBG & 4)
     void* encode_tiled = nullptr;    // cuTensorMapEncodeTiled, resolved at run time (no link-time libcuda)
     bool tc_attr_set = false;

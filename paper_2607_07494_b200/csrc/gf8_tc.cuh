@@ -112,12 +112,12 @@ __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
 // Bounded spin: a broken pipeline sets *err and lets the kernel drain instead of hanging the GPU.
 __device__ __forceinline__ bool mbar_wait(uint32_t bar, uint32_t parity, int* err) {
     uint32_t done = 0;
-    for (uint32_t spin = 0; spin < (1u << 20); ++spin) {      // (each try sleeps up to 2 us: ~2 s in all)
+    for (uint32_t spin = 0; spin < (1u << 26); ++spin) {
         asm volatile(
             "{\n\t.reg .pred p;\n\t"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
             "selp.u32 %0, 1, 0, p;\n\t}"
-            : "=r"(done) : "r"(bar), "r"(parity), "r"(2000u) : "memory");      // (suspend-time hint, ns: a waiting warp sleeps instead of spinning)
+            : "=r"(done) : "r"(bar), "r"(parity) : "memory");
         if (done) return true;
         if ((spin & 0xFFFF) == 0xFFFF && *(volatile int*)err) return false;
     }
