@@ -188,9 +188,16 @@ gf8_status orthonormalise(gf8_ctx* c, cudaStream_t st, RefreshScratch& rs, doubl
     for (int pass = 0; pass < 2; ++pass) {
         GF_TRY((launch_gemm<double, double, double, double>(c, st, V, 1, k, V, k, 1, rs.Gm, k, k, k, d, nullptr, nullptr,
                                                             1.0, 0.0, pick_splits(c, k, k, d))));
-        cholesky_upper_kernel<<<1, 1024, 0, st>>>(rs.Gm, k);
+        const size_t chol_smem = (size_t)k * (k | 1) * sizeof(double);
+        const int chol_in_smem = chol_smem <= 200 * 1024 ? 1 : 0;
+        if (chol_in_smem && chol_smem > c->chol_smem_set) {
+            CU_TRY(c, cudaFuncSetAttribute(cholesky_upper_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)chol_smem));
+            c->chol_smem_set = chol_smem;
+        }
+        cholesky_upper_kernel<<<1, 1024, chol_in_smem ? chol_smem : 0, st>>>(rs.Gm, k, chol_in_smem);
         LAUNCH_CHECK(c);
-        trisolve_rows_kernel<<<(d + 127) / 128, 128, 0, st>>>(V, rs.Gm, d, k);
+        if (k <= TRI_MAXK) trisolve_rows_warp_kernel<<<(d + TRI_ROWS * TRI_WARPS - 1) / (TRI_ROWS * TRI_WARPS), 32 * TRI_WARPS, 0, st>>>(V, rs.Gm, d, k);
+        else trisolve_rows_kernel<<<(d + 127) / 128, 128, 0, st>>>(V, rs.Gm, d, k);
         LAUNCH_CHECK(c);
     }
     return GF8_OK;
@@ -215,9 +222,12 @@ gf8_status refresh_side(gf8_ctx* c, cudaStream_t st, RefreshScratch& rs, SideSta
                                                        1.0, 0.0, pick_splits(c, d, k, d))));
     GF_TRY((launch_gemm<double, double, double, double>(c, st, V, 1, k, Y, k, 1, rs.Bm, k, k, k, d, nullptr, nullptr,
                                                         1.0, 0.0, pick_splits(c, k, k, d))));
-    const size_t smem = 2 * (size_t)k * k * sizeof(double);
+    const size_t smem = 2 * (size_t)k * (k | 1) * sizeof(double);
     const int use_smem = smem <= 200 * 1024 ? 1 : 0;
-    if (use_smem) CU_TRY(c, cudaFuncSetAttribute(jacobi_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (use_smem && smem > c->jacobi_smem_set) {
+        CU_TRY(c, cudaFuncSetAttribute(jacobi_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        c->jacobi_smem_set = smem;
+    }
     jacobi_kernel<<<1, 1024, use_smem ? smem : 0, st>>>(rs.Bm, rs.Zm, k, use_smem, rs.mu64, rs.Zs, 60);
     LAUNCH_CHECK(c);
     // U = V Zs (FP32 out)

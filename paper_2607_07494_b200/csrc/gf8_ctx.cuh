@@ -114,6 +114,7 @@ struct gf8_ctx {
     size_t fac_cap = 0;              // job records per buffer
     int fac_cur = 0;
     bool fac_attr_set = false;
+    size_t chol_smem_set = 0, jacobi_smem_set = 0;   // dynamic shared memory sizes the refresh kernels are opted in to
     long long* d_prof = nullptr;     // debug profile of the TC kernel (GF8_TC_DBG & 4)
     void* encode_tiled = nullptr;    // cuTensorMapEncodeTiled, resolved at run time (no link-time libcuda)
     bool tc_attr_set = false;
