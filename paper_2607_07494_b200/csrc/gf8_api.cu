@@ -17,6 +17,7 @@ using namespace gf8;
 #include "gf8_fast.cuh"
 #include "gf8_stream_host.cuh"
 #include "gf8_factor.cuh"
+#include "gf8_refresh.cuh"
 
 namespace {
 
@@ -196,7 +197,7 @@ gf8_status orthonormalise(gf8_ctx* c, cudaStream_t st, RefreshScratch& rs, doubl
         }
         cholesky_upper_kernel<<<1, 1024, chol_in_smem ? chol_smem : 0, st>>>(rs.Gm, k, chol_in_smem);
         LAUNCH_CHECK(c);
-        if (k <= TRI_MAXK) trisolve_rows_warp_kernel<<<(d + TRI_ROWS * TRI_WARPS - 1) / (TRI_ROWS * TRI_WARPS), 32 * TRI_WARPS, 0, st>>>(V, rs.Gm, d, k);
+        if (k <= TRI_MAXK) trisolve_rows_warp_kernel<<<(d + TRI_ROWS * TRI_WARPS * TRI_GROUPS - 1) / (TRI_ROWS * TRI_WARPS * TRI_GROUPS), 32 * TRI_WARPS, 0, st>>>(V, rs.Gm, d, k);
         else trisolve_rows_kernel<<<(d + 127) / 128, 128, 0, st>>>(V, rs.Gm, d, k);
         LAUNCH_CHECK(c);
     }
@@ -805,11 +806,9 @@ gf8_status gf8_destroy(gf8_ctx* ctx) {
     cudaDeviceSynchronize();
     for (void* p : ctx->allocs) cudaFree(p);
     for (void* p : ctx->stage_allocs) cudaFree(p);
-    for (int q = 0; q < GF8_REFRESH_STREAMS; ++q) {
-        if (ctx->rs_stream[q]) cudaStreamDestroy(ctx->rs_stream[q]);
-        if (ctx->rs_ev[q]) cudaEventDestroy(ctx->rs_ev[q]);
-    }
-    if (ctx->rs_fork) cudaEventDestroy(ctx->rs_fork);
+    if (ctx->rb_arena) cudaFree(ctx->rb_arena);
+    if (ctx->rb_jobs) cudaFree(ctx->rb_jobs);
+    if (ctx->rb_ev) cudaEventDestroy(ctx->rb_ev);
     if (ctx->aux_stream) { cudaStreamDestroy(ctx->aux_stream); cudaEventDestroy(ctx->aux_fork_ev); cudaEventDestroy(ctx->aux_join_ev); }
     for (auto* v : {&ctx->stage_events, &ctx->stage_event_pool})
         for (const gf8_ctx::StageEvent& e : *v) { cudaEventDestroy(e.a); cudaEventDestroy(e.b); }
@@ -892,13 +891,7 @@ gf8_status gf8_factor_update(gf8_ctx* ctx, int layer, const void* act, const voi
 
 // ---- a2 ---------------------------------------------------------------------------------------------------
 gf8_status gf8_refresh_basis(gf8_ctx* ctx, int layer, int n_iter, void* stream) {
-    GF_TRY(check_layer(ctx, layer));
-    if (n_iter < 0 || n_iter > 1000) return fail(ctx, GF8_ERR_INVALID_ARG, "n_iter out of range");
-    LayerState& L = ctx->layers[layer];
-    CU_TRY(ctx, cudaSetDevice(ctx->device));
-    if (L.in.used) GF_TRY(refresh_side(ctx, (cudaStream_t)stream, ctx->rs[0], L.in, (double)L.desc.damping, n_iter, layer));
-    if (L.out.used) GF_TRY(refresh_side(ctx, (cudaStream_t)stream, ctx->rs[0], L.out, (double)L.desc.damping, n_iter, layer));
-    return GF8_OK;
+    return gf8_refresh_basis_many(ctx, 1, &layer, n_iter, stream);
 }
 
 // ---- codec ------------------------------------------------------------------------------------------------
@@ -975,39 +968,152 @@ gf8_status gf8_factor_update_many(gf8_ctx* ctx, int n, const int* layers, const 
     return factor_update_impl(ctx, n, layers, acts, gouts, T, dt, (cudaStream_t)stream);
 }
 
+namespace {
+// One batch of sides (no side twice) through the batched refresh kernels (gf8_refresh.cuh): every step is one launch.
+gf8_status refresh_batch(gf8_ctx* c, cudaStream_t st, const std::vector<SideState*>& sides, const std::vector<double>& lams,
+                         int n_iter) {
+    using namespace gf8::rb;
+    const int n = (int)sides.size();
+    if (!n) return GF8_OK;
+    GF_TRY(fast_init(c));
+    if (!c->rb_ev) {
+        CU_TRY(c, cudaEventCreateWithFlags(&c->rb_ev, cudaEventDisableTiming));
+        const int jac_smem = 2 * RB_MAXK * (RB_MAXK | 1) * (int)sizeof(double);
+        CU_TRY(c, cudaFuncSetAttribute(rb_jacobi_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, jac_smem));
+        CU_TRY(c, cudaFuncSetAttribute(rb_av_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, AV_SMEM));
+        CU_TRY(c, cudaFuncSetAttribute(rb_rightmul_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, RM_SMEM));
+    }
+    // scratch arena: per side V, Y (d x k), the partial products, four k x k matrices and mu64
+    auto al = [](size_t x) { return (x + 31) & ~size_t(31); };      // (in doubles: 256 B granules)
+    size_t total = 0;
+    std::vector<size_t> off(n);
+    std::vector<RefreshJob> jobs(n);
+    int blocks = 0, max_d = 0, max_chunks = 0;
+    for (int i = 0; i < n; ++i) {
+        const SideState& s = *sides[i];
+        const size_t dk = al((size_t)s.d * s.k), kk = al((size_t)s.k * s.k);
+        const int chunks = (s.d + RB_CHUNK - 1) / RB_CHUNK;
+        off[i] = total;
+        total += 2 * dk + (size_t)chunks * kk + 4 * kk + al(s.k);
+        max_d = std::max(max_d, s.d);
+        max_chunks = std::max(max_chunks, chunks);
+    }
+    if (c->rb_busy) { CU_TRY(c, cudaEventSynchronize(c->rb_ev)); c->rb_busy = false; }
+    if (c->rb_arena_cap < total) {
+        if (c->rb_arena) CU_TRY(c, cudaFree(c->rb_arena));
+        c->rb_arena = nullptr; c->rb_arena_cap = 0;
+        CU_TRY(c, cudaMalloc((void**)&c->rb_arena, total * sizeof(double)));
+        c->rb_arena_cap = total;
+    }
+    if (c->rb_jobs_cap < (size_t)n) {
+        if (c->rb_jobs) CU_TRY(c, cudaFree(c->rb_jobs));
+        c->rb_jobs = nullptr; c->rb_jobs_cap = 0;
+        CU_TRY(c, cudaMalloc(&c->rb_jobs, (size_t)n * sizeof(RefreshJob)));
+        c->rb_jobs_cap = (size_t)n;
+    }
+    for (int i = 0; i < n; ++i) {
+        SideState& s = *sides[i];
+        const size_t dk = al((size_t)s.d * s.k), kk = al((size_t)s.k * s.k);
+        const int chunks = (s.d + RB_CHUNK - 1) / RB_CHUNK;
+        double* p = c->rb_arena + off[i];
+        RefreshJob& j = jobs[i];
+        j.factor = s.factor; j.U = s.U;
+        j.buf[0] = p; p += dk;
+        j.buf[1] = p; p += dk;
+        j.part = p; p += (size_t)chunks * kk;
+        j.Gm = p; p += kk;
+        j.Bm = p; p += kk;
+        j.Zm = p; p += kk;
+        j.Zs = p; p += kk;
+        j.mu64 = p;
+        j.mu = s.mu; j.e = s.e; j.ebar = s.ebar; j.rho = s.rho;
+        j.lam = lams[i]; j.d = s.d; j.k = s.k; j.blk0 = blocks; j.n_chunks = chunks;
+        blocks += (s.d + AV_BM - 1) / AV_BM;
+    }
+    // (pageable source: the runtime stages the records before the call returns)
+    CU_TRY(c, cudaMemcpyAsync(c->rb_jobs, jobs.data(), (size_t)n * sizeof(RefreshJob), cudaMemcpyHostToDevice, st));
+    const RefreshJob* dj = static_cast<const RefreshJob*>(c->rb_jobs);
+    int flip = 0;
+    auto orthonormalise_all = [&]() -> gf8_status {
+        for (int pass = 0; pass < 2; ++pass) {
+            rb_gram_kernel<<<dim3(max_chunks, n), 256, 0, st>>>(dj, flip, flip);
+            LAUNCH_CHECK(c);
+            rb_sum_kernel<<<dim3(4, n), 256, 0, st>>>(dj, 0);
+            LAUNCH_CHECK(c);
+            rb_chol_kernel<<<n, 1024, RB_MAXK * (RB_MAXK | 1) * sizeof(double), st>>>(dj);
+            LAUNCH_CHECK(c);
+            rb_rightmul_kernel<<<dim3((max_d + 63) / 64, n), 256, RM_SMEM, st>>>(dj, flip, 0);
+            LAUNCH_CHECK(c);
+        }
+        return GF8_OK;
+    };
+    rb_widen_kernel<<<dim3(32, n), 256, 0, st>>>(dj, flip);
+    LAUNCH_CHECK(c);
+    GF_TRY(orthonormalise_all());
+    for (int it = 0; it < n_iter; ++it) {
+        rb_av_kernel<<<blocks, 256, AV_SMEM, st>>>(dj, n, flip);
+        LAUNCH_CHECK(c);
+        flip ^= 1;
+        GF_TRY(orthonormalise_all());
+    }
+    // Rayleigh-Ritz: Y = A V, B = V^T Y, eigensolve, U = V Z
+    rb_av_kernel<<<blocks, 256, AV_SMEM, st>>>(dj, n, flip);
+    LAUNCH_CHECK(c);
+    rb_gram_kernel<<<dim3(max_chunks, n), 256, 0, st>>>(dj, flip, flip ^ 1);
+    LAUNCH_CHECK(c);
+    rb_sum_kernel<<<dim3(4, n), 256, 0, st>>>(dj, 1);
+    LAUNCH_CHECK(c);
+    rb_jacobi_kernel<<<n, 1024, 2 * RB_MAXK * (RB_MAXK | 1) * sizeof(double), st>>>(dj, 60);
+    LAUNCH_CHECK(c);
+    rb_rightmul_kernel<<<dim3((max_d + 63) / 64, n), 256, RM_SMEM, st>>>(dj, flip, 1);
+    LAUNCH_CHECK(c);
+    rb_multipliers_kernel<<<n, 256, 0, st>>>(dj);
+    LAUNCH_CHECK(c);
+    CU_TRY(c, cudaEventRecord(c->rb_ev, st));
+    c->rb_busy = true;
+    for (SideState* s : sides) {
+        GF_TRY(fast_pack_basis(c, st, *s));
+        s->has_basis = true;
+    }
+    return GF8_OK;
+}
+}  // namespace
+
 gf8_status gf8_refresh_basis_many(gf8_ctx* ctx, int n, const int* layers, int n_iter, void* stream) {
     if (!ctx) return GF8_ERR_INVALID_ARG;
     if (n < 0 || !layers) return fail(ctx, GF8_ERR_INVALID_ARG, "null argument");
     if (n_iter < 0 || n_iter > 1000) return fail(ctx, GF8_ERR_INVALID_ARG, "n_iter out of range");
-    for (int i = 0; i < n; ++i) GF_TRY(check_layer(ctx, layers[i]));
-    CU_TRY(ctx, cudaSetDevice(ctx->device));
-    // The refresh of one factor is a chain of small, latency-bound launches (CholeskyQR, a single-CTA Jacobi, skinny
-    // products): independent factors run concurrently on the context's side streams, each with its own scratch.
-    cudaStream_t st = (cudaStream_t)stream;
-    if (!ctx->rs_ev[0]) {
-        for (int q = 0; q < GF8_REFRESH_STREAMS; ++q) {
-            CU_TRY(ctx, cudaStreamCreateWithFlags(&ctx->rs_stream[q], cudaStreamNonBlocking));
-            CU_TRY(ctx, cudaEventCreateWithFlags(&ctx->rs_ev[q], cudaEventDisableTiming));
-        }
-        CU_TRY(ctx, cudaEventCreateWithFlags(&ctx->rs_fork, cudaEventDisableTiming));
-    }
-    for (int q = 0; q < GF8_REFRESH_STREAMS; ++q) GF_TRY(alloc_refresh_scratch(ctx, ctx->rs[q]));
-    CU_TRY(ctx, cudaEventRecord(ctx->rs_fork, st));
-    for (int q = 0; q < GF8_REFRESH_STREAMS; ++q) CU_TRY(ctx, cudaStreamWaitEvent(ctx->rs_stream[q], ctx->rs_fork, 0));
-    int job = 0;
+    // every argument is checked before the first launch
     for (int i = 0; i < n; ++i) {
+        GF_TRY(check_layer(ctx, layers[i]));
         LayerState& L = ctx->layers[layers[i]];
         for (SideState* sd : {&L.in, &L.out}) {
             if (!sd->used) continue;
-            const int q = job++ % GF8_REFRESH_STREAMS;
-            GF_TRY(refresh_side(ctx, ctx->rs_stream[q], ctx->rs[q], *sd, (double)L.desc.damping, n_iter, layers[i]));
+            if (!sd->has_factor) return fail(ctx, GF8_ERR_BAD_STATE, "layer %d: no factor accumulated yet", layers[i]);
+            if (!sd->has_start) return fail(ctx, GF8_ERR_BAD_STATE, "layer %d: no start basis (gf8_set_basis first)", layers[i]);
         }
     }
-    for (int q = 0; q < GF8_REFRESH_STREAMS; ++q) {
-        CU_TRY(ctx, cudaEventRecord(ctx->rs_ev[q], ctx->rs_stream[q]));
-        CU_TRY(ctx, cudaStreamWaitEvent(st, ctx->rs_ev[q], 0));
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    // Sides of rank <= 64 go through the batched kernels, one launch per step of the algorithm over all of them (a batch ends
+    // early where a layer repeats); the others walk the per-side chain on the same stream.
+    std::vector<SideState*> batch;
+    std::vector<double> lams;
+    std::vector<int> seen;
+    for (int i = 0; i < n; ++i) {
+        LayerState& L = ctx->layers[layers[i]];
+        if (std::find(seen.begin(), seen.end(), layers[i]) != seen.end()) {
+            GF_TRY(refresh_batch(ctx, st, batch, lams, n_iter));
+            batch.clear(); lams.clear(); seen.clear();
+        }
+        seen.push_back(layers[i]);
+        for (SideState* sd : {&L.in, &L.out}) {
+            if (!sd->used) continue;
+            if (sd->k <= gf8::rb::RB_MAXK) { batch.push_back(sd); lams.push_back((double)L.desc.damping); }
+            else GF_TRY(refresh_side(ctx, st, ctx->rs[0], *sd, (double)L.desc.damping, n_iter, layers[i]));
+        }
     }
-    return GF8_OK;
+    return refresh_batch(ctx, st, batch, lams, n_iter);
 }
 
 // ---- end-to-end with host buffers -----------------------------------------------------------------------------

@@ -10,7 +10,7 @@ namespace gf8 {
 // G row-major in global memory (k <= 512); only the upper triangle is read and written.  With use_smem the matrix is staged in
 // dynamic shared memory (k * (k | 1) doubles: an odd leading dimension keeps column walks off one bank), which turns the
 // three global round trips of every pivot step into shared-memory ones.
-__global__ void __launch_bounds__(1024) cholesky_upper_kernel(double* __restrict__ Gg, int k, int use_smem) {
+__device__ __forceinline__ void cholesky_upper_body(double* __restrict__ Gg, int k, int use_smem) {
     extern __shared__ double s_chol[];
     __shared__ double s_diag, s_dmax;
     const int ld = use_smem ? (k | 1) : k;
@@ -70,42 +70,53 @@ __global__ void __launch_bounds__(1024) cholesky_upper_kernel(double* __restrict
     }
 }
 
+__global__ void __launch_bounds__(1024) cholesky_upper_kernel(double* __restrict__ Gg, int k, int use_smem) {
+    cholesky_upper_body(Gg, k, use_smem);
+}
+
 // ---- V <- V R^-1 (R upper triangular), V d x k FP64, in place -------------------------------------------
 // Row by row x R = v, column-oriented: once x_j = v_j / R_jj is known, v_l -= x_j R_jl for every l > j.
 // A warp takes TRI_ROWS rows at once (independent chains hide the shuffle / FMA latency of each other); a lane holds the
-// elements l = lane, lane + 32 of each (k <= 64).  R and the reciprocals of its diagonal are staged in shared memory.
-constexpr int TRI_ROWS = 4, TRI_WARPS = 8, TRI_MAXK = 64;
-__global__ void __launch_bounds__(32 * TRI_WARPS) trisolve_rows_warp_kernel(double* __restrict__ V, const double* __restrict__ Rm,
-                                                                            int d, int k) {
+// elements l = lane, lane + 32 of each (k <= 64).  R and the reciprocals of its diagonal are staged in shared memory once
+// per CTA, which then walks TRI_GROUPS groups of rows.
+constexpr int TRI_ROWS = 4, TRI_WARPS = 8, TRI_GROUPS = 8, TRI_MAXK = 64;      // a CTA takes TRI_ROWS * TRI_WARPS * TRI_GROUPS = 256 rows
+__device__ __forceinline__ void trisolve_rows_warp_body(double* __restrict__ V, const double* __restrict__ Rm, int d, int k, int blk) {
     __shared__ double s_R[TRI_MAXK * TRI_MAXK];
     __shared__ double s_inv[TRI_MAXK];
     for (int idx = threadIdx.x; idx < k * k; idx += blockDim.x) s_R[idx] = Rm[idx];
     for (int j = threadIdx.x; j < k; j += blockDim.x) s_inv[j] = 1.0 / Rm[(int64_t)j * k + j];
     __syncthreads();
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int r0 = (blockIdx.x * TRI_WARPS + warp) * TRI_ROWS;
-    if (r0 >= d) return;
-    double x[TRI_ROWS][2];
+    for (int g = 0; g < TRI_GROUPS; ++g) {
+        const int r0 = ((blk * TRI_GROUPS + g) * TRI_WARPS + warp) * TRI_ROWS;
+        if (r0 >= d) return;
+        double x[TRI_ROWS][2];
 #pragma unroll
-    for (int t = 0; t < TRI_ROWS; ++t)
+        for (int t = 0; t < TRI_ROWS; ++t)
 #pragma unroll
-        for (int u = 0; u < 2; ++u)
-            x[t][u] = (r0 + t < d && lane + 32 * u < k) ? V[(int64_t)(r0 + t) * k + lane + 32 * u] : 0.0;
-    for (int j = 0; j < k; ++j) {
-        const double inv = s_inv[j];
-        const double rl0 = lane < k ? s_R[j * k + lane] : 0.0, rl1 = lane + 32 < k ? s_R[j * k + lane + 32] : 0.0;
+            for (int u = 0; u < 2; ++u)
+                x[t][u] = (r0 + t < d && lane + 32 * u < k) ? V[(int64_t)(r0 + t) * k + lane + 32 * u] : 0.0;
+        for (int j = 0; j < k; ++j) {
+            const double inv = s_inv[j];
+            const double rl0 = lane < k ? s_R[j * k + lane] : 0.0, rl1 = lane + 32 < k ? s_R[j * k + lane + 32] : 0.0;
 #pragma unroll
-        for (int t = 0; t < TRI_ROWS; ++t) {
-            const double xj = __shfl_sync(0xFFFFFFFFu, j < 32 ? x[t][0] : x[t][1], j & 31) * inv;
-            if (lane == j) x[t][0] = xj; else if (lane > j) x[t][0] = fma(-xj, rl0, x[t][0]);
-            if (lane + 32 == j) x[t][1] = xj; else if (lane + 32 > j) x[t][1] = fma(-xj, rl1, x[t][1]);
+            for (int t = 0; t < TRI_ROWS; ++t) {
+                const double xj = __shfl_sync(0xFFFFFFFFu, j < 32 ? x[t][0] : x[t][1], j & 31) * inv;
+                if (lane == j) x[t][0] = xj; else if (lane > j) x[t][0] = fma(-xj, rl0, x[t][0]);
+                if (lane + 32 == j) x[t][1] = xj; else if (lane + 32 > j) x[t][1] = fma(-xj, rl1, x[t][1]);
+            }
         }
+#pragma unroll
+        for (int t = 0; t < TRI_ROWS; ++t)
+#pragma unroll
+            for (int u = 0; u < 2; ++u)
+                if (r0 + t < d && lane + 32 * u < k) V[(int64_t)(r0 + t) * k + lane + 32 * u] = x[t][u];
     }
-#pragma unroll
-    for (int t = 0; t < TRI_ROWS; ++t)
-#pragma unroll
-        for (int u = 0; u < 2; ++u)
-            if (r0 + t < d && lane + 32 * u < k) V[(int64_t)(r0 + t) * k + lane + 32 * u] = x[t][u];
+}
+
+__global__ void __launch_bounds__(32 * TRI_WARPS) trisolve_rows_warp_kernel(double* __restrict__ V, const double* __restrict__ Rm,
+                                                                            int d, int k) {
+    trisolve_rows_warp_body(V, Rm, d, k, blockIdx.x);
 }
 
 // One thread per row (any k).
@@ -126,9 +137,8 @@ __global__ void __launch_bounds__(128) trisolve_rows_kernel(double* __restrict__
 // dynamic shared memory (use_smem) they are staged there, otherwise the CTA works on global / L2.
 // Round-robin ordering: k-1 rounds of k/2 disjoint rotations per sweep.  Output: mu sorted
 // descending, Zs = Z with its columns permuted into that order.
-__global__ void __launch_bounds__(1024) jacobi_kernel(double* __restrict__ Bg, double* __restrict__ Zg, int k,
-                                                      int use_smem, double* __restrict__ mu_sorted,
-                                                      double* __restrict__ Zs, int max_sweeps) {
+__device__ __forceinline__ void jacobi_body(double* __restrict__ Bg, double* __restrict__ Zg, int k, int use_smem,
+                                            double* __restrict__ mu_sorted, double* __restrict__ Zs, int max_sweeps) {
     extern __shared__ double s_dyn[];
     __shared__ double s_c[256], s_s[256];
     __shared__ int s_p[256], s_q[256];
@@ -249,15 +259,21 @@ __global__ void __launch_bounds__(1024) jacobi_kernel(double* __restrict__ Bg, d
     }
 }
 
+__global__ void __launch_bounds__(1024) jacobi_kernel(double* __restrict__ Bg, double* __restrict__ Zg, int k,
+                                                      int use_smem, double* __restrict__ mu_sorted,
+                                                      double* __restrict__ Zs, int max_sweeps) {
+    jacobi_body(Bg, Zg, k, use_smem, mu_sorted, Zs, max_sweeps);
+}
+
 // ---- trace(A) in FP64 and the multipliers (S2, S3) ---------------------------------------
 //   rho = max(0, (tr A - sum mu) / (d - k)) + lam   (k == d: rho = mu_k + lam)
 //   D_i = sqrt(rho / (mu_i + lam)),  e_i = D_i - 1,  ebar_i = 1/D_i - 1
 // One CTA.  If `trace_from` is null, rho_in is used as given (gf8_set_basis).
-__global__ void __launch_bounds__(256) multipliers_kernel(const float* __restrict__ factor, int d, int k,
-                                                          const double* __restrict__ mu64, const float* __restrict__ mu32,
-                                                          double lam, double rho_in, float* __restrict__ mu_out,
-                                                          float* __restrict__ e, float* __restrict__ ebar,
-                                                          float* __restrict__ rho_out) {
+__device__ __forceinline__ void multipliers_body(const float* __restrict__ factor, int d, int k,
+                                                 const double* __restrict__ mu64, const float* __restrict__ mu32,
+                                                 double lam, double rho_in, float* __restrict__ mu_out,
+                                                 float* __restrict__ e, float* __restrict__ ebar,
+                                                 float* __restrict__ rho_out) {
     __shared__ double s_part[256], s_tr[256];
     __shared__ double s_rho, s_floor;
     double tr = 0.0, sm = 0.0;
@@ -293,6 +309,14 @@ __global__ void __launch_bounds__(256) multipliers_kernel(const float* __restric
         e[i] = (float)(D - 1.0);
         ebar[i] = (float)(1.0 / D - 1.0);
     }
+}
+
+__global__ void __launch_bounds__(256) multipliers_kernel(const float* __restrict__ factor, int d, int k,
+                                                          const double* __restrict__ mu64, const float* __restrict__ mu32,
+                                                          double lam, double rho_in, float* __restrict__ mu_out,
+                                                          float* __restrict__ e, float* __restrict__ ebar,
+                                                          float* __restrict__ rho_out) {
+    multipliers_body(factor, d, k, mu64, mu32, lam, rho_in, mu_out, e, ebar, rho_out);
 }
 
 }  // namespace gf8

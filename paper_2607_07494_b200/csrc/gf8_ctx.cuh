@@ -63,7 +63,6 @@ struct LayerState {
 
 }  // namespace
 
-constexpr int GF8_REFRESH_STREAMS = 16;
 struct RefreshScratch {
     double *V = nullptr, *Y = nullptr, *Gm = nullptr, *Bm = nullptr, *Zm = nullptr, *Zs = nullptr, *mu64 = nullptr;
 };
@@ -85,11 +84,12 @@ struct gf8_ctx {
     std::vector<void*> allocs;
     float* wt_scratch = nullptr;     // max m*n FP32
     // refresh scratch (FP64): one set per concurrent refresh stream (gf8_refresh_basis_many); set 0 serves single calls
-    RefreshScratch rs[GF8_REFRESH_STREAMS];
+    RefreshScratch rs[1];
     size_t rs_dk = 0, rs_k = 0;
-    cudaStream_t rs_stream[GF8_REFRESH_STREAMS] = {};
-    cudaEvent_t rs_ev[GF8_REFRESH_STREAMS] = {};
-    cudaEvent_t rs_fork = nullptr;
+    // batched refresh (gf8_refresh.cuh): scratch arena (doubles), job records, and the event that guards their reuse
+    double* rb_arena = nullptr; size_t rb_arena_cap = 0;
+    void* rb_jobs = nullptr; size_t rb_jobs_cap = 0;
+    cudaEvent_t rb_ev = nullptr; bool rb_busy = false;
     // auxiliary stream: the streaming kernels of Euclidean tensors overlap the tensor-core stages of a batched call
     cudaStream_t aux_stream = nullptr;
     cudaEvent_t aux_fork_ev = nullptr, aux_join_ev = nullptr;

@@ -1,0 +1,314 @@
+// gf8_refresh.cuh -- a2 basis refresh for MANY factor sides at once (Eq. 24; S5).
+//
+// gf8_refresh_basis_many used to walk one chain of ~35 small launches per side on a handful of streams; the chains are
+// latency-bound (single-CTA Cholesky / Jacobi steps, split-K GEMMs with a few hundred CTAs), so a 336-side refresh took
+// 0.33 s.  Here every step of the algorithm is ONE launch over all sides of the call: the launch's grid carries the
+// side (blockIdx.y, or a prefix table of row blocks for the heavy product), so the single-CTA steps of different sides
+// fill the machine together and A V needs no split-K (each CTA runs a whole K loop: fixed summation order).
+//
+// The arithmetic is that of the per-side path (gf8_basis.cuh bodies, FP64 throughout):
+//   V <- U (start basis), orthonormalise (CholeskyQR twice), n_iter times { V <- A V, orthonormalise },
+//   Y = A V, B = V^T Y, Jacobi eigensolve of B, U <- V Z (sorted), multipliers (rho, e, ebar).
+// Ranks k <= 64 only (the triangular solve and the product tile hold a 64-wide panel); other sides take the per-side path.
+#pragma once
+#include "gf8_basis.cuh"
+
+namespace gf8 {
+namespace rb {
+
+constexpr int RB_MAXK = 64;
+constexpr int RB_CHUNK = 256;            // rows of V per partial Gram product
+constexpr int AV_BM = 128, AV_BK = 32;   // A V tile: 128 rows of A, K in steps of 32
+constexpr int AV_LDA = AV_BM + 4;        // leading dimension of the K-major A tile (floats; rows stay 16 B aligned)
+constexpr int AV_SMEM = AV_BK * RB_MAXK * 8 + AV_BK * AV_LDA * 4;
+constexpr int RM_SMEM = (RB_MAXK * (64 + 2) + RB_MAXK * RB_MAXK) * 8;
+
+struct RefreshJob {
+    const float* factor;     // d x d FP32
+    float* U;                // d x k FP32: start basis in, refreshed basis out
+    double* buf[2];          // d x k FP64 each: V and Y take turns
+    double* part;            // ceil(d / RB_CHUNK) partial k x k products
+    double* Gm;              // k x k: Gram matrix / its Cholesky factor
+    double* Bm;              // k x k: Rayleigh-Ritz matrix (destroyed by the eigensolve)
+    double* Zm;              // k x k scratch of the eigensolve (unused when it runs in shared memory)
+    double* Zs;              // k x k eigenvectors, columns sorted by descending eigenvalue
+    double* mu64;            // k
+    float *mu, *e, *ebar, *rho;
+    double lam;
+    int32_t d, k;
+    int32_t blk0;            // first AV_BM-row block of this side in the launch-wide list
+    int32_t n_chunks;
+};
+
+// ---- V <- (double) U ----------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) rb_widen_kernel(const RefreshJob* __restrict__ jobs, int flip) {
+    const RefreshJob& j = jobs[blockIdx.y];
+    const int64_t n = (int64_t)j.d * j.k;
+    double* V = j.buf[flip];
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) V[i] = (double)j.U[i];
+}
+
+// ---- partial products  part[c] = X[chunk c]^T W[chunk c]  (k x k, FP64), X = buf[xa], W = buf[xb] --------------
+// 256 threads, 4 x 4 outputs each; rows of the chunk staged 16 at a time.
+__global__ void __launch_bounds__(256) rb_gram_kernel(const RefreshJob* __restrict__ jobs, int xa, int xb) {
+    const RefreshJob& j = jobs[blockIdx.y];
+    const int c = blockIdx.x;
+    if (c >= j.n_chunks) return;
+    const int d = j.d, k = j.k;
+    const double* X = j.buf[xa];
+    const double* W = j.buf[xb];
+    __shared__ double Xs[16][RB_MAXK + 2], Ws[16][RB_MAXK + 2];
+    const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+    double acc[4][4] = {};
+    const int r_begin = c * RB_CHUNK, r_end = min(d, r_begin + RB_CHUNK);
+    for (int r0 = r_begin; r0 < r_end; r0 += 16) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int idx = tid + 256 * u, l = idx >> 6, col = idx & 63;
+            const bool ok = r0 + l < r_end && col < k;
+            Xs[l][col] = ok ? X[(int64_t)(r0 + l) * k + col] : 0.0;
+            Ws[l][col] = ok ? W[(int64_t)(r0 + l) * k + col] : 0.0;
+        }
+        __syncthreads();
+#pragma unroll
+        for (int l = 0; l < 16; ++l) {
+            double a[4], b[4];
+#pragma unroll
+            for (int r = 0; r < 4; ++r) a[r] = Xs[l][ty * 4 + r];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) b[q] = Ws[l][tx * 4 + q];
+#pragma unroll
+            for (int r = 0; r < 4; ++r)
+#pragma unroll
+                for (int q = 0; q < 4; ++q) acc[r][q] = fma(a[r], b[q], acc[r][q]);
+        }
+        __syncthreads();
+    }
+    double* P = j.part + (int64_t)c * k * k;
+#pragma unroll
+    for (int r = 0; r < 4; ++r)
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int i = ty * 4 + r, l = tx * 4 + q;
+            if (i < k && l < k) P[(int64_t)i * k + l] = acc[r][q];
+        }
+}
+
+// ---- out = sum over chunks of part[c], in chunk order (fixed summation order); to_B: into Bm, else into Gm --------
+__global__ void __launch_bounds__(256) rb_sum_kernel(const RefreshJob* __restrict__ jobs, int to_B) {
+    const RefreshJob& j = jobs[blockIdx.y];
+    const int kk = j.k * j.k;
+    double* out = to_B ? j.Bm : j.Gm;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < kk; i += gridDim.x * blockDim.x) {
+        double s = 0.0;
+        for (int c = 0; c < j.n_chunks; ++c) s += j.part[(int64_t)c * kk + i];
+        out[i] = s;
+    }
+}
+
+// Cholesky factor R of Gm (upper, in place) and then Zs <- R^-1 (upper triangular, zero below the diagonal): the panel is
+// orthonormalised as the product V R^-1 (rb_rightmul_kernel), a register-tiled GEMM, instead of d triangular solves.
+// 16 threads share a column of the inverse: x_c = 1 / R_cc, x_i = -(sum_{i < l <= c} R_il x_l) / R_ii for i = c-1 .. 0.
+__global__ void __launch_bounds__(1024) rb_chol_kernel(const RefreshJob* __restrict__ jobs) {
+    const RefreshJob& j = jobs[blockIdx.x];
+    const int k = j.k;
+    cholesky_upper_body(j.Gm, k, 1);
+    __syncthreads();
+    extern __shared__ double s_inv_dyn[];             // (the Cholesky working copy is dead: its shared memory holds the inverse)
+    double (*s_x)[RB_MAXK + 1] = reinterpret_cast<double (*)[RB_MAXK + 1]>(s_inv_dyn);      // s_x[c][i]: column c of the inverse
+    const int c = threadIdx.x >> 4, sub = threadIdx.x & 15;
+    const double* R = j.Gm;                           // (written by this CTA above; the barrier makes it visible CTA-wide)
+    // (the two columns of a warp run loops of different lengths: every warp-level primitive names its own half-warp)
+    const unsigned hmask = 0xFFFFu << (16 * ((threadIdx.x >> 4) & 1));
+    if (c < k) {
+        for (int i = sub; i < k; i += 16) s_x[c][i] = 0.0;
+        __syncwarp(hmask);
+        if (sub == 0) s_x[c][c] = 1.0 / R[(int64_t)c * k + c];
+        __syncwarp(hmask);
+        for (int i = c - 1; i >= 0; --i) {
+            double part = 0.0;
+            for (int l = i + 1 + sub; l <= c; l += 16) part = fma(R[(int64_t)i * k + l], s_x[c][l], part);
+#pragma unroll
+            for (int o = 8; o > 0; o >>= 1) part += __shfl_xor_sync(hmask, part, o, 16);
+            if (sub == 0) s_x[c][i] = -part / R[(int64_t)i * k + i];
+            __syncwarp(hmask);
+        }
+    }
+    __syncthreads();
+    for (int idx = threadIdx.x; idx < k * k; idx += blockDim.x) {
+        const int i = idx / k, cc = idx % k;
+        j.Zs[idx] = s_x[cc][i];
+    }
+}
+
+// ---- buf[flip] <- buf[flip] * Zs   (to_U = 0: FP64, in place)   or   U <- (float)(buf[flip] * Zs)   (to_U = 1) ------------
+// One CTA per 64 rows; 256 threads, 4 x 4 outputs each; the row panel is staged transposed so that a thread's four row values
+// and four column values are contiguous.
+__global__ void __launch_bounds__(256) rb_rightmul_kernel(const RefreshJob* __restrict__ jobs, int flip, int to_U) {
+    const RefreshJob& j = jobs[blockIdx.y];
+    const int d = j.d, k = j.k;
+    const int r0 = blockIdx.x * 64;
+    if (r0 >= d) return;
+    extern __shared__ __align__(16) double s_rm[];             // RM_SMEM bytes
+    double (*Vt)[64 + 2] = reinterpret_cast<double (*)[64 + 2]>(s_rm);                          // Vt[l][r]
+    double (*Zsh)[RB_MAXK] = reinterpret_cast<double (*)[RB_MAXK]>(s_rm + RB_MAXK * (64 + 2));   // Zsh[l][c]
+    double* V = j.buf[flip];
+    for (int idx = threadIdx.x; idx < RB_MAXK * RB_MAXK; idx += 256) {
+        const int l = idx >> 6, c = idx & 63;
+        Zsh[l][c] = (l < k && c < k) ? j.Zs[(int64_t)l * k + c] : 0.0;
+    }
+    for (int idx = threadIdx.x; idx < 64 * RB_MAXK; idx += 256) {
+        const int r = idx >> 6, l = idx & 63;
+        Vt[l][r] = (r0 + r < d && l < k) ? V[(int64_t)(r0 + r) * k + l] : 0.0;
+    }
+    __syncthreads();
+    const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+    double acc[4][4] = {};
+#pragma unroll 8
+    for (int l = 0; l < RB_MAXK; ++l) {
+        double a[4], b[4];
+#pragma unroll
+        for (int r = 0; r < 4; r += 2) { const double2 t = *reinterpret_cast<const double2*>(&Vt[l][ty * 4 + r]); a[r] = t.x; a[r + 1] = t.y; }
+#pragma unroll
+        for (int q = 0; q < 4; q += 2) { const double2 t = *reinterpret_cast<const double2*>(&Zsh[l][tx * 4 + q]); b[q] = t.x; b[q + 1] = t.y; }
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+            for (int q = 0; q < 4; ++q) acc[r][q] = fma(a[r], b[q], acc[r][q]);
+    }
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const int gi = r0 + ty * 4 + r;
+        if (gi >= d) continue;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int c = tx * 4 + q;
+            if (c >= k) continue;
+            if (to_U) j.U[(int64_t)gi * k + c] = (float)acc[r][q];
+            else V[(int64_t)gi * k + c] = acc[r][q];
+        }
+    }
+}
+
+__global__ void __launch_bounds__(1024) rb_jacobi_kernel(const RefreshJob* __restrict__ jobs, int max_sweeps) {
+    const RefreshJob& j = jobs[blockIdx.x];
+    jacobi_body(j.Bm, j.Zm, j.k, 1, j.mu64, j.Zs, max_sweeps);
+}
+
+__global__ void __launch_bounds__(256) rb_multipliers_kernel(const RefreshJob* __restrict__ jobs) {
+    const RefreshJob& j = jobs[blockIdx.x];
+    multipliers_body(j.factor, j.d, j.k, j.mu64, nullptr, j.lam, 0.0, j.mu, j.e, j.ebar, j.rho);
+}
+
+// ---- Y = A V: buf[flip ^ 1] <- factor (d x d FP32) * buf[flip] (d x k FP64), FP64 accumulate -----------------------
+// One CTA per 128-row block of one side (blockIdx.x walks the launch-wide block list), the whole K = d loop inside it.
+// 256 threads, 8 x 4 outputs each.  The kernel is bound by shared-memory wavefronts, not by the FP64 pipe (a 128-bit shared
+// load costs four wavefronts per warp whatever it broadcasts), so the A tile stays FP32 in shared memory (K-major: the
+// eight row values of a thread are two 128-bit loads) and is widened in registers; a warp of the loader takes 32
+// consecutive rows, which makes the transposing stores conflict-free.  The next tile's global loads are in flight while
+// the current one is multiplied.
+__global__ void __launch_bounds__(256, 2) rb_av_kernel(const RefreshJob* __restrict__ jobs, int n_jobs, int flip) {
+    extern __shared__ __align__(16) double s_av[];                  // AV_SMEM bytes
+    double (*Vs)[RB_MAXK] = reinterpret_cast<double (*)[RB_MAXK]>(s_av);
+    float (*As)[AV_LDA] = reinterpret_cast<float (*)[AV_LDA]>(s_av + AV_BK * RB_MAXK);
+    int lo = 0, hi = n_jobs - 1;
+    while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (jobs[mid].blk0 <= (int)blockIdx.x) lo = mid; else hi = mid - 1; }
+    const RefreshJob& j = jobs[lo];
+    const int d = j.d, k = j.k;
+    const int i0 = ((int)blockIdx.x - j.blk0) * AV_BM;
+    const float* __restrict__ A = j.factor;
+    const double* __restrict__ V = j.buf[flip];
+    double* __restrict__ Y = j.buf[flip ^ 1];
+    const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+    // loader roles: A tile 128 rows x 32 floats = 1024 float4 (4 per thread: row = idx % 128, quad = idx / 128);
+    //               V tile 32 rows x 64 doubles = 1024 double2 (4 per thread: row = idx / 32, pair = idx % 32)
+    float4 pa[4];
+    double2 pv[4];
+    const bool vec_ok = (d & 3) == 0 && (k & 1) == 0;
+    auto fetch = [&](int k0) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int idx = tid + 256 * u, row = idx & 127, quad = idx >> 7;
+            const int gi = i0 + row, gl = k0 + 4 * quad;
+            float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (gi < d) {
+                const float* p = A + (int64_t)gi * d + gl;
+                if (vec_ok && gl + 3 < d) v = __ldg(reinterpret_cast<const float4*>(p));
+                else {
+                    if (gl < d) v.x = p[0];
+                    if (gl + 1 < d) v.y = p[1];
+                    if (gl + 2 < d) v.z = p[2];
+                    if (gl + 3 < d) v.w = p[3];
+                }
+            }
+            pa[u] = v;
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int idx = tid + 256 * u, row = idx >> 5, pair = idx & 31;
+            const int gl = k0 + row, col = 2 * pair;
+            double2 v = make_double2(0.0, 0.0);
+            if (gl < d) {
+                const double* p = V + (int64_t)gl * k + col;
+                if (vec_ok && col + 1 < k) v = *reinterpret_cast<const double2*>(p);
+                else {
+                    if (col < k) v.x = p[0];
+                    if (col + 1 < k) v.y = p[1];
+                }
+            }
+            pv[u] = v;
+        }
+    };
+    auto stash = [&]() {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int idx = tid + 256 * u, row = idx & 127, quad = idx >> 7;
+            As[4 * quad][row] = pa[u].x; As[4 * quad + 1][row] = pa[u].y;
+            As[4 * quad + 2][row] = pa[u].z; As[4 * quad + 3][row] = pa[u].w;
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int idx = tid + 256 * u, row = idx >> 5, pair = idx & 31;
+            *reinterpret_cast<double2*>(&Vs[row][2 * pair]) = pv[u];
+        }
+    };
+    double acc[8][4] = {};
+    fetch(0);
+    for (int k0 = 0; k0 < d; k0 += AV_BK) {
+        stash();
+        __syncthreads();
+        if (k0 + AV_BK < d) fetch(k0 + AV_BK);
+#pragma unroll 8
+        for (int l = 0; l < AV_BK; ++l) {
+            double a[8], b[4];
+#pragma unroll
+            for (int r = 0; r < 8; r += 4) {
+                const float4 t = *reinterpret_cast<const float4*>(&As[l][ty * 8 + r]);
+                a[r] = (double)t.x; a[r + 1] = (double)t.y; a[r + 2] = (double)t.z; a[r + 3] = (double)t.w;
+            }
+#pragma unroll
+            for (int q = 0; q < 4; q += 2) {
+                const double2 t = *reinterpret_cast<const double2*>(&Vs[l][tx * 4 + q]);
+                b[q] = t.x; b[q + 1] = t.y;
+            }
+#pragma unroll
+            for (int r = 0; r < 8; ++r)
+#pragma unroll
+                for (int q = 0; q < 4; ++q) acc[r][q] = fma(a[r], b[q], acc[r][q]);
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+        const int gi = i0 + ty * 8 + r;
+        if (gi >= d) continue;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int col = tx * 4 + q;
+            if (col < k) Y[(int64_t)gi * k + col] = acc[r][q];
+        }
+    }
+}
+
+}  // namespace rb
+}  // namespace gf8
