@@ -19,13 +19,20 @@ SCALE_TENSOR, SCALE_BLOCK128 = 0, 1
 
 
 def build(force=False):
-    """Compile the oracle with g++ (no -ffast-math, no FMA contraction)."""
-    if not force and os.path.exists(_LIB) and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC):
-        return _LIB
-    cmd = ["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off",
-           "-fno-fast-math", "-o", _LIB, _SRC]
-    subprocess.check_call(cmd)
-    return _LIB
+    """Compile the oracle with g++ (no -ffast-math, no FMA contraction).
+
+    GF8_ORACLE_SANITIZE=1 builds and loads an AddressSanitizer + UndefinedBehaviorSanitizer copy instead
+    (libgf8_oracle_san.so; run python with LD_PRELOAD=$(g++ -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0):
+    the hygiene run of profiles/r02_sanitizers.txt."""
+    san = os.environ.get("GF8_ORACLE_SANITIZE") == "1"
+    out = os.path.join(_HERE, "libgf8_oracle_san.so") if san else _LIB
+    if not force and os.path.exists(out) and os.path.getmtime(out) >= os.path.getmtime(_SRC):
+        return out
+    cmd = ["g++", "-O1" if san else "-O2", "-std=c++17", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off", "-fno-fast-math"]
+    if san:
+        cmd += ["-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined"]
+    subprocess.check_call(cmd + ["-o", out, _SRC])
+    return out
 
 
 _lib = None
@@ -54,6 +61,7 @@ def _declare(L):
     L.gf8o_fp8_from_float.restype = C.c_uint8
     L.gf8o_fp8_from_float.argtypes = [C.c_int, C.c_float]
     L.gf8o_quantize.argtypes = [C.c_int, C.c_int, _pf, _i64, _i64, _pb, _pf]
+    L.gf8o_ef_quantize.argtypes = [C.c_int, C.c_int, _pf, _pf, _i64, _i64, _pb, _pf]
     L.gf8o_reduce.argtypes = [C.c_int, C.c_int, C.POINTER(_pb), C.POINTER(_pf), C.c_int, C.c_int,
                               _i64, _i64, _pf]
     L.gf8o_factor_accumulate.argtypes = [_pd, C.c_int, C.c_double, _pd, _i64, _i64]
@@ -113,6 +121,18 @@ def quantize(x_f32, fmt=E4M3, scaling=SCALE_TENSOR):
     sinv = np.empty(n_scales(scaling, m, n), dtype=np.float32)
     lib().gf8o_quantize(fmt, scaling, _p(x, _pf), m, n, _p(codes, _pb), _p(sinv, _pf))
     return codes, sinv
+
+
+def ef_quantize(u_f32, resid_f32, fmt=E4M3, scaling=SCALE_TENSOR):
+    """O8: error-feedback quantizer.  Returns (codes, scale_inv, new residual); the inputs are not modified."""
+    u = np.ascontiguousarray(u_f32, dtype=np.float32)
+    r = np.array(resid_f32, dtype=np.float32, order="C", copy=True)
+    assert u.ndim == 2 and r.shape == u.shape
+    m, n = u.shape
+    codes = np.empty((m, n), np.uint8)
+    sinv = np.empty(n_scales(scaling, m, n), np.float32)
+    lib().gf8o_ef_quantize(fmt, scaling, _p(u, _pf), _p(r, _pf), m, n, _p(codes, _pb), _p(sinv, _pf))
+    return codes, sinv, r
 
 
 def reduce(codes_list, sinv_list, fmt=E4M3, scaling=SCALE_TENSOR, average=True):
@@ -314,6 +334,15 @@ def encode(W, basisG=None, basisA=None, fmt=E4M3, scaling=SCALE_TENSOR):
     x = to_f32(wt)
     codes, sinv = quantize(x, fmt, scaling)
     return codes, sinv, x
+
+
+def encode_ef(W, resid_f32, basisG=None, basisA=None, fmt=E4M3, scaling=SCALE_TENSOR):
+    """O3 + O8 on one gradient: returns (codes, scale_inv, new residual, wt_f32)."""
+    wt = whiten_lowrank(W, basisG.U if basisG else None, basisG.e if basisG else None,
+                        basisA.U if basisA else None, basisA.e if basisA else None)
+    x = to_f32(wt)
+    codes, sinv, r = ef_quantize(x, resid_f32, fmt, scaling)
+    return codes, sinv, r, x
 
 
 def reduce_decoded(codes_list, sinv_list, basisG=None, basisA=None, fmt=E4M3, scaling=SCALE_TENSOR,

@@ -18,6 +18,8 @@
 //   Jacobi / subspace residuals, trace, 2x2 closed form, exact-rank-k one-step, brute force
 //   factor            symmetry, trace, convergence to the generating covariance
 //   reduce            == mean of per-rank dequantisation; R=1 == dequantise
+//   error feedback    zero residual == plain quantizer; worked example (tests/golden/ef_worked_example.txt); the
+//                     telescoping identity sum deq_t = sum u_t + R_0 - R_T; |R| <= half the widest code gap
 // Parity unpinned: the paper's printed Table I / II values (they need the authors' gradients).
 
 #include <cmath>
@@ -151,6 +153,31 @@ void gf8o_reduce(int fmt, int scaling, const uint8_t* const* codes, const float*
                 acc = std::fmaf((float)gf8o_fp8_to_double(fmt, codes[r][i * n + j]), scale_inv[r][sidx], acc);
             if (average) { volatile float t = acc * invR; acc = t; }
             out[i * n + j] = acc;
+        }
+}
+
+// ------------------------------------------------------------------------------------------------
+// O8.  Error feedback in the transformed coordinates (PAPER.md:318 Alg. 1 l.11-15; :354; S10).
+// Per tensor and per rank a residual buffer R (same shape as the gradient, FP32, zero at start):
+//     U~   = U + R                         (l.11; U is the whitened gradient, the FP32 tensor O4 would quantize)
+//     s    = Scale(U~), Q~ = Q(U~; s)      (l.12-13: O4 on U~)
+//     deq  = Dequantize(Q~; s)             (l.14: val(code) * scale_inv)
+//     R   <- U~ - deq                      (l.15)
+// Each line is ONE IEEE FP32 operation per element (add; O4; multiply; subtract), no contraction -- the
+// residual is state carried from step to step, so both sides have to round it the same way.
+// ------------------------------------------------------------------------------------------------
+void gf8o_ef_quantize(int fmt, int scaling, const float* u, float* resid, int64_t m, int64_t n, uint8_t* codes,
+                      float* scale_inv) {
+    std::vector<float> ut((size_t)(m * n));
+    for (int64_t i = 0; i < m * n; ++i) { volatile float t = u[i] + resid[i]; ut[(size_t)i] = t; }
+    gf8o_quantize(fmt, scaling, ut.data(), m, n, codes, scale_inv);
+    const int64_t bn = (n + 127) / 128;
+    for (int64_t i = 0; i < m; ++i)
+        for (int64_t j = 0; j < n; ++j) {
+            const int64_t sidx = scaling == 0 ? 0 : (i / 128) * bn + (j / 128);
+            volatile float deq = (float)gf8o_fp8_to_double(fmt, codes[i * n + j]) * scale_inv[sidx];
+            volatile float r = ut[(size_t)(i * n + j)] - deq;
+            resid[i * n + j] = r;
         }
 }
 

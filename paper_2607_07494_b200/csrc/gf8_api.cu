@@ -806,6 +806,11 @@ gf8_status gf8_destroy(gf8_ctx* ctx) {
     cudaDeviceSynchronize();
     for (void* p : ctx->allocs) cudaFree(p);
     for (void* p : ctx->stage_allocs) cudaFree(p);
+    if (ctx->hs_in) {
+        cudaStreamDestroy(ctx->hs_in); cudaStreamDestroy(ctx->hs_out);
+        cudaEventDestroy(ctx->hs_start); cudaEventDestroy(ctx->hs_done);
+        for (int q = 0; q < GF8_HOST_CHUNKS; ++q) { cudaEventDestroy(ctx->hs_in_ev[q]); cudaEventDestroy(ctx->hs_comp_ev[q]); }
+    }
     if (ctx->rb_arena) cudaFree(ctx->rb_arena);
     if (ctx->rb_jobs) cudaFree(ctx->rb_jobs);
     if (ctx->rb_ev) cudaEventDestroy(ctx->rb_ev);
@@ -1156,29 +1161,73 @@ gf8_status gf8_step_host(gf8_ctx* ctx, int n, const int* layers, const void* con
         ctx->st_dt = (int)dt;
     }
     for (int i = 0; i < n; ++i) {
-        const LayerState& L = ctx->layers[layers[i]];
-        const size_t bytes = (size_t)L.desc.d_out * L.desc.d_in * esz;
-        for (int r = 0; r < R; ++r) {
+        if (!out_host[i]) return fail(ctx, GF8_ERR_INVALID_ARG, "null host output");
+        for (int r = 0; r < R; ++r)
             if (!grads_host[(size_t)i * R + r]) return fail(ctx, GF8_ERR_INVALID_ARG, "null host gradient");
-            CU_TRY(ctx, cudaMemcpyAsync(ctx->st_grads[(size_t)i * R + r], grads_host[(size_t)i * R + r], bytes,
-                                        cudaMemcpyHostToDevice, st));
+    }
+    // The step is cut into chunks of consecutive tensors (balanced by bytes) and pipelined over three streams: the host->device
+    // copies of chunk c + 1 (copy-in stream) overlap the codec of chunk c (the caller's stream) and the device->host copy of
+    // chunk c - 1 (copy-out stream), so the link carries traffic in both directions for the whole step and the kernels hide
+    // behind it.  The caller's stream ends up waiting for the last copy-out: synchronising it completes the step.
+    if (!ctx->hs_in) {
+        CU_TRY(ctx, cudaStreamCreateWithFlags(&ctx->hs_in, cudaStreamNonBlocking));
+        CU_TRY(ctx, cudaStreamCreateWithFlags(&ctx->hs_out, cudaStreamNonBlocking));
+        CU_TRY(ctx, cudaEventCreateWithFlags(&ctx->hs_start, cudaEventDisableTiming));
+        CU_TRY(ctx, cudaEventCreateWithFlags(&ctx->hs_done, cudaEventDisableTiming));
+        for (int q = 0; q < GF8_HOST_CHUNKS; ++q) {
+            CU_TRY(ctx, cudaEventCreateWithFlags(&ctx->hs_in_ev[q], cudaEventDisableTiming));
+            CU_TRY(ctx, cudaEventCreateWithFlags(&ctx->hs_comp_ev[q], cudaEventDisableTiming));
         }
     }
+    size_t total_bytes = 0;
+    for (int i = 0; i < n; ++i) total_bytes += (size_t)ctx->layers[layers[i]].desc.d_out * ctx->layers[layers[i]].desc.d_in;
+    const int n_chunks = std::min(n, GF8_HOST_CHUNKS);
+    std::vector<int> cut(n_chunks + 1, n);
+    cut[0] = 0;
     {
-        std::vector<int> lay((size_t)n * R);
-        for (int i = 0; i < n; ++i)
-            for (int r = 0; r < R; ++r) lay[(size_t)i * R + r] = layers[i];
-        GF_TRY(gf8_encode_many(ctx, n * R, lay.data(), ctx->st_grads.data(), dt, ctx->st_codes.data(), ctx->st_sinv.data(),
-                               stream));
-        GF_TRY(gf8_reduce_decoded_many(ctx, n, layers, (const uint8_t* const*)ctx->st_codes.data(),
-                                       (const float* const*)ctx->st_sinv.data(), R, average, ctx->st_out.data(), dt, stream));
+        size_t acc = 0;
+        int q = 1;
+        for (int i = 0; i < n && q < n_chunks; ++i) {
+            acc += (size_t)ctx->layers[layers[i]].desc.d_out * ctx->layers[layers[i]].desc.d_in;
+            // (a cut never leaves a later chunk without a tensor)
+            if (acc * n_chunks >= total_bytes * q || n - (i + 1) == n_chunks - q) cut[q++] = i + 1;
+        }
     }
-    for (int i = 0; i < n; ++i) {
-        const LayerState& L = ctx->layers[layers[i]];
-        if (!out_host[i]) return fail(ctx, GF8_ERR_INVALID_ARG, "null host output");
-        CU_TRY(ctx, cudaMemcpyAsync(out_host[i], ctx->st_out[i], (size_t)L.desc.d_out * L.desc.d_in * esz,
-                                    cudaMemcpyDeviceToHost, st));
+    // (the staging buffers are reused from step to step: the copies wait for everything the caller's stream holds so far)
+    CU_TRY(ctx, cudaEventRecord(ctx->hs_start, st));
+    CU_TRY(ctx, cudaStreamWaitEvent(ctx->hs_in, ctx->hs_start, 0));
+    CU_TRY(ctx, cudaStreamWaitEvent(ctx->hs_out, ctx->hs_start, 0));
+    std::vector<int> lay;
+    for (int q = 0; q < n_chunks; ++q) {
+        const int i0 = cut[q], i1 = cut[q + 1];
+        if (i1 <= i0) continue;
+        for (int i = i0; i < i1; ++i) {
+            const LayerState& L = ctx->layers[layers[i]];
+            const size_t bytes = (size_t)L.desc.d_out * L.desc.d_in * esz;
+            for (int r = 0; r < R; ++r)
+                CU_TRY(ctx, cudaMemcpyAsync(ctx->st_grads[(size_t)i * R + r], grads_host[(size_t)i * R + r], bytes,
+                                            cudaMemcpyHostToDevice, ctx->hs_in));
+        }
+        CU_TRY(ctx, cudaEventRecord(ctx->hs_in_ev[q], ctx->hs_in));
+        CU_TRY(ctx, cudaStreamWaitEvent(st, ctx->hs_in_ev[q], 0));
+        lay.assign((size_t)(i1 - i0) * R, 0);
+        for (int i = i0; i < i1; ++i)
+            for (int r = 0; r < R; ++r) lay[(size_t)(i - i0) * R + r] = layers[i];
+        GF_TRY(gf8_encode_many(ctx, (i1 - i0) * R, lay.data(), ctx->st_grads.data() + (size_t)i0 * R, dt,
+                               ctx->st_codes.data() + (size_t)i0 * R, ctx->st_sinv.data() + (size_t)i0 * R, stream));
+        GF_TRY(gf8_reduce_decoded_many(ctx, i1 - i0, layers + i0, (const uint8_t* const*)ctx->st_codes.data() + (size_t)i0 * R,
+                                       (const float* const*)ctx->st_sinv.data() + (size_t)i0 * R, R, average,
+                                       ctx->st_out.data() + i0, dt, stream));
+        CU_TRY(ctx, cudaEventRecord(ctx->hs_comp_ev[q], st));
+        CU_TRY(ctx, cudaStreamWaitEvent(ctx->hs_out, ctx->hs_comp_ev[q], 0));
+        for (int i = i0; i < i1; ++i) {
+            const LayerState& L = ctx->layers[layers[i]];
+            CU_TRY(ctx, cudaMemcpyAsync(out_host[i], ctx->st_out[i], (size_t)L.desc.d_out * L.desc.d_in * esz,
+                                        cudaMemcpyDeviceToHost, ctx->hs_out));
+        }
     }
+    CU_TRY(ctx, cudaEventRecord(ctx->hs_done, ctx->hs_out));
+    CU_TRY(ctx, cudaStreamWaitEvent(st, ctx->hs_done, 0));
     return GF8_OK;
 }
 

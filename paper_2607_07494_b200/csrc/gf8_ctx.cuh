@@ -63,6 +63,8 @@ struct LayerState {
 
 }  // namespace
 
+constexpr int GF8_HOST_CHUNKS = 12;   // gf8_step_host pipelines a step in at most this many chunks of tensors
+
 struct RefreshScratch {
     double *V = nullptr, *Y = nullptr, *Gm = nullptr, *Bm = nullptr, *Zm = nullptr, *Zs = nullptr, *mu64 = nullptr;
 };
@@ -95,7 +97,9 @@ struct gf8_ctx {
     cudaEvent_t aux_fork_ev = nullptr, aux_join_ev = nullptr;
     // tap scratch (gf8_quantize_f32 with arbitrary shapes)
     uint32_t* tap_amax = nullptr; float* tap_scale = nullptr; size_t tap_cap = 0;
-    // host-step staging
+    // host-step staging; copy-in / copy-out streams and the per-chunk events of the pipelined gf8_step_host
+    cudaStream_t hs_in = nullptr, hs_out = nullptr;
+    cudaEvent_t hs_start = nullptr, hs_done = nullptr, hs_in_ev[GF8_HOST_CHUNKS] = {}, hs_comp_ev[GF8_HOST_CHUNKS] = {};
     std::vector<void*> stage_allocs;
     std::vector<void*> st_grads; std::vector<uint8_t*> st_codes; std::vector<float*> st_sinv; std::vector<void*> st_out;
     std::vector<int> st_layers; int st_R = 0; int st_dt = -1;

@@ -621,3 +621,38 @@ def test_rank_deficient_factor_with_zero_damping_stays_finite():
     # (rho -> 0 makes the model say the tail carries no curvature: the round trip is finite, not accurate -- the floor only
     #  keeps the multipliers representable)
     assert torch.isfinite(out).all()
+
+
+def test_step_host_matches_the_device_calls_bit_for_bit():
+    """gf8_step_host (pinned HOST buffers, the call bench.py's `e2e` times; pipelined in chunks of tensors over a copy-in, a
+    compute and a copy-out stream) returns exactly the bytes of gf8_encode_many + gf8_reduce_decoded_many on device
+    buffers, for a list with more tensors than chunks, mixed whitened / Euclidean, and again when the staging buffers are
+    reused with new gradients."""
+    shapes = [(256, 384), (384, 256), (128, 640), (400, 272), (256, 256), (192, 320), (320, 192), (176, 656), (512, 128),
+              (256, 384), (384, 384), (128, 128), (640, 256), (1008, 96), (256, 512)]
+    lays = [gf8.Layer(m, n, gf8.SIDE_NONE if i % 4 == 3 else gf8.SIDE_BOTH, 16, 16) for i, (m, n) in enumerate(shapes)]
+    ctx = gf8.create(lays, gf8.PREC_FAST)
+    mu = torch.arange(1, 17, device="cuda", dtype=torch.float32) ** -2.0
+    for i, l in enumerate(lays):
+        if l.side == gf8.SIDE_NONE:
+            continue
+        ctx.set_basis(i, gf8.SIDE_IN, synth.rand_orthonormal(l.d_in, 16, "cuda", 71, i, 1).contiguous(), mu, 0.02)
+        ctx.set_basis(i, gf8.SIDE_OUT, synth.rand_orthonormal(l.d_out, 16, "cuda", 71, i, 2).contiguous(), mu, 0.02)
+    R, n = 2, len(lays)
+    ids = list(range(n))
+    for rep in range(2):
+        hg = [(synth.gradient(lays[i].d_out, lays[i].d_in, "cuda", 72 + rep, i) * (1.0 + r)).to(torch.bfloat16).cpu().pin_memory()
+              for i in ids for r in range(R)]
+        ho = [torch.empty((l.d_out, l.d_in), dtype=torch.bfloat16).pin_memory() for l in lays]
+        ctx.step_host(ids, hg, R, ho)
+        torch.cuda.synchronize()
+        ctx.sync_check()
+        dg = [g.cuda() for g in hg]
+        codes = [torch.empty(g.shape, dtype=torch.uint8, device="cuda") for g in dg]
+        sinvs = [torch.empty(1, dtype=torch.float32, device="cuda") for _ in dg]
+        ctx.encode_many([i for i in ids for _ in range(R)], dg, codes, sinvs)
+        outs = [torch.empty((l.d_out, l.d_in), dtype=torch.bfloat16, device="cuda") for l in lays]
+        ctx.reduce_decoded_many(ids, codes, sinvs, R, outs, average=True)
+        ctx.sync_check()
+        for i in ids:
+            assert torch.equal(ho[i].view(torch.int16), outs[i].cpu().view(torch.int16)), (rep, i)
