@@ -111,6 +111,15 @@ gf8_status gf8_refresh_basis(gf8_ctx* ctx, int layer, int n_iter, void* stream);
 /* a3-a6.  codes[m*n], scale_inv[n_scales] <- FP8 payload of the whitened gradient. */
 gf8_status gf8_encode(gf8_ctx* ctx, int layer, const void* grad, gf8_dtype dt, uint8_t* codes,
                       float* scale_inv, void* stream);
+/* f1.  gf8_encode with ERROR FEEDBACK in the transformed coordinates (PAPER.md:318 Algorithm 1 l.11-15; :354):
+ *   U~ = U + R;  s = Scale(U~);  codes = Q(U~; s);  R <- U~ - Dequantize(codes; s)
+ * U is the whitened gradient (the gradient itself for a GF8_SIDE_NONE layer).  resid: DEVICE, FP32, d_out*d_in, 16-byte
+ * aligned, caller-owned, one buffer per (tensor, rank); zero it before the first step; it is read and overwritten.  Every
+ * element is one IEEE FP32 add, multiply, cast, multiply and subtract: on the same U the codes, scales and residual are
+ * bit-identical to oracle O8.  With resid == 0 the payload equals gf8_encode's.  First correct version: U goes through an
+ * FP32 scratch (the codec's tap path), then two streaming kernels per tensor; see DESIGN.md for its byte budget. */
+gf8_status gf8_encode_ef(gf8_ctx* ctx, int layer, const void* grad, gf8_dtype dt, float* resid, uint8_t* codes,
+                         float* scale_inv, void* stream);
 /* R = 1 case of gf8_reduce_decoded without averaging. */
 gf8_status gf8_decode(gf8_ctx* ctx, int layer, const uint8_t* codes, const float* scale_inv,
                       void* grad_out, gf8_dtype dt, void* stream);
@@ -126,6 +135,10 @@ gf8_status gf8_reduce_decoded(gf8_ctx* ctx, int layer, const uint8_t* const* cod
 gf8_status gf8_encode_many(gf8_ctx* ctx, int n, const int* layers_host, const void* const* grads_host,
                            gf8_dtype dt, uint8_t* const* codes_host, float* const* scale_inv_host,
                            void* stream);
+/* resid_host: HOST array of n device pointers (see gf8_encode_ef). */
+gf8_status gf8_encode_ef_many(gf8_ctx* ctx, int n, const int* layers_host, const void* const* grads_host,
+                              gf8_dtype dt, float* const* resid_host, uint8_t* const* codes_host,
+                              float* const* scale_inv_host, void* stream);
 /* codes_host / scale_inv_host: HOST arrays of n*R device pointers, index [i*R + r]. */
 gf8_status gf8_reduce_decoded_many(gf8_ctx* ctx, int n, const int* layers_host,
                                    const uint8_t* const* codes_host, const float* const* scale_inv_host,

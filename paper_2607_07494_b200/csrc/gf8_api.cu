@@ -18,6 +18,7 @@ using namespace gf8;
 #include "gf8_stream_host.cuh"
 #include "gf8_factor.cuh"
 #include "gf8_refresh.cuh"
+#include "gf8_ef.cuh"
 
 namespace {
 
@@ -811,6 +812,7 @@ gf8_status gf8_destroy(gf8_ctx* ctx) {
         cudaEventDestroy(ctx->hs_start); cudaEventDestroy(ctx->hs_done);
         for (int q = 0; q < GF8_HOST_CHUNKS; ++q) { cudaEventDestroy(ctx->hs_in_ev[q]); cudaEventDestroy(ctx->hs_comp_ev[q]); }
     }
+    if (ctx->ef_scratch) cudaFree(ctx->ef_scratch);
     if (ctx->rb_arena) cudaFree(ctx->rb_arena);
     if (ctx->rb_jobs) cudaFree(ctx->rb_jobs);
     if (ctx->rb_ev) cudaEventDestroy(ctx->rb_ev);
@@ -1119,6 +1121,109 @@ gf8_status gf8_refresh_basis_many(gf8_ctx* ctx, int n, const int* layers, int n_
         }
     }
     return refresh_batch(ctx, st, batch, lams, n_iter);
+}
+
+// ---- f1: encode with error feedback in the transformed coordinates (Alg. 1 l.11-15) ---------------------
+extern "C++" {
+namespace {
+template <typename T>
+gf8_status ef_quantize_dev(gf8_ctx* c, cudaStream_t st, const T* u, float* resid, int64_t m, int64_t n, int fmt, int scaling,
+                           uint32_t* amax_bits, float* scale, uint8_t* codes, float* scale_inv) {
+    const size_t ns = n_scales_of(scaling, m, n);
+    if (scaling == GF8_SCALE_TENSOR) {
+        CU_TRY(c, cudaMemsetAsync(amax_bits, 0, sizeof(uint32_t), st));
+        ef_amax_kernel<T><<<grid_for(c, m * n / 16, 256, 8), 256, 0, st>>>(u, resid, m, n, 0, amax_bits);
+    } else {
+        dim3 grid((unsigned)((n + 127) / 128), (unsigned)((m + 127) / 128));
+        ef_amax_kernel<T><<<grid, 256, 0, st>>>(u, resid, m, n, 1, amax_bits);
+    }
+    LAUNCH_CHECK(c);
+    scales_kernel<<<(int)((ns + 255) / 256), 256, 0, st>>>(amax_bits, (int)ns, fmax_of(fmt), scale, scale_inv);
+    LAUNCH_CHECK(c);
+    const int g = grid_for(c, m * n / 16, 256, 8);
+    if (fmt == GF8_E4M3) ef_cast_kernel<T, 0><<<g, 256, 0, st>>>(u, resid, m, n, scaling, scale, scale_inv, codes);
+    else ef_cast_kernel<T, 1><<<g, 256, 0, st>>>(u, resid, m, n, scaling, scale, scale_inv, codes);
+    LAUNCH_CHECK(c);
+    c->launches += 3;
+    return GF8_OK;
+}
+}  // namespace
+}  // extern "C++"
+
+gf8_status gf8_encode_ef_many(gf8_ctx* ctx, int n, const int* layers, const void* const* grads, gf8_dtype dt,
+                              float* const* resid, uint8_t* const* codes, float* const* scale_inv, void* stream) {
+    if (!ctx) return GF8_ERR_INVALID_ARG;
+    if (n < 0 || !layers || !grads || !resid || !codes || !scale_inv) return fail(ctx, GF8_ERR_INVALID_ARG, "null argument");
+    if (dt != GF8_DT_BF16 && dt != GF8_DT_F32) return fail(ctx, GF8_ERR_INVALID_ARG, "bad dtype");
+    for (int i = 0; i < n; ++i) {
+        GF_TRY(check_layer(ctx, layers[i]));
+        LayerState& L = ctx->layers[layers[i]];
+        if (!grads[i] || !resid[i] || !codes[i] || !scale_inv[i]) return fail(ctx, GF8_ERR_INVALID_ARG, "null pointer");
+        if (!aligned16(grads[i]) || !aligned16(resid[i]) || !aligned16(codes[i]))
+            return fail(ctx, GF8_ERR_UNSUPPORTED, "pointers must be 16-byte aligned");
+        GF_TRY(check_basis(ctx, L, layers[i]));
+    }
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    // Whitened tensors: the codec's tap path writes U = W~ (FP32) for a chunk of problems in one batched call, then the
+    // feedback kernels quantize U + R per tensor.  A chunk holds at most EF_CHUNK_ELEMS elements of scratch.
+    constexpr size_t EF_CHUNK_ELEMS = size_t(1) << 28;
+    int i0 = 0;
+    while (i0 < n) {
+        size_t elems = 0;
+        int i1 = i0;
+        std::vector<int> wl;                    // whitened problems of the chunk
+        std::vector<size_t> woff;
+        for (; i1 < n; ++i1) {
+            const LayerState& L = ctx->layers[layers[i1]];
+            if (L.desc.side == GF8_SIDE_NONE) continue;
+            const size_t mn = (size_t)L.desc.d_out * L.desc.d_in;
+            if (!wl.empty() && elems + mn > EF_CHUNK_ELEMS) break;
+            wl.push_back(i1); woff.push_back(elems);
+            elems += mn;
+        }
+        if (elems > ctx->ef_cap) {
+            CU_TRY(ctx, cudaStreamSynchronize(st));
+            if (ctx->ef_scratch) CU_TRY(ctx, cudaFree(ctx->ef_scratch));
+            ctx->ef_scratch = nullptr; ctx->ef_cap = 0;
+            CU_TRY(ctx, cudaMalloc((void**)&ctx->ef_scratch, elems * sizeof(float)));
+            ctx->ef_cap = elems;
+        }
+        // tensor-core shapes of the chunk in one tapped call; the others through the FP32 SIMT transform
+        std::vector<int> tl; std::vector<const void*> tg; std::vector<float*> tt;
+        for (size_t q = 0; q < wl.size(); ++q) {
+            LayerState& L = ctx->layers[layers[wl[q]]];
+            float* u = ctx->ef_scratch + woff[q];
+            if (L.tc_ok && (ctx->precision == GF8_PREC_FAST || ctx->tc_exact)) { tl.push_back(layers[wl[q]]); tg.push_back(grads[wl[q]]); tt.push_back(u); }
+            else if (dt == GF8_DT_BF16) GF_TRY(transform_simt<bf16>(ctx, st, L, (const bf16*)grads[wl[q]], u, false));
+            else GF_TRY(transform_simt<float>(ctx, st, L, (const float*)grads[wl[q]], u, false));
+        }
+        if (!tl.empty()) GF_TRY(encode_dispatch(ctx, (int)tl.size(), tl.data(), tg.data(), dt, nullptr, nullptr, tt.data(), st));
+        size_t q = 0;
+        for (int i = i0; i < i1; ++i) {
+            LayerState& L = ctx->layers[layers[i]];
+            const int64_t m = L.desc.d_out, nn = L.desc.d_in;
+            if (L.desc.side == GF8_SIDE_NONE) {
+                if (dt == GF8_DT_BF16)
+                    GF_TRY(ef_quantize_dev<bf16>(ctx, st, (const bf16*)grads[i], resid[i], m, nn, L.desc.fmt, L.desc.scaling,
+                                                 L.amax_bits, L.scale, codes[i], scale_inv[i]));
+                else
+                    GF_TRY(ef_quantize_dev<float>(ctx, st, (const float*)grads[i], resid[i], m, nn, L.desc.fmt, L.desc.scaling,
+                                                  L.amax_bits, L.scale, codes[i], scale_inv[i]));
+            } else {
+                GF_TRY(ef_quantize_dev<float>(ctx, st, ctx->ef_scratch + woff[q], resid[i], m, nn, L.desc.fmt, L.desc.scaling,
+                                              L.amax_bits, L.scale, codes[i], scale_inv[i]));
+                ++q;
+            }
+        }
+        i0 = i1;
+    }
+    return GF8_OK;
+}
+
+gf8_status gf8_encode_ef(gf8_ctx* ctx, int layer, const void* grad, gf8_dtype dt, float* resid, uint8_t* codes,
+                         float* scale_inv, void* stream) {
+    return gf8_encode_ef_many(ctx, 1, &layer, &grad, dt, &resid, &codes, &scale_inv, stream);
 }
 
 // ---- end-to-end with host buffers -----------------------------------------------------------------------------

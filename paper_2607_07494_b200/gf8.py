@@ -26,6 +26,7 @@ EXPORTS = [
     "gf8_sync_check", "gf8_set_stage_timing", "gf8_stage_times",
     "gf8_factor_update", "gf8_refresh_basis", "gf8_encode", "gf8_decode", "gf8_reduce_decoded",
     "gf8_encode_many", "gf8_reduce_decoded_many", "gf8_factor_update_many", "gf8_refresh_basis_many",
+    "gf8_encode_ef", "gf8_encode_ef_many",
     "gf8_step_host", "gf8_get_factor", "gf8_set_factor", "gf8_get_basis", "gf8_set_basis",
     "gf8_whiten_f32", "gf8_quantize_f32", "gf8_reduce_f32",
 ]
@@ -89,6 +90,9 @@ def lib():
         L.gf8_decode.argtypes = [vp, i32, vp, vp, vp, i32, vp]
         L.gf8_reduce_decoded.argtypes = [vp, i32, C.POINTER(vp), C.POINTER(vp), i32, i32, vp, i32, vp]
         L.gf8_encode_many.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(vp), i32, C.POINTER(vp), C.POINTER(vp), vp]
+        L.gf8_encode_ef.argtypes = [vp, i32, vp, i32, vp, vp, vp, vp]
+        L.gf8_encode_ef_many.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(vp), i32, C.POINTER(vp), C.POINTER(vp),
+                                         C.POINTER(vp), vp]
         L.gf8_reduce_decoded_many.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(vp), C.POINTER(vp), i32, i32,
                                               C.POINTER(vp), i32, vp]
         L.gf8_factor_update_many.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(vp), C.POINTER(vp), C.POINTER(i64),
@@ -265,6 +269,21 @@ class Ctx:
         dt = dt if dt is not None else _dt(grads[0])
         self._ck(lib().gf8_encode_many(self._h, n, int_array(layers), _ptr_array(grads), dt,
                                        _ptr_array(codes), _ptr_array(scale_invs), _stream()))
+
+    def encode_ef(self, layer, grad: torch.Tensor, resid: torch.Tensor, codes=None, scale_inv=None):
+        """f1: encode with error feedback; `resid` (FP32, the gradient's shape) is read and overwritten."""
+        assert resid.dtype == torch.float32 and resid.shape == grad.shape
+        if codes is None:
+            codes, scale_inv = self._payload_buffers(layer)
+        self._ck(lib().gf8_encode_ef(self._h, layer, _ptr(grad), _dt(grad), _ptr(resid), _ptr(codes), _ptr(scale_inv),
+                                     _stream()))
+        return codes, scale_inv
+
+    def encode_ef_many(self, layers, grads, resids, codes, scale_invs, dt=None):
+        n = len(layers)
+        dt = dt if dt is not None else _dt(grads[0])
+        self._ck(lib().gf8_encode_ef_many(self._h, n, int_array(layers), _ptr_array(grads), dt, _ptr_array(resids),
+                                          _ptr_array(codes), _ptr_array(scale_invs), _stream()))
 
     def reduce_decoded_many(self, layers, codes, scale_invs, R, outs, average=True, dt=None):
         """codes / scale_invs: flat lists of n*R tensors, index [i*R + r]."""

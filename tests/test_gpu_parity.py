@@ -8,7 +8,7 @@ import torch
 
 import oracle
 from paper_2607_07494_b200 import gf8, synth
-from tests._util import Case, bf16_bits, bf16_ordinal, code_mismatch, relfro, to_np64
+from tests._util import Case, bf16_bits, bf16_ordinal, code_mismatch, code_ordinal, relfro, to_np64
 
 pytestmark = pytest.mark.gpu
 
@@ -656,3 +656,78 @@ def test_step_host_matches_the_device_calls_bit_for_bit():
         ctx.sync_check()
         for i in ids:
             assert torch.equal(ho[i].view(torch.int16), outs[i].cpu().view(torch.int16)), (rep, i)
+
+
+# ---- f1: error feedback in the transformed coordinates (Alg. 1 l.11-15) -------------------------------------
+@pytest.mark.parametrize("prec", ["exact", "fast"])
+@pytest.mark.parametrize("scaling", [gf8.SCALE_TENSOR, gf8.SCALE_BLOCK128])
+def test_f1_error_feedback_chain_against_the_oracle(prec, scaling):
+    """Four steps of encode-with-feedback on a whitened tensor (ragged: several tiles and a tail).
+    Stage gate (upstream state handed across, as G3): with the GPU's own tapped U and the residual the GPU holds, the
+    oracle's O8 gives the same codes, scales and new residual BIT FOR BIT at every step.
+    End-to-end gate: the oracle's own chain (FP64 whitening, its own residual) against the GPU's.  Several results are
+    correct here: an element whose U~ sits within the transform tolerance of a rounding boundary may take either
+    neighbouring code, and from then on its residual -- and so its later U~ -- differs by a code step while both chains
+    stay valid.  What is unique is compared: on the elements whose codes have agreed at every earlier step, U~ = U + R
+    agrees within the transform tier, and those elements stay the overwhelming majority (EXACT: the code gate's 1e-4 per
+    step; FAST: the few-% flip rate DESIGN.md reports).  With a zero residual the payload is gf8_encode's."""
+    fast = prec == "fast"
+    c = Case(272, 400, 16, 16, gf8.SIDE_BOTH, "bf16" if fast else "f32", 81, scaling=scaling,
+             precision=gf8.PREC_FAST if fast else gf8.PREC_EXACT)
+    res = torch.zeros((c.m, c.n), dtype=torch.float32, device="cuda")
+    o_res = np.zeros((c.m, c.n), np.float32)
+    tol = (2e-3 + 2.0 ** -9) if fast else TOL_EXACT
+    agree = np.ones((c.m, c.n), bool)
+    for step in range(4):
+        g = c.rank_grad(step).contiguous()
+        before = res.clone()
+        if step == 0:
+            pc, ps = [t.clone() for t in c.ctx.encode(0, g)]
+        codes, sinv = c.ctx.encode_ef(0, g, res)
+        c.ctx.sync_check()
+        u = c.ctx.whiten_f32(0, g)
+        oc, os_, orr = oracle.ef_quantize(u.cpu().numpy(), before.cpu().numpy(), c.fmt, c.scaling)
+        if fast:
+            # the tensor-core transform is deterministic: the tap is the U the call quantized
+            if step == 0:
+                assert torch.equal(codes, pc) and torch.equal(sinv, ps)
+            assert np.array_equal(codes.cpu().numpy(), oc), step
+            assert np.array_equal(sinv.cpu().numpy().view(np.uint32), os_.view(np.uint32)), step
+            assert np.array_equal(res.cpu().numpy().view(np.uint32), orr.view(np.uint32)), step
+        else:
+            # the FP32 SIMT transform sums its split-K partials with atomics: two runs differ in the last bit, so the tap is
+            # the call's U only up to an ulp (the bit-exact statement for this tier is the Euclidean test below)
+            frac, worst = code_mismatch(codes.cpu().numpy(), oc)
+            assert frac <= MISMATCH_FRAC and worst <= 1, (step, frac, worst)
+            assert np.allclose(sinv.cpu().numpy(), os_, rtol=1e-6, atol=0)
+            same = codes.cpu().numpy() == oc
+            assert relfro(res.cpu().numpy()[same], orr[same]) <= 1e-4, step
+        o_before = o_res.copy()
+        o_codes, o_sinv, o_res, wt = oracle.encode_ef(to_np64(g), o_res, c.bG, c.bA, c.fmt, c.scaling)
+        ut_gpu = u.cpu().numpy().astype(np.float64) + before.cpu().numpy()
+        ut_orc = wt.astype(np.float64) + o_before
+        assert relfro(ut_gpu[agree], ut_orc[agree]) <= tol, step
+        d = np.abs(code_ordinal(codes.cpu().numpy()).astype(np.int64) - code_ordinal(o_codes).astype(np.int64))
+        assert fast or d[agree].max() <= 1, step
+        agree &= d == 0
+        assert agree.mean() >= (1.0 - (step + 1) * (0.08 if fast else 4 * MISMATCH_FRAC)), (step, agree.mean())
+
+
+def test_f1_error_feedback_euclidean_tensor_is_bit_exact():
+    """A GF8_SIDE_NONE tensor with feedback: U is the gradient itself, so the whole chain is bit-exact against O8
+    (BF16 and FP32 gradients, both formats, both scalings, batched with a repeated layer = two ranks)."""
+    for dt, fmt, scaling in [(torch.bfloat16, gf8.E4M3, gf8.SCALE_TENSOR), (torch.float32, gf8.E5M2, gf8.SCALE_BLOCK128)]:
+        lay = gf8.Layer(208, 336, gf8.SIDE_NONE, 0, 0, fmt, scaling)
+        ctx = gf8.create([lay], gf8.PREC_FAST)
+        res = [torch.zeros((208, 336), dtype=torch.float32, device="cuda") for _ in range(2)]
+        for step in range(3):
+            gs = [(synth.gradient(208, 336, "cuda", 83 + step, r) * (1 + r)).to(dt).contiguous() for r in range(2)]
+            before = [r.clone() for r in res]
+            codes = [torch.empty((208, 336), dtype=torch.uint8, device="cuda") for _ in range(2)]
+            sinvs = [torch.empty(lay.n_scales(), dtype=torch.float32, device="cuda") for _ in range(2)]
+            ctx.encode_ef_many([0, 0], gs, res, codes, sinvs)
+            ctx.sync_check()
+            for r in range(2):
+                oc, os_, orr = oracle.ef_quantize(gs[r].float().cpu().numpy(), before[r].cpu().numpy(), fmt, scaling)
+                assert np.array_equal(codes[r].cpu().numpy(), oc) and np.array_equal(sinvs[r].cpu().numpy(), os_)
+                assert np.array_equal(res[r].cpu().numpy().view(np.uint32), orr.view(np.uint32))
