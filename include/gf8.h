@@ -18,11 +18,21 @@
  *    codes: one byte per element, same layout.  Block scales: row-major over the
  *    ceil(d_out/128) x ceil(d_in/128) grid.
  *  - d_out and d_in must be multiples of 16 (else GF8_ERR_UNSUPPORTED).
- *  - `stream` is a cudaStream_t passed as void*.  Calls are asynchronous on that stream; they do
- *    not synchronise with the host, run no host eigensolver and have no CPU fallback.
- *  - The ctx owns factors, bases, multipliers and scratch.  encode / decode / reduce allocate
- *    nothing.  Factor accumulators (d^2 FP32 per side) are allocated by the first
- *    gf8_factor_update / gf8_set_factor of a layer.
+ *  - `stream` is a cudaStream_t passed as void*.  Calls are asynchronous on that stream, run no host
+ *    eigensolver and have no CPU fallback.  A ctx serves ONE stream at a time: its scratch is shared by
+ *    consecutive calls, so calls on different streams must be ordered by the caller.
+ *  - The ctx owns factors, bases, multipliers, scratch and cached launch plans.  What a call may do besides
+ *    launching kernels:
+ *      * FIRST call with a new argument list (layers, and for encode / decode the data pointers): builds and caches
+ *        the call's plan -- device item lists and TMA tensor maps -- with cudaMalloc and small synchronous copies.
+ *        A loop that reuses its buffers pays this once (64 plans are kept; the oldest is dropped after a
+ *        device synchronisation).
+ *      * buffers that grow allocate when they grow: factor accumulators (d^2 FP32 per side) at the first
+ *        gf8_factor_update / gf8_set_factor of a layer, the refresh arena, the error-feedback scratch, the
+ *        staging of gf8_step_host.
+ *      * steady state: no allocation, no host synchronisation -- except that the pinned records of the batched
+ *        factor / refresh calls are double-buffered and a call waits (cudaEventSynchronize) for the call two
+ *        before it if that one is still running.
  *  - Errors: a gf8_status is returned; nothing throws or aborts across the ABI.  Argument errors
  *    are detected before any launch.  gf8_last_error(ctx) gives a message for the last failure.
  *  - One ctx (hence one basis per layer) is shared by all R simulated ranks (S12).

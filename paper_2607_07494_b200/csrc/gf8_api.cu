@@ -660,7 +660,6 @@ gf8_status fast_factor_many(gf8_ctx* c, cudaStream_t st, const std::vector<FacRe
     const int grid = std::min(tiles, c->num_sms);
     factor_gemm_kernel<<<grid, F_THREADS, F_SMEM, st>>>(static_cast<const FactorJob*>(c->fac_d[b]), (int)n, tiles, c->d_err);
     LAUNCH_CHECK(c);
-    ++c->launches;
     CU_TRY(c, cudaEventRecord(c->fac_ev[b], st));
     c->fac_busy[b] = true;
     return GF8_OK;
@@ -1144,7 +1143,6 @@ gf8_status ef_quantize_dev(gf8_ctx* c, cudaStream_t st, const T* u, float* resid
     if (fmt == GF8_E4M3) ef_cast_kernel<T, 0><<<g, 256, 0, st>>>(u, resid, m, n, scaling, scale, scale_inv, codes);
     else ef_cast_kernel<T, 1><<<g, 256, 0, st>>>(u, resid, m, n, scaling, scale, scale_inv, codes);
     LAUNCH_CHECK(c);
-    c->launches += 3;
     return GF8_OK;
 }
 }  // namespace

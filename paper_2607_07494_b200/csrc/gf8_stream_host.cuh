@@ -154,7 +154,7 @@ gf8_status splan_build(gf8_ctx* c, SPlan* p, const std::vector<int>& lay, bool t
         const long long bytes = (long long)t.m * t.n * 2;
         // lead control: the last tensor that lies wholly more than S_LEAD_BYTES of gradient behind this one must be complete
         while (gate_next < i && T[gate_next].byte_pos + (long long)T[gate_next].m * T[gate_next].n * 2 + S_LEAD_BYTES <= t.byte_pos) ++gate_next;
-        const int gate = (tap || gate_next == 0 || getenv("GF8_P1ONLY")) ? -1 : gate_next - 1, gate_total = gate >= 0 ? T[gate].n_tiles : 0;
+        const int gate = (tap || gate_next == 0) ? -1 : gate_next - 1, gate_total = gate >= 0 ? T[gate].n_tiles : 0;
         for (int i0 = 0; t.useA && i0 < t.m; i0 += 256) p1.push_back({K_PANEL_P, i, i0, std::min(256, t.m - i0), gate, gate_total, 0, 0});
         for (int j0 = 0; t.useG && j0 < t.n; j0 += 256) p1.push_back({K_PANEL_Q, i, j0, std::min(256, t.n - j0), gate, gate_total, 0, 0});
         byte_pos += bytes;
@@ -173,7 +173,7 @@ gf8_status splan_build(gf8_ctx* c, SPlan* p, const std::vector<int>& lay, bool t
         auto emit = [&](int i, int pass) {
             for (int k = 0; k < T[i].n_tiles; ++k) tiles.push_back({i, (k / T[i].tiles_n) | ((k % T[i].tiles_n) << 16), pass, 0});
         };
-        for (int i = 0; i < nT && !getenv("GF8_P1ONLY"); ++i) {
+        for (int i = 0; i < nT; ++i) {
             if (T[i].mode == M_AMAX) { emit(i, P_AMAX); pendB.push_back({i, tiles.size()}); }
             else emit(i, P_SINGLE);
             while (headB < pendB.size() && tiles.size() - pendB[headB].second >= (size_t)S_PASS_LAG) emit(pendB[headB++].first, P_CAST);

@@ -731,3 +731,56 @@ def test_f1_error_feedback_euclidean_tensor_is_bit_exact():
                 oc, os_, orr = oracle.ef_quantize(gs[r].float().cpu().numpy(), before[r].cpu().numpy(), fmt, scaling)
                 assert np.array_equal(codes[r].cpu().numpy(), oc) and np.array_equal(sinvs[r].cpu().numpy(), os_)
                 assert np.array_equal(res[r].cpu().numpy().view(np.uint32), orr.view(np.uint32))
+
+
+def test_no_writes_outside_the_output_buffers():
+    """compute-sanitizer is closed on the GPU pool (profiles/r02_sanitizers.txt), so out-of-bounds stores are looked for
+    directly: every output of encode_many, encode_ef_many and reduce_decoded_many (codes, scales, residuals, gradients) is
+    carved out of one arena with 4 KB canary bands before, between and after; ragged shapes, whitened and Euclidean, both
+    scalings.  After the calls every canary byte must be untouched."""
+    shapes = [(272, 400, gf8.SIDE_BOTH, gf8.SCALE_TENSOR), (400, 464, gf8.SIDE_BOTH, gf8.SCALE_BLOCK128),
+              (208, 336, gf8.SIDE_NONE, gf8.SCALE_TENSOR), (144, 1008, gf8.SIDE_IN, gf8.SCALE_TENSOR),
+              (1008, 96, gf8.SIDE_NONE, gf8.SCALE_BLOCK128), (640, 256, gf8.SIDE_OUT, gf8.SCALE_TENSOR)]
+    lays = [gf8.Layer(m, n, side, 16, 16, gf8.E4M3, sc) for m, n, side, sc in shapes]
+    ctx = gf8.create(lays, gf8.PREC_FAST)
+    mu = torch.arange(1, 17, device="cuda", dtype=torch.float32) ** -2.0
+    for i, l in enumerate(lays):
+        if l.side & gf8.SIDE_IN:
+            ctx.set_basis(i, gf8.SIDE_IN, synth.rand_orthonormal(l.d_in, 16, "cuda", 91, i, 1).contiguous(), mu, 0.02)
+        if l.side & gf8.SIDE_OUT:
+            ctx.set_basis(i, gf8.SIDE_OUT, synth.rand_orthonormal(l.d_out, 16, "cuda", 91, i, 2).contiguous(), mu, 0.02)
+    R, BAND = 2, 4096
+    sizes = []                                        # (bytes, dtype, shape) of every output, in arena order
+    for l in lays:
+        for _ in range(R):
+            sizes += [(l.d_out * l.d_in, torch.uint8, (l.d_out, l.d_in)), (4 * l.n_scales(), torch.float32, (l.n_scales(),)),
+                      (4 * l.d_out * l.d_in, torch.float32, (l.d_out, l.d_in))]
+        sizes.append((2 * l.d_out * l.d_in, torch.bfloat16, (l.d_out, l.d_in)))
+    offs, pos = [], BAND
+    for nbytes, _, _ in sizes:
+        offs.append(pos)
+        pos += (nbytes + 255) // 256 * 256 + BAND
+    arena = torch.full((pos,), 0xA5, dtype=torch.uint8, device="cuda")
+    views = [arena[o:o + nb].view(dt).view(shape) for o, (nb, dt, shape) in zip(offs, sizes)]
+    mask = torch.ones(pos, dtype=torch.bool, device="cuda")
+    for o, (nb, _, _) in zip(offs, sizes):
+        mask[o:o + nb] = False
+    it = iter(views)
+    codes, sinvs, resid, outs = [], [], [], []
+    for l in lays:
+        for _ in range(R):
+            codes.append(next(it)); sinvs.append(next(it)); resid.append(next(it))
+        outs.append(next(it))
+    for r in resid:
+        r.zero_()
+    ids = [i for i in range(len(lays)) for _ in range(R)]
+    grads = [(synth.gradient(lays[i].d_out, lays[i].d_in, "cuda", 92, i) * (1.0 + q % R)).to(torch.bfloat16).contiguous()
+             for q, i in enumerate(ids)]
+    ctx.encode_many(ids, grads, codes, sinvs)
+    ctx.reduce_decoded_many(list(range(len(lays))), codes, sinvs, R, outs, average=True)
+    ctx.encode_ef_many(ids, grads, resid, codes, sinvs)
+    ctx.reduce_decoded_many(list(range(len(lays))), codes, sinvs, R, outs, average=True)
+    ctx.sync_check()
+    torch.cuda.synchronize()
+    assert bool((arena[mask] == 0xA5).all()), "a kernel wrote outside its output buffer"
+    assert all(bool(torch.isfinite(o.float()).all()) for o in outs)
