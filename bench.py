@@ -252,7 +252,8 @@ def run_reference(args):
 class Workload:
     """One codec workload resident in HBM: R simulated ranks x every tensor of a config, with its library context."""
 
-    def __init__(self, cfg_index, dev, layers=None, ranks=None, precision="fast", side=None, synthetic_basis=False, refresh_iters=2):
+    def __init__(self, cfg_index, dev, layers=None, ranks=None, precision="fast", side=None, synthetic_basis=False, refresh_iters=2,
+                 error_feedback=False):
         import torch
         from paper_2607_07494_b200 import gf8, synth
         self.torch, self.gf8, self.synth = torch, gf8, synth
@@ -327,10 +328,18 @@ class Workload:
         self.a_codes = gf8.ptr_array([self.codes[r][i] for i in ids for r in range(R)])
         self.a_sinvs = gf8.ptr_array([self.sinvs[r][i] for i in ids for r in range(R)])
         self.a_outs = gf8.ptr_array(self.outs)
+        # f1 (variant): one FP32 residual per (tensor, rank), zero at start, carried from step to step
+        self.resid = self.a_resid = None
+        if error_feedback:
+            self.resid = [[torch.zeros((t.d_out, t.d_in), dtype=torch.float32, device=dev) for t in cfg.tensors] for _ in range(R)]
+            self.a_resid = gf8.ptr_array([self.resid[r][i] for i in ids for r in range(R)])
         torch.cuda.synchronize()
 
     def encode_all(self):
-        self.ctx.encode_many(self.a_ids_all, self.a_grads, self.a_codes, self.a_sinvs, dt=self.dtc)
+        if self.a_resid is not None:
+            self.ctx.encode_ef_many(self.a_ids_all, self.a_grads, self.a_resid, self.a_codes, self.a_sinvs, dt=self.dtc)
+        else:
+            self.ctx.encode_many(self.a_ids_all, self.a_grads, self.a_codes, self.a_sinvs, dt=self.dtc)
 
     def reduce_all(self):
         self.ctx.reduce_decoded_many(self.a_ids, self.a_codes, self.a_sinvs, self.R, self.a_outs, average=True, dt=self.dtc)
@@ -364,8 +373,8 @@ class Workload:
         return e0.elapsed_time(e1), enc, red
 
     def free(self):
-        self.grads = self.codes = self.sinvs = self.outs = None
-        self.a_grads = self.a_codes = self.a_sinvs = self.a_outs = None
+        self.grads = self.codes = self.sinvs = self.outs = self.resid = None
+        self.a_grads = self.a_codes = self.a_sinvs = self.a_outs = self.a_resid = None
         self.ctx.destroy()
         self.torch.cuda.empty_cache()
 
@@ -524,6 +533,8 @@ def run_gf8(args):
             "config1 (llama300m-shaped, R=4, k=32)": variant("cfg1", dev, vs, cfg_index=1),
             "config4 (llama600m-shaped stress, R=16)": variant("cfg4", dev, vs, cfg_index=4),
             "exact (EXACT tier, FP32 SIMT path: the 1e-4 code gate; configs[2], first 2 layers)": variant("exact", dev, 2, cfg_index=2, layers=2, precision="exact"),
+            "error_feedback (f1, Alg. 1 l.11-15: encode with an FP32 residual per tensor and rank; first version, own launches; configs[2])":
+                variant("ef", dev, vs, cfg_index=2, error_feedback=True),
         }
 
     if rank == 0:
