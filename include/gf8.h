@@ -130,6 +130,21 @@ gf8_status gf8_encode(gf8_ctx* ctx, int layer, const void* grad, gf8_dtype dt, u
  * FP32 scratch (the codec's tap path), then two streaming kernels per tensor; see DESIGN.md for its byte budget. */
 gf8_status gf8_encode_ef(gf8_ctx* ctx, int layer, const void* grad, gf8_dtype dt, float* resid, uint8_t* codes,
                          float* scale_inv, void* stream);
+/* f2.  Synchronised scales (Algorithm 1 l.4-5 "s <- Scale(Wg); s <- AllReduce_MAX(s)", l.17-19 scale-
+ * synchronisation steps): the amax on its own, and the cast with an agreed amax.
+ *   gf8_amax: amax_out[n_scales] (DEVICE, FP32) <- amax of the tensor the quantizer would see (the whitened gradient; the
+ *             gradient itself for a GF8_SIDE_NONE layer), per tensor or per 128 x 128 block.  The caller takes the maximum
+ *             over ranks (its all-reduce) and passes it back as amax_sync.
+ *   gf8_encode_scaled: scale = fmax / amax_sync, scale_inv = amax_sync / fmax (the quantizer's rule and degenerate cases),
+ *             codes = Q(x * scale); scale_inv[n_scales] is written.  With amax_sync == gf8_amax's output the payload equals
+ *             gf8_encode's.
+ * f3.  Vulnerability profile: hits (DEVICE, two 64-bit counters, caller-zeroed, may be NULL) accumulates
+ *             hits[0] += number of codes equal to +-(largest finite value), hits[1] += number of nonzero inputs whose code
+ *             is +-0 or +-(smallest subnormal) -- fused into the cast, no extra pass.  A layer's score is
+ *             (hits[0] + hits[1]) / elements averaged over the profiling window (S16). */
+gf8_status gf8_amax(gf8_ctx* ctx, int layer, const void* grad, gf8_dtype dt, float* amax_out, void* stream);
+gf8_status gf8_encode_scaled(gf8_ctx* ctx, int layer, const void* grad, gf8_dtype dt, const float* amax_sync,
+                             uint8_t* codes, float* scale_inv, unsigned long long* hits, void* stream);
 /* R = 1 case of gf8_reduce_decoded without averaging. */
 gf8_status gf8_decode(gf8_ctx* ctx, int layer, const uint8_t* codes, const float* scale_inv,
                       void* grad_out, gf8_dtype dt, void* stream);

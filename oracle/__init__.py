@@ -61,6 +61,8 @@ def _declare(L):
     L.gf8o_fp8_from_float.restype = C.c_uint8
     L.gf8o_fp8_from_float.argtypes = [C.c_int, C.c_float]
     L.gf8o_quantize.argtypes = [C.c_int, C.c_int, _pf, _i64, _i64, _pb, _pf]
+    L.gf8o_amax.argtypes = [C.c_int, _pf, _i64, _i64, _pf]
+    L.gf8o_quantize_scaled.argtypes = [C.c_int, C.c_int, _pf, _i64, _i64, _pf, _pb, _pf, C.POINTER(C.c_uint64)]
     L.gf8o_ef_quantize.argtypes = [C.c_int, C.c_int, _pf, _pf, _i64, _i64, _pb, _pf]
     L.gf8o_reduce.argtypes = [C.c_int, C.c_int, C.POINTER(_pb), C.POINTER(_pf), C.c_int, C.c_int,
                               _i64, _i64, _pf]
@@ -121,6 +123,28 @@ def quantize(x_f32, fmt=E4M3, scaling=SCALE_TENSOR):
     sinv = np.empty(n_scales(scaling, m, n), dtype=np.float32)
     lib().gf8o_quantize(fmt, scaling, _p(x, _pf), m, n, _p(codes, _pb), _p(sinv, _pf))
     return codes, sinv
+
+
+def amax(x_f32, scaling=SCALE_TENSOR):
+    """O9: amax per tensor / per 128 x 128 block (bit-pattern maximum of |x|)."""
+    x = np.ascontiguousarray(x_f32, dtype=np.float32)
+    m, n = x.shape
+    out = np.empty(n_scales(scaling, m, n), np.float32)
+    lib().gf8o_amax(scaling, _p(x, _pf), m, n, _p(out, _pf))
+    return out
+
+
+def quantize_scaled(x_f32, amax_sync, fmt=E4M3, scaling=SCALE_TENSOR):
+    """O9: cast with an externally agreed amax.  Returns (codes, scale_inv, (upper hits, lower hits))."""
+    x = np.ascontiguousarray(x_f32, dtype=np.float32)
+    m, n = x.shape
+    a = np.ascontiguousarray(amax_sync, dtype=np.float32)
+    assert a.shape == (n_scales(scaling, m, n),)
+    codes = np.empty((m, n), np.uint8)
+    sinv = np.empty_like(a)
+    hits = (C.c_uint64 * 2)()
+    lib().gf8o_quantize_scaled(fmt, scaling, _p(x, _pf), m, n, _p(a, _pf), _p(codes, _pb), _p(sinv, _pf), hits)
+    return codes, sinv, (int(hits[0]), int(hits[1]))
 
 
 def ef_quantize(u_f32, resid_f32, fmt=E4M3, scaling=SCALE_TENSOR):

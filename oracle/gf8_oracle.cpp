@@ -18,6 +18,8 @@
 //   Jacobi / subspace residuals, trace, 2x2 closed form, exact-rank-k one-step, brute force
 //   factor            symmetry, trace, convergence to the generating covariance
 //   reduce            == mean of per-rank dequantisation; R=1 == dequantise
+//   sync scale / hits own amax == plain quantizer; doubled amax halves every value; hand-worked hit counts
+//                     (tests/golden/boundary_hits_example.txt); counts against the decoded table
 //   error feedback    zero residual == plain quantizer; worked example (tests/golden/ef_worked_example.txt); the
 //                     telescoping identity sum deq_t = sum u_t + R_0 - R_T; |R| <= half the widest code gap
 // Parity unpinned: the paper's printed Table I / II values (they need the authors' gradients).
@@ -179,6 +181,56 @@ void gf8o_ef_quantize(int fmt, int scaling, const float* u, float* resid, int64_
             volatile float r = ut[(size_t)(i * n + j)] - deq;
             resid[i * n + j] = r;
         }
+}
+
+// ------------------------------------------------------------------------------------------------
+// O9.  Synchronised scales and the vulnerability profile (f2, f3).
+//   f2 (Alg. 1 l.4-5 "s <- Scale(Wg); s <- AllReduce_MAX(s)"; l.17-19 scale-synchronisation steps): the
+//   amax is taken on its own (gf8o_amax), the ranks exchange it (max), and the cast uses the agreed value:
+//       scale = fmax / amax_sync, scale_inv = amax_sync / fmax     (O4's rule, same degenerate cases), code = Q(x * scale).
+//   f3 ("count how often encoded values hit the upper and lower FP8 boundaries"): with the codes of such a cast,
+//       upper hit: the code is +-(largest finite value)                      (the value saturated or rounded up to fmax)
+//       lower hit: x != 0 and the code is +-0 or +-(smallest subnormal)      (the value fell to the bottom of the format)
+//   (S16: the paper does not define "boundary"; the ratio of hits to elements is the layer's vulnerability score.)
+// ------------------------------------------------------------------------------------------------
+void gf8o_amax(int scaling, const float* x, int64_t m, int64_t n, float* amax) {
+    const int64_t bm = scaling == 0 ? 1 : (m + 127) / 128, bn = scaling == 0 ? 1 : (n + 127) / 128;
+    for (int64_t b = 0; b < bm * bn; ++b) {
+        const int64_t r0 = scaling == 0 ? 0 : (b / bn) * 128, r1 = scaling == 0 ? m : std::min(m, r0 + 128);
+        const int64_t c0 = scaling == 0 ? 0 : (b % bn) * 128, c1 = scaling == 0 ? n : std::min(n, c0 + 128);
+        uint32_t ab = 0;
+        for (int64_t i = r0; i < r1; ++i)
+            for (int64_t j = c0; j < c1; ++j) ab = std::max(ab, f2u(x[i * n + j]) & 0x7FFFFFFFu);
+        amax[b] = u2f(ab);
+    }
+}
+
+void gf8o_quantize_scaled(int fmt, int scaling, const float* x, int64_t m, int64_t n, const float* amax_sync,
+                          uint8_t* codes, float* scale_inv, uint64_t* hits2) {
+    const int64_t bn = (n + 127) / 128;
+    const float fmax = (float)gf8o_fp8_max(fmt);
+    const uint8_t top = gf8o_fp8_from_float(fmt, fmax);      // code of the largest finite value
+    uint64_t upper = 0, lower = 0;
+    const int64_t ns = scaling == 0 ? 1 : ((m + 127) / 128) * bn;
+    std::vector<float> scale((size_t)ns);
+    for (int64_t b = 0; b < ns; ++b) {
+        const float amax = amax_sync[b];
+        float sc = fmax / amax, si = amax / fmax;
+        if (amax == 0.0f || !std::isfinite(amax) || !std::isfinite(sc)) { sc = 1.0f; si = 1.0f; }
+        scale[(size_t)b] = sc;
+        scale_inv[b] = si;
+    }
+    for (int64_t i = 0; i < m; ++i)
+        for (int64_t j = 0; j < n; ++j) {
+            const int64_t sidx = scaling == 0 ? 0 : (i / 128) * bn + (j / 128);
+            volatile float y = x[i * n + j] * scale[(size_t)sidx];
+            const uint8_t c = gf8o_fp8_from_float(fmt, y);
+            codes[i * n + j] = c;
+            const uint8_t mag = c & 0x7F;
+            if (mag == (top & 0x7F)) ++upper;
+            if (x[i * n + j] != 0.0f && mag <= 1) ++lower;
+        }
+    if (hits2) { hits2[0] = upper; hits2[1] = lower; }
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -1224,6 +1224,97 @@ gf8_status gf8_encode_ef(gf8_ctx* ctx, int layer, const void* grad, gf8_dtype dt
     return gf8_encode_ef_many(ctx, 1, &layer, &grad, dt, &resid, &codes, &scale_inv, stream);
 }
 
+// ---- f2 / f3: amax on its own, and the cast with an agreed amax (+ boundary-hit counters) ---------------------------------
+extern "C++" {
+namespace {
+// The FP32 tensor the quantizer would see: the whitened gradient (tap path into the EF scratch), or null for a Euclidean layer
+// (the gradient itself is quantized).
+gf8_status quantizer_input(gf8_ctx* ctx, cudaStream_t st, int layer, const void* grad, gf8_dtype dt, const float** u) {
+    LayerState& L = ctx->layers[layer];
+    *u = nullptr;
+    if (L.desc.side == GF8_SIDE_NONE) return GF8_OK;
+    const size_t mn = (size_t)L.desc.d_out * L.desc.d_in;
+    if (mn > ctx->ef_cap) {
+        CU_TRY(ctx, cudaStreamSynchronize(st));
+        if (ctx->ef_scratch) CU_TRY(ctx, cudaFree(ctx->ef_scratch));
+        ctx->ef_scratch = nullptr; ctx->ef_cap = 0;
+        CU_TRY(ctx, cudaMalloc((void**)&ctx->ef_scratch, mn * sizeof(float)));
+        ctx->ef_cap = mn;
+    }
+    float* out = ctx->ef_scratch;
+    if (L.tc_ok && (ctx->precision == GF8_PREC_FAST || ctx->tc_exact))
+        GF_TRY(encode_dispatch(ctx, 1, &layer, &grad, dt, nullptr, nullptr, &out, st));
+    else if (dt == GF8_DT_BF16) GF_TRY(transform_simt<bf16>(ctx, st, L, (const bf16*)grad, out, false));
+    else GF_TRY(transform_simt<float>(ctx, st, L, (const float*)grad, out, false));
+    *u = out;
+    return GF8_OK;
+}
+template <typename T>
+gf8_status amax_dev(gf8_ctx* c, cudaStream_t st, const T* x, int64_t m, int64_t n, int scaling, uint32_t* amax_bits) {
+    if (scaling == GF8_SCALE_TENSOR) {
+        CU_TRY(c, cudaMemsetAsync(amax_bits, 0, sizeof(uint32_t), st));
+        const int64_t nvec = m * n * (int64_t)sizeof(T) / 16;
+        amax_tensor_kernel<T><<<grid_for(c, (nvec + 3) / 4, 256, 8), 256, 0, st>>>(x, m * n, amax_bits);
+    } else {
+        dim3 grid((unsigned)((n + 127) / 128), (unsigned)((m + 127) / 128));
+        amax_block_kernel<T><<<grid, 256, 0, st>>>(x, m, n, amax_bits);
+    }
+    LAUNCH_CHECK(c);
+    return GF8_OK;
+}
+template <typename T>
+gf8_status cast_scaled_dev(gf8_ctx* c, cudaStream_t st, const T* x, int64_t m, int64_t n, int fmt, int scaling,
+                           const float* scale, uint8_t* codes, unsigned long long* hits) {
+    const int g = grid_for(c, m * n / 16, 256, 8);
+    if (fmt == GF8_E4M3) cast_scaled_kernel<T, 0><<<g, 256, 0, st>>>(x, m, n, scaling, scale, codes, hits);
+    else cast_scaled_kernel<T, 1><<<g, 256, 0, st>>>(x, m, n, scaling, scale, codes, hits);
+    LAUNCH_CHECK(c);
+    return GF8_OK;
+}
+}  // namespace
+}  // extern "C++"
+
+gf8_status gf8_amax(gf8_ctx* ctx, int layer, const void* grad, gf8_dtype dt, float* amax_out, void* stream) {
+    GF_TRY(check_layer(ctx, layer));
+    LayerState& L = ctx->layers[layer];
+    if (!grad || !amax_out) return fail(ctx, GF8_ERR_INVALID_ARG, "null pointer");
+    if (!aligned16(grad)) return fail(ctx, GF8_ERR_UNSUPPORTED, "pointers must be 16-byte aligned");
+    if (dt != GF8_DT_BF16 && dt != GF8_DT_F32) return fail(ctx, GF8_ERR_INVALID_ARG, "bad dtype");
+    GF_TRY(check_basis(ctx, L, layer));
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t m = L.desc.d_out, n = L.desc.d_in;
+    const float* u = nullptr;
+    GF_TRY(quantizer_input(ctx, st, layer, grad, dt, &u));
+    if (u) GF_TRY(amax_dev<float>(ctx, st, u, m, n, L.desc.scaling, L.amax_bits));
+    else if (dt == GF8_DT_BF16) GF_TRY(amax_dev<bf16>(ctx, st, (const bf16*)grad, m, n, L.desc.scaling, L.amax_bits));
+    else GF_TRY(amax_dev<float>(ctx, st, (const float*)grad, m, n, L.desc.scaling, L.amax_bits));
+    amax_bits_to_float_kernel<<<(int)((L.n_scales + 255) / 256), 256, 0, st>>>(L.amax_bits, (int)L.n_scales, amax_out);
+    LAUNCH_CHECK(ctx);
+    return GF8_OK;
+}
+
+gf8_status gf8_encode_scaled(gf8_ctx* ctx, int layer, const void* grad, gf8_dtype dt, const float* amax_sync, uint8_t* codes,
+                             float* scale_inv, unsigned long long* hits, void* stream) {
+    GF_TRY(check_layer(ctx, layer));
+    LayerState& L = ctx->layers[layer];
+    if (!grad || !amax_sync || !codes || !scale_inv) return fail(ctx, GF8_ERR_INVALID_ARG, "null pointer");
+    if (!aligned16(grad) || !aligned16(codes)) return fail(ctx, GF8_ERR_UNSUPPORTED, "pointers must be 16-byte aligned");
+    if (dt != GF8_DT_BF16 && dt != GF8_DT_F32) return fail(ctx, GF8_ERR_INVALID_ARG, "bad dtype");
+    GF_TRY(check_basis(ctx, L, layer));
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t m = L.desc.d_out, n = L.desc.d_in;
+    const float* u = nullptr;
+    GF_TRY(quantizer_input(ctx, st, layer, grad, dt, &u));
+    scales_from_float_kernel<<<(int)((L.n_scales + 255) / 256), 256, 0, st>>>(amax_sync, (int)L.n_scales, fmax_of(L.desc.fmt), L.scale,
+                                                                              scale_inv);
+    LAUNCH_CHECK(ctx);
+    if (u) return cast_scaled_dev<float>(ctx, st, u, m, n, L.desc.fmt, L.desc.scaling, L.scale, codes, hits);
+    if (dt == GF8_DT_BF16) return cast_scaled_dev<bf16>(ctx, st, (const bf16*)grad, m, n, L.desc.fmt, L.desc.scaling, L.scale, codes, hits);
+    return cast_scaled_dev<float>(ctx, st, (const float*)grad, m, n, L.desc.fmt, L.desc.scaling, L.scale, codes, hits);
+}
+
 // ---- end-to-end with host buffers -----------------------------------------------------------------------------
 gf8_status gf8_step_host(gf8_ctx* ctx, int n, const int* layers, const void* const* grads_host, int R, int average,
                          void* const* out_host, gf8_dtype dt, void* stream) {

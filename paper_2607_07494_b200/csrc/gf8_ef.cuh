@@ -114,3 +114,83 @@ __global__ void __launch_bounds__(256) ef_cast_kernel(const T* __restrict__ u, f
 }
 
 }  // namespace gf8
+
+// ---- f2 / f3: cast with an externally agreed amax, boundary-hit counters fused into it ------------------------------------
+// (Alg. 1 l.4-5 and l.17-19: s <- AllReduce_MAX(s); "count how often encoded values hit the
+//  upper and lower FP8 boundaries".)  scale / scale_inv follow from amax_sync by the quantizer's rule (scales_kernel);
+//  upper hit: |code| is the largest finite value; lower hit: x != 0 and |code| is zero or the smallest subnormal.
+//  hits (nullable): two 64-bit counters, accumulated with one atomic pair per CTA.
+namespace gf8 {
+
+template <typename T, int FMT>
+__global__ void __launch_bounds__(256) cast_scaled_kernel(const T* __restrict__ x, int64_t m, int64_t n, int scaling,
+                                                          const float* __restrict__ scale, uint8_t* __restrict__ codes,
+                                                          unsigned long long* __restrict__ hits) {
+    constexpr uint32_t TOP = FMT == 0 ? 0x7Eu : 0x7Bu;        // E4M3 448 = S.1111.110, E5M2 57344 = S.11110.11
+    const int64_t ngroups = m * n / 16;
+    const int64_t bn = (n + 127) / 128;
+    uint32_t up = 0, lo = 0;
+    for (int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; g < ngroups; g += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t e0 = g * 16;
+        float s;
+        if (scaling == 0) s = __ldg(scale);
+        else { const int64_t r = e0 / n, c = e0 % n; s = __ldg(scale + (r / 128) * bn + c / 128); }
+        float f[16];
+        if (sizeof(T) == 2) {
+            const uint4* p = reinterpret_cast<const uint4*>(x + e0);
+            const uint4 a = ld_stream(p), b = ld_stream(p + 1);
+            unpack_bf16x8(a, f);
+            unpack_bf16x8(b, f + 8);
+        } else {
+            const uint4* p = reinterpret_cast<const uint4*>(x + e0);
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const uint4 a = ld_stream(p + u);
+                f[4 * u] = __uint_as_float(a.x); f[4 * u + 1] = __uint_as_float(a.y);
+                f[4 * u + 2] = __uint_as_float(a.z); f[4 * u + 3] = __uint_as_float(a.w);
+            }
+        }
+        uint32_t w[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+            w[q] = f32x4_to_fp8x4<FMT>(__fmul_rn(f[4 * q], s), __fmul_rn(f[4 * q + 1], s), __fmul_rn(f[4 * q + 2], s), __fmul_rn(f[4 * q + 3], s));
+        st_stream(reinterpret_cast<uint4*>(codes + e0), make_uint4(w[0], w[1], w[2], w[3]));
+        if (hits) {
+#pragma unroll
+            for (int q = 0; q < 16; ++q) {
+                const uint32_t mag = (w[q >> 2] >> (8 * (q & 3))) & 0x7Fu;
+                up += mag == TOP;
+                lo += (mag <= 1u) && (f[q] != 0.0f);
+            }
+        }
+    }
+    if (hits) {
+        __shared__ uint32_t s_up[8], s_lo[8];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) { up += __shfl_xor_sync(0xFFFFFFFFu, up, o); lo += __shfl_xor_sync(0xFFFFFFFFu, lo, o); }
+        if ((threadIdx.x & 31) == 0) { s_up[threadIdx.x >> 5] = up; s_lo[threadIdx.x >> 5] = lo; }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            unsigned long long u = 0, l = 0;
+            for (int q = 0; q < 8; ++q) { u += s_up[q]; l += s_lo[q]; }
+            if (u) atomicAdd(hits, u);
+            if (l) atomicAdd(hits + 1, l);
+        }
+    }
+}
+
+__global__ void amax_bits_to_float_kernel(const uint32_t* __restrict__ bits, int n, float* __restrict__ out) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = __uint_as_float(bits[i]);
+}
+__global__ void scales_from_float_kernel(const float* __restrict__ amax, int n, float fmax, float* __restrict__ scale,
+                                         float* __restrict__ scale_inv) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float s, si;
+    scales_from_amax(__float_as_uint(amax[i]) & 0x7FFFFFFFu, fmax, s, si);
+    scale[i] = s;
+    scale_inv[i] = si;
+}
+
+}  // namespace gf8

@@ -26,7 +26,7 @@ EXPORTS = [
     "gf8_sync_check", "gf8_set_stage_timing", "gf8_stage_times",
     "gf8_factor_update", "gf8_refresh_basis", "gf8_encode", "gf8_decode", "gf8_reduce_decoded",
     "gf8_encode_many", "gf8_reduce_decoded_many", "gf8_factor_update_many", "gf8_refresh_basis_many",
-    "gf8_encode_ef", "gf8_encode_ef_many",
+    "gf8_encode_ef", "gf8_encode_ef_many", "gf8_amax", "gf8_encode_scaled",
     "gf8_step_host", "gf8_get_factor", "gf8_set_factor", "gf8_get_basis", "gf8_set_basis",
     "gf8_whiten_f32", "gf8_quantize_f32", "gf8_reduce_f32",
 ]
@@ -90,6 +90,8 @@ def lib():
         L.gf8_decode.argtypes = [vp, i32, vp, vp, vp, i32, vp]
         L.gf8_reduce_decoded.argtypes = [vp, i32, C.POINTER(vp), C.POINTER(vp), i32, i32, vp, i32, vp]
         L.gf8_encode_many.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(vp), i32, C.POINTER(vp), C.POINTER(vp), vp]
+        L.gf8_amax.argtypes = [vp, i32, vp, i32, vp, vp]
+        L.gf8_encode_scaled.argtypes = [vp, i32, vp, i32, vp, vp, vp, vp, vp]
         L.gf8_encode_ef.argtypes = [vp, i32, vp, i32, vp, vp, vp, vp]
         L.gf8_encode_ef_many.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(vp), i32, C.POINTER(vp), C.POINTER(vp),
                                          C.POINTER(vp), vp]
@@ -269,6 +271,21 @@ class Ctx:
         dt = dt if dt is not None else _dt(grads[0])
         self._ck(lib().gf8_encode_many(self._h, n, int_array(layers), _ptr_array(grads), dt,
                                        _ptr_array(codes), _ptr_array(scale_invs), _stream()))
+
+    def amax(self, layer, grad: torch.Tensor):
+        """f2: amax (per tensor / per block) of what the quantizer would see for this gradient."""
+        out = torch.empty(self.layers[layer].n_scales(), dtype=torch.float32, device=self._tdev)
+        self._ck(lib().gf8_amax(self._h, layer, _ptr(grad), _dt(grad), _ptr(out), _stream()))
+        return out
+
+    def encode_scaled(self, layer, grad: torch.Tensor, amax_sync: torch.Tensor, hits: Optional[torch.Tensor] = None):
+        """f2 / f3: cast with an agreed amax; `hits` (int64[2] on the device, accumulated) counts upper / lower boundary hits."""
+        codes, scale_inv = self._payload_buffers(layer)
+        assert amax_sync.dtype == torch.float32 and amax_sync.numel() == self.layers[layer].n_scales()
+        assert hits is None or (hits.dtype == torch.int64 and hits.numel() == 2)
+        self._ck(lib().gf8_encode_scaled(self._h, layer, _ptr(grad), _dt(grad), _ptr(amax_sync), _ptr(codes), _ptr(scale_inv),
+                                         _ptr(hits), _stream()))
+        return codes, scale_inv
 
     def encode_ef(self, layer, grad: torch.Tensor, resid: torch.Tensor, codes=None, scale_inv=None):
         """f1: encode with error feedback; `resid` (FP32, the gradient's shape) is read and overwritten."""

@@ -784,3 +784,64 @@ def test_no_writes_outside_the_output_buffers():
     torch.cuda.synchronize()
     assert bool((arena[mask] == 0xA5).all()), "a kernel wrote outside its output buffer"
     assert all(bool(torch.isfinite(o.float()).all()) for o in outs)
+
+
+# ---- f2 / f3: synchronised scales and the boundary-hit profile (PAPER.md:310 Alg. 1 l.4-5, l.17-19; :277) ---------------
+@pytest.mark.parametrize("fmt", [gf8.E4M3, gf8.E5M2])
+@pytest.mark.parametrize("scaling", [gf8.SCALE_TENSOR, gf8.SCALE_BLOCK128])
+@pytest.mark.parametrize("dt", [torch.bfloat16, torch.float32])
+def test_f2_f3_euclidean_amax_scaled_cast_and_hits_bit_exact(fmt, scaling, dt):
+    """The Euclidean branch with a synchronised scale: the amax of each of two ranks, their maximum (the all-reduce), the
+    cast of both with the agreed value and the boundary-hit counters fused into it -- bit for bit against oracle O9,
+    on a ragged, heavy-tailed tensor.  With a rank's own amax the payload is gf8_encode's."""
+    lay = gf8.Layer(400, 272, gf8.SIDE_NONE, 0, 0, fmt, scaling)
+    ctx = gf8.create([lay], gf8.PREC_FAST)
+    g = torch.Generator(device="cuda").manual_seed(7 + fmt + 2 * scaling)
+    xs = [(torch.randn(400, 272, device="cuda", generator=g) * torch.exp(3 * torch.randn(400, 272, device="cuda", generator=g))
+           * (1 + r)).to(dt).contiguous() for r in range(2)]
+    xs[0][5, 7] = 0.0
+    am = [ctx.amax(0, x) for x in xs]
+    for x, a in zip(xs, am):
+        assert np.array_equal(a.cpu().numpy(), oracle.amax(x.float().cpu().numpy(), scaling))
+        c_own, s_own = [t.clone() for t in ctx.encode_scaled(0, x, a)]
+        c_ref, s_ref = ctx.encode(0, x)
+        assert torch.equal(c_own, c_ref) and torch.equal(s_own, s_ref)
+    sync = torch.maximum(am[0], am[1])
+    hits = torch.zeros(2, dtype=torch.int64, device="cuda")
+    want_up = want_lo = 0
+    for x in xs:
+        codes, sinv = ctx.encode_scaled(0, x, sync, hits)
+        oc, os_, (up, lo) = oracle.quantize_scaled(x.float().cpu().numpy(), sync.cpu().numpy(), fmt, scaling)
+        assert np.array_equal(codes.cpu().numpy(), oc) and np.array_equal(sinv.cpu().numpy().view(np.uint32), os_.view(np.uint32))
+        want_up += up; want_lo += lo
+    ctx.sync_check()
+    assert hits.tolist() == [want_up, want_lo] and want_up > 0 and want_lo > 0
+
+
+@pytest.mark.parametrize("prec", ["exact", "fast"])
+def test_f2_whitened_layer_with_an_agreed_scale(prec):
+    """Scale-synchronisation step of a GeoFP8 layer (Alg. 1 l.17-19): amax and cast act on the whitened gradient.  Stage gate:
+    on the GPU's own tapped U the amax, codes, scale and hit counts are the oracle's (FAST: bit for bit, the tensor-core
+    transform is deterministic; EXACT: the SIMT transform's atomics move the last bit, so within the code gate)."""
+    fast = prec == "fast"
+    c = Case(272, 400, 16, 16, gf8.SIDE_BOTH, "bf16" if fast else "f32", 85, precision=gf8.PREC_FAST if fast else gf8.PREC_EXACT)
+    g0, g1 = c.rank_grad(0).contiguous(), c.rank_grad(1).contiguous()
+    sync = torch.maximum(c.ctx.amax(0, g0), c.ctx.amax(0, g1))
+    hits = torch.zeros(2, dtype=torch.int64, device="cuda")
+    codes, sinv = c.ctx.encode_scaled(0, g0, sync, hits)
+    c.ctx.sync_check()
+    u = c.ctx.whiten_f32(0, g0).cpu().numpy()
+    oc, os_, (up, lo) = oracle.quantize_scaled(u, sync.cpu().numpy(), c.fmt, c.scaling)
+    assert np.array_equal(sinv.cpu().numpy().view(np.uint32), os_.view(np.uint32))
+    if fast:
+        assert np.array_equal(c.ctx.amax(0, g0).cpu().numpy(), oracle.amax(u))
+        assert np.array_equal(codes.cpu().numpy(), oc) and hits.tolist() == [up, lo]
+    else:
+        frac, worst = code_mismatch(codes.cpu().numpy(), oc)
+        assert frac <= MISMATCH_FRAC and worst <= 1
+        assert abs(hits[0].item() - up) <= 2 and abs(hits[1].item() - lo) <= max(2, lo // 100)
+    # end to end against the oracle's own whitening: the agreed amax is within the transform tier
+    _, _, wt0 = c.oracle_encode(g0)
+    _, _, wt1 = c.oracle_encode(g1)
+    want = max(np.abs(wt0).max(), np.abs(wt1).max())
+    assert abs(sync.item() - want) <= (2e-2 if fast else 1e-4) * want
