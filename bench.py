@@ -331,7 +331,7 @@ class Workload:
         # f1 (variant): one FP32 residual per (tensor, rank), zero at start, carried from step to step
         self.resid = self.a_resid = None
         if error_feedback:
-            self.resid = [[torch.zeros((t.d_out, t.d_in), dtype=torch.float32, device=dev) for t in cfg.tensors] for _ in range(R)]
+            self.resid = [[ctx.resid_new(i) for i in ids] for _ in range(R)]
             self.a_resid = gf8.ptr_array([self.resid[r][i] for i in ids for r in range(R)])
         torch.cuda.synchronize()
 

@@ -123,11 +123,15 @@ gf8_status gf8_encode(gf8_ctx* ctx, int layer, const void* grad, gf8_dtype dt, u
                       float* scale_inv, void* stream);
 /* f1.  gf8_encode with ERROR FEEDBACK in the transformed coordinates (PAPER.md:318 Algorithm 1 l.11-15; :354):
  *   U~ = U + R;  s = Scale(U~);  codes = Q(U~; s);  R <- U~ - Dequantize(codes; s)
- * U is the whitened gradient (the gradient itself for a GF8_SIDE_NONE layer).  resid: DEVICE, FP32, d_out*d_in, 16-byte
- * aligned, caller-owned, one buffer per (tensor, rank); zero it before the first step; it is read and overwritten.  Every
- * element is one IEEE FP32 add, multiply, cast, multiply and subtract: on the same U the codes, scales and residual are
- * bit-identical to oracle O8.  With resid == 0 the payload equals gf8_encode's.  First correct version: U goes through an
- * FP32 scratch (the codec's tap path), then two streaming kernels per tensor; see DESIGN.md for its byte budget. */
+ * U is the whitened gradient (the gradient itself for a GF8_SIDE_NONE layer).  resid: DEVICE, FP32, gf8_resid_size()
+ * floats, 16-byte aligned, caller-owned, one buffer per (tensor, rank); zero it before the first step; it is read and
+ * overwritten and is OPAQUE state: FAST contexts keep the residual of a whitened tensor-core layer (BF16 gradients) in the
+ * tile order of the update epilogue, into which the feedback is fused; every other case is row-major.  gf8_resid_export
+ * writes it out row-major [d_out][d_in] (out: DEVICE, d_out*d_in floats; dt = the gradients' type the buffer was used with).
+ * Every element is one IEEE FP32 add, multiply, cast, multiply and subtract: on the same U the codes, scales and residual are
+ * bit-identical to oracle O8.  With resid == 0 the payload equals gf8_encode's. */
+gf8_status gf8_resid_size(gf8_ctx* ctx, int layer, size_t* n_floats);
+gf8_status gf8_resid_export(gf8_ctx* ctx, int layer, gf8_dtype dt, const float* resid, float* out, void* stream);
 gf8_status gf8_encode_ef(gf8_ctx* ctx, int layer, const void* grad, gf8_dtype dt, float* resid, uint8_t* codes,
                          float* scale_inv, void* stream);
 /* f2.  Synchronised scales (Algorithm 1 l.4-5 "s <- Scale(Wg); s <- AllReduce_MAX(s)", l.17-19 scale-

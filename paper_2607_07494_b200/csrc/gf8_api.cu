@@ -295,7 +295,7 @@ gf8_status reduce_decoded_one(gf8_ctx* c, int layer, const uint8_t* const* codes
 
 
 // ---- FAST path: batched calls through cached plans of tensor-core items ---------------------------------------
-enum { PLAN_ENCODE = 1, PLAN_DECODE = 2, PLAN_WHITEN = 3 };
+enum { PLAN_ENCODE = 1, PLAN_DECODE = 2, PLAN_WHITEN = 3, PLAN_ENCODE_EF = 4 };
 
 inline void key_ptr(std::vector<uint64_t>& k, const void* p) { k.push_back((uint64_t)(uintptr_t)p); }
 
@@ -320,8 +320,11 @@ gf8_status aux_join(gf8_ctx* c, cudaStream_t st) {
 }
 
 // encode (PLAN_ENCODE) or the transform tap (PLAN_WHITEN: codes == nullptr, taps[i] receives FP32 W~).
+// resid != nullptr (f1, error feedback; every problem must be a tensor-core shape): resid[i] is the problem's FP32 residual,
+// added to W~ in the epilogues of the update passes and rewritten by the cast (gf8_tc.cuh, ef_add32 / ef_store32).
 gf8_status fast_encode_many(gf8_ctx* c, int n, const int* layers, const void* const* grads, gf8_dtype dt,
-                            uint8_t* const* codes, float* const* sinv, float* const* taps, cudaStream_t st) {
+                            uint8_t* const* codes, float* const* sinv, float* const* taps, cudaStream_t st,
+                            float* const* resid = nullptr) {
     using namespace gf8::tc;
     const bool tap = taps != nullptr;
     for (int i = 0; i < n; ++i) {
@@ -333,13 +336,14 @@ gf8_status fast_encode_many(gf8_ctx* c, int n, const int* layers, const void* co
         GF_TRY(check_basis(c, L, layers[i]));
     }
     std::vector<uint64_t> key;
-    key.push_back(tap ? PLAN_WHITEN : PLAN_ENCODE);
+    key.push_back(tap ? PLAN_WHITEN : (resid ? PLAN_ENCODE_EF : PLAN_ENCODE));
     key.push_back((uint64_t)dt);
     key.push_back((uint64_t)n);
     for (int i = 0; i < n; ++i) {
         key.push_back((uint64_t)layers[i]);
         key_ptr(key, grads[i]);
         if (tap) key_ptr(key, taps[i]); else { key_ptr(key, codes[i]); key_ptr(key, sinv[i]); }
+        if (resid) key_ptr(key, resid[i]);
     }
     Plan* p = nullptr;
     auto found = c->plans.find(key);
@@ -347,6 +351,7 @@ gf8_status fast_encode_many(gf8_ctx* c, int n, const int* layers, const void* co
     else {
         p = new (std::nothrow) Plan();
         if (!p) return fail(c, GF8_ERR_NOMEM, "host allocation failed");
+        p->ef = resid != nullptr;
         PlanBuilder pb;
         std::map<int, size_t> occurrence;
         std::vector<int> tc_idx;
@@ -402,7 +407,9 @@ gf8_status fast_encode_many(gf8_ctx* c, int n, const int* layers, const void* co
                     f.out_map = pb.add_map(codes[i], mc);
                 }
             }
-            add_transform(pb, L, slot, src_map, src_lo_map, false, split, f, c->opt);
+            EngineOptions opt = c->opt;
+            if (resid) { f.resid = resid[i]; opt.fuse = false; }      // (the parked-tile update has no feedback epilogue)
+            add_transform(pb, L, slot, src_map, src_lo_map, false, split, f, opt);
         }
         if (s == GF8_OK) s = plan_finish(c, pb, p);
         if (s == GF8_OK) s = plan_store(c, key, p);
@@ -1148,6 +1155,22 @@ gf8_status ef_quantize_dev(gf8_ctx* c, cudaStream_t st, const T* u, float* resid
 }  // namespace
 }  // extern "C++"
 
+namespace {
+// Is this layer's residual kept in the tensor-core epilogue's tiled layout (gf8_tc.cuh, EF_TILE) for gradients of type dt?
+bool ef_tiled(const gf8_ctx* ctx, const LayerState& L, gf8_dtype dt) {
+    return dt == GF8_DT_BF16 && ctx->precision == GF8_PREC_FAST && L.tc_ok && L.desc.side != GF8_SIDE_NONE;
+}
+__global__ void resid_export_kernel(const float* __restrict__ resid, int64_t m, int64_t n, float* __restrict__ out) {
+    const int64_t nct = (n + 127) >> 7;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < m * n; idx += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t i = idx / n, j = idx % n;
+        const int r = (int)(i & 127), c = (int)(j & 127);
+        const int64_t tile = ((i >> 7) * nct + (j >> 7)) * gf8::tc::EF_TILE;
+        out[idx] = resid[tile + ((((c >> 6) * 2 + ((c >> 5) & 1)) * 8 + ((c & 31) >> 2)) * 128 + r) * 4 + (c & 3)];
+    }
+}
+}  // namespace
+
 gf8_status gf8_encode_ef_many(gf8_ctx* ctx, int n, const int* layers, const void* const* grads, gf8_dtype dt,
                               float* const* resid, uint8_t* const* codes, float* const* scale_inv, void* stream) {
     if (!ctx) return GF8_ERR_INVALID_ARG;
@@ -1163,21 +1186,36 @@ gf8_status gf8_encode_ef_many(gf8_ctx* ctx, int n, const int* layers, const void
     }
     CU_TRY(ctx, cudaSetDevice(ctx->device));
     cudaStream_t st = (cudaStream_t)stream;
-    // Whitened tensors: the codec's tap path writes U = W~ (FP32) for a chunk of problems in one batched call, then the
-    // feedback kernels quantize U + R per tensor.  A chunk holds at most EF_CHUNK_ELEMS elements of scratch.
+    // FAST + BF16 gradients of tensor-core shapes: the feedback is FUSED into the update epilogues of the item engine (one
+    // batched call, 5 launches: the residual is added in the amax pass and in the cast pass, which also rewrites it).
+    std::vector<int> fused, rest;
+    for (int i = 0; i < n; ++i) {
+        const LayerState& L = ctx->layers[layers[i]];
+        if (ef_tiled(ctx, L, dt)) fused.push_back(i);
+        else rest.push_back(i);
+    }
+    if (!fused.empty()) {
+        std::vector<int> fl; std::vector<const void*> fg; std::vector<float*> fr; std::vector<uint8_t*> fc; std::vector<float*> fs;
+        for (int i : fused) { fl.push_back(layers[i]); fg.push_back(grads[i]); fr.push_back(resid[i]); fc.push_back(codes[i]); fs.push_back(scale_inv[i]); }
+        GF_TRY(fast_encode_many(ctx, (int)fused.size(), fl.data(), fg.data(), dt, fc.data(), fs.data(), nullptr, st, fr.data()));
+    }
+    // The rest.  Whitened tensors: the codec's tap path writes U = W~ (FP32) for a chunk of problems in one batched call, then
+    // the feedback kernels quantize U + R per tensor; a chunk holds at most EF_CHUNK_ELEMS elements of scratch.  Euclidean
+    // tensors: the feedback kernels act on the gradient itself.
     constexpr size_t EF_CHUNK_ELEMS = size_t(1) << 28;
+    const int nr = (int)rest.size();
     int i0 = 0;
-    while (i0 < n) {
+    while (i0 < nr) {
         size_t elems = 0;
         int i1 = i0;
-        std::vector<int> wl;                    // whitened problems of the chunk
+        std::vector<int> wl;                    // whitened problems of the chunk (indices into the call's lists)
         std::vector<size_t> woff;
-        for (; i1 < n; ++i1) {
-            const LayerState& L = ctx->layers[layers[i1]];
+        for (; i1 < nr; ++i1) {
+            const LayerState& L = ctx->layers[layers[rest[i1]]];
             if (L.desc.side == GF8_SIDE_NONE) continue;
             const size_t mn = (size_t)L.desc.d_out * L.desc.d_in;
             if (!wl.empty() && elems + mn > EF_CHUNK_ELEMS) break;
-            wl.push_back(i1); woff.push_back(elems);
+            wl.push_back(rest[i1]); woff.push_back(elems);
             elems += mn;
         }
         if (elems > ctx->ef_cap) {
@@ -1198,7 +1236,8 @@ gf8_status gf8_encode_ef_many(gf8_ctx* ctx, int n, const int* layers, const void
         }
         if (!tl.empty()) GF_TRY(encode_dispatch(ctx, (int)tl.size(), tl.data(), tg.data(), dt, nullptr, nullptr, tt.data(), st));
         size_t q = 0;
-        for (int i = i0; i < i1; ++i) {
+        for (int k = i0; k < i1; ++k) {
+            const int i = rest[k];
             LayerState& L = ctx->layers[layers[i]];
             const int64_t m = L.desc.d_out, nn = L.desc.d_in;
             if (L.desc.side == GF8_SIDE_NONE) {
@@ -1216,6 +1255,30 @@ gf8_status gf8_encode_ef_many(gf8_ctx* ctx, int n, const int* layers, const void
         }
         i0 = i1;
     }
+    return GF8_OK;
+}
+
+gf8_status gf8_resid_size(gf8_ctx* ctx, int layer, size_t* n_floats) {
+    GF_TRY(check_layer(ctx, layer));
+    if (!n_floats) return fail(ctx, GF8_ERR_INVALID_ARG, "null pointer");
+    const LayerState& L = ctx->layers[layer];
+    *n_floats = (size_t)((L.desc.d_out + 127) / 128) * ((L.desc.d_in + 127) / 128) * gf8::tc::EF_TILE;
+    return GF8_OK;
+}
+
+gf8_status gf8_resid_export(gf8_ctx* ctx, int layer, gf8_dtype dt, const float* resid, float* out, void* stream) {
+    GF_TRY(check_layer(ctx, layer));
+    if (!resid || !out) return fail(ctx, GF8_ERR_INVALID_ARG, "null pointer");
+    if (dt != GF8_DT_BF16 && dt != GF8_DT_F32) return fail(ctx, GF8_ERR_INVALID_ARG, "bad dtype");
+    const LayerState& L = ctx->layers[layer];
+    CU_TRY(ctx, cudaSetDevice(ctx->device));
+    const int64_t m = L.desc.d_out, n = L.desc.d_in;
+    if (!ef_tiled(ctx, L, dt)) {
+        CU_TRY(ctx, cudaMemcpyAsync(out, resid, sizeof(float) * (size_t)(m * n), cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+        return GF8_OK;
+    }
+    resid_export_kernel<<<grid_for(ctx, m * n, 256, 8), 256, 0, (cudaStream_t)stream>>>(resid, m, n, out);
+    LAUNCH_CHECK(ctx);
     return GF8_OK;
 }
 

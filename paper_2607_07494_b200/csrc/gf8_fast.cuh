@@ -17,6 +17,7 @@ struct Plan {
     int stage_off[8] = {0, 0, 0, 0, 0, 0, 0, 0}, stage_cnt[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     int stage_wide[8] = {0, 0, 0, 0, 0, 0, 0, 0};  // the stage holds 256-row panel items: wide operand stages (kmode 3)
     int stage_base[8] = {0, 0, 0, 0, 0, 0, 0, 0};  // streamed base tiles per item in that stage's launch (0, 1 or 2)
+    bool ef = false;                     // f1: the update stages run the error-feedback instance of the kernel
     int runs = 0;                        // launches so far: the first one acquires its tensor maps with proxy fences
     int* d_ctr = nullptr;                // one item counter per stage (dynamic item hand-out), zeroed before every run
     uint32_t* d_amax = nullptr;          // one word per TC problem (per-tensor scaling)
@@ -54,7 +55,9 @@ gf8_status fast_init(gf8_ctx* c) {
     GF_TRY(dmalloc(c, &c->d_err, 4));
     GF_TRY(dmalloc(c, &c->d_prof, (size_t)32768));
     CU_TRY(c, cudaMemset(c->d_err, 0, 4 * sizeof(int)));
-    CU_TRY(c, cudaFuncSetAttribute(gf8::tc::tc_items_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    CU_TRY(c, cudaFuncSetAttribute(gf8::tc::tc_items_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   gf8::tc::SMEM_BYTES));
+    CU_TRY(c, cudaFuncSetAttribute(gf8::tc::tc_items_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                    gf8::tc::SMEM_BYTES));
     return GF8_OK;
 }
@@ -151,20 +154,27 @@ gf8_status fast_slot(gf8_ctx* c, LayerState& L, size_t idx, bool need_src16, boo
     if (!L.slots[idx]) {
         Slot* s = new (std::nothrow) Slot();
         if (!s) return fail(c, GF8_ERR_NOMEM, "host allocation failed");
+        // the slot is published only once every buffer and map exists: a failed attempt leaves no half-built slot behind
+        // (its device buffers stay on the context's allocation list and are released by gf8_destroy)
+        auto init = [&]() -> gf8_status {
+            if (kpA) {
+                GF_TRY(dmalloc(c, &s->Pp, m * kpA));
+                GF_TRY(make_map(c, s->map_Pp, s->Pp, m, kpA, kpA));
+            }
+            if (kpG) {
+                GF_TRY(dmalloc(c, &s->Qt, n * kpG));
+                GF_TRY(dmalloc(c, &s->Qpt, n * kpG));
+                GF_TRY(make_map(c, s->map_Qpt, s->Qpt, n, kpG, kpG));
+            }
+            if (kpA && kpG) {
+                GF_TRY(dmalloc(c, &s->SEA, kpG * kpA));
+                GF_TRY(make_map(c, s->map_SEA, s->SEA, kpG, kpA, kpA));
+            }
+            return GF8_OK;
+        };
+        const gf8_status st = init();
+        if (st != GF8_OK) { delete s; return st; }
         L.slots[idx] = s;
-        if (kpA) {
-            GF_TRY(dmalloc(c, &s->Pp, m * kpA));
-            GF_TRY(make_map(c, s->map_Pp, s->Pp, m, kpA, kpA));
-        }
-        if (kpG) {
-            GF_TRY(dmalloc(c, &s->Qt, n * kpG));
-            GF_TRY(dmalloc(c, &s->Qpt, n * kpG));
-            GF_TRY(make_map(c, s->map_Qpt, s->Qpt, n, kpG, kpG));
-        }
-        if (kpA && kpG) {
-            GF_TRY(dmalloc(c, &s->SEA, kpG * kpA));
-            GF_TRY(make_map(c, s->map_SEA, s->SEA, kpG, kpA, kpA));
-        }
     }
     Slot* s = L.slots[idx];
     if (need_src16 && !s->src16) {
@@ -227,6 +237,7 @@ struct Final {                  // what the last stage of a transform does with 
     uint32_t* done;             // fused update: the tensor's parked-tile counter (next to its amax word)
     int base_map[2];            // TMA-streamed base tile(s) (hi [+ lo]); -1: base read straight from global memory
     int out_map;                // TMA store map of the output (codes or BF16); -1: direct stores
+    float* resid;               // f1: the tensor's FP32 error-feedback residual (null: plain codec)
 };
 
 inline Item blank_item() {
@@ -357,6 +368,7 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
             it.base_type = f.base_type; it.base_map[0] = f.base_map[0] + 1;
             it.row0 = i0; it.col0 = 0; it.rows = std::min(256, m - i0); it.cols = n;
             it.mode = f.mode; it.out = f.out; it.out_ld = n; it.out_map = f.out_map; it.scale_inv_out = f.scale_inv;
+            it.out_lo = f.resid;                                   // (amax / cast modes: out_lo carries the feedback residual)
             if (f.mode == EPI_AMAX) {
                 it.amax = f.amax;
                 pb.stage[5].push_back(it);
@@ -390,13 +402,13 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
                 it.base = f.done; it.base_ld = n_tiles;
                 pb.stage[7].push_back(it);
             } else if (f.mode == EPI_AMAX) {
-                it.amax = f.amax;
+                it.amax = f.amax; it.out_lo = f.resid; it.out_ld = n;
                 pb.stage[3].push_back(it);
                 it.mode = EPI_CAST; it.out = f.out; it.out_ld = n; it.scale_inv_out = f.scale_inv; it.out_map = f.out_map;
                 it.write_scale = (i0 == 0 && j0 == 0) ? 1 : 0;
                 pb.stage[4].push_back(it);
             } else if (f.mode == EPI_BLOCKCAST) {
-                it.out = f.out; it.out_ld = n; it.out_map = f.out_map;
+                it.out = f.out; it.out_ld = n; it.out_map = f.out_map; it.out_lo = f.resid;
                 it.scale_inv_out = f.scale_inv + (size_t)(i0 / 128) * tiles_n + j0 / 128;
                 pb.stage[3].push_back(it);
             } else {
@@ -582,7 +594,8 @@ gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
             else { CU_TRY(c, cudaEventCreate(&sev.a)); CU_TRY(c, cudaEventCreate(&sev.b)); }
             CU_TRY(c, cudaEventRecord(sev.a, st));
         }
-        gf8::tc::tc_items_kernel<<<grid, gf8::tc::THREADS, gf8::tc::SMEM_BYTES, st>>>(
+        auto* kern = (p->ef && s >= 3) ? gf8::tc::tc_items_kernel<true> : gf8::tc::tc_items_kernel<false>;     // (f1: update stages only)
+        kern<<<grid, gf8::tc::THREADS, gf8::tc::SMEM_BYTES, st>>>(
             p->d_items + p->stage_off[s], p->stage_cnt[s], p->d_maps, c->d_err, n_stages, n_base, n_bslots, kmode, dbg, (dbg & 4) ? c->d_prof : nullptr,
             (fuse || c->opt.static_items) ? nullptr : p->d_ctr + s);
         if (c->stage_timing) { CU_TRY(c, cudaEventRecord(sev.b, st)); c->stage_events.push_back(sev); }

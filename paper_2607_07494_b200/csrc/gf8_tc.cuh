@@ -439,6 +439,43 @@ __device__ __forceinline__ void tile_values32(uint32_t taddr, uint32_t row, int 
 
 // Returns true if a TMA store was issued from `tile` (the caller waits for its smem reads before reuse).
 // All eight warps share the tile: warp w covers rows 32 (w & 3) .. +31 of the 64-column half w >> 2.
+// ---- error feedback (f1; Alg. 1 l.11-15) fused into the update epilogue --------------------------------------
+// An EPI_AMAX / EPI_CAST / EPI_BLOCKCAST item whose out_lo is non-null carries the tensor's FP32 residual R there: the epilogue
+// quantizes U~ = W~ + R and, in the cast, writes R <- U~ - val(code) * scale_inv.  One FP32 rounding per operation, like oracle
+// O8.  R lives in the EPILOGUE'S OWN LAYOUT ("tiled", EF_TILE floats per 128 x 128 tile, tiles row-major over the padded
+// tensor): element (r, 64 h + 32 g + 4 q + e) of a tile sits at (((2 h + g) 8 + q) 128 + r) 4 + e, so that the 32 lanes of a
+// warp -- 32 consecutive rows -- read one contiguous 512 B per load instruction.  (With a row-major R every lane touches its
+// own 128 B line: the load/store unit then serialises 32 lines per instruction and the two update passes take 15 + 30 ms
+// instead of 2 + 3.3, measured.)  gf8_resid_export converts to row-major.
+// `valid` = columns of this 32-column group inside the tensor (multiple of 4).
+constexpr int EF_TILE = 128 * 128;
+__device__ __forceinline__ void ef_add32(const float* __restrict__ grp /* tile + ((2h+g) 8 * 128 + r) * 4 */, int valid, float* v) {
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        if (4 * q < valid) {
+            const float4 t = __ldcg(reinterpret_cast<const float4*>(grp + q * 512));
+            v[4 * q] = __fadd_rn(v[4 * q], t.x); v[4 * q + 1] = __fadd_rn(v[4 * q + 1], t.y);
+            v[4 * q + 2] = __fadd_rn(v[4 * q + 2], t.z); v[4 * q + 3] = __fadd_rn(v[4 * q + 3], t.w);
+        }
+    }
+}
+template <int FMT>
+__device__ __forceinline__ void ef_store32(float* __restrict__ grp, int valid, const float* ut, const uint4& c0, const uint4& c1, float si) {
+    const uint32_t w[8] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        if (4 * q < valid) {
+            float val[4];
+            fp8x4_to_f32x4<FMT>(w[q], val);
+            float4 o;
+            o.x = __fsub_rn(ut[4 * q], __fmul_rn(val[0], si)); o.y = __fsub_rn(ut[4 * q + 1], __fmul_rn(val[1], si));
+            o.z = __fsub_rn(ut[4 * q + 2], __fmul_rn(val[2], si)); o.w = __fsub_rn(ut[4 * q + 3], __fmul_rn(val[3], si));
+            __stcg(reinterpret_cast<float4*>(grp + q * 512), o);
+        }
+    }
+}
+
+template <bool EF>
 __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc, uint32_t tile, int n_base, int warp,
                                               int lane, uint32_t* s_red, const CUtensorMap* maps, float cast_scale, float cast_si,
                                               int row0, int col0, bool write_scale, float* sinv_out, uint32_t* run_max) {
@@ -451,13 +488,20 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
     const bool lead = r == 0 && h0 == 0;
     const int mode = it.mode, fmt = it.fmt;
     float v[32];
-    float scale = 1.0f;
+    float scale = 1.0f, si_cast = cast_si;
+    // error feedback: the tensor's residual row segment under this tile (null: plain codec)
+    float* resid = (EF && (mode == EPI_AMAX || mode == EPI_CAST || mode == EPI_BLOCKCAST)) ? reinterpret_cast<float*>(it.out_lo) : nullptr;
+    const bool ef_row_ok = row0 + r < it.row0 + it.rows;
+    // (this thread's first group in the tile: h = 0, g = 0, q = 0)
+    float* resid_row = resid ? resid + ((int64_t)(row0 >> 7) * ((it.out_ld + 127) >> 7) + (col0 >> 7)) * EF_TILE + r * 4 : nullptr;
+    const int ef_cols = it.col0 + it.cols - col0;            // columns of the tensor from this tile's origin on
     if (mode == EPI_BLOCKCAST || mode == EPI_AMAX) {
         uint32_t loc = 0;
         for (int h = h0; h < h1; ++h)
 #pragma unroll
             for (int g = 0; g < 2; ++g) {
                 tile_values32(taddr0 + 64u * h, row_lo + 16384u * h, n_base, r, g, v);
+                if (resid && ef_row_ok) ef_add32(resid_row + (2 * h + g) * 4096, ef_cols - 64 * h - 32 * g, v);
                 // max |v| two elements per instruction (FMNMX3, NaN-propagating: a NaN amax orders above every finite value
                 // as an integer, like the bit-pattern maximum it replaces)
                 float mx = __uint_as_float(loc);
@@ -475,6 +519,7 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
         const uint32_t bits = epi_block_max(loc, warp, lane, s_red);
         float si;
         scales_from_amax(bits, fmt == 0 ? 448.0f : 57344.0f, scale, si);
+        si_cast = si;
         if (lead) *sinv_out = si;
     } else if (mode == EPI_CAST) {
         scale = cast_scale;                       // (from the tensor's amax, once per item by the caller)
@@ -491,8 +536,13 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
 #pragma unroll
             for (int g = 0; g < 2; ++g) {
                 tile_values32(taddr0 + 64u * h, row_lo + 16384u * h, n_base, r, g, v);
+                if (resid && ef_row_ok) ef_add32(resid_row + (2 * h + g) * 4096, ef_cols - 64 * h - 32 * g, v);
                 cd[2 * g] = fmt == 0 ? codes16<0>(v, scale) : codes16<1>(v, scale);
                 cd[2 * g + 1] = fmt == 0 ? codes16<0>(v + 16, scale) : codes16<1>(v + 16, scale);
+                if (resid && ef_row_ok) {
+                    if (fmt == 0) ef_store32<0>(resid_row + (2 * h + g) * 4096, ef_cols - 64 * h - 32 * g, v, cd[2 * g], cd[2 * g + 1], si_cast);
+                    else ef_store32<1>(resid_row + (2 * h + g) * 4096, ef_cols - 64 * h - 32 * g, v, cd[2 * g], cd[2 * g + 1], si_cast);
+                }
             }
             if (row_ok) {
                 uint8_t* p = reinterpret_cast<uint8_t*>(it.out) + (int64_t)grow * it.out_ld + col0 + 64 * h;
@@ -554,6 +604,8 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
 // TMEM accumulators).  The producer warp copies each item descriptor into a 4-slot shared-memory ring one item
 // ahead, so no role waits on a global load.  `err` is set (and the kernel drains) if a barrier wait times out,
 // so a pipeline bug cannot hang the GPU.
+// EF: the error-feedback epilogue (f1) is compiled into its own instance, so the default kernel keeps its registers.
+template <bool EF>
 __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __restrict__ items, int n_items,
                                                               const CUtensorMap* __restrict__ maps, int* err,
                                                               int n_stages, int n_base, int n_bslots, int kmode, int dbg_in,
@@ -1115,8 +1167,26 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 const Item& it = *item_slot(slot);
                 const int nrb = (it.rows + 127) >> 7, nct = (it.cols + 127) >> 7;
                 uint32_t run_max = 0;
+                // error feedback: the residual of a tile is asked into L2 two tiles ahead (a warp's share of a tile is 16 chunks
+                // of 512 B = 64 lines: two per lane), so the epilogue's loads find it there instead of waiting on DRAM
+                const float* ef_base = (EF && (it.mode == EPI_AMAX || it.mode == EPI_CAST || it.mode == EPI_BLOCKCAST))
+                                           ? reinterpret_cast<const float*>(it.out_lo) : nullptr;
+                auto ef_prefetch = [&](int t) {
+                    if (!ef_base || t >= nct * nrb) return;
+                    const int pct = t / nrb, prb = t % nrb;
+                    const float* tile = ef_base + ((int64_t)((it.row0 >> 7) + prb) * ((it.out_ld + 127) >> 7) + pct) * EF_TILE;
+#pragma unroll
+                    for (int u = 0; u < 2; ++u) {
+                        const int line = 2 * lane + u, chunk = line >> 2, sub = line & 3;      // chunk = g * 8 + q of this warp's half
+                        const float* a = tile + (((2 * (warp >> 2) + (chunk >> 3)) * 8 + (chunk & 7)) * 128 + 32 * (warp & 3) + 8 * sub) * 4;
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(a));
+                    }
+                };
+                ef_prefetch(0);
+                ef_prefetch(1);
                 for (int ct = 0; ct < nct && ok; ++ct)
                     for (int rb = 0; rb < nrb && ok; ++rb, ++s_tiles) {
+                        ef_prefetch(ct * nrb + rb + 2);
                         const uint32_t sacc = s_tiles % n_acc, saph = (s_tiles / n_acc) & 1u;
                         const uint32_t sbs = s_bs, sbph = s_bph;       // = s_tiles % n_bslots, (s_tiles / n_bslots) & 1
                         if (++s_bs == (uint32_t)n_bslots) { s_bs = 0; s_bph ^= 1u; }
@@ -1127,7 +1197,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                         tc_fence_after();
                         const long long t_s0 = prof ? clock64() : 0;
                         if (!(dbg & 32))
-                            epilogue_tile(it, tmem_base + sacc * 128u, base_tile(sbs), 1, warp, lane, s_red, maps, cast_scale, cast_si,
+                            epilogue_tile<EF>(it, tmem_base + sacc * 128u, base_tile(sbs), 1, warp, lane, s_red, maps, cast_scale, cast_si,
                                           it.row0 + 128 * rb, 128 * ct, it.write_scale != 0 && ct == 0 && rb == 0,
                                           it.mode == EPI_BLOCKCAST ? it.scale_inv_out + (size_t)((it.row0 >> 7) + rb) * nct + ct
                                                                    : it.scale_inv_out,
@@ -1155,7 +1225,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
             const Item& it = *item_slot(slot);
             bool stored = false;
             if (it.base_map[0] >= 0)
-                stored = epilogue_tile(it, tmem_base + acc * 128u, base_tile(bs), it.base_map[1] >= 0 ? 2 : 1, warp, lane, s_red, maps, cast_scale, cast_si,
+                stored = epilogue_tile<EF>(it, tmem_base + acc * 128u, base_tile(bs), it.base_map[1] >= 0 ? 2 : 1, warp, lane, s_red, maps, cast_scale, cast_si,
                                        it.row0, it.col0, it.write_scale != 0, it.scale_inv_out, nullptr);
             else {
                 epilogue(it, tmem_base + acc * 128u, warp, lane, s_red);

@@ -26,7 +26,7 @@ EXPORTS = [
     "gf8_sync_check", "gf8_set_stage_timing", "gf8_stage_times",
     "gf8_factor_update", "gf8_refresh_basis", "gf8_encode", "gf8_decode", "gf8_reduce_decoded",
     "gf8_encode_many", "gf8_reduce_decoded_many", "gf8_factor_update_many", "gf8_refresh_basis_many",
-    "gf8_encode_ef", "gf8_encode_ef_many", "gf8_amax", "gf8_encode_scaled",
+    "gf8_encode_ef", "gf8_encode_ef_many", "gf8_resid_size", "gf8_resid_export", "gf8_amax", "gf8_encode_scaled",
     "gf8_step_host", "gf8_get_factor", "gf8_set_factor", "gf8_get_basis", "gf8_set_basis",
     "gf8_whiten_f32", "gf8_quantize_f32", "gf8_reduce_f32",
 ]
@@ -92,6 +92,8 @@ def lib():
         L.gf8_encode_many.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(vp), i32, C.POINTER(vp), C.POINTER(vp), vp]
         L.gf8_amax.argtypes = [vp, i32, vp, i32, vp, vp]
         L.gf8_encode_scaled.argtypes = [vp, i32, vp, i32, vp, vp, vp, vp, vp]
+        L.gf8_resid_size.argtypes = [vp, i32, C.POINTER(C.c_size_t)]
+        L.gf8_resid_export.argtypes = [vp, i32, i32, vp, vp, vp]
         L.gf8_encode_ef.argtypes = [vp, i32, vp, i32, vp, vp, vp, vp]
         L.gf8_encode_ef_many.argtypes = [vp, i32, C.POINTER(i32), C.POINTER(vp), i32, C.POINTER(vp), C.POINTER(vp),
                                          C.POINTER(vp), vp]
@@ -287,9 +289,22 @@ class Ctx:
                                          _ptr(hits), _stream()))
         return codes, scale_inv
 
+    def resid_new(self, layer):
+        """A zeroed error-feedback residual for `layer` (opaque FP32 state, gf8_resid_size floats)."""
+        n = C.c_size_t()
+        self._ck(lib().gf8_resid_size(self._h, layer, C.byref(n)))
+        return torch.zeros(n.value, dtype=torch.float32, device=self._tdev)
+
+    def resid_export(self, layer, resid: torch.Tensor, dt=DT_BF16):
+        """The residual as a row-major [d_out][d_in] FP32 tensor (dt: the gradient type the buffer was used with)."""
+        l = self.layers[layer]
+        out = torch.empty((l.d_out, l.d_in), dtype=torch.float32, device=self._tdev)
+        self._ck(lib().gf8_resid_export(self._h, layer, dt, _ptr(resid), _ptr(out), _stream()))
+        return out
+
     def encode_ef(self, layer, grad: torch.Tensor, resid: torch.Tensor, codes=None, scale_inv=None):
-        """f1: encode with error feedback; `resid` (FP32, the gradient's shape) is read and overwritten."""
-        assert resid.dtype == torch.float32 and resid.shape == grad.shape
+        """f1: encode with error feedback; `resid` (from resid_new) is read and overwritten."""
+        assert resid.dtype == torch.float32
         if codes is None:
             codes, scale_inv = self._payload_buffers(layer)
         self._ck(lib().gf8_encode_ef(self._h, layer, _ptr(grad), _dt(grad), _ptr(resid), _ptr(codes), _ptr(scale_inv),
