@@ -659,7 +659,7 @@ def test_step_host_matches_the_device_calls_bit_for_bit():
 
 
 # ---- f1: error feedback in the transformed coordinates (Alg. 1 l.11-15) -------------------------------------
-@pytest.mark.parametrize("prec", ["exact", "fast"])
+@pytest.mark.parametrize("prec", ["exact", "fast", "fast-k96"])
 @pytest.mark.parametrize("scaling", [gf8.SCALE_TENSOR, gf8.SCALE_BLOCK128])
 def test_f1_error_feedback_chain_against_the_oracle(prec, scaling):
     """Four steps of encode-with-feedback on a whitened tensor (ragged: several tiles and a tail).
@@ -671,9 +671,12 @@ def test_f1_error_feedback_chain_against_the_oracle(prec, scaling):
     stay valid.  What is unique is compared: on the elements whose codes have agreed at every earlier step, U~ = U + R
     agrees within the transform tier, and those elements stay the overwhelming majority (EXACT: the code gate's 1e-4 per
     step; FAST: the few-% flip rate DESIGN.md reports).  With a zero residual the payload is gf8_encode's."""
-    fast = prec == "fast"
-    c = Case(272, 400, 16, 16, gf8.SIDE_BOTH, "bf16" if fast else "f32", 81, scaling=scaling,
-             precision=gf8.PREC_FAST if fast else gf8.PREC_EXACT)
+    fast = prec != "exact"
+    if prec == "fast-k96":        # ranks above 64: the update runs as 128 x 128 tile items instead of strips
+        c = Case(400, 592, 96, 80, gf8.SIDE_BOTH, "bf16", 86, scaling=scaling, precision=gf8.PREC_FAST, q=2)
+    else:
+        c = Case(272, 400, 16, 16, gf8.SIDE_BOTH, "bf16" if fast else "f32", 81, scaling=scaling,
+                 precision=gf8.PREC_FAST if fast else gf8.PREC_EXACT)
     res = c.ctx.resid_new(0)                           # opaque state; resid_export gives the row-major view
     gdt = gf8.DT_BF16 if fast else gf8.DT_F32
     o_res = np.zeros((c.m, c.n), np.float32)
