@@ -19,8 +19,9 @@ namespace rb {
 constexpr int RB_MAXK = 64;
 constexpr int RB_CHUNK = 256;            // rows of V per partial Gram product
 constexpr int AV_BM = 128, AV_BK = 32;   // A V tile: 128 rows of A, K in steps of 32
-constexpr int AV_LDA = AV_BM + 4;        // leading dimension of the K-major A tile (floats; rows stay 16 B aligned)
-constexpr int AV_SMEM = AV_BK * RB_MAXK * 8 + AV_BK * AV_LDA * 4;
+constexpr int AV_LDA = AV_BM + 8;        // leading dimension of the K-major A tile (floats): 8 banks per K row, fragment loads conflict-free
+constexpr int AV_LDV = RB_MAXK + 8;      // leading dimension of the V tile (doubles): K rows 16 banks apart, the two-wavefront minimum
+constexpr int AV_SMEM = AV_BK * AV_LDV * 8 + AV_BK * AV_LDA * 4;
 constexpr int RM_SMEM = (RB_MAXK * (64 + 2) + RB_MAXK * RB_MAXK) * 8;
 
 struct RefreshJob {
@@ -202,15 +203,16 @@ __global__ void __launch_bounds__(256) rb_multipliers_kernel(const RefreshJob* _
 
 // ---- Y = A V: buf[flip ^ 1] <- factor (d x d FP32) * buf[flip] (d x k FP64), FP64 accumulate -----------------------
 // One CTA per 128-row block of one side (blockIdx.x walks the launch-wide block list), the whole K = d loop inside it.
-// 256 threads, 8 x 4 outputs each.  The kernel is bound by shared-memory wavefronts, not by the FP64 pipe (a 128-bit shared
-// load costs four wavefronts per warp whatever it broadcasts), so the A tile stays FP32 in shared memory (K-major: the
-// eight row values of a thread are two 128-bit loads) and is widened in registers; a warp of the loader takes 32
-// consecutive rows, which makes the transposing stores conflict-free.  The next tile's global loads are in flight while
-// the current one is multiplied.
+// The product runs on the FP64 tensor-core path (mma.sync m8n8k4, DMMA): a warp owns 16 rows x 64 columns = 2 x 8 MMA
+// tiles, so one K = 4 step is 2 + 8 fragment loads for 16 MMAs.  The CUDA-core version of this kernel (8 x 4 register tiles)
+// was bound by shared-memory wavefronts at 47 % of the FP64 pipe (ncu: a 128-bit shared load costs four wavefronts per warp
+// whatever it broadcasts); the fragments need a fifth of that traffic.  The A tile stays FP32 in shared memory (K-major)
+// and is widened in registers; a warp of the loader takes 32 consecutive rows, so the transposing stores are
+// conflict-free.  The next tile's global loads are in flight while the current one is multiplied.
 __global__ void __launch_bounds__(256, 2) rb_av_kernel(const RefreshJob* __restrict__ jobs, int n_jobs, int flip) {
     extern __shared__ __align__(16) double s_av[];                  // AV_SMEM bytes
-    double (*Vs)[RB_MAXK] = reinterpret_cast<double (*)[RB_MAXK]>(s_av);
-    float (*As)[AV_LDA] = reinterpret_cast<float (*)[AV_LDA]>(s_av + AV_BK * RB_MAXK);
+    double (*Vs)[AV_LDV] = reinterpret_cast<double (*)[AV_LDV]>(s_av);
+    float (*As)[AV_LDA] = reinterpret_cast<float (*)[AV_LDA]>(s_av + AV_BK * AV_LDV);
     int lo = 0, hi = n_jobs - 1;
     while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (jobs[mid].blk0 <= (int)blockIdx.x) lo = mid; else hi = mid - 1; }
     const RefreshJob& j = jobs[lo];
@@ -219,7 +221,7 @@ __global__ void __launch_bounds__(256, 2) rb_av_kernel(const RefreshJob* __restr
     const float* __restrict__ A = j.factor;
     const double* __restrict__ V = j.buf[flip];
     double* __restrict__ Y = j.buf[flip ^ 1];
-    const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
+    const int tid = threadIdx.x;
     // loader roles: A tile 128 rows x 32 floats = 1024 float4 (4 per thread: row = idx % 128, quad = idx / 128);
     //               V tile 32 rows x 64 doubles = 1024 double2 (4 per thread: row = idx / 32, pair = idx % 32)
     float4 pa[4];
@@ -272,40 +274,39 @@ __global__ void __launch_bounds__(256, 2) rb_av_kernel(const RefreshJob* __restr
             *reinterpret_cast<double2*>(&Vs[row][2 * pair]) = pv[u];
         }
     };
-    double acc[8][4] = {};
+    const int warp = tid >> 5, lane = tid & 31, fr = lane >> 2, fk = lane & 3;      // fragment row / column group, K index
+    double acc[2][8][2] = {};
     fetch(0);
     for (int k0 = 0; k0 < d; k0 += AV_BK) {
         stash();
         __syncthreads();
         if (k0 + AV_BK < d) fetch(k0 + AV_BK);
-#pragma unroll 8
-        for (int l = 0; l < AV_BK; ++l) {
-            double a[8], b[4];
 #pragma unroll
-            for (int r = 0; r < 8; r += 4) {
-                const float4 t = *reinterpret_cast<const float4*>(&As[l][ty * 8 + r]);
-                a[r] = (double)t.x; a[r + 1] = (double)t.y; a[r + 2] = (double)t.z; a[r + 3] = (double)t.w;
-            }
+        for (int ks = 0; ks < AV_BK / 4; ++ks) {
+            const int kk = 4 * ks + fk;
+            double a[2], b[8];
 #pragma unroll
-            for (int q = 0; q < 4; q += 2) {
-                const double2 t = *reinterpret_cast<const double2*>(&Vs[l][tx * 4 + q]);
-                b[q] = t.x; b[q + 1] = t.y;
-            }
+            for (int mb = 0; mb < 2; ++mb) a[mb] = (double)As[kk][16 * warp + 8 * mb + fr];
 #pragma unroll
-            for (int r = 0; r < 8; ++r)
+            for (int nb = 0; nb < 8; ++nb) b[nb] = Vs[kk][8 * nb + fr];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) acc[r][q] = fma(a[r], b[q], acc[r][q]);
+            for (int mb = 0; mb < 2; ++mb)
+#pragma unroll
+                for (int nb = 0; nb < 8; ++nb)
+                    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+                                 : "+d"(acc[mb][nb][0]), "+d"(acc[mb][nb][1]) : "d"(a[mb]), "d"(b[nb]));
         }
         __syncthreads();
     }
 #pragma unroll
-    for (int r = 0; r < 8; ++r) {
-        const int gi = i0 + ty * 8 + r;
+    for (int mb = 0; mb < 2; ++mb) {
+        const int gi = i0 + 16 * warp + 8 * mb + fr;
         if (gi >= d) continue;
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const int col = tx * 4 + q;
-            if (col < k) Y[(int64_t)gi * k + col] = acc[r][q];
+        for (int nb = 0; nb < 8; ++nb) {
+            const int col = 8 * nb + 2 * fk;
+            if (col < k) Y[(int64_t)gi * k + col] = acc[mb][nb][0];
+            if (col + 1 < k) Y[(int64_t)gi * k + col + 1] = acc[mb][nb][1];
         }
     }
 }
