@@ -22,7 +22,6 @@ constexpr int AV_BM = 128, AV_BK = 32;   // A V tile: 128 rows of A, K in steps 
 constexpr int AV_LDA = AV_BM + 8;        // leading dimension of the K-major A tile (floats): 8 banks per K row, fragment loads conflict-free
 constexpr int AV_LDV = RB_MAXK + 8;      // leading dimension of the V tile (doubles): K rows 16 banks apart, the two-wavefront minimum
 constexpr int AV_SMEM = AV_BK * AV_LDV * 8 + AV_BK * AV_LDA * 4;
-constexpr int RM_SMEM = (RB_MAXK * (64 + 2) + RB_MAXK * RB_MAXK) * 8;
 
 struct RefreshJob {
     const float* factor;     // d x d FP32
@@ -50,7 +49,13 @@ __global__ void __launch_bounds__(256) rb_widen_kernel(const RefreshJob* __restr
 }
 
 // ---- partial products  part[c] = X[chunk c]^T W[chunk c]  (k x k, FP64), X = buf[xa], W = buf[xb] --------------
-// 256 threads, 4 x 4 outputs each; rows of the chunk staged 16 at a time.
+// FP64 tensor-core path (mma.sync m8n8k4): warp w owns rows 8 w .. 8 w + 7 of the product and all 64 columns (8 MMA tiles);
+// 32 rows of the chunk are staged per step.  Leading dimension 72 doubles: the four K rows of a fragment load fall 16 banks
+// apart, the two-wavefront minimum of a 64-bit warp load.
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+constexpr int RB_LD = RB_MAXK + 8;
 __global__ void __launch_bounds__(256) rb_gram_kernel(const RefreshJob* __restrict__ jobs, int xa, int xb) {
     const RefreshJob& j = jobs[blockIdx.y];
     const int c = blockIdx.x;
@@ -58,13 +63,13 @@ __global__ void __launch_bounds__(256) rb_gram_kernel(const RefreshJob* __restri
     const int d = j.d, k = j.k;
     const double* X = j.buf[xa];
     const double* W = j.buf[xb];
-    __shared__ double Xs[16][RB_MAXK + 2], Ws[16][RB_MAXK + 2];
-    const int tid = threadIdx.x, tx = tid & 15, ty = tid >> 4;
-    double acc[4][4] = {};
+    __shared__ double Xs[32][RB_LD], Ws[32][RB_LD];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, fr = lane >> 2, fk = lane & 3;
+    double acc[8][2] = {};
     const int r_begin = c * RB_CHUNK, r_end = min(d, r_begin + RB_CHUNK);
-    for (int r0 = r_begin; r0 < r_end; r0 += 16) {
+    for (int r0 = r_begin; r0 < r_end; r0 += 32) {
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
+        for (int u = 0; u < 8; ++u) {
             const int idx = tid + 256 * u, l = idx >> 6, col = idx & 63;
             const bool ok = r0 + l < r_end && col < k;
             Xs[l][col] = ok ? X[(int64_t)(r0 + l) * k + col] : 0.0;
@@ -72,27 +77,21 @@ __global__ void __launch_bounds__(256) rb_gram_kernel(const RefreshJob* __restri
         }
         __syncthreads();
 #pragma unroll
-        for (int l = 0; l < 16; ++l) {
-            double a[4], b[4];
+        for (int ks = 0; ks < 8; ++ks) {
+            const double a = Xs[4 * ks + fk][8 * warp + fr];
 #pragma unroll
-            for (int r = 0; r < 4; ++r) a[r] = Xs[l][ty * 4 + r];
-#pragma unroll
-            for (int q = 0; q < 4; ++q) b[q] = Ws[l][tx * 4 + q];
-#pragma unroll
-            for (int r = 0; r < 4; ++r)
-#pragma unroll
-                for (int q = 0; q < 4; ++q) acc[r][q] = fma(a[r], b[q], acc[r][q]);
+            for (int nb = 0; nb < 8; ++nb) dmma884(acc[nb][0], acc[nb][1], a, Ws[4 * ks + fk][8 * nb + fr]);
         }
         __syncthreads();
     }
     double* P = j.part + (int64_t)c * k * k;
+    const int i = 8 * warp + fr;
 #pragma unroll
-    for (int r = 0; r < 4; ++r)
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const int i = ty * 4 + r, l = tx * 4 + q;
-            if (i < k && l < k) P[(int64_t)i * k + l] = acc[r][q];
-        }
+    for (int nb = 0; nb < 8; ++nb) {
+        const int l = 8 * nb + 2 * fk;
+        if (i < k && l < k) P[(int64_t)i * k + l] = acc[nb][0];
+        if (i < k && l + 1 < k) P[(int64_t)i * k + l + 1] = acc[nb][1];
+    }
 }
 
 // ---- out = sum over chunks of part[c], in chunk order (fixed summation order); to_B: into Bm, else into Gm --------
@@ -143,16 +142,18 @@ __global__ void __launch_bounds__(1024) rb_chol_kernel(const RefreshJob* __restr
 }
 
 // ---- buf[flip] <- buf[flip] * Zs   (to_U = 0: FP64, in place)   or   U <- (float)(buf[flip] * Zs)   (to_U = 1) ------------
-// One CTA per 64 rows; 256 threads, 4 x 4 outputs each; the row panel is staged transposed so that a thread's four row values
-// and four column values are contiguous.
+// One CTA per 64 rows, FP64 tensor-core path: warp w owns rows 8 w .. 8 w + 7 and all 64 columns; K = k <= 64.  The row panel
+// stays row-major in shared memory (leading dimension 68 doubles: the eight rows of an A fragment load fall 8 banks apart).
+constexpr int RM_LDV = RB_MAXK + 4;
+constexpr int RM_SMEM = (64 * RM_LDV + RB_MAXK * RB_LD) * 8;
 __global__ void __launch_bounds__(256) rb_rightmul_kernel(const RefreshJob* __restrict__ jobs, int flip, int to_U) {
     const RefreshJob& j = jobs[blockIdx.y];
     const int d = j.d, k = j.k;
     const int r0 = blockIdx.x * 64;
     if (r0 >= d) return;
     extern __shared__ __align__(16) double s_rm[];             // RM_SMEM bytes
-    double (*Vt)[64 + 2] = reinterpret_cast<double (*)[64 + 2]>(s_rm);                          // Vt[l][r]
-    double (*Zsh)[RB_MAXK] = reinterpret_cast<double (*)[RB_MAXK]>(s_rm + RB_MAXK * (64 + 2));   // Zsh[l][c]
+    double (*Vsh)[RM_LDV] = reinterpret_cast<double (*)[RM_LDV]>(s_rm);                       // Vsh[r][l]
+    double (*Zsh)[RB_LD] = reinterpret_cast<double (*)[RB_LD]>(s_rm + 64 * RM_LDV);          // Zsh[l][c]
     double* V = j.buf[flip];
     for (int idx = threadIdx.x; idx < RB_MAXK * RB_MAXK; idx += 256) {
         const int l = idx >> 6, c = idx & 63;
@@ -160,33 +161,28 @@ __global__ void __launch_bounds__(256) rb_rightmul_kernel(const RefreshJob* __re
     }
     for (int idx = threadIdx.x; idx < 64 * RB_MAXK; idx += 256) {
         const int r = idx >> 6, l = idx & 63;
-        Vt[l][r] = (r0 + r < d && l < k) ? V[(int64_t)(r0 + r) * k + l] : 0.0;
+        Vsh[r][l] = (r0 + r < d && l < k) ? V[(int64_t)(r0 + r) * k + l] : 0.0;
     }
     __syncthreads();
-    const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
-    double acc[4][4] = {};
-#pragma unroll 8
-    for (int l = 0; l < RB_MAXK; ++l) {
-        double a[4], b[4];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, fr = lane >> 2, fk = lane & 3;
+    double acc[8][2] = {};
 #pragma unroll
-        for (int r = 0; r < 4; r += 2) { const double2 t = *reinterpret_cast<const double2*>(&Vt[l][ty * 4 + r]); a[r] = t.x; a[r + 1] = t.y; }
+    for (int ks = 0; ks < RB_MAXK / 4; ++ks) {
+        const double a = Vsh[8 * warp + fr][4 * ks + fk];
 #pragma unroll
-        for (int q = 0; q < 4; q += 2) { const double2 t = *reinterpret_cast<const double2*>(&Zsh[l][tx * 4 + q]); b[q] = t.x; b[q + 1] = t.y; }
-#pragma unroll
-        for (int r = 0; r < 4; ++r)
-#pragma unroll
-            for (int q = 0; q < 4; ++q) acc[r][q] = fma(a[r], b[q], acc[r][q]);
+        for (int nb = 0; nb < 8; ++nb) dmma884(acc[nb][0], acc[nb][1], a, Zsh[4 * ks + fk][8 * nb + fr]);
     }
+    const int gi = r0 + 8 * warp + fr;
+    if (gi < d) {
 #pragma unroll
-    for (int r = 0; r < 4; ++r) {
-        const int gi = r0 + ty * 4 + r;
-        if (gi >= d) continue;
+        for (int nb = 0; nb < 8; ++nb) {
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const int c = tx * 4 + q;
-            if (c >= k) continue;
-            if (to_U) j.U[(int64_t)gi * k + c] = (float)acc[r][q];
-            else V[(int64_t)gi * k + c] = acc[r][q];
+            for (int e = 0; e < 2; ++e) {
+                const int c = 8 * nb + 2 * fk + e;
+                if (c >= k) continue;
+                if (to_U) j.U[(int64_t)gi * k + c] = (float)acc[nb][e];
+                else V[(int64_t)gi * k + c] = acc[nb][e];
+            }
         }
     }
 }
