@@ -211,6 +211,25 @@ gf8_status gf8_reduce_f32(gf8_ctx* ctx, int fmt, int scaling, const uint8_t* con
                           const float* const* scale_inv_host, int R, int average, int64_t m, int64_t n,
                           float* out, void* stream);
 
+/* ---- no-allocation entry point ------------------------------------------------------------------------------------- */
+/* The quantizer (a5 + a6; gf8_quantize_f32's arithmetic, bit for bit) for callers that cannot call cudaMalloc: code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid it.  It takes NO context and calls no cudaMalloc, cudaFree
+ * or allocating library routine: the amax words and scales it needs between its kernels live in a static device array of
+ * GF8_NOALLOC_MAX_SCALES entries (512 KB, held by every GPU that loads the library until the process exits).
+ *   in: DEVICE, m x n FP32 row-major; codes: DEVICE, m*n bytes; scale_inv: DEVICE, 1 float (GF8_SCALE_TENSOR) or
+ *   ceil(m/128)*ceil(n/128) floats (GF8_SCALE_BLOCK128); n a multiple of 16; pointers 16-byte aligned.  It runs on the
+ *   CURRENT device (cudaSetDevice is the caller's), asynchronously on `stream`.
+ *   Limit: at most GF8_NOALLOC_MAX_SCALES scales, i.e. any size with per-tensor scaling and up to 65536 blocks of 128 x 128
+ *   (e.g. 32768 x 32768) with per-block scaling; beyond that GF8_ERR_UNSUPPORTED with a message (gf8_noalloc_last_error,
+ *   thread-local) and nothing is launched.
+ *   Every call on a device shares the one array: calls that OVERLAP on the GPU (different streams, or graph branches
+ *   without an edge between them) race on it -- order them on one stream.  The array keeps the previous call's contents;
+ *   the call clears what must start at zero itself. */
+#define GF8_NOALLOC_MAX_SCALES 65536
+gf8_status gf8_quantize_f32_noalloc(int fmt, int scaling, const float* in, int64_t m, int64_t n, uint8_t* codes,
+                                    float* scale_inv, void* stream);
+const char* gf8_noalloc_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -3,6 +3,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1597,6 +1598,97 @@ gf8_status gf8_reduce_f32(gf8_ctx* ctx, int fmt, int scaling, const uint8_t* con
     if (!aligned16(out)) return fail(ctx, GF8_ERR_UNSUPPORTED, "pointers must be 16-byte aligned");
     CU_TRY(ctx, cudaSetDevice(ctx->device));
     return reduce_dev<float>(ctx, (cudaStream_t)stream, codes, scale_inv, R, average, m, n, fmt, scaling, out);
+}
+
+// ---- the quantizer for callers that cannot allocate (CUDA graph capture, tight serving loops, harnesses that forbid it) ---
+// gf8_quantize_f32 keeps its amax words and scales in context scratch that grows with cudaMalloc, and a context itself is
+// built with cudaMalloc.  This variant needs no context and allocates nothing: that scratch lives in a file-scope device
+// array of GF8_NOALLOC_MAX_SCALES (amax word, scale) pairs = 512 KB, which every GPU that loads the library holds until exit.
+// In host code the array's name is only a stand-in: the device address comes from cudaGetSymbolAddress, once per device,
+// with that device current.
+}  // extern "C"
+
+namespace {
+struct NoallocScratch {
+    uint32_t amax_bits[GF8_NOALLOC_MAX_SCALES];
+    float scale[GF8_NOALLOC_MAX_SCALES];
+};
+static __device__ __align__(256) NoallocScratch g_noalloc_scratch;
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+NoallocScratch* g_noalloc_ptr[NOALLOC_MAX_DEVICES] = {};      // device address of the array, per device (set-up: first call)
+int g_noalloc_sms[NOALLOC_MAX_DEVICES] = {};
+std::mutex g_noalloc_mutex;
+thread_local char g_noalloc_err[256] = "";
+
+gf8_status noalloc_fail(gf8_status st, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_noalloc_err, sizeof(g_noalloc_err), fmt, ap);
+    va_end(ap);
+    return st;
+}
+}  // namespace
+
+extern "C" {
+
+const char* gf8_noalloc_last_error(void) { return g_noalloc_err; }
+
+gf8_status gf8_quantize_f32_noalloc(int fmt, int scaling, const float* in, int64_t m, int64_t n, uint8_t* codes,
+                                    float* scale_inv, void* stream) {
+    if (!in || !codes || !scale_inv) return noalloc_fail(GF8_ERR_INVALID_ARG, "null pointer");
+    if (fmt < 0 || fmt > 1 || scaling < 0 || scaling > 1 || m < 1 || n < 1) return noalloc_fail(GF8_ERR_INVALID_ARG, "bad argument");
+    if (n % 16 || (m * n) % 16) return noalloc_fail(GF8_ERR_UNSUPPORTED, "n must be a multiple of 16");
+    if (!aligned16(in) || !aligned16(codes)) return noalloc_fail(GF8_ERR_UNSUPPORTED, "pointers must be 16-byte aligned");
+    if (m > 0x7FFFFFFF || n > 0x7FFFFFFF) return noalloc_fail(GF8_ERR_UNSUPPORTED, "dimension too large");
+    const size_t ns = n_scales_of(scaling, m, n);
+    if (ns > (size_t)GF8_NOALLOC_MAX_SCALES)
+        return noalloc_fail(GF8_ERR_UNSUPPORTED,
+                            "%lld x %lld with per-block scaling needs %zu scales; the static scratch of gf8_quantize_f32_noalloc "
+                            "holds GF8_NOALLOC_MAX_SCALES = %d (use gf8_quantize_f32)", (long long)m, (long long)n, ns,
+                            (int)GF8_NOALLOC_MAX_SCALES);
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return noalloc_fail(GF8_ERR_CUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return noalloc_fail(GF8_ERR_UNSUPPORTED, "device index %d out of range", dev);
+    NoallocScratch* sc = nullptr;
+    int sms = 0;
+    {
+        std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+        if (!g_noalloc_ptr[dev]) {          // set-up, once per device, with that device current
+            void* ptr = nullptr;
+            e = cudaGetSymbolAddress(&ptr, g_noalloc_scratch);
+            if (e != cudaSuccess || !ptr) return noalloc_fail(GF8_ERR_CUDA, "cudaGetSymbolAddress: %s", cudaGetErrorString(e));
+            int n_sm = 0;
+            e = cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+            if (e != cudaSuccess || n_sm < 1) return noalloc_fail(GF8_ERR_CUDA, "cudaDeviceGetAttribute: %s", cudaGetErrorString(e));
+            g_noalloc_sms[dev] = n_sm;
+            g_noalloc_ptr[dev] = static_cast<NoallocScratch*>(ptr);
+        }
+        sc = g_noalloc_ptr[dev];
+        sms = g_noalloc_sms[dev];
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    auto grid = [&](int64_t work_items) {
+        int64_t blocks = (work_items + 255) / 256;
+        return (int)std::max<int64_t>(1, std::min<int64_t>(blocks, (int64_t)sms * 8));
+    };
+    // the array keeps the last call's contents: the per-tensor amax word is an atomic-max target and must start at zero
+    // (the per-block amax kernel overwrites every word it owns)
+    if (scaling == GF8_SCALE_TENSOR) {
+        e = cudaMemsetAsync(sc->amax_bits, 0, sizeof(uint32_t), st);
+        if (e != cudaSuccess) return noalloc_fail(GF8_ERR_CUDA, "cudaMemsetAsync: %s", cudaGetErrorString(e));
+        amax_tensor_kernel<float><<<grid((m * n / 4 + 3) / 4), 256, 0, st>>>(in, m * n, sc->amax_bits);
+    } else {
+        dim3 g2((unsigned)((n + 127) / 128), (unsigned)((m + 127) / 128));
+        amax_block_kernel<float><<<g2, 256, 0, st>>>(in, m, n, sc->amax_bits);
+    }
+    scales_kernel<<<(int)((ns + 255) / 256), 256, 0, st>>>(sc->amax_bits, (int)ns, fmax_of(fmt), sc->scale, scale_inv);
+    if (fmt == GF8_E4M3) cast_kernel<float, 0><<<grid(m * n / 16), 256, 0, st>>>(in, m, n, scaling, sc->scale, codes);
+    else cast_kernel<float, 1><<<grid(m * n / 16), 256, 0, st>>>(in, m, n, scaling, sc->scale, codes);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return noalloc_fail(GF8_ERR_CUDA, "kernel launch: %s", cudaGetErrorString(e));
+    return GF8_OK;
 }
 
 }  // extern "C"

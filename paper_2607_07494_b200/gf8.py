@@ -29,6 +29,7 @@ EXPORTS = [
     "gf8_encode_ef", "gf8_encode_ef_many", "gf8_resid_size", "gf8_resid_export", "gf8_amax", "gf8_encode_scaled",
     "gf8_step_host", "gf8_get_factor", "gf8_set_factor", "gf8_get_basis", "gf8_set_basis",
     "gf8_whiten_f32", "gf8_quantize_f32", "gf8_reduce_f32",
+    "gf8_quantize_f32_noalloc", "gf8_noalloc_last_error",
 ]
 
 
@@ -110,8 +111,11 @@ def lib():
         L.gf8_whiten_f32.argtypes = [vp, i32, vp, i32, vp, vp]
         L.gf8_quantize_f32.argtypes = [vp, i32, i32, vp, i64, i64, vp, vp, vp]
         L.gf8_reduce_f32.argtypes = [vp, i32, i32, C.POINTER(vp), C.POINTER(vp), i32, i32, i64, i64, vp, vp]
+        L.gf8_quantize_f32_noalloc.argtypes = [i32, i32, vp, i64, i64, vp, vp, vp]
+        L.gf8_noalloc_last_error.restype = C.c_char_p
+        L.gf8_noalloc_last_error.argtypes = []
         for name in EXPORTS:
-            if name not in ("gf8_status_string", "gf8_last_error", "gf8_launch_count"):
+            if name not in ("gf8_status_string", "gf8_last_error", "gf8_launch_count", "gf8_noalloc_last_error"):
                 getattr(L, name).restype = i32
         _lib = L
     return _lib
@@ -386,3 +390,15 @@ class Ctx:
 
 def create(layers: List[Layer], precision: int = PREC_EXACT, device: Optional[int] = None) -> Ctx:
     return Ctx(layers, precision, device)
+
+
+def quantize_f32_noalloc(x: torch.Tensor, codes: torch.Tensor, scale_inv: torch.Tensor, fmt=E4M3, scaling=SCALE_TENSOR):
+    """gf8_quantize_f32_noalloc: the quantizer without a context and without any allocation (static device scratch);
+    the caller passes the output buffers.  Runs on x's device, on torch's current stream."""
+    assert x.dtype == torch.float32 and x.dim() == 2 and x.is_cuda and codes.dtype == torch.uint8 and scale_inv.dtype == torch.float32
+    m, n = x.shape
+    with torch.cuda.device(x.device):
+        st = lib().gf8_quantize_f32_noalloc(fmt, scaling, _ptr(x), m, n, _ptr(codes), _ptr(scale_inv), _stream())
+    if st != 0:
+        raise Gf8Error(st, lib().gf8_noalloc_last_error().decode())
+    return codes, scale_inv
