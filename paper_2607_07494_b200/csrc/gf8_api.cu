@@ -1042,6 +1042,7 @@ gf8_status refresh_batch(gf8_ctx* c, cudaStream_t st, const std::vector<SideStat
         j.mu64 = p;
         j.mu = s.mu; j.e = s.e; j.ebar = s.ebar; j.rho = s.rho;
         j.lam = lams[i]; j.d = s.d; j.k = s.k; j.blk0 = blocks; j.n_chunks = chunks;
+        j.U16 = s.U16; j.Ut16 = s.Ut16; j.U16_lo = s.U16_lo; j.Ut16_lo = s.Ut16_lo; j.kp = s.kp; j.pad_ = 0;
         blocks += (s.d + AV_BM - 1) / AV_BM;
     }
     // (pageable source: the runtime stages the records before the call returns)
@@ -1083,12 +1084,11 @@ gf8_status refresh_batch(gf8_ctx* c, cudaStream_t st, const std::vector<SideStat
     LAUNCH_CHECK(c);
     rb_multipliers_kernel<<<n, 256, 0, st>>>(dj);
     LAUNCH_CHECK(c);
+    rb_pack_kernel<<<dim3(48, n), 256, 0, st>>>(dj);
+    LAUNCH_CHECK(c);
     CU_TRY(c, cudaEventRecord(c->rb_ev, st));
     c->rb_busy = true;
-    for (SideState* s : sides) {
-        GF_TRY(fast_pack_basis(c, st, *s));
-        s->has_basis = true;
-    }
+    for (SideState* s : sides) s->has_basis = true;
     return GF8_OK;
 }
 }  // namespace

@@ -38,6 +38,9 @@ struct RefreshJob {
     int32_t d, k;
     int32_t blk0;            // first AV_BM-row block of this side in the launch-wide list
     int32_t n_chunks;
+    // FAST path: BF16 copies of the refreshed basis for the tensor-core engine (null: the side has none), rank padded to kp
+    __nv_bfloat16 *U16, *Ut16, *U16_lo, *Ut16_lo;
+    int32_t kp, pad_;
 };
 
 // ---- V <- (double) U ----------------------------------------------------------------------------------
@@ -304,6 +307,24 @@ __global__ void __launch_bounds__(256, 2) rb_av_kernel(const RefreshJob* __restr
             if (col < k) Y[(int64_t)gi * k + col] = acc[mb][nb][0];
             if (col + 1 < k) Y[(int64_t)gi * k + col + 1] = acc[mb][nb][1];
         }
+    }
+}
+
+// ---- U (d x k FP32) -> U16 (d x kp BF16, zero-padded), its transpose Ut16 (kp x d) and the residuals U - bf16(U) --------
+// (the per-side pack_basis_kernel of gf8_fast.cuh, for all sides of the call in one launch)
+__global__ void __launch_bounds__(256) rb_pack_kernel(const RefreshJob* __restrict__ jobs) {
+    const RefreshJob& j = jobs[blockIdx.y];
+    if (!j.U16) return;
+    const int d = j.d, k = j.k, kp = j.kp;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < (int64_t)d * kp; idx += (int64_t)gridDim.x * blockDim.x) {
+        const int i = (int)(idx / kp), col = (int)(idx % kp);
+        const float x = col < k ? j.U[(int64_t)i * k + col] : 0.0f;
+        const __nv_bfloat16 v = __float2bfloat16_rn(x);
+        const __nv_bfloat16 lo = __float2bfloat16_rn(x - __bfloat162float(v));
+        j.U16[idx] = v;
+        j.Ut16[(int64_t)col * d + i] = v;
+        j.U16_lo[idx] = lo;
+        j.Ut16_lo[(int64_t)col * d + i] = lo;
     }
 }
 
