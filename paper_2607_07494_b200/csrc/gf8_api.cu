@@ -409,7 +409,7 @@ gf8_status fast_encode_many(gf8_ctx* c, int n, const int* layers, const void* co
                 }
             }
             EngineOptions opt = c->opt;
-            if (resid) { f.resid = resid[i]; opt.fuse = false; }      // (the parked-tile update has no feedback epilogue)
+            if (resid) { f.resid = resid[i]; opt.fuse = false; opt.pair = false; }      // (no feedback epilogue in the parked-tile / pair updates)
             add_transform(pb, L, slot, src_map, src_lo_map, false, split, f, opt);
         }
         if (s == GF8_OK) s = plan_finish(c, pb, p);
@@ -758,6 +758,7 @@ gf8_status gf8_create(gf8_ctx** out, int device, const gf8_layer_desc* layers, i
     c->use_stream = getenv("GF8_STREAM") != nullptr;
     c->opt.nostrip = getenv("GF8_TC_NOSTRIP") != nullptr; c->opt.fuse = getenv("GF8_TC_FUSE") != nullptr;
     c->opt.notri = getenv("GF8_TC_NOTRI") != nullptr; c->opt.static_items = getenv("GF8_TC_STATIC") != nullptr;
+    c->opt.pair = getenv("GF8_TC_PAIR") != nullptr;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) == cudaSuccess) c->num_sms = prop.multiProcessorCount;
     c->layers.resize(n_layers);

@@ -75,6 +75,7 @@ struct EngineOptions {
     bool fuse = false;           // GF8_TC_FUSE: single-pass update with W~ parked in TMEM (static round-robin; slower: DESIGN.md 5)
     bool notri = false;          // GF8_TC_NOTRI: split products as three K-loops instead of interleaved per K-atom
     bool static_items = false;   // GF8_TC_STATIC: static item assignment instead of the atomic hand-out
+    bool pair = false;           // GF8_TC_PAIR: both update passes of the encode in ONE launch of (amax, cast) item pairs
 };
 
 struct gf8_ctx {

@@ -18,6 +18,7 @@ struct Plan {
     int stage_wide[8] = {0, 0, 0, 0, 0, 0, 0, 0};  // the stage holds 256-row panel items: wide operand stages (kmode 3)
     int stage_base[8] = {0, 0, 0, 0, 0, 0, 0, 0};  // streamed base tiles per item in that stage's launch (0, 1 or 2)
     bool ef = false;                     // f1: the update stages run the error-feedback instance of the kernel
+    bool pair5 = false;                  // stage 5 holds (amax item, cast item) pairs: one launch for both update passes (kmode 6)
     int runs = 0;                        // launches so far: the first one acquires its tensor maps with proxy fences
     int* d_ctr = nullptr;                // one item counter per stage (dynamic item hand-out), zeroed before every run
     uint32_t* d_amax = nullptr;          // one word per TC problem (per-tensor scaling)
@@ -210,6 +211,7 @@ struct PlanBuilder {
     std::vector<Item> stage[8];
     std::vector<int> prob0;                    // stage 0: the problem (add_transform call) each item belongs to
     int cur_problem = 0;
+    bool pair_ok = true;                       // every strip item of stages 5 / 6 so far can run in a pair launch
     // registers both box heights of a buffer; returns the index of the 64-row-box map, +1 is the 128-row-box map
     int add_map(const void* key, const CUtensorMap* m2) {
         auto it = map_index.find(key);
@@ -359,25 +361,44 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
     // to bring in per output tile (96 KB -> 48 KB) and amortises the per-item hand-shakes over 2 x n / 128 tiles.
     if (!split && kpA + kpG <= 128 && f.base_map[0] >= 0 && f.base_map[1] < 0 && f.out_map >= 0 &&
         (f.mode == EPI_AMAX || f.mode == EPI_BLOCKCAST) && !opt.nostrip && !opt.fuse) {
-        for (int i0 = 0; i0 < m; i0 += 256) {
+        // Pair launches (opt-in, GF8_TC_PAIR=1; per-tensor scaling): the strips are cut into sub-strips of about PAIR_TILES column
+        // tiles (393 KB of gradient), each an (amax item, cast item) pair that one CTA runs back to back; the cast items start
+        // once the tensor's `done` word has counted every amax item (8 epilogue warps each).  148 sub-strips in flight are 58 MB:
+        // the cast pass finds its gradient tiles in L2 (measured: 12.9 GB of DRAM reads for both passes instead of 23.4).  A
+        // tensor must not have more pairs than the launch has CTAs (its join would never complete), and a sub-strip must be
+        // longer than the base ring (see the producer's deferred claim).  Not the default: DESIGN.md 5 says why it is not faster.
+        constexpr int PAIR_TILES = 6;                        // column tiles per sub-strip (768 columns)
+        const bool pairs = f.mode == EPI_AMAX && opt.pair && !opt.static_items && f.done;
+        const int col_tiles = (n + 127) / 128;
+        const int n_chunk = pairs ? (col_tiles + PAIR_TILES - 1) / PAIR_TILES : 1;      // column tiles spread evenly over the chunks
+        const int n_pairs = ((m + 255) / 256) * n_chunk;
+        if (!pairs || n_pairs > c_num_sms / 2) pb.pair_ok = false;
+        for (int i0 = 0; i0 < m; i0 += 256)
+          for (int q = 0, c0 = 0; q < n_chunk; ++q) {
+            const int cw = pairs ? 128 * (col_tiles / n_chunk + (q < col_tiles % n_chunk ? 1 : 0)) : n;
+            const int c_this = c0;
+            c0 += cw;
             Item it = blank_item();
             int seg = 0;
             it.N = 128; it.fmt = f.fmt; it.strip = 1;
-            if (useA) add_product(it, seg, mPp, mUA, kpA / 64, 0, i0, 0, 0);
-            if (useG) add_product(it, seg, mUG, mQpt, kpG / 64, 0, i0, 0, 0);
+            if (useA) add_product(it, seg, mPp, mUA, kpA / 64, 0, i0, 0, c_this);
+            if (useG) add_product(it, seg, mUG, mQpt, kpG / 64, 0, i0, 0, c_this);
             it.base_type = f.base_type; it.base_map[0] = f.base_map[0] + 1;
-            it.row0 = i0; it.col0 = 0; it.rows = std::min(256, m - i0); it.cols = n;
+            it.row0 = i0; it.col0 = c_this; it.rows = std::min(256, m - i0); it.cols = std::min(cw, n - c_this);
+            if (((it.rows + 127) / 128) * ((it.cols + 127) / 128) < 4) pb.pair_ok = false;      // (longer than the base ring)
             it.mode = f.mode; it.out = f.out; it.out_ld = n; it.out_map = f.out_map; it.scale_inv_out = f.scale_inv;
             it.out_lo = f.resid;                                   // (amax / cast modes: out_lo carries the feedback residual)
             if (f.mode == EPI_AMAX) {
                 it.amax = f.amax;
+                if (pairs) { it.sync = 1; it.base = f.done; it.base_ld = (int64_t)n_pairs * gf8::tc::EPI_WARPS; }
                 pb.stage[5].push_back(it);
-                it.mode = EPI_CAST; it.write_scale = i0 == 0 ? 1 : 0;
+                it.mode = EPI_CAST; it.write_scale = (i0 == 0 && c_this == 0) ? 1 : 0;
+                if (pairs) it.sync = 2;
                 pb.stage[6].push_back(it);
             } else {
                 pb.stage[5].push_back(it);
             }
-        }
+          }
         return;
     }
     for (int i0 = 0; i0 < m; i0 += 128)
@@ -492,8 +513,23 @@ gf8_status plan_finish(gf8_ctx* c, PlanBuilder& pb, Plan* p) {
         }
         pb.stage[0].swap(sorted);
     }
+    // pair launch: stage 5 becomes (amax item, cast item) pairs in call order; otherwise the sync marks are dropped and the two
+    // passes run as two launches
+    bool pair5 = pb.pair_ok && !pb.stage[5].empty() && pb.stage[5].size() == pb.stage[6].size();
+    for (size_t i = 0; pair5 && i < pb.stage[5].size(); ++i) pair5 = pb.stage[5][i].sync == 1 && pb.stage[6][i].sync == 2;
+    if (pair5) {
+        std::vector<Item> merged;
+        merged.reserve(2 * pb.stage[5].size());
+        for (size_t i = 0; i < pb.stage[5].size(); ++i) { merged.push_back(pb.stage[5][i]); merged.push_back(pb.stage[6][i]); }
+        pb.stage[5].swap(merged);
+        pb.stage[6].clear();
+    } else {
+        for (int s = 5; s <= 6; ++s)
+            for (Item& it : pb.stage[s]) if (it.sync) { it.sync = 0; it.base = nullptr; it.base_ld = 0; }
+    }
+    p->pair5 = pair5;
     for (int s = 0; s < 8; ++s) {
-        const bool grouped = s == 0 && pb.prob0.size() == pb.stage[0].size();
+        const bool grouped = (s == 0 && pb.prob0.size() == pb.stage[0].size()) || (s == 5 && pair5);
         if (!grouped) std::stable_sort(pb.stage[s].begin(), pb.stage[s].end(), [](const Item& a, const Item& b) {
             int64_t ta = 0, tb = 0;
             for (int g = 0; g < gf8::tc::NSEG; ++g) { ta += a.atoms[g]; tb += b.atoms[g]; }
@@ -547,12 +583,13 @@ gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
     if (p->d_ctr) CU_TRY(c, cudaMemsetAsync(p->d_ctr, 0, 8 * sizeof(int), st));
     for (int s = 0; s < 8; ++s) {
         if (!p->stage_cnt[s]) continue;
-        const int grid = std::min(p->stage_cnt[s], c->num_sms);
+        const bool pair = s == 5 && p->pair5;
+        const int grid = std::min(pair ? p->stage_cnt[s] / 2 : p->stage_cnt[s], c->num_sms);
         const int n_base = p->stage_base[s];
         // shared-memory split: update stages keep a short operand ring (their operands are L2-resident) and give
         // the rest to base tiles in flight (the HBM stream); panel stages give everything to the operand ring
         const int fuse = s == 7 ? 1 : 0, strip = (s == 5 || s == 6) ? 1 : 0, wide = p->stage_wide[s] && !n_base ? 1 : 0;
-        const int kmode = fuse ? 1 : (strip ? 2 : (wide ? (p->stage_wide[s] == 5 ? 5 : (p->stage_wide[s] == 3 ? 4 : 3)) : 0));
+        const int kmode = fuse ? 1 : (pair ? 6 : strip ? 2 : (wide ? (p->stage_wide[s] == 5 ? 5 : (p->stage_wide[s] == 3 ? 4 : 3)) : 0));
         // shared-memory split of the tile-mode update stages: 3 operand stages + the rest as base tiles in flight
         int n_stages = n_base ? (strip ? 4 : 3) : (wide ? (p->stage_wide[s] == 5 ? 2 : (p->stage_wide[s] == 3 ? 4 : 5)) : gf8::tc::MAX_STAGES), dbg = 0;
 #ifdef GF8_DEBUG

@@ -75,7 +75,9 @@ struct __align__(16) Item {
     int32_t b_mn;                 // 1: B is MN-major too (the factor GEMM X^T X reads both operands from X)
     int32_t strip;                // 1: strip item of the update (up to 256 rows x all columns; see tc_items_kernel)
     int32_t tri;                  // 1: segments 0..2 are the split products hi*hi, lo*hi, hi*lo of one operand pair: in a kmode 5
-    int32_t pad_;                 //    launch every K-atom brings A_hi, A_lo, B_hi, B_lo in once and feeds all three
+    int32_t sync;                 //    launch every K-atom brings A_hi, A_lo, B_hi, B_lo in once and feeds all three
+                                  // sync (pair launches, kmode 6): 1 = amax item, counts itself done in *(uint32_t*)base once per
+                                  // epilogue warp; 2 = cast item, starts when that counter has reached base_ld
     int64_t base_ld, out_ld;
     const void* base;
     void* out;
@@ -621,7 +623,10 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
     long long* const prof = prof_in;
 #endif
     const int fuse = kmode == 1 ? 1 : 0;           // kmode: 0 = tile items, 1 = fused update (TMEM-parked), 2 = strip items
-    const bool strip = kmode == 2;
+    // kmode 6 = strip items in PAIRS (amax item, cast item of the same sub-strip, adjacent in the list): a CTA claims a pair, so
+    // the cast pass re-reads its gradient tiles right after the amax pass has brought them in (L2), one launch for both passes
+    const bool pair = kmode == 6;
+    const bool strip = kmode == 2 || pair;
     // ctr != null: items are handed out dynamically (atomic counter, list order = start order), so item durations may
     // differ without idling CTAs and the planner's ordering decides which items run at the same time (L2 reuse).
     // The fused update keeps the static round-robin (its cast of parked tiles counts on it).
@@ -709,7 +714,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
         auto claim = [&](int after) {          // index of this CTA's next item (claimed one item ahead of its use)
             if (!dyn) return after + (int)gridDim.x;
             int v = 0;
-            if (lane == 0) v = atomicAdd(ctr, 1);
+            if (lane == 0) v = atomicAdd(ctr, pair ? 2 : 1);
             return __shfl_sync(0xFFFFFFFFu, v, 0);
         };
         int i = dyn ? claim(0) : (int)blockIdx.x;
@@ -728,8 +733,13 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
             if (lane < NCHUNK) reinterpret_cast<uint4*>(s_items + slot * ITEM_BYTES)[lane] = nxt;
             __syncwarp();
             if (lane == 0) mbar_arrive(ifull_bar(slot));
-            i = claim(i);
-            if (i < n_items && lane < NCHUNK) nxt = __ldg(reinterpret_cast<const uint4*>(items + i) + lane);
+            // pair launches: the amax item (even index) is followed by its cast item; the NEXT pair is claimed only after the
+            // cast item's loads have been issued, i.e. after its epilogue has passed the tensor's join (the base ring is shorter
+            // than a sub-strip): a pair claimed earlier could hold an amax item that this CTA's own waiting cast item needs
+            const bool defer_claim = pair && (i & 1);
+            if (pair && !(i & 1)) i = i + 1;
+            else if (!defer_claim) i = claim(i);
+            if (!defer_claim && i < n_items && lane < NCHUNK) nxt = __ldg(reinterpret_cast<const uint4*>(items + i) + lane);
             if (strip) {
                 // strip item: one base tile per (column tile, row block), in the order the epilogue consumes them
                 const Item& it = *item_slot(slot);
@@ -747,11 +757,15 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                             mbar_expect_tx(bfull_bar(bs), TILE_BYTES);
 #pragma unroll
                             for (int h = 0; h < 2; ++h)
-                                tma_load_2d(base_tile(bs) + h * 16384u, mp, 128 * ct + 64 * h, row0 + 128 * rb, bfull_bar(bs));
+                                tma_load_2d(base_tile(bs) + h * 16384u, mp, it.col0 + 128 * ct + 64 * h, row0 + 128 * rb, bfull_bar(bs));
                             }
                         }
                         __syncwarp();
                     }
+                if (defer_claim && ok) {
+                    i = claim(i);
+                    if (i < n_items && lane < NCHUNK) nxt = __ldg(reinterpret_cast<const uint4*>(items + i) + lane);
+                }
             } else if (n_base > 0) {
                 // the item's base tile(s): hi [+ lo], each two 64-column halves of 128 rows (converged warp, one
                 // elected lane issues)
@@ -1157,6 +1171,20 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
             if (ok && dyn && item_slot(slot)->mode == EPI_END) break;
             // the tensor's amax (EPI_CAST) is fetched before the data waits, so its latency hides behind them
             float cast_scale = 1.0f, cast_si = 1.0f;
+            if (ok && item_slot(slot)->mode == EPI_CAST && item_slot(slot)->sync == 2) {
+                // join: every amax item of the tensor has counted itself done (each after its atomicMax and a fence)
+                if (lane == 0) {
+                    const volatile uint32_t* cnt = reinterpret_cast<const volatile uint32_t*>(item_slot(slot)->base);
+                    const uint32_t want = (uint32_t)item_slot(slot)->base_ld;
+                    uint32_t spins = 0;
+                    while (*cnt < want) {
+                        __nanosleep(200);
+                        if (++spins > (1u << 23) || *reinterpret_cast<volatile int*>(err)) { atomicExch(err, 2); ok = false; break; }
+                    }
+                    __threadfence();
+                }
+                ok = __shfl_sync(0xFFFFFFFFu, ok ? 1 : 0, 0) != 0;
+            }
             if (ok && item_slot(slot)->mode == EPI_CAST)
                 scales_from_amax(*reinterpret_cast<volatile uint32_t*>(item_slot(slot)->amax), item_slot(slot)->fmt == 0 ? 448.0f : 57344.0f,
                                  cast_scale, cast_si);
@@ -1174,7 +1202,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 auto ef_prefetch = [&](int t) {
                     if (!ef_base || t >= nct * nrb) return;
                     const int pct = t / nrb, prb = t % nrb;
-                    const float* tile = ef_base + ((int64_t)((it.row0 >> 7) + prb) * ((it.out_ld + 127) >> 7) + pct) * EF_TILE;
+                    const float* tile = ef_base + ((int64_t)((it.row0 >> 7) + prb) * ((it.out_ld + 127) >> 7) + (it.col0 >> 7) + pct) * EF_TILE;
 #pragma unroll
                     for (int u = 0; u < 2; ++u) {
                         const int line = 2 * lane + u, chunk = line >> 2, sub = line & 3;      // chunk = g * 8 + q of this warp's half
@@ -1198,7 +1226,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                         const long long t_s0 = prof ? clock64() : 0;
                         if (!(dbg & 32))
                             epilogue_tile<EF>(it, tmem_base + sacc * 128u, base_tile(sbs), 1, warp, lane, s_red, maps, cast_scale, cast_si,
-                                          it.row0 + 128 * rb, 128 * ct, it.write_scale != 0 && ct == 0 && rb == 0,
+                                          it.row0 + 128 * rb, it.col0 + 128 * ct, it.write_scale != 0 && ct == 0 && rb == 0,
                                           it.mode == EPI_BLOCKCAST ? it.scale_inv_out + (size_t)((it.row0 >> 7) + rb) * nct + ct
                                                                    : it.scale_inv_out,
                                           &run_max);
@@ -1210,7 +1238,13 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                     }
                 if (ok && it.mode == EPI_AMAX) {
                     run_max = warp_max_u32(run_max);
-                    if (lane == 0 && run_max != 0u) atomicMax(it.amax, run_max);
+                    if (lane == 0) {
+                        if (run_max != 0u) atomicMax(it.amax, run_max);
+                        if (it.sync == 1) {       // (the maximum is performed before the count: fence between the two atomics)
+                            __threadfence();
+                            atomicAdd(reinterpret_cast<uint32_t*>(const_cast<void*>(it.base)), 1u);
+                        }
+                    }
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(iempty_bar(slot));

@@ -420,6 +420,41 @@ def test_fast_fused_update_matches_two_pass(monkeypatch):
         assert torch.equal(outs[0][0][r], outs[1][0][r]) and torch.equal(outs[0][1][r], outs[1][1][r])
 
 
+@pytest.mark.parametrize("name", ["llama600m-q", "wide-1to4", "tall-4to1", "ragged-wide-panels"])
+def test_fast_pair_launch_matches_two_pass(name, monkeypatch):
+    """The opt-in pair launch (GF8_TC_PAIR=1 when the context is created: both update passes in one launch of (amax item,
+    cast item) pairs over sub-strips, the cast items joining on the tensor's amax through a counter in global memory) produces
+    the same codes and scales as the default amax launch + cast launch.  Shapes: square with two column chunks, 1:4 with
+    several chunks of unequal width, 4:1, and a ragged one whose sub-strips are too short (falls back to two launches)."""
+    c = fcase(name)
+    gs = [c.rank_grad(r) for r in range(4)]
+
+    def fresh():
+        ctx = gf8.create([c.layer], gf8.PREC_FAST)
+        for side in (gf8.SIDE_IN, gf8.SIDE_OUT):
+            U, mu, rho = c.ctx.get_basis(0, side)
+            ctx.set_basis(0, side, U, mu, rho)
+        return ctx
+
+    outs, launches = [], []
+    for pair in (False, True):
+        if pair:
+            monkeypatch.setenv("GF8_TC_PAIR", "1")
+        ctx = fresh()
+        codes = [torch.empty((c.m, c.n), dtype=torch.uint8, device="cuda") for _ in gs]
+        sinvs = [torch.empty(1, dtype=torch.float32, device="cuda") for _ in gs]
+        for _ in range(2):                       # (twice: the second run reuses the plan and its zeroed counters)
+            before = ctx.launch_count()
+            ctx.encode_many([0] * len(gs), gs, codes, sinvs)
+            ctx.sync_check()
+        launches.append(ctx.launch_count() - before)
+        outs.append((codes, sinvs))
+    for r in range(len(gs)):
+        assert torch.equal(outs[0][0][r], outs[1][0][r]) and torch.equal(outs[0][1][r], outs[1][1][r])
+    if name != "ragged-wide-panels":
+        assert launches[1] == launches[0] - 1, launches      # one launch fewer: the two update passes have become one
+
+
 @pytest.mark.parametrize("name", ["ragged-bf16", "wide-k96"])
 def test_fast_g6_factor_on_tensor_cores(name):
     """a1 on the tcgen05 engine (BF16 samples, both MMA operands MN-major views of X): BF16 products are exact in
