@@ -528,11 +528,13 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
         if (write_scale && lead) *sinv_out = cast_si;
     }
     if (mode == EPI_CAST || mode == EPI_BLOCKCAST) {
-        // 64 codes per row half, written straight from registers: every thread owns 64 contiguous bytes of its row
-        // (four 16-byte stores; L2 merges the sectors), so the cast needs neither shared-memory staging nor a
-        // generic -> async proxy fence, and the base slot goes back to the producer at once.
-        const int grow = row0 + r;
-        const bool row_ok = grow < it.row0 + it.rows;
+        // 64 codes per row half and thread.  Written straight from registers, a warp's store instruction would touch 32 different
+        // 128 B lines with 16 bytes each, and L1TEX takes them one line per cycle: 1024 cycles per tile, more than the rest of
+        // the cast epilogue (measured: 1757 cycles per tile against 685 for the amax epilogue).  So the warp transposes its
+        // 32 x 64 B through the 4 KB of the base tile that only it reads (its 32 rows of this column half, dead once the values
+        // are in registers): afterwards four lanes hold the 64 contiguous bytes of a row and an instruction touches 8 lines.
+        // No CTA-level barrier and no proxy fence are involved, so the base slot still goes back to the producer at once.
+        const int q4 = warp & 3, l_row = lane >> 2, l_chk = lane & 3;
         for (int h = h0; h < h1; ++h) {
             uint4 cd[4];
 #pragma unroll
@@ -546,12 +548,22 @@ __device__ __forceinline__ bool epilogue_tile(const Item& it, uint32_t tmem_acc,
                     else ef_store32<1>(resid_row + (2 * h + g) * 4096, ef_cols - 64 * h - 32 * g, v, cd[2 * g], cd[2 * g + 1], si_cast);
                 }
             }
-            if (row_ok) {
-                uint8_t* p = reinterpret_cast<uint8_t*>(it.out) + (int64_t)grow * it.out_ld + col0 + 64 * h;
+            // staging: row l of the warp keeps its chunk q at 16-byte slot 4 l + (q ^ ((l >> 1) & 3)) (4 wavefronts per
+            // instruction both ways: the minimum for 512 bytes)
+            const uint32_t stg = tile + 16384u * (uint32_t)h + 4096u * (uint32_t)q4;
+            __syncwarp();                                     // (every lane has read its base values)
 #pragma unroll
-                for (int q = 0; q < 4; ++q)
-                    if (col0 + 64 * h + 16 * q < it.col0 + it.cols) *reinterpret_cast<uint4*>(p + 16 * q) = cd[q];
+            for (int q = 0; q < 4; ++q) sts128(stg + (uint32_t)(4 * lane + (q ^ ((lane >> 1) & 3))) * 16u, cd[q]);
+            __syncwarp();
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int lr = 8 * j + l_row;                 // row of the warp this lane stores a piece of
+                const uint4 piece = lds128(stg + (uint32_t)(4 * lr + (l_chk ^ ((lr >> 1) & 3))) * 16u);
+                const int grow = row0 + 32 * q4 + lr, gcol = col0 + 64 * h + 16 * l_chk;
+                if (grow < it.row0 + it.rows && gcol < it.col0 + it.cols)
+                    *reinterpret_cast<uint4*>(reinterpret_cast<uint8_t*>(it.out) + (int64_t)grow * it.out_ld + gcol) = piece;
             }
+            __syncwarp();                                     // (the staging area is read before the next half overwrites... its own)
         }
         return false;
     }
