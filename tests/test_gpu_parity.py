@@ -607,6 +607,46 @@ def test_bad_state_and_argument_errors():
     assert e.value.status == 3
 
 
+# ---- degenerate inputs on the fused tensor-core path (S13) ----------------------------------------------------------------
+@pytest.mark.parametrize("scaling", [gf8.SCALE_TENSOR, gf8.SCALE_BLOCK128])
+def test_fast_degenerate_gradients_follow_the_quantizer_rules(scaling):
+    """The FAST encode on the inputs the method's rules single out (S13), several per batched call: an all-zero gradient
+    (amax = 0 => scale = scale_inv = 1, every code +-0), a gradient whose only nonzero element is tiny (2^-120: fmax / amax
+    overflows => scale = 1), one huge finite element (the rest falls to the bottom of the format), and non-finite elements
+    (NaN / Inf dominate the amax => scale = 1, NaN code for them).  Gate: G3-self -- codes and scales are those of the ORACLE
+    quantizer applied to the GPU's own tapped W~ -- and decode of the zero payload is exactly zero.  Empty batched calls
+    (n = 0) are accepted."""
+    c = Case(400, 464, 32, 48, gf8.SIDE_BOTH, "bf16", 9, q=2, scaling=scaling, precision=gf8.PREC_FAST)
+    base = c.rank_grad(0).contiguous()
+    zero = torch.zeros_like(base)
+    tiny = torch.zeros_like(base); tiny[37, 211] = 2.0 ** -120
+    huge = base.clone(); huge[5, 7] = 3.0e38
+    nonf = base.clone(); nonf[1, 2] = float("nan"); nonf[300, 400] = float("inf"); nonf[399, 463] = float("-inf")
+    gs = [zero, tiny, huge, nonf]
+    codes = [torch.empty((c.m, c.n), dtype=torch.uint8, device="cuda") for _ in gs]
+    sinvs = [torch.empty(c.layer.n_scales(), dtype=torch.float32, device="cuda") for _ in gs]
+    c.ctx.encode_many([0] * len(gs), gs, codes, sinvs)
+    c.ctx.sync_check()
+    tab = oracle.fp8_table(c.fmt)
+    for k, g in enumerate(gs):
+        tap = c.ctx.whiten_f32(0, g).cpu().numpy()
+        oc, os_ = oracle.quantize(tap, c.fmt, c.scaling)
+        gc = codes[k].cpu().numpy()
+        assert np.array_equal(sinvs[k].cpu().numpy().view(np.uint32), os_.view(np.uint32)), k
+        nan_o = np.isnan(tab[oc])
+        assert np.array_equal(np.isnan(tab[gc]), nan_o), k                    # (a NaN code has two spellings per sign)
+        assert np.array_equal(gc[~nan_o], oc[~nan_o]), k
+    assert bool((sinvs[0] == 1.0).all()) and bool(((codes[0] & 0x7F) == 0).all())
+    assert bool((sinvs[1] == 1.0).all())
+    out = c.ctx.reduce_decoded(0, [codes[0], codes[0]], [sinvs[0], sinvs[0]], True, dt=gf8.DT_BF16)
+    c.ctx.sync_check()
+    assert bool((out.float() == 0).all())
+    # n = 0: nothing to do, no error
+    c.ctx.encode_many([], [], [], [], dt=gf8.DT_BF16)
+    c.ctx.reduce_decoded_many([], [], [], 2, [], dt=gf8.DT_BF16)
+    c.ctx.sync_check()
+
+
 # ---- chain: whole pipeline, each side on its own upstream state (reported, loosely bounded) --------------
 def test_chain_config0_reports_metrics():
     cfg = synth.config(0)
