@@ -33,9 +33,9 @@
  *      * steady state: no allocation, no host synchronisation -- except that the pinned records of the batched
  *        factor / refresh calls are double-buffered and a call waits (cudaEventSynchronize) for the call two
  *        before it if that one is still running.
- *  - Reproducibility: the FAST path (tensor cores) and the batched geometry calls are deterministic (fixed summation
- *    orders).  The EXACT path's FP32 SIMT transform sums its split-K partials with atomics: results agree with the oracle
- *    within the EXACT gates but may differ in the last bit from run to run.
+ *  - Reproducibility: every path sums in a fixed order (tensor-core pipelines, the batched geometry calls, and the FP32 /
+ *    FP64 SIMT GEMM, whose split-K partial products go through a workspace and are added up in split order): the same call
+ *    on the same inputs returns the same bits from run to run.
  *  - Errors: a gf8_status is returned; nothing throws or aborts across the ABI.  Argument errors
  *    are detected before any launch.  gf8_last_error(ctx) gives a message for the last failure.
  *  - One ctx (hence one basis per layer) is shared by all R simulated ranks (S12).

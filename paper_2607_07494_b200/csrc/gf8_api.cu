@@ -29,15 +29,26 @@ gf8_status launch_gemm(gf8_ctx* c, cudaStream_t st, const TA* A, int64_t sa_i, i
                        int64_t sb_l, int64_t sb_j, TC* C, int64_t ldc, int M, int N, int K, const float* lscale,
                        const float* rowscale, TAcc alpha, TAcc beta, int splits = 1) {
     if (M <= 0 || N <= 0) return GF8_OK;
-    GemmArgs<TA, TB, TC, TAcc> g{A, sa_i, sa_l, B, sb_l, sb_j, C, ldc, M, N, K, lscale, rowscale, alpha, beta};
-    if (splits > 1) {
-        // split-K accumulates atomically: C must hold beta*C already.  Only beta in {0,1} is used.
-        if (beta == (TAcc)0) {
-            if (ldc != N) return fail(c, GF8_ERR_INVALID_ARG, "split-K gemm needs a dense C");
-            CU_TRY(c, cudaMemsetAsync(C, 0, sizeof(TC) * (size_t)M * N, st));
-        }
-    }
+    GemmArgs<TA, TB, TC, TAcc> g{A, sa_i, sa_l, B, sb_l, sb_j, C, ldc, M, N, K, lscale, rowscale, alpha, beta, nullptr};
     dim3 grid((N + SG_BN - 1) / SG_BN, (M + SG_BM - 1) / SG_BM, splits);
+    if (splits > 1) {
+        // split-K: every split writes its partial product to the context's workspace and a second kernel adds them up in
+        // split order, so the result does not depend on the order in which the CTAs finish (EXACT results are reproducible)
+        const size_t need = sizeof(TAcc) * (size_t)splits * M * N;
+        if (need > c->gemm_ws_bytes) {
+            CU_TRY(c, cudaStreamSynchronize(st));
+            if (c->gemm_ws) CU_TRY(c, cudaFree(c->gemm_ws));
+            c->gemm_ws = nullptr; c->gemm_ws_bytes = 0;
+            CU_TRY(c, cudaMalloc(&c->gemm_ws, need));
+            c->gemm_ws_bytes = need;
+        }
+        g.ws = static_cast<TAcc*>(c->gemm_ws);
+        simt_gemm_kernel<TA, TB, TC, TAcc><<<grid, 256, 0, st>>>(g);
+        LAUNCH_CHECK(c);
+        splitk_sum_kernel<TC, TAcc><<<grid_for(c, (int64_t)M * N, 256, 4), 256, 0, st>>>(g.ws, splits, M, N, C, ldc, beta, rowscale);
+        LAUNCH_CHECK(c);
+        return GF8_OK;
+    }
     simt_gemm_kernel<TA, TB, TC, TAcc><<<grid, 256, 0, st>>>(g);
     LAUNCH_CHECK(c);
     return GF8_OK;
@@ -820,6 +831,7 @@ gf8_status gf8_destroy(gf8_ctx* ctx) {
         cudaEventDestroy(ctx->hs_start); cudaEventDestroy(ctx->hs_done);
         for (int q = 0; q < GF8_HOST_CHUNKS; ++q) { cudaEventDestroy(ctx->hs_in_ev[q]); cudaEventDestroy(ctx->hs_comp_ev[q]); }
     }
+    if (ctx->gemm_ws) cudaFree(ctx->gemm_ws);
     if (ctx->ef_scratch) cudaFree(ctx->ef_scratch);
     if (ctx->rb_arena) cudaFree(ctx->rb_arena);
     if (ctx->rb_jobs) cudaFree(ctx->rb_jobs);

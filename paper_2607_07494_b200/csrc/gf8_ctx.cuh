@@ -96,6 +96,7 @@ struct gf8_ctx {
     // auxiliary stream: the streaming kernels of Euclidean tensors overlap the tensor-core stages of a batched call
     cudaStream_t aux_stream = nullptr;
     cudaEvent_t aux_fork_ev = nullptr, aux_join_ev = nullptr;
+    void* gemm_ws = nullptr; size_t gemm_ws_bytes = 0;   // split-K workspace of the SIMT GEMM (partial products, summed in order)
     float* ef_scratch = nullptr; size_t ef_cap = 0;   // FP32 W~ of a chunk of problems (gf8_encode_ef_many)
     // tap scratch (gf8_quantize_f32 with arbitrary shapes)
     uint32_t* tap_amax = nullptr; float* tap_scale = nullptr; size_t tap_cap = 0;

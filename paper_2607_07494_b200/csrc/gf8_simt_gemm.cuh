@@ -7,7 +7,8 @@
 //
 //   C[i][j] = rowscale[i] * ( alpha * sum_l A(i,l) * lscale[l] * B(l,j) + beta * C[i][j] )
 //   A(i,l) = A[i*sa_i + l*sa_l],  B(l,j) = B[l*sb_l + j*sb_j],  C row-major with leading dim ldc.
-// gridDim.z > 1 splits K; partial sums are then atomically added into C (caller pre-sets C).
+// gridDim.z > 1 splits K; each split writes its partial product to the workspace g.ws and splitk_sum_kernel adds them up in
+// split order (deterministic); without a workspace the partial sums are added into C atomically (caller pre-sets C).
 #pragma once
 #include "gf8_common.cuh"
 
@@ -22,6 +23,8 @@ struct GemmArgs {
     const float* lscale;    // length K or nullptr
     const float* rowscale;  // length M or nullptr
     TAcc alpha, beta;
+    TAcc* ws;               // split-K workspace [gridDim.z][M][N] (deterministic: summed in split order by splitk_sum_kernel),
+                            // or nullptr: partial sums are added into C atomically
 };
 
 template <typename TC, typename TAcc> __device__ __forceinline__ void store_c(TC* p, TAcc v);
@@ -102,7 +105,9 @@ __global__ void __launch_bounds__(256) simt_gemm_kernel(const GemmArgs<TA, TB, T
             const int gj = j0 + tx * 4 + c;
             if (gj >= g.N) continue;
             TC* p = g.C + (int64_t)gi * g.ldc + gj;
-            if (nsplit > 1) {
+            if (nsplit > 1 && g.ws) {
+                g.ws[((int64_t)blockIdx.z * g.M + gi) * g.N + gj] = rs * g.alpha * acc[r][c];
+            } else if (nsplit > 1) {
                 atomicAdd(p, (TC)(rs * g.alpha * acc[r][c]));
             } else {
                 TAcc v = g.alpha * acc[r][c];
@@ -110,6 +115,21 @@ __global__ void __launch_bounds__(256) simt_gemm_kernel(const GemmArgs<TA, TB, T
                 store_c<TC, TAcc>(p, rs * v);
             }
         }
+    }
+}
+
+// C[i][j] = (beta != 0 ? rowscale[i] * beta * C[i][j] : 0) + sum over splits z = 0, 1, ... of ws[z][i][j]  (fixed order)
+template <typename TC, typename TAcc>
+__global__ void __launch_bounds__(256) splitk_sum_kernel(const TAcc* __restrict__ ws, int splits, int M, int N, TC* __restrict__ C,
+                                                         int64_t ldc, TAcc beta, const float* __restrict__ rowscale) {
+    const int64_t total = (int64_t)M * N;
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
+        const int i = (int)(idx / N), j = (int)(idx % N);
+        TC* p = C + (int64_t)i * ldc + j;
+        TAcc s = (TAcc)0;
+        if (beta != (TAcc)0) s = (rowscale ? (TAcc)rowscale[i] : (TAcc)1) * beta * (TAcc)(*p);
+        for (int z = 0; z < splits; ++z) s += ws[(int64_t)z * total + idx];
+        store_c<TC, TAcc>(p, s);
     }
 }
 
