@@ -589,7 +589,10 @@ gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
         // shared-memory split: update stages keep a short operand ring (their operands are L2-resident) and give
         // the rest to base tiles in flight (the HBM stream); panel stages give everything to the operand ring
         const int fuse = s == 7 ? 1 : 0, strip = (s == 5 || s == 6) ? 1 : 0, wide = p->stage_wide[s] && !n_base ? 1 : 0;
-        const int kmode = fuse ? 1 : (pair ? 6 : strip ? 2 : (wide ? (p->stage_wide[s] == 5 ? 5 : (p->stage_wide[s] == 3 ? 4 : 3)) : 0));
+        const int kmode0 = fuse ? 1 : (pair ? 6 : strip ? 2 : (wide ? (p->stage_wide[s] == 5 ? 5 : (p->stage_wide[s] == 3 ? 4 : 3)) : 0));
+        // tile items with streamed bases (the update stages of decode and of ranks above 64) are handed out in runs of 8
+        const int claim_chunk = ((s == 3 || s == 4) && n_base > 0 && !fuse) ? 8 : 1;
+        const int kmode = kmode0 | (claim_chunk > 1 ? claim_chunk << 8 : 0);
         // shared-memory split of the tile-mode update stages: 3 operand stages + the rest as base tiles in flight
         int n_stages = n_base ? (strip ? 4 : 3) : (wide ? (p->stage_wide[s] == 5 ? 2 : (p->stage_wide[s] == 3 ? 4 : 5)) : gf8::tc::MAX_STAGES), dbg = 0;
 #ifdef GF8_DEBUG

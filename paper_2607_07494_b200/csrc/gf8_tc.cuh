@@ -637,6 +637,11 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
     const int fuse = kmode == 1 ? 1 : 0;           // kmode: 0 = tile items, 1 = fused update (TMEM-parked), 2 = strip items
     // kmode 6 = strip items in PAIRS (amax item, cast item of the same sub-strip, adjacent in the list): a CTA claims a pair, so
     // the cast pass re-reads its gradient tiles right after the amax pass has brought them in (L2), one launch for both passes
+    // (bits 8.. of kmode: claim granularity.  A CTA takes `chunk` consecutive items per claim, so that tile items -- whose ten
+    //  tensor maps change with the tensor -- come in runs of the same tensor: every new map costs its TMA instruction a
+    //  descriptor fetch, and a CTA that gets one or two tiles per tensor pays that on every item)
+    const int chunk = (kmode >> 8) > 0 ? (kmode >> 8) : 1;
+    kmode &= 0xFF;
     const bool pair = kmode == 6;
     const bool strip = kmode == 2 || pair;
     // ctr != null: items are handed out dynamically (atomic counter, list order = start order), so item durations may
@@ -726,7 +731,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
         auto claim = [&](int after) {          // index of this CTA's next item (claimed one item ahead of its use)
             if (!dyn) return after + (int)gridDim.x;
             int v = 0;
-            if (lane == 0) v = atomicAdd(ctr, pair ? 2 : 1);
+            if (lane == 0) v = atomicAdd(ctr, pair ? 2 : chunk);
             return __shfl_sync(0xFFFFFFFFu, v, 0);
         };
         int i = dyn ? claim(0) : (int)blockIdx.x;
@@ -750,6 +755,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
             // than a sub-strip): a pair claimed earlier could hold an amax item that this CTA's own waiting cast item needs
             const bool defer_claim = pair && (i & 1);
             if (pair && !(i & 1)) i = i + 1;
+            else if (dyn && !pair && chunk > 1 && (i + 1) % chunk != 0 && i + 1 < n_items) i = i + 1;     // (next item of the claimed run)
             else if (!defer_claim) i = claim(i);
             if (!defer_claim && i < n_items && lane < NCHUNK) nxt = __ldg(reinterpret_cast<const uint4*>(items + i) + lane);
             if (strip) {
