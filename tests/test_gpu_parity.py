@@ -72,7 +72,7 @@ def test_g1_quantizer_edge_values(ctx0, fmt):
 # ---- G4: reduce, bit-exact ------------------------------------------------------------------------------
 @pytest.mark.parametrize("fmt", [gf8.E4M3, gf8.E5M2])
 @pytest.mark.parametrize("scaling", [gf8.SCALE_TENSOR, gf8.SCALE_BLOCK128])
-@pytest.mark.parametrize("R,average", [(1, False), (2, True), (5, True), (16, True)])
+@pytest.mark.parametrize("R,average", [(1, False), (2, True), (5, True), (16, True), (64, True)])      # 64 = GF8_MAX_R
 def test_g4_reduce_bit_exact(ctx0, fmt, scaling, R, average):
     rng = np.random.default_rng(R * 7 + fmt)
     m, n = 200, 272
@@ -605,6 +605,33 @@ def test_bad_state_and_argument_errors():
     with pytest.raises(gf8.Gf8Error) as e:                                 # misaligned codes pointer
         ctx2.encode(0, G, codes[1:256 * 256 + 1].view(256, 256), torch.zeros(1, device="cuda"))
     assert e.value.status == 3
+
+
+def test_fast_reduce_decoded_at_the_maximum_rank_count():
+    """GF8_MAX_R = 64 payloads through the FAST batched decode (the grouped reduction takes the ranks eight at a time) for a
+    whitened and a Euclidean tensor: G5 against the oracle on oracle payloads (whitened), bit-exact (Euclidean); R = 65 is
+    rejected before any launch."""
+    R = 64
+    c = fcase("ragged-bf16")
+    pays = [c.oracle_encode(c.rank_grad(r))[:2] for r in range(R)]
+    want = c.oracle_reduce_decoded([p[0] for p in pays], [p[1] for p in pays])
+    dc, ds = [_dev(p[0]) for p in pays], [_dev(p[1]) for p in pays]
+    out = torch.empty((c.m, c.n), dtype=torch.bfloat16, device="cuda")
+    c.ctx.reduce_decoded_many([0], dc, ds, R, [out], average=True)
+    c.ctx.sync_check()
+    assert relfro(to_np64(out), want) <= TOL_FAST_BF16
+    with pytest.raises(gf8.Gf8Error) as e:
+        c.ctx.reduce_decoded_many([0], dc + dc[:1], ds + ds[:1], R + 1, [out], average=True)
+    assert e.value.status == 1
+    lay = gf8.Layer(208, 336, gf8.SIDE_NONE)
+    ctx = gf8.create([lay], gf8.PREC_FAST)
+    rng = np.random.default_rng(64)
+    ep = [oracle.quantize(rng.normal(0, 1 + r % 5, (208, 336)).astype(np.float32)) for r in range(R)]
+    wantE = oracle.reduce([p[0] for p in ep], [p[1] for p in ep])
+    outE = torch.empty((208, 336), dtype=torch.bfloat16, device="cuda")
+    ctx.reduce_decoded_many([0], [_dev(p[0]) for p in ep], [_dev(p[1]) for p in ep], R, [outE], average=True)
+    ctx.sync_check()
+    assert np.array_equal(bf16_bits(outE), oracle.to_bf16_bits(wantE.astype(np.float64)))
 
 
 # ---- degenerate inputs on the fused tensor-core path (S13) ----------------------------------------------------------------
