@@ -719,9 +719,8 @@ gf8_status gf8_stage_times(gf8_ctx* ctx, float* ms_out, int* n_out, void* stream
         float ms = 0.0f;
         CU_TRY(ctx, cudaEventSynchronize(e.b));
         CU_TRY(ctx, cudaEventElapsedTime(&ms, e.a, e.b));
-        const int bucket = e.stage >= 8 ? 0 : e.stage;        // (row bands of the panel stage count as panel launches)
-        ms_out[bucket] += ms;
-        n_out[bucket] += 1;
+        ms_out[e.stage] += ms;
+        n_out[e.stage] += 1;
         ctx->stage_event_pool.push_back(e);
     }
     ctx->stage_events.clear();

@@ -9,22 +9,14 @@
 
 // A cached launch plan: everything a batched call needs on the device, built on first use of a given
 // argument list (steady-state training calls repeat the same pointers every step).
-// Stages of a plan.  0..7 as listed in Plan; 8..10 are the ROW BANDS 1..3 of the panel stage (band 0 is stage 0): tall problems
-// (m >= 2 n) cut the K loop of their column panels Q^T = src^T U_G into bands of about n rows, band b accumulating onto band
-// b - 1's FP32 result, and list each band's row panels with it, so that every launch sweeps squarish pieces whose second reader
-// finds them in L2 (a 4096 x 1536 tensor's 2 MB column panels otherwise keep 164 MB in flight on 148 CTAs: a third of the
-// re-reads hit).  Launch order: 0, 8, 9, 10, 1, 2, ..., 7.
-constexpr int N_STAGES = 11;
-constexpr int STAGE_ORDER[N_STAGES] = {0, 8, 9, 10, 1, 2, 3, 4, 5, 6, 7};
-
 struct Plan {
     CUtensorMap* d_maps = nullptr;
     gf8::tc::Item* d_items = nullptr;
     // stages: 0 P' and Q^T, 1 S, 2 Q'^T, 3 update tiles (amax / block cast / store), 4 update tiles (cast),
     //         5 update strips (amax / block cast), 6 update strips (cast), 7 fused update (opt-in)
-    int stage_off[N_STAGES] = {}, stage_cnt[N_STAGES] = {};
-    int stage_wide[N_STAGES] = {};       // the stage holds 256-row panel items: wide operand stages (kmode 3)
-    int stage_base[N_STAGES] = {};       // streamed base tiles per item in that stage's launch (0, 1 or 2)
+    int stage_off[8] = {0, 0, 0, 0, 0, 0, 0, 0}, stage_cnt[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    int stage_wide[8] = {0, 0, 0, 0, 0, 0, 0, 0};  // the stage holds 256-row panel items: wide operand stages (kmode 3)
+    int stage_base[8] = {0, 0, 0, 0, 0, 0, 0, 0};  // streamed base tiles per item in that stage's launch (0, 1 or 2)
     bool ef = false;                     // f1: the update stages run the error-feedback instance of the kernel
     bool pair5 = false;                  // stage 5 holds (amax item, cast item) pairs: one launch for both update passes (kmode 6)
     int runs = 0;                        // launches so far: the first one acquires its tensor maps with proxy fences
@@ -216,7 +208,7 @@ gf8_status fast_slot(gf8_ctx* c, LayerState& L, size_t idx, bool need_src16, boo
 struct PlanBuilder {
     std::vector<CUtensorMap> maps;
     std::map<const void*, int> map_index;      // buffer -> index (static maps are shared by all problems)
-    std::vector<Item> stage[N_STAGES];
+    std::vector<Item> stage[8];
     std::vector<int> prob0;                    // stage 0: the problem (add_transform call) each item belongs to
     int cur_problem = 0;
     bool pair_ok = true;                       // every strip item of stages 5 / 6 so far can run in a pair launch
@@ -305,52 +297,35 @@ void add_transform(PlanBuilder& pb, LayerState& L, Slot* s, int src_map, int src
     auto push0 = [&](const Item& it) { pb.stage[0].push_back(it); pb.prob0.push_back(problem); };
     // (kp <= 64: one item covers 256 rows, its two 128-row accumulators share every basis atom the loader brings in)
     const int stepA = kpA <= 64 ? 256 : 128, stepG = kpG <= 64 ? 256 : 128;
-    // Row bands (see N_STAGES): tall problems with both sides whitened, single-pass BF16 operands, kp <= 64 on both sides
-    int band_rows = m, n_bands = 1;
-    if (useA && useG && !split && !inverse && kpA <= 64 && kpG <= 64 && m >= 2 * n) {
-        band_rows = (n + 255) / 256 * 256;
-        n_bands = (m + band_rows - 1) / band_rows;
-        if (n_bands > 4) { n_bands = 4; band_rows = ((m + 3) / 4 + 255) / 256 * 256; }
-    }
-    auto push_band = [&](const Item& it, int band) {
-        if (band == 0) push0(it);
-        else pb.stage[7 + band].push_back(it);
-    };
-    for (int band = 0; band < n_bands; ++band) {
-        const int r_lo = band * band_rows, r_hi = std::min(m, r_lo + band_rows);
-        if (useG)      // Q^T = src^T U_G : column panels (A is MN-major), K = the band's rows
-            for (int j0 = 0; j0 < n; j0 += stepG)
-                for (int nc = 0; nc < kpG; nc += 128) {
-                    Item it = blank_item();
-                    int seg = 0;
-                    it.a_mn = 1; it.N = std::min(128, kpG - nc);
-                    add_product(it, seg, mSrc, mUGt, (r_hi - r_lo + 63) / 64, j0, r_lo, r_lo, nc);
-                    it.tri = (seg == 3 && it.N <= 64) ? 1 : 0;
-                    it.mode = EPI_STORE; it.row0 = j0; it.col0 = nc; it.rows = std::min(stepG, n - j0); it.cols = it.N;
-                    if (useA) {
-                        it.out = s->Qt; it.out_ld = kpG; it.out_type = TY_F32;
-                        if (band > 0) { it.base = s->Qt; it.base_ld = kpG; it.base_type = TY_F32; }     // + the bands before
-                    } else {
-                        it.out = s->Qpt; it.out_lo = split ? s->Qpt_lo : nullptr; it.out_ld = kpG; it.out_type = TY_BF16;
-                        it.colscale = eG + nc;
-                    }
-                    push_band(it, band);
+    if (useA)      // P' = (src U_A) E_A : row panels
+        for (int i0 = 0; i0 < m; i0 += stepA)
+            for (int nc = 0; nc < kpA; nc += 128) {
+                Item it = blank_item();
+                int seg = 0;
+                it.N = std::min(128, kpA - nc);
+                add_product(it, seg, mSrc, mUAt, (n + 63) / 64, 0, i0, 0, nc);
+                it.tri = (seg == 3 && it.N <= 64) ? 1 : 0;      // split products of one operand pair: interleaved per K-atom
+                it.mode = EPI_STORE; it.out = s->Pp; it.out_lo = split ? s->Pp_lo : nullptr; it.out_ld = kpA;
+                it.out_type = TY_BF16; it.colscale = eA + nc;
+                it.row0 = i0; it.col0 = nc; it.rows = std::min(stepA, m - i0); it.cols = it.N;
+                push0(it);
+            }
+    if (useG) {    // Q^T = src^T U_G : column panels (A is MN-major)
+        for (int j0 = 0; j0 < n; j0 += stepG)
+            for (int nc = 0; nc < kpG; nc += 128) {
+                Item it = blank_item();
+                int seg = 0;
+                it.a_mn = 1; it.N = std::min(128, kpG - nc);
+                add_product(it, seg, mSrc, mUGt, (m + 63) / 64, j0, 0, 0, nc);
+                it.tri = (seg == 3 && it.N <= 64) ? 1 : 0;
+                it.mode = EPI_STORE; it.row0 = j0; it.col0 = nc; it.rows = std::min(stepG, n - j0); it.cols = it.N;
+                if (useA) { it.out = s->Qt; it.out_ld = kpG; it.out_type = TY_F32; }
+                else {
+                    it.out = s->Qpt; it.out_lo = split ? s->Qpt_lo : nullptr; it.out_ld = kpG; it.out_type = TY_BF16;
+                    it.colscale = eG + nc;
                 }
-        if (useA)      // P' = (src U_A) E_A : the row panels of the band
-            for (int i0 = r_lo; i0 < r_hi; i0 += stepA)
-                for (int nc = 0; nc < kpA; nc += 128) {
-                    Item it = blank_item();
-                    int seg = 0;
-                    it.N = std::min(128, kpA - nc);
-                    add_product(it, seg, mSrc, mUAt, (n + 63) / 64, 0, i0, 0, nc);
-                    it.tri = (seg == 3 && it.N <= 64) ? 1 : 0;      // split products of one operand pair: interleaved per K-atom
-                    it.mode = EPI_STORE; it.out = s->Pp; it.out_lo = split ? s->Pp_lo : nullptr; it.out_ld = kpA;
-                    it.out_type = TY_BF16; it.colscale = eA + nc;
-                    it.row0 = i0; it.col0 = nc; it.rows = std::min(stepA, r_hi - i0); it.cols = it.N;
-                    push_band(it, band);
-                }
-    }
-    if (useG) {
+                push0(it);
+            }
         if (useA) {
             // (S E_A)^T = P'^T U_G, stored transposed as SEA[g][a]
             for (int a0 = 0; a0 < kpA; a0 += 128)
@@ -553,8 +528,8 @@ gf8_status plan_finish(gf8_ctx* c, PlanBuilder& pb, Plan* p) {
             for (Item& it : pb.stage[s]) if (it.sync) { it.sync = 0; it.base = nullptr; it.base_ld = 0; }
     }
     p->pair5 = pair5;
-    for (int s = 0; s < N_STAGES; ++s) {
-        const bool grouped = (s == 0 && pb.prob0.size() == pb.stage[0].size()) || (s == 5 && pair5) || s >= 8;
+    for (int s = 0; s < 8; ++s) {
+        const bool grouped = (s == 0 && pb.prob0.size() == pb.stage[0].size()) || (s == 5 && pair5);
         if (!grouped) std::stable_sort(pb.stage[s].begin(), pb.stage[s].end(), [](const Item& a, const Item& b) {
             int64_t ta = 0, tb = 0;
             for (int g = 0; g < gf8::tc::NSEG; ++g) { ta += a.atoms[g]; tb += b.atoms[g]; }
@@ -582,7 +557,7 @@ gf8_status plan_finish(gf8_ctx* c, PlanBuilder& pb, Plan* p) {
     p->d_maps = (CUtensorMap*)q;
     if (cudaMalloc(&q, all.size() * sizeof(Item)) != cudaSuccess) { cudaGetLastError(); return fail(c, GF8_ERR_NOMEM, "plan items"); }
     p->d_items = (Item*)q;
-    if (cudaMalloc(&q, N_STAGES * sizeof(int)) != cudaSuccess) { cudaGetLastError(); return fail(c, GF8_ERR_NOMEM, "plan counters"); }
+    if (cudaMalloc(&q, 8 * sizeof(int)) != cudaSuccess) { cudaGetLastError(); return fail(c, GF8_ERR_NOMEM, "plan counters"); }
     p->d_ctr = (int*)q;
     CU_TRY(c, cudaMemcpy(p->d_maps, pb.maps.data(), pb.maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice));
     CU_TRY(c, cudaMemcpy(p->d_items, all.data(), all.size() * sizeof(Item), cudaMemcpyHostToDevice));
@@ -605,9 +580,8 @@ gf8_status plan_store(gf8_ctx* c, const std::vector<uint64_t>& key, Plan* p) {
 
 gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
     p->runs++;
-    if (p->d_ctr) CU_TRY(c, cudaMemsetAsync(p->d_ctr, 0, N_STAGES * sizeof(int), st));
-    for (int so = 0; so < N_STAGES; ++so) {
-        const int s = STAGE_ORDER[so];
+    if (p->d_ctr) CU_TRY(c, cudaMemsetAsync(p->d_ctr, 0, 8 * sizeof(int), st));
+    for (int s = 0; s < 8; ++s) {
         if (!p->stage_cnt[s]) continue;
         const bool pair = s == 5 && p->pair5;
         const int grid = std::min(pair ? p->stage_cnt[s] / 2 : p->stage_cnt[s], c->num_sms);
