@@ -344,3 +344,25 @@ def test_cfg4_stress_R16_with_periodic_refresh_at_size():
         assert np.array_equal(pc[7], oc) and np.array_equal(ps[7], os_), t.name
         # the 16 independent perturbations average out: the decoded mean is close to the shared gradient
         assert relfro(to_np64(outs[i]), to_np64(G[i])) <= 0.1
+
+
+@pytest.mark.parametrize("scaling", [gf8.SCALE_TENSOR, gf8.SCALE_BLOCK128])
+def test_largest_whitened_shape_embedding_sized(scaling):
+    """Maximum sizes: a WHITENED tensor of the configs' largest shape (32000 x 1024: the embedding / LM head, which the
+    configs leave Euclidean) and its transpose-shaped sibling (1024 x 8192), two ranks each, through the batched calls:
+    250-row-block strips, 125 strips per tensor, side BOTH at k = 32.  Bases are seeded orthonormal matrices handed in with
+    set_basis (a 32000^2 factor is not part of any config); G2 / G5 on sampled elements, G3-self on the whole tensor."""
+    shapes = [(32000, 1024), (1024, 8192)]
+    k, lam, R = 32, 1e-3, 2
+    lays = [gf8.Layer(m, n, gf8.SIDE_BOTH, k, k, gf8.E4M3, scaling, lam) for m, n in shapes]
+    ctx = gf8.create(lays, gf8.PREC_FAST)
+    mu = torch.arange(1, k + 1, device="cuda", dtype=torch.float32) ** -2.0
+    for i, (m, n) in enumerate(shapes):
+        ctx.set_basis(i, gf8.SIDE_IN, synth.rand_orthonormal(n, k, "cuda", 77, i, 1).contiguous(), mu, 1.0 / k / n + lam)
+        ctx.set_basis(i, gf8.SIDE_OUT, synth.rand_orthonormal(m, k, "cuda", 77, i, 2).contiguous(), mu, 1.0 / k / m + lam)
+    grads = {}
+    for i, (m, n) in enumerate(shapes):
+        G = synth.gradient(m, n, "cuda", 78, i)
+        grads[i] = [synth.rank_gradient(G, r, 79).to(torch.bfloat16).contiguous() for r in range(R)]
+        del G
+    codec_checks(ctx, [0, 1], {0: shapes[0], 1: shapes[1]}, grads, R, lam, gf8.E4M3, scaling, 1, 80, k_note="max-size")
