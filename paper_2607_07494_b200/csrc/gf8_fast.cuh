@@ -606,7 +606,9 @@ gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
 #ifdef GF8_DEBUG
         // GF8_TC_DBG (debug only, results are wrong with the ablation bits): 1 skip the MMAs, 2 skip the tensor-map
         // fences, 4 print a per-role wait profile, 32 skip the strip epilogue's work, 64 skip the strip base loads,
-        // 128 skip the strip B loads, 256 print each stage's device time (serialises the stream)
+        // 128 skip the strip B loads, 256 print each stage's device time (serialises the stream), 2048 (with 4) print the
+        // timeline of CTA 1's items 6..15 per role (tile items: publish / loads / MMA / epilogue, cycles), 4096 / 8192 / 16384
+        // skip the base loads / column multipliers / stores of the panel epilogue
         if (const char* e = getenv("GF8_TC_DBG")) dbg = atoi(e);
         if (const char* e = getenv("GF8_TC_ONLY")) only = atoi(e);
         if (only >= 0 && only != s) continue;
@@ -646,6 +648,23 @@ gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
             cudaEventRecord(ev1, st); cudaEventSynchronize(ev1); cudaEventElapsedTime(&ms, ev0, ev1);
             fprintf(stderr, "stage %d: %d items, %.1f us\n", s, p->stage_cnt[s], ms * 1e3);
             cudaEventDestroy(ev0); cudaEventDestroy(ev1);
+        }
+        if ((dbg & 2048) && (dbg & 4)) {      // bit 11: item timeline of CTA 1 (tile items): cycles since the CTA's first event
+            std::vector<long long> t(5 * 48 * 4);
+            cudaDeviceSynchronize();
+            cudaMemcpy(t.data(), c->d_prof + 8192, t.size() * sizeof(long long), cudaMemcpyDeviceToHost);
+            long long t0 = 0;
+            for (long long x : t) if (x > 0 && (t0 == 0 || x < t0)) t0 = x;
+            const char* rn[5] = {"prod", "ldA", "ldB", "mma", "epi"};
+            for (int it = 6; it < 16; ++it) {
+                fprintf(stderr, "stage %d item %2d:", s, it);
+                for (int r = 0; r < 5; ++r) {
+                    fprintf(stderr, "  %s", rn[r]);
+                    for (int e = 0; e < 4; ++e) { const long long x = t[(r * 48 + it) * 4 + e]; fprintf(stderr, " %6lld", x > 0 ? x - t0 : -1); }
+                }
+                fprintf(stderr, "\n");
+            }
+            cudaMemset(c->d_prof + 8192, 0, t.size() * sizeof(long long));
         }
         if (dbg & 4) {
             std::vector<long long> h((size_t)c->num_sms * 36);

@@ -265,7 +265,7 @@ __device__ __forceinline__ uint32_t epi_block_max(uint32_t loc, int warp, int la
 
 // One accumulator tile -> global memory with the base (if any) read straight from global memory: the small
 // panels (P', Q^T, S, Q'^T) and FP32 gradients.  Thread = one row, 16 columns per tcgen05.ld.
-__device__ __forceinline__ void epilogue(const Item& it, uint32_t tmem_acc, int warp, int lane, uint32_t* s_red, int rblk = 0) {
+__device__ __forceinline__ void epilogue(const Item& it, uint32_t tmem_acc, int warp, int lane, uint32_t* s_red, int rblk = 0, int dbgx = 0) {
     // rblk = 1: the second row block of a 256-row panel item (rows 128.., accumulator 64 columns further on)
     const int r = rblk * 128 + (warp & 3) * 32 + lane, half = warp >> 2;
     const bool row_ok = r < it.rows;
@@ -313,7 +313,10 @@ __device__ __forceinline__ void epilogue(const Item& it, uint32_t tmem_acc, int 
             }
             continue;
         }
-        load_base16(it, grow * it.base_ld + it.col0 + c0, v);
+        if (dbgx & 4096) {
+#pragma unroll
+            for (int u = 0; u < 16; ++u) v[u] = 0.0f;
+        } else load_base16(it, grow * it.base_ld + it.col0 + c0, v);
 #pragma unroll
         for (int u = 0; u < 16; ++u) v[u] += __uint_as_float(a[u]);
         if (it.mode == EPI_AMAX) {
@@ -323,11 +326,12 @@ __device__ __forceinline__ void epilogue(const Item& it, uint32_t tmem_acc, int 
             uint8_t* p = reinterpret_cast<uint8_t*>(it.out) + grow * it.out_ld + it.col0 + c0;
             *reinterpret_cast<uint4*>(p) = it.fmt == 0 ? codes16<0>(v, scale) : codes16<1>(v, scale);
         } else {   // EPI_STORE
-            if (it.colscale) {
+            if (it.colscale && !(dbgx & 8192)) {
 #pragma unroll
                 for (int u = 0; u < 16; ++u) v[u] *= __ldg(it.colscale + c0 + u);
             }
             const int64_t off = grow * it.out_ld + it.col0 + c0;
+            if ((dbgx & 16384) && v[0] != 12345.0f) continue;
             if (it.out_type == TY_F32) {
                 float4* o = reinterpret_cast<float4*>(reinterpret_cast<float*>(it.out) + off);
 #pragma unroll
@@ -721,6 +725,11 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
     // optional profile (prof != nullptr): cycles each role spends in each kind of wait, per CTA
     long long pw[6] = {0, 0, 0, 0, 0, 0};
     const long long t_start = clock64();
+#ifdef GF8_DEBUG
+#define TRC(role, item, ev) do { if ((dbg & 2048) && prof && blockIdx.x == 1 && (item) < 48u && lane == 0) prof[8192 + ((role) * 48 + (item)) * 4 + (ev)] = clock64(); } while (0)
+#else
+#define TRC(role, item, ev) do {} while (0)
+#endif
 #define TWAIT(slot, expr) ([&]() { const long long _t0 = prof ? clock64() : 0; const bool _r = (expr); if (prof) pw[slot] += clock64() - _t0; return _r; })()
     if (warp == PRODUCER_WARP) {
         // ===== item fetch (whole warp) + TMA producer (lane 0) =====
@@ -750,6 +759,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
             if (lane < NCHUNK) reinterpret_cast<uint4*>(s_items + slot * ITEM_BYTES)[lane] = nxt;
             __syncwarp();
             if (lane == 0) mbar_arrive(ifull_bar(slot));
+            TRC(0, n_done, 0);
             // pair launches: the amax item (even index) is followed by its cast item; the NEXT pair is claimed only after the
             // cast item's loads have been issued, i.e. after its epilogue has passed the tensor's join (the base ring is shorter
             // than a sub-strip): a pair claimed earlier could hold an amax item that this CTA's own waiting cast item needs
@@ -809,6 +819,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                     }
                     __syncwarp();
                 }
+                TRC(0, n_done, 1);
             }
             ok = __shfl_sync(0xFFFFFFFFu, ok, 0);
         }
@@ -905,6 +916,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                     if (elect_one()) mbar_arrive(iempty_bar(slot));
                     continue;
                 }
+                TRC(is_b ? 2 : 1, n_done, 0);
 #pragma unroll 1
                 for (int seg = 0; seg < NSEG && ok; ++seg) {
                     const int na = it.atoms[seg];
@@ -933,9 +945,11 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                             }
                         }
                         __syncwarp();
+                        if (seg == 0 && t == 0) TRC(is_b ? 2 : 1, n_done, 1);
                         if (++stage == (uint32_t)n_stages) { stage = 0; phase ^= 1u; }
                     }
                 }
+                TRC(is_b ? 2 : 1, n_done, 2);
                 __syncwarp();
                 if (elect_one()) mbar_arrive(iempty_bar(slot));
             }
@@ -1000,15 +1014,18 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 }
                 __syncwarp();
                 if (elect_one()) mbar_arrive(iempty_bar(slot));
+                TRC(3, n_done, 0);
                 const uint32_t acc = n_done % n_acc, aphase = (n_done / n_acc) & 1u;
                 if (!(ok = TWAIT(1, mbar_wait(tempty_bar(acc), aphase ^ 1u, err)))) break;
                 tc_fence_after();
+                TRC(3, n_done, 1);
                 const uint32_t d = tmem_base + acc * 128u;
                 const bool nrb2 = wide && it.rows > 128;
                 if (tri) total = it.atoms[0];              // one ring stage per K-atom carries all three products
                 for (int t = 0; t < total; ++t) {
                     if (!(ok = TWAIT(2, mbar_wait(full_bar(stage), phase, err)))) break;
                     tc_fence_after();
+                    if (t == 0) TRC(3, n_done, 2);
                     const uint32_t sa = smem0 + stage * stage_bytes, sb = sa + b_off;
                     if (elect_one()) {
 #pragma unroll
@@ -1039,6 +1056,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 }
                 if (ok && elect_one()) tc_commit(tfull_bar(acc));   // accumulator complete -> epilogue
                 __syncwarp();
+                TRC(3, n_done, 3);
             }
             // Drain: commits complete in issue order, so once this last one has arrived no mbarrier arrive of this
             // issuer is still in flight when the CTA exits (a late arrive would land in the shared memory of the
@@ -1268,8 +1286,11 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 if (lane == 0) mbar_arrive(iempty_bar(slot));
                 continue;
             }
+            if (warp == 0) TRC(4, n_done, 0);
             if (ok && n_base > 0) ok = TWAIT(1, mbar_wait(bfull_bar(bs), bphase, err));
+            if (warp == 0) TRC(4, n_done, 1);
             ok = ok && TWAIT(2, mbar_wait(tfull_bar(acc), aphase, err));
+            if (warp == 0) TRC(4, n_done, 2);
             const long long t_e0 = prof ? clock64() : 0;
             ok = __all_sync(0xFFFFFFFFu, ok);
             if (!ok) break;
@@ -1280,11 +1301,12 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                 stored = epilogue_tile<EF>(it, tmem_base + acc * 128u, base_tile(bs), it.base_map[1] >= 0 ? 2 : 1, warp, lane, s_red, maps, cast_scale, cast_si,
                                        it.row0, it.col0, it.write_scale != 0, it.scale_inv_out, nullptr);
             else {
-                epilogue(it, tmem_base + acc * 128u, warp, lane, s_red);
-                if (wide && it.rows > 128) epilogue(it, tmem_base + acc * 128u, warp, lane, s_red, 1);
+                epilogue(it, tmem_base + acc * 128u, warp, lane, s_red, 0, dbg);
+                if (wide && it.rows > 128) epilogue(it, tmem_base + acc * 128u, warp, lane, s_red, 1, dbg);
             }
             tc_fence_before();
             __syncwarp();
+            if (warp == 0) TRC(4, n_done, 3);
             if (prof) pw[3] += clock64() - t_e0;
             const long long t_p0 = prof ? clock64() : 0;
             if (lane == 0) { mbar_arrive(tempty_bar(acc)); mbar_arrive(iempty_bar(slot)); }
