@@ -605,7 +605,7 @@ gf8_status plan_run_stages(gf8_ctx* c, cudaStream_t st, Plan* p) {
         if (fuse && grid < c->num_sms && p->stage_cnt[s] > grid) return fail(c, GF8_ERR_BAD_STATE, "fused stage needs a full grid");
 #ifdef GF8_DEBUG
         // GF8_TC_DBG (debug only, results are wrong with the ablation bits): 1 skip the MMAs, 2 skip the tensor-map
-        // fences, 4 print a per-role wait profile, 32 skip the strip epilogue's work, 64 skip the strip base loads,
+        // fences, 4 print a per-role wait profile, 32 skip the update epilogue's work, 64 skip the streamed base loads,
         // 128 skip the strip B loads, 256 print each stage's device time (serialises the stream), 2048 (with 4) print the
         // timeline of CTA 1's items 6..15 per role (tile items: publish / loads / MMA / epilogue, cycles), 4096 / 8192 / 16384
         // skip the base loads / column multipliers / stores of the panel epilogue

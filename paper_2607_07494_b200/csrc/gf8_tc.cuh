@@ -806,7 +806,7 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
                     if (bm0 >= 0) acq(maps + bm0);
                     if (bm1 >= 0) acq(maps + bm1);
                     if (elect_one()) {
-                        if (nb == 0) mbar_arrive(bfull_bar(acc));
+                        if (nb == 0 || (dbg & 64)) mbar_arrive(bfull_bar(acc));
                         else {
                             mbar_expect_tx(bfull_bar(acc), (uint32_t)nb * TILE_BYTES);
                             for (int b = 0; b < nb; ++b) {
@@ -1297,7 +1297,8 @@ __global__ void __launch_bounds__(THREADS, 1) tc_items_kernel(const Item* __rest
             tc_fence_after();
             const Item& it = *item_slot(slot);
             bool stored = false;
-            if (it.base_map[0] >= 0)
+            if (dbg & 32) {
+            } else if (it.base_map[0] >= 0)
                 stored = epilogue_tile<EF>(it, tmem_base + acc * 128u, base_tile(bs), it.base_map[1] >= 0 ? 2 : 1, warp, lane, s_red, maps, cast_scale, cast_si,
                                        it.row0, it.col0, it.write_scale != 0, it.scale_inv_out, nullptr);
             else {
